@@ -1,0 +1,349 @@
+"""oracle/apd_oracle.py -- TEST INFRASTRUCTURE, not the product.
+
+fp64 CPU oracle for the APD hot path, written from the paper (arxiv 2403.03571,
+PAPER.md) and DESIGN.md's readings.  Only tests/, __graft_entry__.smoke() and
+bench.py's cpu_baseline / ``--impl reference`` legs may import this; the product
+path (paper_2403_03571_b200) never does, and this module never imports it.
+
+  oracle_assign  -- the DEFINITION (exact brute force): Algorithm 1
+                    plus the discrete dual and gradient, eq. (2.7)-(2.8)
+                    and the discrete centroid of Algorithm 3.
+                    The O(N*M) loop is oracle/apd_oracle.c; the reductions are here.
+  oracle_solve   -- Algorithm 2 step by step; the paper only fixes
+                    "W0 = 0, L-BFGS [70], stop when |v_i - m_i|P|| <= eps v_i for all i";
+                    the L-BFGS details are DESIGN.md reading S9 and bind this file AND
+                    the CUDA path identically.
+
+Pins (tests/test_oracle_pins.py): P1 Voronoi brute force, P2 half-space power diagram,
+P3 exact rational arithmetic, P4 concentric ellipse volume, P5 Moebius sphere, P6
+tessellation, P7 dual identity, P8 super-gradient / finite differences, P9 concavity,
+P10 gauge, P11 exact symmetries, P12 monotonicity, P13 trivial optimum, P14 closed-form
+solved weights, P15 post-condition.
+PARITY UNPINNED against the paper: L-BFGS iteration/evaluation counts and the particular w
+among the valid ones (the paper prints none for a regenerable input) -- see DESIGN.md.
+"""
+from __future__ import annotations
+
+import ctypes
+import dataclasses
+import math
+import os
+import subprocess
+from typing import List, Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "apd_oracle.c")
+_LIB = os.path.join(_HERE, "liboracle_apd.so")
+_lib = None
+
+OK = 0
+NOT_CONVERGED = 1
+
+
+def build(force: bool = False) -> str:
+    """Compile the C part with gcc (-O2, fp64, OpenMP over voxels; no fast-math)."""
+    if force or (not os.path.exists(_LIB)) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-fopenmp", "-fPIC", "-shared", "-std=c99", "-o", _LIB, _SRC, "-lm"]
+        subprocess.run(cmd, check=True)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        build()
+        lib = ctypes.CDLL(_LIB)
+        p = ctypes.c_void_p
+        lib.oracle_apd_assign.restype = ctypes.c_int
+        lib.oracle_apd_assign.argtypes = [ctypes.c_int, p, p, p, ctypes.c_int64, p, p, p,
+                                          ctypes.c_int64, p, p, p, p, p, p]
+        lib.oracle_apd_cost_of.restype = ctypes.c_int
+        lib.oracle_apd_cost_of.argtypes = [ctypes.c_int, p, p, p, ctypes.c_int64, p, p, p,
+                                           ctypes.c_int64, p, p, p]
+        lib.oracle_apd_num_threads.restype = ctypes.c_int
+        _lib = lib
+    return _lib
+
+
+def num_threads() -> int:
+    return int(_load().oracle_apd_num_threads())
+
+
+@dataclasses.dataclass
+class Grid:
+    """Regular discretisation of a box: voxel (ix,iy[,iz]) is centred at
+    lo + (i + 1/2) s, s_k = (hi_k - lo_k)/n_k, |P| = prod s_k; linear index j = (iz*ny+iy)*nx+ix
+    (x fastest; reading S3)."""
+    dim: int
+    n: Sequence[int]
+    lo: Sequence[float]
+    hi: Sequence[float]
+
+    @property
+    def N(self) -> int:
+        return int(np.prod([int(k) for k in self.n[: self.dim]]))
+
+    @property
+    def s(self) -> np.ndarray:
+        return (np.asarray(self.hi[: self.dim], dtype=np.float64)
+                - np.asarray(self.lo[: self.dim], dtype=np.float64)) / np.asarray(self.n[: self.dim], dtype=np.float64)
+
+    @property
+    def voxel_volume(self) -> float:
+        return float(np.prod(self.s))
+
+    @property
+    def domain_volume(self) -> float:
+        return float(np.prod(np.asarray(self.hi[: self.dim], dtype=np.float64)
+                             - np.asarray(self.lo[: self.dim], dtype=np.float64)))
+
+
+def _ptr(a):
+    return None if a is None else a.ctypes.data_as(ctypes.c_void_p)
+
+
+def _grid_arrays(grid: Grid):
+    n = np.ones(3, dtype=np.int64)
+    n[: grid.dim] = np.asarray(grid.n[: grid.dim], dtype=np.int64)
+    lo = np.zeros(3, dtype=np.float64)
+    hi = np.zeros(3, dtype=np.float64)
+    lo[: grid.dim] = grid.lo[: grid.dim]
+    hi[: grid.dim] = grid.hi[: grid.dim]
+    return n, lo, hi
+
+
+def _widen(X, A, w, dim):
+    X = np.ascontiguousarray(np.asarray(X), dtype=np.float64).reshape(-1, dim)   # exact widening of fp32
+    M = X.shape[0]
+    A = np.ascontiguousarray(np.asarray(A), dtype=np.float64).reshape(M, dim, dim)
+    w = np.ascontiguousarray(np.asarray(w), dtype=np.float64).reshape(M)
+    return X, A, w, M
+
+
+@dataclasses.dataclass
+class AssignResult:
+    labels: np.ndarray            # int32 [n_sel]
+    best: np.ndarray              # fp64  min_i C_ij
+    qbest: np.ndarray             # fp64  |y_j - x_label|^2_A
+    second: Optional[np.ndarray]  # fp64  runner-up cost
+    runner: Optional[np.ndarray]  # int32 runner-up index
+    count: Optional[np.ndarray] = None     # int64 [M]  m_i
+    vol: Optional[np.ndarray] = None       # fp64 [M]   m_i |P|
+    dual: Optional[float] = None           # eq. (2.7) literally (None when v is None)
+    dual_min_part: Optional[float] = None  # |P| * sum_j min_i C_ij  (= dual - <v,w>, identity I1)
+    quad_part: Optional[float] = None      # |P| * sum_j |y_j - x_{H_j}|^2_A
+    idxsum: Optional[np.ndarray] = None    # int64 [M, d] sum of voxel indices per cell
+    centroids: Optional[np.ndarray] = None  # fp64 [M, d]
+    err: Optional[float] = None            # max_i |vol_i - v_i| / v_i  (eq. 2.5)
+
+
+def oracle_assign(grid: Grid, X, A, w, v=None, sel=None, diagnostics: bool = True) -> AssignResult:
+    """Algorithm 1 on the voxels `sel` (all when None) and, when all voxels are evaluated,
+    the reductions of eq. (2.7)-(2.8).  X, A, w: the SAME fp32 arrays the GPU gets (widened
+    exactly to fp64 here)."""
+    lib = _load()
+    X, A, w, M = _widen(X, A, w, grid.dim)
+    n, lo, hi = _grid_arrays(grid)
+    if sel is None:
+        n_sel = grid.N
+        sel_arr = None
+    else:
+        sel_arr = np.ascontiguousarray(sel, dtype=np.int64)
+        n_sel = sel_arr.size
+    labels = np.empty(n_sel, dtype=np.int32)
+    best = np.empty(n_sel, dtype=np.float64)
+    qbest = np.empty(n_sel, dtype=np.float64)
+    second = np.empty(n_sel, dtype=np.float64) if diagnostics else None
+    runner = np.empty(n_sel, dtype=np.int32) if diagnostics else None
+    rc = lib.oracle_apd_assign(grid.dim, _ptr(n), _ptr(lo), _ptr(hi), M, _ptr(X), _ptr(A), _ptr(w),
+                               n_sel, _ptr(sel_arr), _ptr(labels), _ptr(best), _ptr(qbest),
+                               _ptr(second), _ptr(runner))
+    if rc != 0:
+        raise ValueError(f"oracle_apd_assign: bad arguments (rc={rc})")
+    res = AssignResult(labels=labels, best=best, qbest=qbest, second=second, runner=runner)
+    if sel is not None:
+        return res
+
+    # ---- reductions over ALL voxels: eq. (2.7), (2.8), Alg. 3 centroid -----------------
+    P = grid.voxel_volume
+    count = np.bincount(labels, minlength=M).astype(np.int64)            # m_i
+    res.count = count
+    res.vol = count.astype(np.float64) * P                               # sum_{H_j=i} |P|, eq. (2.8)
+    T = math.fsum(qbest.tolist()) if n_sel <= (1 << 22) else float(np.sum(qbest, dtype=np.longdouble))
+    S = math.fsum(best.tolist()) if n_sel <= (1 << 22) else float(np.sum(best, dtype=np.longdouble))
+    res.quad_part = P * T
+    res.dual_min_part = P * S
+    if v is not None:
+        v64 = np.asarray(v, dtype=np.float64).reshape(M)
+        # eq. (2.7), literally:  sum_i (v_i - vol_i) w_i  +  sum_j |P| |y_j - x_{H_j}|^2
+        res.dual = math.fsum(((v64 - res.vol) * w).tolist()) + P * T
+        res.err = float(np.max(np.abs(res.vol - v64) / v64))             # eq. (2.5)
+    # centroid: x_i <- sum_{H_j=i} |P| y_j / sum_{H_j=i} |P|.  With
+    # y = lo + (idx + 1/2) s this is lo + s (idxsum_i / m_i + 1/2); an empty cell keeps x_i (S5).
+    d = grid.dim
+    nx = int(n[0]); ny = int(n[1])
+    j = np.arange(n_sel, dtype=np.int64)
+    comps = [j % nx, (j // nx) % ny, j // (nx * ny)]
+    idxsum = np.zeros((M, d), dtype=np.int64)
+    for k in range(d):
+        # integer-valued fp64 weights: every partial sum is an integer < 2^53, hence exact
+        idxsum[:, k] = np.bincount(labels, weights=comps[k].astype(np.float64), minlength=M).round().astype(np.int64)
+    res.idxsum = idxsum
+    cen = X.copy()
+    nz = count > 0
+    s = grid.s
+    for k in range(d):
+        cen[nz, k] = lo[k] + s[k] * (idxsum[nz, k] / count[nz] + 0.5)
+    res.centroids = cen
+    return res
+
+
+def oracle_cost_of(grid: Grid, X, A, w, sel, seed) -> np.ndarray:
+    """fp64 cost C_ij of the named seed i = seed[t] at voxel j = sel[t] (parity rule 1)."""
+    lib = _load()
+    X, A, w, M = _widen(X, A, w, grid.dim)
+    n, lo, hi = _grid_arrays(grid)
+    sel = np.ascontiguousarray(sel, dtype=np.int64)
+    seed = np.ascontiguousarray(seed, dtype=np.int32)
+    out = np.empty(sel.size, dtype=np.float64)
+    rc = lib.oracle_apd_cost_of(grid.dim, _ptr(n), _ptr(lo), _ptr(hi), M, _ptr(X), _ptr(A), _ptr(w),
+                                sel.size, _ptr(sel), _ptr(seed), _ptr(out))
+    if rc != 0:
+        raise ValueError(f"oracle_apd_cost_of: bad arguments (rc={rc})")
+    return out
+
+
+# ----------------------------------------------------------------------------------------
+# Algorithm 2 with the L-BFGS of DESIGN.md reading S9
+# ----------------------------------------------------------------------------------------
+@dataclasses.dataclass
+class SolveResult:
+    status: int                   # OK / NOT_CONVERGED
+    w: np.ndarray                 # fp64 iterate
+    w32: np.ndarray               # fl32(w): exactly what the final evaluation used
+    labels: np.ndarray
+    vol: np.ndarray
+    iters: int
+    evals: int
+    err: float
+    dual: float
+    trajectory: Optional[List[dict]] = None
+
+
+def _two_loop(g, S_hist, Y_hist, rho, gamma):
+    """Liu-Nocedal two-loop recursion [70]: returns H*g with H0 = gamma*I."""
+    q = g.copy()
+    alphas = []
+    for s_i, y_i, r_i in zip(reversed(S_hist), reversed(Y_hist), reversed(rho)):
+        a = r_i * float(np.dot(s_i, q))
+        alphas.append(a)
+        q = q - a * y_i
+    r = gamma * q
+    for (s_i, y_i, r_i), a in zip(zip(S_hist, Y_hist, rho), reversed(alphas)):
+        b = r_i * float(np.dot(y_i, r))
+        r = r + s_i * (a - b)
+    return r
+
+
+def oracle_solve(grid: Grid, X, A, v, eps: float, w_init=None, history: int = 10,
+                 max_iters: int = 1000, max_evals: Optional[int] = None,
+                 record: bool = False) -> SolveResult:
+    """Maximise g~ (eq. 2.7) <=> minimise f = -g~ from W0 = 0 (Alg. 2 step 2) with L-BFGS,
+    stop when max_i |vol_i - v_i|/v_i <= eps (Alg. 2 step 3, eq. 2.5; '<=' is reading S7).
+    Specification S9 (shared with the CUDA path):
+      * fp64 optimiser state; every evaluation uses fl32(w) (round-to-nearest-even), S10
+      * f = -g~(fl32 w), grad f = vol - v  (eq. 2.8 with the sign of f)
+      * first-direction scale gamma = l^(2-d)/d, l = (|Omega|/M)^(1/d)  (S9a)
+      * weak-Wolfe bracketing line search, c1 = 1e-4, c2 = 0.9, alpha0 = 1, <= 30 trials:
+        Armijo fails -> hi = alpha; curvature fails -> lo = alpha; alpha = (lo+hi)/2 or 2 alpha
+      * stopping test after EVERY evaluation (S9c)
+      * curvature pair kept iff s.y > 1e-12 |s||y|; then gamma = s.y / y.y
+      * line-search failure: clear the history and retry once with p = -gamma g; else NOT_CONVERGED
+      * NOT_CONVERGED returns the evaluated point with the smallest err.
+    """
+    d = grid.dim
+    M = np.asarray(X).reshape(-1, d).shape[0]
+    v64 = np.asarray(v, dtype=np.float64).reshape(M)
+    if max_evals is None:
+        max_evals = 20 * max_iters
+    c1, c2 = 1e-4, 0.9
+    traj: Optional[List[dict]] = [] if record else None
+
+    best = {"err": math.inf}
+
+    def evaluate(wd, tag):
+        w32 = wd.astype(np.float32)                     # RNE rounding, S10
+        r = oracle_assign(grid, X, A, w32, v=v64, diagnostics=False)
+        f = -r.dual
+        g = r.vol - v64
+        if r.err < best["err"]:
+            best.update(err=r.err, w=wd.copy(), w32=w32.copy(), labels=r.labels, vol=r.vol, dual=r.dual)
+        if traj is not None:
+            traj.append(dict(tag=tag, w=wd.copy(), f=f, err=r.err))
+        return f, g, r.err, w32, r
+
+    def finish(status, wd, w32, r, iters, evals):
+        return SolveResult(status=status, w=wd, w32=w32, labels=r.labels, vol=r.vol, iters=iters,
+                           evals=evals, err=r.err, dual=r.dual, trajectory=traj)
+
+    def finish_best(iters, evals):
+        return SolveResult(status=NOT_CONVERGED, w=best["w"], w32=best["w32"], labels=best["labels"],
+                           vol=best["vol"], iters=iters, evals=evals, err=best["err"], dual=best["dual"],
+                           trajectory=traj)
+
+    w = np.zeros(M, dtype=np.float64) if w_init is None else np.asarray(w_init, dtype=np.float64).copy()
+    f, g, err, w32, r = evaluate(w, "init")
+    evals, iters = 1, 0
+    if err <= eps:
+        return finish(OK, w, w32, r, iters, evals)
+
+    ell = (grid.domain_volume / M) ** (1.0 / d)
+    gamma = ell ** (2 - d) / d
+    S_hist: List[np.ndarray] = []
+    Y_hist: List[np.ndarray] = []
+    rho: List[float] = []
+
+    while True:
+        p = -_two_loop(g, S_hist, Y_hist, rho, gamma)
+        gp = float(np.dot(g, p))
+        if gp >= 0.0:
+            S_hist, Y_hist, rho = [], [], []
+            p = -gamma * g
+            gp = float(np.dot(g, p))
+        alpha, lo_a, hi_a = 1.0, 0.0, math.inf
+        accepted = False
+        for _trial in range(30):
+            w_try = w + alpha * p
+            f1, g1, err1, w32_1, r1 = evaluate(w_try, "ls")
+            evals += 1
+            if err1 <= eps:
+                return finish(OK, w_try, w32_1, r1, iters + 1, evals)
+            if f1 > f + c1 * alpha * gp:
+                hi_a = alpha
+            elif float(np.dot(g1, p)) < c2 * gp:
+                lo_a = alpha
+            else:
+                accepted = True
+                break
+            if evals >= max_evals:
+                return finish_best(iters, evals)
+            alpha = 0.5 * (lo_a + hi_a) if math.isfinite(hi_a) else 2.0 * alpha
+        if not accepted:
+            if S_hist:
+                S_hist, Y_hist, rho = [], [], []
+                continue                                  # retry once with p = -gamma g
+            return finish_best(iters, evals)
+        s = alpha * p
+        yv = g1 - g
+        sy = float(np.dot(s, yv))
+        if sy > 1e-12 * math.sqrt(float(np.dot(s, s))) * math.sqrt(float(np.dot(yv, yv))):
+            S_hist.append(s); Y_hist.append(yv); rho.append(1.0 / sy)
+            if len(S_hist) > history:
+                S_hist.pop(0); Y_hist.pop(0); rho.pop(0)
+            gamma = sy / float(np.dot(yv, yv))
+        w, f, g = w_try, f1, g1
+        iters += 1
+        if iters >= max_iters or evals >= max_evals:
+            return finish_best(iters, evals)
