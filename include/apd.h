@@ -1,0 +1,160 @@
+/*
+ * apd.h -- C ABI of libapd_b200: anisotropic power diagrams (APDs) by semi-discrete optimal
+ * transport on one NVIDIA B200 (sm_100a).  Hot path of arxiv 2403.03571:
+ *
+ *   apd_assign : Algorithm 1 "pixel method" fused with the discrete dual
+ *                and its gradient, eq. (2.7)-(2.8), and the discrete
+ *                centroid of Algorithm 3.
+ *   apd_solve  : Algorithm 2: L-BFGS ascent on the weights until every
+ *                cell volume is within tolerance, eq. (2.5).
+ *
+ * Notation (SURVEY.md / DESIGN.md): M grains (seeds), N voxels, n voxels per axis, d = dim.
+ * All arithmetic of the path runs in the library's CUDA kernels; there is no CPU fallback
+ * and no other architecture.  Plain pointers and sizes only; every array pointer says whether
+ * it is DEVICE or HOST memory.  The caller owns every array; the library owns only the
+ * apd_ctx workspace and keeps no caller pointer after a call returns.
+ *
+ * Errors never cross the ABI as exceptions/aborts: every call returns an apd_status.
+ */
+#ifndef APD_B200_H
+#define APD_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  APD_OK            = 0,   /* success (apd_solve: tolerance met)                                  */
+  APD_NOT_CONVERGED = 1,   /* apd_solve only: limits hit / line search failed; outputs hold the
+                              evaluated iterate with the smallest max relative volume error;
+                              the caller may refine the grid (Alg. 2 step 4)        */
+  APD_E_ARG         = -1,  /* bad argument (see each call); nothing was launched                   */
+  APD_E_CUDA        = -2,  /* CUDA runtime failure; text via apd_last_error                        */
+  APD_E_ARCH        = -3   /* the device is not compute capability 10.x                            */
+} apd_status;
+
+/* Regular discretisation of a box (eq. 2.6).  Voxel (ix,iy,iz) is the box
+ * P(y,s) centred at y_k = lo_k + (i_k + 1/2) s_k with s_k = (hi_k - lo_k)/n_k; |P| = prod s_k.
+ * Linear index j = (iz*ny + iy)*nx + ix (x fastest).  The voxel list is never stored: the
+ * kernels generate y from the thread index.  n[2], lo[2], hi[2] are ignored when dim == 2. */
+typedef struct {
+  int32_t dim;           /* 2 or 3 */
+  int32_t n[3];          /* voxels per axis, each >= 1; N = prod n_k must be < 2^31 */
+  double  lo[3], hi[3];  /* hi_k > lo_k */
+} apd_grid;
+
+/* Which implementation of the voxel x seed reduction runs (all give labels by the same rule:
+ * fp32 cost, lowest seed index among equal fp32 costs). */
+enum {
+  APD_KERNEL_AUTO   = 0,   /* the fastest one (currently APD_KERNEL_ROWPOLY)                      */
+  APD_KERNEL_DIRECT = 1,   /* un-hoisted direct form: 12 (3D) / 7 (2D) FP32 instr. per pair;
+                              the reference kernel the FP32-pipe fraction is quoted on             */
+  APD_KERNEL_ROWPOLY = 2   /* row-hoisted quadratic in the in-row offset, packed f32x2, deferred
+                              argmin                                                                */
+};
+
+typedef struct {
+  int32_t kernel;          /* APD_KERNEL_*                                   default AUTO         */
+  int32_t cull;            /* 0 brute force, 1 exact conservative tile culling  default 0         */
+  int32_t lbfgs_history;   /* m of L-BFGS                                     default 10          */
+  int32_t max_iters;       /* apd_solve iteration limit                       default 1000        */
+  int32_t max_evals;       /* apd_solve evaluation limit; 0 = 20*max_iters    default 0           */
+  int32_t reserved[3];     /* must be 0                                                           */
+} apd_opts;
+
+/* Fills *o with the defaults above. */
+void apd_default_opts(apd_opts* o);
+
+typedef struct apd_ctx apd_ctx;
+
+/* Creates a context on CUDA device `device` able to handle up to max_seeds grains in `dim`
+ * dimensions.  Allocates the workspace (packed seed table, integer histograms, dual partials,
+ * L-BFGS state: O(max_seeds) bytes; nothing proportional to the voxel count).
+ * Returns APD_E_ARCH if the device is not sm_100-class, APD_E_ARG on dim not in {2,3} or
+ * max_seeds < 1, APD_E_CUDA on allocation failure (*out is then NULL). */
+int  apd_create(apd_ctx** out, int32_t dim, int32_t max_seeds, int32_t device);
+void apd_destroy(apd_ctx* ctx);                 /* NULL is allowed */
+/* Text of the last error of this context ("" if none); with ctx == NULL, of the last failed
+ * apd_create on this thread.  The pointer stays valid until the next call on the context. */
+const char* apd_last_error(const apd_ctx* ctx);
+
+/* One evaluation: Algorithm 1 + eq. (2.7)-(2.8) at the given weights.
+ *   X          [M,dim]      DEVICE fp32 row-major, seed positions x_i
+ *   A          [M,dim,dim]  DEVICE fp32 row-major, anisotropy matrices; the quadratic form of
+ *                           the matrix as given is used, i.e. that of (A+A^T)/2 (reading S13)
+ *   w          [M]          DEVICE fp32 weights
+ *   target_vol [M]          DEVICE fp32 or NULL.  NULL: `dual` is |P| sum_j min_i C_ij, the
+ *                           v-independent part of eq. (2.7) (reading S6)
+ *   labels     [N]          DEVICE int32 out or NULL (store skipped).  labels[j] = 0-based
+ *                           index of a seed minimising C_ij = |y_j - x_i|^2_{A_i} - w_i
+ *                           evaluated in fp32; among equal fp32 costs the lowest index (S1)
+ *   vol        [M]          DEVICE fp64 out, required: (voxels labelled i) * |P|   (eq. 2.8)
+ *   dual       [1]          DEVICE fp64 out, required: g~(W) of eq. (2.7)
+ *   max_rel_err[1]          DEVICE fp64 out or NULL: max_i |vol_i - v_i| / v_i (eq. 2.5);
+ *                           written only when target_vol != NULL
+ *   centroids  [M,dim]      DEVICE fp64 out or NULL: discrete centroid of each cell
+ *                           (PAPER.md:178); an empty cell returns its seed x_i (S5)
+ *   pairs_evaluated [1]     DEVICE uint64 out or NULL: voxel-seed pairs whose cost was
+ *                           evaluated (= N*M without culling)
+ * Asynchronous on `cuda_stream` (a cudaStream_t; NULL = the legacy default stream): returns
+ * after enqueueing; outputs are valid once the stream reaches this point.
+ * APD_E_ARG: NULL ctx/grid/required pointer, grid.dim != ctx dim, n_k < 1, hi <= lo,
+ * N >= 2^31, M < 1 or M > max_seeds, unknown opts value.  opts == NULL means defaults. */
+int apd_assign(apd_ctx* ctx, const apd_grid* grid, int32_t M,
+               const float* X, const float* A, const float* w, const float* target_vol,
+               int32_t* labels, double* vol, double* dual, double* max_rel_err,
+               double* centroids, uint64_t* pairs_evaluated,
+               const apd_opts* opts, void* cuda_stream);
+
+/* Algorithm 2: maximise g~ over W from W0 = w_init (0 when NULL, Alg. 2 step 2) by L-BFGS
+ * until max_i |vol_i - v_i|/v_i <= tol (eq. 2.5; "<=" is reading S7).  The optimiser is
+ * DESIGN.md's specification S9, identical to oracle/apd_oracle.py: fp64 state on the device,
+ * every evaluation at fl32(w), weak-Wolfe bracketing line search, stopping test after every
+ * evaluation.  The loop runs on the device; the host reads one mapped status word per
+ * evaluation and nothing else.
+ *   X, A, target_vol, w_init   DEVICE fp32 in (as apd_assign); sum target_vol must equal
+ *                              |Omega| to 1e-5 relative else APD_E_ARG
+ *   w          [M]  DEVICE fp32 out, required: exactly the weights the final evaluation used
+ *   labels     [N]  DEVICE int32 out or NULL: Algorithm 1 at the returned w
+ *   vol        [M]  DEVICE fp64 out or NULL: cell volumes at the returned w
+ *   w64        [M]  DEVICE fp64 out or NULL: the optimiser's fp64 iterate (w = fl32(w64))
+ *   iters, evals, max_rel_err, dual   HOST out, each may be NULL
+ * Blocks until the solve has finished (synchronises `cuda_stream`).
+ * Returns APD_OK, APD_NOT_CONVERGED, or a negative error. */
+int apd_solve(apd_ctx* ctx, const apd_grid* grid, int32_t M,
+              const float* X, const float* A, const float* target_vol, double tol,
+              const float* w_init, float* w, int32_t* labels, double* vol, double* w64,
+              int32_t* iters, int32_t* evals, double* max_rel_err, double* dual,
+              const apd_opts* opts, void* cuda_stream);
+
+/* Same two calls with HOST arrays: the library allocates device buffers, copies in, runs the
+ * device call above, copies the results out and frees.  Every pointer is HOST memory; NULL is
+ * allowed where the device call allows it.  Synchronous. */
+int apd_assign_host(apd_ctx* ctx, const apd_grid* grid, int32_t M,
+                    const float* X, const float* A, const float* w, const float* target_vol,
+                    int32_t* labels, double* vol, double* dual, double* max_rel_err,
+                    double* centroids, uint64_t* pairs_evaluated, const apd_opts* opts);
+int apd_solve_host(apd_ctx* ctx, const apd_grid* grid, int32_t M,
+                   const float* X, const float* A, const float* target_vol, double tol,
+                   const float* w_init, float* w, int32_t* labels, double* vol, double* w64,
+                   int32_t* iters, int32_t* evals, double* max_rel_err, double* dual,
+                   const apd_opts* opts);
+
+/* Measurement helpers: not part of the method.
+ * apd_last_kernel_ms: device time in ms (CUDA events on the launching stream) of the voxel x
+ *   seed kernel of the most recent apd_assign on this context; synchronises that event.
+ *   Returns a negative value if no evaluation has run.
+ * apd_fp32_probe: runs a register-only FP32 microbenchmark on `device` and returns the
+ *   achieved rate in *ops_per_s (HOST): variant 0 = scalar FFMA (2 flop each), 1 = packed
+ *   fma.rn.f32x2 (4 flop each), 2 = 3-input min.f32, 3 = the ROWPOLY inner-loop mix
+ *   (2 f32x2 FMA + 1 three-input min).  *ops_per_s counts FMA lanes (variants 0,1), min
+ *   instructions x32 lanes (2) or voxel-seed pairs (3).  Synchronous. */
+double apd_last_kernel_ms(apd_ctx* ctx);
+int    apd_fp32_probe(int32_t device, int32_t variant, double* ops_per_s, double* sm_clock_mhz);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* APD_B200_H */

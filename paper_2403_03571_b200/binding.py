@@ -1,0 +1,246 @@
+"""Thin ctypes binding of libapd_b200.so (include/apd.h).  Argument marshalling only: every step
+of the path runs in the library's CUDA kernels.  PyTorch supplies device memory and the stream.
+
+There is NO fallback: if the shared library is missing or fails to load, importing a compute
+entry point raises.  This module never imports ``oracle/``.
+"""
+from __future__ import annotations
+
+import ctypes
+import dataclasses
+import os
+from typing import Optional, Sequence
+
+import torch
+
+_PKG = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_PKG, "libapd_b200.so")
+
+APD_OK = 0
+APD_NOT_CONVERGED = 1
+APD_E_ARG = -1
+APD_E_CUDA = -2
+APD_E_ARCH = -3
+
+KERNEL_AUTO = 0
+KERNEL_DIRECT = 1
+KERNEL_ROWPOLY = 2
+
+
+class ApdError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"libapd_b200 status {status}: {msg}")
+        self.status = status
+
+
+class apd_grid(ctypes.Structure):
+    _fields_ = [("dim", ctypes.c_int32), ("n", ctypes.c_int32 * 3),
+                ("lo", ctypes.c_double * 3), ("hi", ctypes.c_double * 3)]
+
+
+class apd_opts(ctypes.Structure):
+    _fields_ = [("kernel", ctypes.c_int32), ("cull", ctypes.c_int32), ("lbfgs_history", ctypes.c_int32),
+                ("max_iters", ctypes.c_int32), ("max_evals", ctypes.c_int32), ("reserved", ctypes.c_int32 * 3)]
+
+
+_lib = None
+_P = ctypes.c_void_p
+
+
+def load_library() -> ctypes.CDLL:
+    """Loads libapd_b200.so; raises (never falls back) when it is absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_2403_03571_b200.build` "
+                          "(there is no CPU or PyTorch fallback)")
+    lib = ctypes.CDLL(LIB_PATH)
+    lib.apd_default_opts.restype = None
+    lib.apd_default_opts.argtypes = [ctypes.POINTER(apd_opts)]
+    lib.apd_create.restype = ctypes.c_int
+    lib.apd_create.argtypes = [ctypes.POINTER(_P), ctypes.c_int32, ctypes.c_int32, ctypes.c_int32]
+    lib.apd_destroy.restype = None
+    lib.apd_destroy.argtypes = [_P]
+    lib.apd_last_error.restype = ctypes.c_char_p
+    lib.apd_last_error.argtypes = [_P]
+    lib.apd_assign.restype = ctypes.c_int
+    lib.apd_assign.argtypes = [_P, ctypes.POINTER(apd_grid), ctypes.c_int32] + [_P] * 10 + [ctypes.POINTER(apd_opts), _P]
+    lib.apd_solve.restype = ctypes.c_int
+    lib.apd_solve.argtypes = ([_P, ctypes.POINTER(apd_grid), ctypes.c_int32, _P, _P, _P, ctypes.c_double]
+                              + [_P] * 5 + [ctypes.POINTER(ctypes.c_int32), ctypes.POINTER(ctypes.c_int32),
+                                            ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double),
+                                            ctypes.POINTER(apd_opts), _P])
+    lib.apd_assign_host.restype = ctypes.c_int
+    lib.apd_assign_host.argtypes = [_P, ctypes.POINTER(apd_grid), ctypes.c_int32] + [_P] * 10 + [ctypes.POINTER(apd_opts)]
+    lib.apd_solve_host.restype = ctypes.c_int
+    lib.apd_solve_host.argtypes = ([_P, ctypes.POINTER(apd_grid), ctypes.c_int32, _P, _P, _P, ctypes.c_double]
+                                   + [_P] * 5 + [ctypes.POINTER(ctypes.c_int32), ctypes.POINTER(ctypes.c_int32),
+                                                 ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double),
+                                                 ctypes.POINTER(apd_opts)])
+    lib.apd_last_kernel_ms.restype = ctypes.c_double
+    lib.apd_last_kernel_ms.argtypes = [_P]
+    lib.apd_fp32_probe.restype = ctypes.c_int
+    lib.apd_fp32_probe.argtypes = [ctypes.c_int32, ctypes.c_int32, ctypes.POINTER(ctypes.c_double),
+                                   ctypes.POINTER(ctypes.c_double)]
+    _lib = lib
+    return lib
+
+
+EXPORTED_SYMBOLS = ["apd_default_opts", "apd_create", "apd_destroy", "apd_last_error", "apd_assign", "apd_solve",
+                    "apd_assign_host", "apd_solve_host", "apd_last_kernel_ms", "apd_fp32_probe"]
+
+
+def make_grid(dim: int, n: Sequence[int], lo: Sequence[float], hi: Sequence[float]) -> apd_grid:
+    g = apd_grid()
+    g.dim = dim
+    for k in range(3):
+        g.n[k] = int(n[k]) if k < dim else 1
+        g.lo[k] = float(lo[k]) if k < dim else 0.0
+        g.hi[k] = float(hi[k]) if k < dim else 1.0
+    return g
+
+
+def make_opts(kernel: int = KERNEL_AUTO, cull: int = 0, lbfgs_history: int = 10, max_iters: int = 1000,
+              max_evals: int = 0) -> apd_opts:
+    o = apd_opts()
+    load_library().apd_default_opts(ctypes.byref(o))
+    o.kernel, o.cull, o.lbfgs_history, o.max_iters, o.max_evals = kernel, cull, lbfgs_history, max_iters, max_evals
+    return o
+
+
+def _dev(t: Optional[torch.Tensor], dtype, name: str, numel: Optional[int] = None):
+    if t is None:
+        return None
+    if not (t.is_cuda and t.dtype == dtype and t.is_contiguous()):
+        raise TypeError(f"{name}: expected a contiguous CUDA tensor of dtype {dtype}")
+    if numel is not None and t.numel() != numel:
+        raise ValueError(f"{name}: expected {numel} elements, got {t.numel()}")
+    return ctypes.c_void_p(t.data_ptr())
+
+
+def _host(a, dtype, name: str, numel: Optional[int] = None):
+    if a is None:
+        return None
+    if not (isinstance(a, torch.Tensor) and not a.is_cuda and a.dtype == dtype and a.is_contiguous()):
+        raise TypeError(f"{name}: expected a contiguous CPU tensor of dtype {dtype}")
+    if numel is not None and a.numel() != numel:
+        raise ValueError(f"{name}: expected {numel} elements, got {a.numel()}")
+    return ctypes.c_void_p(a.data_ptr())
+
+
+@dataclasses.dataclass
+class SolveInfo:
+    status: int
+    iters: int
+    evals: int
+    max_rel_err: float
+    dual: float
+
+
+class ApdContext:
+    """Owns an apd_ctx (workspace on one B200)."""
+
+    def __init__(self, dim: int, max_seeds: int, device: int = 0):
+        self._lib = load_library()
+        self._h = _P()
+        rc = self._lib.apd_create(ctypes.byref(self._h), dim, max_seeds, device)
+        if rc != APD_OK:
+            raise ApdError(rc, (self._lib.apd_last_error(None) or b"").decode())
+        self.dim, self.max_seeds, self.device = dim, max_seeds, device
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.apd_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, rc: int, allow=(APD_OK,)):
+        if rc not in allow:
+            raise ApdError(rc, (self._lib.apd_last_error(self._h) or b"").decode())
+        return rc
+
+    def _stream(self):
+        return ctypes.c_void_p(torch.cuda.current_stream(self.device).cuda_stream)
+
+    # -- device-pointer calls -----------------------------------------------------------------
+    def apd_assign(self, grid: apd_grid, X, A, w, target_vol=None, labels=None, vol=None, dual=None,
+                   max_rel_err=None, centroids=None, pairs_evaluated=None, opts: Optional[apd_opts] = None):
+        """apd_assign of include/apd.h on CUDA tensors; asynchronous on torch's current stream."""
+        d = grid.dim
+        M = X.shape[0]
+        rc = self._lib.apd_assign(
+            self._h, ctypes.byref(grid), M, _dev(X, torch.float32, "X", M * d), _dev(A, torch.float32, "A", M * d * d),
+            _dev(w, torch.float32, "w", M), _dev(target_vol, torch.float32, "target_vol", M),
+            _dev(labels, torch.int32, "labels"), _dev(vol, torch.float64, "vol", M),
+            _dev(dual, torch.float64, "dual", 1), _dev(max_rel_err, torch.float64, "max_rel_err", 1),
+            _dev(centroids, torch.float64, "centroids", M * d), _dev(pairs_evaluated, torch.int64, "pairs_evaluated", 1),
+            ctypes.byref(opts) if opts is not None else None, self._stream())
+        self._check(rc)
+
+    def apd_solve(self, grid: apd_grid, X, A, target_vol, tol: float, w_init=None, w=None, labels=None, vol=None,
+                  w64=None, opts: Optional[apd_opts] = None) -> SolveInfo:
+        """apd_solve of include/apd.h on CUDA tensors; blocks until finished."""
+        d = grid.dim
+        M = X.shape[0]
+        it, ev = ctypes.c_int32(0), ctypes.c_int32(0)
+        err, dual = ctypes.c_double(0.0), ctypes.c_double(0.0)
+        rc = self._lib.apd_solve(
+            self._h, ctypes.byref(grid), M, _dev(X, torch.float32, "X", M * d), _dev(A, torch.float32, "A", M * d * d),
+            _dev(target_vol, torch.float32, "target_vol", M), float(tol), _dev(w_init, torch.float32, "w_init", M),
+            _dev(w, torch.float32, "w", M), _dev(labels, torch.int32, "labels"), _dev(vol, torch.float64, "vol", M),
+            _dev(w64, torch.float64, "w64", M), ctypes.byref(it), ctypes.byref(ev), ctypes.byref(err),
+            ctypes.byref(dual), ctypes.byref(opts) if opts is not None else None, self._stream())
+        self._check(rc, allow=(APD_OK, APD_NOT_CONVERGED))
+        return SolveInfo(rc, it.value, ev.value, err.value, dual.value)
+
+    # -- host-pointer calls -------------------------------------------------------------------
+    def apd_assign_host(self, grid: apd_grid, X, A, w, target_vol=None, labels=None, vol=None, centroids=None,
+                        opts: Optional[apd_opts] = None):
+        """apd_assign_host on CPU tensors (pinned or not); returns (dual, max_rel_err, pairs)."""
+        d = grid.dim
+        M = X.shape[0]
+        dual, err = ctypes.c_double(0.0), ctypes.c_double(0.0)
+        pairs = ctypes.c_uint64(0)
+        rc = self._lib.apd_assign_host(
+            self._h, ctypes.byref(grid), M, _host(X, torch.float32, "X", M * d), _host(A, torch.float32, "A", M * d * d),
+            _host(w, torch.float32, "w", M), _host(target_vol, torch.float32, "target_vol", M),
+            _host(labels, torch.int32, "labels"), _host(vol, torch.float64, "vol", M),
+            ctypes.cast(ctypes.byref(dual), _P), ctypes.cast(ctypes.byref(err), _P),
+            _host(centroids, torch.float64, "centroids", M * d), ctypes.cast(ctypes.byref(pairs), _P),
+            ctypes.byref(opts) if opts is not None else None)
+        self._check(rc)
+        return dual.value, err.value, pairs.value
+
+    def apd_solve_host(self, grid: apd_grid, X, A, target_vol, tol: float, w_init=None, w=None, labels=None,
+                       vol=None, w64=None, opts: Optional[apd_opts] = None) -> SolveInfo:
+        d = grid.dim
+        M = X.shape[0]
+        it, ev = ctypes.c_int32(0), ctypes.c_int32(0)
+        err, dual = ctypes.c_double(0.0), ctypes.c_double(0.0)
+        rc = self._lib.apd_solve_host(
+            self._h, ctypes.byref(grid), M, _host(X, torch.float32, "X", M * d), _host(A, torch.float32, "A", M * d * d),
+            _host(target_vol, torch.float32, "target_vol", M), float(tol), _host(w_init, torch.float32, "w_init", M),
+            _host(w, torch.float32, "w", M), _host(labels, torch.int32, "labels"), _host(vol, torch.float64, "vol", M),
+            _host(w64, torch.float64, "w64", M), ctypes.byref(it), ctypes.byref(ev), ctypes.byref(err),
+            ctypes.byref(dual), ctypes.byref(opts) if opts is not None else None)
+        self._check(rc, allow=(APD_OK, APD_NOT_CONVERGED))
+        return SolveInfo(rc, it.value, ev.value, err.value, dual.value)
+
+    def last_kernel_ms(self) -> float:
+        return float(self._lib.apd_last_kernel_ms(self._h))
+
+
+def apd_fp32_probe(variant: int, device: int = 0):
+    """(ops_per_s, sm_clock_mhz) of the library's FP32 microbenchmark `variant` (include/apd.h)."""
+    lib = load_library()
+    ops, mhz = ctypes.c_double(0.0), ctypes.c_double(0.0)
+    rc = lib.apd_fp32_probe(device, variant, ctypes.byref(ops), ctypes.byref(mhz))
+    if rc != APD_OK:
+        raise ApdError(rc, "apd_fp32_probe failed")
+    return ops.value, mhz.value

@@ -1,0 +1,186 @@
+// apd_api.cu -- the C ABI of include/apd.h: context, argument validation, apd_assign and the
+// host-buffer wrappers.  Host logic only; every step of the path runs in the kernels.
+#include "apd_internal.cuh"
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+using namespace apd;
+
+static thread_local std::string g_create_err;
+
+#define APD_CUDA_TRY(ctx, call)                                                              \
+  do {                                                                                       \
+    cudaError_t e__ = (call);                                                                \
+    if (e__ != cudaSuccess) {                                                                \
+      (ctx)->err = std::string(#call) + ": " + cudaGetErrorString(e__);                      \
+      return APD_E_CUDA;                                                                     \
+    }                                                                                        \
+  } while (0)
+
+extern "C" void apd_default_opts(apd_opts* o) {
+  if (!o) return;
+  std::memset(o, 0, sizeof(*o));
+  o->kernel = APD_KERNEL_AUTO;
+  o->cull = 0;
+  o->lbfgs_history = 10;
+  o->max_iters = 1000;
+  o->max_evals = 0;
+}
+
+static void free_ws(Workspace& ws) {
+  cudaFree(ws.seeds); cudaFree(ws.count); cudaFree(ws.idxsum); cudaFree(ws.dual_partial);
+  cudaFree(ws.sstate); cudaFree(ws.svec); cudaFree(ws.w32); cudaFree(ws.e_vol); cudaFree(ws.e_scal);
+  if (ws.report) cudaFreeHost(ws.report);
+  for (int i = 0; i < 2; ++i) if (ws.sev[i]) cudaEventDestroy(ws.sev[i]);
+  if (ws.ev0) cudaEventDestroy(ws.ev0);
+  if (ws.ev1) cudaEventDestroy(ws.ev1);
+  ws = Workspace();
+}
+
+extern "C" int apd_create(apd_ctx** out, int32_t dim, int32_t max_seeds, int32_t device) {
+  if (!out) { g_create_err = "apd_create: out is NULL"; return APD_E_ARG; }
+  *out = nullptr;
+  if (dim != 2 && dim != 3) { g_create_err = "apd_create: dim must be 2 or 3"; return APD_E_ARG; }
+  if (max_seeds < 1) { g_create_err = "apd_create: max_seeds must be >= 1"; return APD_E_ARG; }
+  cudaDeviceProp prop;
+  cudaError_t e = cudaGetDeviceProperties(&prop, device);
+  if (e != cudaSuccess) { g_create_err = std::string("cudaGetDeviceProperties: ") + cudaGetErrorString(e); return APD_E_CUDA; }
+  if (prop.major != 10) {
+    g_create_err = "apd_create: device is compute capability " + std::to_string(prop.major) + "." +
+                   std::to_string(prop.minor) + "; this library is built for sm_100a only";
+    return APD_E_ARCH;
+  }
+  e = cudaSetDevice(device);
+  if (e != cudaSuccess) { g_create_err = std::string("cudaSetDevice: ") + cudaGetErrorString(e); return APD_E_CUDA; }
+  apd_ctx* c = new (std::nothrow) apd_ctx();
+  if (!c) { g_create_err = "apd_create: out of host memory"; return APD_E_CUDA; }
+  Workspace& ws = c->ws;
+  ws.dim = dim; ws.max_seeds = max_seeds; ws.device = device; ws.sm_count = prop.multiProcessorCount;
+  const size_t m_pad = ((size_t)max_seeds + SEED_CHUNK - 1) / SEED_CHUNK * SEED_CHUNK;
+  ws.partial_cap = 1 << 16;
+  bool ok = cudaMalloc(&ws.seeds, m_pad * rec_floats(dim) * sizeof(float)) == cudaSuccess &&
+            cudaMalloc(&ws.count, (size_t)max_seeds * sizeof(unsigned int)) == cudaSuccess &&
+            cudaMalloc(&ws.idxsum, (size_t)max_seeds * 3 * sizeof(unsigned long long)) == cudaSuccess &&
+            cudaMalloc(&ws.dual_partial, ws.partial_cap * sizeof(double)) == cudaSuccess &&
+            cudaEventCreate(&ws.ev0) == cudaSuccess && cudaEventCreate(&ws.ev1) == cudaSuccess;
+  if (!ok) {
+    g_create_err = std::string("apd_create: workspace allocation failed: ") + cudaGetErrorString(cudaGetLastError());
+    free_ws(ws);
+    delete c;
+    return APD_E_CUDA;
+  }
+  *out = c;
+  return APD_OK;
+}
+
+extern "C" void apd_destroy(apd_ctx* ctx) {
+  if (!ctx) return;
+  cudaSetDevice(ctx->ws.device);
+  free_ws(ctx->ws);
+  delete ctx;
+}
+
+extern "C" const char* apd_last_error(const apd_ctx* ctx) {
+  return ctx ? ctx->err.c_str() : g_create_err.c_str();
+}
+
+namespace apd {
+
+// Validates the grid and fills the device-side description.  Returns "" or an error text.
+std::string make_grid(const apd_ctx* ctx, const apd_grid* grid, int kernel, GridDev* g) {
+  if (!grid) return "grid is NULL";
+  if (grid->dim != ctx->ws.dim) return "grid.dim differs from the context's dim";
+  const int d = grid->dim;
+  long long N = 1;
+  double P = 1.0;
+  GridDev out;
+  std::memset(&out, 0, sizeof(out));
+  out.dim = d;
+  int n[3] = {1, 1, 1};
+  for (int k = 0; k < d; ++k) {
+    if (grid->n[k] < 1) return "grid.n[k] must be >= 1";
+    if (!(grid->hi[k] > grid->lo[k]) || !std::isfinite(grid->hi[k]) || !std::isfinite(grid->lo[k]))
+      return "grid needs finite hi[k] > lo[k]";
+    n[k] = grid->n[k];
+    N *= n[k];
+    if (N >= (1ll << 31)) return "grid has 2^31 voxels or more";
+    out.lo[k] = grid->lo[k];
+    out.s[k] = (grid->hi[k] - grid->lo[k]) / (double)n[k];
+    P *= out.s[k];
+  }
+  out.nx = n[0]; out.ny = n[1]; out.nz = n[2];
+  out.voxel_volume = P;
+  assign_tile_counts(kernel, d, out.nx, out.ny, out.nz, &out.tiles_x, &out.tiles_y, &out.tiles_z);
+  *g = out;
+  return "";
+}
+
+int resolve_kernel(const apd_opts* o, std::string* err) {
+  int k = o ? o->kernel : APD_KERNEL_AUTO;
+  if (k != APD_KERNEL_AUTO && k != APD_KERNEL_DIRECT && k != APD_KERNEL_ROWPOLY) { *err = "unknown opts.kernel"; return -1; }
+  if (o && (o->cull != 0 && o->cull != 1)) { *err = "opts.cull must be 0 or 1"; return -1; }
+  if (o && (o->reserved[0] || o->reserved[1] || o->reserved[2])) { *err = "opts.reserved must be 0"; return -1; }
+  if (k == APD_KERNEL_AUTO) k = APD_KERNEL_DIRECT;
+  return k;
+}
+
+// Enqueues one evaluation (pack -> assign -> finalize) on `st`.  All pointers device.
+int enqueue_evaluation(apd_ctx* ctx, const GridDev& g, int kernel, int M, const float* X, const float* A,
+                       const float* w, const float* target_vol, int32_t* labels, double* vol, double* dual,
+                       double* max_rel_err, double* centroids, uint64_t* pairs, bool timed,
+                       const int* done_flag, cudaStream_t st) {
+  Workspace& ws = ctx->ws;
+  const int M_pad = (M + SEED_CHUNK - 1) / SEED_CHUNK * SEED_CHUNK;
+  const int n_tiles = g.tiles_x * g.tiles_y * g.tiles_z;
+  if ((size_t)n_tiles > ws.partial_cap) {
+    // grow the per-tile partial buffer (stream-ordered free/alloc keeps earlier work valid)
+    APD_CUDA_TRY(ctx, cudaStreamSynchronize(st));
+    APD_CUDA_TRY(ctx, cudaFree(ws.dual_partial));
+    ws.dual_partial = nullptr;
+    ws.partial_cap = (size_t)n_tiles;
+    APD_CUDA_TRY(ctx, cudaMalloc(&ws.dual_partial, ws.partial_cap * sizeof(double)));
+  }
+  APD_CUDA_TRY(ctx, launch_pack_seeds(g.dim, M, M_pad, X, A, w, ws.seeds, ws.count,
+                                      centroids ? ws.idxsum : nullptr, done_flag, st));
+  AssignArgs a;
+  a.g = g; a.M = M; a.M_pad = M_pad; a.seeds = ws.seeds; a.labels = labels; a.count = ws.count;
+  a.idxsum = centroids ? ws.idxsum : nullptr; a.dual_partial = ws.dual_partial;
+  a.done_flag = done_flag;
+  if (timed) APD_CUDA_TRY(ctx, cudaEventRecord(ws.ev0, st));
+  APD_CUDA_TRY(ctx, launch_assign(kernel, a, st));
+  if (timed) { APD_CUDA_TRY(ctx, cudaEventRecord(ws.ev1, st)); ws.timed = true; }
+  APD_CUDA_TRY(ctx, launch_finalize(g, M, n_tiles, ws.count, a.idxsum, ws.dual_partial, X, w, target_vol, vol,
+                                    dual, max_rel_err, centroids, pairs, done_flag, st));
+  return APD_OK;
+}
+
+}  // namespace apd
+
+extern "C" int apd_assign(apd_ctx* ctx, const apd_grid* grid, int32_t M, const float* X, const float* A,
+                          const float* w, const float* target_vol, int32_t* labels, double* vol, double* dual,
+                          double* max_rel_err, double* centroids, uint64_t* pairs_evaluated,
+                          const apd_opts* opts, void* cuda_stream) {
+  if (!ctx) return APD_E_ARG;
+  ctx->err.clear();
+  std::string e;
+  const int kernel = resolve_kernel(opts, &e);
+  if (kernel < 0) { ctx->err = "apd_assign: " + e; return APD_E_ARG; }
+  if (M < 1 || M > ctx->ws.max_seeds) { ctx->err = "apd_assign: M out of range [1, max_seeds]"; return APD_E_ARG; }
+  if (!X || !A || !w || !vol || !dual) { ctx->err = "apd_assign: X, A, w, vol and dual are required"; return APD_E_ARG; }
+  GridDev g;
+  e = make_grid(ctx, grid, kernel, &g);
+  if (!e.empty()) { ctx->err = "apd_assign: " + e; return APD_E_ARG; }
+  APD_CUDA_TRY(ctx, cudaSetDevice(ctx->ws.device));
+  return enqueue_evaluation(ctx, g, kernel, M, X, A, w, target_vol, labels, vol, dual, max_rel_err, centroids,
+                            pairs_evaluated, true, nullptr, static_cast<cudaStream_t>(cuda_stream));
+}
+
+extern "C" double apd_last_kernel_ms(apd_ctx* ctx) {
+  if (!ctx || !ctx->ws.timed) return -1.0;
+  if (cudaEventSynchronize(ctx->ws.ev1) != cudaSuccess) return -1.0;
+  float ms = 0.f;
+  if (cudaEventElapsedTime(&ms, ctx->ws.ev0, ctx->ws.ev1) != cudaSuccess) return -1.0;
+  return (double)ms;
+}

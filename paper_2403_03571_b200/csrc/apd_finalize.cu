@@ -1,0 +1,81 @@
+// apd_finalize.cu -- a9: turn the integer histograms and the per-tile partial sums of one
+// evaluation into vol (eq. 2.8), the dual g~ (eq. 2.7, via
+// identity I1: g~ = sum_i v_i w_i + |P| sum_j min_i C_ij), the stopping quantity of eq. (2.5)
+// and the discrete centroids.  One CTA, fixed reduction order:
+// the result is bitwise reproducible run to run.
+#include "apd_internal.cuh"
+#include "apd_device.cuh"
+
+namespace apd {
+
+constexpr int FIN_THREADS = 1024;
+
+__device__ __forceinline__ double block_max_double(double v, double* scratch) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_down_sync(0xffffffffu, v, o));
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  __syncthreads();
+  if (lane == 0) scratch[wid] = v;
+  __syncthreads();
+  double t = 0.0;
+  if (threadIdx.x == 0)
+    for (int i = 0; i < FIN_THREADS / 32; ++i) t = fmax(t, scratch[i]);
+  return t;
+}
+
+__global__ void __launch_bounds__(FIN_THREADS) finalize_kernel(
+    GridDev g, int M, int n_partials, const unsigned int* __restrict__ count,
+    const unsigned long long* __restrict__ idxsum, const double* __restrict__ dual_partial,
+    const float* __restrict__ X, const float* __restrict__ w, const float* __restrict__ target_vol,
+    double* __restrict__ vol, double* __restrict__ dual, double* __restrict__ max_rel_err,
+    double* __restrict__ centroids, uint64_t* __restrict__ pairs_evaluated,
+    const int* __restrict__ done_flag) {
+  __shared__ double scratch[FIN_THREADS / 32];
+  if (done_flag && *done_flag) return;
+  const int tid = threadIdx.x;
+  const double P = g.voxel_volume;
+  double vw = 0.0, err = 0.0;
+  for (int i = tid; i < M; i += FIN_THREADS) {
+    const unsigned int c = count[i];
+    const double vi = (double)c * P;                       // m_i |P|
+    vol[i] = vi;
+    if (target_vol) {
+      const double tv = (double)target_vol[i];
+      vw += tv * (double)w[i];
+      err = fmax(err, fabs(vi - tv) / tv);                 // eq. (2.5)
+    }
+    if (centroids) {
+      for (int k = 0; k < g.dim; ++k) {
+        double ck;
+        if (c > 0) ck = g.lo[k] + g.s[k] * ((double)idxsum[(size_t)i * 3 + k] / (double)c + 0.5);
+        else       ck = (double)X[(size_t)i * g.dim + k];  // empty cell keeps its seed (reading S5)
+        centroids[(size_t)i * g.dim + k] = ck;
+      }
+    }
+  }
+  double smin = 0.0;
+  for (int t = tid; t < n_partials; t += FIN_THREADS) smin += dual_partial[t];
+
+  const double vw_tot = block_sum_double<FIN_THREADS>(vw, scratch);
+  __syncthreads();
+  const double smin_tot = block_sum_double<FIN_THREADS>(smin, scratch);
+  const double err_tot = block_max_double(err, scratch);
+  if (tid == 0) {
+    *dual = vw_tot + P * smin_tot;
+    if (max_rel_err && target_vol) *max_rel_err = err_tot;
+    if (pairs_evaluated)
+      *pairs_evaluated = (uint64_t)g.nx * (uint64_t)g.ny * (uint64_t)g.nz * (uint64_t)M;
+  }
+}
+
+cudaError_t launch_finalize(const GridDev& g, int M, int n_partials, const unsigned int* count,
+                            const unsigned long long* idxsum, const double* dual_partial,
+                            const float* X, const float* w, const float* target_vol,
+                            double* vol, double* dual, double* max_rel_err, double* centroids,
+                            uint64_t* pairs_evaluated, const int* done_flag, cudaStream_t st) {
+  finalize_kernel<<<1, FIN_THREADS, 0, st>>>(g, M, n_partials, count, idxsum, dual_partial, X, w, target_vol,
+                                             vol, dual, max_rel_err, centroids, pairs_evaluated, done_flag);
+  return cudaGetLastError();
+}
+
+}  // namespace apd

@@ -1,0 +1,130 @@
+// apd_host.cu -- apd_assign_host / apd_solve_host: the same calls with HOST arrays.  The library
+// allocates device buffers, copies in (cudaMemcpyAsync, one per array), runs the device call,
+// copies out.  Used for the end-to-end ("e2e") measurement and by callers without a device
+// allocator of their own.
+#include "apd_internal.cuh"
+#include <vector>
+
+namespace {
+
+struct DevBufs {
+  std::vector<void*> ptrs;
+  ~DevBufs() { for (void* p : ptrs) cudaFree(p); }
+  template <typename T>
+  cudaError_t alloc(T** out, size_t count) {
+    void* p = nullptr;
+    cudaError_t e = cudaMalloc(&p, count * sizeof(T));
+    if (e == cudaSuccess) ptrs.push_back(p);
+    *out = static_cast<T*>(p);
+    return e;
+  }
+};
+
+#define HOST_TRY(call)                                                              \
+  do {                                                                              \
+    cudaError_t e__ = (call);                                                       \
+    if (e__ != cudaSuccess) {                                                       \
+      ctx->err = std::string(#call) + ": " + cudaGetErrorString(e__);               \
+      return APD_E_CUDA;                                                            \
+    }                                                                               \
+  } while (0)
+
+long long grid_voxels(const apd_grid* g) {
+  long long N = 1;
+  for (int k = 0; k < g->dim && k < 3; ++k) N *= (g->n[k] > 0 ? g->n[k] : 0);
+  return N;
+}
+
+}  // namespace
+
+extern "C" int apd_assign_host(apd_ctx* ctx, const apd_grid* grid, int32_t M, const float* X, const float* A,
+                               const float* w, const float* target_vol, int32_t* labels, double* vol,
+                               double* dual, double* max_rel_err, double* centroids,
+                               uint64_t* pairs_evaluated, const apd_opts* opts) {
+  if (!ctx) return APD_E_ARG;
+  ctx->err.clear();
+  if (!grid || (grid->dim != 2 && grid->dim != 3) || M < 1 || !X || !A || !w || !vol || !dual) {
+    ctx->err = "apd_assign_host: bad arguments";
+    return APD_E_ARG;
+  }
+  const int d = grid->dim;
+  const long long N = grid_voxels(grid);
+  if (N < 1 || N >= (1ll << 31)) { ctx->err = "apd_assign_host: bad grid"; return APD_E_ARG; }
+  HOST_TRY(cudaSetDevice(ctx->ws.device));
+  DevBufs b;
+  float *dX, *dA, *dw, *dv = nullptr;
+  int32_t* dl = nullptr;
+  double *dvol, *dscal, *dcen = nullptr;
+  uint64_t* dpairs;
+  HOST_TRY(b.alloc(&dX, (size_t)M * d));
+  HOST_TRY(b.alloc(&dA, (size_t)M * d * d));
+  HOST_TRY(b.alloc(&dw, (size_t)M));
+  if (target_vol) HOST_TRY(b.alloc(&dv, (size_t)M));
+  if (labels) HOST_TRY(b.alloc(&dl, (size_t)N));
+  HOST_TRY(b.alloc(&dvol, (size_t)M));
+  HOST_TRY(b.alloc(&dscal, 2));
+  if (centroids) HOST_TRY(b.alloc(&dcen, (size_t)M * d));
+  HOST_TRY(b.alloc(&dpairs, 1));
+  cudaStream_t st = nullptr;
+  HOST_TRY(cudaMemcpyAsync(dX, X, sizeof(float) * M * d, cudaMemcpyHostToDevice, st));
+  HOST_TRY(cudaMemcpyAsync(dA, A, sizeof(float) * M * d * d, cudaMemcpyHostToDevice, st));
+  HOST_TRY(cudaMemcpyAsync(dw, w, sizeof(float) * M, cudaMemcpyHostToDevice, st));
+  if (target_vol) HOST_TRY(cudaMemcpyAsync(dv, target_vol, sizeof(float) * M, cudaMemcpyHostToDevice, st));
+  HOST_TRY(cudaMemsetAsync(dscal, 0, 2 * sizeof(double), st));
+  const int rc = apd_assign(ctx, grid, M, dX, dA, dw, dv, dl, dvol, dscal, dscal + 1, dcen, dpairs, opts, st);
+  if (rc != APD_OK) return rc;
+  if (labels) HOST_TRY(cudaMemcpyAsync(labels, dl, sizeof(int32_t) * N, cudaMemcpyDeviceToHost, st));
+  HOST_TRY(cudaMemcpyAsync(vol, dvol, sizeof(double) * M, cudaMemcpyDeviceToHost, st));
+  double scal[2] = {0, 0};
+  HOST_TRY(cudaMemcpyAsync(scal, dscal, sizeof(scal), cudaMemcpyDeviceToHost, st));
+  if (centroids) HOST_TRY(cudaMemcpyAsync(centroids, dcen, sizeof(double) * M * d, cudaMemcpyDeviceToHost, st));
+  uint64_t pairs = 0;
+  HOST_TRY(cudaMemcpyAsync(&pairs, dpairs, sizeof(pairs), cudaMemcpyDeviceToHost, st));
+  HOST_TRY(cudaStreamSynchronize(st));
+  *dual = scal[0];
+  if (max_rel_err && target_vol) *max_rel_err = scal[1];
+  if (pairs_evaluated) *pairs_evaluated = pairs;
+  return APD_OK;
+}
+
+extern "C" int apd_solve_host(apd_ctx* ctx, const apd_grid* grid, int32_t M, const float* X, const float* A,
+                              const float* target_vol, double tol, const float* w_init, float* w,
+                              int32_t* labels, double* vol, double* w64, int32_t* iters, int32_t* evals,
+                              double* max_rel_err, double* dual, const apd_opts* opts) {
+  if (!ctx) return APD_E_ARG;
+  ctx->err.clear();
+  if (!grid || (grid->dim != 2 && grid->dim != 3) || M < 1 || !X || !A || !target_vol || !w) {
+    ctx->err = "apd_solve_host: bad arguments";
+    return APD_E_ARG;
+  }
+  const int d = grid->dim;
+  const long long N = grid_voxels(grid);
+  if (N < 1 || N >= (1ll << 31)) { ctx->err = "apd_solve_host: bad grid"; return APD_E_ARG; }
+  HOST_TRY(cudaSetDevice(ctx->ws.device));
+  DevBufs b;
+  float *dX, *dA, *dv, *dwi = nullptr, *dw;
+  int32_t* dl = nullptr;
+  double *dvol = nullptr, *dw64 = nullptr;
+  HOST_TRY(b.alloc(&dX, (size_t)M * d));
+  HOST_TRY(b.alloc(&dA, (size_t)M * d * d));
+  HOST_TRY(b.alloc(&dv, (size_t)M));
+  if (w_init) HOST_TRY(b.alloc(&dwi, (size_t)M));
+  HOST_TRY(b.alloc(&dw, (size_t)M));
+  if (labels) HOST_TRY(b.alloc(&dl, (size_t)N));
+  if (vol) HOST_TRY(b.alloc(&dvol, (size_t)M));
+  if (w64) HOST_TRY(b.alloc(&dw64, (size_t)M));
+  cudaStream_t st = nullptr;
+  HOST_TRY(cudaMemcpyAsync(dX, X, sizeof(float) * M * d, cudaMemcpyHostToDevice, st));
+  HOST_TRY(cudaMemcpyAsync(dA, A, sizeof(float) * M * d * d, cudaMemcpyHostToDevice, st));
+  HOST_TRY(cudaMemcpyAsync(dv, target_vol, sizeof(float) * M, cudaMemcpyHostToDevice, st));
+  if (w_init) HOST_TRY(cudaMemcpyAsync(dwi, w_init, sizeof(float) * M, cudaMemcpyHostToDevice, st));
+  const int rc = apd_solve(ctx, grid, M, dX, dA, dv, tol, dwi, dw, dl, dvol, dw64, iters, evals, max_rel_err,
+                           dual, opts, st);
+  if (rc < 0) return rc;
+  HOST_TRY(cudaMemcpyAsync(w, dw, sizeof(float) * M, cudaMemcpyDeviceToHost, st));
+  if (labels) HOST_TRY(cudaMemcpyAsync(labels, dl, sizeof(int32_t) * N, cudaMemcpyDeviceToHost, st));
+  if (vol) HOST_TRY(cudaMemcpyAsync(vol, dvol, sizeof(double) * M, cudaMemcpyDeviceToHost, st));
+  if (w64) HOST_TRY(cudaMemcpyAsync(w64, dw64, sizeof(double) * M, cudaMemcpyDeviceToHost, st));
+  HOST_TRY(cudaStreamSynchronize(st));
+  return rc;
+}

@@ -1,0 +1,100 @@
+// apd_internal.cuh -- declarations shared by the translation units of libapd_b200 (sm_100a only).
+// Nothing here is shared with oracle/: the oracle is an independent fp64 CPU program.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string>
+#include "../../include/apd.h"
+
+namespace apd {
+
+// Packed seed record: REC floats per seed, 16-byte aligned so a chunk
+// of seeds is one contiguous cp.async.bulk (TMA 1-D bulk copy) source.
+//   3D (12 floats): x y z a11 | a12' a13' a22 a23' | a33 nw 0 0      a_kl' = A_kl + A_lk
+//   2D ( 8 floats): x y a11 a12' | a22 nw 0 0                        nw = -w
+// The table is padded to a multiple of SEED_CHUNK with records {0.., nw = +inf} whose cost is
+// +inf and therefore never wins the strict '<' argmin.
+constexpr int REC3 = 12;
+constexpr int REC2 = 8;
+constexpr int SEED_CHUNK = 128;                  // seeds per smem stage
+constexpr int SEED_STAGES = 2;                   // double buffer
+
+__host__ __device__ constexpr int rec_floats(int dim) { return dim == 3 ? REC3 : REC2; }
+
+// Grid as the kernels see it.  Voxel centres are formed in fp64 exactly as the definition
+// and split into fp32 hi + lo parts.
+struct GridDev {
+  int dim;
+  int nx, ny, nz;
+  double lo[3];
+  double s[3];          // voxel side lengths
+  double voxel_volume;  // |P|
+  int tiles_x, tiles_y, tiles_z;
+};
+
+struct AssignArgs {
+  GridDev g;
+  int M;                 // real seeds
+  int M_pad;             // padded to SEED_CHUNK
+  const float* seeds;    // [M_pad, REC]
+  int32_t* labels;       // [N] or nullptr
+  unsigned int* count;   // [M] voxels per cell (exact integers: eq. 2.8)
+  unsigned long long* idxsum;  // [M,3] sum of voxel indices per axis, or nullptr
+  double* dual_partial;  // [n_tiles] sum over the tile of min_i C_ij
+  const int* done_flag;  // solve loop only: kernels return at once when *done_flag != 0; else nullptr
+};
+
+struct Workspace {
+  int dim = 0, max_seeds = 0, device = 0, sm_count = 0;
+  float* seeds = nullptr;              // packed table [M_pad, REC]
+  unsigned int* count = nullptr;       // [max_seeds]
+  unsigned long long* idxsum = nullptr;  // [max_seeds,3]
+  double* dual_partial = nullptr;      // [partial_cap]
+  size_t partial_cap = 0;
+  cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+  bool timed = false;
+  // apd_solve state (apd_lbfgs.cu), allocated on first use
+  struct SolveState* sstate = nullptr;  // device scalars
+  double* svec = nullptr;               // device fp64 vectors: w, g, p, w_try, w_best, g_new, q, S[m], Y[m]
+  int svec_hist = 0;                    // history capacity svec was sized for
+  float* w32 = nullptr;                 // [max_seeds] fl32(w) the next evaluation uses
+  double* e_vol = nullptr;              // [max_seeds] evaluation outputs inside the solve loop
+  double* e_scal = nullptr;             // [2] dual, max_rel_err
+  struct SolveReport* report = nullptr; // pinned, mapped host memory the step kernel writes
+  cudaEvent_t sev[2] = {nullptr, nullptr};
+};
+
+// kernels (apd_kernels.cu)
+cudaError_t launch_pack_seeds(int dim, int M, int M_pad, const float* X, const float* A, const float* w,
+                              float* seeds, unsigned int* count, unsigned long long* idxsum,
+                              const int* done_flag, cudaStream_t st);
+cudaError_t launch_assign(int kernel, const AssignArgs& a, cudaStream_t st);
+void assign_tile_counts(int kernel, int dim, int nx, int ny, int nz, int* tx, int* ty, int* tz);
+cudaError_t launch_finalize(const GridDev& g, int M, int n_partials, const unsigned int* count,
+                            const unsigned long long* idxsum, const double* dual_partial,
+                            const float* X, const float* w, const float* target_vol,
+                            double* vol, double* dual, double* max_rel_err, double* centroids,
+                            uint64_t* pairs_evaluated, const int* done_flag, cudaStream_t st);
+
+// What the device-side optimiser reports to the host (mapped pinned memory).
+struct SolveReport {
+  volatile int done;      // 0 running, 1 finished
+  volatile int status;    // apd_status
+  volatile int iters, evals;
+  volatile double err, dual;
+};
+
+// host helpers shared by apd_api.cu and apd_lbfgs.cu
+std::string make_grid(const apd_ctx* ctx, const apd_grid* grid, int kernel, GridDev* g);
+int resolve_kernel(const apd_opts* o, std::string* err);
+int enqueue_evaluation(apd_ctx* ctx, const GridDev& g, int kernel, int M, const float* X, const float* A,
+                       const float* w, const float* target_vol, int32_t* labels, double* vol, double* dual,
+                       double* max_rel_err, double* centroids, uint64_t* pairs, bool timed,
+                       const int* done_flag, cudaStream_t st);
+
+}  // namespace apd
+
+struct apd_ctx {
+  apd::Workspace ws;
+  std::string err;
+};

@@ -1,0 +1,134 @@
+// apd_probe.cu -- register-only FP32 microbenchmarks that define the measured FP32 roofline
+// denominators of DESIGN.md "Measurement" (MEASURED_PEAKS.json holds no FP32 CUDA-core figure).
+// Not part of the method.
+#include "apd_internal.cuh"
+#include "apd_device.cuh"
+
+namespace apd {
+
+constexpr int PROBE_ACC = 16;
+constexpr int PROBE_ITERS = 8192;
+
+__device__ __forceinline__ unsigned long long globaltimer_ns() {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+  return t;
+}
+
+template <int VARIANT>
+__global__ void __launch_bounds__(256) probe_kernel(float* out, const float* in, unsigned long long* clk) {
+  const int tid = blockIdx.x * blockDim.x + threadIdx.x;
+  unsigned long long c0 = 0, t0 = 0;
+  if (tid == 0) { c0 = clock64(); t0 = globaltimer_ns(); }
+  const float b = in[threadIdx.x & 31], c = in[32 + (threadIdx.x & 31)];
+  float res = 0.f;
+  if (VARIANT == 0) {
+    float acc[PROBE_ACC];
+#pragma unroll
+    for (int k = 0; k < PROBE_ACC; ++k) acc[k] = (float)k * c;
+    for (int it = 0; it < PROBE_ITERS; ++it) {
+#pragma unroll
+      for (int k = 0; k < PROBE_ACC; ++k) asm volatile("fma.rn.f32 %0, %0, %1, %2;" : "+f"(acc[k]) : "f"(b), "f"(c));
+    }
+#pragma unroll
+    for (int k = 0; k < PROBE_ACC; ++k) res += acc[k];
+  } else if (VARIANT == 1) {
+    f2 acc[PROBE_ACC];
+    const f2 bb = f2_pack(b, b), cc = f2_pack(c, c);
+#pragma unroll
+    for (int k = 0; k < PROBE_ACC; ++k) acc[k] = f2_pack((float)k * c, (float)k);
+    for (int it = 0; it < PROBE_ITERS; ++it) {
+#pragma unroll
+      for (int k = 0; k < PROBE_ACC; ++k) asm volatile("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(acc[k]) : "l"(bb), "l"(cc));
+    }
+#pragma unroll
+    for (int k = 0; k < PROBE_ACC; ++k) { float lo, hi; f2_unpack(acc[k], lo, hi); res += lo + hi; }
+  } else if (VARIANT == 2) {
+    float acc[PROBE_ACC];
+#pragma unroll
+    for (int k = 0; k < PROBE_ACC; ++k) acc[k] = (float)k * c;
+    for (int it = 0; it < PROBE_ITERS; ++it) {
+#pragma unroll
+      for (int k = 0; k < PROBE_ACC; ++k) asm volatile("min.f32 %0, %0, %1, %2;" : "+f"(acc[k]) : "f"(b), "f"(c));
+    }
+#pragma unroll
+    for (int k = 0; k < PROBE_ACC; ++k) res += acc[k];
+  } else {
+    // the ROWPOLY inner loop: per voxel k and seed pair: u = fma2(a11, t_k, B); c = fma2(t_k, u, R);
+    // best_k = min3(best_k, c.lo, c.hi)
+    f2 tt[PROBE_ACC];
+    float best[PROBE_ACC];
+#pragma unroll
+    for (int k = 0; k < PROBE_ACC; ++k) { tt[k] = f2_pack((float)k * c, (float)k * c); best[k] = 3.0e38f; }
+    f2 a11 = f2_pack(b, c), B = f2_pack(c, b), R = f2_pack(b + c, b - c);
+    const f2 inc = f2_pack(1e-3f, 2e-3f);
+    for (int it = 0; it < PROBE_ITERS; ++it) {
+#pragma unroll
+      for (int k = 0; k < PROBE_ACC; ++k) {
+        f2 u, cst;
+        float lo, hi;
+        asm volatile("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(u) : "l"(a11), "l"(tt[k]), "l"(B));
+        asm volatile("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(cst) : "l"(tt[k]), "l"(u), "l"(R));
+        f2_unpack(cst, lo, hi);
+        asm volatile("min.f32 %0, %0, %1, %2;" : "+f"(best[k]) : "f"(lo), "f"(hi));
+      }
+      B = f2_add(B, inc);
+      R = f2_add(R, inc);
+    }
+#pragma unroll
+    for (int k = 0; k < PROBE_ACC; ++k) res += best[k];
+  }
+  if (res == 123.456f) out[tid] = res;   // keeps the work alive without a store in practice
+  if (tid == 0) { clk[0] = clock64() - c0; clk[1] = globaltimer_ns() - t0; }
+}
+
+}  // namespace apd
+
+extern "C" int apd_fp32_probe(int32_t device, int32_t variant, double* ops_per_s, double* sm_clock_mhz) {
+  using namespace apd;
+  if (variant < 0 || variant > 3 || !ops_per_s) return APD_E_ARG;
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return APD_E_CUDA;
+  if (prop.major != 10) return APD_E_ARCH;
+  if (cudaSetDevice(device) != cudaSuccess) return APD_E_CUDA;
+  float *d_in = nullptr, *d_out = nullptr;
+  unsigned long long* d_clk = nullptr;
+  const int blocks = prop.multiProcessorCount * 8, threads = 256;
+  float h_in[64];
+  for (int i = 0; i < 64; ++i) h_in[i] = 0.999f + 1e-4f * (float)i;
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  int rc = APD_E_CUDA;
+  do {
+    if (cudaMalloc(&d_in, sizeof(h_in)) != cudaSuccess) break;
+    if (cudaMalloc(&d_out, sizeof(float) * blocks * threads) != cudaSuccess) break;
+    if (cudaMalloc(&d_clk, 2 * sizeof(unsigned long long)) != cudaSuccess) break;
+    if (cudaMemcpy(d_in, h_in, sizeof(h_in), cudaMemcpyHostToDevice) != cudaSuccess) break;
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) break;
+    double best_ms = 1e30;
+    for (int rep = 0; rep < 5; ++rep) {   // rep 0-1 warm up
+      cudaEventRecord(e0, nullptr);
+      switch (variant) {
+        case 0: probe_kernel<0><<<blocks, threads>>>(d_out, d_in, d_clk); break;
+        case 1: probe_kernel<1><<<blocks, threads>>>(d_out, d_in, d_clk); break;
+        case 2: probe_kernel<2><<<blocks, threads>>>(d_out, d_in, d_clk); break;
+        default: probe_kernel<3><<<blocks, threads>>>(d_out, d_in, d_clk); break;
+      }
+      cudaEventRecord(e1, nullptr);
+      if (cudaEventSynchronize(e1) != cudaSuccess) { best_ms = -1; break; }
+      float ms = 0.f;
+      cudaEventElapsedTime(&ms, e0, e1);
+      if (rep >= 2 && ms < best_ms) best_ms = ms;
+    }
+    if (best_ms <= 0) break;
+    unsigned long long h_clk[2] = {0, 0};
+    if (cudaMemcpy(h_clk, d_clk, sizeof(h_clk), cudaMemcpyDeviceToHost) != cudaSuccess) break;
+    const double per_thread = (double)PROBE_ITERS * PROBE_ACC * ((variant == 1 || variant == 3) ? 2.0 : 1.0);
+    *ops_per_s = per_thread * (double)blocks * threads / (best_ms * 1e-3);
+    if (sm_clock_mhz) *sm_clock_mhz = h_clk[1] ? (double)h_clk[0] / (double)h_clk[1] * 1e3 : 0.0;
+    rc = APD_OK;
+  } while (0);
+  if (e0) cudaEventDestroy(e0);
+  if (e1) cudaEventDestroy(e1);
+  cudaFree(d_in); cudaFree(d_out); cudaFree(d_clk);
+  return rc;
+}
