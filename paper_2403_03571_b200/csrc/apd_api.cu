@@ -122,7 +122,7 @@ int resolve_kernel(const apd_opts* o, std::string* err) {
   if (k != APD_KERNEL_AUTO && k != APD_KERNEL_DIRECT && k != APD_KERNEL_ROWPOLY) { *err = "unknown opts.kernel"; return -1; }
   if (o && (o->cull != 0 && o->cull != 1)) { *err = "opts.cull must be 0 or 1"; return -1; }
   if (o && (o->reserved[0] || o->reserved[1] || o->reserved[2])) { *err = "opts.reserved must be 0"; return -1; }
-  if (k == APD_KERNEL_AUTO) k = APD_KERNEL_DIRECT;
+  if (k == APD_KERNEL_AUTO) k = APD_KERNEL_ROWPOLY;
   return k;
 }
 
@@ -142,8 +142,12 @@ int enqueue_evaluation(apd_ctx* ctx, const GridDev& g, int kernel, int M, const 
     ws.partial_cap = (size_t)n_tiles;
     APD_CUDA_TRY(ctx, cudaMalloc(&ws.dual_partial, ws.partial_cap * sizeof(double)));
   }
-  APD_CUDA_TRY(ctx, launch_pack_seeds(g.dim, M, M_pad, X, A, w, ws.seeds, ws.count,
-                                      centroids ? ws.idxsum : nullptr, done_flag, st));
+  if (kernel == APD_KERNEL_ROWPOLY)
+    APD_CUDA_TRY(ctx, launch_pack_pairs(g.dim, M, M_pad, X, A, w, ws.seeds, ws.count,
+                                        centroids ? ws.idxsum : nullptr, done_flag, st));
+  else
+    APD_CUDA_TRY(ctx, launch_pack_seeds(g.dim, M, M_pad, X, A, w, ws.seeds, ws.count,
+                                        centroids ? ws.idxsum : nullptr, done_flag, st));
   AssignArgs a;
   a.g = g; a.M = M; a.M_pad = M_pad; a.seeds = ws.seeds; a.labels = labels; a.count = ws.count;
   a.idxsum = centroids ? ws.idxsum : nullptr; a.dual_partial = ws.dual_partial;

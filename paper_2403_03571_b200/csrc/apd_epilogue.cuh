@@ -1,0 +1,56 @@
+// apd_epilogue.cuh -- rows a5 + a6 for one thread's row of V voxels, shared by the assign kernels.
+#pragma once
+#include "apd_internal.cuh"
+
+namespace apd {
+
+// Shared epilogue of every assign kernel (a5 + a6) for one thread's row of V voxels:
+// label store, run-length aggregated integer histogram updates, fp64 sum of the min-costs.
+template <int V>
+__device__ __forceinline__ double row_epilogue(const AssignArgs& a, bool row_valid, int ix0, int iy, int iz,
+                                               const float (&best)[V], const int (&lab)[V]) {
+  double dsum = 0.0;
+  if (!row_valid) return dsum;
+  const int nvalid = min(V, a.g.nx - ix0);
+  const long long j0 = ((long long)iz * a.g.ny + iy) * a.g.nx + ix0;
+  if (a.labels) {
+    if (nvalid == V && (a.g.nx & 3) == 0) {
+      int4* p = reinterpret_cast<int4*>(a.labels + j0);      // j0 % 4 == 0 because nx % 4 == 0, ix0 % V == 0
+#pragma unroll
+      for (int k = 0; k < V / 4; ++k) p[k] = make_int4(lab[4 * k], lab[4 * k + 1], lab[4 * k + 2], lab[4 * k + 3]);
+    } else {
+#pragma unroll
+      for (int k = 0; k < V; ++k) if (k < nvalid) a.labels[j0 + k] = lab[k];
+    }
+  }
+  // run-length aggregation: consecutive voxels of a row mostly share their label
+  int run_lab = lab[0];
+  unsigned int run_cnt = 0;
+  unsigned long long run_sx = 0;
+#pragma unroll
+  for (int k = 0; k < V; ++k) {
+    if (k < nvalid) {
+      dsum += (double)best[k];
+      if (lab[k] != run_lab) {
+        atomicAdd(a.count + run_lab, run_cnt);
+        if (a.idxsum) {
+          atomicAdd(a.idxsum + (size_t)run_lab * 3 + 0, run_sx);
+          atomicAdd(a.idxsum + (size_t)run_lab * 3 + 1, (unsigned long long)run_cnt * iy);
+          atomicAdd(a.idxsum + (size_t)run_lab * 3 + 2, (unsigned long long)run_cnt * iz);
+        }
+        run_lab = lab[k]; run_cnt = 0; run_sx = 0;
+      }
+      run_cnt += 1;
+      run_sx += (unsigned long long)(ix0 + k);
+    }
+  }
+  atomicAdd(a.count + run_lab, run_cnt);
+  if (a.idxsum) {
+    atomicAdd(a.idxsum + (size_t)run_lab * 3 + 0, run_sx);
+    atomicAdd(a.idxsum + (size_t)run_lab * 3 + 1, (unsigned long long)run_cnt * iy);
+    atomicAdd(a.idxsum + (size_t)run_lab * 3 + 2, (unsigned long long)run_cnt * iz);
+  }
+  return dsum;
+}
+
+}  // namespace apd

@@ -69,6 +69,12 @@ cudaError_t launch_pack_seeds(int dim, int M, int M_pad, const float* X, const f
                               float* seeds, unsigned int* count, unsigned long long* idxsum,
                               const int* done_flag, cudaStream_t st);
 cudaError_t launch_assign(int kernel, const AssignArgs& a, cudaStream_t st);
+// ROWPOLY kernel (apd_rowpoly.cu): its own pair-interleaved seed table
+cudaError_t launch_pack_pairs(int dim, int M, int M_pad, const float* X, const float* A, const float* w,
+                              float* seeds, unsigned int* count, unsigned long long* idxsum,
+                              const int* done_flag, cudaStream_t st);
+cudaError_t launch_assign_rowpoly(const AssignArgs& a, cudaStream_t st);
+void rowpoly_tile_counts(int dim, int nx, int ny, int nz, int* tx, int* ty, int* tz);
 void assign_tile_counts(int kernel, int dim, int nx, int ny, int nz, int* tx, int* ty, int* tz);
 cudaError_t launch_finalize(const GridDev& g, int M, int n_partials, const unsigned int* count,
                             const unsigned long long* idxsum, const double* dual_partial,

@@ -7,6 +7,7 @@
 // centroids.
 #include "apd_internal.cuh"
 #include "apd_device.cuh"
+#include "apd_epilogue.cuh"
 #include <math_constants.h>
 
 namespace apd {
@@ -71,55 +72,6 @@ cudaError_t launch_pack_seeds(int dim, int M, int M_pad, const float* X, const f
 template <int DIM> struct DirectGeom;
 template <> struct DirectGeom<3> { static constexpr int V = 8, TXT = 4, TYT = 8, TZT = 8; };
 template <> struct DirectGeom<2> { static constexpr int V = 8, TXT = 8, TYT = 32, TZT = 1; };
-
-// Shared epilogue of every assign kernel (a5 + a6) for one thread's row of V voxels:
-// label store, run-length aggregated integer histogram updates, fp64 sum of the min-costs.
-template <int V>
-__device__ __forceinline__ double row_epilogue(const AssignArgs& a, bool row_valid, int ix0, int iy, int iz,
-                                               const float (&best)[V], const int (&lab)[V]) {
-  double dsum = 0.0;
-  if (!row_valid) return dsum;
-  const int nvalid = min(V, a.g.nx - ix0);
-  const long long j0 = ((long long)iz * a.g.ny + iy) * a.g.nx + ix0;
-  if (a.labels) {
-    if (nvalid == V && (a.g.nx & 3) == 0) {
-      int4* p = reinterpret_cast<int4*>(a.labels + j0);      // j0 % 4 == 0 because nx % 4 == 0, ix0 % V == 0
-#pragma unroll
-      for (int k = 0; k < V / 4; ++k) p[k] = make_int4(lab[4 * k], lab[4 * k + 1], lab[4 * k + 2], lab[4 * k + 3]);
-    } else {
-#pragma unroll
-      for (int k = 0; k < V; ++k) if (k < nvalid) a.labels[j0 + k] = lab[k];
-    }
-  }
-  // run-length aggregation: consecutive voxels of a row mostly share their label
-  int run_lab = lab[0];
-  unsigned int run_cnt = 0;
-  unsigned long long run_sx = 0;
-#pragma unroll
-  for (int k = 0; k < V; ++k) {
-    if (k < nvalid) {
-      dsum += (double)best[k];
-      if (lab[k] != run_lab) {
-        atomicAdd(a.count + run_lab, run_cnt);
-        if (a.idxsum) {
-          atomicAdd(a.idxsum + (size_t)run_lab * 3 + 0, run_sx);
-          atomicAdd(a.idxsum + (size_t)run_lab * 3 + 1, (unsigned long long)run_cnt * iy);
-          atomicAdd(a.idxsum + (size_t)run_lab * 3 + 2, (unsigned long long)run_cnt * iz);
-        }
-        run_lab = lab[k]; run_cnt = 0; run_sx = 0;
-      }
-      run_cnt += 1;
-      run_sx += (unsigned long long)(ix0 + k);
-    }
-  }
-  atomicAdd(a.count + run_lab, run_cnt);
-  if (a.idxsum) {
-    atomicAdd(a.idxsum + (size_t)run_lab * 3 + 0, run_sx);
-    atomicAdd(a.idxsum + (size_t)run_lab * 3 + 1, (unsigned long long)run_cnt * iy);
-    atomicAdd(a.idxsum + (size_t)run_lab * 3 + 2, (unsigned long long)run_cnt * iz);
-  }
-  return dsum;
-}
 
 // fp32 voxel centre: the fp64 definition lo + (i + 1/2) s rounded once to fp32.
 __device__ __forceinline__ float centre_f32(double lo, double s, int i) {
@@ -221,7 +173,7 @@ __global__ void __launch_bounds__(256) assign_direct_kernel(const AssignArgs a) 
 static inline int cdiv(int a, int b) { return (a + b - 1) / b; }
 
 void assign_tile_counts(int kernel, int dim, int nx, int ny, int nz, int* tx, int* ty, int* tz) {
-  (void)kernel;
+  if (kernel == APD_KERNEL_ROWPOLY) { rowpoly_tile_counts(dim, nx, ny, nz, tx, ty, tz); return; }
   if (dim == 3) {
     using G = DirectGeom<3>;
     *tx = cdiv(nx, G::TXT * G::V); *ty = cdiv(ny, G::TYT); *tz = cdiv(nz, G::TZT);
@@ -232,7 +184,7 @@ void assign_tile_counts(int kernel, int dim, int nx, int ny, int nz, int* tx, in
 }
 
 cudaError_t launch_assign(int kernel, const AssignArgs& a, cudaStream_t st) {
-  (void)kernel;
+  if (kernel == APD_KERNEL_ROWPOLY) return launch_assign_rowpoly(a, st);
   const int n_tiles = a.g.tiles_x * a.g.tiles_y * a.g.tiles_z;
   if (a.g.dim == 3) assign_direct_kernel<3><<<n_tiles, 256, 0, st>>>(a);
   else              assign_direct_kernel<2><<<n_tiles, 256, 0, st>>>(a);

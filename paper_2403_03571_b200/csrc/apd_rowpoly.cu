@@ -1,0 +1,238 @@
+// apd_rowpoly.cu -- the ROWPOLY voxel x seed kernel (rows a1-a6 of DESIGN.md's path table).
+//
+// Same definition as the DIRECT kernel -- C_ij = |y_j - x_i|^2_{A_i} - w_i (eq. 2.1),
+// H_j = argmin_i C_ij with the lowest index among equal fp32 costs (reading S1) --
+// re-associated for the machine:
+//   * a thread owns a ROW of V voxels contiguous in x.  With d0 = x_row0 - x_i and tau_k = k s_x the
+//     cost along the row is the quadratic  c(tau) = a11 tau^2 + B' tau + R',
+//        B' = 2 a11 d0 + (a12' dy + a13' dz),   R' = cost at the row's first voxel,
+//     so a pair costs 2 FMA (Horner) after a per-(row, seed) set-up of 14 operations;
+//   * all arithmetic is packed f32x2 (FFMA2) over PAIRS OF SEEDS (the seed table is stored
+//     pair-interleaved), one 3-input min folds both lanes into the running minimum;
+//   * the inner loop keeps only the minimum.  After every GROUP seeds the minima are compared with
+//     their values before the group; a voxel whose minimum dropped has its argmin inside that
+//     group, and the (rare) rescan recomputes the group with the same instructions and takes the
+//     first seed whose cost equals the new minimum.
+#include "apd_internal.cuh"
+#include "apd_device.cuh"
+#include "apd_epilogue.cuh"
+#include <math_constants.h>
+
+namespace apd {
+
+// pair-interleaved seed table: PREC floats per PAIR of seeds
+//   3D (20): X0 X1 Y0 Y1 | Z0 Z1 a11 a11 | a12' a12' a13' a13' | a22 a22 a23' a23' | a33 a33 nw nw
+//   2D (12): X0 X1 Y0 Y1 | a11 a11 a12' a12' | a22 a22 nw nw
+constexpr int PREC3 = 20;
+constexpr int PREC2 = 12;
+
+template <int DIM>
+__global__ void pack_pairs_kernel(int M, int M_pad, const float* __restrict__ X, const float* __restrict__ A,
+                                  const float* __restrict__ w, float* __restrict__ seeds,
+                                  unsigned int* __restrict__ count, unsigned long long* __restrict__ idxsum,
+                                  const int* __restrict__ done_flag) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= M_pad) return;
+  if (done_flag && *done_flag) return;
+  constexpr int NP = (DIM == 3) ? 10 : 6;
+  constexpr int PREC = (DIM == 3) ? PREC3 : PREC2;
+  float r[NP];
+#pragma unroll
+  for (int k = 0; k < NP; ++k) r[k] = 0.0f;
+  if (i < M) {
+    if (DIM == 3) {
+      const float* a = A + (size_t)i * 9;
+      r[0] = X[i * 3 + 0]; r[1] = X[i * 3 + 1]; r[2] = X[i * 3 + 2];
+      r[3] = a[0]; r[4] = a[1] + a[3]; r[5] = a[2] + a[6]; r[6] = a[4]; r[7] = a[5] + a[7]; r[8] = a[8];
+      r[9] = -w[i];
+    } else {
+      const float* a = A + (size_t)i * 4;
+      r[0] = X[i * 2 + 0]; r[1] = X[i * 2 + 1];
+      r[2] = a[0]; r[3] = a[1] + a[2]; r[4] = a[3];
+      r[5] = -w[i];
+    }
+    count[i] = 0u;
+    if (idxsum) { idxsum[i * 3 + 0] = 0ull; idxsum[i * 3 + 1] = 0ull; idxsum[i * 3 + 2] = 0ull; }
+  } else {
+    r[NP - 1] = CUDART_INF_F;   // padding seed: cost +inf
+  }
+  float* dst = seeds + (size_t)(i >> 1) * PREC + (i & 1);
+#pragma unroll
+  for (int k = 0; k < NP; ++k) dst[2 * k] = r[k];
+}
+
+cudaError_t launch_pack_pairs(int dim, int M, int M_pad, const float* X, const float* A, const float* w,
+                              float* seeds, unsigned int* count, unsigned long long* idxsum,
+                              const int* done_flag, cudaStream_t st) {
+  const int nb = (M_pad + 127) / 128;
+  if (dim == 3) pack_pairs_kernel<3><<<nb, 128, 0, st>>>(M, M_pad, X, A, w, seeds, count, idxsum, done_flag);
+  else          pack_pairs_kernel<2><<<nb, 128, 0, st>>>(M, M_pad, X, A, w, seeds, count, idxsum, done_flag);
+  return cudaGetLastError();
+}
+
+// Per-(row, seed pair) coefficients of the row quadratic.
+struct RowCoef { f2 a11, Bp, Rp; };
+
+template <int DIM>
+__device__ __forceinline__ RowCoef row_setup(const float* __restrict__ sp /* one pair record in smem */,
+                                             f2 x0, f2 yy, f2 yz) {
+  RowCoef o;
+  if (DIM == 3) {
+    const ulonglong2 q0 = *reinterpret_cast<const ulonglong2*>(sp);        // X, Y
+    const ulonglong2 q1 = *reinterpret_cast<const ulonglong2*>(sp + 4);    // Z, a11
+    const ulonglong2 q2 = *reinterpret_cast<const ulonglong2*>(sp + 8);    // a12', a13'
+    const ulonglong2 q3 = *reinterpret_cast<const ulonglong2*>(sp + 12);   // a22, a23'
+    const ulonglong2 q4 = *reinterpret_cast<const ulonglong2*>(sp + 16);   // a33, nw
+    const f2 d0 = f2_sub(x0, q0.x), dy = f2_sub(yy, q0.y), dz = f2_sub(yz, q1.x);
+    const f2 a11 = q1.y;
+    const f2 E = f2_fma(q2.x, dy, f2_mul(q2.y, dz));                       // a12' dy + a13' dz
+    const f2 u = f2_fma(q3.y, dz, f2_mul(q3.x, dy));                       // a22 dy + a23' dz
+    f2 R = f2_fma(dy, u, q4.y);                                            // ... - w
+    R = f2_fma(dz, f2_mul(q4.x, dz), R);                                   // + a33 dz^2
+    o.a11 = a11;
+    o.Bp = f2_fma(f2_add(a11, a11), d0, E);                                // 2 a11 d0 + E
+    o.Rp = f2_fma(d0, f2_fma(a11, d0, E), R);                              // cost at the row's first voxel
+  } else {
+    const ulonglong2 q0 = *reinterpret_cast<const ulonglong2*>(sp);        // X, Y
+    const ulonglong2 q1 = *reinterpret_cast<const ulonglong2*>(sp + 4);    // a11, a12'
+    const ulonglong2 q2 = *reinterpret_cast<const ulonglong2*>(sp + 8);    // a22, nw
+    const f2 d0 = f2_sub(x0, q0.x), dy = f2_sub(yy, q0.y);
+    const f2 a11 = q1.x;
+    const f2 E = f2_mul(q1.y, dy);                                         // a12' dy
+    const f2 R = f2_fma(dy, f2_mul(q2.x, dy), q2.y);                       // a22 dy^2 - w
+    o.a11 = a11;
+    o.Bp = f2_fma(f2_add(a11, a11), d0, E);
+    o.Rp = f2_fma(d0, f2_fma(a11, d0, E), R);
+  }
+  return o;
+}
+
+__device__ __forceinline__ f2 row_cost(const RowCoef& c, f2 tt) {
+  return f2_fma(tt, f2_fma(c.a11, tt, c.Bp), c.Rp);
+}
+
+template <int DIM, int V_, int TXT_, int TYT_, int TZT_>
+struct RowGeom {
+  static constexpr int V = V_, TXT = TXT_, TYT = TYT_, TZT = TZT_, THREADS = TXT_ * TYT_ * TZT_;
+};
+using RowGeom3 = RowGeom<3, 16, 1, 16, 8>;    // tile 16 x 16 x 8 voxels, 128 threads
+using RowGeom2 = RowGeom<2, 16, 4, 32, 1>;    // tile 64 x 32 pixels, 128 threads
+
+constexpr int ROW_GROUP = 16;                 // seeds between two argmin checks
+
+template <int DIM, class G>
+__global__ void __launch_bounds__(G::THREADS) assign_rowpoly_kernel(const AssignArgs a) {
+  constexpr int V = G::V;
+  constexpr int PREC = (DIM == 3) ? PREC3 : PREC2;
+  constexpr int CHUNK_PAIRS = SEED_CHUNK / 2;
+  constexpr uint32_t CHUNK_BYTES = CHUNK_PAIRS * PREC * sizeof(float);
+  constexpr int GROUP_PAIRS = ROW_GROUP / 2;
+  __shared__ __align__(128) float s_seeds[SEED_STAGES][CHUNK_PAIRS * PREC];
+  __shared__ __align__(8) uint64_t s_full[SEED_STAGES];
+  __shared__ double s_red[G::THREADS / 32];
+
+  if (a.done_flag && *a.done_flag) return;
+  const int tid = threadIdx.x;
+  const int tx = tid % G::TXT, ty = (tid / G::TXT) % G::TYT, tz = tid / (G::TXT * G::TYT);
+  const int b = blockIdx.x;
+  const int bx = b % a.g.tiles_x, by = (b / a.g.tiles_x) % a.g.tiles_y, bz = b / (a.g.tiles_x * a.g.tiles_y);
+  const int ix0 = (bx * G::TXT + tx) * V, iy = by * G::TYT + ty, iz = bz * G::TZT + tz;
+  const bool row_valid = (ix0 < a.g.nx) && (iy < a.g.ny) && (iz < a.g.nz);
+
+  const int nchunks = a.M_pad / SEED_CHUNK;
+  if (tid == 0) {
+    for (int s = 0; s < SEED_STAGES; ++s) mbar_init(&s_full[s], 1);
+    mbar_fence_init();
+    for (int s = 0; s < SEED_STAGES && s < nchunks; ++s) {
+      mbar_arrive_expect_tx(&s_full[s], CHUNK_BYTES);
+      tma_bulk_g2s(s_seeds[s], a.seeds + (size_t)s * CHUNK_PAIRS * PREC, CHUNK_BYTES, &s_full[s]);
+    }
+  }
+  __syncthreads();
+
+  // a1: coordinates from the thread index (fp64 definition rounded once to fp32)
+  const float x0f = (float)(a.g.lo[0] + ((double)ix0 + 0.5) * a.g.s[0]);
+  const float yyf = (float)(a.g.lo[1] + ((double)iy + 0.5) * a.g.s[1]);
+  const float yzf = (DIM == 3) ? (float)(a.g.lo[2] + ((double)iz + 0.5) * a.g.s[2]) : 0.0f;
+  const f2 x0 = f2_pack(x0f, x0f), yy = f2_pack(yyf, yyf), yz = f2_pack(yzf, yzf);
+  f2 tt[V];
+#pragma unroll
+  for (int k = 0; k < V; ++k) {
+    // in-row offset of voxel k from the row's first voxel, taken between the two fp32 centres
+    const float t = (float)((a.g.lo[0] + ((double)(ix0 + k) + 0.5) * a.g.s[0]) - (double)x0f);
+    tt[k] = f2_pack(t, t);
+  }
+
+  float best[V];
+  int lab[V];
+#pragma unroll
+  for (int k = 0; k < V; ++k) { best[k] = CUDART_INF_F; lab[k] = 0; }
+
+  for (int c = 0; c < nchunks; ++c) {
+    const int stage = c % SEED_STAGES;
+    mbar_wait(&s_full[stage], (uint32_t)((c / SEED_STAGES) & 1));
+    const float* sp = s_seeds[stage];
+    for (int gidx = 0; gidx < CHUNK_PAIRS / GROUP_PAIRS; ++gidx) {
+      const float* gp = sp + gidx * GROUP_PAIRS * PREC;
+      float prev[V];
+#pragma unroll
+      for (int k = 0; k < V; ++k) prev[k] = best[k];
+#pragma unroll 2
+      for (int p = 0; p < GROUP_PAIRS; ++p) {
+        const RowCoef rc = row_setup<DIM>(gp + p * PREC, x0, yy, yz);
+#pragma unroll
+        for (int k = 0; k < V; ++k) {
+          float lo, hi;
+          f2_unpack(row_cost(rc, tt[k]), lo, hi);
+          best[k] = min3f(best[k], lo, hi);
+        }
+      }
+      unsigned int mask = 0u;
+#pragma unroll
+      for (int k = 0; k < V; ++k) mask |= (best[k] < prev[k]) ? (1u << k) : 0u;
+      if (mask) {
+        // a4, deferred: the new minimum of every flagged voxel lies in this group; recompute the
+        // group with the same instructions and take the first seed that attains it
+        const int ibase = c * SEED_CHUNK + gidx * ROW_GROUP;
+        for (int p = 0; p < GROUP_PAIRS && mask; ++p) {
+          const RowCoef rc = row_setup<DIM>(gp + p * PREC, x0, yy, yz);
+#pragma unroll
+          for (int k = 0; k < V; ++k) {
+            if (mask & (1u << k)) {
+              float lo, hi;
+              f2_unpack(row_cost(rc, tt[k]), lo, hi);
+              if (lo == best[k]) { lab[k] = ibase + 2 * p; mask &= ~(1u << k); }
+              else if (hi == best[k]) { lab[k] = ibase + 2 * p + 1; mask &= ~(1u << k); }
+            }
+          }
+        }
+      }
+    }
+    __syncthreads();
+    if (tid == 0 && c + SEED_STAGES < nchunks) {
+      mbar_arrive_expect_tx(&s_full[stage], CHUNK_BYTES);
+      tma_bulk_g2s(s_seeds[stage], a.seeds + (size_t)(c + SEED_STAGES) * CHUNK_PAIRS * PREC, CHUNK_BYTES,
+                   &s_full[stage]);
+    }
+  }
+
+  const double dsum = row_epilogue<V>(a, row_valid, ix0, iy, iz, best, lab);
+  const double tot = block_sum_double<G::THREADS>(dsum, s_red);
+  if (tid == 0) a.dual_partial[b] = tot;
+}
+
+static inline int cdiv_i(int x, int y) { return (x + y - 1) / y; }
+
+void rowpoly_tile_counts(int dim, int nx, int ny, int nz, int* tx, int* ty, int* tz) {
+  if (dim == 3) { *tx = cdiv_i(nx, RowGeom3::TXT * RowGeom3::V); *ty = cdiv_i(ny, RowGeom3::TYT); *tz = cdiv_i(nz, RowGeom3::TZT); }
+  else          { *tx = cdiv_i(nx, RowGeom2::TXT * RowGeom2::V); *ty = cdiv_i(ny, RowGeom2::TYT); *tz = 1; }
+}
+
+cudaError_t launch_assign_rowpoly(const AssignArgs& a, cudaStream_t st) {
+  const int n_tiles = a.g.tiles_x * a.g.tiles_y * a.g.tiles_z;
+  if (a.g.dim == 3) assign_rowpoly_kernel<3, RowGeom3><<<n_tiles, RowGeom3::THREADS, 0, st>>>(a);
+  else              assign_rowpoly_kernel<2, RowGeom2><<<n_tiles, RowGeom2::THREADS, 0, st>>>(a);
+  return cudaGetLastError();
+}
+
+}  // namespace apd

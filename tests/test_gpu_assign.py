@@ -5,7 +5,7 @@ import pytest
 import torch
 
 from paper_2403_03571_b200 import workloads
-from tests import parity
+import apd_parity as parity
 
 pytestmark = pytest.mark.gpu
 
@@ -179,8 +179,9 @@ def test_argument_errors(apd):
     with pytest.raises(apd.ApdError):
         ctx.apd_assign(bad, X, A, w, vol=vol, dual=dual)
     g3 = apd.make_grid(3, (8, 8, 8), (0, 0, 0), (1, 1, 1))
-    with pytest.raises(apd.ApdError):
-        ctx.apd_assign(g3, X, A, w, vol=vol, dual=dual)           # dim differs from the context's
+    wl3 = workloads.make_random(3, (8, 8, 8), 4, 1)
+    with pytest.raises(apd.ApdError):                             # dim differs from the context's
+        ctx.apd_assign(g3, torch.from_numpy(wl3.X).to(dev), torch.from_numpy(wl3.A).to(dev), w, vol=vol, dual=dual)
     ok = apd.make_grid(2, (8, 8), (0, 0), (1, 1))
     with pytest.raises(apd.ApdError):
         ctx.apd_assign(ok, X, A, w, vol=vol, dual=dual, opts=apd.make_opts(kernel=99))
