@@ -1,0 +1,142 @@
+"""GPU parity of apd_solve (Algorithm 2) against oracle_solve, which follows the
+same specification S9 step by step.  Parity rule 5: at equal tolerance, equal options
+AND equal iters/evals the centred weights agree to 1e-4 relative; independently of the
+trajectory, the oracle's own evaluation at the GPU's weights must meet the tolerance (P15)."""
+import numpy as np
+import pytest
+import torch
+
+from paper_2403_03571_b200 import workloads
+import apd_parity as parity
+from oracle.apd_oracle import oracle_assign, oracle_solve, OK, NOT_CONVERGED
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def apd():
+    from paper_2403_03571_b200 import binding
+    binding.load_library()
+    return binding
+
+
+def run_solve(apd, wl, eps, w_init=None, kernel=0, history=10, max_iters=1000, max_evals=0):
+    dev = torch.device("cuda:0")
+    ctx = apd.ApdContext(wl.dim, wl.M)
+    grid = apd.make_grid(wl.dim, wl.n, wl.lo, wl.hi)
+    X = torch.from_numpy(wl.X).to(dev); A = torch.from_numpy(wl.A).to(dev); v = torch.from_numpy(wl.v).to(dev)
+    wi = torch.from_numpy(np.ascontiguousarray(w_init, dtype=np.float32)).to(dev) if w_init is not None else None
+    w = torch.zeros(wl.M, dtype=torch.float32, device=dev)
+    w64 = torch.zeros(wl.M, dtype=torch.float64, device=dev)
+    labels = torch.full((wl.N,), -1, dtype=torch.int32, device=dev)
+    vol = torch.zeros(wl.M, dtype=torch.float64, device=dev)
+    info = ctx.apd_solve(grid, X, A, v, eps, w_init=wi, w=w, labels=labels, vol=vol, w64=w64,
+                         opts=apd.make_opts(kernel=kernel, lbfgs_history=history, max_iters=max_iters,
+                                            max_evals=max_evals))
+    return info, w.cpu().numpy(), w64.cpu().numpy(), labels.cpu().numpy(), vol.cpu().numpy()
+
+
+def check_against_oracle(wl, eps, info, w32, w64, labels, vol, orc, require_same_path=True):
+    grid = parity.grid_of(wl)
+    # P15 / post-condition, judged by the ORACLE at the GPU's weights
+    chk = oracle_assign(grid, wl.X, wl.A, w32, v=wl.v)
+    P = grid.voxel_volume
+    assert np.array_equal(np.rint(vol / P).astype(np.int64), np.bincount(labels, minlength=wl.M))
+    nm = parity.check_labels(grid, wl.X, wl.A, w32, labels, chk)["mismatches"]
+    np.testing.assert_array_equal(w32, w64.astype(np.float32))        # w is exactly fl32 of the fp64 iterate
+    if info.status == 0:
+        assert chk.err <= eps + 2 * nm * P / float(wl.v.min()), f"oracle err {chk.err} > eps"
+        assert info.max_rel_err <= eps
+    same = (info.iters == orc.iters and info.evals == orc.evals and info.status == orc.status)
+    if require_same_path:
+        assert same, f"trajectory differs: gpu iters/evals/status {info.iters}/{info.evals}/{info.status} vs " \
+                     f"oracle {orc.iters}/{orc.evals}/{orc.status}"
+    if same:
+        a = w64 - w64.mean(); b = orc.w - orc.w.mean()
+        scale = max(np.abs(b).max(), 1e-300)
+        assert np.abs(a - b).max() <= 1e-4 * scale, f"weights differ by {np.abs(a - b).max() / scale:.3e} relative"
+        assert abs(info.dual - orc.dual) <= 1e-6 * max(abs(orc.dual), 1e-300) + 1e-12
+    return same
+
+
+def test_cfg1_full(apd):
+    wl = workloads.make_config(1)
+    orc = oracle_solve(parity.grid_of(wl), wl.X, wl.A, wl.v, wl.eps)
+    info, w32, w64, labels, vol = run_solve(apd, wl, wl.eps)
+    assert orc.status == OK and info.status == 0
+    check_against_oracle(wl, wl.eps, info, w32, w64, labels, vol, orc)
+    print(f"cfg1: iters {info.iters} evals {info.evals} err {info.max_rel_err:.4g}")
+
+
+@pytest.mark.parametrize("kernel", [1, 2])
+@pytest.mark.parametrize("cfg,n,M,eps", [(2, (256, 256), 60, 0.01), (3, (64, 64, 64), 80, 0.01),
+                                         (4, (96, 96, 96), 150, 0.02), (5, (80, 80, 80), 120, 0.02)])
+def test_reduced_configs_same_trajectory(apd, cfg, n, M, eps, kernel):
+    wl = workloads.make_config(cfg, n=n, M=M)
+    orc = oracle_solve(parity.grid_of(wl), wl.X, wl.A, wl.v, eps)
+    info, w32, w64, labels, vol = run_solve(apd, wl, eps, kernel=kernel)
+    same = check_against_oracle(wl, eps, info, w32, w64, labels, vol, orc, require_same_path=False)
+    print(f"cfg{cfg} reduced: gpu {info.iters}/{info.evals}/{info.status} err {info.max_rel_err:.4g}; "
+          f"oracle {orc.iters}/{orc.evals}/{orc.status} err {orc.err:.4g}; same path: {same}")
+    assert same, "GPU and oracle left the common L-BFGS trajectory"
+
+
+def test_P13_trivial_optimum(apd):
+    """Seeds on a regular lattice, A = I, equal targets: W = 0 is optimal, iters = 0 (PAPER.md:150 W0 = 0)."""
+    k, n = 4, 32
+    g = (np.arange(k) + 0.5) / k
+    X = np.stack(np.meshgrid(g, g, g, indexing="ij"), -1).reshape(-1, 3).astype(np.float32)
+    M = X.shape[0]
+    A = np.tile(np.eye(3, dtype=np.float32), (M, 1, 1))
+    wl = workloads.Workload("lattice", 3, (n, n, n), (0.0,) * 3, (1.0,) * 3, X, A,
+                            np.full(M, 1.0 / M, np.float32), np.zeros(M, np.float32))
+    info, w32, w64, labels, vol = run_solve(apd, wl, 0.01)
+    assert info.status == 0 and info.iters == 0 and info.evals == 1
+    assert np.all(w32 == 0) and np.allclose(vol, 1.0 / M, rtol=0, atol=1e-15)
+
+
+def test_P14_closed_form_weights(apd):
+    """2D, seeds (1/4,1/2),(3/4,1/2), A = I, targets (0.3,0.7): boundary x = 1/2 - (w2-w1) => w2 - w1 = 0.2."""
+    n = 200
+    X = np.array([[0.25, 0.5], [0.75, 0.5]], np.float32)
+    A = np.tile(np.eye(2, dtype=np.float32), (2, 1, 1))
+    wl = workloads.Workload("two", 2, (n, n), (0.0, 0.0), (1.0, 1.0), X, A, np.array([0.3, 0.7], np.float32),
+                            np.zeros(2, np.float32))
+    info, w32, w64, labels, vol = run_solve(apd, wl, 0.01)
+    assert info.status == 0
+    # |vol_1 - 0.3| <= 0.003 => boundary within 0.003 (+ one pixel) of x = 0.3
+    assert abs((w64[1] - w64[0]) - 0.2) <= 0.003 + 1.0 / n
+    assert abs(w64.sum()) < 1e-12                                     # gauge: sum w stays 0 (identity I3)
+
+
+def test_warm_start_and_not_converged(apd):
+    wl = workloads.make_config(3, n=(48, 48, 48), M=60)
+    orc = oracle_solve(parity.grid_of(wl), wl.X, wl.A, wl.v, 0.01, max_iters=3)
+    info, w32, w64, labels, vol = run_solve(apd, wl, 0.01, max_iters=3)
+    assert orc.status == NOT_CONVERGED and info.status == 1
+    check_against_oracle(wl, 0.01, info, w32, w64, labels, vol, orc)
+    # warm start from the returned fp32 weights (Alg. 3 warm start W0^{k+1} = W^k)
+    orc2 = oracle_solve(parity.grid_of(wl), wl.X, wl.A, wl.v, 0.01, w_init=w32)
+    info2, w32b, w64b, labels2, vol2 = run_solve(apd, wl, 0.01, w_init=w32)
+    assert info2.status == 0 and orc2.status == OK
+    check_against_oracle(wl, 0.01, info2, w32b, w64b, labels2, vol2, orc2)
+
+
+def test_bad_target_volumes(apd):
+    wl = workloads.make_config(1)
+    wl.v[:] = wl.v * 1.01
+    with pytest.raises(apd.ApdError) as e:
+        run_solve(apd, wl, 0.01)
+    assert e.value.status == apd.APD_E_ARG
+
+
+def test_solve_host_matches_device(apd):
+    wl = workloads.make_config(2, n=(128, 128), M=40)
+    info, w32, w64, labels, vol = run_solve(apd, wl, 0.01)
+    ctx = apd.ApdContext(2, 40)
+    grid = apd.make_grid(wl.dim, wl.n, wl.lo, wl.hi)
+    w = torch.empty(40, dtype=torch.float32); lab = torch.empty(wl.N, dtype=torch.int32)
+    info2 = ctx.apd_solve_host(grid, torch.from_numpy(wl.X), torch.from_numpy(wl.A), torch.from_numpy(wl.v), 0.01,
+                               w=w, labels=lab)
+    assert (info2.status, info2.iters, info2.evals) == (info.status, info.iters, info.evals)
+    assert np.array_equal(w.numpy(), w32) and np.array_equal(lab.numpy(), labels)
