@@ -112,7 +112,8 @@ std::string make_grid(const apd_ctx* ctx, const apd_grid* grid, int kernel, Grid
   }
   out.nx = n[0]; out.ny = n[1]; out.nz = n[2];
   out.voxel_volume = P;
-  assign_tile_counts(kernel, d, out.nx, out.ny, out.nz, &out.tiles_x, &out.tiles_y, &out.tiles_z);
+  out.row_long = assign_tile_counts(kernel, d, out.nx, out.ny, out.nz, ctx->ws.sm_count, &out.tiles_x, &out.tiles_y,
+                                    &out.tiles_z);
   *g = out;
   return "";
 }

@@ -30,6 +30,7 @@ struct GridDev {
   double s[3];          // voxel side lengths
   double voxel_volume;  // |P|
   int tiles_x, tiles_y, tiles_z;
+  int row_long;         // ROWPOLY kernel: 1 = rows of 32 voxels per thread, 0 = rows of 16
 };
 
 struct AssignArgs {
@@ -74,8 +75,8 @@ cudaError_t launch_pack_pairs(int dim, int M, int M_pad, const float* X, const f
                               float* seeds, unsigned int* count, unsigned long long* idxsum,
                               const int* done_flag, cudaStream_t st);
 cudaError_t launch_assign_rowpoly(const AssignArgs& a, cudaStream_t st);
-void rowpoly_tile_counts(int dim, int nx, int ny, int nz, int* tx, int* ty, int* tz);
-void assign_tile_counts(int kernel, int dim, int nx, int ny, int nz, int* tx, int* ty, int* tz);
+int rowpoly_tile_counts(int dim, int nx, int ny, int nz, int sm_count, int* tx, int* ty, int* tz);
+int assign_tile_counts(int kernel, int dim, int nx, int ny, int nz, int sm_count, int* tx, int* ty, int* tz);
 cudaError_t launch_finalize(const GridDev& g, int M, int n_partials, const unsigned int* count,
                             const unsigned long long* idxsum, const double* dual_partial,
                             const float* X, const float* w, const float* target_vol,

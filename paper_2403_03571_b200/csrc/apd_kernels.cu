@@ -172,8 +172,9 @@ __global__ void __launch_bounds__(256) assign_direct_kernel(const AssignArgs a) 
 
 static inline int cdiv(int a, int b) { return (a + b - 1) / b; }
 
-void assign_tile_counts(int kernel, int dim, int nx, int ny, int nz, int* tx, int* ty, int* tz) {
-  if (kernel == APD_KERNEL_ROWPOLY) { rowpoly_tile_counts(dim, nx, ny, nz, tx, ty, tz); return; }
+// Returns the ROWPOLY row-length choice (0 for the DIRECT kernel).
+int assign_tile_counts(int kernel, int dim, int nx, int ny, int nz, int sm_count, int* tx, int* ty, int* tz) {
+  if (kernel == APD_KERNEL_ROWPOLY) return rowpoly_tile_counts(dim, nx, ny, nz, sm_count, tx, ty, tz);
   if (dim == 3) {
     using G = DirectGeom<3>;
     *tx = cdiv(nx, G::TXT * G::V); *ty = cdiv(ny, G::TYT); *tz = cdiv(nz, G::TZT);
@@ -181,6 +182,7 @@ void assign_tile_counts(int kernel, int dim, int nx, int ny, int nz, int* tx, in
     using G = DirectGeom<2>;
     *tx = cdiv(nx, G::TXT * G::V); *ty = cdiv(ny, G::TYT); *tz = 1;
   }
+  return 0;
 }
 
 cudaError_t launch_assign(int kernel, const AssignArgs& a, cudaStream_t st) {

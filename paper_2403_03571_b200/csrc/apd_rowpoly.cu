@@ -111,25 +111,75 @@ __device__ __forceinline__ f2 row_cost(const RowCoef& c, f2 tt) {
   return f2_fma(tt, f2_fma(c.a11, tt, c.Bp), c.Rp);
 }
 
-template <int DIM, int V_, int TXT_, int TYT_, int TZT_>
+// Tile geometry: THREADS = TXT*TYT*TZT threads, each owns a row of V voxels contiguous in x, so the tile is
+// (TXT*V) x TYT x TZT voxels.  MINB = CTAs per SM the register allocation is held to.
+template <int DIM, int V_, int TXT_, int TYT_, int TZT_, int MINB_>
 struct RowGeom {
-  static constexpr int V = V_, TXT = TXT_, TYT = TYT_, TZT = TZT_, THREADS = TXT_ * TYT_ * TZT_;
+  static constexpr int V = V_, TXT = TXT_, TYT = TYT_, TZT = TZT_, THREADS = TXT_ * TYT_ * TZT_, MINB = MINB_;
 };
-using RowGeom3 = RowGeom<3, 16, 1, 16, 8>;    // tile 16 x 16 x 8 voxels, 128 threads
-using RowGeom2 = RowGeom<2, 16, 4, 32, 1>;    // tile 64 x 32 pixels, 128 threads
+#ifndef ROWMINB
+#define ROWMINB 4
+#endif
+#ifndef ROWBATCH
+#define ROWBATCH 8
+#endif
+#ifndef ROWUNROLL
+#define ROWUNROLL 1
+#endif
+// Two row lengths are built.  LONG rows (V = 32) amortise the per-(row, seed) set-up best and are used once the
+// grid gives every SM at least ROW_LONG_MIN_WAVES waves of long-row tiles; smaller grids take SHORT rows (V = 16),
+// whose tiles are half as big, so that all SMs have work.
+using RowGeom3L = RowGeom<3, 32, 1, 16, 8, ROWMINB>;    // tile 32 x 16 x 8 voxels, 128 threads
+using RowGeom3S = RowGeom<3, 16, 1, 16, 8, ROWMINB>;    // tile 16 x 16 x 8 voxels
+using RowGeom2L = RowGeom<2, 32, 2, 64, 1, ROWMINB>;    // tile 64 x 64 pixels
+using RowGeom2S = RowGeom<2, 16, 2, 64, 1, ROWMINB>;    // tile 32 x 64 pixels
+constexpr int ROW_LONG_MIN_WAVES = 2;
 
-constexpr int ROW_GROUP = 16;                 // seeds between two argmin checks
+#ifndef ROWGROUP
+#define ROWGROUP 16
+#endif
+constexpr int ROW_GROUP = ROWGROUP;                 // seeds between two argmin checks
+#ifndef ROWSTAGES
+#define ROWSTAGES 4
+#endif
+constexpr int ROW_STAGES = ROWSTAGES;                 // smem ring of seed chunks
+constexpr int ROW_BATCH = ROWBATCH;
+constexpr int ROW_UNROLL = ROWUNROLL;
+
+// Dynamic shared memory of one CTA:
+//   seeds [ROW_STAGES][CHUNK_PAIRS*PREC] f32 | prev [V][THREADS] f32 | lab [V][THREADS] i32 |
+//   full[ROW_STAGES], empty[ROW_STAGES] mbarriers | red [THREADS/32] f64
+// prev[k][tid] = the minimum of voxel k as of its last label update (== best[k] except inside the group that
+// lowers it); prev and lab live in shared memory because they are touched once per ROW_GROUP seeds, which
+// leaves the registers to the V running minima and to the interleaved FMA chains.
+template <int DIM, class G>
+struct RowSmem {
+  static constexpr int PREC = (DIM == 3) ? PREC3 : PREC2;
+  static constexpr int CHUNK_PAIRS = SEED_CHUNK / 2;
+  static constexpr size_t SEED_BYTES = (size_t)ROW_STAGES * CHUNK_PAIRS * PREC * sizeof(float);
+  static constexpr size_t PREV_OFF = SEED_BYTES;
+  static constexpr size_t LAB_OFF = PREV_OFF + (size_t)G::V * G::THREADS * sizeof(float);
+  static constexpr size_t BAR_OFF = LAB_OFF + (size_t)G::V * G::THREADS * sizeof(int);
+  static constexpr size_t RED_OFF = BAR_OFF + 2 * ROW_STAGES * sizeof(uint64_t);
+  static constexpr size_t BYTES = RED_OFF + (G::THREADS / 32) * sizeof(double);
+};
 
 template <int DIM, class G>
-__global__ void __launch_bounds__(G::THREADS) assign_rowpoly_kernel(const AssignArgs a) {
-  constexpr int V = G::V;
-  constexpr int PREC = (DIM == 3) ? PREC3 : PREC2;
-  constexpr int CHUNK_PAIRS = SEED_CHUNK / 2;
+__global__ void __launch_bounds__(G::THREADS, G::MINB) assign_rowpoly_kernel(const AssignArgs a) {
+  constexpr int V = G::V, T = G::THREADS;
+  using S = RowSmem<DIM, G>;
+  constexpr int PREC = S::PREC;
+  constexpr int CHUNK_PAIRS = S::CHUNK_PAIRS;
   constexpr uint32_t CHUNK_BYTES = CHUNK_PAIRS * PREC * sizeof(float);
   constexpr int GROUP_PAIRS = ROW_GROUP / 2;
-  __shared__ __align__(128) float s_seeds[SEED_STAGES][CHUNK_PAIRS * PREC];
-  __shared__ __align__(8) uint64_t s_full[SEED_STAGES];
-  __shared__ double s_red[G::THREADS / 32];
+  static_assert(V <= 32 && V % ROW_BATCH == 0, "row mask is 32 bits");
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  float* s_seeds = reinterpret_cast<float*>(smem_raw);
+  float4* s_prev4 = reinterpret_cast<float4*>(smem_raw + S::PREV_OFF);   // [V/4][T]
+  int* s_lab = reinterpret_cast<int*>(smem_raw + S::LAB_OFF);
+  uint64_t* s_full = reinterpret_cast<uint64_t*>(smem_raw + S::BAR_OFF);
+  uint64_t* s_empty = s_full + ROW_STAGES;
+  double* s_red = reinterpret_cast<double*>(smem_raw + S::RED_OFF);
 
   if (a.done_flag && *a.done_flag) return;
   const int tid = threadIdx.x;
@@ -141,14 +191,14 @@ __global__ void __launch_bounds__(G::THREADS) assign_rowpoly_kernel(const Assign
 
   const int nchunks = a.M_pad / SEED_CHUNK;
   if (tid == 0) {
-    for (int s = 0; s < SEED_STAGES; ++s) mbar_init(&s_full[s], 1);
+    for (int s = 0; s < ROW_STAGES; ++s) { mbar_init(&s_full[s], 1); mbar_init(&s_empty[s], T / 32); }
     mbar_fence_init();
-    for (int s = 0; s < SEED_STAGES && s < nchunks; ++s) {
+    for (int s = 0; s < ROW_STAGES && s < nchunks; ++s) {
       mbar_arrive_expect_tx(&s_full[s], CHUNK_BYTES);
-      tma_bulk_g2s(s_seeds[s], a.seeds + (size_t)s * CHUNK_PAIRS * PREC, CHUNK_BYTES, &s_full[s]);
+      tma_bulk_g2s(s_seeds + (size_t)s * CHUNK_PAIRS * PREC, a.seeds + (size_t)s * CHUNK_PAIRS * PREC, CHUNK_BYTES,
+                   &s_full[s]);
     }
   }
-  __syncthreads();
 
   // a1: coordinates from the thread index (fp64 definition rounded once to fp32)
   const float x0f = (float)(a.g.lo[0] + ((double)ix0 + 0.5) * a.g.s[0]);
@@ -156,43 +206,73 @@ __global__ void __launch_bounds__(G::THREADS) assign_rowpoly_kernel(const Assign
   const float yzf = (DIM == 3) ? (float)(a.g.lo[2] + ((double)iz + 0.5) * a.g.s[2]) : 0.0f;
   const f2 x0 = f2_pack(x0f, x0f), yy = f2_pack(yyf, yyf), yz = f2_pack(yzf, yzf);
   f2 tt[V];
+  float best[V];
 #pragma unroll
   for (int k = 0; k < V; ++k) {
     // in-row offset of voxel k from the row's first voxel, taken between the two fp32 centres
     const float t = (float)((a.g.lo[0] + ((double)(ix0 + k) + 0.5) * a.g.s[0]) - (double)x0f);
     tt[k] = f2_pack(t, t);
+    best[k] = CUDART_INF_F;
+    s_lab[k * T + tid] = 0;
   }
-
-  float best[V];
-  int lab[V];
 #pragma unroll
-  for (int k = 0; k < V; ++k) { best[k] = CUDART_INF_F; lab[k] = 0; }
+  for (int k4 = 0; k4 < V / 4; ++k4)
+    s_prev4[k4 * T + tid] = make_float4(CUDART_INF_F, CUDART_INF_F, CUDART_INF_F, CUDART_INF_F);
+  __syncthreads();   // barrier initialisation visible to every thread
 
   for (int c = 0; c < nchunks; ++c) {
-    const int stage = c % SEED_STAGES;
-    mbar_wait(&s_full[stage], (uint32_t)((c / SEED_STAGES) & 1));
-    const float* sp = s_seeds[stage];
+    const int stage = c % ROW_STAGES;
+    if (tid == 0 && c >= 1 && c + ROW_STAGES - 1 < nchunks) {
+      // refill the stage every warp left at iteration c-1 with chunk c + ROW_STAGES - 1
+      const int s2 = (c - 1) % ROW_STAGES;
+      mbar_wait(&s_empty[s2], (uint32_t)(((c - 1) / ROW_STAGES) & 1));
+      mbar_arrive_expect_tx(&s_full[s2], CHUNK_BYTES);
+      tma_bulk_g2s(s_seeds + (size_t)s2 * CHUNK_PAIRS * PREC,
+                   a.seeds + (size_t)(c + ROW_STAGES - 1) * CHUNK_PAIRS * PREC, CHUNK_BYTES, &s_full[s2]);
+    }
+    mbar_wait(&s_full[stage], (uint32_t)((c / ROW_STAGES) & 1));
+    const float* sp = s_seeds + (size_t)stage * CHUNK_PAIRS * PREC;
     for (int gidx = 0; gidx < CHUNK_PAIRS / GROUP_PAIRS; ++gidx) {
       const float* gp = sp + gidx * GROUP_PAIRS * PREC;
-      float prev[V];
-#pragma unroll
-      for (int k = 0; k < V; ++k) prev[k] = best[k];
-#pragma unroll 2
+#pragma unroll ROW_UNROLL
       for (int p = 0; p < GROUP_PAIRS; ++p) {
         const RowCoef rc = row_setup<DIM>(gp + p * PREC, x0, yy, yz);
 #pragma unroll
-        for (int k = 0; k < V; ++k) {
-          float lo, hi;
-          f2_unpack(row_cost(rc, tt[k]), lo, hi);
-          best[k] = min3f(best[k], lo, hi);
+        for (int k0 = 0; k0 < V; k0 += ROW_BATCH) {
+          f2 u[ROW_BATCH];
+#pragma unroll
+          for (int j = 0; j < ROW_BATCH; ++j) u[j] = f2_fma(rc.a11, tt[k0 + j], rc.Bp);
+#pragma unroll
+          for (int j = 0; j < ROW_BATCH; ++j) u[j] = f2_fma(tt[k0 + j], u[j], rc.Rp);
+#pragma unroll
+          for (int j = 0; j < ROW_BATCH; ++j) {
+            float lo, hi;
+            f2_unpack(u[j], lo, hi);
+            best[k0 + j] = min3f(best[k0 + j], lo, hi);
+          }
         }
       }
-      unsigned int mask = 0u;
+      asm volatile("" ::: "memory");   // keep the prev[] loads below the group loop (they would cost V registers)
+      // fast path: did ANY of the row's minima drop in this group?  (V/4 LDS.128 + V compares)
+      bool any = false;
 #pragma unroll
-      for (int k = 0; k < V; ++k) mask |= (best[k] < prev[k]) ? (1u << k) : 0u;
-      if (mask) {
+      for (int k4 = 0; k4 < V / 4; ++k4) {
+        const float4 pv = s_prev4[k4 * T + tid];
+        any |= (best[4 * k4] < pv.x) | (best[4 * k4 + 1] < pv.y) | (best[4 * k4 + 2] < pv.z) | (best[4 * k4 + 3] < pv.w);
+      }
+      if (any) {
         // a4, deferred: the new minimum of every flagged voxel lies in this group; recompute the
         // group with the same instructions and take the first seed that attains it
+        unsigned int mask = 0u;
+#pragma unroll
+        for (int k4 = 0; k4 < V / 4; ++k4) {
+          float4 pv = s_prev4[k4 * T + tid];
+          if (best[4 * k4] < pv.x) { mask |= 1u << (4 * k4); pv.x = best[4 * k4]; }
+          if (best[4 * k4 + 1] < pv.y) { mask |= 2u << (4 * k4); pv.y = best[4 * k4 + 1]; }
+          if (best[4 * k4 + 2] < pv.z) { mask |= 4u << (4 * k4); pv.z = best[4 * k4 + 2]; }
+          if (best[4 * k4 + 3] < pv.w) { mask |= 8u << (4 * k4); pv.w = best[4 * k4 + 3]; }
+          s_prev4[k4 * T + tid] = pv;
+        }
         const int ibase = c * SEED_CHUNK + gidx * ROW_GROUP;
         for (int p = 0; p < GROUP_PAIRS && mask; ++p) {
           const RowCoef rc = row_setup<DIM>(gp + p * PREC, x0, yy, yz);
@@ -201,38 +281,56 @@ __global__ void __launch_bounds__(G::THREADS) assign_rowpoly_kernel(const Assign
             if (mask & (1u << k)) {
               float lo, hi;
               f2_unpack(row_cost(rc, tt[k]), lo, hi);
-              if (lo == best[k]) { lab[k] = ibase + 2 * p; mask &= ~(1u << k); }
-              else if (hi == best[k]) { lab[k] = ibase + 2 * p + 1; mask &= ~(1u << k); }
+              if (lo == best[k]) { s_lab[k * T + tid] = ibase + 2 * p; mask &= ~(1u << k); }
+              else if (hi == best[k]) { s_lab[k * T + tid] = ibase + 2 * p + 1; mask &= ~(1u << k); }
             }
           }
         }
       }
     }
-    __syncthreads();
-    if (tid == 0 && c + SEED_STAGES < nchunks) {
-      mbar_arrive_expect_tx(&s_full[stage], CHUNK_BYTES);
-      tma_bulk_g2s(s_seeds[stage], a.seeds + (size_t)(c + SEED_STAGES) * CHUNK_PAIRS * PREC, CHUNK_BYTES,
-                   &s_full[stage]);
-    }
+    __syncwarp();
+    if ((tid & 31) == 0) mbar_arrive(&s_empty[stage]);
   }
 
+  int lab[V];
+#pragma unroll
+  for (int k = 0; k < V; ++k) lab[k] = s_lab[k * T + tid];
   const double dsum = row_epilogue<V>(a, row_valid, ix0, iy, iz, best, lab);
-  const double tot = block_sum_double<G::THREADS>(dsum, s_red);
+  const double tot = block_sum_double<T>(dsum, s_red);
   if (tid == 0) a.dual_partial[b] = tot;
 }
 
 static inline int cdiv_i(int x, int y) { return (x + y - 1) / y; }
 
-void rowpoly_tile_counts(int dim, int nx, int ny, int nz, int* tx, int* ty, int* tz) {
-  if (dim == 3) { *tx = cdiv_i(nx, RowGeom3::TXT * RowGeom3::V); *ty = cdiv_i(ny, RowGeom3::TYT); *tz = cdiv_i(nz, RowGeom3::TZT); }
-  else          { *tx = cdiv_i(nx, RowGeom2::TXT * RowGeom2::V); *ty = cdiv_i(ny, RowGeom2::TYT); *tz = 1; }
+template <class G>
+static void tiles_of(int nx, int ny, int nz, int* tx, int* ty, int* tz) {
+  *tx = cdiv_i(nx, G::TXT * G::V); *ty = cdiv_i(ny, G::TYT); *tz = cdiv_i(nz, G::TZT);
+}
+
+// Picks the row length (returned: 0 = SHORT, 1 = LONG) and the tile counts for a grid.
+int rowpoly_tile_counts(int dim, int nx, int ny, int nz, int sm_count, int* tx, int* ty, int* tz) {
+  if (dim == 3) tiles_of<RowGeom3L>(nx, ny, nz, tx, ty, tz); else tiles_of<RowGeom2L>(nx, ny, 1, tx, ty, tz);
+  if ((long long)(*tx) * (*ty) * (*tz) >= (long long)ROW_LONG_MIN_WAVES * ROWMINB * sm_count) return 1;
+  if (dim == 3) tiles_of<RowGeom3S>(nx, ny, nz, tx, ty, tz); else tiles_of<RowGeom2S>(nx, ny, 1, tx, ty, tz);
+  return 0;
+}
+
+template <int DIM, class G>
+static cudaError_t launch_rowpoly_t(const AssignArgs& a, int n_tiles, cudaStream_t st) {
+  constexpr size_t bytes = RowSmem<DIM, G>::BYTES;
+  // opt in to > 48 KB of dynamic shared memory (per device; a host-side attribute write, no launch)
+  cudaError_t e = cudaFuncSetAttribute(assign_rowpoly_kernel<DIM, G>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       (int)bytes);
+  if (e != cudaSuccess) return e;
+  assign_rowpoly_kernel<DIM, G><<<n_tiles, G::THREADS, bytes, st>>>(a);
+  return cudaGetLastError();
 }
 
 cudaError_t launch_assign_rowpoly(const AssignArgs& a, cudaStream_t st) {
   const int n_tiles = a.g.tiles_x * a.g.tiles_y * a.g.tiles_z;
-  if (a.g.dim == 3) assign_rowpoly_kernel<3, RowGeom3><<<n_tiles, RowGeom3::THREADS, 0, st>>>(a);
-  else              assign_rowpoly_kernel<2, RowGeom2><<<n_tiles, RowGeom2::THREADS, 0, st>>>(a);
-  return cudaGetLastError();
+  if (a.g.dim == 3)
+    return a.g.row_long ? launch_rowpoly_t<3, RowGeom3L>(a, n_tiles, st) : launch_rowpoly_t<3, RowGeom3S>(a, n_tiles, st);
+  return a.g.row_long ? launch_rowpoly_t<2, RowGeom2L>(a, n_tiles, st) : launch_rowpoly_t<2, RowGeom2S>(a, n_tiles, st);
 }
 
 }  // namespace apd
