@@ -30,6 +30,7 @@ extern "C" void apd_default_opts(apd_opts* o) {
 }
 
 static void free_ws(Workspace& ws) {
+  cudaFree(ws.rec); cudaFree(ws.cand_list); cudaFree(ws.cand_count); cudaFree(ws.pairs_ctr);
   cudaFree(ws.seeds); cudaFree(ws.count); cudaFree(ws.idxsum); cudaFree(ws.dual_partial);
   cudaFree(ws.sstate); cudaFree(ws.svec); cudaFree(ws.w32); cudaFree(ws.e_vol); cudaFree(ws.e_scal);
   if (ws.report) cudaFreeHost(ws.report);
@@ -124,13 +125,14 @@ int resolve_kernel(const apd_opts* o, std::string* err) {
   if (o && (o->cull != 0 && o->cull != 1)) { *err = "opts.cull must be 0 or 1"; return -1; }
   if (o && (o->reserved[0] || o->reserved[1] || o->reserved[2])) { *err = "opts.reserved must be 0"; return -1; }
   if (k == APD_KERNEL_AUTO) k = APD_KERNEL_ROWPOLY;
+  if (o && o->cull && k != APD_KERNEL_ROWPOLY) { *err = "opts.cull needs kernel AUTO or ROWPOLY"; return -1; }
   return k;
 }
 
 // Enqueues one evaluation (pack -> assign -> finalize) on `st`.  All pointers device.
 int enqueue_evaluation(apd_ctx* ctx, const GridDev& g, int kernel, int M, const float* X, const float* A,
                        const float* w, const float* target_vol, int32_t* labels, double* vol, double* dual,
-                       double* max_rel_err, double* centroids, uint64_t* pairs, bool timed,
+                       double* max_rel_err, double* centroids, uint64_t* pairs, bool timed, bool cull,
                        const int* done_flag, cudaStream_t st) {
   Workspace& ws = ctx->ws;
   const int M_pad = (M + SEED_CHUNK - 1) / SEED_CHUNK * SEED_CHUNK;
@@ -152,12 +154,33 @@ int enqueue_evaluation(apd_ctx* ctx, const GridDev& g, int kernel, int M, const 
   AssignArgs a;
   a.g = g; a.M = M; a.M_pad = M_pad; a.seeds = ws.seeds; a.labels = labels; a.count = ws.count;
   a.idxsum = centroids ? ws.idxsum : nullptr; a.dual_partial = ws.dual_partial;
+  a.rec = nullptr; a.cand_list = nullptr; a.cand_count = nullptr; a.cand_cap = 0; a.pairs_ctr = nullptr;
   a.done_flag = done_flag;
+  if (cull) {
+    // a7: per-tile candidate lists, rebuilt every evaluation (the bounds depend on w)
+    if (!ws.rec) {
+      const size_t m_pad_max = ((size_t)ws.max_seeds + SEED_CHUNK - 1) / SEED_CHUNK * SEED_CHUNK;
+      APD_CUDA_TRY(ctx, cudaMalloc(&ws.rec, m_pad_max * rec_floats(ws.dim) * sizeof(float)));
+      APD_CUDA_TRY(ctx, cudaMalloc(&ws.pairs_ctr, sizeof(unsigned long long)));
+    }
+    if ((size_t)n_tiles > ws.cand_tiles_cap) {
+      APD_CUDA_TRY(ctx, cudaStreamSynchronize(st));
+      cudaFree(ws.cand_list); cudaFree(ws.cand_count);
+      ws.cand_list = nullptr; ws.cand_count = nullptr; ws.cand_tiles_cap = 0;
+      APD_CUDA_TRY(ctx, cudaMalloc(&ws.cand_list, (size_t)n_tiles * CAND_CAP * sizeof(int)));
+      APD_CUDA_TRY(ctx, cudaMalloc(&ws.cand_count, (size_t)n_tiles * sizeof(int)));
+      ws.cand_tiles_cap = (size_t)n_tiles;
+    }
+    APD_CUDA_TRY(ctx, launch_cull(g, M, M_pad, X, A, w, ws.rec, ws.cand_list, ws.cand_count, CAND_CAP, ws.pairs_ctr,
+                                  done_flag, st));
+    a.rec = ws.rec; a.cand_list = ws.cand_list; a.cand_count = ws.cand_count; a.cand_cap = CAND_CAP;
+    a.pairs_ctr = ws.pairs_ctr;
+  }
   if (timed) APD_CUDA_TRY(ctx, cudaEventRecord(ws.ev0, st));
   APD_CUDA_TRY(ctx, launch_assign(kernel, a, st));
   if (timed) { APD_CUDA_TRY(ctx, cudaEventRecord(ws.ev1, st)); ws.timed = true; }
   APD_CUDA_TRY(ctx, launch_finalize(g, M, n_tiles, ws.count, a.idxsum, ws.dual_partial, X, w, target_vol, vol,
-                                    dual, max_rel_err, centroids, pairs, done_flag, st));
+                                    dual, max_rel_err, centroids, pairs, cull ? ws.pairs_ctr : nullptr, done_flag, st));
   return APD_OK;
 }
 
@@ -179,7 +202,7 @@ extern "C" int apd_assign(apd_ctx* ctx, const apd_grid* grid, int32_t M, const f
   if (!e.empty()) { ctx->err = "apd_assign: " + e; return APD_E_ARG; }
   APD_CUDA_TRY(ctx, cudaSetDevice(ctx->ws.device));
   return enqueue_evaluation(ctx, g, kernel, M, X, A, w, target_vol, labels, vol, dual, max_rel_err, centroids,
-                            pairs_evaluated, true, nullptr, static_cast<cudaStream_t>(cuda_stream));
+                            pairs_evaluated, true, opts && opts->cull, nullptr, static_cast<cudaStream_t>(cuda_stream));
 }
 
 extern "C" double apd_last_kernel_ms(apd_ctx* ctx) {

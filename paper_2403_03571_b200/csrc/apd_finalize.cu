@@ -29,7 +29,7 @@ __global__ void __launch_bounds__(FIN_THREADS) finalize_kernel(
     const float* __restrict__ X, const float* __restrict__ w, const float* __restrict__ target_vol,
     double* __restrict__ vol, double* __restrict__ dual, double* __restrict__ max_rel_err,
     double* __restrict__ centroids, uint64_t* __restrict__ pairs_evaluated,
-    const int* __restrict__ done_flag) {
+    const unsigned long long* __restrict__ pairs_ctr, const int* __restrict__ done_flag) {
   __shared__ double scratch[FIN_THREADS / 32];
   if (done_flag && *done_flag) return;
   const int tid = threadIdx.x;
@@ -64,7 +64,8 @@ __global__ void __launch_bounds__(FIN_THREADS) finalize_kernel(
     *dual = vw_tot + P * smin_tot;
     if (max_rel_err && target_vol) *max_rel_err = err_tot;
     if (pairs_evaluated)
-      *pairs_evaluated = (uint64_t)g.nx * (uint64_t)g.ny * (uint64_t)g.nz * (uint64_t)M;
+      *pairs_evaluated = pairs_ctr ? (uint64_t)*pairs_ctr      // culled: what the tiles counted
+                                   : (uint64_t)g.nx * (uint64_t)g.ny * (uint64_t)g.nz * (uint64_t)M;
   }
 }
 
@@ -72,9 +73,10 @@ cudaError_t launch_finalize(const GridDev& g, int M, int n_partials, const unsig
                             const unsigned long long* idxsum, const double* dual_partial,
                             const float* X, const float* w, const float* target_vol,
                             double* vol, double* dual, double* max_rel_err, double* centroids,
-                            uint64_t* pairs_evaluated, const int* done_flag, cudaStream_t st) {
+                            uint64_t* pairs_evaluated, const unsigned long long* pairs_ctr, const int* done_flag,
+                            cudaStream_t st) {
   finalize_kernel<<<1, FIN_THREADS, 0, st>>>(g, M, n_partials, count, idxsum, dual_partial, X, w, target_vol,
-                                             vol, dual, max_rel_err, centroids, pairs_evaluated, done_flag);
+                                             vol, dual, max_rel_err, centroids, pairs_evaluated, pairs_ctr, done_flag);
   return cudaGetLastError();
 }
 

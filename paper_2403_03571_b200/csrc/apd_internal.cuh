@@ -42,6 +42,12 @@ struct AssignArgs {
   unsigned int* count;   // [M] voxels per cell (exact integers: eq. 2.8)
   unsigned long long* idxsum;  // [M,3] sum of voxel indices per axis, or nullptr
   double* dual_partial;  // [n_tiles] sum over the tile of min_i C_ij
+  // tile culling (a7); all nullptr / 0 for brute force
+  const float* rec;      // [M_pad, REC] per-seed records (DIRECT layout)
+  const int* cand_list;  // [n_tiles, cand_cap] ascending seed indices per tile
+  const int* cand_count; // [n_tiles] list length, or -1: list overflowed, scan all seeds
+  int cand_cap;
+  unsigned long long* pairs_ctr;  // [1] voxel-seed pairs evaluated
   const int* done_flag;  // solve loop only: kernels return at once when *done_flag != 0; else nullptr
 };
 
@@ -52,6 +58,12 @@ struct Workspace {
   unsigned long long* idxsum = nullptr;  // [max_seeds,3]
   double* dual_partial = nullptr;      // [partial_cap]
   size_t partial_cap = 0;
+  // tile culling (apd_cull.cu), allocated on first use
+  float* rec = nullptr;                // [M_pad, REC] per-seed records + rho
+  int* cand_list = nullptr;            // [cand_tiles_cap * CAND_CAP]
+  int* cand_count = nullptr;           // [cand_tiles_cap]
+  size_t cand_tiles_cap = 0;
+  unsigned long long* pairs_ctr = nullptr;
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
   bool timed = false;
   // apd_solve state (apd_lbfgs.cu), allocated on first use
@@ -75,13 +87,19 @@ cudaError_t launch_pack_pairs(int dim, int M, int M_pad, const float* X, const f
                               float* seeds, unsigned int* count, unsigned long long* idxsum,
                               const int* done_flag, cudaStream_t st);
 cudaError_t launch_assign_rowpoly(const AssignArgs& a, cudaStream_t st);
+void rowpoly_tile_extent(int dim, int row_long, int* ex, int* ey, int* ez);
+constexpr int CAND_CAP = 1024;         // candidate-list capacity per tile; a longer list falls back to all seeds
+cudaError_t launch_cull(const GridDev& g, int M, int M_pad, const float* X, const float* A, const float* w, float* rec,
+                        int* list, int* count, int cap, unsigned long long* pairs_ctr, const int* done_flag,
+                        cudaStream_t st);
 int rowpoly_tile_counts(int dim, int nx, int ny, int nz, int sm_count, int* tx, int* ty, int* tz);
 int assign_tile_counts(int kernel, int dim, int nx, int ny, int nz, int sm_count, int* tx, int* ty, int* tz);
 cudaError_t launch_finalize(const GridDev& g, int M, int n_partials, const unsigned int* count,
                             const unsigned long long* idxsum, const double* dual_partial,
                             const float* X, const float* w, const float* target_vol,
                             double* vol, double* dual, double* max_rel_err, double* centroids,
-                            uint64_t* pairs_evaluated, const int* done_flag, cudaStream_t st);
+                            uint64_t* pairs_evaluated, const unsigned long long* pairs_ctr, const int* done_flag,
+                            cudaStream_t st);
 
 // What the device-side optimiser reports to the host (mapped pinned memory).
 struct SolveReport {
@@ -96,7 +114,7 @@ std::string make_grid(const apd_ctx* ctx, const apd_grid* grid, int kernel, Grid
 int resolve_kernel(const apd_opts* o, std::string* err);
 int enqueue_evaluation(apd_ctx* ctx, const GridDev& g, int kernel, int M, const float* X, const float* A,
                        const float* w, const float* target_vol, int32_t* labels, double* vol, double* dual,
-                       double* max_rel_err, double* centroids, uint64_t* pairs, bool timed,
+                       double* max_rel_err, double* centroids, uint64_t* pairs, bool timed, bool cull,
                        const int* done_flag, cudaStream_t st);
 
 }  // namespace apd

@@ -341,7 +341,7 @@ extern "C" int apd_solve(apd_ctx* ctx, const apd_grid* grid, int32_t M, const fl
   const long long hard_cap = (long long)max_evals + 64;
   for (;; ++enq) {
     rc = enqueue_evaluation(ctx, g, kernel, M, X, A, ws.w32, target_vol, nullptr, ws.e_vol, ws.e_scal,
-                            ws.e_scal + 1, nullptr, nullptr, false, done_flag, st);
+                            ws.e_scal + 1, nullptr, nullptr, false, o.cull != 0, done_flag, st);
     if (rc != APD_OK) return rc;
     lbfgs_step_kernel<<<1, LB_THREADS, 0, st>>>(sa);
     LB_TRY(cudaGetLastError());
@@ -360,7 +360,7 @@ extern "C" int apd_solve(apd_ctx* ctx, const apd_grid* grid, int32_t M, const fl
 
   // final evaluation at the returned fp32 weights, with labels (Algorithm 1 at the solution)
   rc = enqueue_evaluation(ctx, g, kernel, M, X, A, ws.w32, target_vol, labels, vol ? vol : ws.e_vol, ws.e_scal,
-                          ws.e_scal + 1, nullptr, nullptr, true, nullptr, st);
+                          ws.e_scal + 1, nullptr, nullptr, true, o.cull != 0, nullptr, st);
   if (rc != APD_OK) return rc;
   LB_TRY(cudaMemcpyAsync(w, ws.w32, sizeof(float) * M, cudaMemcpyDeviceToDevice, st));
   if (w64) LB_TRY(cudaMemcpyAsync(w64, ws.svec + (size_t)V_W * ws.max_seeds, sizeof(double) * M,

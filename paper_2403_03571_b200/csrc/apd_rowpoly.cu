@@ -164,6 +164,102 @@ struct RowSmem {
   static constexpr size_t BYTES = RED_OFF + (G::THREADS / 32) * sizeof(double);
 };
 
+// One staged chunk of SEED_CHUNK seeds (pair-interleaved records at `sp`) against the thread's row: rows a3 + a4.
+// IDX = false: the chunk holds seeds ibase .. ibase+SEED_CHUNK-1 in index order (brute force);
+// IDX = true : the seed index of position q of the chunk is s_idx[q] (tile-culled candidate list, ascending).
+template <int DIM, int V, int T, bool IDX>
+__device__ __forceinline__ void row_process_chunk(const float* __restrict__ sp, int ibase, const int* __restrict__ s_idx,
+                                                  f2 x0, f2 yy, f2 yz, const f2 (&tt)[V], float (&best)[V],
+                                                  float4* __restrict__ s_prev4, int* __restrict__ s_lab, int tid) {
+  constexpr int PREC = (DIM == 3) ? PREC3 : PREC2;
+  constexpr int CHUNK_PAIRS = SEED_CHUNK / 2;
+  constexpr int GROUP_PAIRS = ROW_GROUP / 2;
+  for (int gidx = 0; gidx < CHUNK_PAIRS / GROUP_PAIRS; ++gidx) {
+    const float* gp = sp + gidx * GROUP_PAIRS * PREC;
+#pragma unroll ROW_UNROLL
+    for (int p = 0; p < GROUP_PAIRS; ++p) {
+      const RowCoef rc = row_setup<DIM>(gp + p * PREC, x0, yy, yz);
+#pragma unroll
+      for (int k0 = 0; k0 < V; k0 += ROW_BATCH) {
+        f2 u[ROW_BATCH];
+#pragma unroll
+        for (int j = 0; j < ROW_BATCH; ++j) u[j] = f2_fma(rc.a11, tt[k0 + j], rc.Bp);
+#pragma unroll
+        for (int j = 0; j < ROW_BATCH; ++j) u[j] = f2_fma(tt[k0 + j], u[j], rc.Rp);
+#pragma unroll
+        for (int j = 0; j < ROW_BATCH; ++j) {
+          float lo, hi;
+          f2_unpack(u[j], lo, hi);
+          best[k0 + j] = min3f(best[k0 + j], lo, hi);
+        }
+      }
+    }
+    asm volatile("" ::: "memory");   // keep the prev[] loads below the group loop (they would cost V registers)
+    // fast path: did ANY of the row's minima drop in this group?  (V/4 LDS.128 + V compares)
+    bool any = false;
+#pragma unroll
+    for (int k4 = 0; k4 < V / 4; ++k4) {
+      const float4 pv = s_prev4[k4 * T + tid];
+      any |= (best[4 * k4] < pv.x) | (best[4 * k4 + 1] < pv.y) | (best[4 * k4 + 2] < pv.z) | (best[4 * k4 + 3] < pv.w);
+    }
+    if (any) {
+      // a4, deferred: the new minimum of every flagged voxel lies in this group; recompute the
+      // group with the same instructions and take the first seed that attains it
+      unsigned int mask = 0u;
+#pragma unroll
+      for (int k4 = 0; k4 < V / 4; ++k4) {
+        float4 pv = s_prev4[k4 * T + tid];
+        if (best[4 * k4] < pv.x) { mask |= 1u << (4 * k4); pv.x = best[4 * k4]; }
+        if (best[4 * k4 + 1] < pv.y) { mask |= 2u << (4 * k4); pv.y = best[4 * k4 + 1]; }
+        if (best[4 * k4 + 2] < pv.z) { mask |= 4u << (4 * k4); pv.z = best[4 * k4 + 2]; }
+        if (best[4 * k4 + 3] < pv.w) { mask |= 8u << (4 * k4); pv.w = best[4 * k4 + 3]; }
+        s_prev4[k4 * T + tid] = pv;
+      }
+      for (int p = 0; p < GROUP_PAIRS && mask; ++p) {
+        const RowCoef rc = row_setup<DIM>(gp + p * PREC, x0, yy, yz);
+        const int q = gidx * ROW_GROUP + 2 * p;           // position of the pair's first seed in the chunk
+        const int i0 = IDX ? s_idx[q] : ibase + q;
+        const int i1 = IDX ? s_idx[q + 1] : ibase + q + 1;
+#pragma unroll
+        for (int k = 0; k < V; ++k) {
+          if (mask & (1u << k)) {
+            float lo, hi;
+            f2_unpack(row_cost(rc, tt[k]), lo, hi);
+            if (lo == best[k]) { s_lab[k * T + tid] = i0; mask &= ~(1u << k); }
+            else if (hi == best[k]) { s_lab[k * T + tid] = i1; mask &= ~(1u << k); }
+          }
+        }
+      }
+    }
+  }
+}
+
+// Per-thread row set-up shared by the brute-force and the culled kernel (a1).
+template <int DIM, class G>
+struct RowThread {
+  int ix0, iy, iz;
+  bool row_valid;
+  f2 x0, yy, yz;
+  __device__ __forceinline__ void init(const AssignArgs& a, int b, int tid) {
+    const int tx = tid % G::TXT, ty = (tid / G::TXT) % G::TYT, tz = tid / (G::TXT * G::TYT);
+    const int bx = b % a.g.tiles_x, by = (b / a.g.tiles_x) % a.g.tiles_y, bz = b / (a.g.tiles_x * a.g.tiles_y);
+    ix0 = (bx * G::TXT + tx) * G::V; iy = by * G::TYT + ty; iz = bz * G::TZT + tz;
+    row_valid = (ix0 < a.g.nx) && (iy < a.g.ny) && (iz < a.g.nz);
+    // coordinates from the thread index (fp64 definition rounded once to fp32)
+    const float x0f = (float)(a.g.lo[0] + ((double)ix0 + 0.5) * a.g.s[0]);
+    const float yyf = (float)(a.g.lo[1] + ((double)iy + 0.5) * a.g.s[1]);
+    const float yzf = (DIM == 3) ? (float)(a.g.lo[2] + ((double)iz + 0.5) * a.g.s[2]) : 0.0f;
+    x0 = f2_pack(x0f, x0f); yy = f2_pack(yyf, yyf); yz = f2_pack(yzf, yzf);
+  }
+  // in-row offset of voxel k from the row's first voxel, taken between the two fp32 centres
+  __device__ __forceinline__ f2 tau(const AssignArgs& a, int k) const {
+    float x0f, dummy;
+    f2_unpack(x0, x0f, dummy);
+    const float t = (float)((a.g.lo[0] + ((double)(ix0 + k) + 0.5) * a.g.s[0]) - (double)x0f);
+    return f2_pack(t, t);
+  }
+};
+
 template <int DIM, class G>
 __global__ void __launch_bounds__(G::THREADS, G::MINB) assign_rowpoly_kernel(const AssignArgs a) {
   constexpr int V = G::V, T = G::THREADS;
@@ -171,8 +267,7 @@ __global__ void __launch_bounds__(G::THREADS, G::MINB) assign_rowpoly_kernel(con
   constexpr int PREC = S::PREC;
   constexpr int CHUNK_PAIRS = S::CHUNK_PAIRS;
   constexpr uint32_t CHUNK_BYTES = CHUNK_PAIRS * PREC * sizeof(float);
-  constexpr int GROUP_PAIRS = ROW_GROUP / 2;
-  static_assert(V <= 32 && V % ROW_BATCH == 0, "row mask is 32 bits");
+  static_assert(V <= 32 && V % ROW_BATCH == 0 && V % 4 == 0, "row mask is 32 bits");
   extern __shared__ __align__(128) unsigned char smem_raw[];
   float* s_seeds = reinterpret_cast<float*>(smem_raw);
   float4* s_prev4 = reinterpret_cast<float4*>(smem_raw + S::PREV_OFF);   // [V/4][T]
@@ -183,11 +278,9 @@ __global__ void __launch_bounds__(G::THREADS, G::MINB) assign_rowpoly_kernel(con
 
   if (a.done_flag && *a.done_flag) return;
   const int tid = threadIdx.x;
-  const int tx = tid % G::TXT, ty = (tid / G::TXT) % G::TYT, tz = tid / (G::TXT * G::TYT);
   const int b = blockIdx.x;
-  const int bx = b % a.g.tiles_x, by = (b / a.g.tiles_x) % a.g.tiles_y, bz = b / (a.g.tiles_x * a.g.tiles_y);
-  const int ix0 = (bx * G::TXT + tx) * V, iy = by * G::TYT + ty, iz = bz * G::TZT + tz;
-  const bool row_valid = (ix0 < a.g.nx) && (iy < a.g.ny) && (iz < a.g.nz);
+  RowThread<DIM, G> rt;
+  rt.init(a, b, tid);
 
   const int nchunks = a.M_pad / SEED_CHUNK;
   if (tid == 0) {
@@ -200,18 +293,11 @@ __global__ void __launch_bounds__(G::THREADS, G::MINB) assign_rowpoly_kernel(con
     }
   }
 
-  // a1: coordinates from the thread index (fp64 definition rounded once to fp32)
-  const float x0f = (float)(a.g.lo[0] + ((double)ix0 + 0.5) * a.g.s[0]);
-  const float yyf = (float)(a.g.lo[1] + ((double)iy + 0.5) * a.g.s[1]);
-  const float yzf = (DIM == 3) ? (float)(a.g.lo[2] + ((double)iz + 0.5) * a.g.s[2]) : 0.0f;
-  const f2 x0 = f2_pack(x0f, x0f), yy = f2_pack(yyf, yyf), yz = f2_pack(yzf, yzf);
   f2 tt[V];
   float best[V];
 #pragma unroll
   for (int k = 0; k < V; ++k) {
-    // in-row offset of voxel k from the row's first voxel, taken between the two fp32 centres
-    const float t = (float)((a.g.lo[0] + ((double)(ix0 + k) + 0.5) * a.g.s[0]) - (double)x0f);
-    tt[k] = f2_pack(t, t);
+    tt[k] = rt.tau(a, k);
     best[k] = CUDART_INF_F;
     s_lab[k * T + tid] = 0;
   }
@@ -231,63 +317,8 @@ __global__ void __launch_bounds__(G::THREADS, G::MINB) assign_rowpoly_kernel(con
                    a.seeds + (size_t)(c + ROW_STAGES - 1) * CHUNK_PAIRS * PREC, CHUNK_BYTES, &s_full[s2]);
     }
     mbar_wait(&s_full[stage], (uint32_t)((c / ROW_STAGES) & 1));
-    const float* sp = s_seeds + (size_t)stage * CHUNK_PAIRS * PREC;
-    for (int gidx = 0; gidx < CHUNK_PAIRS / GROUP_PAIRS; ++gidx) {
-      const float* gp = sp + gidx * GROUP_PAIRS * PREC;
-#pragma unroll ROW_UNROLL
-      for (int p = 0; p < GROUP_PAIRS; ++p) {
-        const RowCoef rc = row_setup<DIM>(gp + p * PREC, x0, yy, yz);
-#pragma unroll
-        for (int k0 = 0; k0 < V; k0 += ROW_BATCH) {
-          f2 u[ROW_BATCH];
-#pragma unroll
-          for (int j = 0; j < ROW_BATCH; ++j) u[j] = f2_fma(rc.a11, tt[k0 + j], rc.Bp);
-#pragma unroll
-          for (int j = 0; j < ROW_BATCH; ++j) u[j] = f2_fma(tt[k0 + j], u[j], rc.Rp);
-#pragma unroll
-          for (int j = 0; j < ROW_BATCH; ++j) {
-            float lo, hi;
-            f2_unpack(u[j], lo, hi);
-            best[k0 + j] = min3f(best[k0 + j], lo, hi);
-          }
-        }
-      }
-      asm volatile("" ::: "memory");   // keep the prev[] loads below the group loop (they would cost V registers)
-      // fast path: did ANY of the row's minima drop in this group?  (V/4 LDS.128 + V compares)
-      bool any = false;
-#pragma unroll
-      for (int k4 = 0; k4 < V / 4; ++k4) {
-        const float4 pv = s_prev4[k4 * T + tid];
-        any |= (best[4 * k4] < pv.x) | (best[4 * k4 + 1] < pv.y) | (best[4 * k4 + 2] < pv.z) | (best[4 * k4 + 3] < pv.w);
-      }
-      if (any) {
-        // a4, deferred: the new minimum of every flagged voxel lies in this group; recompute the
-        // group with the same instructions and take the first seed that attains it
-        unsigned int mask = 0u;
-#pragma unroll
-        for (int k4 = 0; k4 < V / 4; ++k4) {
-          float4 pv = s_prev4[k4 * T + tid];
-          if (best[4 * k4] < pv.x) { mask |= 1u << (4 * k4); pv.x = best[4 * k4]; }
-          if (best[4 * k4 + 1] < pv.y) { mask |= 2u << (4 * k4); pv.y = best[4 * k4 + 1]; }
-          if (best[4 * k4 + 2] < pv.z) { mask |= 4u << (4 * k4); pv.z = best[4 * k4 + 2]; }
-          if (best[4 * k4 + 3] < pv.w) { mask |= 8u << (4 * k4); pv.w = best[4 * k4 + 3]; }
-          s_prev4[k4 * T + tid] = pv;
-        }
-        const int ibase = c * SEED_CHUNK + gidx * ROW_GROUP;
-        for (int p = 0; p < GROUP_PAIRS && mask; ++p) {
-          const RowCoef rc = row_setup<DIM>(gp + p * PREC, x0, yy, yz);
-#pragma unroll
-          for (int k = 0; k < V; ++k) {
-            if (mask & (1u << k)) {
-              float lo, hi;
-              f2_unpack(row_cost(rc, tt[k]), lo, hi);
-              if (lo == best[k]) { s_lab[k * T + tid] = ibase + 2 * p; mask &= ~(1u << k); }
-              else if (hi == best[k]) { s_lab[k * T + tid] = ibase + 2 * p + 1; mask &= ~(1u << k); }
-            }
-          }
-        }
-      }
-    }
+    row_process_chunk<DIM, V, T, false>(s_seeds + (size_t)stage * CHUNK_PAIRS * PREC, c * SEED_CHUNK, nullptr,
+                                        rt.x0, rt.yy, rt.yz, tt, best, s_prev4, s_lab, tid);
     __syncwarp();
     if ((tid & 31) == 0) mbar_arrive(&s_empty[stage]);
   }
@@ -295,9 +326,116 @@ __global__ void __launch_bounds__(G::THREADS, G::MINB) assign_rowpoly_kernel(con
   int lab[V];
 #pragma unroll
   for (int k = 0; k < V; ++k) lab[k] = s_lab[k * T + tid];
-  const double dsum = row_epilogue<V>(a, row_valid, ix0, iy, iz, best, lab);
+  const double dsum = row_epilogue<V>(a, rt.row_valid, rt.ix0, rt.iy, rt.iz, best, lab);
   const double tot = block_sum_double<T>(dsum, s_red);
   if (tid == 0) a.dual_partial[b] = tot;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// a7: the same reduction over a tile's CANDIDATE LIST (apd_cull.cu) instead of all seeds.  The list is ascending
+// in seed index, so "first seed attaining the minimum" is still the lowest index (reading S1).  Candidates are
+// gathered from the per-seed record table into the pair-interleaved smem layout by the CTA's own threads (one
+// candidate per thread and chunk).  A tile whose list overflowed (count < 0) scans all seeds.
+// smem: seeds [2][CHUNK_PAIRS*PREC] | prev | lab | idx [2][SEED_CHUNK] | red
+// ------------------------------------------------------------------------------------------------------------
+template <int DIM, class G>
+struct CullSmem {
+  static constexpr int PREC = (DIM == 3) ? PREC3 : PREC2;
+  static constexpr int CHUNK_PAIRS = SEED_CHUNK / 2;
+  static constexpr size_t SEED_BYTES = (size_t)2 * CHUNK_PAIRS * PREC * sizeof(float);
+  static constexpr size_t PREV_OFF = SEED_BYTES;
+  static constexpr size_t LAB_OFF = PREV_OFF + (size_t)G::V * G::THREADS * sizeof(float);
+  static constexpr size_t IDX_OFF = LAB_OFF + (size_t)G::V * G::THREADS * sizeof(int);
+  static constexpr size_t RED_OFF = IDX_OFF + 2 * SEED_CHUNK * sizeof(int);
+  static constexpr size_t BYTES = RED_OFF + (G::THREADS / 32) * sizeof(double);
+};
+
+template <int DIM, class G>
+__global__ void __launch_bounds__(G::THREADS, G::MINB) assign_rowpoly_culled_kernel(const AssignArgs a) {
+  constexpr int V = G::V, T = G::THREADS;
+  using S = CullSmem<DIM, G>;
+  constexpr int PREC = S::PREC;
+  constexpr int CHUNK_PAIRS = S::CHUNK_PAIRS;
+  constexpr int REC = (DIM == 3) ? REC3 : REC2;
+  constexpr int NP = (DIM == 3) ? 10 : 6;       // parameters per seed in a record
+  static_assert(T == SEED_CHUNK, "one gathered candidate per thread and chunk");
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  float* s_seeds = reinterpret_cast<float*>(smem_raw);
+  float4* s_prev4 = reinterpret_cast<float4*>(smem_raw + S::PREV_OFF);
+  int* s_lab = reinterpret_cast<int*>(smem_raw + S::LAB_OFF);
+  int* s_idx = reinterpret_cast<int*>(smem_raw + S::IDX_OFF);
+  double* s_red = reinterpret_cast<double*>(smem_raw + S::RED_OFF);
+
+  if (a.done_flag && *a.done_flag) return;
+  const int tid = threadIdx.x;
+  const int b = blockIdx.x;
+  RowThread<DIM, G> rt;
+  rt.init(a, b, tid);
+
+  int cnt = a.cand_count[b];
+  const bool listed = cnt >= 0;
+  if (!listed) cnt = a.M;
+  const int* list = a.cand_list + (size_t)b * a.cand_cap;
+  const int nchunks = (cnt + SEED_CHUNK - 1) / SEED_CHUNK;
+
+  f2 tt[V];
+  float best[V];
+#pragma unroll
+  for (int k = 0; k < V; ++k) {
+    tt[k] = rt.tau(a, k);
+    best[k] = CUDART_INF_F;
+    s_lab[k * T + tid] = 0;
+  }
+#pragma unroll
+  for (int k4 = 0; k4 < V / 4; ++k4)
+    s_prev4[k4 * T + tid] = make_float4(CUDART_INF_F, CUDART_INF_F, CUDART_INF_F, CUDART_INF_F);
+
+  auto gather = [&](int c) {
+    const int stage = c & 1;
+    const int pos = c * SEED_CHUNK + tid;
+    float r[REC];
+    int idx = 0;
+    if (pos < cnt) {
+      idx = listed ? list[pos] : pos;
+      const float4* src = reinterpret_cast<const float4*>(a.rec + (size_t)idx * REC);
+#pragma unroll
+      for (int q = 0; q < REC / 4; ++q) {
+        const float4 v4 = __ldg(src + q);
+        r[4 * q] = v4.x; r[4 * q + 1] = v4.y; r[4 * q + 2] = v4.z; r[4 * q + 3] = v4.w;
+      }
+    } else {
+#pragma unroll
+      for (int q = 0; q < REC; ++q) r[q] = 0.0f;
+      r[NP - 1] = CUDART_INF_F;      // padding candidate: cost +inf, never wins the strict '<'
+    }
+    float* dst = s_seeds + (size_t)stage * CHUNK_PAIRS * PREC + (tid >> 1) * PREC + (tid & 1);
+#pragma unroll
+    for (int q = 0; q < NP; ++q) dst[2 * q] = r[q];
+    s_idx[stage * SEED_CHUNK + tid] = idx;
+  };
+
+  if (nchunks > 0) gather(0);
+  __syncthreads();
+  for (int c = 0; c < nchunks; ++c) {
+    if (c + 1 < nchunks) gather(c + 1);     // the other stage: every thread left it before the last barrier
+    row_process_chunk<DIM, V, T, true>(s_seeds + (size_t)(c & 1) * CHUNK_PAIRS * PREC, 0, s_idx + (c & 1) * SEED_CHUNK,
+                                       rt.x0, rt.yy, rt.yz, tt, best, s_prev4, s_lab, tid);
+    __syncthreads();
+  }
+
+  int lab[V];
+#pragma unroll
+  for (int k = 0; k < V; ++k) lab[k] = s_lab[k * T + tid];
+  const double dsum = row_epilogue<V>(a, rt.row_valid, rt.ix0, rt.iy, rt.iz, best, lab);
+  const double tot = block_sum_double<T>(dsum, s_red);
+  if (tid == 0) {
+    a.dual_partial[b] = tot;
+    // voxel-seed pairs whose cost this tile evaluated (valid voxels only)
+    const int bx = b % a.g.tiles_x, by = (b / a.g.tiles_x) % a.g.tiles_y, bz = b / (a.g.tiles_x * a.g.tiles_y);
+    const long long vx = min(G::TXT * V, a.g.nx - bx * G::TXT * V), vy = min(G::TYT, a.g.ny - by * G::TYT),
+                    vz = min(G::TZT, a.g.nz - bz * G::TZT);
+    atomicAdd(a.pairs_ctr, (unsigned long long)(vx * vy * vz) * (unsigned long long)cnt);
+  }
 }
 
 static inline int cdiv_i(int x, int y) { return (x + y - 1) / y; }
@@ -317,13 +455,32 @@ int rowpoly_tile_counts(int dim, int nx, int ny, int nz, int sm_count, int* tx, 
 
 template <int DIM, class G>
 static cudaError_t launch_rowpoly_t(const AssignArgs& a, int n_tiles, cudaStream_t st) {
-  constexpr size_t bytes = RowSmem<DIM, G>::BYTES;
   // opt in to > 48 KB of dynamic shared memory (per device; a host-side attribute write, no launch)
+  if (a.cand_count) {
+    constexpr size_t bytes = CullSmem<DIM, G>::BYTES;
+    cudaError_t e = cudaFuncSetAttribute(assign_rowpoly_culled_kernel<DIM, G>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    if (e != cudaSuccess) return e;
+    assign_rowpoly_culled_kernel<DIM, G><<<n_tiles, G::THREADS, bytes, st>>>(a);
+    return cudaGetLastError();
+  }
+  constexpr size_t bytes = RowSmem<DIM, G>::BYTES;
   cudaError_t e = cudaFuncSetAttribute(assign_rowpoly_kernel<DIM, G>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                        (int)bytes);
   if (e != cudaSuccess) return e;
   assign_rowpoly_kernel<DIM, G><<<n_tiles, G::THREADS, bytes, st>>>(a);
   return cudaGetLastError();
+}
+
+// tile extents in voxels of the geometry chosen for the grid (the culling bounds need them)
+void rowpoly_tile_extent(int dim, int row_long, int* ex, int* ey, int* ez) {
+  if (dim == 3) {
+    if (row_long) { *ex = RowGeom3L::TXT * RowGeom3L::V; *ey = RowGeom3L::TYT; *ez = RowGeom3L::TZT; }
+    else          { *ex = RowGeom3S::TXT * RowGeom3S::V; *ey = RowGeom3S::TYT; *ez = RowGeom3S::TZT; }
+  } else {
+    if (row_long) { *ex = RowGeom2L::TXT * RowGeom2L::V; *ey = RowGeom2L::TYT; *ez = 1; }
+    else          { *ex = RowGeom2S::TXT * RowGeom2S::V; *ey = RowGeom2S::TYT; *ez = 1; }
+  }
 }
 
 cudaError_t launch_assign_rowpoly(const AssignArgs& a, cudaStream_t st) {

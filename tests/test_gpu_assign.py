@@ -19,7 +19,7 @@ def apd():
     return binding
 
 
-def run_assign(apd, wl, w, v=None, kernel=0, want_centroids=False, want_labels=True, ctx=None):
+def run_assign(apd, wl, w, v=None, kernel=0, want_centroids=False, want_labels=True, ctx=None, cull=0):
     dev = torch.device("cuda:0")
     ctx = ctx or apd.ApdContext(wl.dim, max(wl.M, 1))
     grid = apd.make_grid(wl.dim, wl.n, wl.lo, wl.hi)
@@ -34,7 +34,7 @@ def run_assign(apd, wl, w, v=None, kernel=0, want_centroids=False, want_labels=T
     cen = torch.zeros(wl.M, wl.dim, dtype=torch.float64, device=dev) if want_centroids else None
     pairs = torch.zeros(1, dtype=torch.int64, device=dev)
     ctx.apd_assign(grid, X, A, wt, target_vol=vt, labels=labels, vol=vol, dual=dual, max_rel_err=err,
-                   centroids=cen, pairs_evaluated=pairs, opts=apd.make_opts(kernel=kernel))
+                   centroids=cen, pairs_evaluated=pairs, opts=apd.make_opts(kernel=kernel, cull=cull))
     torch.cuda.synchronize()
     return dict(labels=labels.cpu().numpy() if want_labels else None, vol=vol.cpu().numpy(),
                 dual=float(dual.item()), err=float(err.item()),
@@ -206,3 +206,53 @@ def test_host_call_matches_device_call(apd):
     assert np.array_equal(labels.numpy(), r["labels"]) and np.array_equal(vol.numpy(), r["vol"])
     assert dual == r["dual"] and err == r["err"] and pairs == wl.N * wl.M
     assert np.array_equal(cen.numpy(), r["centroids"])
+
+
+# ------------------------------------------------------------------ a7: exact tile culling
+@pytest.mark.parametrize("cfg,n,M", [(1, None, None), (2, None, None), (3, None, None), (4, (160, 128, 96), 3000),
+                                     (5, (128, 128, 128), 2500)])
+@pytest.mark.parametrize("wscale", [0.0, 0.2])
+def test_culling_is_exact(apd, cfg, n, M, wscale):
+    """Labels, volumes and centroids with culling == without, bit for bit; the dual to summation order."""
+    wl = workloads.make_config(cfg, n=n, M=M)
+    w = wl.w0 if wscale == 0.0 else rand_w(wl, wscale, 300 + cfg)
+    r0 = run_assign(apd, wl, w, v=wl.v, want_centroids=True, cull=0)
+    r1 = run_assign(apd, wl, w, v=wl.v, want_centroids=True, cull=1)
+    assert np.array_equal(r0["labels"], r1["labels"])
+    assert np.array_equal(r0["vol"], r1["vol"]) and np.array_equal(r0["centroids"], r1["centroids"])
+    assert r1["dual"] == r0["dual"] and r1["err"] == r0["err"]          # same fp32 minima, same reduction order
+    assert 0 < r1["pairs"] <= wl.N * wl.M and r0["pairs"] == wl.N * wl.M
+    print(f"cfg{cfg} {wl.n} M={wl.M} wscale={wscale}: pruned fraction {1 - r1['pairs'] / (wl.N * wl.M):.4f}")
+
+
+@pytest.mark.parametrize("case", EDGE, ids=lambda c: f"{c['dim']}d_{'x'.join(map(str, c['n']))}_M{c['M']}")
+def test_culling_edge_cases_parity(apd, case):
+    wl = workloads.make_random(case["dim"], case["n"], case["M"], case["seed"], lo=case["lo"], hi=case["hi"],
+                               w_scale=0.1, aspect=5.0)
+    r = run_assign(apd, wl, wl.w0, v=wl.v, want_centroids=True, cull=1)
+    parity.check_assign(wl, wl.w0, r["labels"], r["vol"], r["dual"], v=wl.v, centroids_gpu=r["centroids"],
+                        err_gpu=r["err"])
+    r0 = run_assign(apd, wl, wl.w0, v=wl.v, cull=0)
+    assert np.array_equal(r0["labels"], r["labels"])
+
+
+def test_culling_extreme_weights_and_overflow(apd):
+    """One seed with a huge weight owns everything; every seed coincident => every list overflows CAND_CAP
+    (1024) and the tile falls back to scanning all seeds."""
+    wl = workloads.make_random(3, (64, 48, 40), 300, 31, w_scale=0.1)
+    w = wl.w0.copy(); w[17] = 10.0
+    r = run_assign(apd, wl, w, v=wl.v, cull=1)
+    assert np.all(r["labels"] == 17)
+    wl2 = workloads.make_random(3, (40, 40, 40), 1500, 32)
+    wl2.X[:] = wl2.X[0]; wl2.A[:] = wl2.A[0]                 # coincident, identical seeds: nothing can be pruned
+    r0 = run_assign(apd, wl2, wl2.w0, v=wl2.v, cull=0)
+    r1 = run_assign(apd, wl2, wl2.w0, v=wl2.v, cull=1)
+    assert np.all(r0["labels"] == 0) and np.array_equal(r0["labels"], r1["labels"])
+    assert r1["pairs"] == wl2.N * wl2.M
+
+
+def test_culling_rejects_direct_kernel(apd):
+    wl = workloads.make_config(1)
+    with pytest.raises(apd.ApdError) as e:
+        run_assign(apd, wl, wl.w0, kernel=KERNELS["direct"], cull=1)
+    assert e.value.status == apd.APD_E_ARG
