@@ -129,6 +129,11 @@ int apd_solve(apd_ctx* ctx, const apd_grid* grid, int32_t M,
               int32_t* iters, int32_t* evals, double* max_rel_err, double* dual,
               const apd_opts* opts, void* cuda_stream);
 
+/* Convergence history of the most recent apd_solve on this context: (dual g~, max relative volume error) of every
+ * evaluation in order (at most the first 8192).  dual_hist, err_hist: HOST out, [cap] each.  Returns the number of
+ * entries written (>= 0), or a negative apd_status.  Synchronous. */
+int apd_solve_history(apd_ctx* ctx, double* dual_hist, double* err_hist, int32_t cap);
+
 /* Same two calls with HOST arrays: the library allocates device buffers, copies in, runs the
  * device call above, copies the results out and frees.  Every pointer is HOST memory; NULL is
  * allowed where the device call allows it.  Synchronous. */

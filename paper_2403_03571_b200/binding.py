@@ -78,6 +78,8 @@ def load_library() -> ctypes.CDLL:
                                    + [_P] * 5 + [ctypes.POINTER(ctypes.c_int32), ctypes.POINTER(ctypes.c_int32),
                                                  ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double),
                                                  ctypes.POINTER(apd_opts)])
+    lib.apd_solve_history.restype = ctypes.c_int
+    lib.apd_solve_history.argtypes = [_P, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double), ctypes.c_int32]
     lib.apd_last_kernel_ms.restype = ctypes.c_double
     lib.apd_last_kernel_ms.argtypes = [_P]
     lib.apd_fp32_probe.restype = ctypes.c_int
@@ -88,7 +90,7 @@ def load_library() -> ctypes.CDLL:
 
 
 EXPORTED_SYMBOLS = ["apd_default_opts", "apd_create", "apd_destroy", "apd_last_error", "apd_assign", "apd_solve",
-                    "apd_assign_host", "apd_solve_host", "apd_last_kernel_ms", "apd_fp32_probe"]
+                    "apd_assign_host", "apd_solve_host", "apd_solve_history", "apd_last_kernel_ms", "apd_fp32_probe"]
 
 
 def make_grid(dim: int, n: Sequence[int], lo: Sequence[float], hi: Sequence[float]) -> apd_grid:
@@ -231,6 +233,16 @@ class ApdContext:
             ctypes.byref(dual), ctypes.byref(opts) if opts is not None else None)
         self._check(rc, allow=(APD_OK, APD_NOT_CONVERGED))
         return SolveInfo(rc, it.value, ev.value, err.value, dual.value)
+
+    def solve_history(self, cap: int = 8192):
+        """(dual, max_rel_err) numpy arrays, one entry per evaluation of the most recent apd_solve."""
+        import numpy as np
+        d = (ctypes.c_double * cap)()
+        e = (ctypes.c_double * cap)()
+        n = self._lib.apd_solve_history(self._h, d, e, cap)
+        if n < 0:
+            self._check(n)
+        return np.array(d[:n], dtype=np.float64), np.array(e[:n], dtype=np.float64)
 
     def last_kernel_ms(self) -> float:
         return float(self._lib.apd_last_kernel_ms(self._h))

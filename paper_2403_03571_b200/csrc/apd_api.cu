@@ -32,7 +32,7 @@ extern "C" void apd_default_opts(apd_opts* o) {
 static void free_ws(Workspace& ws) {
   cudaFree(ws.rec); cudaFree(ws.cand_list); cudaFree(ws.cand_count); cudaFree(ws.pairs_ctr);
   cudaFree(ws.seeds); cudaFree(ws.count); cudaFree(ws.idxsum); cudaFree(ws.dual_partial);
-  cudaFree(ws.sstate); cudaFree(ws.svec); cudaFree(ws.w32); cudaFree(ws.e_vol); cudaFree(ws.e_scal);
+  cudaFree(ws.sstate); cudaFree(ws.svec); cudaFree(ws.w32); cudaFree(ws.e_vol); cudaFree(ws.e_scal); cudaFree(ws.hist);
   if (ws.report) cudaFreeHost(ws.report);
   for (int i = 0; i < 2; ++i) if (ws.sev[i]) cudaEventDestroy(ws.sev[i]);
   if (ws.ev0) cudaEventDestroy(ws.ev0);

@@ -73,6 +73,8 @@ struct Workspace {
   float* w32 = nullptr;                 // [max_seeds] fl32(w) the next evaluation uses
   double* e_vol = nullptr;              // [max_seeds] evaluation outputs inside the solve loop
   double* e_scal = nullptr;             // [2] dual, max_rel_err
+  double* hist = nullptr;               // [2 * SOLVE_HIST_CAP] (dual, err) per evaluation of the last solve
+  int hist_len = 0;
   struct SolveReport* report = nullptr; // pinned, mapped host memory the step kernel writes
   cudaEvent_t sev[2] = {nullptr, nullptr};
 };
@@ -88,6 +90,7 @@ cudaError_t launch_pack_pairs(int dim, int M, int M_pad, const float* X, const f
                               const int* done_flag, cudaStream_t st);
 cudaError_t launch_assign_rowpoly(const AssignArgs& a, cudaStream_t st);
 void rowpoly_tile_extent(int dim, int row_long, int* ex, int* ey, int* ez);
+constexpr int SOLVE_HIST_CAP = 8192;    // evaluations of a solve whose (dual, err) are kept for apd_solve_history
 constexpr int CAND_CAP = 1024;         // candidate-list capacity per tile; a longer list falls back to all seeds
 cudaError_t launch_cull(const GridDev& g, int M, int M_pad, const float* X, const float* A, const float* w, float* rec,
                         int* list, int* count, int cap, unsigned long long* pairs_ctr, const int* done_flag,

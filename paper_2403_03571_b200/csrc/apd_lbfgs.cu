@@ -16,6 +16,7 @@
 #include "apd_internal.cuh"
 #include "apd_device.cuh"
 #include <cmath>
+#include <vector>
 
 namespace apd {
 
@@ -41,6 +42,8 @@ struct StepArgs {
   const double* e_scal;  // [0] dual, [1] max_rel_err
   float* w32;          // next evaluation's weights
   SolveReport* report; // mapped host memory
+  double* hist;        // [2 * hist_cap] (dual, max_rel_err) of every evaluation, in order
+  int hist_cap;
 };
 
 // Sum over the block, identical value returned to every thread; fixed order.
@@ -148,6 +151,7 @@ __global__ void __launch_bounds__(LB_THREADS) lbfgs_step_kernel(StepArgs a) {
     vsum += tv;
   }
   evals += 1;
+  if (tid == 0 && evals <= a.hist_cap) { a.hist[2 * (evals - 1)] = -f1; a.hist[2 * (evals - 1) + 1] = err1; }
   const double* w_eval = (phase == 0) ? w : wtry;
   if (err1 < best_err) {
     best_err = err1; best_dual = -f1;
@@ -281,6 +285,7 @@ static int ensure_solve_state(apd_ctx* ctx, int hist) {
     LB_TRY(cudaMalloc(&ws.w32, ms * sizeof(float)));
     LB_TRY(cudaMalloc(&ws.e_vol, ms * sizeof(double)));
     LB_TRY(cudaMalloc(&ws.e_scal, 2 * sizeof(double)));
+    LB_TRY(cudaMalloc(&ws.hist, 2 * (size_t)SOLVE_HIST_CAP * sizeof(double)));
     LB_TRY(cudaHostAlloc(&ws.report, sizeof(SolveReport), cudaHostAllocMapped));
     LB_TRY(cudaEventCreateWithFlags(&ws.sev[0], cudaEventDisableTiming));
     LB_TRY(cudaEventCreateWithFlags(&ws.sev[1], cudaEventDisableTiming));
@@ -328,6 +333,8 @@ extern "C" int apd_solve(apd_ctx* ctx, const apd_grid* grid, int32_t M, const fl
   StepArgs sa;
   sa.st = ws.sstate; sa.vec = ws.svec; sa.stride = ws.max_seeds; sa.M = M; sa.v = target_vol;
   sa.e_vol = ws.e_vol; sa.e_scal = ws.e_scal; sa.w32 = ws.w32;
+  sa.hist = ws.hist; sa.hist_cap = SOLVE_HIST_CAP;
+  ws.hist_len = 0;
   SolveReport* dev_report = nullptr;
   LB_TRY(cudaHostGetDevicePointer((void**)&dev_report, ws.report, 0));
   sa.report = dev_report;
@@ -366,9 +373,25 @@ extern "C" int apd_solve(apd_ctx* ctx, const apd_grid* grid, int32_t M, const fl
   if (w64) LB_TRY(cudaMemcpyAsync(w64, ws.svec + (size_t)V_W * ws.max_seeds, sizeof(double) * M,
                                   cudaMemcpyDeviceToDevice, st));
   LB_TRY(cudaStreamSynchronize(st));
+  ws.hist_len = ws.report->evals < SOLVE_HIST_CAP ? ws.report->evals : SOLVE_HIST_CAP;
   if (iters) *iters = ws.report->iters;
   if (evals) *evals = ws.report->evals;
   if (max_rel_err) *max_rel_err = ws.report->err;
   if (dual) *dual = ws.report->dual;
   return status;
+}
+
+extern "C" int apd_solve_history(apd_ctx* ctx, double* dual_hist, double* err_hist, int32_t cap) {
+  if (!ctx || cap < 0 || (cap > 0 && (!dual_hist || !err_hist))) return APD_E_ARG;
+  Workspace& ws = ctx->ws;
+  const int n = ws.hist_len < cap ? ws.hist_len : cap;
+  if (n <= 0 || !ws.hist) return 0;
+  std::vector<double> h(2 * (size_t)n);
+  if (cudaSetDevice(ws.device) != cudaSuccess ||
+      cudaMemcpy(h.data(), ws.hist, h.size() * sizeof(double), cudaMemcpyDeviceToHost) != cudaSuccess) {
+    ctx->err = "apd_solve_history: copy failed";
+    return APD_E_CUDA;
+  }
+  for (int k = 0; k < n; ++k) { dual_hist[k] = h[2 * k]; err_hist[k] = h[2 * k + 1]; }
+  return n;
 }

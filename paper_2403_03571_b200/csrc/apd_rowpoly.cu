@@ -170,11 +170,11 @@ struct RowSmem {
 template <int DIM, int V, int T, bool IDX>
 __device__ __forceinline__ void row_process_chunk(const float* __restrict__ sp, int ibase, const int* __restrict__ s_idx,
                                                   f2 x0, f2 yy, f2 yz, const f2 (&tt)[V], float (&best)[V],
-                                                  float4* __restrict__ s_prev4, int* __restrict__ s_lab, int tid) {
+                                                  float4* __restrict__ s_prev4, int* __restrict__ s_lab, int tid,
+                                                  int ngroups = SEED_CHUNK / ROW_GROUP) {
   constexpr int PREC = (DIM == 3) ? PREC3 : PREC2;
-  constexpr int CHUNK_PAIRS = SEED_CHUNK / 2;
   constexpr int GROUP_PAIRS = ROW_GROUP / 2;
-  for (int gidx = 0; gidx < CHUNK_PAIRS / GROUP_PAIRS; ++gidx) {
+  for (int gidx = 0; gidx < ngroups; ++gidx) {
     const float* gp = sp + gidx * GROUP_PAIRS * PREC;
 #pragma unroll ROW_UNROLL
     for (int p = 0; p < GROUP_PAIRS; ++p) {
@@ -418,8 +418,10 @@ __global__ void __launch_bounds__(G::THREADS, G::MINB) assign_rowpoly_culled_ker
   __syncthreads();
   for (int c = 0; c < nchunks; ++c) {
     if (c + 1 < nchunks) gather(c + 1);     // the other stage: every thread left it before the last barrier
+    // only the groups of ROW_GROUP seeds that hold a real candidate (the tail of the last one is padding)
+    const int ngroups = min(SEED_CHUNK / ROW_GROUP, (cnt - c * SEED_CHUNK + ROW_GROUP - 1) / ROW_GROUP);
     row_process_chunk<DIM, V, T, true>(s_seeds + (size_t)(c & 1) * CHUNK_PAIRS * PREC, 0, s_idx + (c & 1) * SEED_CHUNK,
-                                       rt.x0, rt.yy, rt.yz, tt, best, s_prev4, s_lab, tid);
+                                       rt.x0, rt.yy, rt.yz, tt, best, s_prev4, s_lab, tid, ngroups);
     __syncthreads();
   }
 
