@@ -165,8 +165,8 @@ def run_reference(args):
 # ------------------------------------------------------------------------------------------------
 # Algorithmic FP32 work per voxel-seed pair of each kernel form:
 #   DIRECT  : 3 FADD + 3 FMUL + 6 FFMA               = 18 flop   (12 FP32 instructions, 3D)
-#   ROWPOLY : 2 FMA (Horner) + 21 flop set-up per (row of 16 voxels, seed) = 4 + 21/16 = 5.3125 flop
-FLOP_PER_PAIR = {1: 18.0, 2: 4.0 + 21.0 / 16.0}
+#   ROWPOLY : 2 FMA (Horner) + 21 flop set-up per (row of 32 voxels, seed) = 4 + 21/32 = 4.65625 flop
+FLOP_PER_PAIR = {1: 18.0, 2: 4.0 + 21.0 / 32.0}
 FP32_LANES_PER_SM = 128
 # dram__bytes_read.sum + dram__bytes_write.sum of one assign_rowpoly_kernel launch on this workload, from the
 # `ncu --set full` capture summarised in profiles/ (None until a capture exists)
@@ -220,7 +220,6 @@ def run_ours(args):
     sampler.start()
     time.sleep(0.3)
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    kern_ms = []
     barrier()
     t0 = time.time()
     for i in range(args.steps):
@@ -230,7 +229,6 @@ def run_ours(args):
         ev[i][1].record()
         if i % 8 == 7 or i == args.steps - 1:
             torch.cuda.synchronize()
-        kern_ms.append(None)
     barrier()
     t1 = time.time()
     clocks = sampler.stop(t0, t1)
@@ -312,15 +310,52 @@ def run_ours(args):
                                         "peak": peak_tflops, "unit": "TFLOP/s", "frac": dach / peak_tflops,
                                         "kernel_ms": dm, "gpairs": wl.pairs / (dm * 1e-3) / 1e9, "flop_per_pair": 18.0}
         if not args.no_solve:
-            wS = torch.zeros(wl.M, dtype=torch.float32, device=dev)
-            torch.cuda.synchronize()
-            ts = time.perf_counter()
-            info = ctx.apd_solve(grid, X, A, v, wl.eps, w=wS, labels=labels, vol=vol,
-                                 opts=apd.make_opts(kernel=args.kernel, max_iters=args.solve_max_iters))
-            torch.cuda.synchronize()
-            extra["solve"] = {"workload": f"cfg{WORKLOAD_CFG} apd_solve, tol {wl.eps}", "seconds": time.perf_counter() - ts,
-                              "status": info.status, "iters": info.iters, "evals": info.evals,
-                              "max_rel_err": info.max_rel_err, "dual": info.dual}
+            pairs_t = torch.zeros(1, dtype=torch.int64, device=dev)
+            oc = apd.make_opts(kernel=args.kernel, cull=1)
+            c_ms = []
+            for _ in range(5):
+                flush.zero_()
+                e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+                e0.record()
+                ctx.apd_assign(grid, X, A, w, target_vol=v, labels=labels, vol=vol, dual=dual, max_rel_err=err,
+                               pairs_evaluated=pairs_t, opts=oc)
+                e1.record(); torch.cuda.synchronize()
+                c_ms.append(e0.elapsed_time(e1))
+            cm = float(np.mean(c_ms[2:]))
+            extra["culled_assign"] = {"workload": f"cfg{WORKLOAD_CFG}, opts.cull=1 (exact tile culling, labels identical)",
+                                      "ms_per_step": cm, "pairs_evaluated": int(pairs_t.item()),
+                                      "pruned_fraction": 1.0 - pairs_t.item() / wl.pairs,
+                                      "effective_gpairs": wl.pairs / (cm * 1e-3) / 1e9}
+
+            def solve_leg(ctx_, grid_, X_, A_, v_, wl_, labels_, vol_, cull):
+                wS = torch.zeros(wl_.M, dtype=torch.float32, device=dev)
+                torch.cuda.synchronize()
+                ts = time.perf_counter()
+                info = ctx_.apd_solve(grid_, X_, A_, v_, wl_.eps, w=wS, labels=labels_, vol=vol_,
+                                      opts=apd.make_opts(kernel=args.kernel, cull=cull, max_iters=args.solve_max_iters))
+                torch.cuda.synchronize()
+                return {"seconds": time.perf_counter() - ts, "tol": wl_.eps, "cull": cull, "status": info.status,
+                        "iters": info.iters, "evals": info.evals, "max_rel_err": info.max_rel_err, "dual": info.dual}
+
+            extra["solve"] = dict(workload=f"cfg{WORKLOAD_CFG} apd_solve", **solve_leg(ctx, grid, X, A, v, wl, labels, vol, 1))
+            extra["solve_brute_force"] = dict(workload=f"cfg{WORKLOAD_CFG} apd_solve",
+                                              **solve_leg(ctx, grid, X, A, v, wl, labels, vol, 0))
+            if not args.no_cfg5:
+                wl5 = workloads.make_config(5)
+                ctx5 = apd.ApdContext(wl5.dim, wl5.M, device=local)
+                grid5 = apd.make_grid(wl5.dim, wl5.n, wl5.lo, wl5.hi)
+                X5 = torch.from_numpy(wl5.X).to(dev); A5 = torch.from_numpy(wl5.A).to(dev)
+                v5 = torch.from_numpy(wl5.v).to(dev)
+                lab5 = torch.empty(wl5.N, dtype=torch.int32, device=dev)
+                vol5 = torch.zeros(wl5.M, dtype=torch.float64, device=dev)
+                extra["solve_cfg5"] = dict(workload=f"cfg5 apd_solve: {'x'.join(map(str, wl5.n))} voxels x {wl5.M} grains",
+                                           **solve_leg(ctx5, grid5, X5, A5, v5, wl5, lab5, vol5, 1))
+                w5 = torch.zeros(wl5.M, dtype=torch.float32, device=dev)
+                ctx5.apd_assign(grid5, X5, A5, w5, target_vol=v5, labels=lab5, vol=vol5, dual=dual, max_rel_err=err,
+                                pairs_evaluated=pairs_t, opts=oc)
+                torch.cuda.synchronize()
+                extra["solve_cfg5"]["pruned_fraction_at_w0"] = 1.0 - pairs_t.item() / wl5.pairs
+                del lab5
         cb = None
         if world == 1 and not args.no_cpu:
             cb = cpu_baseline(wl, args.cpu_seconds)
@@ -354,6 +389,7 @@ def main():
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-probe", action="store_true")
     ap.add_argument("--no-direct", action="store_true")
+    ap.add_argument("--no-cfg5", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--solve-max-iters", type=int, default=1000)
     args = ap.parse_args()
