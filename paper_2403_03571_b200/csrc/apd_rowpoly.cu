@@ -145,6 +145,7 @@ constexpr int ROW_GROUP = ROWGROUP;                 // seeds between two argmin 
 constexpr int ROW_STAGES = ROWSTAGES;                 // smem ring of seed chunks
 constexpr int ROW_BATCH = ROWBATCH;
 constexpr int ROW_UNROLL = ROWUNROLL;
+constexpr int RESCAN_W = 4;                  // flagged voxels resolved together in one argmin rescan
 
 // Dynamic shared memory of one CTA:
 //   seeds [ROW_STAGES][CHUNK_PAIRS*PREC] f32 | prev [V][THREADS] f32 | lab [V][THREADS] i32 |
@@ -170,7 +171,8 @@ struct RowSmem {
 template <int DIM, int V, int T, bool IDX>
 __device__ __forceinline__ void row_process_chunk(const float* __restrict__ sp, int ibase, const int* __restrict__ s_idx,
                                                   f2 x0, f2 yy, f2 yz, const f2 (&tt)[V], float (&best)[V],
-                                                  float4* __restrict__ s_prev4, int* __restrict__ s_lab, int tid,
+                                                  float4* __restrict__ s_prev4, int* __restrict__ s_lab,
+                                                  const float* __restrict__ s_tt, int tid,
                                                   int ngroups = SEED_CHUNK / ROW_GROUP) {
   constexpr int PREC = (DIM == 3) ? PREC3 : PREC2;
   constexpr int GROUP_PAIRS = ROW_GROUP / 2;
@@ -215,19 +217,57 @@ __device__ __forceinline__ void row_process_chunk(const float* __restrict__ sp, 
         if (best[4 * k4 + 3] < pv.w) { mask |= 8u << (4 * k4); pv.w = best[4 * k4 + 3]; }
         s_prev4[k4 * T + tid] = pv;
       }
-      for (int p = 0; p < GROUP_PAIRS && mask; ++p) {
-        const RowCoef rc = row_setup<DIM>(gp + p * PREC, x0, yy, yz);
-        const int q = gidx * ROW_GROUP + 2 * p;           // position of the pair's first seed in the chunk
-        const int i0 = IDX ? s_idx[q] : ibase + q;
-        const int i1 = IDX ? s_idx[q + 1] : ibase + q + 1;
+      // culled lists (all candidates are near: events in most groups, few voxels each): resolve RESCAN_W flagged
+      // voxels at a time: their in-row offsets come from the CTA's offset table and their
+      // new minima from prev (both shared memory), so no register array is indexed dynamically and the pair loop
+      // below is branch-light
+      if constexpr (!IDX) {
+        // brute force: events are rare (a few per cent of the groups) and early ones flag most of the row: one
+        // predicated pass over all V voxels measured fastest
+        for (int p = 0; p < GROUP_PAIRS && mask; ++p) {
+          const RowCoef rc = row_setup<DIM>(gp + p * PREC, x0, yy, yz);
+          const int q = gidx * ROW_GROUP + 2 * p;
+          const int i0 = IDX ? s_idx[q] : ibase + q;
+          const int i1 = IDX ? s_idx[q + 1] : ibase + q + 1;
 #pragma unroll
-        for (int k = 0; k < V; ++k) {
-          if (mask & (1u << k)) {
-            float lo, hi;
-            f2_unpack(row_cost(rc, tt[k]), lo, hi);
-            if (lo == best[k]) { s_lab[k * T + tid] = i0; mask &= ~(1u << k); }
-            else if (hi == best[k]) { s_lab[k * T + tid] = i1; mask &= ~(1u << k); }
+          for (int k = 0; k < V; ++k) {
+            if (mask & (1u << k)) {
+              float lo, hi;
+              f2_unpack(row_cost(rc, tt[k]), lo, hi);
+              if (lo == best[k]) { s_lab[k * T + tid] = i0; mask &= ~(1u << k); }
+              else if (hi == best[k]) { s_lab[k * T + tid] = i1; mask &= ~(1u << k); }
+            }
           }
+        }
+      } else while (mask) {
+        const float* s_prevf = reinterpret_cast<const float*>(s_prev4);
+        f2 t4[RESCAN_W];
+        float tg[RESCAN_W];
+        int kk[RESCAN_W];
+#pragma unroll
+        for (int j = 0; j < RESCAN_W; ++j) {
+          const bool on = mask != 0u;
+          kk[j] = on ? (__ffs((int)mask) - 1) : 0;
+          mask &= mask - 1u;                       // 0 stays 0
+          const float t = s_tt[kk[j]];
+          t4[j] = f2_pack(t, t);
+          tg[j] = on ? s_prevf[(((kk[j] >> 2) * T + tid) << 2) + (kk[j] & 3)] : CUDART_NAN_F;   // NaN never matches
+        }
+        for (int p = 0; p < GROUP_PAIRS; ++p) {
+          const RowCoef rc = row_setup<DIM>(gp + p * PREC, x0, yy, yz);
+          const int q = gidx * ROW_GROUP + 2 * p;           // position of the pair's first seed in the chunk
+          const int i0 = IDX ? s_idx[q] : ibase + q;
+          const int i1 = IDX ? s_idx[q + 1] : ibase + q + 1;
+          bool open = false;
+#pragma unroll
+          for (int j = 0; j < RESCAN_W; ++j) {
+            float lo, hi;
+            f2_unpack(row_cost(rc, t4[j]), lo, hi);
+            if (lo == tg[j]) { s_lab[kk[j] * T + tid] = i0; tg[j] = CUDART_NAN_F; }
+            else if (hi == tg[j]) { s_lab[kk[j] * T + tid] = i1; tg[j] = CUDART_NAN_F; }
+            open |= (tg[j] == tg[j]);
+          }
+          if (!open) break;
         }
       }
     }
@@ -318,7 +358,7 @@ __global__ void __launch_bounds__(G::THREADS, G::MINB) assign_rowpoly_kernel(con
     }
     mbar_wait(&s_full[stage], (uint32_t)((c / ROW_STAGES) & 1));
     row_process_chunk<DIM, V, T, false>(s_seeds + (size_t)stage * CHUNK_PAIRS * PREC, c * SEED_CHUNK, nullptr,
-                                        rt.x0, rt.yy, rt.yz, tt, best, s_prev4, s_lab, tid);
+                                        rt.x0, rt.yy, rt.yz, tt, best, s_prev4, s_lab, nullptr, tid);
     __syncwarp();
     if ((tid & 31) == 0) mbar_arrive(&s_empty[stage]);
   }
@@ -347,7 +387,8 @@ struct CullSmem {
   static constexpr size_t LAB_OFF = PREV_OFF + (size_t)G::V * G::THREADS * sizeof(float);
   static constexpr size_t IDX_OFF = LAB_OFF + (size_t)G::V * G::THREADS * sizeof(int);
   static constexpr size_t RED_OFF = IDX_OFF + 2 * SEED_CHUNK * sizeof(int);
-  static constexpr size_t BYTES = RED_OFF + (G::THREADS / 32) * sizeof(double);
+  static constexpr size_t TT_OFF = RED_OFF + (G::THREADS / 32) * sizeof(double);   // [TXT][V] in-row offsets
+  static constexpr size_t BYTES = TT_OFF + (size_t)G::TXT * G::V * sizeof(float);
 };
 
 template <int DIM, class G>
@@ -365,6 +406,7 @@ __global__ void __launch_bounds__(G::THREADS, G::MINB) assign_rowpoly_culled_ker
   int* s_lab = reinterpret_cast<int*>(smem_raw + S::LAB_OFF);
   int* s_idx = reinterpret_cast<int*>(smem_raw + S::IDX_OFF);
   double* s_red = reinterpret_cast<double*>(smem_raw + S::RED_OFF);
+  float* s_tt = reinterpret_cast<float*>(smem_raw + S::TT_OFF);
 
   if (a.done_flag && *a.done_flag) return;
   const int tid = threadIdx.x;
@@ -385,6 +427,7 @@ __global__ void __launch_bounds__(G::THREADS, G::MINB) assign_rowpoly_culled_ker
     tt[k] = rt.tau(a, k);
     best[k] = CUDART_INF_F;
     s_lab[k * T + tid] = 0;
+    if (tid < G::TXT) { float t, t_; f2_unpack(tt[k], t, t_); s_tt[tid * V + k] = t; }   // tid == tx for these threads
   }
 #pragma unroll
   for (int k4 = 0; k4 < V / 4; ++k4)
@@ -421,7 +464,7 @@ __global__ void __launch_bounds__(G::THREADS, G::MINB) assign_rowpoly_culled_ker
     // only the groups of ROW_GROUP seeds that hold a real candidate (the tail of the last one is padding)
     const int ngroups = min(SEED_CHUNK / ROW_GROUP, (cnt - c * SEED_CHUNK + ROW_GROUP - 1) / ROW_GROUP);
     row_process_chunk<DIM, V, T, true>(s_seeds + (size_t)(c & 1) * CHUNK_PAIRS * PREC, 0, s_idx + (c & 1) * SEED_CHUNK,
-                                       rt.x0, rt.yy, rt.yz, tt, best, s_prev4, s_lab, tid, ngroups);
+                                       rt.x0, rt.yy, rt.yz, tt, best, s_prev4, s_lab, s_tt + (tid % G::TXT) * V, tid, ngroups);
     __syncthreads();
   }
 
