@@ -134,6 +134,25 @@ int apd_solve(apd_ctx* ctx, const apd_grid* grid, int32_t M,
  * entries written (>= 0), or a negative apd_status.  Synchronous. */
 int apd_solve_history(apd_ctx* ctx, double* dual_hist, double* err_hist, int32_t cap);
 
+/* Algorithm 3, generalised Lloyd: K rounds of { Algorithm 2 from the previous weights; seeds <-
+ * discrete centroids of the cells (an empty cell keeps its seed) }, then a final Algorithm 2.
+ *   X  [M,dim] DEVICE fp32 IN/OUT: X^0 on entry, X^K on return (each round's centroids rounded to fp32)
+ *   A, target_vol, w_init, w, labels, vol: as apd_solve (w_init is W_0^0; NULL = 0); labels/vol describe the final APD
+ *   iters, evals: HOST out, totals over all K+1 solves; max_rel_err: HOST out, of the final solve
+ * A round that ends APD_NOT_CONVERGED continues from its best iterate; the return value is the final solve's status
+ * (or a negative error).  K = 0 is apd_solve.  Blocks until finished. */
+int apd_lloyd(apd_ctx* ctx, const apd_grid* grid, int32_t M, float* X, const float* A, const float* target_vol,
+              double tol, int32_t K, const float* w_init, float* w, int32_t* labels, double* vol,
+              int32_t* iters, int32_t* evals, double* max_rel_err, const apd_opts* opts, void* cuda_stream);
+
+/* Resolution rules of PAPER.md:182-197 for a cubic grid of M voxels per axis on a domain of volume |Omega|:
+ * |Omega| / M^D < factor * v_min with factor = eps (necessary: one misassigned voxel is already the tolerance; eq. 2.9
+ * when v_min = |Omega|/N) or eps / 2^D (practical, eq. 2.10).  apd_resolution_bound returns the real number M must
+ * EXCEED (Table 1 of the paper prints it rounded to the nearest integer); apd_choose_resolution the smallest integer M
+ * that satisfies the strict inequality.  Host-only, no device work.  Negative on bad arguments. */
+double  apd_resolution_bound(int32_t dim, double domain_volume, double v_min, double eps, int32_t practical);
+int32_t apd_choose_resolution(int32_t dim, double domain_volume, double v_min, double eps, int32_t practical);
+
 /* Same two calls with HOST arrays: the library allocates device buffers, copies in, runs the
  * device call above, copies the results out and frees.  Every pointer is HOST memory; NULL is
  * allowed where the device call allows it.  Synchronous. */

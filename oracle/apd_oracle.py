@@ -347,3 +347,42 @@ def oracle_solve(grid: Grid, X, A, v, eps: float, w_init=None, history: int = 10
         iters += 1
         if iters >= max_iters or evals >= max_evals:
             return finish_best(iters, evals)
+
+
+# ----------------------------------------------------------------------------------------
+# Algorithm 3, generalised Lloyd, and the resolution rules
+# ----------------------------------------------------------------------------------------
+def oracle_lloyd(grid: Grid, X0, A, v, eps: float, K: int, w_init=None, **solve_kw):
+    """K rounds of { Algorithm 2 from W_0^k ; x_i^{k+1} = discrete centroid of cell i (PAPER.md:176-178) ;
+    W_0^{k+1} = W^k }, then a final Algorithm 2 (step 8).  Seeds are fp32 inputs of every round
+    (the centroid is rounded to fp32, as the CUDA path does); an empty cell keeps its seed (reading S5); a round
+    that ends NOT_CONVERGED continues from its best iterate.  Returns (X^K fp32, final SolveResult, iters, evals)."""
+    d = grid.dim
+    X = np.ascontiguousarray(np.asarray(X0, dtype=np.float32).reshape(-1, d)).copy()
+    w0 = w_init
+    iters = evals = 0
+    for k in range(K + 1):
+        r = oracle_solve(grid, X, A, v, eps, w_init=w0, **solve_kw)
+        iters += r.iters
+        evals += r.evals
+        if k == K:
+            return X, r, iters, evals
+        c = oracle_assign(grid, X, A, r.w32, v=v, diagnostics=False).centroids
+        X = np.ascontiguousarray(c.astype(np.float32))
+        w0 = r.w32
+
+
+def resolution_bound(dim: int, domain_volume: float, v_min: float, eps: float, practical: bool) -> float:
+    """The real number M must exceed: |Omega|/M^D < eps v_min (eq. 2.9 when v_min = |Omega|/N) or
+    |Omega|/M^D < (eps/2^D) v_min (eq. 2.10, PAPER.md:195-197)."""
+    factor = eps / (2 ** dim) if practical else eps
+    return (domain_volume / (factor * v_min)) ** (1.0 / dim)
+
+
+def choose_resolution(dim: int, domain_volume: float, v_min: float, eps: float, practical: bool) -> int:
+    """Smallest integer M satisfying the strict inequality, by direct search (no closed form trusted)."""
+    factor = eps / (2 ** dim) if practical else eps
+    m = 1
+    while not (domain_volume / float(m) ** dim < factor * v_min):
+        m += 1
+    return m

@@ -78,6 +78,14 @@ def load_library() -> ctypes.CDLL:
                                    + [_P] * 5 + [ctypes.POINTER(ctypes.c_int32), ctypes.POINTER(ctypes.c_int32),
                                                  ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double),
                                                  ctypes.POINTER(apd_opts)])
+    lib.apd_lloyd.restype = ctypes.c_int
+    lib.apd_lloyd.argtypes = ([_P, ctypes.POINTER(apd_grid), ctypes.c_int32, _P, _P, _P, ctypes.c_double, ctypes.c_int32]
+                              + [_P] * 4 + [ctypes.POINTER(ctypes.c_int32), ctypes.POINTER(ctypes.c_int32),
+                                            ctypes.POINTER(ctypes.c_double), ctypes.POINTER(apd_opts), _P])
+    lib.apd_resolution_bound.restype = ctypes.c_double
+    lib.apd_resolution_bound.argtypes = [ctypes.c_int32, ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_int32]
+    lib.apd_choose_resolution.restype = ctypes.c_int32
+    lib.apd_choose_resolution.argtypes = [ctypes.c_int32, ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_int32]
     lib.apd_solve_history.restype = ctypes.c_int
     lib.apd_solve_history.argtypes = [_P, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double), ctypes.c_int32]
     lib.apd_last_kernel_ms.restype = ctypes.c_double
@@ -90,7 +98,8 @@ def load_library() -> ctypes.CDLL:
 
 
 EXPORTED_SYMBOLS = ["apd_default_opts", "apd_create", "apd_destroy", "apd_last_error", "apd_assign", "apd_solve",
-                    "apd_assign_host", "apd_solve_host", "apd_solve_history", "apd_last_kernel_ms", "apd_fp32_probe"]
+                    "apd_assign_host", "apd_solve_host", "apd_solve_history", "apd_lloyd", "apd_resolution_bound",
+                    "apd_choose_resolution", "apd_last_kernel_ms", "apd_fp32_probe"]
 
 
 def make_grid(dim: int, n: Sequence[int], lo: Sequence[float], hi: Sequence[float]) -> apd_grid:
@@ -234,6 +243,22 @@ class ApdContext:
         self._check(rc, allow=(APD_OK, APD_NOT_CONVERGED))
         return SolveInfo(rc, it.value, ev.value, err.value, dual.value)
 
+    def apd_lloyd(self, grid: apd_grid, X, A, target_vol, tol: float, K: int, w_init=None, w=None, labels=None,
+                  vol=None, opts: Optional[apd_opts] = None) -> SolveInfo:
+        """apd_lloyd of include/apd.h (Algorithm 3) on CUDA tensors; X is updated in place; blocks until finished."""
+        d = grid.dim
+        M = X.shape[0]
+        it, ev = ctypes.c_int32(0), ctypes.c_int32(0)
+        err = ctypes.c_double(0.0)
+        rc = self._lib.apd_lloyd(
+            self._h, ctypes.byref(grid), M, _dev(X, torch.float32, "X", M * d), _dev(A, torch.float32, "A", M * d * d),
+            _dev(target_vol, torch.float32, "target_vol", M), float(tol), int(K),
+            _dev(w_init, torch.float32, "w_init", M), _dev(w, torch.float32, "w", M), _dev(labels, torch.int32, "labels"),
+            _dev(vol, torch.float64, "vol", M), ctypes.byref(it), ctypes.byref(ev), ctypes.byref(err),
+            ctypes.byref(opts) if opts is not None else None, self._stream())
+        self._check(rc, allow=(APD_OK, APD_NOT_CONVERGED))
+        return SolveInfo(rc, it.value, ev.value, err.value, float("nan"))
+
     def solve_history(self, cap: int = 8192):
         """(dual, max_rel_err) numpy arrays, one entry per evaluation of the most recent apd_solve."""
         import numpy as np
@@ -246,6 +271,14 @@ class ApdContext:
 
     def last_kernel_ms(self) -> float:
         return float(self._lib.apd_last_kernel_ms(self._h))
+
+
+def apd_resolution_bound(dim: int, domain_volume: float, v_min: float, eps: float, practical: bool) -> float:
+    return float(load_library().apd_resolution_bound(dim, domain_volume, v_min, eps, int(practical)))
+
+
+def apd_choose_resolution(dim: int, domain_volume: float, v_min: float, eps: float, practical: bool) -> int:
+    return int(load_library().apd_choose_resolution(dim, domain_volume, v_min, eps, int(practical)))
 
 
 def apd_fp32_probe(variant: int, device: int = 0):

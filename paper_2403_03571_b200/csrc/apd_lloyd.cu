@@ -1,0 +1,87 @@
+// apd_lloyd.cu -- NEXT rows f1 and f2 of DESIGN.md: Algorithm 3 (generalised Lloyd) as a host loop
+// over apd_solve + the discrete centroids of the same pass, and the resolution rules of PAPER.md:182-197.
+#include "apd_internal.cuh"
+#include <cmath>
+
+namespace apd {
+
+// x_i^{k+1} = fl32(discrete centroid of cell i)  (an empty cell keeps its seed, reading S5 --
+// the finalize kernel already wrote x_i into `centroids` for it)
+__global__ void centroids_to_seeds_kernel(int n, const double* __restrict__ centroids, float* __restrict__ X) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) X[i] = (float)centroids[i];
+}
+
+}  // namespace apd
+
+using namespace apd;
+
+#define LL_TRY(call)                                                                \
+  do {                                                                              \
+    cudaError_t e__ = (call);                                                       \
+    if (e__ != cudaSuccess) {                                                       \
+      ctx->err = std::string(#call) + ": " + cudaGetErrorString(e__);               \
+      rc = APD_E_CUDA;                                                              \
+      goto done;                                                                    \
+    }                                                                               \
+  } while (0)
+
+extern "C" int apd_lloyd(apd_ctx* ctx, const apd_grid* grid, int32_t M, float* X, const float* A,
+                         const float* target_vol, double tol, int32_t K, const float* w_init, float* w,
+                         int32_t* labels, double* vol, int32_t* iters, int32_t* evals, double* max_rel_err,
+                         const apd_opts* opts, void* cuda_stream) {
+  if (!ctx) return APD_E_ARG;
+  ctx->err.clear();
+  if (K < 0) { ctx->err = "apd_lloyd: K must be >= 0"; return APD_E_ARG; }
+  if (!grid || !X || !A || !target_vol || !w || M < 1) { ctx->err = "apd_lloyd: grid, X, A, target_vol and w are required"; return APD_E_ARG; }
+  const int d = grid->dim;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  double *cen = nullptr, *v64 = nullptr, *scal = nullptr;
+  int rc = APD_OK, it_sum = 0, ev_sum = 0;
+  double err = 0.0;
+  if (cudaSetDevice(ctx->ws.device) != cudaSuccess) { ctx->err = "apd_lloyd: cudaSetDevice failed"; return APD_E_CUDA; }
+  LL_TRY(cudaMalloc(&cen, sizeof(double) * (size_t)M * d));
+  LL_TRY(cudaMalloc(&v64, sizeof(double) * (size_t)M));
+  LL_TRY(cudaMalloc(&scal, sizeof(double) * 2));
+  for (int k = 0; k <= K; ++k) {
+    // Alg. 3 step 4 / 8: Algorithm 2 from W_0^k (W_0^0 = w_init or 0, then W_0^{k+1} = W^k)
+    int it = 0, ev = 0;
+    const bool last = (k == K);
+    rc = apd_solve(ctx, grid, M, X, A, target_vol, tol, k == 0 ? w_init : w, w, last ? labels : nullptr,
+                   last ? vol : nullptr, nullptr, &it, &ev, &err, nullptr, opts, cuda_stream);
+    it_sum += it; ev_sum += ev;
+    if (rc < 0) goto done;
+    if (last) break;
+    // Alg. 3 step 5: seeds <- discrete centroids of the APD just found (one more evaluation, with index sums)
+    rc = apd_assign(ctx, grid, M, X, A, w, target_vol, nullptr, v64, scal, scal + 1, cen, nullptr, opts, cuda_stream);
+    if (rc < 0) goto done;
+    centroids_to_seeds_kernel<<<(M * d + 255) / 256, 256, 0, st>>>(M * d, cen, X);
+    LL_TRY(cudaGetLastError());
+  }
+  LL_TRY(cudaStreamSynchronize(st));
+done:
+  cudaFree(cen); cudaFree(v64); cudaFree(scal);
+  if (iters) *iters = it_sum;
+  if (evals) *evals = ev_sum;
+  if (max_rel_err) *max_rel_err = err;
+  return rc;
+}
+
+// PAPER.md:182-197.  Smallest integer M (voxels per axis of a cubic grid on a domain of volume |Omega|) with
+//   |Omega| / M^D < factor * v_min,   factor = eps (necessary, eq. 2.9 for general v) or eps / 2^D (practical, eq. 2.10).
+extern "C" double apd_resolution_bound(int32_t dim, double domain_volume, double v_min, double eps, int32_t practical) {
+  if ((dim != 2 && dim != 3) || !(domain_volume > 0.0) || !(v_min > 0.0) || !(eps > 0.0)) return -1.0;
+  const double factor = practical ? eps / std::pow(2.0, (double)dim) : eps;
+  return std::pow(domain_volume / (factor * v_min), 1.0 / (double)dim);   // M must be GREATER than this
+}
+
+extern "C" int32_t apd_choose_resolution(int32_t dim, double domain_volume, double v_min, double eps, int32_t practical) {
+  const double b = apd_resolution_bound(dim, domain_volume, v_min, eps, practical);
+  if (!(b >= 0.0) || b > 2.0e9) return -1;
+  long long m = (long long)std::floor(b) + 1;                              // first integer strictly above the bound
+  // guard the strict inequality against the rounding of pow()
+  const double factor = practical ? eps / std::pow(2.0, (double)dim) : eps;
+  while (m > 1 && domain_volume / std::pow((double)(m - 1), (double)dim) < factor * v_min) --m;
+  while (!(domain_volume / std::pow((double)m, (double)dim) < factor * v_min)) ++m;
+  return (int32_t)m;
+}

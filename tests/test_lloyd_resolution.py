@@ -1,0 +1,132 @@
+"""NEXT rows f1/f2: Algorithm 3 and the resolution rules.
+CPU part pins the oracle (Table 1 as printed; lattice fixed point; centroid step); GPU part is parity."""
+import os
+
+import numpy as np
+import pytest
+
+from paper_2403_03571_b200 import workloads
+from oracle.apd_oracle import (Grid, OK, choose_resolution, oracle_assign, oracle_lloyd, oracle_solve,
+                               resolution_bound)
+
+GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "paper_table1.txt")
+
+
+def table1():
+    rows = [l.split() for l in open(GOLDEN) if l.strip() and not l.startswith("#")]
+    return [(int(a), int(b), int(c)) for a, b, c in rows]
+
+
+def test_P16_table1_as_printed():
+    """(N/eps)^(1/D) rounded to the nearest integer reproduces all 18 printed values (eq. 2.9 with v_i = 1/N)."""
+    rows = table1()
+    assert len(rows) == 18
+    for D, N, M in rows:
+        assert int(np.floor(resolution_bound(D, 1.0, 1.0 / N, 0.01, practical=False) + 0.5)) == M
+
+
+def test_choose_resolution_is_the_strict_inequality():
+    for D, N, _ in table1():
+        for practical in (False, True):
+            m = choose_resolution(D, 1.0, 1.0 / N, 0.01, practical)
+            f = 0.01 / 2 ** D if practical else 0.01
+            rhs = f * (1.0 / N)      # the same double expression as the rule's right-hand side (exact ties exist:
+            assert 1.0 / m ** D < rhs and not (1.0 / (m - 1) ** D < rhs)      # 1/500^2 vs 0.01/2500)
+    # "choosing M equal to two times the value given by (2.9)" == eq. (2.10)  (Table 1 caption)
+    assert abs(resolution_bound(3, 1.0, 1e-4, 0.01, True) - 2 * resolution_bound(3, 1.0, 1e-4, 0.01, False)) < 1e-9
+
+
+def lattice(k, n, d):
+    g = (np.arange(k) + 0.5) / k
+    X = np.stack(np.meshgrid(*([g] * d), indexing="ij"), -1).reshape(-1, d).astype(np.float32)
+    M = X.shape[0]
+    A = np.tile(np.eye(d, dtype=np.float32), (M, 1, 1))
+    return workloads.Workload("lattice", d, (n,) * d, (0.0,) * d, (1.0,) * d, X, A,
+                              np.full(M, 1.0 / M, np.float32), np.zeros(M, np.float32))
+
+
+def test_lloyd_lattice_is_a_fixed_point():
+    """Seeds on a regular lattice, A = I, equal targets: every cell is a box centred at its seed, so the centroid
+    step leaves X unchanged and every solve stops at iters = 0."""
+    wl = lattice(4, 32, 2)
+    X, r, iters, evals = oracle_lloyd(Grid(2, wl.n, wl.lo, wl.hi), wl.X, wl.A, wl.v, 0.01, K=3)
+    assert np.array_equal(X, wl.X) and r.status == OK and iters == 0 and evals == 4
+
+
+def test_lloyd_centroid_step_and_warm_start():
+    """One round by hand: X^1 = fl32(centroids of the optimal APD of X^0), W_0^1 = W^0; Lloyd
+    moves seeds towards their cells' centroids, so seed-to-centroid distances shrink from round to round."""
+    wl = workloads.make_config(1)
+    grid = Grid(2, wl.n, wl.lo, wl.hi)
+    r0 = oracle_solve(grid, wl.X, wl.A, wl.v, 0.01)
+    c0 = oracle_assign(grid, wl.X, wl.A, r0.w32, v=wl.v).centroids
+    X1, r1, _, _ = oracle_lloyd(grid, wl.X, wl.A, wl.v, 0.01, K=1)
+    assert np.array_equal(X1, c0.astype(np.float32))
+    r1_by_hand = oracle_solve(grid, X1, wl.A, wl.v, 0.01, w_init=r0.w32)
+    assert np.array_equal(r1.w32, r1_by_hand.w32) and r1.status == OK
+    X4, r4, _, _ = oracle_lloyd(grid, wl.X, wl.A, wl.v, 0.01, K=4)
+    c4 = oracle_assign(grid, X4, wl.A, r4.w32, v=wl.v).centroids
+    assert np.abs(c4 - X4).max() < np.abs(c0 - wl.X).max()
+
+
+# ------------------------------------------------------------------------------------------------ GPU
+@pytest.fixture(scope="module")
+def apd():
+    from paper_2403_03571_b200 import binding
+    binding.load_library()
+    return binding
+
+
+def test_resolution_helpers_match_oracle():
+    """Host-only entry points of the C ABI (no device work): callable without a GPU."""
+    from paper_2403_03571_b200 import binding
+    for D, N, M in table1():
+        b = binding.apd_resolution_bound(D, 1.0, 1.0 / N, 0.01, False)
+        assert int(np.floor(b + 0.5)) == M
+        for practical in (False, True):
+            assert binding.apd_choose_resolution(D, 1.0, 1.0 / N, 0.01, practical) == \
+                choose_resolution(D, 1.0, 1.0 / N, 0.01, practical)
+    assert binding.apd_choose_resolution(4, 1.0, 0.1, 0.01, False) == -1
+
+
+def run_lloyd(apd, wl, eps, K, cull=0):
+    import torch
+    dev = torch.device("cuda:0")
+    ctx = apd.ApdContext(wl.dim, wl.M)
+    grid = apd.make_grid(wl.dim, wl.n, wl.lo, wl.hi)
+    X = torch.from_numpy(wl.X.copy()).to(dev); A = torch.from_numpy(wl.A).to(dev); v = torch.from_numpy(wl.v).to(dev)
+    w = torch.zeros(wl.M, dtype=torch.float32, device=dev)
+    labels = torch.full((wl.N,), -1, dtype=torch.int32, device=dev)
+    vol = torch.zeros(wl.M, dtype=torch.float64, device=dev)
+    info = ctx.apd_lloyd(grid, X, A, v, eps, K, w=w, labels=labels, vol=vol, opts=apd.make_opts(cull=cull))
+    return info, X.cpu().numpy(), w.cpu().numpy(), labels.cpu().numpy(), vol.cpu().numpy()
+
+
+@pytest.mark.gpu
+def test_gpu_lloyd_lattice_fixed_point(apd):
+    wl = lattice(4, 32, 3)
+    info, X, w, labels, vol = run_lloyd(apd, wl, 0.01, K=2)
+    assert info.status == 0 and info.iters == 0 and info.evals == 3
+    assert np.array_equal(X, wl.X) and np.all(w == 0)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("cfg,n,M,eps,cull", [(1, None, None, 0.01, 0), (2, (256, 256), 60, 0.01, 1),
+                                              (3, (64, 64, 64), 80, 0.02, 1)])
+def test_gpu_lloyd_parity(apd, cfg, n, M, eps, cull):
+    """K = 2 rounds against oracle_lloyd.  The two optimisers agree to ~1e-3 in w (parity rule 5), which moves a
+    handful of boundary voxels, so the seeds after two centroid steps agree to a small fraction of a voxel; the
+    post-condition is judged by the oracle at the GPU's (X, w)."""
+    wl = workloads.make_config(cfg, n=n, M=M)
+    grid = Grid(wl.dim, wl.n, wl.lo, wl.hi)
+    Xo, ro, it_o, ev_o = oracle_lloyd(grid, wl.X, wl.A, wl.v, eps, K=2)
+    info, X, w, labels, vol = run_lloyd(apd, wl, eps, K=2, cull=cull)
+    assert info.status == ro.status == OK
+    h = 1.0 / max(wl.n)
+    assert np.abs(X - Xo).max() <= 0.25 * h, f"seeds differ by {np.abs(X - Xo).max() / h:.3f} voxels"
+    chk = oracle_assign(grid, X, wl.A, w, v=wl.v)
+    nm = int((labels != chk.labels).sum())
+    assert nm < max(1e-5 * wl.N, 1) or nm == 0
+    assert chk.err <= eps + 2 * nm * grid.voxel_volume / float(wl.v.min())
+    assert abs(info.evals - ev_o) <= max(6, ev_o // 3)
+    print(f"cfg{cfg}: gpu evals {info.evals} vs oracle {ev_o}; max seed diff {np.abs(X - Xo).max() / h:.4f} voxels")
