@@ -97,6 +97,23 @@ class ClockSampler:
                 "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def max_over_ranks(x: float, world: int, device) -> float:
+    """Replicas-only multi-GPU rule: every rank times its own replica, the job's time is the
+    MAX over ranks.  `device` is where the one-element tensor lives (cuda:<local> under NCCL, cpu under gloo)."""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(pairs_per_rank: int, world: int, ms_per_step: float) -> float:
+    """Whole-job G pairs/s: all ranks' pairs over the max-over-ranks time of a step."""
+    return world * pairs_per_rank / (ms_per_step * 1e-3) / 1e9
+
+
 def measured_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -139,7 +156,7 @@ def run_reference(args):
     if int(os.environ.get("RANK", "0")) != 0:
         return
     wl = workloads.make_config(WORKLOAD_CFG)
-    per_step_s = max(2.0, min(20.0, 150.0 / max(1, args.steps + args.warmup)))
+    per_step_s = args.ref_seconds if args.ref_seconds > 0 else max(2.0, min(20.0, 150.0 / max(1, args.steps + args.warmup)))
     for _ in range(args.warmup):
         oracle_sample_rate(wl, per_step_s)
     t_pairs, t_s, cores, nvox = 0.0, 0.0, 0, 0
@@ -242,12 +259,9 @@ def run_ours(args):
         k_ms.append(ctx.last_kernel_ms())
     kernel_ms = float(np.mean(k_ms))
 
-    if world > 1:
-        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks(total_ms, world, dev)
     ms_per_step = total_ms / args.steps
-    value = world * wl.pairs / (ms_per_step * 1e-3) / 1e9
+    value = aggregate_value(wl.pairs, world, ms_per_step)
 
     # ---- e2e: the same evaluation through the HOST-buffer C-ABI call (pinned host tensors; H2D of the inputs,
     #      D2H of labels + volumes + dual inside the timed region) ----
@@ -263,10 +277,7 @@ def run_ours(args):
         ctx.apd_assign_host(grid, hX, hA, hw, target_vol=hv, labels=hlab, vol=hvol, opts=opts)
     torch.cuda.synchronize()
     e2e_s = (time.perf_counter() - te) / e2e_steps
-    if world > 1:
-        t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s = max_over_ranks(e2e_s, world, dev)
     h2d = 4 * (hX.numel() + hA.numel() + hw.numel() + hv.numel())
     d2h = 4 * hlab.numel() + 8 * hvol.numel() + 16 + 8
 
@@ -392,6 +403,7 @@ def main():
     ap.add_argument("--no-cfg5", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--solve-max-iters", type=int, default=1000)
+    ap.add_argument("--ref-seconds", type=float, default=0.0, help="--impl reference: CPU seconds per step (0 = auto)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
