@@ -30,7 +30,8 @@ extern "C" void apd_default_opts(apd_opts* o) {
 }
 
 static void free_ws(Workspace& ws) {
-  cudaFree(ws.rec); cudaFree(ws.cand_list); cudaFree(ws.cand_count); cudaFree(ws.pairs_ctr);
+  cudaFree(ws.rec); cudaFree(ws.brick_list); cudaFree(ws.brick_count); cudaFree(ws.super_list);
+  cudaFree(ws.super_count); cudaFree(ws.pairs_ctr);
   cudaFree(ws.seeds); cudaFree(ws.count); cudaFree(ws.idxsum); cudaFree(ws.dual_partial);
   cudaFree(ws.sstate); cudaFree(ws.svec); cudaFree(ws.w32); cudaFree(ws.e_vol); cudaFree(ws.e_scal); cudaFree(ws.hist);
   if (ws.report) cudaFreeHost(ws.report);
@@ -90,7 +91,7 @@ extern "C" const char* apd_last_error(const apd_ctx* ctx) {
 namespace apd {
 
 // Validates the grid and fills the device-side description.  Returns "" or an error text.
-std::string make_grid(const apd_ctx* ctx, const apd_grid* grid, int kernel, GridDev* g) {
+std::string make_grid(const apd_ctx* ctx, const apd_grid* grid, int kernel, bool cull, GridDev* g) {
   if (!grid) return "grid is NULL";
   if (grid->dim != ctx->ws.dim) return "grid.dim differs from the context's dim";
   const int d = grid->dim;
@@ -113,7 +114,7 @@ std::string make_grid(const apd_ctx* ctx, const apd_grid* grid, int kernel, Grid
   }
   out.nx = n[0]; out.ny = n[1]; out.nz = n[2];
   out.voxel_volume = P;
-  out.row_long = assign_tile_counts(kernel, d, out.nx, out.ny, out.nz, ctx->ws.sm_count, &out.tiles_x, &out.tiles_y,
+  out.row_long = assign_tile_counts(kernel, d, out.nx, out.ny, out.nz, ctx->ws.sm_count, cull, &out.tiles_x, &out.tiles_y,
                                     &out.tiles_z);
   *g = out;
   return "";
@@ -137,12 +138,13 @@ int enqueue_evaluation(apd_ctx* ctx, const GridDev& g, int kernel, int M, const 
   Workspace& ws = ctx->ws;
   const int M_pad = (M + SEED_CHUNK - 1) / SEED_CHUNK * SEED_CHUNK;
   const int n_tiles = g.tiles_x * g.tiles_y * g.tiles_z;
-  if ((size_t)n_tiles > ws.partial_cap) {
+  const int n_partials = cull ? 4 * n_tiles : n_tiles;      // the culled kernel writes one partial per brick (warp)
+  if ((size_t)n_partials > ws.partial_cap) {
     // grow the per-tile partial buffer (stream-ordered free/alloc keeps earlier work valid)
     APD_CUDA_TRY(ctx, cudaStreamSynchronize(st));
     APD_CUDA_TRY(ctx, cudaFree(ws.dual_partial));
     ws.dual_partial = nullptr;
-    ws.partial_cap = (size_t)n_tiles;
+    ws.partial_cap = (size_t)n_partials;
     APD_CUDA_TRY(ctx, cudaMalloc(&ws.dual_partial, ws.partial_cap * sizeof(double)));
   }
   if (kernel == APD_KERNEL_ROWPOLY)
@@ -154,32 +156,39 @@ int enqueue_evaluation(apd_ctx* ctx, const GridDev& g, int kernel, int M, const 
   AssignArgs a;
   a.g = g; a.M = M; a.M_pad = M_pad; a.seeds = ws.seeds; a.labels = labels; a.count = ws.count;
   a.idxsum = centroids ? ws.idxsum : nullptr; a.dual_partial = ws.dual_partial;
-  a.rec = nullptr; a.cand_list = nullptr; a.cand_count = nullptr; a.cand_cap = 0; a.pairs_ctr = nullptr;
+  a.rec = nullptr; a.brick_list = nullptr; a.brick_count = nullptr; a.super_list = nullptr; a.super_count = nullptr;
+  a.super_x = a.super_y = 0; a.pairs_ctr = nullptr;
   a.done_flag = done_flag;
   if (cull) {
-    // a7: per-tile candidate lists, rebuilt every evaluation (the bounds depend on w)
+    // a7: two-level candidate lists, rebuilt every evaluation (the bounds depend on w)
+    int nsx, nsy, nsz;
+    cull_super_counts(g, &nsx, &nsy, &nsz);
+    const size_t n_super = (size_t)nsx * nsy * nsz, n_bricks = (size_t)n_tiles * 4;
     if (!ws.rec) {
       const size_t m_pad_max = ((size_t)ws.max_seeds + SEED_CHUNK - 1) / SEED_CHUNK * SEED_CHUNK;
       APD_CUDA_TRY(ctx, cudaMalloc(&ws.rec, m_pad_max * rec_floats(ws.dim) * sizeof(float)));
       APD_CUDA_TRY(ctx, cudaMalloc(&ws.pairs_ctr, sizeof(unsigned long long)));
     }
-    if ((size_t)n_tiles > ws.cand_tiles_cap) {
+    if (n_bricks > ws.brick_cap_n || n_super > ws.super_cap_n) {
       APD_CUDA_TRY(ctx, cudaStreamSynchronize(st));
-      cudaFree(ws.cand_list); cudaFree(ws.cand_count);
-      ws.cand_list = nullptr; ws.cand_count = nullptr; ws.cand_tiles_cap = 0;
-      APD_CUDA_TRY(ctx, cudaMalloc(&ws.cand_list, (size_t)n_tiles * CAND_CAP * sizeof(int)));
-      APD_CUDA_TRY(ctx, cudaMalloc(&ws.cand_count, (size_t)n_tiles * sizeof(int)));
-      ws.cand_tiles_cap = (size_t)n_tiles;
+      cudaFree(ws.brick_list); cudaFree(ws.brick_count); cudaFree(ws.super_list); cudaFree(ws.super_count);
+      ws.brick_list = ws.brick_count = ws.super_list = ws.super_count = nullptr;
+      ws.brick_cap_n = ws.super_cap_n = 0;
+      APD_CUDA_TRY(ctx, cudaMalloc(&ws.brick_list, n_bricks * BRICK_CAP * sizeof(int)));
+      APD_CUDA_TRY(ctx, cudaMalloc(&ws.brick_count, n_bricks * sizeof(int)));
+      APD_CUDA_TRY(ctx, cudaMalloc(&ws.super_list, n_super * SUPER_CAP * sizeof(int)));
+      APD_CUDA_TRY(ctx, cudaMalloc(&ws.super_count, n_super * sizeof(int)));
+      ws.brick_cap_n = n_bricks; ws.super_cap_n = n_super;
     }
-    APD_CUDA_TRY(ctx, launch_cull(g, M, M_pad, X, A, w, ws.rec, ws.cand_list, ws.cand_count, CAND_CAP, ws.pairs_ctr,
-                                  done_flag, st));
-    a.rec = ws.rec; a.cand_list = ws.cand_list; a.cand_count = ws.cand_count; a.cand_cap = CAND_CAP;
-    a.pairs_ctr = ws.pairs_ctr;
+    CullBuffers cb{ws.rec, ws.brick_list, ws.brick_count, ws.super_list, ws.super_count, ws.pairs_ctr};
+    APD_CUDA_TRY(ctx, launch_cull(g, M, M_pad, X, A, w, cb, nsx, nsy, nsz, done_flag, st));
+    a.rec = ws.rec; a.brick_list = ws.brick_list; a.brick_count = ws.brick_count; a.super_list = ws.super_list;
+    a.super_count = ws.super_count; a.super_x = nsx; a.super_y = nsy; a.pairs_ctr = ws.pairs_ctr;
   }
   if (timed) APD_CUDA_TRY(ctx, cudaEventRecord(ws.ev0, st));
   APD_CUDA_TRY(ctx, launch_assign(kernel, a, st));
   if (timed) { APD_CUDA_TRY(ctx, cudaEventRecord(ws.ev1, st)); ws.timed = true; }
-  APD_CUDA_TRY(ctx, launch_finalize(g, M, n_tiles, ws.count, a.idxsum, ws.dual_partial, X, w, target_vol, vol,
+  APD_CUDA_TRY(ctx, launch_finalize(g, M, n_partials, ws.count, a.idxsum, ws.dual_partial, X, w, target_vol, vol,
                                     dual, max_rel_err, centroids, pairs, cull ? ws.pairs_ctr : nullptr, done_flag, st));
   return APD_OK;
 }
@@ -198,7 +207,7 @@ extern "C" int apd_assign(apd_ctx* ctx, const apd_grid* grid, int32_t M, const f
   if (M < 1 || M > ctx->ws.max_seeds) { ctx->err = "apd_assign: M out of range [1, max_seeds]"; return APD_E_ARG; }
   if (!X || !A || !w || !vol || !dual) { ctx->err = "apd_assign: X, A, w, vol and dual are required"; return APD_E_ARG; }
   GridDev g;
-  e = make_grid(ctx, grid, kernel, &g);
+  e = make_grid(ctx, grid, kernel, opts && opts->cull, &g);
   if (!e.empty()) { ctx->err = "apd_assign: " + e; return APD_E_ARG; }
   APD_CUDA_TRY(ctx, cudaSetDevice(ctx->ws.device));
   return enqueue_evaluation(ctx, g, kernel, M, X, A, w, target_vol, labels, vol, dual, max_rel_err, centroids,

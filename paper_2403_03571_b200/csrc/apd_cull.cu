@@ -10,6 +10,10 @@
 // All bounds are taken in fp32 with a relative slack of 2^-16 on every term, three orders above the rounding of the
 // fp32 cost evaluation, so rounding can never prune a winner (test: labels with culling == labels without, bit-exact).
 // A must be positive definite for the bound to hold (PAPER.md:51-54 assumes it; the library does not check).
+// Two levels keep the bound pass O(M) per SUPER-TILE instead of per tile: level 1 builds a parent list for every
+// super-tile (64 x 32 x 32 voxels) from all seeds; level 2 builds the list of every BRICK (the 16 x 4 x 8 voxels one
+// warp of the culled kernel owns) from its parent's list.  A pruned seed loses everywhere in its box, and a brick lies
+// inside its super-tile, so a seed missing from the parent list cannot win in the brick either.
 #include "apd_internal.cuh"
 #include "apd_device.cuh"
 #include <math_constants.h>
@@ -19,16 +23,33 @@ namespace apd {
 constexpr float CULL_EPS = 1.0f / 65536.0f;
 constexpr int CULL_THREADS = 256;
 
-// Per-seed record table in the DIRECT layout (apd_internal.cuh) plus rho_i in the first spare slot.
+// max over the corners (+-hx, +-hy[, +-hz]) of |h|_A: the diagonal part plus the largest of the sign patterns of
+// the off-diagonal part (r = packed record: a_kl' are the doubled off-diagonals)
+template <int DIM>
+__device__ __forceinline__ float box_radius(const float* r, float hx, float hy, float hz) {
+  float q;
+  if (DIM == 3) {
+    const float dg = r[3] * hx * hx + r[6] * hy * hy + r[8] * hz * hz;
+    const float p12 = r[4] * hx * hy, p13 = r[5] * hx * hz, p23 = r[7] * hy * hz;
+    q = dg + fmaxf(fmaxf(p12 + p13 + p23, p12 - p13 - p23), fmaxf(-p12 + p13 - p23, -p12 - p13 + p23));
+  } else {
+    q = r[2] * hx * hx + r[4] * hy * hy + fabsf(r[3] * hx * hy);
+  }
+  return sqrtf(fmaxf(q, 0.0f)) * (1.0f + 4.0f * CULL_EPS);
+}
+
+// Per-seed record table in the DIRECT layout (apd_internal.cuh) plus rho_i of a brick and of a super-tile in the
+// two spare slots.  hb = half-extents of the box of voxel centres of a brick, hs = of a super-tile.
 template <int DIM>
 __global__ void cull_pack_kernel(int M, int M_pad, const float* __restrict__ X, const float* __restrict__ A,
-                                 const float* __restrict__ w, float hx, float hy, float hz, float* __restrict__ rec,
+                                 const float* __restrict__ w, float3 hb, float3 hs, float* __restrict__ rec,
                                  unsigned long long* __restrict__ pairs_ctr, const int* __restrict__ done_flag) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (done_flag && *done_flag) return;
   if (i == 0) *pairs_ctr = 0ull;
   if (i >= M_pad) return;
   constexpr int REC = (DIM == 3) ? REC3 : REC2;
+  constexpr int NP = (DIM == 3) ? 10 : 6;
   float r[REC];
 #pragma unroll
   for (int k = 0; k < REC; ++k) r[k] = 0.0f;
@@ -38,22 +59,16 @@ __global__ void cull_pack_kernel(int M, int M_pad, const float* __restrict__ X, 
       r[0] = X[i * 3 + 0]; r[1] = X[i * 3 + 1]; r[2] = X[i * 3 + 2];
       r[3] = a[0]; r[4] = a[1] + a[3]; r[5] = a[2] + a[6]; r[6] = a[4]; r[7] = a[5] + a[7]; r[8] = a[8];
       r[9] = -w[i];
-      // max over the box corners (+-hx, +-hy, +-hz) of h^T A h: the diagonal part plus the largest of the four
-      // sign patterns of the off-diagonal part
-      const float dg = r[3] * hx * hx + r[6] * hy * hy + r[8] * hz * hz;
-      const float p12 = r[4] * hx * hy, p13 = r[5] * hx * hz, p23 = r[7] * hy * hz;
-      const float off = fmaxf(fmaxf(p12 + p13 + p23, p12 - p13 - p23), fmaxf(-p12 + p13 - p23, -p12 - p13 + p23));
-      r[10] = sqrtf(fmaxf(dg + off, 0.0f)) * (1.0f + 4.0f * CULL_EPS);
     } else {
       const float* a = A + (size_t)i * 4;
       r[0] = X[i * 2 + 0]; r[1] = X[i * 2 + 1];
       r[2] = a[0]; r[3] = a[1] + a[2]; r[4] = a[3];
       r[5] = -w[i];
-      const float dg = r[2] * hx * hx + r[4] * hy * hy;
-      r[6] = sqrtf(fmaxf(dg + fabsf(r[3] * hx * hy), 0.0f)) * (1.0f + 4.0f * CULL_EPS);
     }
+    r[NP] = box_radius<DIM>(r, hb.x, hb.y, hb.z);
+    r[NP + 1] = box_radius<DIM>(r, hs.x, hs.y, hs.z);
   } else {
-    r[(DIM == 3) ? 9 : 5] = CUDART_INF_F;
+    r[NP - 1] = CUDART_INF_F;
   }
   float4* dst = reinterpret_cast<float4*>(rec + (size_t)i * REC);
 #pragma unroll
@@ -61,20 +76,23 @@ __global__ void cull_pack_kernel(int M, int M_pad, const float* __restrict__ X, 
 }
 
 struct CullArgs {
-  GridDev g;
-  int ex, ey, ez;        // tile extents in voxels
+  GridDev g;               // tiles_* = CTA tiles of the culled kernel
   int M;
   const float* rec;
-  int* list;             // [n_tiles, cap]
-  int* count;            // [n_tiles]
-  int cap;
+  int* super_list;         // [n_super, SUPER_CAP]
+  int* super_count;        // [n_super]
+  int nsx, nsy, nsz;       // super-tiles per axis
+  int* brick_list;         // [n_tiles * 4, BRICK_CAP]
+  int* brick_count;        // [n_tiles * 4]
+  float3 ht;               // half-extents of the box of voxel centres of a CTA tile
   const int* done_flag;
 };
 
-// s_i = |y0 - x_i|_{A_i}, rho_i and -w_i of one seed
-template <int DIM>
+// s_i = |y0 - x_i|_{A_i}, rho_i (SLOT 0 = brick, 1 = super-tile: stored; 2 = box of half-extents ht: computed) and
+// -w_i of one seed
+template <int DIM, int SLOT>
 __device__ __forceinline__ void seed_bounds(const float* __restrict__ rec, int i, float y0x, float y0y, float y0z,
-                                            float* s, float* rho, float* nw) {
+                                            float* s, float* rho, float* nw, float3 ht = make_float3(0.f, 0.f, 0.f)) {
   if (DIM == 3) {
     const float4* p = reinterpret_cast<const float4*>(rec + (size_t)i * REC3);
     const float4 p0 = __ldg(p), p1 = __ldg(p + 1), p2 = __ldg(p + 2);
@@ -82,14 +100,26 @@ __device__ __forceinline__ void seed_bounds(const float* __restrict__ rec, int i
     float q = dx * fmaf(p1.y, dz, fmaf(p1.x, dy, p0.w * dx));
     q = fmaf(dy, fmaf(p1.w, dz, p1.z * dy), q);
     q = fmaf(dz, p2.x * dz, q);
-    *s = sqrtf(fmaxf(q, 0.0f)); *rho = p2.z; *nw = p2.y;
+    *s = sqrtf(fmaxf(q, 0.0f)); *nw = p2.y;
+    if (SLOT == 2) {
+      const float r[9] = {0.f, 0.f, 0.f, p0.w, p1.x, p1.y, p1.z, p1.w, p2.x};
+      *rho = box_radius<3>(r, ht.x, ht.y, ht.z);
+    } else {
+      *rho = SLOT ? p2.w : p2.z;
+    }
   } else {
     const float4* p = reinterpret_cast<const float4*>(rec + (size_t)i * REC2);
     const float4 p0 = __ldg(p), p1 = __ldg(p + 1);
     const float dx = y0x - p0.x, dy = y0y - p0.y;
     float q = dx * fmaf(p0.w, dy, p0.z * dx);
     q = fmaf(dy, p1.x * dy, q);
-    *s = sqrtf(fmaxf(q, 0.0f)); *rho = p1.z; *nw = p1.y;
+    *s = sqrtf(fmaxf(q, 0.0f)); *nw = p1.y;
+    if (SLOT == 2) {
+      const float r[5] = {0.f, 0.f, p0.z, p0.w, p1.x};
+      *rho = box_radius<2>(r, ht.x, ht.y, 0.0f);
+    } else {
+      *rho = SLOT ? p1.w : p1.z;
+    }
   }
 }
 
@@ -102,25 +132,33 @@ __device__ __forceinline__ float lower_bound(float s, float rho, float nw) {
   return r * r * (1.0f - CULL_EPS) + nw - CULL_EPS * fabsf(nw);
 }
 
-// One CTA per tile: pass 1 U_T = min_k upper bound, pass 2 ordered compaction of {i : lower bound_i <= U_T}.
+// centre, along one axis, of the box spanned by the centres of voxels i0 .. i0+e-1
+__device__ __forceinline__ float box_centre(double lo, double s, int i0, int e) {
+  return (float)(lo + ((double)i0 + 0.5 * (double)(e - 1) + 0.5) * s);
+}
+
+// LEVEL 1 -- one CTA per super-tile over ALL seeds: pass 1 U = min_k upper bound, pass 2 ordered compaction of
+// {i : lower bound_i <= U} into the super-tile's parent list.
 template <int DIM>
-__global__ void __launch_bounds__(CULL_THREADS) cull_tiles_kernel(const CullArgs c) {
+__global__ void __launch_bounds__(CULL_THREADS) cull_super_kernel(const CullArgs c) {
   __shared__ float s_min[CULL_THREADS / 32];
   __shared__ int s_wsum[CULL_THREADS / 32];
   __shared__ float s_U;
   if (c.done_flag && *c.done_flag) return;
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   const int b = blockIdx.x;
-  const int bx = b % c.g.tiles_x, by = (b / c.g.tiles_x) % c.g.tiles_y, bz = b / (c.g.tiles_x * c.g.tiles_y);
-  // centre of the box spanned by the tile's voxel centres
-  const float y0x = (float)(c.g.lo[0] + ((double)(bx * c.ex) + 0.5 * (double)(c.ex - 1) + 0.5) * c.g.s[0]);
-  const float y0y = (float)(c.g.lo[1] + ((double)(by * c.ey) + 0.5 * (double)(c.ey - 1) + 0.5) * c.g.s[1]);
-  const float y0z = (DIM == 3) ? (float)(c.g.lo[2] + ((double)(bz * c.ez) + 0.5 * (double)(c.ez - 1) + 0.5) * c.g.s[2]) : 0.0f;
+  const int sx = b % c.nsx, sy = (b / c.nsx) % c.nsy, sz = b / (c.nsx * c.nsy);
+  constexpr int EX = (DIM == 3) ? SUPER3_TX * CULL_TILE3_X : SUPER2_TX * CULL_TILE2_X;
+  constexpr int EY = (DIM == 3) ? SUPER3_TY * CULL_TILE3_Y : SUPER2_TY * CULL_TILE2_Y;
+  constexpr int EZ = (DIM == 3) ? SUPER3_TZ * CULL_TILE3_Z : 1;
+  const float y0x = box_centre(c.g.lo[0], c.g.s[0], sx * EX, EX);
+  const float y0y = box_centre(c.g.lo[1], c.g.s[1], sy * EY, EY);
+  const float y0z = (DIM == 3) ? box_centre(c.g.lo[2], c.g.s[2], sz * EZ, EZ) : 0.0f;
 
   float umin = CUDART_INF_F;
   for (int i = tid; i < c.M; i += CULL_THREADS) {
     float s, rho, nw;
-    seed_bounds<DIM>(c.rec, i, y0x, y0y, y0z, &s, &rho, &nw);
+    seed_bounds<DIM, 1>(c.rec, i, y0x, y0y, y0z, &s, &rho, &nw);
     umin = fminf(umin, upper_bound(s, rho, nw));
   }
 #pragma unroll
@@ -136,14 +174,14 @@ __global__ void __launch_bounds__(CULL_THREADS) cull_tiles_kernel(const CullArgs
   __syncthreads();
   const float U = s_U;
 
-  int* list = c.list + (size_t)b * c.cap;
+  int* list = c.super_list + (size_t)b * SUPER_CAP;
   int base = 0;
   for (int i0 = 0; i0 < c.M; i0 += CULL_THREADS) {
     const int i = i0 + tid;
     bool keep = false;
     if (i < c.M) {
       float s, rho, nw;
-      seed_bounds<DIM>(c.rec, i, y0x, y0y, y0z, &s, &rho, &nw);
+      seed_bounds<DIM, 1>(c.rec, i, y0x, y0y, y0z, &s, &rho, &nw);
       keep = !(lower_bound(s, rho, nw) > U);       // NaN keeps the seed
     }
     const unsigned int bal = __ballot_sync(0xffffffffu, keep);
@@ -154,32 +192,163 @@ __global__ void __launch_bounds__(CULL_THREADS) cull_tiles_kernel(const CullArgs
     for (int k = 0; k < CULL_THREADS / 32; ++k) { const int n = s_wsum[k]; if (k < wid) off += n; tot += n; }
     if (keep) {
       const int pos = off + __popc(bal & ((1u << lane) - 1u));
-      if (pos < c.cap) list[pos] = i;
+      if (pos < SUPER_CAP) list[pos] = i;
     }
     base += tot;
     __syncthreads();
   }
-  if (tid == 0) c.count[b] = (base <= c.cap) ? base : -1;
+  if (tid == 0) c.super_count[b] = (base <= SUPER_CAP) ? base : -1;
 }
 
-cudaError_t launch_cull(const GridDev& g, int M, int M_pad, const float* X, const float* A, const float* w, float* rec,
-                        int* list, int* count, int cap, unsigned long long* pairs_ctr, const int* done_flag,
-                        cudaStream_t st) {
-  int ex, ey, ez;
-  rowpoly_tile_extent(g.dim, g.row_long, &ex, &ey, &ez);
-  const float hx = (float)(0.5 * (double)(ex - 1) * g.s[0]), hy = (float)(0.5 * (double)(ey - 1) * g.s[1]),
-              hz = (g.dim == 3) ? (float)(0.5 * (double)(ez - 1) * g.s[2]) : 0.0f;
+// LEVEL 2 -- one CTA per CTA tile of the culled kernel.  (a) The 4 warps together cut the super-tile's parent list
+// (all seeds if that overflowed) down to the seeds that can win somewhere in the CTA TILE, kept in shared memory;
+// (b) each warp then cuts that list down to its own brick.  Same two passes (U = min upper bound, ordered
+// compaction of lower bound <= U) at both steps.
+constexpr int TILE_CAP = 768;
+template <int DIM>
+__global__ void __launch_bounds__(128) cull_bricks_kernel(const CullArgs c) {
+  __shared__ int s_tile[TILE_CAP];
+  __shared__ float s_min[4];
+  __shared__ int s_wsum[4];
+  if (c.done_flag && *c.done_flag) return;
+  const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+  const int b = blockIdx.x;
+  const int bx = b % c.g.tiles_x, by = (b / c.g.tiles_x) % c.g.tiles_y, bz = b / (c.g.tiles_x * c.g.tiles_y);
+  constexpr int TX = (DIM == 3) ? CULL_TILE3_X : CULL_TILE2_X, TY = (DIM == 3) ? CULL_TILE3_Y : CULL_TILE2_Y,
+                TZ = (DIM == 3) ? CULL_TILE3_Z : 1;
+  constexpr int STX = (DIM == 3) ? SUPER3_TX : SUPER2_TX, STY = (DIM == 3) ? SUPER3_TY : SUPER2_TY,
+                STZ = (DIM == 3) ? SUPER3_TZ : 1;
+  const int sup = ((bz / STZ) * c.nsy + by / STY) * c.nsx + bx / STX;
+  int n = c.super_count[sup];
+  const int* plist = c.super_list + (size_t)sup * SUPER_CAP;
+  if (n < 0) { n = c.M; plist = nullptr; }
+
+  // (a) CTA-tile list
+  {
+    const float t0x = box_centre(c.g.lo[0], c.g.s[0], bx * TX, TX);
+    const float t0y = box_centre(c.g.lo[1], c.g.s[1], by * TY, TY);
+    const float t0z = (DIM == 3) ? box_centre(c.g.lo[2], c.g.s[2], bz * TZ, TZ) : 0.0f;
+    float umin = CUDART_INF_F;
+    for (int pos = tid; pos < n; pos += 128) {
+      const int i = plist ? __ldg(plist + pos) : pos;
+      float s, rho, nw;
+      seed_bounds<DIM, 2>(c.rec, i, t0x, t0y, t0z, &s, &rho, &nw, c.ht);
+      umin = fminf(umin, upper_bound(s, rho, nw));
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) umin = fminf(umin, __shfl_xor_sync(0xffffffffu, umin, o));
+    if (lane == 0) s_min[w] = umin;
+    __syncthreads();
+    const float U = fminf(fminf(s_min[0], s_min[1]), fminf(s_min[2], s_min[3]));
+    int base = 0;
+    for (int p0 = 0; p0 < n; p0 += 128) {
+      const int pos = p0 + tid;
+      bool keep = false;
+      int i = 0;
+      if (pos < n) {
+        i = plist ? __ldg(plist + pos) : pos;
+        float s, rho, nw;
+        seed_bounds<DIM, 2>(c.rec, i, t0x, t0y, t0z, &s, &rho, &nw, c.ht);
+        keep = !(lower_bound(s, rho, nw) > U);
+      }
+      const unsigned int bal = __ballot_sync(0xffffffffu, keep);
+      __syncthreads();                       // s_wsum of the previous round has been read
+      if (lane == 0) s_wsum[w] = __popc(bal);
+      __syncthreads();
+      int off = base, tot = 0;
+#pragma unroll
+      for (int k = 0; k < 4; ++k) { const int m = s_wsum[k]; if (k < w) off += m; tot += m; }
+      if (keep) {
+        const int q = off + __popc(bal & ((1u << lane) - 1u));
+        if (q < TILE_CAP) s_tile[q] = i;
+      }
+      base += tot;
+    }
+    __syncthreads();
+    if (base <= TILE_CAP) { n = base; plist = s_tile; }      // else: the bricks cut the parent list directly
+  }
+  const bool from_smem = (plist == s_tile);
+  auto cand = [&](int pos) { return from_smem ? s_tile[pos] : (plist ? __ldg(plist + pos) : pos); };
+
+  // (b) brick lists
+  int ox, oy, oz, ex, ey, ez;
+  brick_box(DIM, w, &ox, &oy, &oz, &ex, &ey, &ez);
+  const float y0x = box_centre(c.g.lo[0], c.g.s[0], bx * TX + ox, ex);
+  const float y0y = box_centre(c.g.lo[1], c.g.s[1], by * TY + oy, ey);
+  const float y0z = (DIM == 3) ? box_centre(c.g.lo[2], c.g.s[2], bz * TZ + oz, ez) : 0.0f;
+
+  float umin = CUDART_INF_F;
+  for (int pos = lane; pos < n; pos += 32) {
+    float s, rho, nw;
+    seed_bounds<DIM, 0>(c.rec, cand(pos), y0x, y0y, y0z, &s, &rho, &nw);
+    umin = fminf(umin, upper_bound(s, rho, nw));
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) umin = fminf(umin, __shfl_xor_sync(0xffffffffu, umin, o));
+  const float U = umin;
+
+  const size_t brick = (size_t)b * 4 + w;
+  int* list = c.brick_list + brick * BRICK_CAP;
+  int base = 0;
+  for (int p0 = 0; p0 < n; p0 += 32) {
+    const int pos = p0 + lane;
+    bool keep = false;
+    int i = 0;
+    if (pos < n) {
+      i = cand(pos);
+      float s, rho, nw;
+      seed_bounds<DIM, 0>(c.rec, i, y0x, y0y, y0z, &s, &rho, &nw);
+      keep = !(lower_bound(s, rho, nw) > U);
+    }
+    const unsigned int bal = __ballot_sync(0xffffffffu, keep);
+    if (keep) {
+      const int q = base + __popc(bal & ((1u << lane) - 1u));
+      if (q < BRICK_CAP) list[q] = i;
+    }
+    base += __popc(bal);
+  }
+  if (lane == 0) c.brick_count[brick] = (base <= BRICK_CAP) ? base : -1;
+}
+
+void cull_super_counts(const GridDev& g, int* nsx, int* nsy, int* nsz) {
+  if (g.dim == 3) {
+    *nsx = (g.tiles_x + SUPER3_TX - 1) / SUPER3_TX; *nsy = (g.tiles_y + SUPER3_TY - 1) / SUPER3_TY;
+    *nsz = (g.tiles_z + SUPER3_TZ - 1) / SUPER3_TZ;
+  } else {
+    *nsx = (g.tiles_x + SUPER2_TX - 1) / SUPER2_TX; *nsy = (g.tiles_y + SUPER2_TY - 1) / SUPER2_TY; *nsz = 1;
+  }
+}
+
+cudaError_t launch_cull(const GridDev& g, int M, int M_pad, const float* X, const float* A, const float* w,
+                        const CullBuffers& cb, int nsx, int nsy, int nsz, const int* done_flag, cudaStream_t st) {
+  // half-extents of the boxes of voxel CENTRES of a brick and of a super-tile
+  int ox, oy, oz, ex, ey, ez;
+  brick_box(g.dim, 0, &ox, &oy, &oz, &ex, &ey, &ez);
+  const int sex = (g.dim == 3) ? SUPER3_TX * CULL_TILE3_X : SUPER2_TX * CULL_TILE2_X;
+  const int sey = (g.dim == 3) ? SUPER3_TY * CULL_TILE3_Y : SUPER2_TY * CULL_TILE2_Y;
+  const int sez = (g.dim == 3) ? SUPER3_TZ * CULL_TILE3_Z : 1;
+  auto half = [&](int e, int k) { return (float)(0.5 * (double)(e - 1) * g.s[k]); };
+  const float3 hb = make_float3(half(ex, 0), half(ey, 1), g.dim == 3 ? half(ez, 2) : 0.0f);
+  const float3 hs = make_float3(half(sex, 0), half(sey, 1), g.dim == 3 ? half(sez, 2) : 0.0f);
   const int nb = (M_pad + 127) / 128;
-  if (g.dim == 3) cull_pack_kernel<3><<<nb, 128, 0, st>>>(M, M_pad, X, A, w, hx, hy, hz, rec, pairs_ctr, done_flag);
-  else            cull_pack_kernel<2><<<nb, 128, 0, st>>>(M, M_pad, X, A, w, hx, hy, hz, rec, pairs_ctr, done_flag);
+  if (g.dim == 3) cull_pack_kernel<3><<<nb, 128, 0, st>>>(M, M_pad, X, A, w, hb, hs, cb.rec, cb.pairs_ctr, done_flag);
+  else            cull_pack_kernel<2><<<nb, 128, 0, st>>>(M, M_pad, X, A, w, hb, hs, cb.rec, cb.pairs_ctr, done_flag);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
   CullArgs c;
-  c.g = g; c.ex = ex; c.ey = ey; c.ez = ez; c.M = M; c.rec = rec; c.list = list; c.count = count; c.cap = cap;
+  c.g = g; c.M = M; c.rec = cb.rec; c.super_list = cb.super_list; c.super_count = cb.super_count;
+  c.nsx = nsx; c.nsy = nsy; c.nsz = nsz; c.brick_list = cb.brick_list; c.brick_count = cb.brick_count;
   c.done_flag = done_flag;
+  c.ht = make_float3(half(g.dim == 3 ? CULL_TILE3_X : CULL_TILE2_X, 0), half(g.dim == 3 ? CULL_TILE3_Y : CULL_TILE2_Y, 1),
+                     g.dim == 3 ? half(CULL_TILE3_Z, 2) : 0.0f);
+  const int n_super = nsx * nsy * nsz;
   const int n_tiles = g.tiles_x * g.tiles_y * g.tiles_z;
-  if (g.dim == 3) cull_tiles_kernel<3><<<n_tiles, CULL_THREADS, 0, st>>>(c);
-  else            cull_tiles_kernel<2><<<n_tiles, CULL_THREADS, 0, st>>>(c);
+  if (g.dim == 3) cull_super_kernel<3><<<n_super, CULL_THREADS, 0, st>>>(c);
+  else            cull_super_kernel<2><<<n_super, CULL_THREADS, 0, st>>>(c);
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  if (g.dim == 3) cull_bricks_kernel<3><<<n_tiles, 128, 0, st>>>(c);
+  else            cull_bricks_kernel<2><<<n_tiles, 128, 0, st>>>(c);
   return cudaGetLastError();
 }
 

@@ -42,11 +42,16 @@ struct AssignArgs {
   unsigned int* count;   // [M] voxels per cell (exact integers: eq. 2.8)
   unsigned long long* idxsum;  // [M,3] sum of voxel indices per axis, or nullptr
   double* dual_partial;  // [n_tiles] sum over the tile of min_i C_ij
-  // tile culling (a7); all nullptr / 0 for brute force
-  const float* rec;      // [M_pad, REC] per-seed records (DIRECT layout)
-  const int* cand_list;  // [n_tiles, cand_cap] ascending seed indices per tile
-  const int* cand_count; // [n_tiles] list length, or -1: list overflowed, scan all seeds
-  int cand_cap;
+  // culling (a7); all nullptr / 0 for brute force.  Two levels: SUPER-TILES (groups of CTA tiles) hold a parent
+  // candidate list each; every BRICK (the voxels of one warp, 4 per CTA tile) holds its own list, a subset of its
+  // parent's.  Lists are ascending in seed index.  count < 0 = the list overflowed its capacity: fall back one
+  // level (brick -> parent -> all seeds).
+  const float* rec;        // [M_pad, REC] per-seed records (DIRECT layout) + rho_brick, rho_super
+  const int* brick_list;   // [n_tiles * 4, BRICK_CAP]
+  const int* brick_count;  // [n_tiles * 4]
+  const int* super_list;   // [n_super, SUPER_CAP]
+  const int* super_count;  // [n_super]
+  int super_x, super_y;    // super-tiles per axis (x, y); super-tile of CTA tile (bx,by,bz) = (bx/SUPER_TX, ...)
   unsigned long long* pairs_ctr;  // [1] voxel-seed pairs evaluated
   const int* done_flag;  // solve loop only: kernels return at once when *done_flag != 0; else nullptr
 };
@@ -58,11 +63,14 @@ struct Workspace {
   unsigned long long* idxsum = nullptr;  // [max_seeds,3]
   double* dual_partial = nullptr;      // [partial_cap]
   size_t partial_cap = 0;
-  // tile culling (apd_cull.cu), allocated on first use
-  float* rec = nullptr;                // [M_pad, REC] per-seed records + rho
-  int* cand_list = nullptr;            // [cand_tiles_cap * CAND_CAP]
-  int* cand_count = nullptr;           // [cand_tiles_cap]
-  size_t cand_tiles_cap = 0;
+  // culling (apd_cull.cu), allocated on first use
+  float* rec = nullptr;                // [M_pad, REC] per-seed records + rho_brick, rho_super
+  int* brick_list = nullptr;           // [brick_cap_n * BRICK_CAP]
+  int* brick_count = nullptr;          // [brick_cap_n]
+  size_t brick_cap_n = 0;
+  int* super_list = nullptr;           // [super_cap_n * SUPER_CAP]
+  int* super_count = nullptr;          // [super_cap_n]
+  size_t super_cap_n = 0;
   unsigned long long* pairs_ctr = nullptr;
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
   bool timed = false;
@@ -89,14 +97,36 @@ cudaError_t launch_pack_pairs(int dim, int M, int M_pad, const float* X, const f
                               float* seeds, unsigned int* count, unsigned long long* idxsum,
                               const int* done_flag, cudaStream_t st);
 cudaError_t launch_assign_rowpoly(const AssignArgs& a, cudaStream_t st);
-void rowpoly_tile_extent(int dim, int row_long, int* ex, int* ey, int* ez);
-constexpr int SOLVE_HIST_CAP = 8192;    // evaluations of a solve whose (dual, err) are kept for apd_solve_history
-constexpr int CAND_CAP = 1024;         // candidate-list capacity per tile; a longer list falls back to all seeds
-cudaError_t launch_cull(const GridDev& g, int M, int M_pad, const float* X, const float* A, const float* w, float* rec,
-                        int* list, int* count, int cap, unsigned long long* pairs_ctr, const int* done_flag,
+// ---- culling geometry (a7) --------------------------------------------------------------------------------
+// The culled kernel always runs the SHORT-row geometry: CTA tile 16 x 16 x 8 voxels (3D) / 32 x 64 pixels (2D),
+// 128 threads = 4 warps, each warp owning one BRICK of 32 rows of 16 voxels:
+//   3D: brick w = x [0,16) x y [4w, 4w+4) x z [0,8)      lane -> (y = lane & 3, z = lane >> 2)
+//   2D: brick w = x [16 (w&1), +16) x y [32 (w>>1), +32)   lane -> y
+// A SUPER-TILE is SUPER_T{X,Y,Z} CTA tiles per axis: 64 x 32 x 32 voxels (3D) / 128 x 128 pixels (2D).
+constexpr int CULL_TILE3_X = 16, CULL_TILE3_Y = 16, CULL_TILE3_Z = 8;
+constexpr int CULL_TILE2_X = 32, CULL_TILE2_Y = 64;
+constexpr int SUPER3_TX = 4, SUPER3_TY = 2, SUPER3_TZ = 4;
+constexpr int SUPER2_TX = 4, SUPER2_TY = 2;
+constexpr int BRICK_CAP = 256;         // candidate-list capacity of a brick
+constexpr int SUPER_CAP = 4096;        // candidate-list capacity of a super-tile
+constexpr int SOLVE_HIST_CAP = 8192;   // evaluations of a solve whose (dual, err) are kept for apd_solve_history
+
+// origin (relative to the CTA tile) and extent, in voxels, of brick w
+__host__ __device__ inline void brick_box(int dim, int w, int* ox, int* oy, int* oz, int* ex, int* ey, int* ez) {
+  if (dim == 3) { *ox = 0; *oy = 4 * w; *oz = 0; *ex = 16; *ey = 4; *ez = 8; }
+  else          { *ox = 16 * (w & 1); *oy = 32 * (w >> 1); *oz = 0; *ex = 16; *ey = 32; *ez = 1; }
+}
+
+struct CullBuffers {
+  float* rec; int* brick_list; int* brick_count; int* super_list; int* super_count;
+  unsigned long long* pairs_ctr;
+};
+cudaError_t launch_cull(const GridDev& g, int M, int M_pad, const float* X, const float* A, const float* w,
+                        const CullBuffers& cb, int n_super_x, int n_super_y, int n_super_z, const int* done_flag,
                         cudaStream_t st);
-int rowpoly_tile_counts(int dim, int nx, int ny, int nz, int sm_count, int* tx, int* ty, int* tz);
-int assign_tile_counts(int kernel, int dim, int nx, int ny, int nz, int sm_count, int* tx, int* ty, int* tz);
+void cull_super_counts(const GridDev& g, int* nsx, int* nsy, int* nsz);
+int rowpoly_tile_counts(int dim, int nx, int ny, int nz, int sm_count, bool cull, int* tx, int* ty, int* tz);
+int assign_tile_counts(int kernel, int dim, int nx, int ny, int nz, int sm_count, bool cull, int* tx, int* ty, int* tz);
 cudaError_t launch_finalize(const GridDev& g, int M, int n_partials, const unsigned int* count,
                             const unsigned long long* idxsum, const double* dual_partial,
                             const float* X, const float* w, const float* target_vol,
@@ -113,7 +143,7 @@ struct SolveReport {
 };
 
 // host helpers shared by apd_api.cu and apd_lbfgs.cu
-std::string make_grid(const apd_ctx* ctx, const apd_grid* grid, int kernel, GridDev* g);
+std::string make_grid(const apd_ctx* ctx, const apd_grid* grid, int kernel, bool cull, GridDev* g);
 int resolve_kernel(const apd_opts* o, std::string* err);
 int enqueue_evaluation(apd_ctx* ctx, const GridDev& g, int kernel, int M, const float* X, const float* A,
                        const float* w, const float* target_vol, int32_t* labels, double* vol, double* dual,

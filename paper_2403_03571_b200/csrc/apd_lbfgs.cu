@@ -317,7 +317,7 @@ extern "C" int apd_solve(apd_ctx* ctx, const apd_grid* grid, int32_t M, const fl
   if (o.max_iters < 1 || o.max_evals < 0) { ctx->err = "apd_solve: max_iters >= 1 and max_evals >= 0 required"; return APD_E_ARG; }
   const int max_evals = o.max_evals ? o.max_evals : (o.max_iters > (1 << 26) ? (1 << 30) : 20 * o.max_iters);
   GridDev g;
-  e = make_grid(ctx, grid, kernel, &g);
+  e = make_grid(ctx, grid, kernel, o.cull != 0, &g);
   if (!e.empty()) { ctx->err = "apd_solve: " + e; return APD_E_ARG; }
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   LB_TRY(cudaSetDevice(ctx->ws.device));

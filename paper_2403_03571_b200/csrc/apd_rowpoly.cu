@@ -145,7 +145,6 @@ constexpr int ROW_GROUP = ROWGROUP;                 // seeds between two argmin 
 constexpr int ROW_STAGES = ROWSTAGES;                 // smem ring of seed chunks
 constexpr int ROW_BATCH = ROWBATCH;
 constexpr int ROW_UNROLL = ROWUNROLL;
-constexpr int RESCAN_W = 4;                  // flagged voxels resolved together in one argmin rescan
 
 // Dynamic shared memory of one CTA:
 //   seeds [ROW_STAGES][CHUNK_PAIRS*PREC] f32 | prev [V][THREADS] f32 | lab [V][THREADS] i32 |
@@ -165,18 +164,15 @@ struct RowSmem {
   static constexpr size_t BYTES = RED_OFF + (G::THREADS / 32) * sizeof(double);
 };
 
-// One staged chunk of SEED_CHUNK seeds (pair-interleaved records at `sp`) against the thread's row: rows a3 + a4.
-// IDX = false: the chunk holds seeds ibase .. ibase+SEED_CHUNK-1 in index order (brute force);
-// IDX = true : the seed index of position q of the chunk is s_idx[q] (tile-culled candidate list, ascending).
-template <int DIM, int V, int T, bool IDX>
-__device__ __forceinline__ void row_process_chunk(const float* __restrict__ sp, int ibase, const int* __restrict__ s_idx,
-                                                  f2 x0, f2 yy, f2 yz, const f2 (&tt)[V], float (&best)[V],
-                                                  float4* __restrict__ s_prev4, int* __restrict__ s_lab,
-                                                  const float* __restrict__ s_tt, int tid,
-                                                  int ngroups = SEED_CHUNK / ROW_GROUP) {
+// One staged chunk of SEED_CHUNK seeds ibase .. ibase+SEED_CHUNK-1 (pair-interleaved records at `sp`) against the
+// thread's row: rows a3 + a4 of the brute-force kernel.
+template <int DIM, int V, int T>
+__device__ __forceinline__ void row_process_chunk(const float* __restrict__ sp, int ibase, f2 x0, f2 yy, f2 yz,
+                                                  const f2 (&tt)[V], float (&best)[V], float4* __restrict__ s_prev4,
+                                                  int* __restrict__ s_lab, int tid) {
   constexpr int PREC = (DIM == 3) ? PREC3 : PREC2;
   constexpr int GROUP_PAIRS = ROW_GROUP / 2;
-  for (int gidx = 0; gidx < ngroups; ++gidx) {
+  for (int gidx = 0; gidx < SEED_CHUNK / ROW_GROUP; ++gidx) {
     const float* gp = sp + gidx * GROUP_PAIRS * PREC;
 #pragma unroll ROW_UNROLL
     for (int p = 0; p < GROUP_PAIRS; ++p) {
@@ -205,8 +201,9 @@ __device__ __forceinline__ void row_process_chunk(const float* __restrict__ sp, 
       any |= (best[4 * k4] < pv.x) | (best[4 * k4 + 1] < pv.y) | (best[4 * k4 + 2] < pv.z) | (best[4 * k4 + 3] < pv.w);
     }
     if (any) {
-      // a4, deferred: the new minimum of every flagged voxel lies in this group; recompute the
-      // group with the same instructions and take the first seed that attains it
+      // a4, deferred: the new minimum of every flagged voxel lies in this group; recompute the group with the same
+      // instructions and take the first seed that attains it.  Events are rare (a few per cent of the groups) and
+      // the early ones flag most of the row: one predicated pass over all V voxels measured fastest.
       unsigned int mask = 0u;
 #pragma unroll
       for (int k4 = 0; k4 < V / 4; ++k4) {
@@ -217,57 +214,17 @@ __device__ __forceinline__ void row_process_chunk(const float* __restrict__ sp, 
         if (best[4 * k4 + 3] < pv.w) { mask |= 8u << (4 * k4); pv.w = best[4 * k4 + 3]; }
         s_prev4[k4 * T + tid] = pv;
       }
-      // culled lists (all candidates are near: events in most groups, few voxels each): resolve RESCAN_W flagged
-      // voxels at a time: their in-row offsets come from the CTA's offset table and their
-      // new minima from prev (both shared memory), so no register array is indexed dynamically and the pair loop
-      // below is branch-light
-      if constexpr (!IDX) {
-        // brute force: events are rare (a few per cent of the groups) and early ones flag most of the row: one
-        // predicated pass over all V voxels measured fastest
-        for (int p = 0; p < GROUP_PAIRS && mask; ++p) {
-          const RowCoef rc = row_setup<DIM>(gp + p * PREC, x0, yy, yz);
-          const int q = gidx * ROW_GROUP + 2 * p;
-          const int i0 = IDX ? s_idx[q] : ibase + q;
-          const int i1 = IDX ? s_idx[q + 1] : ibase + q + 1;
+      for (int p = 0; p < GROUP_PAIRS && mask; ++p) {
+        const RowCoef rc = row_setup<DIM>(gp + p * PREC, x0, yy, yz);
+        const int i0 = ibase + gidx * ROW_GROUP + 2 * p;
 #pragma unroll
-          for (int k = 0; k < V; ++k) {
-            if (mask & (1u << k)) {
-              float lo, hi;
-              f2_unpack(row_cost(rc, tt[k]), lo, hi);
-              if (lo == best[k]) { s_lab[k * T + tid] = i0; mask &= ~(1u << k); }
-              else if (hi == best[k]) { s_lab[k * T + tid] = i1; mask &= ~(1u << k); }
-            }
-          }
-        }
-      } else while (mask) {
-        const float* s_prevf = reinterpret_cast<const float*>(s_prev4);
-        f2 t4[RESCAN_W];
-        float tg[RESCAN_W];
-        int kk[RESCAN_W];
-#pragma unroll
-        for (int j = 0; j < RESCAN_W; ++j) {
-          const bool on = mask != 0u;
-          kk[j] = on ? (__ffs((int)mask) - 1) : 0;
-          mask &= mask - 1u;                       // 0 stays 0
-          const float t = s_tt[kk[j]];
-          t4[j] = f2_pack(t, t);
-          tg[j] = on ? s_prevf[(((kk[j] >> 2) * T + tid) << 2) + (kk[j] & 3)] : CUDART_NAN_F;   // NaN never matches
-        }
-        for (int p = 0; p < GROUP_PAIRS; ++p) {
-          const RowCoef rc = row_setup<DIM>(gp + p * PREC, x0, yy, yz);
-          const int q = gidx * ROW_GROUP + 2 * p;           // position of the pair's first seed in the chunk
-          const int i0 = IDX ? s_idx[q] : ibase + q;
-          const int i1 = IDX ? s_idx[q + 1] : ibase + q + 1;
-          bool open = false;
-#pragma unroll
-          for (int j = 0; j < RESCAN_W; ++j) {
+        for (int k = 0; k < V; ++k) {
+          if (mask & (1u << k)) {
             float lo, hi;
-            f2_unpack(row_cost(rc, t4[j]), lo, hi);
-            if (lo == tg[j]) { s_lab[kk[j] * T + tid] = i0; tg[j] = CUDART_NAN_F; }
-            else if (hi == tg[j]) { s_lab[kk[j] * T + tid] = i1; tg[j] = CUDART_NAN_F; }
-            open |= (tg[j] == tg[j]);
+            f2_unpack(row_cost(rc, tt[k]), lo, hi);
+            if (lo == best[k]) { s_lab[k * T + tid] = i0; mask &= ~(1u << k); }
+            else if (hi == best[k]) { s_lab[k * T + tid] = i0 + 1; mask &= ~(1u << k); }
           }
-          if (!open) break;
         }
       }
     }
@@ -283,6 +240,9 @@ struct RowThread {
   __device__ __forceinline__ void init(const AssignArgs& a, int b, int tid) {
     const int tx = tid % G::TXT, ty = (tid / G::TXT) % G::TYT, tz = tid / (G::TXT * G::TYT);
     const int bx = b % a.g.tiles_x, by = (b / a.g.tiles_x) % a.g.tiles_y, bz = b / (a.g.tiles_x * a.g.tiles_y);
+    init_at(a, bx, by, bz, tx, ty, tz);
+  }
+  __device__ __forceinline__ void init_at(const AssignArgs& a, int bx, int by, int bz, int tx, int ty, int tz) {
     ix0 = (bx * G::TXT + tx) * G::V; iy = by * G::TYT + ty; iz = bz * G::TZT + tz;
     row_valid = (ix0 < a.g.nx) && (iy < a.g.ny) && (iz < a.g.nz);
     // coordinates from the thread index (fp64 definition rounded once to fp32)
@@ -357,8 +317,8 @@ __global__ void __launch_bounds__(G::THREADS, G::MINB) assign_rowpoly_kernel(con
                    a.seeds + (size_t)(c + ROW_STAGES - 1) * CHUNK_PAIRS * PREC, CHUNK_BYTES, &s_full[s2]);
     }
     mbar_wait(&s_full[stage], (uint32_t)((c / ROW_STAGES) & 1));
-    row_process_chunk<DIM, V, T, false>(s_seeds + (size_t)stage * CHUNK_PAIRS * PREC, c * SEED_CHUNK, nullptr,
-                                        rt.x0, rt.yy, rt.yz, tt, best, s_prev4, s_lab, nullptr, tid);
+    row_process_chunk<DIM, V, T>(s_seeds + (size_t)stage * CHUNK_PAIRS * PREC, c * SEED_CHUNK, rt.x0, rt.yy, rt.yz, tt,
+                                 best, s_prev4, s_lab, tid);
     __syncwarp();
     if ((tid & 31) == 0) mbar_arrive(&s_empty[stage]);
   }
@@ -372,74 +332,65 @@ __global__ void __launch_bounds__(G::THREADS, G::MINB) assign_rowpoly_kernel(con
 }
 
 // ------------------------------------------------------------------------------------------------------------
-// a7: the same reduction over a tile's CANDIDATE LIST (apd_cull.cu) instead of all seeds.  The list is ascending
-// in seed index, so "first seed attaining the minimum" is still the lowest index (reading S1).  Candidates are
-// gathered from the per-seed record table into the pair-interleaved smem layout by the CTA's own threads (one
-// candidate per thread and chunk).  A tile whose list overflowed (count < 0) scans all seeds.
-// smem: seeds [2][CHUNK_PAIRS*PREC] | prev | lab | idx [2][SEED_CHUNK] | red
+// a7: the same reduction over CANDIDATE LISTS (apd_cull.cu) instead of all seeds.  Every warp owns one brick of
+// 32 rows x 16 voxels and walks ITS OWN list (a few dozen seeds) in chunks of 32 candidates: the lanes gather one
+// candidate each from the per-seed record table into the warp's pair-interleaved staging buffer, __syncwarp, then the
+// same row polynomial.  With lists this short every seed is a likely winner, so the argmin is tracked INLINE
+// (min3, one compare for "dropped", one for "which lane") instead of by deferred rescans; labels stay in registers.
+// Lists are ascending in seed index and the compare is strict, so ties still go to the lowest index (reading S1).
+// The four warps of a CTA never synchronise: each writes its own dual partial.
+// smem: per warp 2 stages x (16 pair records + 32 indices)
 // ------------------------------------------------------------------------------------------------------------
-template <int DIM, class G>
-struct CullSmem {
-  static constexpr int PREC = (DIM == 3) ? PREC3 : PREC2;
-  static constexpr int CHUNK_PAIRS = SEED_CHUNK / 2;
-  static constexpr size_t SEED_BYTES = (size_t)2 * CHUNK_PAIRS * PREC * sizeof(float);
-  static constexpr size_t PREV_OFF = SEED_BYTES;
-  static constexpr size_t LAB_OFF = PREV_OFF + (size_t)G::V * G::THREADS * sizeof(float);
-  static constexpr size_t IDX_OFF = LAB_OFF + (size_t)G::V * G::THREADS * sizeof(int);
-  static constexpr size_t RED_OFF = IDX_OFF + 2 * SEED_CHUNK * sizeof(int);
-  static constexpr size_t TT_OFF = RED_OFF + (G::THREADS / 32) * sizeof(double);   // [TXT][V] in-row offsets
-  static constexpr size_t BYTES = TT_OFF + (size_t)G::TXT * G::V * sizeof(float);
-};
+constexpr int WCHUNK = 32;                      // candidates per warp-chunk
+template <int DIM> struct CullGeom;
+template <> struct CullGeom<3> { static constexpr int V = 16, TXT = 1, TYT = CULL_TILE3_Y, TZT = CULL_TILE3_Z, THREADS = 128; };
+template <> struct CullGeom<2> { static constexpr int V = 16, TXT = 2, TYT = CULL_TILE2_Y, TZT = 1, THREADS = 128; };
+static_assert(CullGeom<3>::TXT * CullGeom<3>::V == CULL_TILE3_X && CullGeom<2>::TXT * CullGeom<2>::V == CULL_TILE2_X, "tile");
 
-template <int DIM, class G>
-__global__ void __launch_bounds__(G::THREADS, G::MINB) assign_rowpoly_culled_kernel(const AssignArgs a) {
-  constexpr int V = G::V, T = G::THREADS;
-  using S = CullSmem<DIM, G>;
-  constexpr int PREC = S::PREC;
-  constexpr int CHUNK_PAIRS = S::CHUNK_PAIRS;
+template <int DIM>
+__global__ void __launch_bounds__(128, 4) assign_rowpoly_culled_kernel(const AssignArgs a) {
+  using G = CullGeom<DIM>;
+  constexpr int V = G::V;
+  constexpr int PREC = (DIM == 3) ? PREC3 : PREC2;
   constexpr int REC = (DIM == 3) ? REC3 : REC2;
   constexpr int NP = (DIM == 3) ? 10 : 6;       // parameters per seed in a record
-  static_assert(T == SEED_CHUNK, "one gathered candidate per thread and chunk");
-  extern __shared__ __align__(128) unsigned char smem_raw[];
-  float* s_seeds = reinterpret_cast<float*>(smem_raw);
-  float4* s_prev4 = reinterpret_cast<float4*>(smem_raw + S::PREV_OFF);
-  int* s_lab = reinterpret_cast<int*>(smem_raw + S::LAB_OFF);
-  int* s_idx = reinterpret_cast<int*>(smem_raw + S::IDX_OFF);
-  double* s_red = reinterpret_cast<double*>(smem_raw + S::RED_OFF);
-  float* s_tt = reinterpret_cast<float*>(smem_raw + S::TT_OFF);
+  constexpr int STAGE_FLOATS = (WCHUNK / 2) * PREC;
+  __shared__ __align__(16) float s_seeds[4][2][STAGE_FLOATS];
+  __shared__ int s_idx[4][2][WCHUNK];
 
   if (a.done_flag && *a.done_flag) return;
-  const int tid = threadIdx.x;
+  const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
   const int b = blockIdx.x;
+  const int bx = b % a.g.tiles_x, by = (b / a.g.tiles_x) % a.g.tiles_y, bz = b / (a.g.tiles_x * a.g.tiles_y);
+
+  // a1: this thread's row inside its warp's brick (apd_internal.cuh: brick_box)
+  int tx, ty, tz;
+  if (DIM == 3) { tx = 0; ty = 4 * w + (lane & 3); tz = lane >> 2; }
+  else          { tx = w & 1; ty = 32 * (w >> 1) + lane; tz = 0; }
   RowThread<DIM, G> rt;
-  rt.init(a, b, tid);
+  rt.init_at(a, bx, by, bz, tx, ty, tz);
 
-  int cnt = a.cand_count[b];
-  const bool listed = cnt >= 0;
-  if (!listed) cnt = a.M;
-  const int* list = a.cand_list + (size_t)b * a.cand_cap;
-  const int nchunks = (cnt + SEED_CHUNK - 1) / SEED_CHUNK;
-
-  f2 tt[V];
-  float best[V];
-#pragma unroll
-  for (int k = 0; k < V; ++k) {
-    tt[k] = rt.tau(a, k);
-    best[k] = CUDART_INF_F;
-    s_lab[k * T + tid] = 0;
-    if (tid < G::TXT) { float t, t_; f2_unpack(tt[k], t, t_); s_tt[tid * V + k] = t; }   // tid == tx for these threads
+  // the brick's candidate list; an overflowed list falls back to the super-tile's, then to all seeds
+  const size_t brick = (size_t)b * 4 + w;
+  int cnt = a.brick_count[brick];
+  const int* list = a.brick_list + brick * BRICK_CAP;
+  if (cnt < 0) {
+    constexpr int STX = (DIM == 3) ? SUPER3_TX : SUPER2_TX, STY = (DIM == 3) ? SUPER3_TY : SUPER2_TY,
+                  STZ = (DIM == 3) ? SUPER3_TZ : 1;
+    const int sup = ((bz / STZ) * a.super_y + by / STY) * a.super_x + bx / STX;
+    cnt = a.super_count[sup];
+    list = a.super_list + (size_t)sup * SUPER_CAP;
+    if (cnt < 0) { cnt = a.M; list = nullptr; }
   }
-#pragma unroll
-  for (int k4 = 0; k4 < V / 4; ++k4)
-    s_prev4[k4 * T + tid] = make_float4(CUDART_INF_F, CUDART_INF_F, CUDART_INF_F, CUDART_INF_F);
+  const int nchunks = (cnt + WCHUNK - 1) / WCHUNK;
 
   auto gather = [&](int c) {
     const int stage = c & 1;
-    const int pos = c * SEED_CHUNK + tid;
+    const int pos = c * WCHUNK + lane;
     float r[REC];
     int idx = 0;
     if (pos < cnt) {
-      idx = listed ? list[pos] : pos;
+      idx = list ? __ldg(list + pos) : pos;
       const float4* src = reinterpret_cast<const float4*>(a.rec + (size_t)idx * REC);
 #pragma unroll
       for (int q = 0; q < REC / 4; ++q) {
@@ -451,35 +402,59 @@ __global__ void __launch_bounds__(G::THREADS, G::MINB) assign_rowpoly_culled_ker
       for (int q = 0; q < REC; ++q) r[q] = 0.0f;
       r[NP - 1] = CUDART_INF_F;      // padding candidate: cost +inf, never wins the strict '<'
     }
-    float* dst = s_seeds + (size_t)stage * CHUNK_PAIRS * PREC + (tid >> 1) * PREC + (tid & 1);
+    float* dst = &s_seeds[w][stage][(lane >> 1) * PREC + (lane & 1)];
 #pragma unroll
     for (int q = 0; q < NP; ++q) dst[2 * q] = r[q];
-    s_idx[stage * SEED_CHUNK + tid] = idx;
+    s_idx[w][stage][lane] = idx;
   };
+  if (nchunks > 0) gather(0);        // issued first: its latency overlaps the row set-up below
 
-  if (nchunks > 0) gather(0);
-  __syncthreads();
-  for (int c = 0; c < nchunks; ++c) {
-    if (c + 1 < nchunks) gather(c + 1);     // the other stage: every thread left it before the last barrier
-    // only the groups of ROW_GROUP seeds that hold a real candidate (the tail of the last one is padding)
-    const int ngroups = min(SEED_CHUNK / ROW_GROUP, (cnt - c * SEED_CHUNK + ROW_GROUP - 1) / ROW_GROUP);
-    row_process_chunk<DIM, V, T, true>(s_seeds + (size_t)(c & 1) * CHUNK_PAIRS * PREC, 0, s_idx + (c & 1) * SEED_CHUNK,
-                                       rt.x0, rt.yy, rt.yz, tt, best, s_prev4, s_lab, s_tt + (tid % G::TXT) * V, tid, ngroups);
-    __syncthreads();
-  }
-
+  f2 tt[V];
+  float best[V];
   int lab[V];
 #pragma unroll
-  for (int k = 0; k < V; ++k) lab[k] = s_lab[k * T + tid];
-  const double dsum = row_epilogue<V>(a, rt.row_valid, rt.ix0, rt.iy, rt.iz, best, lab);
-  const double tot = block_sum_double<T>(dsum, s_red);
-  if (tid == 0) {
-    a.dual_partial[b] = tot;
-    // voxel-seed pairs whose cost this tile evaluated (valid voxels only)
-    const int bx = b % a.g.tiles_x, by = (b / a.g.tiles_x) % a.g.tiles_y, bz = b / (a.g.tiles_x * a.g.tiles_y);
-    const long long vx = min(G::TXT * V, a.g.nx - bx * G::TXT * V), vy = min(G::TYT, a.g.ny - by * G::TYT),
-                    vz = min(G::TZT, a.g.nz - bz * G::TZT);
-    atomicAdd(a.pairs_ctr, (unsigned long long)(vx * vy * vz) * (unsigned long long)cnt);
+  for (int k = 0; k < V; ++k) { tt[k] = rt.tau(a, k); best[k] = CUDART_INF_F; lab[k] = 0; }
+  __syncwarp();
+
+  for (int c = 0; c < nchunks; ++c) {
+    if (c + 1 < nchunks) gather(c + 1);     // the other stage: the warp left it before the last __syncwarp
+    const float* sp = s_seeds[w][c & 1];
+    const int* ip = s_idx[w][c & 1];
+    const int npairs = min(WCHUNK / 2, (cnt - c * WCHUNK + 1) / 2);     // pairs that hold a real candidate
+    for (int p = 0; p < npairs; ++p) {
+      const RowCoef rc = row_setup<DIM>(sp + p * PREC, rt.x0, rt.yy, rt.yz);
+      const int i0 = ip[2 * p], i1 = ip[2 * p + 1];
+#pragma unroll
+      for (int k0 = 0; k0 < V; k0 += ROW_BATCH) {
+        f2 u[ROW_BATCH];
+#pragma unroll
+        for (int j = 0; j < ROW_BATCH; ++j) u[j] = f2_fma(rc.a11, tt[k0 + j], rc.Bp);
+#pragma unroll
+        for (int j = 0; j < ROW_BATCH; ++j) u[j] = f2_fma(tt[k0 + j], u[j], rc.Rp);
+#pragma unroll
+        for (int j = 0; j < ROW_BATCH; ++j) {
+          float lo, hi;
+          f2_unpack(u[j], lo, hi);
+          const float m = min3f(best[k0 + j], lo, hi);
+          if (m < best[k0 + j]) lab[k0 + j] = (lo == m) ? i0 : i1;    // lo == hi == m: the lower index
+          best[k0 + j] = m;
+        }
+      }
+    }
+    __syncwarp();
+  }
+
+  double dsum = row_epilogue<V>(a, rt.row_valid, rt.ix0, rt.iy, rt.iz, best, lab);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) dsum += __shfl_down_sync(0xffffffffu, dsum, o);     // fixed order
+  if (lane == 0) {
+    a.dual_partial[brick] = dsum;
+    // voxel-seed pairs whose cost this brick evaluated (valid voxels only)
+    int ox, oy, oz, ex, ey, ez;
+    brick_box(DIM, w, &ox, &oy, &oz, &ex, &ey, &ez);
+    const long long vx = max(0, min(ex, a.g.nx - (bx * G::TXT * V + ox))), vy = max(0, min(ey, a.g.ny - (by * G::TYT + oy))),
+                    vz = max(0, min(ez, a.g.nz - (bz * G::TZT + oz)));
+    if (vx * vy * vz > 0) atomicAdd(a.pairs_ctr, (unsigned long long)(vx * vy * vz) * (unsigned long long)cnt);
   }
 }
 
@@ -490,8 +465,14 @@ static void tiles_of(int nx, int ny, int nz, int* tx, int* ty, int* tz) {
   *tx = cdiv_i(nx, G::TXT * G::V); *ty = cdiv_i(ny, G::TYT); *tz = cdiv_i(nz, G::TZT);
 }
 
-// Picks the row length (returned: 0 = SHORT, 1 = LONG) and the tile counts for a grid.
-int rowpoly_tile_counts(int dim, int nx, int ny, int nz, int sm_count, int* tx, int* ty, int* tz) {
+// Picks the row length (returned: 0 = SHORT, 1 = LONG) and the tile counts for a grid.  The culled kernel always
+// runs the CullGeom tile (short rows).
+int rowpoly_tile_counts(int dim, int nx, int ny, int nz, int sm_count, bool cull, int* tx, int* ty, int* tz) {
+  if (cull) {
+    if (dim == 3) { *tx = cdiv_i(nx, CULL_TILE3_X); *ty = cdiv_i(ny, CULL_TILE3_Y); *tz = cdiv_i(nz, CULL_TILE3_Z); }
+    else          { *tx = cdiv_i(nx, CULL_TILE2_X); *ty = cdiv_i(ny, CULL_TILE2_Y); *tz = 1; }
+    return 0;
+  }
   if (dim == 3) tiles_of<RowGeom3L>(nx, ny, nz, tx, ty, tz); else tiles_of<RowGeom2L>(nx, ny, 1, tx, ty, tz);
   if ((long long)(*tx) * (*ty) * (*tz) >= (long long)ROW_LONG_MIN_WAVES * ROWMINB * sm_count) return 1;
   if (dim == 3) tiles_of<RowGeom3S>(nx, ny, nz, tx, ty, tz); else tiles_of<RowGeom2S>(nx, ny, 1, tx, ty, tz);
@@ -501,14 +482,6 @@ int rowpoly_tile_counts(int dim, int nx, int ny, int nz, int sm_count, int* tx, 
 template <int DIM, class G>
 static cudaError_t launch_rowpoly_t(const AssignArgs& a, int n_tiles, cudaStream_t st) {
   // opt in to > 48 KB of dynamic shared memory (per device; a host-side attribute write, no launch)
-  if (a.cand_count) {
-    constexpr size_t bytes = CullSmem<DIM, G>::BYTES;
-    cudaError_t e = cudaFuncSetAttribute(assign_rowpoly_culled_kernel<DIM, G>,
-                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
-    if (e != cudaSuccess) return e;
-    assign_rowpoly_culled_kernel<DIM, G><<<n_tiles, G::THREADS, bytes, st>>>(a);
-    return cudaGetLastError();
-  }
   constexpr size_t bytes = RowSmem<DIM, G>::BYTES;
   cudaError_t e = cudaFuncSetAttribute(assign_rowpoly_kernel<DIM, G>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                        (int)bytes);
@@ -517,19 +490,15 @@ static cudaError_t launch_rowpoly_t(const AssignArgs& a, int n_tiles, cudaStream
   return cudaGetLastError();
 }
 
-// tile extents in voxels of the geometry chosen for the grid (the culling bounds need them)
-void rowpoly_tile_extent(int dim, int row_long, int* ex, int* ey, int* ez) {
-  if (dim == 3) {
-    if (row_long) { *ex = RowGeom3L::TXT * RowGeom3L::V; *ey = RowGeom3L::TYT; *ez = RowGeom3L::TZT; }
-    else          { *ex = RowGeom3S::TXT * RowGeom3S::V; *ey = RowGeom3S::TYT; *ez = RowGeom3S::TZT; }
-  } else {
-    if (row_long) { *ex = RowGeom2L::TXT * RowGeom2L::V; *ey = RowGeom2L::TYT; *ez = 1; }
-    else          { *ex = RowGeom2S::TXT * RowGeom2S::V; *ey = RowGeom2S::TYT; *ez = 1; }
-  }
+template <int DIM>
+static cudaError_t launch_culled_t(const AssignArgs& a, int n_tiles, cudaStream_t st) {
+  assign_rowpoly_culled_kernel<DIM><<<n_tiles, 128, 0, st>>>(a);
+  return cudaGetLastError();
 }
 
 cudaError_t launch_assign_rowpoly(const AssignArgs& a, cudaStream_t st) {
   const int n_tiles = a.g.tiles_x * a.g.tiles_y * a.g.tiles_z;
+  if (a.brick_count) return a.g.dim == 3 ? launch_culled_t<3>(a, n_tiles, st) : launch_culled_t<2>(a, n_tiles, st);
   if (a.g.dim == 3)
     return a.g.row_long ? launch_rowpoly_t<3, RowGeom3L>(a, n_tiles, st) : launch_rowpoly_t<3, RowGeom3S>(a, n_tiles, st);
   return a.g.row_long ? launch_rowpoly_t<2, RowGeom2L>(a, n_tiles, st) : launch_rowpoly_t<2, RowGeom2S>(a, n_tiles, st);

@@ -64,13 +64,14 @@ def test_configs_full_parity(apd, cfg, kernel, wscale):
 
 
 # ------------------------------------------------------------------ configs 4-5 at full size: sampled voxels
-@pytest.mark.parametrize("kernel", ["auto"])
+@pytest.mark.parametrize("kernel,cull", [("auto", 0), ("auto", 1)])
 @pytest.mark.parametrize("cfg,nsample", [(4, 60000), (5, 30000)])
-def test_large_configs_sampled_parity(apd, cfg, nsample, kernel):
+def test_large_configs_sampled_parity(apd, cfg, nsample, kernel, cull):
     from oracle.apd_oracle import oracle_assign
     wl = workloads.make_config(cfg)
     w = rand_w(wl, 0.1, 200 + cfg)
-    r = run_assign(apd, wl, w, v=wl.v, kernel=KERNELS[kernel])
+    r = run_assign(apd, wl, w, v=wl.v, kernel=KERNELS[kernel], cull=cull)
+    assert (r["pairs"] == wl.N * wl.M) if not cull else (0 < r["pairs"] < 0.02 * wl.N * wl.M)
     grid = parity.grid_of(wl)
     sel = workloads.voxel_sample(wl.N, nsample, cfg)
     orc = oracle_assign(grid, wl.X, wl.A, w, sel=sel)
@@ -84,7 +85,7 @@ def test_large_configs_sampled_parity(apd, cfg, nsample, kernel):
     est = float(np.dot(wl.v.astype(np.float64), w.astype(np.float64))) + float(np.mean(orc.best))
     se = float(np.std(orc.best)) / np.sqrt(len(sel))
     assert abs(r["dual"] - est) < 6 * se + 1e-9
-    print(f"cfg{cfg} sampled: {info}")
+    print(f"cfg{cfg} cull={cull} sampled: {info}; pruned fraction {1 - r['pairs'] / (wl.N * wl.M):.5f}")
 
 
 # ------------------------------------------------------------------ edge cases
@@ -213,14 +214,15 @@ def test_host_call_matches_device_call(apd):
                                      (5, (128, 128, 128), 2500)])
 @pytest.mark.parametrize("wscale", [0.0, 0.2])
 def test_culling_is_exact(apd, cfg, n, M, wscale):
-    """Labels, volumes and centroids with culling == without, bit for bit; the dual to summation order."""
+    """Labels, volumes and centroids with culling == without, bit for bit (grids small enough that brute force runs
+    the same short-row arithmetic as the culled kernel); the dual up to the order of the fp64 partial sums."""
     wl = workloads.make_config(cfg, n=n, M=M)
     w = wl.w0 if wscale == 0.0 else rand_w(wl, wscale, 300 + cfg)
     r0 = run_assign(apd, wl, w, v=wl.v, want_centroids=True, cull=0)
     r1 = run_assign(apd, wl, w, v=wl.v, want_centroids=True, cull=1)
     assert np.array_equal(r0["labels"], r1["labels"])
     assert np.array_equal(r0["vol"], r1["vol"]) and np.array_equal(r0["centroids"], r1["centroids"])
-    assert r1["dual"] == r0["dual"] and r1["err"] == r0["err"]          # same fp32 minima, same reduction order
+    assert abs(r1["dual"] - r0["dual"]) <= 1e-13 * abs(r0["dual"]) and r1["err"] == r0["err"]   # same fp32 minima
     assert 0 < r1["pairs"] <= wl.N * wl.M and r0["pairs"] == wl.N * wl.M
     print(f"cfg{cfg} {wl.n} M={wl.M} wscale={wscale}: pruned fraction {1 - r1['pairs'] / (wl.N * wl.M):.4f}")
 
@@ -237,8 +239,8 @@ def test_culling_edge_cases_parity(apd, case):
 
 
 def test_culling_extreme_weights_and_overflow(apd):
-    """One seed with a huge weight owns everything; every seed coincident => every list overflows CAND_CAP
-    (1024) and the tile falls back to scanning all seeds."""
+    """One seed with a huge weight owns everything; every seed coincident => every brick list overflows BRICK_CAP
+    (256) and falls back to its super-tile's list, and beyond SUPER_CAP (4096) to scanning all seeds."""
     wl = workloads.make_random(3, (64, 48, 40), 300, 31, w_scale=0.1)
     w = wl.w0.copy(); w[17] = 10.0
     r = run_assign(apd, wl, w, v=wl.v, cull=1)
@@ -249,6 +251,11 @@ def test_culling_extreme_weights_and_overflow(apd):
     r1 = run_assign(apd, wl2, wl2.w0, v=wl2.v, cull=1)
     assert np.all(r0["labels"] == 0) and np.array_equal(r0["labels"], r1["labels"])
     assert r1["pairs"] == wl2.N * wl2.M
+    # more coincident seeds than a super-tile list holds (4096): brick -> super-tile -> all seeds
+    wl3 = workloads.make_random(3, (20, 12, 10), 4200, 33)
+    wl3.X[:] = wl3.X[0]; wl3.A[:] = wl3.A[0]
+    r3 = run_assign(apd, wl3, wl3.w0, v=wl3.v, cull=1)
+    assert np.all(r3["labels"] == 0) and r3["pairs"] == wl3.N * wl3.M
 
 
 def test_culling_rejects_direct_kernel(apd):
