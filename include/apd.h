@@ -134,6 +134,11 @@ int apd_solve(apd_ctx* ctx, const apd_grid* grid, int32_t M,
  * entries written (>= 0), or a negative apd_status.  Synchronous. */
 int apd_solve_history(apd_ctx* ctx, double* dual_hist, double* err_hist, int32_t cap);
 
+/* Counters of the most recent apd_solve on this context (HOST out, each may be NULL): evaluations recorded by
+ * apd_solve_history, and how many evaluations of the loop rebuilt the culling candidate lists (with opts.cull the
+ * lists are built with a slack on the bounds and reused while the weights stay within it; 0 without culling). */
+int apd_solve_stats(const apd_ctx* ctx, int32_t* evals_recorded, int32_t* cull_rebuilds);
+
 /* Algorithm 3, generalised Lloyd: K rounds of { Algorithm 2 from the previous weights; seeds <-
  * discrete centroids of the cells (an empty cell keeps its seed) }, then a final Algorithm 2.
  *   X  [M,dim] DEVICE fp32 IN/OUT: X^0 on entry, X^K on return (each round's centroids rounded to fp32)

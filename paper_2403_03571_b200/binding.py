@@ -78,6 +78,8 @@ def load_library() -> ctypes.CDLL:
                                    + [_P] * 5 + [ctypes.POINTER(ctypes.c_int32), ctypes.POINTER(ctypes.c_int32),
                                                  ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double),
                                                  ctypes.POINTER(apd_opts)])
+    lib.apd_solve_stats.restype = ctypes.c_int
+    lib.apd_solve_stats.argtypes = [_P, ctypes.POINTER(ctypes.c_int32), ctypes.POINTER(ctypes.c_int32)]
     lib.apd_lloyd.restype = ctypes.c_int
     lib.apd_lloyd.argtypes = ([_P, ctypes.POINTER(apd_grid), ctypes.c_int32, _P, _P, _P, ctypes.c_double, ctypes.c_int32]
                               + [_P] * 4 + [ctypes.POINTER(ctypes.c_int32), ctypes.POINTER(ctypes.c_int32),
@@ -98,7 +100,7 @@ def load_library() -> ctypes.CDLL:
 
 
 EXPORTED_SYMBOLS = ["apd_default_opts", "apd_create", "apd_destroy", "apd_last_error", "apd_assign", "apd_solve",
-                    "apd_assign_host", "apd_solve_host", "apd_solve_history", "apd_lloyd", "apd_resolution_bound",
+                    "apd_assign_host", "apd_solve_host", "apd_solve_history", "apd_solve_stats", "apd_lloyd", "apd_resolution_bound",
                     "apd_choose_resolution", "apd_last_kernel_ms", "apd_fp32_probe"]
 
 
@@ -258,6 +260,12 @@ class ApdContext:
             ctypes.byref(opts) if opts is not None else None, self._stream())
         self._check(rc, allow=(APD_OK, APD_NOT_CONVERGED))
         return SolveInfo(rc, it.value, ev.value, err.value, float("nan"))
+
+    def solve_stats(self):
+        """(evaluations recorded, candidate-list rebuilds) of the most recent apd_solve."""
+        n, r = ctypes.c_int32(0), ctypes.c_int32(0)
+        self._check(self._lib.apd_solve_stats(self._h, ctypes.byref(n), ctypes.byref(r)))
+        return n.value, r.value
 
     def solve_history(self, cap: int = 8192):
         """(dual, max_rel_err) numpy arrays, one entry per evaluation of the most recent apd_solve."""

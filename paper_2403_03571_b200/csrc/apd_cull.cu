@@ -86,6 +86,10 @@ struct CullArgs {
   int* brick_count;        // [n_tiles * 4]
   float3 ht;               // half-extents of the box of voxel centres of a CTA tile
   const int* done_flag;
+  // list reuse inside apd_solve: the lists are rebuilt only when *rebuild != 0, with the slack *delta on both
+  // bounds, which keeps them valid for every w' with max_i |w'_i - w_i| <= delta.  nullptr: always rebuild, delta 0.
+  const int* rebuild;
+  const float* delta;
 };
 
 // s_i = |y0 - x_i|_{A_i}, rho_i (SLOT 0 = brick, 1 = super-tile: stored; 2 = box of half-extents ht: computed) and
@@ -145,6 +149,8 @@ __global__ void __launch_bounds__(CULL_THREADS) cull_super_kernel(const CullArgs
   __shared__ int s_wsum[CULL_THREADS / 32];
   __shared__ float s_U;
   if (c.done_flag && *c.done_flag) return;
+  if (c.rebuild && !*c.rebuild) return;
+  const float delta = c.delta ? *c.delta : 0.0f;
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   const int b = blockIdx.x;
   const int sx = b % c.nsx, sy = (b / c.nsx) % c.nsy, sz = b / (c.nsx * c.nsy);
@@ -172,7 +178,7 @@ __global__ void __launch_bounds__(CULL_THREADS) cull_super_kernel(const CullArgs
     s_U = u;
   }
   __syncthreads();
-  const float U = s_U;
+  const float U = s_U + 2.0f * delta * (1.0f + CULL_EPS);
 
   int* list = c.super_list + (size_t)b * SUPER_CAP;
   int base = 0;
@@ -211,6 +217,8 @@ __global__ void __launch_bounds__(128) cull_bricks_kernel(const CullArgs c) {
   __shared__ float s_min[4];
   __shared__ int s_wsum[4];
   if (c.done_flag && *c.done_flag) return;
+  if (c.rebuild && !*c.rebuild) return;
+  const float delta = c.delta ? *c.delta : 0.0f;
   const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
   const int b = blockIdx.x;
   const int bx = b % c.g.tiles_x, by = (b / c.g.tiles_x) % c.g.tiles_y, bz = b / (c.g.tiles_x * c.g.tiles_y);
@@ -239,7 +247,7 @@ __global__ void __launch_bounds__(128) cull_bricks_kernel(const CullArgs c) {
     for (int o = 16; o > 0; o >>= 1) umin = fminf(umin, __shfl_xor_sync(0xffffffffu, umin, o));
     if (lane == 0) s_min[w] = umin;
     __syncthreads();
-    const float U = fminf(fminf(s_min[0], s_min[1]), fminf(s_min[2], s_min[3]));
+    const float U = fminf(fminf(s_min[0], s_min[1]), fminf(s_min[2], s_min[3])) + 2.0f * delta * (1.0f + CULL_EPS);
     int base = 0;
     for (int p0 = 0; p0 < n; p0 += 128) {
       const int pos = p0 + tid;
@@ -285,7 +293,7 @@ __global__ void __launch_bounds__(128) cull_bricks_kernel(const CullArgs c) {
   }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) umin = fminf(umin, __shfl_xor_sync(0xffffffffu, umin, o));
-  const float U = umin;
+  const float U = umin + 2.0f * delta * (1.0f + CULL_EPS);
 
   const size_t brick = (size_t)b * 4 + w;
   int* list = c.brick_list + brick * BRICK_CAP;
@@ -320,7 +328,8 @@ void cull_super_counts(const GridDev& g, int* nsx, int* nsy, int* nsz) {
 }
 
 cudaError_t launch_cull(const GridDev& g, int M, int M_pad, const float* X, const float* A, const float* w,
-                        const CullBuffers& cb, int nsx, int nsy, int nsz, const int* done_flag, cudaStream_t st) {
+                        const CullBuffers& cb, int nsx, int nsy, int nsz, const int* done_flag, const int* rebuild,
+                        const float* delta, cudaStream_t st) {
   // half-extents of the boxes of voxel CENTRES of a brick and of a super-tile
   int ox, oy, oz, ex, ey, ez;
   brick_box(g.dim, 0, &ox, &oy, &oz, &ex, &ey, &ez);
@@ -338,7 +347,7 @@ cudaError_t launch_cull(const GridDev& g, int M, int M_pad, const float* X, cons
   CullArgs c;
   c.g = g; c.M = M; c.rec = cb.rec; c.super_list = cb.super_list; c.super_count = cb.super_count;
   c.nsx = nsx; c.nsy = nsy; c.nsz = nsz; c.brick_list = cb.brick_list; c.brick_count = cb.brick_count;
-  c.done_flag = done_flag;
+  c.done_flag = done_flag; c.rebuild = rebuild; c.delta = delta;
   c.ht = make_float3(half(g.dim == 3 ? CULL_TILE3_X : CULL_TILE2_X, 0), half(g.dim == 3 ? CULL_TILE3_Y : CULL_TILE2_Y, 1),
                      g.dim == 3 ? half(CULL_TILE3_Z, 2) : 0.0f);
   const int n_super = nsx * nsy * nsz;

@@ -79,10 +79,12 @@ struct Workspace {
   double* svec = nullptr;               // device fp64 vectors: w, g, p, w_try, w_best, g_new, q, S[m], Y[m]
   int svec_hist = 0;                    // history capacity svec was sized for
   float* w32 = nullptr;                 // [max_seeds] fl32(w) the next evaluation uses
+  float* wref = nullptr;                // [max_seeds] weights the current candidate lists were built at
   double* e_vol = nullptr;              // [max_seeds] evaluation outputs inside the solve loop
   double* e_scal = nullptr;             // [2] dual, max_rel_err
   double* hist = nullptr;               // [2 * SOLVE_HIST_CAP] (dual, err) per evaluation of the last solve
   int hist_len = 0;
+  int last_rebuilds = 0;                // candidate-list rebuilds of the last solve (0 without culling)
   struct SolveReport* report = nullptr; // pinned, mapped host memory the step kernel writes
   cudaEvent_t sev[2] = {nullptr, nullptr};
 };
@@ -123,7 +125,7 @@ struct CullBuffers {
 };
 cudaError_t launch_cull(const GridDev& g, int M, int M_pad, const float* X, const float* A, const float* w,
                         const CullBuffers& cb, int n_super_x, int n_super_y, int n_super_z, const int* done_flag,
-                        cudaStream_t st);
+                        const int* rebuild, const float* delta, cudaStream_t st);
 void cull_super_counts(const GridDev& g, int* nsx, int* nsy, int* nsz);
 int rowpoly_tile_counts(int dim, int nx, int ny, int nz, int sm_count, bool cull, int* tx, int* ty, int* tz);
 int assign_tile_counts(int kernel, int dim, int nx, int ny, int nz, int sm_count, bool cull, int* tx, int* ty, int* tz);
@@ -140,6 +142,7 @@ struct SolveReport {
   volatile int status;    // apd_status
   volatile int iters, evals;
   volatile double err, dual;
+  volatile int cull_rebuilds;   // evaluations of the solve loop that rebuilt the candidate lists
 };
 
 // host helpers shared by apd_api.cu and apd_lbfgs.cu
@@ -148,7 +151,8 @@ int resolve_kernel(const apd_opts* o, std::string* err);
 int enqueue_evaluation(apd_ctx* ctx, const GridDev& g, int kernel, int M, const float* X, const float* A,
                        const float* w, const float* target_vol, int32_t* labels, double* vol, double* dual,
                        double* max_rel_err, double* centroids, uint64_t* pairs, bool timed, bool cull,
-                       const int* done_flag, cudaStream_t st);
+                       const int* done_flag, cudaStream_t st, const int* cull_rebuild = nullptr,
+                       const float* cull_delta = nullptr);
 
 }  // namespace apd
 

@@ -28,6 +28,10 @@ struct SolveState {
   int done, phase, iters, evals, trial, hist_len, hist_start, hist_cap, max_iters, max_evals;
   double f, gp, alpha, lo, hi, gamma, eps, best_err, best_dual, domain_volume;
   double rho[LB_MAX_HIST];
+  // candidate-list reuse (apd_cull.cu): the lists were built at wref with slack cull_delta and stay valid while
+  // max_i |w32_i - wref_i| <= cull_delta
+  int cull_rebuild, cull_rebuilds;
+  float cull_delta, cull_cap;
 };
 
 enum { V_W = 0, V_G, V_P, V_WTRY, V_WBEST, V_GNEW, V_Q, V_HIST };   // rows of svec
@@ -44,7 +48,12 @@ struct StepArgs {
   SolveReport* report; // mapped host memory
   double* hist;        // [2 * hist_cap] (dual, max_rel_err) of every evaluation, in order
   int hist_cap;
+  float* wref;         // weights the candidate lists were built at (culling only)
 };
+
+constexpr double CULL_DELTA_FACTOR = 4.0;   // slack of a rebuilt list = this x the last change of the weights ...
+constexpr double CULL_CAP_FACTOR = 0.5;     // ... but at most this x the mean min-cost of the first evaluation (a larger
+                                            // slack would lengthen every list by more than it saves in rebuilds)
 
 // Sum over the block, identical value returned to every thread; fixed order.
 __device__ __forceinline__ double block_allsum(double v, double* scratch) {
@@ -56,6 +65,18 @@ __device__ __forceinline__ double block_allsum(double v, double* scratch) {
   double t = 0.0;
 #pragma unroll
   for (int i = 0; i < LB_THREADS / 32; ++i) t += scratch[i];
+  return t;
+}
+
+__device__ __forceinline__ double block_allmax(double v, double* scratch) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+  __syncthreads();
+  if ((threadIdx.x & 31) == 0) scratch[threadIdx.x >> 5] = v;
+  __syncthreads();
+  double t = 0.0;
+#pragma unroll
+  for (int i = 0; i < LB_THREADS / 32; ++i) t = fmax(t, scratch[i]);
   return t;
 }
 
@@ -102,9 +123,11 @@ __global__ void solve_init_kernel(StepArgs a, const float* w_init, int hist_cap,
     const double w = w_init ? (double)w_init[i] : 0.0;     // Alg. 2 step 2: W0 = 0
     a.vec[(size_t)V_W * a.stride + i] = w;
     a.w32[i] = (float)w;
+    a.wref[i] = (float)w;
   }
   if (i == 0) {
     SolveState* st = a.st;
+    st->cull_rebuild = 1; st->cull_rebuilds = 1; st->cull_delta = 0.0f; st->cull_cap = 0.0f;
     st->done = 0; st->phase = 0; st->iters = 0; st->evals = 0; st->trial = 0;
     st->hist_len = 0; st->hist_start = 0; st->hist_cap = hist_cap;
     st->max_iters = max_iters; st->max_evals = max_evals;
@@ -112,7 +135,7 @@ __global__ void solve_init_kernel(StepArgs a, const float* w_init, int hist_cap,
     st->gamma = gamma0; st->eps = eps; st->best_err = INFINITY; st->best_dual = 0.0;
     st->domain_volume = domain_volume;
     a.report->done = 0; a.report->status = APD_OK; a.report->iters = 0; a.report->evals = 0;
-    a.report->err = 0.0; a.report->dual = 0.0;
+    a.report->err = 0.0; a.report->dual = 0.0; a.report->cull_rebuilds = 0;
   }
 }
 
@@ -160,7 +183,14 @@ __global__ void __launch_bounds__(LB_THREADS) lbfgs_step_kernel(StepArgs a) {
 
   int finish = 0;          // 1: OK at w_eval, 2: NOT_CONVERGED at best, 3: bad target volumes
   bool need_direction = false;
+  float cull_cap = st->cull_cap;
   if (phase == 0) {
+    // cost scale for the list-reuse slack: mean over the voxels of min_i C_ij = (g~ - <v, w>) / |Omega|  (identity I1)
+    double vw = 0.0;
+    for (int i = tid; i < M; i += LB_THREADS) vw += (double)a.v[i] * (double)a.w32[i];
+    vw = block_allsum(vw, scratch);
+    const double scale = fabs(a.e_scal[0] - vw) / st->domain_volume;
+    cull_cap = isfinite(scale) ? (float)(CULL_CAP_FACTOR * scale) : 0.0f;
     vsum = block_allsum(vsum, scratch);
     if (!(fabs(vsum - st->domain_volume) <= 1e-5 * st->domain_volume)) finish = 3;
     else if (err1 <= eps) finish = 1;
@@ -233,12 +263,27 @@ __global__ void __launch_bounds__(LB_THREADS) lbfgs_step_kernel(StepArgs a) {
     alpha = 1.0; lo = 0.0; hi = INFINITY; trial = 0;
   }
 
+  int cull_rebuild = 1;
+  float cull_delta = 0.0f;
   if (finish == 0) {
     // next trial point w + alpha p, rounded to fp32 for the evaluation (S10)
+    double step_max = 0.0, ref_max = 0.0;   // max |change since the last evaluation|, max |distance from wref|
     for (int i = tid; i < M; i += LB_THREADS) {
       const double wt = __dadd_rn(w[i], __dmul_rn(alpha, p[i]));
       wtry[i] = wt;
-      a.w32[i] = (float)wt;
+      const float wn = (float)wt;
+      step_max = fmax(step_max, fabs((double)wn - (double)a.w32[i]));     // differences of floats: exact in fp64
+      ref_max = fmax(ref_max, fabs((double)wn - (double)a.wref[i]));
+      a.w32[i] = wn;
+    }
+    step_max = block_allmax(step_max, scratch);
+    ref_max = block_allmax(ref_max, scratch);
+    cull_delta = st->cull_delta;
+    cull_rebuild = !(ref_max <= (double)cull_delta);
+    if (cull_rebuild) {
+      // the next evaluation rebuilds its candidate lists at the new weights, valid within delta of them
+      cull_delta = fminf((float)(CULL_DELTA_FACTOR * step_max), cull_cap);
+      for (int i = tid; i < M; i += LB_THREADS) a.wref[i] = a.w32[i];
     }
   } else if (finish == 1) {
     if (phase != 0) for (int i = tid; i < M; i += LB_THREADS) w[i] = wtry[i];
@@ -251,12 +296,14 @@ __global__ void __launch_bounds__(LB_THREADS) lbfgs_step_kernel(StepArgs a) {
     st->hist_len = hist_len; st->hist_start = hist_start;
     st->f = f; st->gp = gp; st->alpha = alpha; st->lo = lo; st->hi = hi; st->gamma = gamma;
     st->best_err = best_err; st->best_dual = best_dual;
+    st->cull_cap = cull_cap; st->cull_rebuild = cull_rebuild; st->cull_delta = cull_delta; st->cull_rebuilds += (finish == 0 && cull_rebuild);
     if (finish) {
       st->done = 1;
       a.report->status = (finish == 1) ? APD_OK : (finish == 2 ? APD_NOT_CONVERGED : APD_E_ARG);
       a.report->iters = iters; a.report->evals = evals;
       a.report->err = (finish == 2) ? best_err : err1;
       a.report->dual = (finish == 2) ? best_dual : -f1;
+      a.report->cull_rebuilds = st->cull_rebuilds;
       __threadfence_system();
       a.report->done = 1;
       __threadfence_system();
@@ -283,6 +330,7 @@ static int ensure_solve_state(apd_ctx* ctx, int hist) {
   if (!ws.sstate) {
     LB_TRY(cudaMalloc(&ws.sstate, sizeof(SolveState)));
     LB_TRY(cudaMalloc(&ws.w32, ms * sizeof(float)));
+    LB_TRY(cudaMalloc(&ws.wref, ms * sizeof(float)));
     LB_TRY(cudaMalloc(&ws.e_vol, ms * sizeof(double)));
     LB_TRY(cudaMalloc(&ws.e_scal, 2 * sizeof(double)));
     LB_TRY(cudaMalloc(&ws.hist, 2 * (size_t)SOLVE_HIST_CAP * sizeof(double)));
@@ -333,7 +381,7 @@ extern "C" int apd_solve(apd_ctx* ctx, const apd_grid* grid, int32_t M, const fl
   StepArgs sa;
   sa.st = ws.sstate; sa.vec = ws.svec; sa.stride = ws.max_seeds; sa.M = M; sa.v = target_vol;
   sa.e_vol = ws.e_vol; sa.e_scal = ws.e_scal; sa.w32 = ws.w32;
-  sa.hist = ws.hist; sa.hist_cap = SOLVE_HIST_CAP;
+  sa.hist = ws.hist; sa.hist_cap = SOLVE_HIST_CAP; sa.wref = ws.wref;
   ws.hist_len = 0;
   SolveReport* dev_report = nullptr;
   LB_TRY(cudaHostGetDevicePointer((void**)&dev_report, ws.report, 0));
@@ -348,7 +396,8 @@ extern "C" int apd_solve(apd_ctx* ctx, const apd_grid* grid, int32_t M, const fl
   const long long hard_cap = (long long)max_evals + 64;
   for (;; ++enq) {
     rc = enqueue_evaluation(ctx, g, kernel, M, X, A, ws.w32, target_vol, nullptr, ws.e_vol, ws.e_scal,
-                            ws.e_scal + 1, nullptr, nullptr, false, o.cull != 0, done_flag, st);
+                            ws.e_scal + 1, nullptr, nullptr, false, o.cull != 0, done_flag, st, &ws.sstate->cull_rebuild,
+                            &ws.sstate->cull_delta);
     if (rc != APD_OK) return rc;
     lbfgs_step_kernel<<<1, LB_THREADS, 0, st>>>(sa);
     LB_TRY(cudaGetLastError());
@@ -374,11 +423,19 @@ extern "C" int apd_solve(apd_ctx* ctx, const apd_grid* grid, int32_t M, const fl
                                   cudaMemcpyDeviceToDevice, st));
   LB_TRY(cudaStreamSynchronize(st));
   ws.hist_len = ws.report->evals < SOLVE_HIST_CAP ? ws.report->evals : SOLVE_HIST_CAP;
+  ws.last_rebuilds = o.cull ? ws.report->cull_rebuilds : 0;
   if (iters) *iters = ws.report->iters;
   if (evals) *evals = ws.report->evals;
   if (max_rel_err) *max_rel_err = ws.report->err;
   if (dual) *dual = ws.report->dual;
   return status;
+}
+
+extern "C" int apd_solve_stats(const apd_ctx* ctx, int32_t* evals_recorded, int32_t* cull_rebuilds) {
+  if (!ctx) return APD_E_ARG;
+  if (evals_recorded) *evals_recorded = ctx->ws.hist_len;
+  if (cull_rebuilds) *cull_rebuilds = ctx->ws.last_rebuilds;
+  return APD_OK;
 }
 
 extern "C" int apd_solve_history(apd_ctx* ctx, double* dual_hist, double* err_hist, int32_t cap) {

@@ -117,6 +117,34 @@ def test_culled_solve_is_the_same_solve(apd):
     assert np.array_equal(a[5][1], b[5][1])
 
 
+def test_full_size_culled_solve_against_brute_force_evaluation(apd):
+    """cfg 4 at full size (256^3 x 10^4): apd_solve with culling (candidate lists reused across evaluations), then ONE
+    brute-force evaluation at the returned weights: same labels except fp32 near-ties (the brute-force kernel runs
+    long rows there), same volumes up to those voxels, tolerance met."""
+    wl = workloads.make_config(4)
+    dev = torch.device("cuda:0")
+    ctx = apd.ApdContext(wl.dim, wl.M)
+    grid = apd.make_grid(wl.dim, wl.n, wl.lo, wl.hi)
+    X = torch.from_numpy(wl.X).to(dev); A = torch.from_numpy(wl.A).to(dev); v = torch.from_numpy(wl.v).to(dev)
+    w = torch.zeros(wl.M, dtype=torch.float32, device=dev)
+    lab_c = torch.empty(wl.N, dtype=torch.int32, device=dev); vol_c = torch.zeros(wl.M, dtype=torch.float64, device=dev)
+    info = ctx.apd_solve(grid, X, A, v, wl.eps, w=w, labels=lab_c, vol=vol_c, opts=apd.make_opts(cull=1))
+    n_rec, rebuilds = ctx.solve_stats()
+    assert info.status == 0 and info.max_rel_err <= wl.eps and n_rec == info.evals
+    assert 1 <= rebuilds < info.evals, f"{rebuilds} rebuilds in {info.evals} evaluations: lists are not being reused"
+    lab_b = torch.empty(wl.N, dtype=torch.int32, device=dev); vol_b = torch.zeros(wl.M, dtype=torch.float64, device=dev)
+    dual = torch.zeros(1, dtype=torch.float64, device=dev); err = torch.zeros(1, dtype=torch.float64, device=dev)
+    ctx.apd_assign(grid, X, A, w, target_vol=v, labels=lab_b, vol=vol_b, dual=dual, max_rel_err=err,
+                   opts=apd.make_opts(cull=0))
+    torch.cuda.synchronize()
+    nm = int((lab_b != lab_c).sum().item())
+    P = 1.0 / wl.N
+    assert nm < 1e-5 * wl.N
+    assert float((vol_b - vol_c).abs().sum().item()) <= 2 * nm * P + 1e-15
+    assert float(err.item()) <= wl.eps + 2 * nm * P / float(wl.v.min())
+    print(f"cfg4 full: {info.evals} evaluations, {rebuilds} list rebuilds, {nm} label differences vs brute force")
+
+
 def test_P13_trivial_optimum(apd):
     """Seeds on a regular lattice, A = I, equal targets: W = 0 is optimal, iters = 0 (PAPER.md:150 W0 = 0)."""
     k, n = 4, 32
