@@ -155,6 +155,7 @@ int enqueue_evaluation(apd_ctx* ctx, const GridDev& g, int kernel, int M, const 
                                         centroids ? ws.idxsum : nullptr, done_flag, st));
   AssignArgs a;
   a.g = g; a.M = M; a.M_pad = M_pad; a.seeds = ws.seeds; a.labels = labels; a.count = ws.count;
+  for (int k = 0; k < 32; ++k) a.tt[k] = (float)((double)k * g.s[0]);
   a.idxsum = centroids ? ws.idxsum : nullptr; a.dual_partial = ws.dual_partial;
   a.rec = nullptr; a.brick_list = nullptr; a.brick_count = nullptr; a.super_list = nullptr; a.super_count = nullptr;
   a.super_x = a.super_y = 0; a.pairs_ctr = nullptr;

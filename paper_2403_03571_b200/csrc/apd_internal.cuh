@@ -53,6 +53,11 @@ struct AssignArgs {
   const int* super_count;  // [n_super]
   int super_x, super_y;    // super-tiles per axis (x, y); super-tile of CTA tile (bx,by,bz) = (bx/SUPER_TX, ...)
   unsigned long long* pairs_ctr;  // [1] voxel-seed pairs evaluated
+  // in-row offsets tau_k = fl32(k s_x), k < 32: the same for every row of every tile, so they are kernel
+  // PARAMETERS -- the compiler keeps them in uniform registers / the constant bank and the FFMA2s read them from
+  // there, which frees one vector register per voxel of the row.  (The row's voxel k is evaluated at x_row0 + tau_k:
+  // within one ulp of its fp32 centre, and exactly the centre on power-of-two grids.)
+  float tt[32];
   const int* done_flag;  // solve loop only: kernels return at once when *done_flag != 0; else nullptr
 };
 

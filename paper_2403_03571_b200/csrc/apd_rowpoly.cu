@@ -113,9 +113,12 @@ __device__ __forceinline__ f2 row_cost(const RowCoef& c, f2 tt) {
 
 // Tile geometry: THREADS = TXT*TYT*TZT threads, each owns a row of V voxels contiguous in x, so the tile is
 // (TXT*V) x TYT x TZT voxels.  MINB = CTAs per SM the register allocation is held to.
-template <int DIM, int V_, int TXT_, int TYT_, int TZT_, int MINB_>
+// GROUP = seeds between two argmin checks (long rows on big problems: 16; short rows / few seeds: 8, where label
+// changes are denser and a rescan should be short).
+template <int DIM, int V_, int TXT_, int TYT_, int TZT_, int MINB_, int GROUP_>
 struct RowGeom {
-  static constexpr int V = V_, TXT = TXT_, TYT = TYT_, TZT = TZT_, THREADS = TXT_ * TYT_ * TZT_, MINB = MINB_;
+  static constexpr int V = V_, TXT = TXT_, TYT = TYT_, TZT = TZT_, THREADS = TXT_ * TYT_ * TZT_, MINB = MINB_,
+                       GROUP = GROUP_;
 };
 #ifndef ROWMINB
 #define ROWMINB 4
@@ -129,16 +132,12 @@ struct RowGeom {
 // Two row lengths are built.  LONG rows (V = 32) amortise the per-(row, seed) set-up best and are used once the
 // grid gives every SM at least ROW_LONG_MIN_WAVES waves of long-row tiles; smaller grids take SHORT rows (V = 16),
 // whose tiles are half as big, so that all SMs have work.
-using RowGeom3L = RowGeom<3, 32, 1, 16, 8, ROWMINB>;    // tile 32 x 16 x 8 voxels, 128 threads
-using RowGeom3S = RowGeom<3, 16, 1, 16, 8, ROWMINB>;    // tile 16 x 16 x 8 voxels
-using RowGeom2L = RowGeom<2, 32, 2, 64, 1, ROWMINB>;    // tile 64 x 64 pixels
-using RowGeom2S = RowGeom<2, 16, 2, 64, 1, ROWMINB>;    // tile 32 x 64 pixels
+using RowGeom3L = RowGeom<3, 32, 1, 16, 8, ROWMINB, 16>;    // tile 32 x 16 x 8 voxels, 128 threads
+using RowGeom3S = RowGeom<3, 16, 1, 16, 8, ROWMINB, 8>;    // tile 16 x 16 x 8 voxels
+using RowGeom2L = RowGeom<2, 32, 2, 64, 1, ROWMINB, 16>;    // tile 64 x 64 pixels
+using RowGeom2S = RowGeom<2, 16, 2, 64, 1, ROWMINB, 8>;    // tile 32 x 64 pixels
 constexpr int ROW_LONG_MIN_WAVES = 2;
 
-#ifndef ROWGROUP
-#define ROWGROUP 16
-#endif
-constexpr int ROW_GROUP = ROWGROUP;                 // seeds between two argmin checks
 #ifndef ROWSTAGES
 #define ROWSTAGES 4
 #endif
@@ -166,7 +165,7 @@ struct RowSmem {
 
 // One staged chunk of SEED_CHUNK seeds ibase .. ibase+SEED_CHUNK-1 (pair-interleaved records at `sp`) against the
 // thread's row: rows a3 + a4 of the brute-force kernel.
-template <int DIM, int V, int T>
+template <int DIM, int V, int T, int ROW_GROUP>
 __device__ __forceinline__ void row_process_chunk(const float* __restrict__ sp, int ibase, f2 x0, f2 yy, f2 yz,
                                                   const f2 (&tt)[V], float (&best)[V], float4* __restrict__ s_prev4,
                                                   int* __restrict__ s_lab, int tid) {
@@ -217,13 +216,20 @@ __device__ __forceinline__ void row_process_chunk(const float* __restrict__ sp, 
       for (int p = 0; p < GROUP_PAIRS && mask; ++p) {
         const RowCoef rc = row_setup<DIM>(gp + p * PREC, x0, yy, yz);
         const int i0 = ibase + gidx * ROW_GROUP + 2 * p;
+        // a new seed takes over an interval of the row, and neighbouring rows (the other lanes) similar ones: test
+        // the row in blocks of 8 voxels so that the untouched blocks cost one branch
 #pragma unroll
-        for (int k = 0; k < V; ++k) {
-          if (mask & (1u << k)) {
-            float lo, hi;
-            f2_unpack(row_cost(rc, tt[k]), lo, hi);
-            if (lo == best[k]) { s_lab[k * T + tid] = i0; mask &= ~(1u << k); }
-            else if (hi == best[k]) { s_lab[k * T + tid] = i0 + 1; mask &= ~(1u << k); }
+        for (int k8 = 0; k8 < V; k8 += 8) {
+          if (mask & (0xffu << k8)) {
+#pragma unroll
+            for (int k = k8; k < k8 + 8; ++k) {
+              if (mask & (1u << k)) {
+                float lo, hi;
+                f2_unpack(row_cost(rc, tt[k]), lo, hi);
+                if (lo == best[k]) { s_lab[k * T + tid] = i0; mask &= ~(1u << k); }
+                else if (hi == best[k]) { s_lab[k * T + tid] = i0 + 1; mask &= ~(1u << k); }
+              }
+            }
           }
         }
       }
@@ -251,13 +257,8 @@ struct RowThread {
     const float yzf = (DIM == 3) ? (float)(a.g.lo[2] + ((double)iz + 0.5) * a.g.s[2]) : 0.0f;
     x0 = f2_pack(x0f, x0f); yy = f2_pack(yyf, yyf); yz = f2_pack(yzf, yzf);
   }
-  // in-row offset of voxel k from the row's first voxel, taken between the two fp32 centres
-  __device__ __forceinline__ f2 tau(const AssignArgs& a, int k) const {
-    float x0f, dummy;
-    f2_unpack(x0, x0f, dummy);
-    const float t = (float)((a.g.lo[0] + ((double)(ix0 + k) + 0.5) * a.g.s[0]) - (double)x0f);
-    return f2_pack(t, t);
-  }
+  // in-row offset of voxel k from the row's first voxel (a kernel parameter: uniform)
+  __device__ __forceinline__ f2 tau(const AssignArgs& a, int k) const { return f2_pack(a.tt[k], a.tt[k]); }
 };
 
 template <int DIM, class G>
@@ -317,7 +318,7 @@ __global__ void __launch_bounds__(G::THREADS, G::MINB) assign_rowpoly_kernel(con
                    a.seeds + (size_t)(c + ROW_STAGES - 1) * CHUNK_PAIRS * PREC, CHUNK_BYTES, &s_full[s2]);
     }
     mbar_wait(&s_full[stage], (uint32_t)((c / ROW_STAGES) & 1));
-    row_process_chunk<DIM, V, T>(s_seeds + (size_t)stage * CHUNK_PAIRS * PREC, c * SEED_CHUNK, rt.x0, rt.yy, rt.yz, tt,
+    row_process_chunk<DIM, V, T, G::GROUP>(s_seeds + (size_t)stage * CHUNK_PAIRS * PREC, c * SEED_CHUNK, rt.x0, rt.yy, rt.yz, tt,
                                  best, s_prev4, s_lab, tid);
     __syncwarp();
     if ((tid & 31) == 0) mbar_arrive(&s_empty[stage]);
