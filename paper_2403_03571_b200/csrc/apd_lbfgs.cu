@@ -16,11 +16,14 @@
 #include "apd_internal.cuh"
 #include "apd_device.cuh"
 #include <cmath>
+#include <cooperative_groups.h>
+namespace cg = cooperative_groups;
 #include <vector>
 
 namespace apd {
 
-constexpr int LB_THREADS = 1024;
+constexpr int LB_THREADS = 256;
+constexpr int LB_CLUSTER = 8;      // CTAs (SMs) of the step kernel's thread-block cluster
 constexpr int LB_MAX_HIST = 64;
 constexpr int LB_MAX_TRIALS = 30;
 
@@ -49,71 +52,212 @@ struct StepArgs {
   double* hist;        // [2 * hist_cap] (dual, max_rel_err) of every evaluation, in order
   int hist_cap;
   float* wref;         // weights the candidate lists were built at (culling only)
+  double* gram;        // [LB_CLUSTER] copies of { (2 hist_cap + 1)^2 Gram matrix, hist_cap rho }, see direction_vf
 };
 
 constexpr double CULL_DELTA_FACTOR = 4.0;   // slack of a rebuilt list = this x the last change of the weights ...
 constexpr double CULL_CAP_FACTOR = 0.5;     // ... but at most this x the mean min-cost of the first evaluation (a larger
                                             // slack would lengthen every list by more than it saves in rebuilds)
 
-// Sum over the block, identical value returned to every thread; fixed order.
-__device__ __forceinline__ double block_allsum(double v, double* scratch) {
+// ---- reductions over the CLUSTER ------------------------------------------------------------------------------
+// The step kernel is ONE thread-block cluster of LB_CLUSTER CTAs (one per SM): a single CTA cannot keep enough loads
+// in flight to stream the L-BFGS vectors (measured: its sweeps ran at pure L2 latency), eight can.  Element i of
+// every length-M vector is owned by one thread of one CTA in every sweep (i = tid + LB_THREADS (rank + LB_CLUSTER k)),
+// so vectors need no synchronisation; scalars come from reductions that return the SAME value, bit for bit, to every
+// thread of every CTA (lanes by shuffle tree, warps in order, CTAs in rank order), which keeps the control flow
+// uniform over the whole cluster.  Cluster partials are exchanged through distributed shared memory; two buffers
+// are used alternately so that one cluster barrier per reduction suffices.
+constexpr int LB_NRED = 13;                          // most values reduced at once (gram_rows)
+
+struct Reducer {
+  double* wbuf;        // [LB_THREADS / 32][LB_NRED]   warp partials of this CTA
+  double* cbuf;        // [2][LB_NRED]                 CTA totals, read by the other CTAs of the cluster
+  int flip;
+  unsigned int rank;
+};
+
+template <int N, bool MAX>
+__device__ __forceinline__ void cluster_all(double (&v)[N], Reducer& r) {
+  cg::cluster_group cluster = cg::this_cluster();
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-  __syncthreads();                       // scratch free
-  if ((threadIdx.x & 31) == 0) scratch[threadIdx.x >> 5] = v;
+  for (int n = 0; n < N; ++n) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      const double u = __shfl_xor_sync(0xffffffffu, v[n], o);
+      v[n] = MAX ? fmax(v[n], u) : v[n] + u;
+    }
+  }
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  __syncthreads();                                   // wbuf free (its last readers are past this point)
+  if (lane == 0) {
+#pragma unroll
+    for (int n = 0; n < N; ++n) r.wbuf[wid * LB_NRED + n] = v[n];
+  }
   __syncthreads();
-  double t = 0.0;
+  r.flip ^= 1;
+  double* mine = r.cbuf + r.flip * LB_NRED;
+  if (threadIdx.x < N) {
+    double t = r.wbuf[threadIdx.x];
 #pragma unroll
-  for (int i = 0; i < LB_THREADS / 32; ++i) t += scratch[i];
-  return t;
+    for (int k = 1; k < LB_THREADS / 32; ++k) {
+      const double u = r.wbuf[k * LB_NRED + threadIdx.x];
+      t = MAX ? fmax(t, u) : t + u;
+    }
+    mine[threadIdx.x] = t;
+  }
+  cluster.sync();                                    // every CTA's totals are written and visible
+#pragma unroll
+  for (int n = 0; n < N; ++n) {
+    double t = cluster.map_shared_rank(mine, 0)[n];
+#pragma unroll
+    for (int c = 1; c < LB_CLUSTER; ++c) {
+      const double u = cluster.map_shared_rank(mine, c)[n];
+      t = MAX ? fmax(t, u) : t + u;
+    }
+    v[n] = t;
+  }
 }
 
-__device__ __forceinline__ double block_allmax(double v, double* scratch) {
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
-  __syncthreads();
-  if ((threadIdx.x & 31) == 0) scratch[threadIdx.x >> 5] = v;
-  __syncthreads();
-  double t = 0.0;
-#pragma unroll
-  for (int i = 0; i < LB_THREADS / 32; ++i) t = fmax(t, scratch[i]);
-  return t;
+__device__ __forceinline__ double cluster_allsum(double x, Reducer& r) {
+  double v[1] = {x};
+  cluster_all<1, false>(v, r);
+  return v[0];
+}
+__device__ __forceinline__ double cluster_allmax(double x, Reducer& r) {
+  double v[1] = {x};
+  cluster_all<1, true>(v, r);
+  return v[0];
 }
 
-__device__ __forceinline__ double block_dot(const double* a, const double* b, int M, double* scratch) {
-  double p = 0.0;
-  for (int i = threadIdx.x; i < M; i += LB_THREADS) p += a[i] * b[i];
-  return block_allsum(p, scratch);
+// element loop of this thread: for (int i = LB_FIRST(r); i < M; i += LB_STEP)
+#define LB_FIRST(r) ((int)threadIdx.x + LB_THREADS * (int)(r).rank)
+constexpr int LB_STEP = LB_THREADS * LB_CLUSTER;
+
+// ---- the L-BFGS direction in "vector-free" form ---------------------------------------------------------------
+// The two-loop recursion of Liu & Nocedal [70] only ever forms linear combinations of the 2m+1 basis vectors
+// b = (s_0..s_{m-1}, y_0..y_{m-1}, g) and inner products with them, so it can be run on the COEFFICIENTS of q in
+// that basis given the Gram matrix B = b^T b: the same algorithm, the same result up to fp64 rounding, but the 2m
+// dependent passes over the length-M vectors (each a latency-bound reduction) become m/2 Gram passes when a pair is
+// pushed plus ONE combination pass.  Every CTA keeps its own copy of the Gram matrix and of rho in global memory
+// (all copies are identical, no cross-CTA visibility to arrange), in SLOT space (ring slots of S and Y):
+//   index of S slot j = j,  of Y slot j = cap + j,  of g = 2 cap;  leading dimension ld = 2 cap + 1;
+//   a copy is ld*ld doubles of Gram matrix followed by cap doubles of rho.
+__device__ __forceinline__ double* gram_of(const StepArgs& a, int cap, unsigned int rank) {
+  return a.gram + (size_t)rank * ((size_t)(2 * cap + 1) * (2 * cap + 1) + cap);
 }
 
-// p = -H g (two-loop recursion of Liu & Nocedal [70], H0 = gamma I); returns g.p to all threads.
-__device__ double new_direction(const StepArgs& a, SolveState* st, int hist_len, int hist_start, double gamma,
-                                double* scratch, double* s_alpha) {
-  const int M = a.M, stride = a.stride, cap = st->hist_cap;
+// Inner products of the NNEW vectors nv[] (Gram indices nidx[]; nv[NNEW-1] is g) with S_j and Y_j of every active
+// slot, and g.g, written to both triangles of this CTA's Gram copy.
+template <int NNEW>
+__device__ void gram_rows(const StepArgs& a, int cap, int hist_len, int hist_start, const double* (&nv)[NNEW],
+                          const int (&nidx)[NNEW], Reducer& r) {
+  const int M = a.M, stride = a.stride, ld = 2 * cap + 1;
+  const double* S = a.vec + (size_t)V_HIST * stride;
+  const double* Y = S + (size_t)cap * stride;
+  double* gm = gram_of(a, cap, r.rank);
+  for (int t0 = 0; t0 < hist_len; t0 += 2) {
+    const bool has1 = t0 + 1 < hist_len;
+    const int j0 = (hist_start + t0) % cap, j1 = has1 ? (hist_start + t0 + 1) % cap : j0;
+    const double *s0 = S + (size_t)j0 * stride, *y0 = Y + (size_t)j0 * stride;
+    const double *s1 = S + (size_t)j1 * stride, *y1 = Y + (size_t)j1 * stride;
+    double acc[LB_NRED];
+#pragma unroll
+    for (int n = 0; n < LB_NRED; ++n) acc[n] = 0.0;
+    for (int i = LB_FIRST(r); i < M; i += LB_STEP) {
+      const double a0 = s0[i], b0 = y0[i], a1 = s1[i], b1 = y1[i];
+      double x[NNEW];
+#pragma unroll
+      for (int n = 0; n < NNEW; ++n) x[n] = nv[n][i];
+#pragma unroll
+      for (int n = 0; n < NNEW; ++n) {
+        acc[4 * n + 0] += x[n] * a0; acc[4 * n + 1] += x[n] * b0;
+        acc[4 * n + 2] += x[n] * a1; acc[4 * n + 3] += x[n] * b1;
+      }
+      acc[12] += x[NNEW - 1] * x[NNEW - 1];
+    }
+    cluster_all<LB_NRED, false>(acc, r);
+    if (threadIdx.x == 0) {
+      for (int n = 0; n < NNEW; ++n) {
+        const int q = nidx[n];
+        gm[(size_t)q * ld + j0] = acc[4 * n + 0]; gm[(size_t)j0 * ld + q] = acc[4 * n + 0];
+        gm[(size_t)q * ld + cap + j0] = acc[4 * n + 1]; gm[(size_t)(cap + j0) * ld + q] = acc[4 * n + 1];
+        if (has1) {
+          gm[(size_t)q * ld + j1] = acc[4 * n + 2]; gm[(size_t)j1 * ld + q] = acc[4 * n + 2];
+          gm[(size_t)q * ld + cap + j1] = acc[4 * n + 3]; gm[(size_t)(cap + j1) * ld + q] = acc[4 * n + 3];
+        }
+      }
+      if (t0 == 0) gm[(size_t)(2 * cap) * ld + 2 * cap] = acc[12];
+    }
+  }
+  __syncthreads();          // thread 0's global writes are ordered before the CTA's reads in direction_vf
+}
+
+// p = -H g with H0 = gamma I; returns g.p to all threads of the cluster.  dyn: dynamic shared memory of the CTA,
+// (2m+1)^2 + (2m+1) + 2m doubles and m ints (m = hist_len <= cap).  Every CTA runs the (tiny) coefficient recursion
+// redundantly on its own Gram copy; the combination pass is shared out over the cluster's threads.
+__device__ double direction_vf(const StepArgs& a, int cap, int hist_len, int hist_start, double gamma, Reducer& r,
+                               double* dyn) {
+  const int M = a.M, stride = a.stride, ld = 2 * cap + 1, hl = hist_len, n = 2 * hl + 1, tid = threadIdx.x;
   double* g = a.vec + (size_t)V_G * stride;
   double* p = a.vec + (size_t)V_P * stride;
-  double* q = a.vec + (size_t)V_Q * stride;
-  double* S = a.vec + (size_t)V_HIST * stride;
-  double* Y = S + (size_t)cap * stride;
-  for (int i = threadIdx.x; i < M; i += LB_THREADS) q[i] = g[i];
-  for (int t = hist_len - 1; t >= 0; --t) {              // newest -> oldest
-    const int slot = (hist_start + t) % cap;
-    const double al = st->rho[slot] * block_dot(S + (size_t)slot * stride, q, M, scratch);
-    if (threadIdx.x == 0) s_alpha[t] = al;
-    const double* y = Y + (size_t)slot * stride;
-    for (int i = threadIdx.x; i < M; i += LB_THREADS) q[i] = __dsub_rn(q[i], __dmul_rn(al, y[i]));
+  const double* S = a.vec + (size_t)V_HIST * stride;
+  const double* Y = S + (size_t)cap * stride;
+  const double* gm = gram_of(a, cap, r.rank);
+  const double* rho_g = gm + (size_t)ld * ld;
+  double* Cm = dyn;                    // [n][n] compact Gram matrix in RING order (0 = oldest pair)
+  double* delta = Cm + n * n;          // [n] coefficients of q, then of r, in the basis (S.., Y.., g)
+  double* al = delta + n;              // [hl]
+  double* rho = al + hl;               // [hl]
+  int* slot_of = reinterpret_cast<int*>(rho + hl);   // [hl]
+  __syncthreads();                     // dyn free
+  for (int e = tid; e < n * n; e += LB_THREADS) {
+    const int rr = e / n, cc = e % n;
+    auto gi = [&](int c) { return c < hl ? (hist_start + c) % cap : (c < 2 * hl ? cap + (hist_start + c - hl) % cap : 2 * cap); };
+    Cm[e] = (hl > 0) ? gm[(size_t)gi(rr) * ld + gi(cc)] : 0.0;
   }
-  for (int i = threadIdx.x; i < M; i += LB_THREADS) q[i] = __dmul_rn(gamma, q[i]);
-  __syncthreads();                                        // s_alpha visible
-  for (int t = 0; t < hist_len; ++t) {                    // oldest -> newest
-    const int slot = (hist_start + t) % cap;
-    const double be = st->rho[slot] * block_dot(Y + (size_t)slot * stride, q, M, scratch);
-    const double coef = s_alpha[t] - be;
-    const double* s = S + (size_t)slot * stride;
-    for (int i = threadIdx.x; i < M; i += LB_THREADS) q[i] = __dadd_rn(q[i], __dmul_rn(s[i], coef));
+  if (tid < hl) { const int sl = (hist_start + tid) % cap; slot_of[tid] = sl; rho[tid] = rho_g[sl]; }
+  __syncthreads();
+  if (tid < 32) {
+    const int lane = tid;
+    for (int j = lane; j < n; j += 32) delta[j] = (j == n - 1) ? 1.0 : 0.0;
+    __syncwarp();
+    for (int t = hl - 1; t >= 0; --t) {                 // newest -> oldest: alpha_t = rho_t s_t.q ; q -= alpha_t y_t
+      double part = 0.0;
+      for (int j = lane; j < n; j += 32) part += delta[j] * Cm[t * n + j];
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
+      const double alv = rho[t] * part;
+      if (lane == 0) { al[t] = alv; delta[hl + t] = __dsub_rn(delta[hl + t], alv); }
+      __syncwarp();
+    }
+    for (int j = lane; j < n; j += 32) delta[j] = __dmul_rn(gamma, delta[j]);    // r = gamma q
+    __syncwarp();
+    for (int t = 0; t < hl; ++t) {                       // oldest -> newest: r += s_t (alpha_t - rho_t y_t.r)
+      double part = 0.0;
+      for (int j = lane; j < n; j += 32) part += delta[j] * Cm[(hl + t) * n + j];
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
+      if (lane == 0) delta[t] = __dadd_rn(delta[t], al[t] - rho[t] * part);
+      __syncwarp();
+    }
   }
-  for (int i = threadIdx.x; i < M; i += LB_THREADS) p[i] = -q[i];
-  return block_dot(g, p, M, scratch);
+  __syncthreads();
+  // combination pass: p = -sum_j delta_j b_j, and g.p in the same sweep
+  const double dg = delta[2 * hl];
+  double gp = 0.0;
+  for (int i = LB_FIRST(r); i < M; i += LB_STEP) {
+    const double gi = g[i];
+    double acc = dg * gi;
+#pragma unroll 4
+    for (int t = 0; t < hl; ++t) {
+      const size_t off = (size_t)slot_of[t] * stride + i;
+      acc += delta[t] * S[off] + delta[hl + t] * Y[off];
+    }
+    const double pi = -acc;
+    p[i] = pi;
+    gp += gi * pi;
+  }
+  return cluster_allsum(gp, r);
 }
 
 __global__ void solve_init_kernel(StepArgs a, const float* w_init, int hist_cap, int max_iters, int max_evals,
@@ -139,13 +283,18 @@ __global__ void solve_init_kernel(StepArgs a, const float* w_init, int hist_cap,
   }
 }
 
-// Runs after every evaluation.  Control flow is uniform over the CTA: every decision is taken on
-// values all threads hold identically (block_allsum results, state scalars read after a sync).
-__global__ void __launch_bounds__(LB_THREADS) lbfgs_step_kernel(StepArgs a) {
-  __shared__ double scratch[LB_THREADS / 32];
-  __shared__ double s_alpha[LB_MAX_HIST];
+// Runs after every evaluation, as one cluster of LB_CLUSTER CTAs.  Control flow is uniform over the cluster: every
+// decision is taken on values all threads hold identically (cluster reductions, state scalars read at entry).
+// Only CTA 0 writes the state scalars, the history trace and the host report.
+__global__ void __cluster_dims__(LB_CLUSTER, 1, 1) __launch_bounds__(LB_THREADS) lbfgs_step_kernel(StepArgs a) {
+  __shared__ double s_wbuf[(LB_THREADS / 32) * LB_NRED];
+  __shared__ double s_cbuf[2 * LB_NRED];
+  extern __shared__ double s_dyn[];        // direction_vf: compact Gram matrix, coefficients (sized by the launch)
+  cg::cluster_group cluster = cg::this_cluster();
+  Reducer red{s_wbuf, s_cbuf, 0, cluster.block_rank()};
   SolveState* st = a.st;
-  if (st->done) return;
+  if (st->done) return;                    // uniform: written by the previous launch
+  const bool lead = red.rank == 0;
   const int M = a.M, stride = a.stride, tid = threadIdx.x;
   double* w = a.vec + (size_t)V_W * stride;
   double* g = a.vec + (size_t)V_G * stride;
@@ -156,47 +305,56 @@ __global__ void __launch_bounds__(LB_THREADS) lbfgs_step_kernel(StepArgs a) {
   double* S = a.vec + (size_t)V_HIST * stride;
   double* Y = S + (size_t)st->hist_cap * stride;
 
-  // copy the scalars (all threads read the same global values before anyone writes them)
+  // copy the scalars (the state is rewritten only at the very end, after several cluster barriers)
   const int phase = st->phase;
   int iters = st->iters, evals = st->evals, trial = st->trial, hist_len = st->hist_len, hist_start = st->hist_start;
   const int cap = st->hist_cap, max_iters = st->max_iters, max_evals = st->max_evals;
   double f = st->f, gp = st->gp, alpha = st->alpha, lo = st->lo, hi = st->hi, gamma = st->gamma;
-  const double eps = st->eps;
+  const double eps = st->eps, domain_volume = st->domain_volume;
   double best_err = st->best_err, best_dual = st->best_dual;
-  const double f1 = -a.e_scal[0], err1 = a.e_scal[1];
-  __syncthreads();
+  float cull_cap = st->cull_cap;
+  const float cull_delta_old = st->cull_delta;
+  const int cull_rebuilds_old = st->cull_rebuilds;
+  const double dual1 = a.e_scal[0], f1 = -dual1, err1 = a.e_scal[1];
 
-  // gradient of f at the evaluated point: vol - v (eq. 2.8)
-  double vsum = 0.0;
-  for (int i = tid; i < M; i += LB_THREADS) {
-    const double tv = (double)a.v[i];
-    gnew[i] = a.e_vol[i] - tv;
-    vsum += tv;
-  }
+  // ONE sweep: gradient of f at the evaluated point, vol - v (eq. 2.8); the best-so-far copy; and, speculatively,
+  // every inner product the line-search tests and the curvature pair need (s = alpha p, y = g1 - g)
   evals += 1;
-  if (tid == 0 && evals <= a.hist_cap) { a.hist[2 * (evals - 1)] = -f1; a.hist[2 * (evals - 1) + 1] = err1; }
+  if (lead && tid == 0 && evals <= a.hist_cap) { a.hist[2 * (evals - 1)] = -f1; a.hist[2 * (evals - 1) + 1] = err1; }
   const double* w_eval = (phase == 0) ? w : wtry;
-  if (err1 < best_err) {
-    best_err = err1; best_dual = -f1;
-    for (int i = tid; i < M; i += LB_THREADS) wbest[i] = w_eval[i];
+  const bool improved = err1 < best_err;
+  if (improved) { best_err = err1; best_dual = -f1; }
+  double sums[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};     // sum v, g1.p, s.y, s.s, y.y, <v, fl32 w>
+  for (int i = LB_FIRST(red); i < M; i += LB_STEP) {
+    const double tv = (double)a.v[i];
+    const double gn = a.e_vol[i] - tv;
+    gnew[i] = gn;
+    sums[0] += tv;
+    if (improved) wbest[i] = w_eval[i];
+    if (phase != 0) {
+      const double pi = p[i];
+      const double si = __dmul_rn(alpha, pi);
+      const double yi = __dsub_rn(gn, g[i]);
+      sums[1] += gn * pi; sums[2] += si * yi; sums[3] += si * si; sums[4] += yi * yi;
+    } else {
+      sums[5] += tv * (double)a.w32[i];
+    }
   }
+  cluster_all<6, false>(sums, red);
+  const double vsum = sums[0], g1p = sums[1], sy = sums[2], ss = sums[3], yy = sums[4];
 
   int finish = 0;          // 1: OK at w_eval, 2: NOT_CONVERGED at best, 3: bad target volumes
   bool need_direction = false;
-  float cull_cap = st->cull_cap;
+  int new_slot = -1;       // ring slot a curvature pair was pushed into by this call, else -1
   if (phase == 0) {
     // cost scale for the list-reuse slack: mean over the voxels of min_i C_ij = (g~ - <v, w>) / |Omega|  (identity I1)
-    double vw = 0.0;
-    for (int i = tid; i < M; i += LB_THREADS) vw += (double)a.v[i] * (double)a.w32[i];
-    vw = block_allsum(vw, scratch);
-    const double scale = fabs(a.e_scal[0] - vw) / st->domain_volume;
+    const double scale = fabs(dual1 - sums[5]) / domain_volume;
     cull_cap = isfinite(scale) ? (float)(CULL_CAP_FACTOR * scale) : 0.0f;
-    vsum = block_allsum(vsum, scratch);
-    if (!(fabs(vsum - st->domain_volume) <= 1e-5 * st->domain_volume)) finish = 3;
+    if (!(fabs(vsum - domain_volume) <= 1e-5 * domain_volume)) finish = 3;
     else if (err1 <= eps) finish = 1;
     else {
       f = f1;
-      for (int i = tid; i < M; i += LB_THREADS) g[i] = gnew[i];
+      for (int i = LB_FIRST(red); i < M; i += LB_STEP) g[i] = gnew[i];
       need_direction = true;
     }
   } else {
@@ -205,7 +363,7 @@ __global__ void __launch_bounds__(LB_THREADS) lbfgs_step_kernel(StepArgs a) {
       bool accepted = false;
       const double armijo_rhs = __dadd_rn(f, __dmul_rn(__dmul_rn(1e-4, alpha), gp));
       if (f1 > armijo_rhs) hi = alpha;
-      else if (block_dot(gnew, p, M, scratch) < __dmul_rn(0.9, gp)) lo = alpha;
+      else if (g1p < __dmul_rn(0.9, gp)) lo = alpha;
       else accepted = true;
       if (!accepted) {
         if (evals >= max_evals) finish = 2;
@@ -218,33 +376,23 @@ __global__ void __launch_bounds__(LB_THREADS) lbfgs_step_kernel(StepArgs a) {
           }
         }
       } else {
-        // s = alpha p, yv = g1 - g  -> candidate curvature pair in the next ring slot
+        // s = alpha p, yv = g1 - g  -> curvature pair in the next ring slot; when the ring is full that slot is
+        // the oldest pair, which is dropped only if the new one is kept
         const int slot = (hist_len < cap) ? (hist_start + hist_len) % cap : hist_start;
         double* s_new = S + (size_t)slot * stride;
         double* y_new = Y + (size_t)slot * stride;
-        double sy = 0.0, ss = 0.0, yy = 0.0;
-        // the pair is first formed in q/gnew-independent temporaries: when the ring is full the
-        // slot being overwritten is the oldest pair, which is dropped only if the new one is kept
-        double* q = a.vec + (size_t)V_Q * stride;
-        for (int i = tid; i < M; i += LB_THREADS) {
-          const double si = __dmul_rn(alpha, p[i]);
-          const double yi = __dsub_rn(gnew[i], g[i]);
-          q[i] = si;
-          sy += si * yi; ss += si * si; yy += yi * yi;
-        }
-        sy = block_allsum(sy, scratch);
-        ss = block_allsum(ss, scratch);
-        yy = block_allsum(yy, scratch);
-        if (sy > 1e-12 * sqrt(ss) * sqrt(yy)) {
-          for (int i = tid; i < M; i += LB_THREADS) {
-            s_new[i] = q[i];
-            y_new[i] = __dsub_rn(gnew[i], g[i]);
-          }
-          if (tid == 0) st->rho[slot] = 1.0 / sy;
+        const bool keep = sy > 1e-12 * sqrt(ss) * sqrt(yy);
+        if (keep) {
+          if (tid == 0) gram_of(a, cap, red.rank)[(size_t)(2 * cap + 1) * (2 * cap + 1) + slot] = 1.0 / sy;   // rho
+          new_slot = slot;
           if (hist_len < cap) hist_len += 1; else hist_start = (hist_start + 1) % cap;
           gamma = sy / yy;
         }
-        for (int i = tid; i < M; i += LB_THREADS) { w[i] = wtry[i]; g[i] = gnew[i]; }
+        for (int i = LB_FIRST(red); i < M; i += LB_STEP) {
+          const double gn = gnew[i];
+          if (keep) { s_new[i] = __dmul_rn(alpha, p[i]); y_new[i] = __dsub_rn(gn, g[i]); }
+          w[i] = wtry[i]; g[i] = gn;
+        }
         f = f1;
         iters += 1;
         if (iters >= max_iters || evals >= max_evals) finish = 2;
@@ -254,11 +402,22 @@ __global__ void __launch_bounds__(LB_THREADS) lbfgs_step_kernel(StepArgs a) {
   }
 
   if (need_direction) {
-    __syncthreads();    // rho / history writes visible
-    gp = new_direction(a, st, hist_len, hist_start, gamma, scratch, s_alpha);
+    if (hist_len > 0) {
+      // refresh the Gram rows that changed: those of the pushed pair (if any) and the row of the new gradient
+      if (new_slot >= 0) {
+        const double* nv[3] = {S + (size_t)new_slot * stride, Y + (size_t)new_slot * stride, g};
+        const int nidx[3] = {new_slot, cap + new_slot, 2 * cap};
+        gram_rows<3>(a, cap, hist_len, hist_start, nv, nidx, red);
+      } else {
+        const double* nv[1] = {g};
+        const int nidx[1] = {2 * cap};
+        gram_rows<1>(a, cap, hist_len, hist_start, nv, nidx, red);
+      }
+    }
+    gp = direction_vf(a, cap, hist_len, hist_start, gamma, red, s_dyn);
     if (gp >= 0.0) {    // safeguard: not a descent direction -> steepest descent scaled by gamma
       hist_len = 0; hist_start = 0;
-      gp = new_direction(a, st, 0, 0, gamma, scratch, s_alpha);
+      gp = direction_vf(a, cap, 0, 0, gamma, red, s_dyn);
     }
     alpha = 1.0; lo = 0.0; hi = INFINITY; trial = 0;
   }
@@ -267,36 +426,36 @@ __global__ void __launch_bounds__(LB_THREADS) lbfgs_step_kernel(StepArgs a) {
   float cull_delta = 0.0f;
   if (finish == 0) {
     // next trial point w + alpha p, rounded to fp32 for the evaluation (S10)
-    double step_max = 0.0, ref_max = 0.0;   // max |change since the last evaluation|, max |distance from wref|
-    for (int i = tid; i < M; i += LB_THREADS) {
+    double mx[2] = {0.0, 0.0};   // max |change since the last evaluation|, max |distance from wref|
+    for (int i = LB_FIRST(red); i < M; i += LB_STEP) {
       const double wt = __dadd_rn(w[i], __dmul_rn(alpha, p[i]));
       wtry[i] = wt;
       const float wn = (float)wt;
-      step_max = fmax(step_max, fabs((double)wn - (double)a.w32[i]));     // differences of floats: exact in fp64
-      ref_max = fmax(ref_max, fabs((double)wn - (double)a.wref[i]));
+      mx[0] = fmax(mx[0], fabs((double)wn - (double)a.w32[i]));     // differences of floats: exact in fp64
+      mx[1] = fmax(mx[1], fabs((double)wn - (double)a.wref[i]));
       a.w32[i] = wn;
     }
-    step_max = block_allmax(step_max, scratch);
-    ref_max = block_allmax(ref_max, scratch);
-    cull_delta = st->cull_delta;
-    cull_rebuild = !(ref_max <= (double)cull_delta);
+    cluster_all<2, true>(mx, red);
+    cull_delta = cull_delta_old;
+    cull_rebuild = !(mx[1] <= (double)cull_delta);
     if (cull_rebuild) {
       // the next evaluation rebuilds its candidate lists at the new weights, valid within delta of them
-      cull_delta = fminf((float)(CULL_DELTA_FACTOR * step_max), cull_cap);
-      for (int i = tid; i < M; i += LB_THREADS) a.wref[i] = a.w32[i];
+      cull_delta = fminf((float)(CULL_DELTA_FACTOR * mx[0]), cull_cap);
+      for (int i = LB_FIRST(red); i < M; i += LB_STEP) a.wref[i] = a.w32[i];
     }
   } else if (finish == 1) {
-    if (phase != 0) for (int i = tid; i < M; i += LB_THREADS) w[i] = wtry[i];
+    if (phase != 0) for (int i = LB_FIRST(red); i < M; i += LB_STEP) w[i] = wtry[i];
   } else if (finish == 2) {
-    for (int i = tid; i < M; i += LB_THREADS) { w[i] = wbest[i]; a.w32[i] = (float)wbest[i]; }
+    for (int i = LB_FIRST(red); i < M; i += LB_STEP) { w[i] = wbest[i]; a.w32[i] = (float)wbest[i]; }
   }
-  __syncthreads();
-  if (tid == 0) {
+  cluster.sync();        // no CTA leaves while its shared memory may still be read; all vector writes are done
+  if (lead && tid == 0) {
     st->phase = 1; st->iters = iters; st->evals = evals; st->trial = trial;
     st->hist_len = hist_len; st->hist_start = hist_start;
     st->f = f; st->gp = gp; st->alpha = alpha; st->lo = lo; st->hi = hi; st->gamma = gamma;
     st->best_err = best_err; st->best_dual = best_dual;
-    st->cull_cap = cull_cap; st->cull_rebuild = cull_rebuild; st->cull_delta = cull_delta; st->cull_rebuilds += (finish == 0 && cull_rebuild);
+    st->cull_cap = cull_cap; st->cull_rebuild = cull_rebuild; st->cull_delta = cull_delta;
+    st->cull_rebuilds = cull_rebuilds_old + (finish == 0 && cull_rebuild);
     if (finish) {
       st->done = 1;
       a.report->status = (finish == 1) ? APD_OK : (finish == 2 ? APD_NOT_CONVERGED : APD_E_ARG);
@@ -341,6 +500,8 @@ static int ensure_solve_state(apd_ctx* ctx, int hist) {
   if (!ws.svec || ws.svec_hist < hist) {
     if (ws.svec) { LB_TRY(cudaDeviceSynchronize()); LB_TRY(cudaFree(ws.svec)); ws.svec = nullptr; }
     LB_TRY(cudaMalloc(&ws.svec, (size_t)(V_HIST + 2 * hist) * ms * sizeof(double)));
+    cudaFree(ws.gram); ws.gram = nullptr;
+    LB_TRY(cudaMalloc(&ws.gram, (size_t)LB_CLUSTER * ((size_t)(2 * hist + 1) * (2 * hist + 1) + hist) * sizeof(double)));
     ws.svec_hist = hist;
   }
   return APD_OK;
@@ -391,6 +552,12 @@ extern "C" int apd_solve(apd_ctx* ctx, const apd_grid* grid, int32_t M, const fl
                                                     gamma0, domain);
   LB_TRY(cudaGetLastError());
 
+  // dynamic shared memory of the step kernel: compact Gram matrix + coefficient vectors of direction_vf
+  const size_t nb = 2 * (size_t)o.lbfgs_history + 1;
+  const size_t dyn_bytes = (nb * nb + nb + 2 * (size_t)o.lbfgs_history) * sizeof(double) + (size_t)o.lbfgs_history * sizeof(int);
+  if (dyn_bytes > 32 * 1024)
+    LB_TRY(cudaFuncSetAttribute(lbfgs_step_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn_bytes));
+  sa.gram = ws.gram;
   const int* done_flag = &ws.sstate->done;
   long long enq = 0;
   const long long hard_cap = (long long)max_evals + 64;
@@ -399,7 +566,7 @@ extern "C" int apd_solve(apd_ctx* ctx, const apd_grid* grid, int32_t M, const fl
                             ws.e_scal + 1, nullptr, nullptr, false, o.cull != 0, done_flag, st, &ws.sstate->cull_rebuild,
                             &ws.sstate->cull_delta);
     if (rc != APD_OK) return rc;
-    lbfgs_step_kernel<<<1, LB_THREADS, 0, st>>>(sa);
+    lbfgs_step_kernel<<<LB_CLUSTER, LB_THREADS, dyn_bytes, st>>>(sa);
     LB_TRY(cudaGetLastError());
     LB_TRY(cudaEventRecord(ws.sev[enq & 1], st));
     if (enq >= 1) {
