@@ -147,7 +147,9 @@ int enqueue_evaluation(apd_ctx* ctx, const GridDev& g, int kernel, int M, const 
     ws.partial_cap = (size_t)n_partials;
     APD_CUDA_TRY(ctx, cudaMalloc(&ws.dual_partial, ws.partial_cap * sizeof(double)));
   }
-  if (kernel == APD_KERNEL_ROWPOLY)
+  if (cull) {
+    // the culled kernel reads the per-seed record table that launch_cull packs (and which zeroes the accumulators)
+  } else if (kernel == APD_KERNEL_ROWPOLY)
     APD_CUDA_TRY(ctx, launch_pack_pairs(g.dim, M, M_pad, X, A, w, ws.seeds, ws.count,
                                         centroids ? ws.idxsum : nullptr, done_flag, st));
   else
@@ -182,15 +184,17 @@ int enqueue_evaluation(apd_ctx* ctx, const GridDev& g, int kernel, int M, const 
       ws.brick_cap_n = n_bricks; ws.super_cap_n = n_super;
     }
     CullBuffers cb{ws.rec, ws.brick_list, ws.brick_count, ws.super_list, ws.super_count, ws.pairs_ctr};
-    APD_CUDA_TRY(ctx, launch_cull(g, M, M_pad, X, A, w, cb, nsx, nsy, nsz, done_flag, cull_rebuild, cull_delta, st));
+    APD_CUDA_TRY(ctx, launch_cull(g, M, M_pad, X, A, w, cb, nsx, nsy, nsz, ws.count, centroids ? ws.idxsum : nullptr, done_flag,
+                                  cull_rebuild, cull_delta, st));
     a.rec = ws.rec; a.brick_list = ws.brick_list; a.brick_count = ws.brick_count; a.super_list = ws.super_list;
     a.super_count = ws.super_count; a.super_x = nsx; a.super_y = nsy; a.pairs_ctr = ws.pairs_ctr;
   }
   if (timed) APD_CUDA_TRY(ctx, cudaEventRecord(ws.ev0, st));
   APD_CUDA_TRY(ctx, launch_assign(kernel, a, st));
   if (timed) { APD_CUDA_TRY(ctx, cudaEventRecord(ws.ev1, st)); ws.timed = true; }
-  APD_CUDA_TRY(ctx, launch_finalize(g, M, n_partials, ws.count, a.idxsum, ws.dual_partial, X, w, target_vol, vol,
-                                    dual, max_rel_err, centroids, pairs, cull ? ws.pairs_ctr : nullptr, done_flag, st));
+  if (vol)     // apd_solve's loop passes vol == nullptr: lbfgs_step_kernel finishes the evaluation itself
+    APD_CUDA_TRY(ctx, launch_finalize(g, M, n_partials, ws.count, a.idxsum, ws.dual_partial, X, w, target_vol, vol,
+                                      dual, max_rel_err, centroids, pairs, cull ? ws.pairs_ctr : nullptr, done_flag, st));
   return APD_OK;
 }
 

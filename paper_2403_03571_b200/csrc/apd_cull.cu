@@ -43,11 +43,16 @@ __device__ __forceinline__ float box_radius(const float* r, float hx, float hy, 
 template <int DIM>
 __global__ void cull_pack_kernel(int M, int M_pad, const float* __restrict__ X, const float* __restrict__ A,
                                  const float* __restrict__ w, float3 hb, float3 hs, float* __restrict__ rec,
-                                 unsigned long long* __restrict__ pairs_ctr, const int* __restrict__ done_flag) {
+                                 unsigned long long* __restrict__ pairs_ctr, unsigned int* __restrict__ count,
+                                 unsigned long long* __restrict__ idxsum, const int* __restrict__ done_flag) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (done_flag && *done_flag) return;
   if (i == 0) *pairs_ctr = 0ull;
   if (i >= M_pad) return;
+  if (i < M) {      // the integer accumulators of the evaluation (the culled path runs no other pack kernel)
+    count[i] = 0u;
+    if (idxsum) { idxsum[i * 3 + 0] = 0ull; idxsum[i * 3 + 1] = 0ull; idxsum[i * 3 + 2] = 0ull; }
+  }
   constexpr int REC = (DIM == 3) ? REC3 : REC2;
   constexpr int NP = (DIM == 3) ? 10 : 6;
   float r[REC];
@@ -328,8 +333,9 @@ void cull_super_counts(const GridDev& g, int* nsx, int* nsy, int* nsz) {
 }
 
 cudaError_t launch_cull(const GridDev& g, int M, int M_pad, const float* X, const float* A, const float* w,
-                        const CullBuffers& cb, int nsx, int nsy, int nsz, const int* done_flag, const int* rebuild,
-                        const float* delta, cudaStream_t st) {
+                        const CullBuffers& cb, int nsx, int nsy, int nsz, unsigned int* count,
+                        unsigned long long* idxsum, const int* done_flag, const int* rebuild, const float* delta,
+                        cudaStream_t st) {
   // half-extents of the boxes of voxel CENTRES of a brick and of a super-tile
   int ox, oy, oz, ex, ey, ez;
   brick_box(g.dim, 0, &ox, &oy, &oz, &ex, &ey, &ez);
@@ -340,8 +346,8 @@ cudaError_t launch_cull(const GridDev& g, int M, int M_pad, const float* X, cons
   const float3 hb = make_float3(half(ex, 0), half(ey, 1), g.dim == 3 ? half(ez, 2) : 0.0f);
   const float3 hs = make_float3(half(sex, 0), half(sey, 1), g.dim == 3 ? half(sez, 2) : 0.0f);
   const int nb = (M_pad + 127) / 128;
-  if (g.dim == 3) cull_pack_kernel<3><<<nb, 128, 0, st>>>(M, M_pad, X, A, w, hb, hs, cb.rec, cb.pairs_ctr, done_flag);
-  else            cull_pack_kernel<2><<<nb, 128, 0, st>>>(M, M_pad, X, A, w, hb, hs, cb.rec, cb.pairs_ctr, done_flag);
+  if (g.dim == 3) cull_pack_kernel<3><<<nb, 128, 0, st>>>(M, M_pad, X, A, w, hb, hs, cb.rec, cb.pairs_ctr, count, idxsum, done_flag);
+  else            cull_pack_kernel<2><<<nb, 128, 0, st>>>(M, M_pad, X, A, w, hb, hs, cb.rec, cb.pairs_ctr, count, idxsum, done_flag);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
   CullArgs c;

@@ -130,8 +130,9 @@ struct CullBuffers {
   unsigned long long* pairs_ctr;
 };
 cudaError_t launch_cull(const GridDev& g, int M, int M_pad, const float* X, const float* A, const float* w,
-                        const CullBuffers& cb, int n_super_x, int n_super_y, int n_super_z, const int* done_flag,
-                        const int* rebuild, const float* delta, cudaStream_t st);
+                        const CullBuffers& cb, int n_super_x, int n_super_y, int n_super_z, unsigned int* count,
+                        unsigned long long* idxsum, const int* done_flag, const int* rebuild, const float* delta,
+                        cudaStream_t st);
 void cull_super_counts(const GridDev& g, int* nsx, int* nsy, int* nsz);
 int rowpoly_tile_counts(int dim, int nx, int ny, int nz, int sm_count, bool cull, int* tx, int* ty, int* tz);
 int assign_tile_counts(int kernel, int dim, int nx, int ny, int nz, int sm_count, bool cull, int* tx, int* ty, int* tz);

@@ -45,8 +45,11 @@ struct StepArgs {
   int stride;          // = max_seeds
   int M;
   const float* v;      // target volumes
-  const double* e_vol; // evaluation outputs
-  const double* e_scal;  // [0] dual, [1] max_rel_err
+  // raw outputs of the evaluation just run (the loop skips finalize_kernel and finishes eq. 2.7 / 2.8 / 2.5 here)
+  const unsigned int* count;      // [M] voxels per cell
+  const double* dual_partial;     // [n_partials] sums of min-costs
+  int n_partials;
+  double voxel_volume;            // |P|
   float* w32;          // next evaluation's weights
   SolveReport* report; // mapped host memory
   double* hist;        // [2 * hist_cap] (dual, max_rel_err) of every evaluation, in order
@@ -315,7 +318,20 @@ __global__ void __cluster_dims__(LB_CLUSTER, 1, 1) __launch_bounds__(LB_THREADS)
   float cull_cap = st->cull_cap;
   const float cull_delta_old = st->cull_delta;
   const int cull_rebuilds_old = st->cull_rebuilds;
-  const double dual1 = a.e_scal[0], f1 = -dual1, err1 = a.e_scal[1];
+
+  // a9 for the loop: g~ = <v, fl32 w> + |P| sum_j min_i C_ij (identity I1), eq. (2.5) error
+  const double P = a.voxel_volume;
+  double s0[2] = {0.0, 0.0};
+  double emax = 0.0;
+  for (int i = LB_FIRST(red); i < M; i += LB_STEP) {
+    const double tv = (double)a.v[i];
+    s0[0] += tv * (double)a.w32[i];
+    emax = fmax(emax, fabs((double)a.count[i] * P - tv) / tv);
+  }
+  for (int t = LB_FIRST(red); t < a.n_partials; t += LB_STEP) s0[1] += a.dual_partial[t];
+  cluster_all<2, false>(s0, red);
+  const double err1 = cluster_allmax(emax, red);
+  const double dual1 = s0[0] + P * s0[1], f1 = -dual1;
 
   // ONE sweep: gradient of f at the evaluated point, vol - v (eq. 2.8); the best-so-far copy; and, speculatively,
   // every inner product the line-search tests and the curvature pair need (s = alpha p, y = g1 - g)
@@ -324,10 +340,10 @@ __global__ void __cluster_dims__(LB_CLUSTER, 1, 1) __launch_bounds__(LB_THREADS)
   const double* w_eval = (phase == 0) ? w : wtry;
   const bool improved = err1 < best_err;
   if (improved) { best_err = err1; best_dual = -f1; }
-  double sums[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};     // sum v, g1.p, s.y, s.s, y.y, <v, fl32 w>
+  double sums[5] = {0.0, 0.0, 0.0, 0.0, 0.0};     // sum v, g1.p, s.y, s.s, y.y
   for (int i = LB_FIRST(red); i < M; i += LB_STEP) {
     const double tv = (double)a.v[i];
-    const double gn = a.e_vol[i] - tv;
+    const double gn = (double)a.count[i] * P - tv;      // m_i |P| - v_i
     gnew[i] = gn;
     sums[0] += tv;
     if (improved) wbest[i] = w_eval[i];
@@ -336,11 +352,9 @@ __global__ void __cluster_dims__(LB_CLUSTER, 1, 1) __launch_bounds__(LB_THREADS)
       const double si = __dmul_rn(alpha, pi);
       const double yi = __dsub_rn(gn, g[i]);
       sums[1] += gn * pi; sums[2] += si * yi; sums[3] += si * si; sums[4] += yi * yi;
-    } else {
-      sums[5] += tv * (double)a.w32[i];
     }
   }
-  cluster_all<6, false>(sums, red);
+  cluster_all<5, false>(sums, red);
   const double vsum = sums[0], g1p = sums[1], sy = sums[2], ss = sums[3], yy = sums[4];
 
   int finish = 0;          // 1: OK at w_eval, 2: NOT_CONVERGED at best, 3: bad target volumes
@@ -348,7 +362,7 @@ __global__ void __cluster_dims__(LB_CLUSTER, 1, 1) __launch_bounds__(LB_THREADS)
   int new_slot = -1;       // ring slot a curvature pair was pushed into by this call, else -1
   if (phase == 0) {
     // cost scale for the list-reuse slack: mean over the voxels of min_i C_ij = (g~ - <v, w>) / |Omega|  (identity I1)
-    const double scale = fabs(dual1 - sums[5]) / domain_volume;
+    const double scale = fabs(P * s0[1]) / domain_volume;
     cull_cap = isfinite(scale) ? (float)(CULL_CAP_FACTOR * scale) : 0.0f;
     if (!(fabs(vsum - domain_volume) <= 1e-5 * domain_volume)) finish = 3;
     else if (err1 <= eps) finish = 1;
@@ -541,7 +555,8 @@ extern "C" int apd_solve(apd_ctx* ctx, const apd_grid* grid, int32_t M, const fl
 
   StepArgs sa;
   sa.st = ws.sstate; sa.vec = ws.svec; sa.stride = ws.max_seeds; sa.M = M; sa.v = target_vol;
-  sa.e_vol = ws.e_vol; sa.e_scal = ws.e_scal; sa.w32 = ws.w32;
+  sa.count = ws.count; sa.voxel_volume = g.voxel_volume; sa.w32 = ws.w32;
+  sa.n_partials = (o.cull ? 4 : 1) * g.tiles_x * g.tiles_y * g.tiles_z;
   sa.hist = ws.hist; sa.hist_cap = SOLVE_HIST_CAP; sa.wref = ws.wref;
   ws.hist_len = 0;
   SolveReport* dev_report = nullptr;
@@ -562,10 +577,11 @@ extern "C" int apd_solve(apd_ctx* ctx, const apd_grid* grid, int32_t M, const fl
   long long enq = 0;
   const long long hard_cap = (long long)max_evals + 64;
   for (;; ++enq) {
-    rc = enqueue_evaluation(ctx, g, kernel, M, X, A, ws.w32, target_vol, nullptr, ws.e_vol, ws.e_scal,
-                            ws.e_scal + 1, nullptr, nullptr, false, o.cull != 0, done_flag, st, &ws.sstate->cull_rebuild,
+    rc = enqueue_evaluation(ctx, g, kernel, M, X, A, ws.w32, target_vol, nullptr, nullptr, nullptr,
+                            nullptr, nullptr, nullptr, false, o.cull != 0, done_flag, st, &ws.sstate->cull_rebuild,
                             &ws.sstate->cull_delta);
     if (rc != APD_OK) return rc;
+    sa.dual_partial = ws.dual_partial;       // (re)allocated by the first enqueue_evaluation
     lbfgs_step_kernel<<<LB_CLUSTER, LB_THREADS, dyn_bytes, st>>>(sa);
     LB_TRY(cudaGetLastError());
     LB_TRY(cudaEventRecord(ws.sev[enq & 1], st));
