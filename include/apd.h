@@ -55,9 +55,16 @@ enum {
                               argmin                                                                */
 };
 
+/* opts.cull = 1: exact culling (not in the paper).  Per block of voxels the library keeps only
+ * the seeds that can be an argmin somewhere in the block (bounds from the triangle inequality in the A_i-norm, taken
+ * conservatively in fp32), nested super-tile -> tile -> 16x4x8-voxel brick, and evaluates those.  The labels are those
+ * of the brute-force reduction with the same fp32 arithmetic (identical bit for bit whenever brute force runs the same
+ * short-row kernel, i.e. on grids below ~10^3 long-row tiles; on larger grids the two can differ on fp32 near-ties).
+ * Requires kernel AUTO or ROWPOLY and positive definite A_i (not checked).  Workspace grows by
+ * O(number of bricks): 1 KiB per 512 voxels.  pairs_evaluated reports the pairs actually evaluated. */
 typedef struct {
   int32_t kernel;          /* APD_KERNEL_*                                   default AUTO         */
-  int32_t cull;            /* 0 brute force, 1 exact conservative tile culling  default 0         */
+  int32_t cull;            /* 0 brute force, 1 exact conservative culling      default 0          */
   int32_t lbfgs_history;   /* m of L-BFGS                                     default 10          */
   int32_t max_iters;       /* apd_solve iteration limit                       default 1000        */
   int32_t max_evals;       /* apd_solve evaluation limit; 0 = 20*max_iters    default 0           */
