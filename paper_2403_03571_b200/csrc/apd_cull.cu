@@ -7,6 +7,8 @@
 //        max(0, s_i - rho_i)^2 - w_i  <=  C_i(y) = |y - x_i|^2_{A_i} - w_i  <=  (s_i + rho_i)^2 - w_i .
 // With U_T = min_k (s_k + rho_k)^2 - w_k, a seed whose lower bound exceeds U_T is beaten at EVERY voxel of the tile by
 // the seed attaining U_T, so it is never an argmin and can be skipped: the labels are those of brute force.
+// The kernels use two sharper forms of the same bounds (lower_bound(): support function of the box along the
+// A-gradient; exact_upper(): exact corner maximum of the best seed's cost) -- derivations at the functions.
 // All bounds are taken in fp32 with a relative slack of 2^-16 on every term, three orders above the rounding of the
 // fp32 cost evaluation, so rounding can never prune a winner (test: labels with culling == labels without, bit-exact).
 // A must be positive definite for the bound to hold (PAPER.md:51-54 assumes it; the library does not check).
@@ -89,7 +91,7 @@ struct CullArgs {
   int nsx, nsy, nsz;       // super-tiles per axis
   int* brick_list;         // [n_tiles * 4, BRICK_CAP]
   int* brick_count;        // [n_tiles * 4]
-  float3 ht;               // half-extents of the box of voxel centres of a CTA tile
+  float3 hb, ht, hs;       // half-extents of the boxes of voxel centres of a brick, a CTA tile, a super-tile
   const int* done_flag;
   // list reuse inside apd_solve: the lists are rebuilt only when *rebuild != 0, with the slack *delta on both
   // bounds, which keeps them valid for every w' with max_i |w'_i - w_i| <= delta.  nullptr: always rebuild, delta 0.
@@ -97,22 +99,26 @@ struct CullArgs {
   const float* delta;
 };
 
-// s_i = |y0 - x_i|_{A_i}, rho_i (SLOT 0 = brick, 1 = super-tile: stored; 2 = box of half-extents ht: computed) and
-// -w_i of one seed
+// For one seed and a box y0 +- h:  s_i = |y0 - x_i|_{A_i};  rho_i = max_corners |(+-h)|_{A_i} (SLOT 0 = brick,
+// 1 = super-tile: stored in the record; 2 = computed);  supp_i = max_{|t_k| <= h_k} t^T A_i (y0 - x_i)
+// = sum_k |(A_i (y0 - x_i))_k| h_k, the support function of the box along the A-gradient at the centre;  -w_i.
 template <int DIM, int SLOT>
 __device__ __forceinline__ void seed_bounds(const float* __restrict__ rec, int i, float y0x, float y0y, float y0z,
-                                            float* s, float* rho, float* nw, float3 ht = make_float3(0.f, 0.f, 0.f)) {
+                                            float3 h, float* s, float* rho, float* supp, float* nw) {
   if (DIM == 3) {
     const float4* p = reinterpret_cast<const float4*>(rec + (size_t)i * REC3);
     const float4 p0 = __ldg(p), p1 = __ldg(p + 1), p2 = __ldg(p + 2);
     const float dx = y0x - p0.x, dy = y0y - p0.y, dz = y0z - p0.z;
-    float q = dx * fmaf(p1.y, dz, fmaf(p1.x, dy, p0.w * dx));
-    q = fmaf(dy, fmaf(p1.w, dz, p1.z * dy), q);
-    q = fmaf(dz, p2.x * dz, q);
+    // g = A d with the symmetric matrix (the record holds doubled off-diagonals)
+    const float gx = fmaf(0.5f * p1.y, dz, fmaf(0.5f * p1.x, dy, p0.w * dx));
+    const float gy = fmaf(0.5f * p1.w, dz, fmaf(p1.z, dy, 0.5f * p1.x * dx));
+    const float gz = fmaf(p2.x, dz, fmaf(0.5f * p1.w, dy, 0.5f * p1.y * dx));
+    const float q = fmaf(dz, gz, fmaf(dy, gy, dx * gx));
     *s = sqrtf(fmaxf(q, 0.0f)); *nw = p2.y;
+    *supp = fmaf(fabsf(gz), h.z, fmaf(fabsf(gy), h.y, fabsf(gx) * h.x));
     if (SLOT == 2) {
       const float r[9] = {0.f, 0.f, 0.f, p0.w, p1.x, p1.y, p1.z, p1.w, p2.x};
-      *rho = box_radius<3>(r, ht.x, ht.y, ht.z);
+      *rho = box_radius<3>(r, h.x, h.y, h.z);
     } else {
       *rho = SLOT ? p2.w : p2.z;
     }
@@ -120,12 +126,14 @@ __device__ __forceinline__ void seed_bounds(const float* __restrict__ rec, int i
     const float4* p = reinterpret_cast<const float4*>(rec + (size_t)i * REC2);
     const float4 p0 = __ldg(p), p1 = __ldg(p + 1);
     const float dx = y0x - p0.x, dy = y0y - p0.y;
-    float q = dx * fmaf(p0.w, dy, p0.z * dx);
-    q = fmaf(dy, p1.x * dy, q);
+    const float gx = fmaf(0.5f * p0.w, dy, p0.z * dx);
+    const float gy = fmaf(p1.x, dy, 0.5f * p0.w * dx);
+    const float q = fmaf(dy, gy, dx * gx);
     *s = sqrtf(fmaxf(q, 0.0f)); *nw = p1.y;
+    *supp = fmaf(fabsf(gy), h.y, fabsf(gx) * h.x);
     if (SLOT == 2) {
       const float r[5] = {0.f, 0.f, p0.z, p0.w, p1.x};
-      *rho = box_radius<2>(r, ht.x, ht.y, 0.0f);
+      *rho = box_radius<2>(r, h.x, h.y, 0.0f);
     } else {
       *rho = SLOT ? p1.w : p1.z;
     }
@@ -136,9 +144,62 @@ __device__ __forceinline__ float upper_bound(float s, float rho, float nw) {
   const float r = s * (1.0f + CULL_EPS) + rho;
   return r * r * (1.0f + CULL_EPS) + nw + CULL_EPS * fabsf(nw);
 }
-__device__ __forceinline__ float lower_bound(float s, float rho, float nw) {
-  const float r = fmaxf(s * (1.0f - CULL_EPS) - rho, 0.0f);
+// Cauchy-Schwarz in the A-inner product: |d0 + t|_A >= <d0 + t, d0>_A / |d0|_A = s + t^T A d0 / s >= s - supp / s
+// (this dominates the ball bound s - rho, since supp <= rho s).  s = 0 gives 0 (fmaxf drops the NaN of 0/0).
+__device__ __forceinline__ float lower_bound(float s, float supp, float nw) {
+  const float r = fmaxf(s * (1.0f - CULL_EPS) - supp * (1.0f + 4.0f * CULL_EPS) / s, 0.0f);
   return r * r * (1.0f - CULL_EPS) + nw - CULL_EPS * fabsf(nw);
+}
+
+// EXACT maximum over the box y0 +- h of C_k = |y - x_k|^2_{A_k} - w_k (plus rounding slack): the cost is convex, so
+// the maximum sits at a corner; with d = y0 - x_k, g = A d:  C_k(y0 + t) = d.g + 2 g.t + t^T A t - w_k.
+// Used for the ONE seed that attains the smallest ball bound of a box: its true worst case is a valid, tighter U.
+template <int DIM>
+__device__ __forceinline__ float exact_upper(const float* __restrict__ rec, int k, float y0x, float y0y, float y0z,
+                                             float3 h) {
+  if (DIM == 3) {
+    const float4* p = reinterpret_cast<const float4*>(rec + (size_t)k * REC3);
+    const float4 p0 = __ldg(p), p1 = __ldg(p + 1), p2 = __ldg(p + 2);
+    const float dx = y0x - p0.x, dy = y0y - p0.y, dz = y0z - p0.z;
+    const float gx = fmaf(0.5f * p1.y, dz, fmaf(0.5f * p1.x, dy, p0.w * dx));
+    const float gy = fmaf(0.5f * p1.w, dz, fmaf(p1.z, dy, 0.5f * p1.x * dx));
+    const float gz = fmaf(p2.x, dz, fmaf(0.5f * p1.w, dy, 0.5f * p1.y * dx));
+    const float q = fmaxf(fmaf(dz, gz, fmaf(dy, gy, dx * gx)), 0.0f);
+    const float lx = 2.0f * gx * h.x, ly = 2.0f * gy * h.y, lz = 2.0f * gz * h.z;
+    const float dg = p0.w * h.x * h.x + p1.z * h.y * h.y + p2.x * h.z * h.z;
+    const float p12 = p1.x * h.x * h.y, p13 = p1.y * h.x * h.z, p23 = p1.w * h.y * h.z;
+    float m = -CUDART_INF_F;
+#pragma unroll
+    for (int c = 0; c < 8; ++c) {
+      const float sx = (c & 1) ? -1.f : 1.f, sy = (c & 2) ? -1.f : 1.f, sz = (c & 4) ? -1.f : 1.f;
+      m = fmaxf(m, sx * lx + sy * ly + sz * lz + sx * sy * p12 + sx * sz * p13 + sy * sz * p23);
+    }
+    const float mag = q + fabsf(lx) + fabsf(ly) + fabsf(lz) + dg + fabsf(p12) + fabsf(p13) + fabsf(p23);
+    return q + dg + m + 8.0f * CULL_EPS * mag + p2.y + CULL_EPS * fabsf(p2.y);
+  } else {
+    const float4* p = reinterpret_cast<const float4*>(rec + (size_t)k * REC2);
+    const float4 p0 = __ldg(p), p1 = __ldg(p + 1);
+    const float dx = y0x - p0.x, dy = y0y - p0.y;
+    const float gx = fmaf(0.5f * p0.w, dy, p0.z * dx);
+    const float gy = fmaf(p1.x, dy, 0.5f * p0.w * dx);
+    const float q = fmaxf(fmaf(dy, gy, dx * gx), 0.0f);
+    const float lx = 2.0f * gx * h.x, ly = 2.0f * gy * h.y;
+    const float dg = p0.z * h.x * h.x + p1.x * h.y * h.y;
+    const float p12 = p0.w * h.x * h.y;
+    const float m = fmaxf(fmaxf(lx + ly + p12, -lx - ly + p12), fmaxf(lx - ly - p12, -lx + ly - p12));
+    const float mag = q + fabsf(lx) + fabsf(ly) + dg + fabsf(p12);
+    return q + dg + m + 8.0f * CULL_EPS * mag + p1.y + CULL_EPS * fabsf(p1.y);
+  }
+}
+
+// (value, index) minimum over a warp; ties to the lower index
+__device__ __forceinline__ void warp_argmin(float& v, int& i) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    const float ov = __shfl_xor_sync(0xffffffffu, v, o);
+    const int oi = __shfl_xor_sync(0xffffffffu, i, o);
+    if (ov < v || (ov == v && oi < i)) { v = ov; i = oi; }
+  }
 }
 
 // centre, along one axis, of the box spanned by the centres of voxels i0 .. i0+e-1
@@ -151,6 +212,7 @@ __device__ __forceinline__ float box_centre(double lo, double s, int i0, int e) 
 template <int DIM>
 __global__ void __launch_bounds__(CULL_THREADS) cull_super_kernel(const CullArgs c) {
   __shared__ float s_min[CULL_THREADS / 32];
+  __shared__ int s_imin[CULL_THREADS / 32];
   __shared__ int s_wsum[CULL_THREADS / 32];
   __shared__ float s_U;
   if (c.done_flag && *c.done_flag) return;
@@ -167,20 +229,22 @@ __global__ void __launch_bounds__(CULL_THREADS) cull_super_kernel(const CullArgs
   const float y0z = (DIM == 3) ? box_centre(c.g.lo[2], c.g.s[2], sz * EZ, EZ) : 0.0f;
 
   float umin = CUDART_INF_F;
+  int imin = 0;
   for (int i = tid; i < c.M; i += CULL_THREADS) {
-    float s, rho, nw;
-    seed_bounds<DIM, 1>(c.rec, i, y0x, y0y, y0z, &s, &rho, &nw);
-    umin = fminf(umin, upper_bound(s, rho, nw));
+    float s, rho, supp, nw;
+    seed_bounds<DIM, 1>(c.rec, i, y0x, y0y, y0z, c.hs, &s, &rho, &supp, &nw);
+    const float u = upper_bound(s, rho, nw);
+    if (u < umin) { umin = u; imin = i; }
   }
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) umin = fminf(umin, __shfl_xor_sync(0xffffffffu, umin, o));
-  if (lane == 0) s_min[wid] = umin;
+  warp_argmin(umin, imin);
+  if (lane == 0) { s_min[wid] = umin; s_imin[wid] = imin; }
   __syncthreads();
   if (tid == 0) {
     float u = s_min[0];
+    int k = s_imin[0];
 #pragma unroll
-    for (int k = 1; k < CULL_THREADS / 32; ++k) u = fminf(u, s_min[k]);
-    s_U = u;
+    for (int j = 1; j < CULL_THREADS / 32; ++j) if (s_min[j] < u) { u = s_min[j]; k = s_imin[j]; }
+    s_U = fminf(u, exact_upper<DIM>(c.rec, k, y0x, y0y, y0z, c.hs));
   }
   __syncthreads();
   const float U = s_U + 2.0f * delta * (1.0f + CULL_EPS);
@@ -191,9 +255,9 @@ __global__ void __launch_bounds__(CULL_THREADS) cull_super_kernel(const CullArgs
     const int i = i0 + tid;
     bool keep = false;
     if (i < c.M) {
-      float s, rho, nw;
-      seed_bounds<DIM, 1>(c.rec, i, y0x, y0y, y0z, &s, &rho, &nw);
-      keep = !(lower_bound(s, rho, nw) > U);       // NaN keeps the seed
+      float s, rho, supp, nw;
+      seed_bounds<DIM, 1>(c.rec, i, y0x, y0y, y0z, c.hs, &s, &rho, &supp, &nw);
+      keep = !(lower_bound(s, supp, nw) > U);      // NaN keeps the seed
     }
     const unsigned int bal = __ballot_sync(0xffffffffu, keep);
     if (lane == 0) s_wsum[wid] = __popc(bal);
@@ -220,6 +284,7 @@ template <int DIM>
 __global__ void __launch_bounds__(128) cull_bricks_kernel(const CullArgs c) {
   __shared__ int s_tile[TILE_CAP];
   __shared__ float s_min[4];
+  __shared__ int s_imin[4];
   __shared__ int s_wsum[4];
   if (c.done_flag && *c.done_flag) return;
   if (c.rebuild && !*c.rebuild) return;
@@ -242,17 +307,23 @@ __global__ void __launch_bounds__(128) cull_bricks_kernel(const CullArgs c) {
     const float t0y = box_centre(c.g.lo[1], c.g.s[1], by * TY, TY);
     const float t0z = (DIM == 3) ? box_centre(c.g.lo[2], c.g.s[2], bz * TZ, TZ) : 0.0f;
     float umin = CUDART_INF_F;
+    int imin = 0;
     for (int pos = tid; pos < n; pos += 128) {
       const int i = plist ? __ldg(plist + pos) : pos;
-      float s, rho, nw;
-      seed_bounds<DIM, 2>(c.rec, i, t0x, t0y, t0z, &s, &rho, &nw, c.ht);
-      umin = fminf(umin, upper_bound(s, rho, nw));
+      float s, rho, supp, nw;
+      seed_bounds<DIM, 2>(c.rec, i, t0x, t0y, t0z, c.ht, &s, &rho, &supp, &nw);
+      const float u = upper_bound(s, rho, nw);
+      if (u < umin) { umin = u; imin = i; }
     }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) umin = fminf(umin, __shfl_xor_sync(0xffffffffu, umin, o));
-    if (lane == 0) s_min[w] = umin;
+    warp_argmin(umin, imin);
+    if (lane == 0) { s_min[w] = umin; s_imin[w] = imin; }
     __syncthreads();
-    const float U = fminf(fminf(s_min[0], s_min[1]), fminf(s_min[2], s_min[3])) + 2.0f * delta * (1.0f + CULL_EPS);
+    float U = s_min[0];
+    int kbest = s_imin[0];
+#pragma unroll
+    for (int j = 1; j < 4; ++j) if (s_min[j] < U) { U = s_min[j]; kbest = s_imin[j]; }
+    if (n > 0) U = fminf(U, exact_upper<DIM>(c.rec, kbest, t0x, t0y, t0z, c.ht));
+    U += 2.0f * delta * (1.0f + CULL_EPS);
     int base = 0;
     for (int p0 = 0; p0 < n; p0 += 128) {
       const int pos = p0 + tid;
@@ -260,9 +331,9 @@ __global__ void __launch_bounds__(128) cull_bricks_kernel(const CullArgs c) {
       int i = 0;
       if (pos < n) {
         i = plist ? __ldg(plist + pos) : pos;
-        float s, rho, nw;
-        seed_bounds<DIM, 2>(c.rec, i, t0x, t0y, t0z, &s, &rho, &nw, c.ht);
-        keep = !(lower_bound(s, rho, nw) > U);
+        float s, rho, supp, nw;
+        seed_bounds<DIM, 2>(c.rec, i, t0x, t0y, t0z, c.ht, &s, &rho, &supp, &nw);
+        keep = !(lower_bound(s, supp, nw) > U);
       }
       const unsigned int bal = __ballot_sync(0xffffffffu, keep);
       __syncthreads();                       // s_wsum of the previous round has been read
@@ -291,13 +362,16 @@ __global__ void __launch_bounds__(128) cull_bricks_kernel(const CullArgs c) {
   const float y0z = (DIM == 3) ? box_centre(c.g.lo[2], c.g.s[2], bz * TZ + oz, ez) : 0.0f;
 
   float umin = CUDART_INF_F;
+  int imin = 0;
   for (int pos = lane; pos < n; pos += 32) {
-    float s, rho, nw;
-    seed_bounds<DIM, 0>(c.rec, cand(pos), y0x, y0y, y0z, &s, &rho, &nw);
-    umin = fminf(umin, upper_bound(s, rho, nw));
+    const int i = cand(pos);
+    float s, rho, supp, nw;
+    seed_bounds<DIM, 0>(c.rec, i, y0x, y0y, y0z, c.hb, &s, &rho, &supp, &nw);
+    const float u = upper_bound(s, rho, nw);
+    if (u < umin) { umin = u; imin = i; }
   }
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) umin = fminf(umin, __shfl_xor_sync(0xffffffffu, umin, o));
+  warp_argmin(umin, imin);
+  if (n > 0) umin = fminf(umin, exact_upper<DIM>(c.rec, imin, y0x, y0y, y0z, c.hb));
   const float U = umin + 2.0f * delta * (1.0f + CULL_EPS);
 
   const size_t brick = (size_t)b * 4 + w;
@@ -309,9 +383,9 @@ __global__ void __launch_bounds__(128) cull_bricks_kernel(const CullArgs c) {
     int i = 0;
     if (pos < n) {
       i = cand(pos);
-      float s, rho, nw;
-      seed_bounds<DIM, 0>(c.rec, i, y0x, y0y, y0z, &s, &rho, &nw);
-      keep = !(lower_bound(s, rho, nw) > U);
+      float s, rho, supp, nw;
+      seed_bounds<DIM, 0>(c.rec, i, y0x, y0y, y0z, c.hb, &s, &rho, &supp, &nw);
+      keep = !(lower_bound(s, supp, nw) > U);
     }
     const unsigned int bal = __ballot_sync(0xffffffffu, keep);
     if (keep) {
@@ -354,6 +428,7 @@ cudaError_t launch_cull(const GridDev& g, int M, int M_pad, const float* X, cons
   c.g = g; c.M = M; c.rec = cb.rec; c.super_list = cb.super_list; c.super_count = cb.super_count;
   c.nsx = nsx; c.nsy = nsy; c.nsz = nsz; c.brick_list = cb.brick_list; c.brick_count = cb.brick_count;
   c.done_flag = done_flag; c.rebuild = rebuild; c.delta = delta;
+  c.hb = hb; c.hs = hs;
   c.ht = make_float3(half(g.dim == 3 ? CULL_TILE3_X : CULL_TILE2_X, 0), half(g.dim == 3 ? CULL_TILE3_Y : CULL_TILE2_Y, 1),
                      g.dim == 3 ? half(CULL_TILE3_Z, 2) : 0.0f);
   const int n_super = nsx * nsy * nsz;
