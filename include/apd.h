@@ -157,6 +157,17 @@ int apd_lloyd(apd_ctx* ctx, const apd_grid* grid, int32_t M, float* X, const flo
               double tol, int32_t K, const float* w_init, float* w, int32_t* labels, double* vol,
               int32_t* iters, int32_t* evals, double* max_rel_err, const apd_opts* opts, void* cuda_stream);
 
+/* Algorithm 2 with its step 4 ("if it is not possible to hit the desired tolerance, increase J and
+ * restart"): apd_solve on `grid`; while it returns APD_NOT_CONVERGED and fewer than max_refinements refinements were
+ * made, every n_k is doubled (the paper gives no rule; reading S18) and apd_solve restarts from the best weights found
+ * so far.  grid: HOST in/out, n[] holds the final resolution on return.  w, vol, w_init: DEVICE as apd_solve (no
+ * labels: their size changes; call apd_assign on the returned grid).  refinements, iters, evals (totals),
+ * max_rel_err (of the last solve): HOST out, may be NULL.  Returns the status of the last solve. */
+int apd_solve_refine(apd_ctx* ctx, apd_grid* grid, int32_t M, const float* X, const float* A,
+                     const float* target_vol, double tol, int32_t max_refinements, const float* w_init, float* w,
+                     double* vol, int32_t* refinements, int32_t* iters, int32_t* evals, double* max_rel_err,
+                     const apd_opts* opts, void* cuda_stream);
+
 /* Resolution rules of PAPER.md:182-197 for a cubic grid of M voxels per axis on a domain of volume |Omega|:
  * |Omega| / M^D < factor * v_min with factor = eps (necessary: one misassigned voxel is already the tolerance; eq. 2.9
  * when v_min = |Omega|/N) or eps / 2^D (practical, eq. 2.10).  apd_resolution_bound returns the real number M must

@@ -386,3 +386,23 @@ def choose_resolution(dim: int, domain_volume: float, v_min: float, eps: float, 
     while not (domain_volume / float(m) ** dim < factor * v_min):
         m += 1
     return m
+
+
+def oracle_solve_refine(grid: Grid, X, A, v, eps: float, max_refinements: int, w_init=None, **solve_kw):
+    """Algorithm 2 with its step 4: while Algorithm 2 ends NOT_CONVERGED, double the voxels per axis
+    (reading S18: the paper gives no rule) and restart from the best weights found so far.
+    Returns (final Grid, SolveResult of the last solve, refinements, total iters, total evals)."""
+    w0 = w_init
+    iters = evals = 0
+    r = 0
+    while True:
+        res = oracle_solve(grid, X, A, v, eps, w_init=w0, **solve_kw)
+        iters += res.iters
+        evals += res.evals
+        if res.status != NOT_CONVERGED or r == max_refinements:
+            return grid, res, r, iters, evals
+        if np.prod([2 * k for k in grid.n], dtype=np.float64) >= 2.0 ** 31:
+            return grid, res, r, iters, evals
+        grid = Grid(grid.dim, tuple(2 * k for k in grid.n), grid.lo, grid.hi)
+        w0 = res.w32
+        r += 1

@@ -84,6 +84,10 @@ def load_library() -> ctypes.CDLL:
     lib.apd_lloyd.argtypes = ([_P, ctypes.POINTER(apd_grid), ctypes.c_int32, _P, _P, _P, ctypes.c_double, ctypes.c_int32]
                               + [_P] * 4 + [ctypes.POINTER(ctypes.c_int32), ctypes.POINTER(ctypes.c_int32),
                                             ctypes.POINTER(ctypes.c_double), ctypes.POINTER(apd_opts), _P])
+    lib.apd_solve_refine.restype = ctypes.c_int
+    lib.apd_solve_refine.argtypes = ([_P, ctypes.POINTER(apd_grid), ctypes.c_int32, _P, _P, _P, ctypes.c_double, ctypes.c_int32]
+                                     + [_P] * 3 + [ctypes.POINTER(ctypes.c_int32)] * 3
+                                     + [ctypes.POINTER(ctypes.c_double), ctypes.POINTER(apd_opts), _P])
     lib.apd_resolution_bound.restype = ctypes.c_double
     lib.apd_resolution_bound.argtypes = [ctypes.c_int32, ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_int32]
     lib.apd_choose_resolution.restype = ctypes.c_int32
@@ -100,7 +104,7 @@ def load_library() -> ctypes.CDLL:
 
 
 EXPORTED_SYMBOLS = ["apd_default_opts", "apd_create", "apd_destroy", "apd_last_error", "apd_assign", "apd_solve",
-                    "apd_assign_host", "apd_solve_host", "apd_solve_history", "apd_solve_stats", "apd_lloyd", "apd_resolution_bound",
+                    "apd_assign_host", "apd_solve_host", "apd_solve_history", "apd_solve_stats", "apd_lloyd", "apd_solve_refine", "apd_resolution_bound",
                     "apd_choose_resolution", "apd_last_kernel_ms", "apd_fp32_probe"]
 
 
@@ -260,6 +264,23 @@ class ApdContext:
             ctypes.byref(opts) if opts is not None else None, self._stream())
         self._check(rc, allow=(APD_OK, APD_NOT_CONVERGED))
         return SolveInfo(rc, it.value, ev.value, err.value, float("nan"))
+
+    def apd_solve_refine(self, grid: apd_grid, X, A, target_vol, tol: float, max_refinements: int, w_init=None,
+                         w=None, vol=None, opts: Optional[apd_opts] = None):
+        """apd_solve_refine of include/apd.h (Algorithm 2 incl. step 4); `grid.n` is updated in place.
+        Returns (SolveInfo, refinements)."""
+        d = grid.dim
+        M = X.shape[0]
+        rf, it, ev = ctypes.c_int32(0), ctypes.c_int32(0), ctypes.c_int32(0)
+        err = ctypes.c_double(0.0)
+        rc = self._lib.apd_solve_refine(
+            self._h, ctypes.byref(grid), M, _dev(X, torch.float32, "X", M * d), _dev(A, torch.float32, "A", M * d * d),
+            _dev(target_vol, torch.float32, "target_vol", M), float(tol), int(max_refinements),
+            _dev(w_init, torch.float32, "w_init", M), _dev(w, torch.float32, "w", M), _dev(vol, torch.float64, "vol", M),
+            ctypes.byref(rf), ctypes.byref(it), ctypes.byref(ev), ctypes.byref(err),
+            ctypes.byref(opts) if opts is not None else None, self._stream())
+        self._check(rc, allow=(APD_OK, APD_NOT_CONVERGED))
+        return SolveInfo(rc, it.value, ev.value, err.value, float("nan")), rf.value
 
     def solve_stats(self):
         """(evaluations recorded, candidate-list rebuilds) of the most recent apd_solve."""

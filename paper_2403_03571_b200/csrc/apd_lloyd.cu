@@ -85,3 +85,33 @@ extern "C" int32_t apd_choose_resolution(int32_t dim, double domain_volume, doub
   while (!(domain_volume / std::pow((double)m, (double)dim) < factor * v_min)) ++m;
   return (int32_t)m;
 }
+
+// Algorithm 2 step 4: "if it is not possible to hit the desired tolerance, increase J and restart".
+// The paper gives no rule for the increase (reading S18): every refinement doubles the voxels per axis and
+// restarts Algorithm 2 from the best weights found so far (the weights do not depend on the resolution).
+extern "C" int apd_solve_refine(apd_ctx* ctx, apd_grid* grid, int32_t M, const float* X, const float* A,
+                                const float* target_vol, double tol, int32_t max_refinements, const float* w_init,
+                                float* w, double* vol, int32_t* refinements, int32_t* iters, int32_t* evals,
+                                double* max_rel_err, const apd_opts* opts, void* cuda_stream) {
+  if (!ctx) return APD_E_ARG;
+  ctx->err.clear();
+  if (!grid || max_refinements < 0 || !w) { ctx->err = "apd_solve_refine: grid, w required, max_refinements >= 0"; return APD_E_ARG; }
+  int it_sum = 0, ev_sum = 0, r = 0, rc = APD_OK;
+  double err = 0.0;
+  for (;; ++r) {
+    int it = 0, ev = 0;
+    rc = apd_solve(ctx, grid, M, X, A, target_vol, tol, r == 0 ? w_init : w, w, nullptr, vol, nullptr, &it, &ev, &err,
+                   nullptr, opts, cuda_stream);
+    it_sum += it; ev_sum += ev;
+    if (rc != APD_NOT_CONVERGED || r == max_refinements) break;
+    long long nvox = 1;
+    for (int k = 0; k < grid->dim; ++k) nvox *= 2ll * grid->n[k];
+    if (nvox >= (1ll << 31)) break;                       // the next grid would exceed the index range
+    for (int k = 0; k < grid->dim; ++k) grid->n[k] *= 2;
+  }
+  if (refinements) *refinements = r;
+  if (iters) *iters = it_sum;
+  if (evals) *evals = ev_sum;
+  if (max_rel_err) *max_rel_err = err;
+  return rc;
+}

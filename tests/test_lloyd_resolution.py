@@ -130,3 +130,47 @@ def test_gpu_lloyd_parity(apd, cfg, n, M, eps, cull):
     assert chk.err <= eps + 2 * nm * grid.voxel_volume / float(wl.v.min())
     assert abs(info.evals - ev_o) <= max(6, ev_o // 3)
     print(f"cfg{cfg}: gpu evals {info.evals} vs oracle {ev_o}; max seed diff {np.abs(X - Xo).max() / h:.4f} voxels")
+
+
+# ------------------------------------------------------------------------------------------------ Alg. 2 step 4
+def coarse_problem():
+    """40 polydisperse grains on 32 x 32 pixels: the smallest grain holds ~8 pixels, so 1% is out of reach
+    (|P| > eps v_min) until the grid has been refined."""
+    return workloads.make_config(2, n=(32, 32), M=40)
+
+
+def test_refine_and_restart_oracle():
+    from oracle.apd_oracle import oracle_solve_refine, NOT_CONVERGED
+    wl = coarse_problem()
+    g0 = Grid(2, wl.n, wl.lo, wl.hi)
+    assert g0.voxel_volume > 0.01 * float(wl.v.min())                       # the necessary condition (2.9) fails
+    assert oracle_solve(g0, wl.X, wl.A, wl.v, 0.01, max_iters=200).status == NOT_CONVERGED
+    g, res, r, iters, evals = oracle_solve_refine(g0, wl.X, wl.A, wl.v, 0.01, 4, max_iters=200)
+    assert res.status == OK and 1 <= r <= 4 and tuple(g.n) == (32 * 2 ** r, 32 * 2 ** r)
+    chk = oracle_assign(g, wl.X, wl.A, res.w32, v=wl.v)                     # post-condition on the FINAL grid
+    assert chk.err <= 0.01
+    # with no refinement allowed the call is Algorithm 2 steps 1-3 alone
+    g1, res1, r1, _, _ = oracle_solve_refine(g0, wl.X, wl.A, wl.v, 0.01, 0, max_iters=200)
+    assert r1 == 0 and res1.status == NOT_CONVERGED and tuple(g1.n) == (32, 32)
+
+
+@pytest.mark.gpu
+def test_gpu_refine_and_restart(apd):
+    import torch
+    from oracle.apd_oracle import oracle_solve_refine
+    wl = coarse_problem()
+    g_or, res, r_or, _, ev_or = oracle_solve_refine(Grid(2, wl.n, wl.lo, wl.hi), wl.X, wl.A, wl.v, 0.01, 4, max_iters=200)
+    dev = torch.device("cuda:0")
+    ctx = apd.ApdContext(2, wl.M)
+    grid = apd.make_grid(2, wl.n, wl.lo, wl.hi)
+    X = torch.from_numpy(wl.X).to(dev); A = torch.from_numpy(wl.A).to(dev); v = torch.from_numpy(wl.v).to(dev)
+    w = torch.zeros(wl.M, dtype=torch.float32, device=dev)
+    vol = torch.zeros(wl.M, dtype=torch.float64, device=dev)
+    info, r = ctx.apd_solve_refine(grid, X, A, v, 0.01, 4, w=w, vol=vol, opts=apd.make_opts(max_iters=200))
+    assert info.status == 0 and r == r_or and (grid.n[0], grid.n[1]) == tuple(g_or.n)
+    chk = oracle_assign(g_or, wl.X, wl.A, w.cpu().numpy(), v=wl.v)          # judged by the oracle on the final grid
+    assert chk.err <= 0.01 + 2 * g_or.voxel_volume / float(wl.v.min())
+    # the coarse, non-converging solves wander (every decision sits on a few pixels): only the order of magnitude of
+    # the work is comparable
+    assert abs(info.evals - ev_or) <= max(10, ev_or // 2)
+    print(f"refinements {r}, final grid {grid.n[0]}x{grid.n[1]}, gpu evals {info.evals} vs oracle {ev_or}")
