@@ -263,3 +263,21 @@ def test_culling_rejects_direct_kernel(apd):
     with pytest.raises(apd.ApdError) as e:
         run_assign(apd, wl, wl.w0, kernel=KERNELS["direct"], cull=1)
     assert e.value.status == apd.APD_E_ARG
+
+
+def test_slab_decomposition_is_exact(apd):
+    """The path shards by voxel slabs with the EXISTING call: a z-slab is an apd_grid with
+    shifted lo/hi and fewer n_z.  On a power-of-two grid the slab's voxel centres are bit-identical, so labels
+    concatenate and the integer counts / min-cost sums add up exactly to the single-grid evaluation."""
+    wl = workloads.make_config(3, n=(64, 64, 64), M=300)
+    w = rand_w(wl, 0.15, 77)
+    full = run_assign(apd, wl, w, v=None)
+    labs, vol, dual = [], np.zeros(wl.M), 0.0
+    for z0, z1 in ((0, 16), (16, 48), (48, 64)):
+        part = workloads.Workload("slab", 3, (64, 64, z1 - z0), (0.0, 0.0, z0 / 64.0), (1.0, 1.0, z1 / 64.0),
+                                  wl.X, wl.A, wl.v, wl.w0)
+        r = run_assign(apd, part, w, v=None)
+        labs.append(r["labels"]); vol += r["vol"]; dual += r["dual"]
+    assert np.array_equal(np.concatenate(labs), full["labels"])
+    assert np.array_equal(vol, full["vol"])                       # integer counts x |P| (a power of two): exact
+    assert abs(dual - full["dual"]) <= 1e-13 * abs(full["dual"])  # same minima, different partial-sum order
