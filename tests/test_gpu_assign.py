@@ -121,16 +121,16 @@ def test_no_target_volume_and_no_labels(apd, kernel):
     assert r2["dual"] == r["dual"] and np.array_equal(r2["vol"], r["vol"])     # bitwise reproducible
 
 
-@pytest.mark.parametrize("kernel", ["direct", "auto"])
+@pytest.mark.parametrize("kernel,cull", [("direct", 0), ("auto", 0), ("auto", 1)])
 @pytest.mark.parametrize("dim", [2, 3])
-def test_exact_ties_lowest_index(apd, kernel, dim):
+def test_exact_ties_lowest_index(apd, kernel, cull, dim):
     """Mirror-symmetric seeds on a power-of-two grid: costs are exactly equal in fp32 AND fp64 on the
     mirror plane's neighbours... here seeds are duplicated, so every voxel ties: lowest index wins (S1)."""
     wl = workloads.make_random(dim, (32,) * dim, 6, 31)
     X = np.concatenate([wl.X, wl.X]); A = np.concatenate([wl.A, wl.A])
     wl2 = workloads.Workload("dup", dim, wl.n, wl.lo, wl.hi, X, A, np.full(12, 1 / 12, np.float32),
                              np.zeros(12, np.float32))
-    r = run_assign(apd, wl2, wl2.w0, kernel=KERNELS[kernel])
+    r = run_assign(apd, wl2, wl2.w0, kernel=KERNELS[kernel], cull=cull)
     assert r["labels"].max() < 6
     parity.check_assign(wl2, wl2.w0, r["labels"], r["vol"], r["dual"])
 
@@ -145,14 +145,14 @@ def test_empty_cell_centroid_is_seed(apd, kernel):
     parity.check_assign(wl, w, r["labels"], r["vol"], r["dual"], v=wl.v, centroids_gpu=r["centroids"])
 
 
-@pytest.mark.parametrize("kernel", ["direct", "auto"])
-def test_P11_exact_scaling_symmetry(apd, kernel):
+@pytest.mark.parametrize("kernel,cull", [("direct", 0), ("auto", 0), ("auto", 1)])
+def test_P11_exact_scaling_symmetry(apd, kernel, cull):
     """(A, w) -> (2A, 2w) doubles every fp32 cost exactly: labels identical, dual doubles exactly."""
     wl = workloads.make_config(3, n=(64, 64, 64), M=200)
     w = rand_w(wl, 0.1, 7)
-    r1 = run_assign(apd, wl, w, kernel=KERNELS[kernel])
+    r1 = run_assign(apd, wl, w, kernel=KERNELS[kernel], cull=cull)
     wl2 = workloads.Workload("x2", wl.dim, wl.n, wl.lo, wl.hi, wl.X, (2 * wl.A).astype(np.float32), wl.v, wl.w0)
-    r2 = run_assign(apd, wl2, (2 * w).astype(np.float32), kernel=KERNELS[kernel])
+    r2 = run_assign(apd, wl2, (2 * w).astype(np.float32), kernel=KERNELS[kernel], cull=cull)
     assert np.array_equal(r1["labels"], r2["labels"])
     assert r2["dual"] == 2.0 * r1["dual"]
 
