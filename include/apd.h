@@ -141,6 +141,18 @@ int apd_solve(apd_ctx* ctx, const apd_grid* grid, int32_t M,
  * entries written (>= 0), or a negative apd_status.  Synchronous. */
 int apd_solve_history(apd_ctx* ctx, double* dual_hist, double* err_hist, int32_t cap);
 
+/* Algorithm 1 + eq. (2.7)-(2.8) on a USER-SUPPLIED discretisation: points y_j with volumes |P_j|,
+ * e.g. element centroids and volumes of a triangulation, a masked or locally refined domain.
+ *   Y     [N,dim]  DEVICE fp32 row-major, sample points        pvol [N]  DEVICE fp32, their volumes |P_j| >= 0
+ *   X, A, w, target_vol, labels, dual, max_rel_err, centroids: as apd_assign (dim = the context's dim)
+ *   vol   [M]      DEVICE fp64 out: sum of |P_j| over the points labelled i
+ *   dual           g~ = sum_i v_i w_i + sum_j |P_j| min_i C_ij;  centroids: sum |P_j| y_j / vol_i (empty cell: x_i)
+ * Volumes are real numbers here, accumulated with fp64 atomics: results are reproducible up to summation order, and
+ * there is no culling (brute force, DIRECT arithmetic).  Asynchronous on cuda_stream.  1 <= N < 2^40. */
+int apd_assign_points(apd_ctx* ctx, int64_t N, const float* Y, const float* pvol, int32_t M, const float* X,
+                      const float* A, const float* w, const float* target_vol, int32_t* labels, double* vol,
+                      double* dual, double* max_rel_err, double* centroids, void* cuda_stream);
+
 /* Counters of the most recent apd_solve on this context (HOST out, each may be NULL): evaluations recorded by
  * apd_solve_history, and how many evaluations of the loop rebuilt the culling candidate lists (with opts.cull the
  * lists are built with a slack on the bounds and reused while the weights stay within it; 0 without culling). */

@@ -406,3 +406,54 @@ def oracle_solve_refine(grid: Grid, X, A, v, eps: float, max_refinements: int, w
         grid = Grid(grid.dim, tuple(2 * k for k in grid.n), grid.lo, grid.hi)
         w0 = res.w32
         r += 1
+
+
+# ----------------------------------------------------------------------------------------
+# user-supplied discretisation: points y_j with volumes |P_j|
+# ----------------------------------------------------------------------------------------
+@dataclasses.dataclass
+class PointsResult:
+    labels: np.ndarray        # [N] argmin, lowest index on ties
+    best: np.ndarray          # [N] min_i C_ij
+    second: np.ndarray        # [N] runner-up cost (inf if M == 1)
+    vol: np.ndarray           # [M] sum of |P_j| over the cell
+    dual: float               # eq. (2.7) with element volumes, literally
+    dual_min_part: float      # sum_j |P_j| min_i C_ij
+    centroids: np.ndarray     # [M,d]
+    err: float
+
+
+def oracle_assign_points(Y, pvol, X, A, w, v=None, chunk: int = 4096) -> PointsResult:
+    """The definition with element volumes: C_ij = (y_j - x_i)^T A_i (y_j - x_i) - w_i, all d^2
+    terms, fp64; H_j = lowest argmin; vol_i = sum_{H_j=i} |P_j|;
+    g~ = sum_i [(v_i - vol_i) w_i + sum_{H_j=i} |P_j| |y_j - x_i|^2_{A_i}]  (eq. 2.7 with |P| -> |P_j|);
+    centroid_i = sum |P_j| y_j / vol_i, the seed itself for an empty cell (reading S5)."""
+    Y = np.asarray(Y, dtype=np.float64)
+    N, d = Y.shape
+    X = np.asarray(X, dtype=np.float64).reshape(-1, d)
+    M = X.shape[0]
+    A = np.asarray(A, dtype=np.float64).reshape(M, d, d)
+    w = np.asarray(w, dtype=np.float64).reshape(M)
+    p = np.asarray(pvol, dtype=np.float64).reshape(N)
+    labels = np.empty(N, dtype=np.int64); best = np.empty(N); second = np.full(N, np.inf); qbest = np.empty(N)
+    for j0 in range(0, N, chunk):
+        D = Y[j0:j0 + chunk, None, :] - X[None, :, :]                        # [n, M, d]
+        q = np.einsum("nmk,mkl,nml->nm", D, A, D)                            # all d^2 terms (S13)
+        c = q - w[None, :]
+        lab = np.argmin(c, axis=1)                                           # first minimum = lowest index (S1)
+        r = np.arange(c.shape[0])
+        labels[j0:j0 + chunk] = lab; best[j0:j0 + chunk] = c[r, lab]; qbest[j0:j0 + chunk] = q[r, lab]
+        if M > 1:
+            c2 = c.copy(); c2[r, lab] = np.inf
+            second[j0:j0 + chunk] = c2.min(axis=1)
+    vol = np.bincount(labels, weights=p, minlength=M)
+    T = float(np.sum(p * qbest))
+    v64 = np.zeros(M) if v is None else np.asarray(v, dtype=np.float64).reshape(M)
+    dual = float(np.sum((v64 - vol) * w)) + T
+    cen = np.empty((M, d))
+    for k in range(d):
+        num = np.bincount(labels, weights=p * Y[:, k], minlength=M)
+        cen[:, k] = np.where(vol > 0, num / np.where(vol > 0, vol, 1.0), X[:, k])
+    err = float(np.max(np.abs(vol - v64) / v64)) if v is not None else float("nan")
+    return PointsResult(labels=labels, best=best, second=second, vol=vol, dual=dual,
+                        dual_min_part=float(np.sum(p * best)), centroids=cen, err=err)

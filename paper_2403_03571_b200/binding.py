@@ -78,6 +78,8 @@ def load_library() -> ctypes.CDLL:
                                    + [_P] * 5 + [ctypes.POINTER(ctypes.c_int32), ctypes.POINTER(ctypes.c_int32),
                                                  ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double),
                                                  ctypes.POINTER(apd_opts)])
+    lib.apd_assign_points.restype = ctypes.c_int
+    lib.apd_assign_points.argtypes = [_P, ctypes.c_int64, _P, _P, ctypes.c_int32] + [_P] * 10
     lib.apd_solve_stats.restype = ctypes.c_int
     lib.apd_solve_stats.argtypes = [_P, ctypes.POINTER(ctypes.c_int32), ctypes.POINTER(ctypes.c_int32)]
     lib.apd_lloyd.restype = ctypes.c_int
@@ -104,7 +106,7 @@ def load_library() -> ctypes.CDLL:
 
 
 EXPORTED_SYMBOLS = ["apd_default_opts", "apd_create", "apd_destroy", "apd_last_error", "apd_assign", "apd_solve",
-                    "apd_assign_host", "apd_solve_host", "apd_solve_history", "apd_solve_stats", "apd_lloyd", "apd_solve_refine", "apd_resolution_bound",
+                    "apd_assign_host", "apd_solve_host", "apd_solve_history", "apd_assign_points", "apd_solve_stats", "apd_lloyd", "apd_solve_refine", "apd_resolution_bound",
                     "apd_choose_resolution", "apd_last_kernel_ms", "apd_fp32_probe"]
 
 
@@ -198,6 +200,20 @@ class ApdContext:
             _dev(dual, torch.float64, "dual", 1), _dev(max_rel_err, torch.float64, "max_rel_err", 1),
             _dev(centroids, torch.float64, "centroids", M * d), _dev(pairs_evaluated, torch.int64, "pairs_evaluated", 1),
             ctypes.byref(opts) if opts is not None else None, self._stream())
+        self._check(rc)
+
+    def apd_assign_points(self, Y, pvol, X, A, w, target_vol=None, labels=None, vol=None, dual=None,
+                          max_rel_err=None, centroids=None):
+        """apd_assign_points of include/apd.h on CUDA tensors (user-supplied points and volumes)."""
+        d = self.dim
+        N, M = Y.shape[0], X.shape[0]
+        rc = self._lib.apd_assign_points(
+            self._h, N, _dev(Y, torch.float32, "Y", N * d), _dev(pvol, torch.float32, "pvol", N), M,
+            _dev(X, torch.float32, "X", M * d), _dev(A, torch.float32, "A", M * d * d), _dev(w, torch.float32, "w", M),
+            _dev(target_vol, torch.float32, "target_vol", M), _dev(labels, torch.int32, "labels", N),
+            _dev(vol, torch.float64, "vol", M), _dev(dual, torch.float64, "dual", 1),
+            _dev(max_rel_err, torch.float64, "max_rel_err", 1), _dev(centroids, torch.float64, "centroids", M * d),
+            self._stream())
         self._check(rc)
 
     def apd_solve(self, grid: apd_grid, X, A, target_vol, tol: float, w_init=None, w=None, labels=None, vol=None,

@@ -77,6 +77,7 @@ struct Workspace {
   int* super_count = nullptr;          // [super_cap_n]
   size_t super_cap_n = 0;
   unsigned long long* pairs_ctr = nullptr;
+  double* pt_acc = nullptr;            // apd_assign_points: fp64 accumulators vol[max_seeds] | csum[max_seeds,3]
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
   bool timed = false;
   // apd_solve state (apd_lbfgs.cu), allocated on first use
