@@ -153,6 +153,17 @@ int apd_assign_points(apd_ctx* ctx, int64_t N, const float* Y, const float* pvol
                       const float* A, const float* w, const float* target_vol, int32_t* labels, double* vol,
                       double* dual, double* max_rel_err, double* centroids, void* cuda_stream);
 
+/* Algorithm 2 on a user-supplied discretisation: the L-BFGS of apd_solve (same specification S9) with every evaluation
+ * done by the point kernel of apd_assign_points.  total_volume = sum_j |P_j| (HOST; it replaces |Omega|: sum
+ * target_vol must equal it to 1e-5 relative, else APD_E_ARG).  Y, pvol, X, A, target_vol, w_init, w, labels [N],
+ * vol [M]: DEVICE as above; iters, evals, max_rel_err: HOST out.  No culling (opts.cull must be 0).  Because cell
+ * volumes are fp64 sums accumulated in no fixed order, two runs can differ in the last bits and, rarely, in a
+ * line-search decision.  Blocks until finished; returns APD_OK, APD_NOT_CONVERGED or a negative error. */
+int apd_solve_points(apd_ctx* ctx, int64_t N, const float* Y, const float* pvol, double total_volume, int32_t M,
+                     const float* X, const float* A, const float* target_vol, double tol, const float* w_init,
+                     float* w, int32_t* labels, double* vol, int32_t* iters, int32_t* evals, double* max_rel_err,
+                     const apd_opts* opts, void* cuda_stream);
+
 /* Counters of the most recent apd_solve on this context (HOST out, each may be NULL): evaluations recorded by
  * apd_solve_history, and how many evaluations of the loop rebuilt the culling candidate lists (with opts.cull the
  * lists are built with a slack on the bounds and reused while the weights stay within it; 0 without culling). */

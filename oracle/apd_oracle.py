@@ -219,6 +219,21 @@ def oracle_cost_of(grid: Grid, X, A, w, sel, seed) -> np.ndarray:
 # Algorithm 2 with the L-BFGS of DESIGN.md reading S9
 # ----------------------------------------------------------------------------------------
 @dataclasses.dataclass
+class PointSet:
+    """A user-supplied discretisation for oracle_solve: points y_j [N,d] with volumes |P_j| [N]."""
+    Y: np.ndarray
+    pvol: np.ndarray
+
+    @property
+    def dim(self) -> int:
+        return int(np.asarray(self.Y).shape[1])
+
+    @property
+    def domain_volume(self) -> float:
+        return float(np.sum(np.asarray(self.pvol, dtype=np.float64)))
+
+
+@dataclasses.dataclass
 class SolveResult:
     status: int                   # OK / NOT_CONVERGED
     w: np.ndarray                 # fp64 iterate
@@ -275,7 +290,10 @@ def oracle_solve(grid: Grid, X, A, v, eps: float, w_init=None, history: int = 10
 
     def evaluate(wd, tag):
         w32 = wd.astype(np.float32)                     # RNE rounding, S10
-        r = oracle_assign(grid, X, A, w32, v=v64, diagnostics=False)
+        if isinstance(grid, PointSet):                  # user-supplied discretisation
+            r = oracle_assign_points(grid.Y, grid.pvol, X, A, w32, v=v64)
+        else:
+            r = oracle_assign(grid, X, A, w32, v=v64, diagnostics=False)
         f = -r.dual
         g = r.vol - v64
         if r.err < best["err"]:

@@ -80,6 +80,11 @@ def load_library() -> ctypes.CDLL:
                                                  ctypes.POINTER(apd_opts)])
     lib.apd_assign_points.restype = ctypes.c_int
     lib.apd_assign_points.argtypes = [_P, ctypes.c_int64, _P, _P, ctypes.c_int32] + [_P] * 10
+    lib.apd_solve_points.restype = ctypes.c_int
+    lib.apd_solve_points.argtypes = ([_P, ctypes.c_int64, _P, _P, ctypes.c_double, ctypes.c_int32, _P, _P, _P,
+                                      ctypes.c_double] + [_P] * 4
+                                     + [ctypes.POINTER(ctypes.c_int32), ctypes.POINTER(ctypes.c_int32),
+                                        ctypes.POINTER(ctypes.c_double), ctypes.POINTER(apd_opts), _P])
     lib.apd_solve_stats.restype = ctypes.c_int
     lib.apd_solve_stats.argtypes = [_P, ctypes.POINTER(ctypes.c_int32), ctypes.POINTER(ctypes.c_int32)]
     lib.apd_lloyd.restype = ctypes.c_int
@@ -106,7 +111,7 @@ def load_library() -> ctypes.CDLL:
 
 
 EXPORTED_SYMBOLS = ["apd_default_opts", "apd_create", "apd_destroy", "apd_last_error", "apd_assign", "apd_solve",
-                    "apd_assign_host", "apd_solve_host", "apd_solve_history", "apd_assign_points", "apd_solve_stats", "apd_lloyd", "apd_solve_refine", "apd_resolution_bound",
+                    "apd_assign_host", "apd_solve_host", "apd_solve_history", "apd_assign_points", "apd_solve_points", "apd_solve_stats", "apd_lloyd", "apd_solve_refine", "apd_resolution_bound",
                     "apd_choose_resolution", "apd_last_kernel_ms", "apd_fp32_probe"]
 
 
@@ -215,6 +220,23 @@ class ApdContext:
             _dev(max_rel_err, torch.float64, "max_rel_err", 1), _dev(centroids, torch.float64, "centroids", M * d),
             self._stream())
         self._check(rc)
+
+    def apd_solve_points(self, Y, pvol, total_volume: float, X, A, target_vol, tol: float, w_init=None, w=None,
+                         labels=None, vol=None, opts: Optional[apd_opts] = None) -> SolveInfo:
+        """apd_solve_points of include/apd.h on CUDA tensors; blocks until finished."""
+        d = self.dim
+        N, M = Y.shape[0], X.shape[0]
+        it, ev = ctypes.c_int32(0), ctypes.c_int32(0)
+        err = ctypes.c_double(0.0)
+        rc = self._lib.apd_solve_points(
+            self._h, N, _dev(Y, torch.float32, "Y", N * d), _dev(pvol, torch.float32, "pvol", N), float(total_volume), M,
+            _dev(X, torch.float32, "X", M * d), _dev(A, torch.float32, "A", M * d * d),
+            _dev(target_vol, torch.float32, "target_vol", M), float(tol), _dev(w_init, torch.float32, "w_init", M),
+            _dev(w, torch.float32, "w", M), _dev(labels, torch.int32, "labels", N), _dev(vol, torch.float64, "vol", M),
+            ctypes.byref(it), ctypes.byref(ev), ctypes.byref(err), ctypes.byref(opts) if opts is not None else None,
+            self._stream())
+        self._check(rc, allow=(APD_OK, APD_NOT_CONVERGED))
+        return SolveInfo(rc, it.value, ev.value, err.value, float("nan"))
 
     def apd_solve(self, grid: apd_grid, X, A, target_vol, tol: float, w_init=None, w=None, labels=None, vol=None,
                   w64=None, opts: Optional[apd_opts] = None) -> SolveInfo:

@@ -144,6 +144,13 @@ cudaError_t launch_finalize(const GridDev& g, int M, int n_partials, const unsig
                             uint64_t* pairs_evaluated, const unsigned long long* pairs_ctr, const int* done_flag,
                             cudaStream_t st);
 
+// apd_points.cu: sizing / allocation of the point-set accumulators, and one evaluation on points.  vol == nullptr
+// leaves the raw outputs (ws.pt_acc volumes, ws.dual_partial) for lbfgs_step_kernel and skips the finalize kernel.
+int points_prepare(apd_ctx* ctx, long long N, int* n_partials, cudaStream_t st);
+int enqueue_points(apd_ctx* ctx, long long N, const float* Y, const float* pvol, int M, const float* X, const float* A,
+                   const float* w, const float* target_vol, int32_t* labels, double* vol, double* dual,
+                   double* max_rel_err, double* centroids, const int* done_flag, int* n_partials, cudaStream_t st);
+
 // What the device-side optimiser reports to the host (mapped pinned memory).
 struct SolveReport {
   volatile int done;      // 0 running, 1 finished

@@ -16,6 +16,7 @@
 #include "apd_internal.cuh"
 #include "apd_device.cuh"
 #include <cmath>
+#include <functional>
 #include <cooperative_groups.h>
 namespace cg = cooperative_groups;
 #include <vector>
@@ -46,7 +47,8 @@ struct StepArgs {
   int M;
   const float* v;      // target volumes
   // raw outputs of the evaluation just run (the loop skips finalize_kernel and finishes eq. 2.7 / 2.8 / 2.5 here)
-  const unsigned int* count;      // [M] voxels per cell
+  const unsigned int* count;      // [M] voxels per cell (grid evaluations), or nullptr:
+  const double* vol_in;           // [M] cell volumes already in fp64 (apd_solve_points; voxel_volume is then 1)
   const double* dual_partial;     // [n_partials] sums of min-costs
   int n_partials;
   double voxel_volume;            // |P|
@@ -326,7 +328,8 @@ __global__ void __cluster_dims__(LB_CLUSTER, 1, 1) __launch_bounds__(LB_THREADS)
   for (int i = LB_FIRST(red); i < M; i += LB_STEP) {
     const double tv = (double)a.v[i];
     s0[0] += tv * (double)a.w32[i];
-    emax = fmax(emax, fabs((double)a.count[i] * P - tv) / tv);
+    const double vi = a.vol_in ? a.vol_in[i] : (double)a.count[i] * P;
+    emax = fmax(emax, fabs(vi - tv) / tv);
   }
   for (int t = LB_FIRST(red); t < a.n_partials; t += LB_STEP) s0[1] += a.dual_partial[t];
   cluster_all<2, false>(s0, red);
@@ -343,7 +346,7 @@ __global__ void __cluster_dims__(LB_CLUSTER, 1, 1) __launch_bounds__(LB_THREADS)
   double sums[5] = {0.0, 0.0, 0.0, 0.0, 0.0};     // sum v, g1.p, s.y, s.s, y.y
   for (int i = LB_FIRST(red); i < M; i += LB_STEP) {
     const double tv = (double)a.v[i];
-    const double gn = (double)a.count[i] * P - tv;      // m_i |P| - v_i
+    const double gn = (a.vol_in ? a.vol_in[i] : (double)a.count[i] * P) - tv;      // m_i |P| - v_i
     gnew[i] = gn;
     sums[0] += tv;
     if (improved) wbest[i] = w_eval[i];
@@ -521,43 +524,24 @@ static int ensure_solve_state(apd_ctx* ctx, int hist) {
   return APD_OK;
 }
 
-extern "C" int apd_solve(apd_ctx* ctx, const apd_grid* grid, int32_t M, const float* X, const float* A,
-                         const float* target_vol, double tol, const float* w_init, float* w, int32_t* labels,
-                         double* vol, double* w64, int32_t* iters, int32_t* evals, double* max_rel_err,
-                         double* dual, const apd_opts* opts, void* cuda_stream) {
-  if (!ctx) return APD_E_ARG;
-  ctx->err.clear();
-  std::string e;
-  const int kernel = resolve_kernel(opts, &e);
-  if (kernel < 0) { ctx->err = "apd_solve: " + e; return APD_E_ARG; }
-  if (M < 1 || M > ctx->ws.max_seeds) { ctx->err = "apd_solve: M out of range [1, max_seeds]"; return APD_E_ARG; }
-  if (!X || !A || !target_vol || !w) { ctx->err = "apd_solve: X, A, target_vol and w are required"; return APD_E_ARG; }
-  if (!(tol > 0.0) || !std::isfinite(tol)) { ctx->err = "apd_solve: tol must be finite and > 0"; return APD_E_ARG; }
-  apd_opts o;
-  apd_default_opts(&o);
-  if (opts) o = *opts;
-  if (o.lbfgs_history < 1 || o.lbfgs_history > LB_MAX_HIST) { ctx->err = "apd_solve: lbfgs_history must be in [1,64]"; return APD_E_ARG; }
-  if (o.max_iters < 1 || o.max_evals < 0) { ctx->err = "apd_solve: max_iters >= 1 and max_evals >= 0 required"; return APD_E_ARG; }
-  const int max_evals = o.max_evals ? o.max_evals : (o.max_iters > (1 << 26) ? (1 << 30) : 20 * o.max_iters);
-  GridDev g;
-  e = make_grid(ctx, grid, kernel, o.cull != 0, &g);
-  if (!e.empty()) { ctx->err = "apd_solve: " + e; return APD_E_ARG; }
-  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-  LB_TRY(cudaSetDevice(ctx->ws.device));
-  int rc = ensure_solve_state(ctx, o.lbfgs_history);
-  if (rc != APD_OK) return rc;
+// The device-driven optimiser loop shared by apd_solve (voxel grids) and apd_solve_points (user points).
+//   loop_eval(done_flag): enqueue one evaluation at ws.w32 that leaves its RAW outputs where `sa` points
+//   final_eval():         enqueue the final, labelled evaluation at ws.w32
+struct SolveHooks {
+  std::function<int(const int*)> loop_eval;
+  std::function<int()> final_eval;
+};
+
+static int solve_common(apd_ctx* ctx, const char* who, int dim, int32_t M, const float* target_vol, double tol,
+                        const float* w_init, float* w, double* w64, const apd_opts& o, double domain, StepArgs sa,
+                        const SolveHooks& hooks, int32_t* iters, int32_t* evals, double* max_rel_err, double* dual,
+                        cudaStream_t st) {
   Workspace& ws = ctx->ws;
-
-  double domain = 1.0;
-  for (int k = 0; k < g.dim; ++k) domain *= (grid->hi[k] - grid->lo[k]);
-  const double ell = std::pow(domain / (double)M, 1.0 / (double)g.dim);
-  const double gamma0 = std::pow(ell, (double)(2 - g.dim)) / (double)g.dim;
-
-  StepArgs sa;
-  sa.st = ws.sstate; sa.vec = ws.svec; sa.stride = ws.max_seeds; sa.M = M; sa.v = target_vol;
-  sa.count = ws.count; sa.voxel_volume = g.voxel_volume; sa.w32 = ws.w32;
-  sa.n_partials = (o.cull ? 4 : 1) * g.tiles_x * g.tiles_y * g.tiles_z;
-  sa.hist = ws.hist; sa.hist_cap = SOLVE_HIST_CAP; sa.wref = ws.wref;
+  const int max_evals = o.max_evals ? o.max_evals : (o.max_iters > (1 << 26) ? (1 << 30) : 20 * o.max_iters);
+  const double ell = std::pow(domain / (double)M, 1.0 / (double)dim);
+  const double gamma0 = std::pow(ell, (double)(2 - dim)) / (double)dim;
+  sa.st = ws.sstate; sa.vec = ws.svec; sa.stride = ws.max_seeds; sa.M = M; sa.v = target_vol; sa.w32 = ws.w32;
+  sa.hist = ws.hist; sa.hist_cap = SOLVE_HIST_CAP; sa.wref = ws.wref; sa.gram = ws.gram;
   ws.hist_len = 0;
   SolveReport* dev_report = nullptr;
   LB_TRY(cudaHostGetDevicePointer((void**)&dev_report, ws.report, 0));
@@ -572,16 +556,13 @@ extern "C" int apd_solve(apd_ctx* ctx, const apd_grid* grid, int32_t M, const fl
   const size_t dyn_bytes = (nb * nb + nb + 2 * (size_t)o.lbfgs_history) * sizeof(double) + (size_t)o.lbfgs_history * sizeof(int);
   if (dyn_bytes > 32 * 1024)
     LB_TRY(cudaFuncSetAttribute(lbfgs_step_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn_bytes));
-  sa.gram = ws.gram;
   const int* done_flag = &ws.sstate->done;
   long long enq = 0;
   const long long hard_cap = (long long)max_evals + 64;
   for (;; ++enq) {
-    rc = enqueue_evaluation(ctx, g, kernel, M, X, A, ws.w32, target_vol, nullptr, nullptr, nullptr,
-                            nullptr, nullptr, nullptr, false, o.cull != 0, done_flag, st, &ws.sstate->cull_rebuild,
-                            &ws.sstate->cull_delta);
+    int rc = hooks.loop_eval(done_flag);
     if (rc != APD_OK) return rc;
-    sa.dual_partial = ws.dual_partial;       // (re)allocated by the first enqueue_evaluation
+    sa.dual_partial = ws.dual_partial;       // (re)allocated by the first evaluation
     lbfgs_step_kernel<<<LB_CLUSTER, LB_THREADS, dyn_bytes, st>>>(sa);
     LB_TRY(cudaGetLastError());
     LB_TRY(cudaEventRecord(ws.sev[enq & 1], st));
@@ -591,15 +572,16 @@ extern "C" int apd_solve(apd_ctx* ctx, const apd_grid* grid, int32_t M, const fl
       LB_TRY(cudaEventSynchronize(ws.sev[(enq - 1) & 1]));
       if (ws.report->done) break;
     }
-    if (enq > hard_cap) { ctx->err = "apd_solve: optimiser did not report completion"; return APD_E_CUDA; }
+    if (enq > hard_cap) { ctx->err = std::string(who) + ": optimiser did not report completion"; return APD_E_CUDA; }
   }
   LB_TRY(cudaStreamSynchronize(st));
   const int status = ws.report->status;
-  if (status == APD_E_ARG) { ctx->err = "apd_solve: sum(target_vol) differs from |Omega| by more than 1e-5 relative"; return APD_E_ARG; }
-
+  if (status == APD_E_ARG) {
+    ctx->err = std::string(who) + ": sum(target_vol) differs from |Omega| by more than 1e-5 relative";
+    return APD_E_ARG;
+  }
   // final evaluation at the returned fp32 weights, with labels (Algorithm 1 at the solution)
-  rc = enqueue_evaluation(ctx, g, kernel, M, X, A, ws.w32, target_vol, labels, vol ? vol : ws.e_vol, ws.e_scal,
-                          ws.e_scal + 1, nullptr, nullptr, true, o.cull != 0, nullptr, st);
+  int rc = hooks.final_eval();
   if (rc != APD_OK) return rc;
   LB_TRY(cudaMemcpyAsync(w, ws.w32, sizeof(float) * M, cudaMemcpyDeviceToDevice, st));
   if (w64) LB_TRY(cudaMemcpyAsync(w64, ws.svec + (size_t)V_W * ws.max_seeds, sizeof(double) * M,
@@ -612,6 +594,94 @@ extern "C" int apd_solve(apd_ctx* ctx, const apd_grid* grid, int32_t M, const fl
   if (max_rel_err) *max_rel_err = ws.report->err;
   if (dual) *dual = ws.report->dual;
   return status;
+}
+
+static int check_solve_opts(apd_ctx* ctx, const char* who, const apd_opts* opts, double tol, apd_opts* o) {
+  apd_default_opts(o);
+  if (opts) *o = *opts;
+  if (!(tol > 0.0) || !std::isfinite(tol)) { ctx->err = std::string(who) + ": tol must be finite and > 0"; return APD_E_ARG; }
+  if (o->lbfgs_history < 1 || o->lbfgs_history > LB_MAX_HIST) { ctx->err = std::string(who) + ": lbfgs_history must be in [1,64]"; return APD_E_ARG; }
+  if (o->max_iters < 1 || o->max_evals < 0) { ctx->err = std::string(who) + ": max_iters >= 1 and max_evals >= 0 required"; return APD_E_ARG; }
+  return APD_OK;
+}
+
+extern "C" int apd_solve(apd_ctx* ctx, const apd_grid* grid, int32_t M, const float* X, const float* A,
+                         const float* target_vol, double tol, const float* w_init, float* w, int32_t* labels,
+                         double* vol, double* w64, int32_t* iters, int32_t* evals, double* max_rel_err,
+                         double* dual, const apd_opts* opts, void* cuda_stream) {
+  if (!ctx) return APD_E_ARG;
+  ctx->err.clear();
+  std::string e;
+  const int kernel = resolve_kernel(opts, &e);
+  if (kernel < 0) { ctx->err = "apd_solve: " + e; return APD_E_ARG; }
+  if (M < 1 || M > ctx->ws.max_seeds) { ctx->err = "apd_solve: M out of range [1, max_seeds]"; return APD_E_ARG; }
+  if (!X || !A || !target_vol || !w) { ctx->err = "apd_solve: X, A, target_vol and w are required"; return APD_E_ARG; }
+  apd_opts o;
+  int rc = check_solve_opts(ctx, "apd_solve", opts, tol, &o);
+  if (rc != APD_OK) return rc;
+  GridDev g;
+  e = make_grid(ctx, grid, kernel, o.cull != 0, &g);
+  if (!e.empty()) { ctx->err = "apd_solve: " + e; return APD_E_ARG; }
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  LB_TRY(cudaSetDevice(ctx->ws.device));
+  rc = ensure_solve_state(ctx, o.lbfgs_history);
+  if (rc != APD_OK) return rc;
+  Workspace& ws = ctx->ws;
+  double domain = 1.0;
+  for (int k = 0; k < g.dim; ++k) domain *= (grid->hi[k] - grid->lo[k]);
+  StepArgs sa;
+  sa.count = ws.count; sa.vol_in = nullptr; sa.voxel_volume = g.voxel_volume;
+  sa.n_partials = (o.cull ? 4 : 1) * g.tiles_x * g.tiles_y * g.tiles_z;
+  SolveHooks hooks;
+  hooks.loop_eval = [&](const int* done_flag) {
+    return enqueue_evaluation(ctx, g, kernel, M, X, A, ws.w32, target_vol, nullptr, nullptr, nullptr, nullptr, nullptr,
+                              nullptr, false, o.cull != 0, done_flag, st, &ws.sstate->cull_rebuild,
+                              &ws.sstate->cull_delta);
+  };
+  hooks.final_eval = [&]() {
+    return enqueue_evaluation(ctx, g, kernel, M, X, A, ws.w32, target_vol, labels, vol ? vol : ws.e_vol, ws.e_scal,
+                              ws.e_scal + 1, nullptr, nullptr, true, o.cull != 0, nullptr, st);
+  };
+  return solve_common(ctx, "apd_solve", g.dim, M, target_vol, tol, w_init, w, w64, o, domain, sa, hooks, iters, evals,
+                      max_rel_err, dual, st);
+}
+
+// Algorithm 2 on a user-supplied discretisation (points with element volumes, apd_points.cu)
+extern "C" int apd_solve_points(apd_ctx* ctx, int64_t N, const float* Y, const float* pvol, double total_volume,
+                                int32_t M, const float* X, const float* A, const float* target_vol, double tol,
+                                const float* w_init, float* w, int32_t* labels, double* vol, int32_t* iters,
+                                int32_t* evals, double* max_rel_err, const apd_opts* opts, void* cuda_stream) {
+  if (!ctx) return APD_E_ARG;
+  ctx->err.clear();
+  if (M < 1 || M > ctx->ws.max_seeds) { ctx->err = "apd_solve_points: M out of range [1, max_seeds]"; return APD_E_ARG; }
+  if (!Y || !pvol || !X || !A || !target_vol || !w || N < 1) { ctx->err = "apd_solve_points: Y, pvol, X, A, target_vol and w are required"; return APD_E_ARG; }
+  if (!(total_volume > 0.0) || !std::isfinite(total_volume)) { ctx->err = "apd_solve_points: total_volume must be the (positive) sum of pvol"; return APD_E_ARG; }
+  apd_opts o;
+  int rc = check_solve_opts(ctx, "apd_solve_points", opts, tol, &o);
+  if (rc != APD_OK) return rc;
+  if (o.cull) { ctx->err = "apd_solve_points: opts.cull is not available on point sets"; return APD_E_ARG; }
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  LB_TRY(cudaSetDevice(ctx->ws.device));
+  rc = ensure_solve_state(ctx, o.lbfgs_history);
+  if (rc != APD_OK) return rc;
+  Workspace& ws = ctx->ws;
+  int n_partials = 0;
+  SolveHooks hooks;
+  hooks.loop_eval = [&](const int* done_flag) {
+    return enqueue_points(ctx, N, Y, pvol, M, X, A, ws.w32, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr,
+                          done_flag, &n_partials, st);
+  };
+  hooks.final_eval = [&]() {
+    return enqueue_points(ctx, N, Y, pvol, M, X, A, ws.w32, target_vol, labels, vol ? vol : ws.e_vol, ws.e_scal,
+                          ws.e_scal + 1, nullptr, nullptr, &n_partials, st);
+  };
+  // the first evaluation allocates the accumulators: run the sizing part now so that StepArgs can point at them
+  rc = points_prepare(ctx, N, &n_partials, st);
+  if (rc != APD_OK) return rc;
+  StepArgs sa;
+  sa.count = nullptr; sa.vol_in = ws.pt_acc; sa.voxel_volume = 1.0; sa.n_partials = n_partials;
+  return solve_common(ctx, "apd_solve_points", ws.dim, M, target_vol, tol, w_init, w, nullptr, o, total_volume, sa,
+                      hooks, iters, evals, max_rel_err, nullptr, st);
 }
 
 extern "C" int apd_solve_stats(const apd_ctx* ctx, int32_t* evals_recorded, int32_t* cull_rebuilds) {

@@ -29,7 +29,15 @@ struct PointArgs {
   double* vol;             // [M]   zeroed before the launch
   double* csum;            // [M,3] zeroed before the launch, or nullptr
   double* dual_partial;    // [n_tiles]
+  const int* done_flag;    // solve loop only
 };
+
+// zeroes the fp64 accumulators of one evaluation (a kernel, so that it can honour done_flag like the rest)
+__global__ void points_zero_kernel(int n, double* acc, const int* done_flag) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (done_flag && *done_flag) return;
+  if (i < n) acc[i] = 0.0;
+}
 
 template <int DIM>
 __global__ void __launch_bounds__(PT_THREADS) assign_points_kernel(const PointArgs a) {
@@ -38,6 +46,7 @@ __global__ void __launch_bounds__(PT_THREADS) assign_points_kernel(const PointAr
   __shared__ __align__(128) float s_seeds[SEED_STAGES][SEED_CHUNK * REC];
   __shared__ __align__(8) uint64_t s_full[SEED_STAGES];
   __shared__ double s_red[PT_THREADS / 32];
+  if (a.done_flag && *a.done_flag) return;
   const int tid = threadIdx.x;
   const long long j0 = (long long)blockIdx.x * PT_TILE + tid;
   const int nchunks = a.M_pad / SEED_CHUNK;
@@ -176,6 +185,54 @@ using namespace apd;
     }                                                                               \
   } while (0)
 
+namespace apd {
+
+int points_prepare(apd_ctx* ctx, long long N, int* n_partials, cudaStream_t st) {
+  Workspace& ws = ctx->ws;
+  const long long n_tiles_ll = (N + PT_TILE - 1) / PT_TILE;
+  if (n_tiles_ll > 0x7fffffffll) { ctx->err = "apd points: too many points"; return APD_E_ARG; }
+  const int n_tiles = (int)n_tiles_ll;
+  if ((size_t)n_tiles > ws.partial_cap) {
+    PT_TRY(cudaStreamSynchronize(st));
+    PT_TRY(cudaFree(ws.dual_partial));
+    ws.dual_partial = nullptr;
+    ws.partial_cap = (size_t)n_tiles;
+    PT_TRY(cudaMalloc(&ws.dual_partial, ws.partial_cap * sizeof(double)));
+  }
+  if (!ws.pt_acc) PT_TRY(cudaMalloc(&ws.pt_acc, (size_t)ws.max_seeds * 4 * sizeof(double)));   // vol[M] | csum[M,3]
+  *n_partials = n_tiles;
+  return APD_OK;
+}
+
+int enqueue_points(apd_ctx* ctx, long long N, const float* Y, const float* pvol, int M, const float* X, const float* A,
+                   const float* w, const float* target_vol, int32_t* labels, double* vol, double* dual,
+                   double* max_rel_err, double* centroids, const int* done_flag, int* n_partials, cudaStream_t st) {
+  Workspace& ws = ctx->ws;
+  int rc = points_prepare(ctx, N, n_partials, st);
+  if (rc != APD_OK) return rc;
+  const int d = ws.dim, n_tiles = *n_partials;
+  const int M_pad = (M + SEED_CHUNK - 1) / SEED_CHUNK * SEED_CHUNK;
+  const int n_acc = ws.max_seeds * 4;
+  points_zero_kernel<<<(n_acc + 255) / 256, 256, 0, st>>>(n_acc, ws.pt_acc, done_flag);
+  PT_TRY(cudaGetLastError());
+  PT_TRY(launch_pack_seeds(d, M, M_pad, X, A, w, ws.seeds, ws.count, nullptr, done_flag, st));
+  PointArgs a;
+  a.dim = d; a.N = N; a.M = M; a.M_pad = M_pad; a.Y = Y; a.pvol = pvol; a.seeds = ws.seeds; a.labels = labels;
+  a.vol = ws.pt_acc; a.csum = centroids ? ws.pt_acc + ws.max_seeds : nullptr; a.dual_partial = ws.dual_partial;
+  a.done_flag = done_flag;
+  if (d == 3) assign_points_kernel<3><<<n_tiles, PT_THREADS, 0, st>>>(a);
+  else        assign_points_kernel<2><<<n_tiles, PT_THREADS, 0, st>>>(a);
+  PT_TRY(cudaGetLastError());
+  if (vol) {
+    finalize_points_kernel<<<1, 1024, 0, st>>>(d, M, n_tiles, ws.pt_acc, a.csum, ws.dual_partial, X, w, target_vol, vol,
+                                               dual, max_rel_err, centroids);
+    PT_TRY(cudaGetLastError());
+  }
+  return APD_OK;
+}
+
+}  // namespace apd
+
 extern "C" int apd_assign_points(apd_ctx* ctx, int64_t N, const float* Y, const float* pvol, int32_t M, const float* X,
                                  const float* A, const float* w, const float* target_vol, int32_t* labels,
                                  double* vol, double* dual, double* max_rel_err, double* centroids,
@@ -188,29 +245,7 @@ extern "C" int apd_assign_points(apd_ctx* ctx, int64_t N, const float* Y, const 
   if (!Y || !pvol || !X || !A || !w || !vol || !dual) { ctx->err = "apd_assign_points: Y, pvol, X, A, w, vol and dual are required"; return APD_E_ARG; }
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   PT_TRY(cudaSetDevice(ws.device));
-  const int d = ws.dim;
-  const int M_pad = (M + SEED_CHUNK - 1) / SEED_CHUNK * SEED_CHUNK;
-  const long long n_tiles_ll = (N + PT_TILE - 1) / PT_TILE;
-  if (n_tiles_ll > 0x7fffffffll) { ctx->err = "apd_assign_points: too many points"; return APD_E_ARG; }
-  const int n_tiles = (int)n_tiles_ll;
-  if ((size_t)n_tiles > ws.partial_cap) {
-    PT_TRY(cudaStreamSynchronize(st));
-    PT_TRY(cudaFree(ws.dual_partial));
-    ws.dual_partial = nullptr;
-    ws.partial_cap = (size_t)n_tiles;
-    PT_TRY(cudaMalloc(&ws.dual_partial, ws.partial_cap * sizeof(double)));
-  }
-  if (!ws.pt_acc) PT_TRY(cudaMalloc(&ws.pt_acc, (size_t)ws.max_seeds * 4 * sizeof(double)));   // vol[M] | csum[M,3]
-  PT_TRY(cudaMemsetAsync(ws.pt_acc, 0, (size_t)ws.max_seeds * 4 * sizeof(double), st));
-  PT_TRY(launch_pack_seeds(d, M, M_pad, X, A, w, ws.seeds, ws.count, nullptr, nullptr, st));
-  PointArgs a;
-  a.dim = d; a.N = N; a.M = M; a.M_pad = M_pad; a.Y = Y; a.pvol = pvol; a.seeds = ws.seeds; a.labels = labels;
-  a.vol = ws.pt_acc; a.csum = centroids ? ws.pt_acc + ws.max_seeds : nullptr; a.dual_partial = ws.dual_partial;
-  if (d == 3) assign_points_kernel<3><<<n_tiles, PT_THREADS, 0, st>>>(a);
-  else        assign_points_kernel<2><<<n_tiles, PT_THREADS, 0, st>>>(a);
-  PT_TRY(cudaGetLastError());
-  finalize_points_kernel<<<1, 1024, 0, st>>>(d, M, n_tiles, ws.pt_acc, a.csum, ws.dual_partial, X, w, target_vol, vol,
-                                             dual, max_rel_err, centroids);
-  PT_TRY(cudaGetLastError());
-  return APD_OK;
+  int n_partials = 0;
+  return enqueue_points(ctx, N, Y, pvol, M, X, A, w, target_vol, labels, vol, dual, max_rel_err, centroids, nullptr,
+                        &n_partials, st);
 }

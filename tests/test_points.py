@@ -134,3 +134,45 @@ def test_gpu_points_on_grid_centres_match_apd_assign(apd):
     assert np.array_equal(labels, lab2.cpu().numpy())
     np.testing.assert_allclose(vol, vol2.cpu().numpy(), rtol=1e-12, atol=0)
     assert abs(dual - float(d2.item())) <= 1e-12 * abs(dual)
+
+
+# ------------------------------------------------------------------------------------------------ Algorithm 2 on points
+def test_oracle_solve_on_points_equals_solve_on_grid():
+    """oracle_solve fed the voxel centres of a grid as a PointSet walks the same trajectory as on the Grid itself."""
+    from oracle.apd_oracle import PointSet, oracle_solve
+    wl = workloads.make_config(1)
+    Y, p = grid_points(wl)
+    a = oracle_solve(Grid(2, wl.n, wl.lo, wl.hi), wl.X, wl.A, wl.v, 0.01)
+    b = oracle_solve(PointSet(Y, p), wl.X, wl.A, wl.v, 0.01)
+    assert (a.status, a.iters, a.evals) == (b.status, b.iters, b.evals)
+    np.testing.assert_allclose(b.w, a.w, rtol=0, atol=1e-9 * np.abs(a.w).max())
+
+
+@pytest.mark.gpu
+def test_gpu_solve_points(apd):
+    """Monte-Carlo discretisation of the unit square (random points, equal volumes): apd_solve_points reaches the
+    tolerance as judged by the ORACLE at the GPU's weights; the optimisers walk closely related paths."""
+    import torch
+    from oracle.apd_oracle import PointSet, oracle_solve
+    rng = np.random.default_rng(5)
+    wl = workloads.make_config(2, n=(8, 8), M=30)
+    N = 60000
+    Y = rng.random((N, 2)).astype(np.float32)
+    p = np.full(N, 1.0 / N, np.float32)
+    tot = float(p.astype(np.float64).sum())
+    wl.v[:] = (wl.v.astype(np.float64) / wl.v.astype(np.float64).sum() * tot).astype(np.float32)
+    orc = oracle_solve(PointSet(Y, p), wl.X, wl.A, wl.v, 0.02)
+    dev = torch.device("cuda:0")
+    ctx = apd.ApdContext(2, wl.M)
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    w = torch.zeros(wl.M, dtype=torch.float32, device=dev)
+    labels = torch.full((N,), -1, dtype=torch.int32, device=dev); vol = torch.zeros(wl.M, dtype=torch.float64, device=dev)
+    info = ctx.apd_solve_points(t(Y), t(p), tot, t(wl.X), t(wl.A), t(wl.v), 0.02, w=w, labels=labels, vol=vol)
+    assert info.status == orc.status == 0 and info.max_rel_err <= 0.02
+    chk = oracle_assign_points(Y, p, wl.X, wl.A, w.cpu().numpy(), v=wl.v)
+    nm = int((labels.cpu().numpy() != chk.labels).sum())
+    assert nm < max(1e-5 * N, 1) or nm == 0
+    assert chk.err <= 0.02 + 2 * nm / N / float(wl.v.min())
+    np.testing.assert_allclose(vol.cpu().numpy(), chk.vol, rtol=0, atol=2 * nm / N + 1e-12)
+    assert abs(info.evals - orc.evals) <= max(4, orc.evals // 4)
+    print(f"solve on points: gpu {info.iters}/{info.evals} err {info.max_rel_err:.4g}; oracle {orc.iters}/{orc.evals}")
