@@ -270,13 +270,15 @@ def run_ours(args):
     hlab = torch.empty(wl.N, dtype=torch.int32).pin_memory()
     hvol = torch.empty(wl.M, dtype=torch.float64).pin_memory()
     e2e_steps = max(3, min(args.steps, 10))
-    ctx.apd_assign_host(grid, hX, hA, hw, target_vol=hv, labels=hlab, vol=hvol, opts=opts)
-    barrier()
-    te = time.perf_counter()
-    for _ in range(e2e_steps):
+    for _ in range(2):
         ctx.apd_assign_host(grid, hX, hA, hw, target_vol=hv, labels=hlab, vol=hvol, opts=opts)
-    torch.cuda.synchronize()
-    e2e_s = (time.perf_counter() - te) / e2e_steps
+    barrier()
+    e2e_each = []
+    for _ in range(e2e_steps):
+        te = time.perf_counter()
+        ctx.apd_assign_host(grid, hX, hA, hw, target_vol=hv, labels=hlab, vol=hvol, opts=opts)   # synchronous
+        e2e_each.append(time.perf_counter() - te)
+    e2e_s = float(np.median(e2e_each))       # per-call wall times; the median shrugs off a host hiccup (max reported)
     e2e_s = max_over_ranks(e2e_s, world, dev)
     h2d = 4 * (hX.numel() + hA.numel() + hw.numel() + hv.numel())
     d2h = 4 * hlab.numel() + 8 * hvol.numel() + 16 + 8
@@ -381,7 +383,8 @@ def run_ours(args):
                            "multi_gpu": "replicas only (no data-path collective)", "kernel": kernel_id},
                 "clocks": clocks, "roofline": roofline, "cpu_baseline": cb,
                 "e2e": {"value": world * wl.pairs / e2e_s / 1e9, "unit": UNIT, "h2d_bytes_per_step": h2d,
-                        "d2h_bytes_per_step": d2h, "ms_per_step": e2e_s * 1e3, "steps": e2e_steps,
+                        "d2h_bytes_per_step": d2h, "ms_per_step": e2e_s * 1e3, "ms_per_step_max": max(e2e_each) * 1e3,
+                        "steps": e2e_steps,
                         "call": "apd_assign_host (pinned host buffers; device alloc + copies inside)"},
                 "gpu_launches": 3 * args.steps, "launches_per_step": ["pack_pairs_kernel", "assign_rowpoly_kernel",
                                                                       "finalize_kernel"]}
