@@ -77,6 +77,7 @@ constexpr int LB_NRED = 13;                          // most values reduced at o
 struct Reducer {
   double* wbuf;        // [LB_THREADS / 32][LB_NRED]   warp partials of this CTA
   double* cbuf;        // [2][LB_NRED]                 CTA totals, read by the other CTAs of the cluster
+  double* tot;         // [LB_NRED]                    cluster totals, for this CTA's threads
   int flip;
   unsigned int rank;
 };
@@ -111,16 +112,20 @@ __device__ __forceinline__ void cluster_all(double (&v)[N], Reducer& r) {
     mine[threadIdx.x] = t;
   }
   cluster.sync();                                    // every CTA's totals are written and visible
-#pragma unroll
-  for (int n = 0; n < N; ++n) {
-    double t = cluster.map_shared_rank(mine, 0)[n];
+  // N threads fetch the other CTAs' totals (one distributed-shared-memory read each: every thread reading all of
+  // them cost more than the sweeps), add them in rank order and hand the result to the CTA through shared memory
+  if (threadIdx.x < N) {
+    double t = cluster.map_shared_rank(mine, 0)[threadIdx.x];
 #pragma unroll
     for (int c = 1; c < LB_CLUSTER; ++c) {
-      const double u = cluster.map_shared_rank(mine, c)[n];
+      const double u = cluster.map_shared_rank(mine, c)[threadIdx.x];
       t = MAX ? fmax(t, u) : t + u;
     }
-    v[n] = t;
+    r.tot[threadIdx.x] = t;
   }
+  __syncthreads();
+#pragma unroll
+  for (int n = 0; n < N; ++n) v[n] = r.tot[n];
 }
 
 __device__ __forceinline__ double cluster_allsum(double x, Reducer& r) {
@@ -294,9 +299,10 @@ __global__ void solve_init_kernel(StepArgs a, const float* w_init, int hist_cap,
 __global__ void __cluster_dims__(LB_CLUSTER, 1, 1) __launch_bounds__(LB_THREADS) lbfgs_step_kernel(StepArgs a) {
   __shared__ double s_wbuf[(LB_THREADS / 32) * LB_NRED];
   __shared__ double s_cbuf[2 * LB_NRED];
+  __shared__ double s_tot[LB_NRED];
   extern __shared__ double s_dyn[];        // direction_vf: compact Gram matrix, coefficients (sized by the launch)
   cg::cluster_group cluster = cg::this_cluster();
-  Reducer red{s_wbuf, s_cbuf, 0, cluster.block_rank()};
+  Reducer red{s_wbuf, s_cbuf, s_tot, 0, cluster.block_rank()};
   SolveState* st = a.st;
   if (st->done) return;                    // uniform: written by the previous launch
   const bool lead = red.rank == 0;
