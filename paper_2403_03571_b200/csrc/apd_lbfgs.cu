@@ -11,8 +11,9 @@
 //   * curvature pair kept iff s.y > 1e-12 |s||y|; then gamma = s.y / y.y
 //   * line-search failure: clear the history and retry with p = -gamma g; with an empty history
 //     NOT_CONVERGED; NOT_CONVERGED returns the evaluated point with the smallest error.
-// The whole state machine is ONE single-CTA kernel (lbfgs_step_kernel) that runs after each
-// evaluation on the same stream; the host only reads the mapped SolveReport.done word.
+// The whole state machine is ONE kernel (lbfgs_step_kernel, a cluster of LB_CLUSTER CTAs) that runs after each
+// evaluation on the same stream; the host only reads the mapped SolveReport.done word.  The same loop serves voxel
+// grids (apd_solve) and user-supplied point sets (apd_solve_points).
 #include "apd_internal.cuh"
 #include "apd_device.cuh"
 #include <cmath>
