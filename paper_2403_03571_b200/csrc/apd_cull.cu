@@ -275,126 +275,222 @@ __global__ void __launch_bounds__(CULL_THREADS) cull_super_kernel(const CullArgs
   if (tid == 0) c.super_count[b] = (base <= SUPER_CAP) ? base : -1;
 }
 
-// LEVEL 2 -- one CTA per CTA tile of the culled kernel.  (a) The 4 warps together cut the super-tile's parent list
-// (all seeds if that overflowed) down to the seeds that can win somewhere in the CTA TILE, kept in shared memory;
-// (b) each warp then cuts that list down to its own brick.  Same two passes (U = min upper bound, ordered
-// compaction of lower bound <= U) at both steps.
+// One seed's record in registers: position, matrix (doubled off-diagonals), -w.
+template <int DIM>
+struct SeedRec {
+  float x, y, z, a11, a12, a13, a22, a23, a33, nw;
+  __device__ __forceinline__ void load(const float* __restrict__ rec, int i) {
+    if (DIM == 3) {
+      const float4* p = reinterpret_cast<const float4*>(rec + (size_t)i * REC3);
+      const float4 p0 = __ldg(p), p1 = __ldg(p + 1), p2 = __ldg(p + 2);
+      x = p0.x; y = p0.y; z = p0.z; a11 = p0.w; a12 = p1.x; a13 = p1.y; a22 = p1.z; a23 = p1.w; a33 = p2.x; nw = p2.y;
+    } else {
+      const float4* p = reinterpret_cast<const float4*>(rec + (size_t)i * REC2);
+      const float4 p0 = __ldg(p), p1 = __ldg(p + 1);
+      x = p0.x; y = p0.y; z = 0.0f; a11 = p0.z; a12 = p0.w; a13 = 0.0f; a22 = p1.x; a23 = 0.0f; a33 = 0.0f; nw = p1.y;
+    }
+  }
+  // rho of a box with half-extents h (does not depend on where the box is)
+  __device__ __forceinline__ float radius(float3 h) const {
+    if (DIM == 3) {
+      const float r[9] = {0.f, 0.f, 0.f, a11, a12, a13, a22, a23, a33};
+      return box_radius<3>(r, h.x, h.y, h.z);
+    } else {
+      const float r[5] = {0.f, 0.f, a11, a12, a22};
+      return box_radius<2>(r, h.x, h.y, 0.0f);
+    }
+  }
+  // s and supp of seed_bounds() for the box y0 +- h -- the same expressions in the same order
+  __device__ __forceinline__ void at(float y0x, float y0y, float y0z, float3 h, float* s, float* supp) const {
+    if (DIM == 3) {
+      const float dx = y0x - x, dy = y0y - y, dz = y0z - z;
+      const float gx = fmaf(0.5f * a13, dz, fmaf(0.5f * a12, dy, a11 * dx));
+      const float gy = fmaf(0.5f * a23, dz, fmaf(a22, dy, 0.5f * a12 * dx));
+      const float gz = fmaf(a33, dz, fmaf(0.5f * a23, dy, 0.5f * a13 * dx));
+      const float q = fmaf(dz, gz, fmaf(dy, gy, dx * gx));
+      *s = sqrtf(fmaxf(q, 0.0f));
+      *supp = fmaf(fabsf(gz), h.z, fmaf(fabsf(gy), h.y, fabsf(gx) * h.x));
+    } else {
+      const float dx = y0x - x, dy = y0y - y;
+      const float gx = fmaf(0.5f * a12, dy, a11 * dx);
+      const float gy = fmaf(a22, dy, 0.5f * a12 * dx);
+      const float q = fmaf(dy, gy, dx * gx);
+      *s = sqrtf(fmaxf(q, 0.0f));
+      *supp = fmaf(fabsf(gy), h.y, fabsf(gx) * h.x);
+    }
+  }
+};
+
+// LEVEL 2 -- one CTA per run of CULL_G CTA tiles adjacent in x (the tiles of one super-tile row, so they share the
+// parent list).  (a) The 4 warps together cut the super-tile's parent list (all seeds if that overflowed) down, for
+// each of the CULL_G tiles, to the seeds that can win somewhere in that CTA TILE, kept in shared memory: every parent
+// record is gathered ONCE per pass and tested against the CULL_G boxes, which is what this kernel is bound by;
+// (b) for each tile in turn, each warp cuts the tile's list down to its own brick.  Same two passes (U = min upper
+// bound, ordered compaction of lower bound <= U) at both steps.
 constexpr int TILE_CAP = 768;
+constexpr int CULL_G = 4;
+static_assert(CULL_G == SUPER3_TX && CULL_G == SUPER2_TX, "a CTA of cull_bricks_kernel covers one super-tile row");
 template <int DIM>
 __global__ void __launch_bounds__(128) cull_bricks_kernel(const CullArgs c) {
-  __shared__ int s_tile[TILE_CAP];
-  __shared__ float s_min[4];
-  __shared__ int s_imin[4];
-  __shared__ int s_wsum[4];
+  __shared__ int s_tile[CULL_G][TILE_CAP];
+  __shared__ float s_min[CULL_G][4];
+  __shared__ int s_imin[CULL_G][4];
+  __shared__ int s_wsum[4][CULL_G];
   if (c.done_flag && *c.done_flag) return;
   if (c.rebuild && !*c.rebuild) return;
   const float delta = c.delta ? *c.delta : 0.0f;
   const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
   const int b = blockIdx.x;
-  const int bx = b % c.g.tiles_x, by = (b / c.g.tiles_x) % c.g.tiles_y, bz = b / (c.g.tiles_x * c.g.tiles_y);
+  const int qx = b % c.nsx, by = (b / c.nsx) % c.g.tiles_y, bz = b / (c.nsx * c.g.tiles_y);
   constexpr int TX = (DIM == 3) ? CULL_TILE3_X : CULL_TILE2_X, TY = (DIM == 3) ? CULL_TILE3_Y : CULL_TILE2_Y,
                 TZ = (DIM == 3) ? CULL_TILE3_Z : 1;
-  constexpr int STX = (DIM == 3) ? SUPER3_TX : SUPER2_TX, STY = (DIM == 3) ? SUPER3_TY : SUPER2_TY,
-                STZ = (DIM == 3) ? SUPER3_TZ : 1;
-  const int sup = ((bz / STZ) * c.nsy + by / STY) * c.nsx + bx / STX;
-  int n = c.super_count[sup];
-  const int* plist = c.super_list + (size_t)sup * SUPER_CAP;
-  if (n < 0) { n = c.M; plist = nullptr; }
+  constexpr int STY = (DIM == 3) ? SUPER3_TY : SUPER2_TY, STZ = (DIM == 3) ? SUPER3_TZ : 1;
+  const int sup = ((bz / STZ) * c.nsy + by / STY) * c.nsx + qx;
+  const int ng = min(CULL_G, c.g.tiles_x - qx * CULL_G);      // tiles of this run inside the grid
+  int n_par = c.super_count[sup];
+  const int* par = c.super_list + (size_t)sup * SUPER_CAP;
+  if (n_par < 0) { n_par = c.M; par = nullptr; }
 
-  // (a) CTA-tile list
+  // (a) CTA-tile lists
+  int n_tile[CULL_G];
   {
-    const float t0x = box_centre(c.g.lo[0], c.g.s[0], bx * TX, TX);
+    float t0x[CULL_G];
+#pragma unroll
+    for (int g = 0; g < CULL_G; ++g) t0x[g] = box_centre(c.g.lo[0], c.g.s[0], (qx * CULL_G + g) * TX, TX);
     const float t0y = box_centre(c.g.lo[1], c.g.s[1], by * TY, TY);
     const float t0z = (DIM == 3) ? box_centre(c.g.lo[2], c.g.s[2], bz * TZ, TZ) : 0.0f;
+    float umin[CULL_G];
+    int imin[CULL_G];
+#pragma unroll
+    for (int g = 0; g < CULL_G; ++g) { umin[g] = CUDART_INF_F; imin[g] = 0; }
+    for (int pos = tid; pos < n_par; pos += 128) {
+      const int i = par ? __ldg(par + pos) : pos;
+      SeedRec<DIM> r;
+      r.load(c.rec, i);
+      const float rho = r.radius(c.ht);
+#pragma unroll
+      for (int g = 0; g < CULL_G; ++g) {
+        float s, supp;
+        r.at(t0x[g], t0y, t0z, c.ht, &s, &supp);
+        const float u = upper_bound(s, rho, r.nw);
+        if (u < umin[g]) { umin[g] = u; imin[g] = i; }
+      }
+    }
+#pragma unroll
+    for (int g = 0; g < CULL_G; ++g) {
+      warp_argmin(umin[g], imin[g]);
+      if (lane == 0) { s_min[g][w] = umin[g]; s_imin[g][w] = imin[g]; }
+    }
+    __syncthreads();
+    float U[CULL_G];
+#pragma unroll
+    for (int g = 0; g < CULL_G; ++g) {
+      float u = s_min[g][0];
+      int kbest = s_imin[g][0];
+#pragma unroll
+      for (int j = 1; j < 4; ++j) if (s_min[g][j] < u) { u = s_min[g][j]; kbest = s_imin[g][j]; }
+      if (n_par > 0) u = fminf(u, exact_upper<DIM>(c.rec, kbest, t0x[g], t0y, t0z, c.ht));
+      U[g] = u + 2.0f * delta * (1.0f + CULL_EPS);
+    }
+    int base[CULL_G];
+#pragma unroll
+    for (int g = 0; g < CULL_G; ++g) base[g] = 0;
+    for (int p0 = 0; p0 < n_par; p0 += 128) {
+      const int pos = p0 + tid;
+      bool keep[CULL_G];
+#pragma unroll
+      for (int g = 0; g < CULL_G; ++g) keep[g] = false;
+      int i = 0;
+      if (pos < n_par) {
+        i = par ? __ldg(par + pos) : pos;
+        SeedRec<DIM> r;
+        r.load(c.rec, i);
+#pragma unroll
+        for (int g = 0; g < CULL_G; ++g) {
+          float s, supp;
+          r.at(t0x[g], t0y, t0z, c.ht, &s, &supp);
+          keep[g] = !(lower_bound(s, supp, r.nw) > U[g]);      // NaN keeps the seed
+        }
+      }
+      unsigned int bal[CULL_G];
+#pragma unroll
+      for (int g = 0; g < CULL_G; ++g) bal[g] = __ballot_sync(0xffffffffu, keep[g]);
+      __syncthreads();                       // s_wsum of the previous round has been read
+      if (lane < CULL_G) {
+        unsigned int m = bal[0];
+#pragma unroll
+        for (int g = 1; g < CULL_G; ++g) if (lane == g) m = bal[g];
+        s_wsum[w][lane] = __popc(m);
+      }
+      __syncthreads();
+#pragma unroll
+      for (int g = 0; g < CULL_G; ++g) {
+        int off = base[g], tot = 0;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) { const int m = s_wsum[k][g]; if (k < w) off += m; tot += m; }
+        if (keep[g]) {
+          const int q = off + __popc(bal[g] & ((1u << lane) - 1u));
+          if (q < TILE_CAP) s_tile[g][q] = i;
+        }
+        base[g] += tot;
+      }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int g = 0; g < CULL_G; ++g) n_tile[g] = (base[g] <= TILE_CAP) ? base[g] : -1;   // -1: bricks cut the parent list
+  }
+
+  // (b) brick lists, tile by tile
+  int ox, oy, oz, ex, ey, ez;
+  brick_box(DIM, w, &ox, &oy, &oz, &ex, &ey, &ez);
+  const float y0y = box_centre(c.g.lo[1], c.g.s[1], by * TY + oy, ey);
+  const float y0z = (DIM == 3) ? box_centre(c.g.lo[2], c.g.s[2], bz * TZ + oz, ez) : 0.0f;
+#pragma unroll
+  for (int g = 0; g < CULL_G; ++g) {
+    if (g >= ng) break;
+    const int bx = qx * CULL_G + g;
+    const bool from_smem = n_tile[g] >= 0;
+    const int n = from_smem ? n_tile[g] : n_par;
+    const int* tl = s_tile[g];
+    auto cand = [&](int pos) { return from_smem ? tl[pos] : (par ? __ldg(par + pos) : pos); };
+    const float y0x = box_centre(c.g.lo[0], c.g.s[0], bx * TX + ox, ex);
+
     float umin = CUDART_INF_F;
     int imin = 0;
-    for (int pos = tid; pos < n; pos += 128) {
-      const int i = plist ? __ldg(plist + pos) : pos;
+    for (int pos = lane; pos < n; pos += 32) {
+      const int i = cand(pos);
       float s, rho, supp, nw;
-      seed_bounds<DIM, 2>(c.rec, i, t0x, t0y, t0z, c.ht, &s, &rho, &supp, &nw);
+      seed_bounds<DIM, 0>(c.rec, i, y0x, y0y, y0z, c.hb, &s, &rho, &supp, &nw);
       const float u = upper_bound(s, rho, nw);
       if (u < umin) { umin = u; imin = i; }
     }
     warp_argmin(umin, imin);
-    if (lane == 0) { s_min[w] = umin; s_imin[w] = imin; }
-    __syncthreads();
-    float U = s_min[0];
-    int kbest = s_imin[0];
-#pragma unroll
-    for (int j = 1; j < 4; ++j) if (s_min[j] < U) { U = s_min[j]; kbest = s_imin[j]; }
-    if (n > 0) U = fminf(U, exact_upper<DIM>(c.rec, kbest, t0x, t0y, t0z, c.ht));
-    U += 2.0f * delta * (1.0f + CULL_EPS);
+    if (n > 0) umin = fminf(umin, exact_upper<DIM>(c.rec, imin, y0x, y0y, y0z, c.hb));
+    const float U = umin + 2.0f * delta * (1.0f + CULL_EPS);
+
+    const size_t tile = ((size_t)bz * c.g.tiles_y + by) * c.g.tiles_x + bx;
+    const size_t brick = tile * 4 + w;
+    int* list = c.brick_list + brick * BRICK_CAP;
     int base = 0;
-    for (int p0 = 0; p0 < n; p0 += 128) {
-      const int pos = p0 + tid;
+    for (int p0 = 0; p0 < n; p0 += 32) {
+      const int pos = p0 + lane;
       bool keep = false;
       int i = 0;
       if (pos < n) {
-        i = plist ? __ldg(plist + pos) : pos;
+        i = cand(pos);
         float s, rho, supp, nw;
-        seed_bounds<DIM, 2>(c.rec, i, t0x, t0y, t0z, c.ht, &s, &rho, &supp, &nw);
+        seed_bounds<DIM, 0>(c.rec, i, y0x, y0y, y0z, c.hb, &s, &rho, &supp, &nw);
         keep = !(lower_bound(s, supp, nw) > U);
       }
       const unsigned int bal = __ballot_sync(0xffffffffu, keep);
-      __syncthreads();                       // s_wsum of the previous round has been read
-      if (lane == 0) s_wsum[w] = __popc(bal);
-      __syncthreads();
-      int off = base, tot = 0;
-#pragma unroll
-      for (int k = 0; k < 4; ++k) { const int m = s_wsum[k]; if (k < w) off += m; tot += m; }
       if (keep) {
-        const int q = off + __popc(bal & ((1u << lane) - 1u));
-        if (q < TILE_CAP) s_tile[q] = i;
+        const int q = base + __popc(bal & ((1u << lane) - 1u));
+        if (q < BRICK_CAP) list[q] = i;
       }
-      base += tot;
+      base += __popc(bal);
     }
-    __syncthreads();
-    if (base <= TILE_CAP) { n = base; plist = s_tile; }      // else: the bricks cut the parent list directly
+    if (lane == 0) c.brick_count[brick] = (base <= BRICK_CAP) ? base : -1;
   }
-  const bool from_smem = (plist == s_tile);
-  auto cand = [&](int pos) { return from_smem ? s_tile[pos] : (plist ? __ldg(plist + pos) : pos); };
-
-  // (b) brick lists
-  int ox, oy, oz, ex, ey, ez;
-  brick_box(DIM, w, &ox, &oy, &oz, &ex, &ey, &ez);
-  const float y0x = box_centre(c.g.lo[0], c.g.s[0], bx * TX + ox, ex);
-  const float y0y = box_centre(c.g.lo[1], c.g.s[1], by * TY + oy, ey);
-  const float y0z = (DIM == 3) ? box_centre(c.g.lo[2], c.g.s[2], bz * TZ + oz, ez) : 0.0f;
-
-  float umin = CUDART_INF_F;
-  int imin = 0;
-  for (int pos = lane; pos < n; pos += 32) {
-    const int i = cand(pos);
-    float s, rho, supp, nw;
-    seed_bounds<DIM, 0>(c.rec, i, y0x, y0y, y0z, c.hb, &s, &rho, &supp, &nw);
-    const float u = upper_bound(s, rho, nw);
-    if (u < umin) { umin = u; imin = i; }
-  }
-  warp_argmin(umin, imin);
-  if (n > 0) umin = fminf(umin, exact_upper<DIM>(c.rec, imin, y0x, y0y, y0z, c.hb));
-  const float U = umin + 2.0f * delta * (1.0f + CULL_EPS);
-
-  const size_t brick = (size_t)b * 4 + w;
-  int* list = c.brick_list + brick * BRICK_CAP;
-  int base = 0;
-  for (int p0 = 0; p0 < n; p0 += 32) {
-    const int pos = p0 + lane;
-    bool keep = false;
-    int i = 0;
-    if (pos < n) {
-      i = cand(pos);
-      float s, rho, supp, nw;
-      seed_bounds<DIM, 0>(c.rec, i, y0x, y0y, y0z, c.hb, &s, &rho, &supp, &nw);
-      keep = !(lower_bound(s, supp, nw) > U);
-    }
-    const unsigned int bal = __ballot_sync(0xffffffffu, keep);
-    if (keep) {
-      const int q = base + __popc(bal & ((1u << lane) - 1u));
-      if (q < BRICK_CAP) list[q] = i;
-    }
-    base += __popc(bal);
-  }
-  if (lane == 0) c.brick_count[brick] = (base <= BRICK_CAP) ? base : -1;
 }
 
 void cull_super_counts(const GridDev& g, int* nsx, int* nsy, int* nsz) {
@@ -432,13 +528,13 @@ cudaError_t launch_cull(const GridDev& g, int M, int M_pad, const float* X, cons
   c.ht = make_float3(half(g.dim == 3 ? CULL_TILE3_X : CULL_TILE2_X, 0), half(g.dim == 3 ? CULL_TILE3_Y : CULL_TILE2_Y, 1),
                      g.dim == 3 ? half(CULL_TILE3_Z, 2) : 0.0f);
   const int n_super = nsx * nsy * nsz;
-  const int n_tiles = g.tiles_x * g.tiles_y * g.tiles_z;
+  const int n_runs = nsx * g.tiles_y * g.tiles_z;      // runs of CULL_G tiles along x
   if (g.dim == 3) cull_super_kernel<3><<<n_super, CULL_THREADS, 0, st>>>(c);
   else            cull_super_kernel<2><<<n_super, CULL_THREADS, 0, st>>>(c);
   e = cudaGetLastError();
   if (e != cudaSuccess) return e;
-  if (g.dim == 3) cull_bricks_kernel<3><<<n_tiles, 128, 0, st>>>(c);
-  else            cull_bricks_kernel<2><<<n_tiles, 128, 0, st>>>(c);
+  if (g.dim == 3) cull_bricks_kernel<3><<<n_runs, 128, 0, st>>>(c);
+  else            cull_bricks_kernel<2><<<n_runs, 128, 0, st>>>(c);
   return cudaGetLastError();
 }
 
