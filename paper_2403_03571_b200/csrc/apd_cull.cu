@@ -40,6 +40,10 @@ __device__ __forceinline__ float box_radius(const float* r, float hx, float hy, 
   return sqrtf(fmaxf(q, 0.0f)) * (1.0f + 4.0f * CULL_EPS);
 }
 
+// sqrt(q) by the hardware reciprocal square root (2 ulp, against the 2^-16 slack every bound carries), 0 for q <= 0;
+// the bound passes are instruction-bound and IEEE sqrt / division are ~10 instructions each
+__device__ __forceinline__ float norm_of(float q) { return q > 0.0f ? q * rsqrtf(q) : 0.0f; }
+
 // Per-seed record table in the DIRECT layout (apd_internal.cuh) plus rho_i of a brick and of a super-tile in the
 // two spare slots.  hb = half-extents of the box of voxel centres of a brick, hs = of a super-tile.
 template <int DIM>
@@ -114,7 +118,7 @@ __device__ __forceinline__ void seed_bounds(const float* __restrict__ rec, int i
     const float gy = fmaf(0.5f * p1.w, dz, fmaf(p1.z, dy, 0.5f * p1.x * dx));
     const float gz = fmaf(p2.x, dz, fmaf(0.5f * p1.w, dy, 0.5f * p1.y * dx));
     const float q = fmaf(dz, gz, fmaf(dy, gy, dx * gx));
-    *s = sqrtf(fmaxf(q, 0.0f)); *nw = p2.y;
+    *s = norm_of(q); *nw = p2.y;
     *supp = fmaf(fabsf(gz), h.z, fmaf(fabsf(gy), h.y, fabsf(gx) * h.x));
     if (SLOT == 2) {
       const float r[9] = {0.f, 0.f, 0.f, p0.w, p1.x, p1.y, p1.z, p1.w, p2.x};
@@ -129,7 +133,7 @@ __device__ __forceinline__ void seed_bounds(const float* __restrict__ rec, int i
     const float gx = fmaf(0.5f * p0.w, dy, p0.z * dx);
     const float gy = fmaf(p1.x, dy, 0.5f * p0.w * dx);
     const float q = fmaf(dy, gy, dx * gx);
-    *s = sqrtf(fmaxf(q, 0.0f)); *nw = p1.y;
+    *s = norm_of(q); *nw = p1.y;
     *supp = fmaf(fabsf(gy), h.y, fabsf(gx) * h.x);
     if (SLOT == 2) {
       const float r[5] = {0.f, 0.f, p0.z, p0.w, p1.x};
@@ -147,7 +151,7 @@ __device__ __forceinline__ float upper_bound(float s, float rho, float nw) {
 // Cauchy-Schwarz in the A-inner product: |d0 + t|_A >= <d0 + t, d0>_A / |d0|_A = s + t^T A d0 / s >= s - supp / s
 // (this dominates the ball bound s - rho, since supp <= rho s).  s = 0 gives 0 (fmaxf drops the NaN of 0/0).
 __device__ __forceinline__ float lower_bound(float s, float supp, float nw) {
-  const float r = fmaxf(s * (1.0f - CULL_EPS) - supp * (1.0f + 4.0f * CULL_EPS) / s, 0.0f);
+  const float r = fmaxf(s * (1.0f - CULL_EPS) - __fdividef(supp * (1.0f + 4.0f * CULL_EPS), s), 0.0f);
   return r * r * (1.0f - CULL_EPS) + nw - CULL_EPS * fabsf(nw);
 }
 
@@ -308,14 +312,14 @@ struct SeedRec {
       const float gy = fmaf(0.5f * a23, dz, fmaf(a22, dy, 0.5f * a12 * dx));
       const float gz = fmaf(a33, dz, fmaf(0.5f * a23, dy, 0.5f * a13 * dx));
       const float q = fmaf(dz, gz, fmaf(dy, gy, dx * gx));
-      *s = sqrtf(fmaxf(q, 0.0f));
+      *s = norm_of(q);
       *supp = fmaf(fabsf(gz), h.z, fmaf(fabsf(gy), h.y, fabsf(gx) * h.x));
     } else {
       const float dx = y0x - x, dy = y0y - y;
       const float gx = fmaf(0.5f * a12, dy, a11 * dx);
       const float gy = fmaf(a22, dy, 0.5f * a12 * dx);
       const float q = fmaf(dy, gy, dx * gx);
-      *s = sqrtf(fmaxf(q, 0.0f));
+      *s = norm_of(q);
       *supp = fmaf(fabsf(gy), h.y, fabsf(gx) * h.x);
     }
   }
