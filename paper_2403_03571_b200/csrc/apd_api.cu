@@ -120,13 +120,21 @@ std::string make_grid(const apd_ctx* ctx, const apd_grid* grid, int kernel, bool
   return "";
 }
 
-int resolve_kernel(const apd_opts* o, std::string* err) {
+// opts -> kernel (AUTO resolved) and whether culling runs.  AUTO on a grid narrower than ROW_MIN_NX voxels in x
+// takes DIRECT and drops opts.cull: the row kernels expand the cost about a row's midpoint, which on such a grid lies
+// several domain widths outside it, and the cancellation costs (1 + 8/nx)^2 in relative precision.
+constexpr int ROW_MIN_NX = 8;
+int resolve_kernel(const apd_opts* o, const apd_grid* grid, bool* cull, std::string* err) {
   int k = o ? o->kernel : APD_KERNEL_AUTO;
   if (k != APD_KERNEL_AUTO && k != APD_KERNEL_DIRECT && k != APD_KERNEL_ROWPOLY) { *err = "unknown opts.kernel"; return -1; }
   if (o && (o->cull != 0 && o->cull != 1)) { *err = "opts.cull must be 0 or 1"; return -1; }
   if (o && (o->reserved[0] || o->reserved[1] || o->reserved[2])) { *err = "opts.reserved must be 0"; return -1; }
-  if (k == APD_KERNEL_AUTO) k = APD_KERNEL_ROWPOLY;
-  if (o && o->cull && k != APD_KERNEL_ROWPOLY) { *err = "opts.cull needs kernel AUTO or ROWPOLY"; return -1; }
+  *cull = o && o->cull;
+  if (k == APD_KERNEL_AUTO) {
+    if (grid && grid->n[0] < ROW_MIN_NX) { *cull = false; return APD_KERNEL_DIRECT; }
+    k = APD_KERNEL_ROWPOLY;
+  }
+  if (*cull && k != APD_KERNEL_ROWPOLY) { *err = "opts.cull needs kernel AUTO or ROWPOLY"; return -1; }
   return k;
 }
 
@@ -157,7 +165,11 @@ int enqueue_evaluation(apd_ctx* ctx, const GridDev& g, int kernel, int M, const 
                                         centroids ? ws.idxsum : nullptr, done_flag, st));
   AssignArgs a;
   a.g = g; a.M = M; a.M_pad = M_pad; a.seeds = ws.seeds; a.labels = labels; a.count = ws.count;
-  for (int k = 0; k < 32; ++k) a.tt[k] = (float)((double)k * g.s[0]);
+  for (int j = 0; j < 16; ++j) {      // in-row offsets from a row's midpoint and their squares (apd_rowpoly.cu: RowTau)
+    const double tau = ((double)j + 0.5) * g.s[0];
+    a.tt[j] = (float)tau;
+    a.tt[16 + j] = (float)(tau * tau);
+  }
   a.idxsum = centroids ? ws.idxsum : nullptr; a.dual_partial = ws.dual_partial;
   a.rec = nullptr; a.brick_list = nullptr; a.brick_count = nullptr; a.super_list = nullptr; a.super_count = nullptr;
   a.super_x = a.super_y = 0; a.pairs_ctr = nullptr;
@@ -207,16 +219,17 @@ extern "C" int apd_assign(apd_ctx* ctx, const apd_grid* grid, int32_t M, const f
   if (!ctx) return APD_E_ARG;
   ctx->err.clear();
   std::string e;
-  const int kernel = resolve_kernel(opts, &e);
+  bool cull = false;
+  const int kernel = resolve_kernel(opts, grid, &cull, &e);
   if (kernel < 0) { ctx->err = "apd_assign: " + e; return APD_E_ARG; }
   if (M < 1 || M > ctx->ws.max_seeds) { ctx->err = "apd_assign: M out of range [1, max_seeds]"; return APD_E_ARG; }
   if (!X || !A || !w || !vol || !dual) { ctx->err = "apd_assign: X, A, w, vol and dual are required"; return APD_E_ARG; }
   GridDev g;
-  e = make_grid(ctx, grid, kernel, opts && opts->cull, &g);
+  e = make_grid(ctx, grid, kernel, cull, &g);
   if (!e.empty()) { ctx->err = "apd_assign: " + e; return APD_E_ARG; }
   APD_CUDA_TRY(ctx, cudaSetDevice(ctx->ws.device));
   return enqueue_evaluation(ctx, g, kernel, M, X, A, w, target_vol, labels, vol, dual, max_rel_err, centroids,
-                            pairs_evaluated, true, opts && opts->cull, nullptr, static_cast<cudaStream_t>(cuda_stream));
+                            pairs_evaluated, true, cull, nullptr, static_cast<cudaStream_t>(cuda_stream));
 }
 
 extern "C" double apd_last_kernel_ms(apd_ctx* ctx) {

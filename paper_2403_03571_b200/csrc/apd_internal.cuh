@@ -53,10 +53,11 @@ struct AssignArgs {
   const int* super_count;  // [n_super]
   int super_x, super_y;    // super-tiles per axis (x, y); super-tile of CTA tile (bx,by,bz) = (bx/SUPER_TX, ...)
   unsigned long long* pairs_ctr;  // [1] voxel-seed pairs evaluated
-  // in-row offsets tau_k = fl32(k s_x), k < 32: the same for every row of every tile, so they are kernel
-  // PARAMETERS -- the compiler keeps them in uniform registers / the constant bank and the FFMA2s read them from
-  // there, which frees one vector register per voxel of the row.  (The row's voxel k is evaluated at x_row0 + tau_k:
-  // within one ulp of its fp32 centre, and exactly the centre on power-of-two grids.)
+  // in-row offsets from a row's midpoint, tt[j] = fl32((j + 1/2) s_x), and their squares tt[16 + j] = fl32(tau_j^2),
+  // j < 16: the same for every row of every tile, so they are kernel PARAMETERS -- the compiler keeps them in
+  // uniform registers / the constant bank and the FFMA2s read them from there, which frees the vector registers.
+  // (Voxel V/2 + j of a row is evaluated at x_mid + tau_j, V/2 - 1 - j at x_mid - tau_j: within one ulp of its fp32
+  // centre, and exactly the centre on power-of-two grids.)
   float tt[32];
   const int* done_flag;  // solve loop only: kernels return at once when *done_flag != 0; else nullptr
 };
@@ -162,7 +163,7 @@ struct SolveReport {
 
 // host helpers shared by apd_api.cu and apd_lbfgs.cu
 std::string make_grid(const apd_ctx* ctx, const apd_grid* grid, int kernel, bool cull, GridDev* g);
-int resolve_kernel(const apd_opts* o, std::string* err);
+int resolve_kernel(const apd_opts* o, const apd_grid* grid, bool* cull, std::string* err);
 int enqueue_evaluation(apd_ctx* ctx, const GridDev& g, int kernel, int M, const float* X, const float* A,
                        const float* w, const float* target_vol, int32_t* labels, double* vol, double* dual,
                        double* max_rel_err, double* centroids, uint64_t* pairs, bool timed, bool cull,

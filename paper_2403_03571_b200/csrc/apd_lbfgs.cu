@@ -619,13 +619,15 @@ extern "C" int apd_solve(apd_ctx* ctx, const apd_grid* grid, int32_t M, const fl
   if (!ctx) return APD_E_ARG;
   ctx->err.clear();
   std::string e;
-  const int kernel = resolve_kernel(opts, &e);
+  bool cull = false;
+  const int kernel = resolve_kernel(opts, grid, &cull, &e);
   if (kernel < 0) { ctx->err = "apd_solve: " + e; return APD_E_ARG; }
   if (M < 1 || M > ctx->ws.max_seeds) { ctx->err = "apd_solve: M out of range [1, max_seeds]"; return APD_E_ARG; }
   if (!X || !A || !target_vol || !w) { ctx->err = "apd_solve: X, A, target_vol and w are required"; return APD_E_ARG; }
   apd_opts o;
   int rc = check_solve_opts(ctx, "apd_solve", opts, tol, &o);
   if (rc != APD_OK) return rc;
+  o.cull = cull ? 1 : 0;
   GridDev g;
   e = make_grid(ctx, grid, kernel, o.cull != 0, &g);
   if (!e.empty()) { ctx->err = "apd_solve: " + e; return APD_E_ARG; }

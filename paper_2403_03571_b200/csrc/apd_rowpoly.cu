@@ -3,10 +3,12 @@
 // Same definition as the DIRECT kernel -- C_ij = |y_j - x_i|^2_{A_i} - w_i (eq. 2.1),
 // H_j = argmin_i C_ij with the lowest index among equal fp32 costs (reading S1) --
 // re-associated for the machine:
-//   * a thread owns a ROW of V voxels contiguous in x.  With d0 = x_row0 - x_i and tau_k = k s_x the
-//     cost along the row is the quadratic  c(tau) = a11 tau^2 + B' tau + R',
-//        B' = 2 a11 d0 + (a12' dy + a13' dz),   R' = cost at the row's first voxel,
-//     so a pair costs 2 FMA (Horner) after a per-(row, seed) set-up of 14 operations;
+//   * a thread owns a ROW of V voxels contiguous in x.  With dc = x_c - x_i, x_c the MIDPOINT of the row, the cost
+//     along the row is the quadratic  c(tau) = a11 tau^2 + B' tau + R',
+//        B' = 2 a11 dc + (a12' dy + a13' dz),   R' = cost at the midpoint,
+//     and the voxels sit at tau = +-tau_j, tau_j = (j + 1/2) s_x, j < V/2.  The even part is shared by the two:
+//        e_j = fma(a11, tau_j^2, R'),   c(+tau_j) = fma(B', tau_j, e_j),   c(-tau_j) = fma(-B', tau_j, e_j),
+//     so a pair costs 1.5 FMA after a per-(row, seed) set-up of 15 operations;
 //   * all arithmetic is packed f32x2 (FFMA2) over PAIRS OF SEEDS (the seed table is stored
 //     pair-interleaved), one 3-input min folds both lanes into the running minimum;
 //   * the inner loop keeps only the minimum.  After every GROUP seeds the minima are compared with
@@ -19,6 +21,11 @@
 #include <math_constants.h>
 
 namespace apd {
+
+#ifndef ROWBATCH
+#define ROWBATCH 8
+#endif
+constexpr int ROW_BATCH = ROWBATCH;                   // voxels of a row whose FMA chains are interleaved
 
 // pair-interleaved seed table: PREC floats per PAIR of seeds
 //   3D (20): X0 X1 Y0 Y1 | Z0 Z1 a11 a11 | a12' a12' a13' a13' | a22 a22 a23' a23' | a33 a33 nw nw
@@ -71,7 +78,7 @@ cudaError_t launch_pack_pairs(int dim, int M, int M_pad, const float* X, const f
 }
 
 // Per-(row, seed pair) coefficients of the row quadratic.
-struct RowCoef { f2 a11, Bp, Rp; };
+struct RowCoef { f2 a11, Bp, nBp, Rp; };      // nBp = -Bp
 
 template <int DIM>
 __device__ __forceinline__ RowCoef row_setup(const float* __restrict__ sp /* one pair record in smem */,
@@ -90,8 +97,8 @@ __device__ __forceinline__ RowCoef row_setup(const float* __restrict__ sp /* one
     f2 R = f2_fma(dy, u, q4.y);                                            // ... - w
     R = f2_fma(dz, f2_mul(q4.x, dz), R);                                   // + a33 dz^2
     o.a11 = a11;
-    o.Bp = f2_fma(f2_add(a11, a11), d0, E);                                // 2 a11 d0 + E
-    o.Rp = f2_fma(d0, f2_fma(a11, d0, E), R);                              // cost at the row's first voxel
+    o.Bp = f2_fma(f2_add(a11, a11), d0, E);                                // 2 a11 dc + E
+    o.Rp = f2_fma(d0, f2_fma(a11, d0, E), R);                              // cost at the row's midpoint
   } else {
     const ulonglong2 q0 = *reinterpret_cast<const ulonglong2*>(sp);        // X, Y
     const ulonglong2 q1 = *reinterpret_cast<const ulonglong2*>(sp + 4);    // a11, a12'
@@ -104,11 +111,44 @@ __device__ __forceinline__ RowCoef row_setup(const float* __restrict__ sp /* one
     o.Bp = f2_fma(f2_add(a11, a11), d0, E);
     o.Rp = f2_fma(d0, f2_fma(a11, d0, E), R);
   }
+  o.nBp = o.Bp ^ 0x8000000080000000ull;                                    // both sign bits (integer pipe)
   return o;
 }
 
-__device__ __forceinline__ f2 row_cost(const RowCoef& c, f2 tt) {
-  return f2_fma(tt, f2_fma(c.a11, tt, c.Bp), c.Rp);
+// In-row offsets of a thread: tt[j] = tau_j, tsq[j] = fl32(tau_j^2), j < V/2 (kernel parameters: uniform registers).
+// Voxel V/2 + j of the row sits at +tau_j, voxel V/2 - 1 - j at -tau_j.
+template <int V>
+struct RowTau { f2 tt[V / 2], tsq[V / 2]; };
+
+// cost of voxel k of the row, for both seeds of the pair -- the same instructions as the main loop
+template <int V>
+__device__ __forceinline__ f2 row_cost(const RowCoef& c, const RowTau<V>& t, int k) {
+  const int j = (k >= V / 2) ? k - V / 2 : V / 2 - 1 - k;
+  return f2_fma((k >= V / 2) ? c.Bp : c.nBp, t.tt[j], f2_fma(c.a11, t.tsq[j], c.Rp));
+}
+
+// The main loop of one (row, seed pair): 3 FFMA2 + 2 three-input minima per 2 voxels x 2 seeds.  F(k, lo, hi) takes
+// the two costs of voxel k.
+template <int V, class F>
+__device__ __forceinline__ void row_sweep(const RowCoef& rc, const RowTau<V>& t, F&& f) {
+  constexpr int HB = ROW_BATCH / 2;
+  static_assert((V / 2) % HB == 0, "batch");
+#pragma unroll
+  for (int j0 = 0; j0 < V / 2; j0 += HB) {
+    f2 e[HB], cp[HB], cm[HB];
+#pragma unroll
+    for (int j = 0; j < HB; ++j) e[j] = f2_fma(rc.a11, t.tsq[j0 + j], rc.Rp);
+#pragma unroll
+    for (int j = 0; j < HB; ++j) { cp[j] = f2_fma(rc.Bp, t.tt[j0 + j], e[j]); cm[j] = f2_fma(rc.nBp, t.tt[j0 + j], e[j]); }
+#pragma unroll
+    for (int j = 0; j < HB; ++j) {
+      float lo, hi;
+      f2_unpack(cp[j], lo, hi);
+      f(V / 2 + j0 + j, lo, hi);
+      f2_unpack(cm[j], lo, hi);
+      f(V / 2 - 1 - (j0 + j), lo, hi);
+    }
+  }
 }
 
 // Tile geometry: THREADS = TXT*TYT*TZT threads, each owns a row of V voxels contiguous in x, so the tile is
@@ -122,9 +162,6 @@ struct RowGeom {
 };
 #ifndef ROWMINB
 #define ROWMINB 4
-#endif
-#ifndef ROWBATCH
-#define ROWBATCH 8
 #endif
 #ifndef ROWUNROLL
 #define ROWUNROLL 1
@@ -142,7 +179,6 @@ constexpr int ROW_LONG_MIN_WAVES = 2;
 #define ROWSTAGES 4
 #endif
 constexpr int ROW_STAGES = ROWSTAGES;                 // smem ring of seed chunks
-constexpr int ROW_BATCH = ROWBATCH;
 constexpr int ROW_UNROLL = ROWUNROLL;
 
 // Dynamic shared memory of one CTA:
@@ -167,7 +203,7 @@ struct RowSmem {
 // thread's row: rows a3 + a4 of the brute-force kernel.
 template <int DIM, int V, int T, int ROW_GROUP>
 __device__ __forceinline__ void row_process_chunk(const float* __restrict__ sp, int ibase, f2 x0, f2 yy, f2 yz,
-                                                  const f2 (&tt)[V], float (&best)[V], float4* __restrict__ s_prev4,
+                                                  const RowTau<V>& tt, float (&best)[V], float4* __restrict__ s_prev4,
                                                   int* __restrict__ s_lab, int tid) {
   constexpr int PREC = (DIM == 3) ? PREC3 : PREC2;
   constexpr int GROUP_PAIRS = ROW_GROUP / 2;
@@ -176,20 +212,7 @@ __device__ __forceinline__ void row_process_chunk(const float* __restrict__ sp, 
 #pragma unroll ROW_UNROLL
     for (int p = 0; p < GROUP_PAIRS; ++p) {
       const RowCoef rc = row_setup<DIM>(gp + p * PREC, x0, yy, yz);
-#pragma unroll
-      for (int k0 = 0; k0 < V; k0 += ROW_BATCH) {
-        f2 u[ROW_BATCH];
-#pragma unroll
-        for (int j = 0; j < ROW_BATCH; ++j) u[j] = f2_fma(rc.a11, tt[k0 + j], rc.Bp);
-#pragma unroll
-        for (int j = 0; j < ROW_BATCH; ++j) u[j] = f2_fma(tt[k0 + j], u[j], rc.Rp);
-#pragma unroll
-        for (int j = 0; j < ROW_BATCH; ++j) {
-          float lo, hi;
-          f2_unpack(u[j], lo, hi);
-          best[k0 + j] = min3f(best[k0 + j], lo, hi);
-        }
-      }
+      row_sweep<V>(rc, tt, [&](int k, float lo, float hi) { best[k] = min3f(best[k], lo, hi); });
     }
     asm volatile("" ::: "memory");   // keep the prev[] loads below the group loop (they would cost V registers)
     // fast path: did ANY of the row's minima drop in this group?  (V/4 LDS.128 + V compares)
@@ -225,7 +248,7 @@ __device__ __forceinline__ void row_process_chunk(const float* __restrict__ sp, 
             for (int k = k8; k < k8 + 8; ++k) {
               if (mask & (1u << k)) {
                 float lo, hi;
-                f2_unpack(row_cost(rc, tt[k]), lo, hi);
+                f2_unpack(row_cost<V>(rc, tt, k), lo, hi);
                 if (lo == best[k]) { s_lab[k * T + tid] = i0; mask &= ~(1u << k); }
                 else if (hi == best[k]) { s_lab[k * T + tid] = i0 + 1; mask &= ~(1u << k); }
               }
@@ -251,14 +274,17 @@ struct RowThread {
   __device__ __forceinline__ void init_at(const AssignArgs& a, int bx, int by, int bz, int tx, int ty, int tz) {
     ix0 = (bx * G::TXT + tx) * G::V; iy = by * G::TYT + ty; iz = bz * G::TZT + tz;
     row_valid = (ix0 < a.g.nx) && (iy < a.g.ny) && (iz < a.g.nz);
-    // coordinates from the thread index (fp64 definition rounded once to fp32)
-    const float x0f = (float)(a.g.lo[0] + ((double)ix0 + 0.5) * a.g.s[0]);
+    // coordinates from the thread index (fp64 definition rounded once to fp32); x0 = the row's midpoint
+    const float x0f = (float)(a.g.lo[0] + ((double)ix0 + 0.5 * (double)G::V) * a.g.s[0]);
     const float yyf = (float)(a.g.lo[1] + ((double)iy + 0.5) * a.g.s[1]);
     const float yzf = (DIM == 3) ? (float)(a.g.lo[2] + ((double)iz + 0.5) * a.g.s[2]) : 0.0f;
     x0 = f2_pack(x0f, x0f); yy = f2_pack(yyf, yyf); yz = f2_pack(yzf, yzf);
   }
-  // in-row offset of voxel k from the row's first voxel (a kernel parameter: uniform)
-  __device__ __forceinline__ f2 tau(const AssignArgs& a, int k) const { return f2_pack(a.tt[k], a.tt[k]); }
+  // in-row offsets from the midpoint (kernel parameters: uniform)
+  __device__ __forceinline__ void tau(const AssignArgs& a, RowTau<G::V>& t) const {
+#pragma unroll
+    for (int j = 0; j < G::V / 2; ++j) { t.tt[j] = f2_pack(a.tt[j], a.tt[j]); t.tsq[j] = f2_pack(a.tt[16 + j], a.tt[16 + j]); }
+  }
 };
 
 template <int DIM, class G>
@@ -268,7 +294,7 @@ __global__ void __launch_bounds__(G::THREADS, G::MINB) assign_rowpoly_kernel(con
   constexpr int PREC = S::PREC;
   constexpr int CHUNK_PAIRS = S::CHUNK_PAIRS;
   constexpr uint32_t CHUNK_BYTES = CHUNK_PAIRS * PREC * sizeof(float);
-  static_assert(V <= 32 && V % ROW_BATCH == 0 && V % 4 == 0, "row mask is 32 bits");
+  static_assert(V <= 32 && V % 4 == 0, "row mask is 32 bits; a.tt holds 16 + 16 offsets");
   extern __shared__ __align__(128) unsigned char smem_raw[];
   float* s_seeds = reinterpret_cast<float*>(smem_raw);
   float4* s_prev4 = reinterpret_cast<float4*>(smem_raw + S::PREV_OFF);   // [V/4][T]
@@ -294,11 +320,11 @@ __global__ void __launch_bounds__(G::THREADS, G::MINB) assign_rowpoly_kernel(con
     }
   }
 
-  f2 tt[V];
+  RowTau<V> tt;
+  rt.tau(a, tt);
   float best[V];
 #pragma unroll
   for (int k = 0; k < V; ++k) {
-    tt[k] = rt.tau(a, k);
     best[k] = CUDART_INF_F;
     s_lab[k * T + tid] = 0;
   }
@@ -410,11 +436,12 @@ __global__ void __launch_bounds__(128, 4) assign_rowpoly_culled_kernel(const Ass
   };
   if (nchunks > 0) gather(0);        // issued first: its latency overlaps the row set-up below
 
-  f2 tt[V];
+  RowTau<V> tt;
+  rt.tau(a, tt);
   float best[V];
   int lab[V];
 #pragma unroll
-  for (int k = 0; k < V; ++k) { tt[k] = rt.tau(a, k); best[k] = CUDART_INF_F; lab[k] = 0; }
+  for (int k = 0; k < V; ++k) { best[k] = CUDART_INF_F; lab[k] = 0; }
   __syncwarp();
 
   for (int c = 0; c < nchunks; ++c) {
@@ -425,22 +452,11 @@ __global__ void __launch_bounds__(128, 4) assign_rowpoly_culled_kernel(const Ass
     for (int p = 0; p < npairs; ++p) {
       const RowCoef rc = row_setup<DIM>(sp + p * PREC, rt.x0, rt.yy, rt.yz);
       const int i0 = ip[2 * p], i1 = ip[2 * p + 1];
-#pragma unroll
-      for (int k0 = 0; k0 < V; k0 += ROW_BATCH) {
-        f2 u[ROW_BATCH];
-#pragma unroll
-        for (int j = 0; j < ROW_BATCH; ++j) u[j] = f2_fma(rc.a11, tt[k0 + j], rc.Bp);
-#pragma unroll
-        for (int j = 0; j < ROW_BATCH; ++j) u[j] = f2_fma(tt[k0 + j], u[j], rc.Rp);
-#pragma unroll
-        for (int j = 0; j < ROW_BATCH; ++j) {
-          float lo, hi;
-          f2_unpack(u[j], lo, hi);
-          const float m = min3f(best[k0 + j], lo, hi);
-          if (m < best[k0 + j]) lab[k0 + j] = (lo == m) ? i0 : i1;    // lo == hi == m: the lower index
-          best[k0 + j] = m;
-        }
-      }
+      row_sweep<V>(rc, tt, [&](int k, float lo, float hi) {
+        const float m = min3f(best[k], lo, hi);
+        if (m < best[k]) lab[k] = (lo == m) ? i0 : i1;    // lo == hi == m: the lower index
+        best[k] = m;
+      });
     }
     __syncwarp();
   }
