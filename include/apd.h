@@ -48,15 +48,16 @@ typedef struct {
 /* Which implementation of the voxel x seed reduction runs (all give labels by the same rule:
  * fp32 cost, lowest seed index among equal fp32 costs). */
 enum {
-  APD_KERNEL_AUTO   = 0,   /* the fastest one: APD_KERNEL_ROWPOLY, except on grids narrower than 8
-                              voxels in x, which take APD_KERNEL_DIRECT (and ignore opts.cull): the
-                              row kernels expand the cost about the midpoint of a 16- or 32-voxel
-                              row, which there lies several domain widths outside the domain and
-                              costs up to (1 + 8/n[0])^2 in relative precision                     */
+  APD_KERNEL_AUTO   = 0,   /* the fastest one: APD_KERNEL_ROWPOLY, except on grids with n[0] < 8 (3D
+                              also n[1] < 8 or n[2] < 4), which take APD_KERNEL_DIRECT (and ignore
+                              opts.cull): the row kernels expand the cost about the midpoint of a
+                              row / tile, which there lies several domain widths outside the domain
+                              and costs up to (1 + 8/n)^2 in relative precision                    */
   APD_KERNEL_DIRECT = 1,   /* un-hoisted direct form: 12 (3D) / 7 (2D) FP32 instr. per pair;
                               the reference kernel the FP32-pipe fraction is quoted on             */
-  APD_KERNEL_ROWPOLY = 2   /* row-hoisted quadratic in the offset from the row's midpoint (1.5 FMA per
-                              pair), packed f32x2, deferred argmin                                 */
+  APD_KERNEL_ROWPOLY = 2   /* quadratic in the offset from the row's midpoint (1.5 FMA per pair) with
+                              coefficients polynomial in the row's offset from the tile's midpoint,
+                              packed f32x2, deferred argmin                                        */
 };
 
 /* opts.cull = 1: exact culling (not in the paper).  Per block of voxels the library keeps only

@@ -120,10 +120,15 @@ std::string make_grid(const apd_ctx* ctx, const apd_grid* grid, int kernel, bool
   return "";
 }
 
-// opts -> kernel (AUTO resolved) and whether culling runs.  AUTO on a grid narrower than ROW_MIN_NX voxels in x
-// takes DIRECT and drops opts.cull: the row kernels expand the cost about a row's midpoint, which on such a grid lies
-// several domain widths outside it, and the cancellation costs (1 + 8/nx)^2 in relative precision.
-constexpr int ROW_MIN_NX = 8;
+// opts -> kernel (AUTO resolved) and whether culling runs.  AUTO on a grid with fewer voxels along an axis than
+// half a tile of the row kernels (x: 8, y: 8 in 3D, z: 4) takes DIRECT and drops opts.cull: those kernels expand the
+// cost about a row's midpoint in x and (3D) the tile's midpoint in y and z, which on such a grid lie several domain
+// widths outside it, and the cancellation costs up to (1 + 8/n)^2 in relative precision.
+static bool narrow_grid(const apd_grid* grid) {
+  if (!grid) return false;
+  if (grid->n[0] < 8) return true;
+  return grid->dim == 3 && (grid->n[1] < 8 || grid->n[2] < 4);
+}
 int resolve_kernel(const apd_opts* o, const apd_grid* grid, bool* cull, std::string* err) {
   int k = o ? o->kernel : APD_KERNEL_AUTO;
   if (k != APD_KERNEL_AUTO && k != APD_KERNEL_DIRECT && k != APD_KERNEL_ROWPOLY) { *err = "unknown opts.kernel"; return -1; }
@@ -131,7 +136,7 @@ int resolve_kernel(const apd_opts* o, const apd_grid* grid, bool* cull, std::str
   if (o && (o->reserved[0] || o->reserved[1] || o->reserved[2])) { *err = "opts.reserved must be 0"; return -1; }
   *cull = o && o->cull;
   if (k == APD_KERNEL_AUTO) {
-    if (grid && grid->n[0] < ROW_MIN_NX) { *cull = false; return APD_KERNEL_DIRECT; }
+    if (narrow_grid(grid)) { *cull = false; return APD_KERNEL_DIRECT; }
     k = APD_KERNEL_ROWPOLY;
   }
   if (*cull && k != APD_KERNEL_ROWPOLY) { *err = "opts.cull needs kernel AUTO or ROWPOLY"; return -1; }

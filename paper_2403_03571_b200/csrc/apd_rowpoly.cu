@@ -80,36 +80,65 @@ cudaError_t launch_pack_pairs(int dim, int M, int M_pad, const float* X, const f
 // Per-(row, seed pair) coefficients of the row quadratic.
 struct RowCoef { f2 a11, Bp, nBp, Rp; };      // nBp = -Bp
 
+// 3D: B' and R' are themselves polynomials in the row's offset (Y, Z) from the TILE's reference point
+// (x_c, y_0, z_0) = (row midpoint in x, tile midpoint in y and z):
+//      B' = b0 + a12' Y + a13' Z,      R' = r0 + r1 Y + r2 Z + a22 Y^2 + a23' Y Z + a33 Z^2,
+// with d = (x_c, y_0, z_0) - x_i:  b0 = 2 a11 dx + a12' dy + a13' dz (the x-derivative of the cost at the reference
+// point), r1 = a12' dx + 2 a22 dy + a23' dz, r2 = a13' dx + a23' dy + 2 a33 dz (its y- and z-derivatives) and
+// r0 = the cost there.  cook3() turns a seed's (x, y, z, -w) into (b0, r1, r2, r0) ONCE per (tile, seed) -- in the
+// brute-force kernel thread t of the CTA does it in place for seed t of every staged chunk, in the culled kernel
+// the lane that gathers a candidate -- and the per-(row, seed) set-up shrinks from 14 to 7 FMA.  Both kernels call
+// this one function with explicit roundings, so their costs agree bit for bit.
+struct Cooked3 { float b0, r1, r2, r0; };
+__device__ __forceinline__ Cooked3 cook3(float X, float Y, float Z, float a11, float a12, float a13, float a22,
+                                         float a23, float a33, float nw, float xc, float y0, float z0) {
+  const float dx = __fsub_rn(xc, X), dy = __fsub_rn(y0, Y), dz = __fsub_rn(z0, Z);
+  const float E0 = fmaf(a12, dy, __fmul_rn(a13, dz));                      // a12' dy + a13' dz
+  const float u0 = fmaf(a23, dz, __fmul_rn(a22, dy));                      // a22 dy + a23' dz
+  float R0 = fmaf(dy, u0, nw);                                             // ... - w
+  R0 = fmaf(dz, __fmul_rn(a33, dz), R0);                                   // + a33 dz^2
+  Cooked3 o;
+  o.b0 = fmaf(__fadd_rn(a11, a11), dx, E0);
+  o.r0 = fmaf(dx, fmaf(a11, dx, E0), R0);
+  o.r1 = fmaf(a12, dx, fmaf(__fadd_rn(a22, a22), dy, __fmul_rn(a23, dz)));
+  o.r2 = fmaf(a13, dx, fmaf(a23, dy, __fmul_rn(__fadd_rn(a33, a33), dz)));
+  return o;
+}
+
+// Per-thread constants of the set-up.  2D: the row's midpoint x and its y.  3D: the row's offset (Y, Z) from the
+// tile's reference point and its monomials.
+template <int DIM> struct RowRef;
+template <> struct RowRef<2> { f2 x0, yy; };
+template <> struct RowRef<3> { f2 Y, Z, YY, YZ, ZZ; };
+
+// sp = one pair record in smem; 3D: cooked, i.e. the slots of (X, Y, Z, nw) hold (b0, r1, r2, r0)
 template <int DIM>
-__device__ __forceinline__ RowCoef row_setup(const float* __restrict__ sp /* one pair record in smem */,
-                                             f2 x0, f2 yy, f2 yz) {
+__device__ __forceinline__ RowCoef row_setup(const float* __restrict__ sp, const RowRef<DIM>& rr) {
   RowCoef o;
-  if (DIM == 3) {
-    const ulonglong2 q0 = *reinterpret_cast<const ulonglong2*>(sp);        // X, Y
-    const ulonglong2 q1 = *reinterpret_cast<const ulonglong2*>(sp + 4);    // Z, a11
+  if constexpr (DIM == 3) {
+    const ulonglong2 q0 = *reinterpret_cast<const ulonglong2*>(sp);        // b0, r1
+    const ulonglong2 q1 = *reinterpret_cast<const ulonglong2*>(sp + 4);    // r2, a11
     const ulonglong2 q2 = *reinterpret_cast<const ulonglong2*>(sp + 8);    // a12', a13'
     const ulonglong2 q3 = *reinterpret_cast<const ulonglong2*>(sp + 12);   // a22, a23'
-    const ulonglong2 q4 = *reinterpret_cast<const ulonglong2*>(sp + 16);   // a33, nw
-    const f2 d0 = f2_sub(x0, q0.x), dy = f2_sub(yy, q0.y), dz = f2_sub(yz, q1.x);
-    const f2 a11 = q1.y;
-    const f2 E = f2_fma(q2.x, dy, f2_mul(q2.y, dz));                       // a12' dy + a13' dz
-    const f2 u = f2_fma(q3.y, dz, f2_mul(q3.x, dy));                       // a22 dy + a23' dz
-    f2 R = f2_fma(dy, u, q4.y);                                            // ... - w
-    R = f2_fma(dz, f2_mul(q4.x, dz), R);                                   // + a33 dz^2
-    o.a11 = a11;
-    o.Bp = f2_fma(f2_add(a11, a11), d0, E);                                // 2 a11 dc + E
-    o.Rp = f2_fma(d0, f2_fma(a11, d0, E), R);                              // cost at the row's midpoint
+    const ulonglong2 q4 = *reinterpret_cast<const ulonglong2*>(sp + 16);   // a33, r0
+    o.a11 = q1.y;
+    o.Bp = f2_fma(q2.y, rr.Z, f2_fma(q2.x, rr.Y, q0.x));
+    f2 R = f2_fma(q0.y, rr.Y, q4.y);
+    R = f2_fma(q1.x, rr.Z, R);
+    R = f2_fma(q3.x, rr.YY, R);
+    R = f2_fma(q3.y, rr.YZ, R);
+    o.Rp = f2_fma(q4.x, rr.ZZ, R);
   } else {
     const ulonglong2 q0 = *reinterpret_cast<const ulonglong2*>(sp);        // X, Y
     const ulonglong2 q1 = *reinterpret_cast<const ulonglong2*>(sp + 4);    // a11, a12'
     const ulonglong2 q2 = *reinterpret_cast<const ulonglong2*>(sp + 8);    // a22, nw
-    const f2 d0 = f2_sub(x0, q0.x), dy = f2_sub(yy, q0.y);
+    const f2 d0 = f2_sub(rr.x0, q0.x), dy = f2_sub(rr.yy, q0.y);
     const f2 a11 = q1.x;
     const f2 E = f2_mul(q1.y, dy);                                         // a12' dy
     const f2 R = f2_fma(dy, f2_mul(q2.x, dy), q2.y);                       // a22 dy^2 - w
     o.a11 = a11;
-    o.Bp = f2_fma(f2_add(a11, a11), d0, E);
-    o.Rp = f2_fma(d0, f2_fma(a11, d0, E), R);
+    o.Bp = f2_fma(f2_add(a11, a11), d0, E);                                // 2 a11 dc + E
+    o.Rp = f2_fma(d0, f2_fma(a11, d0, E), R);                              // cost at the row's midpoint
   }
   o.nBp = o.Bp ^ 0x8000000080000000ull;                                    // both sign bits (integer pipe)
   return o;
@@ -161,7 +190,7 @@ struct RowGeom {
                        GROUP = GROUP_;
 };
 #ifndef ROWMINB
-#define ROWMINB 4
+#define ROWMINB 3
 #endif
 #ifndef ROWUNROLL
 #define ROWUNROLL 1
@@ -169,7 +198,10 @@ struct RowGeom {
 // Two row lengths are built.  LONG rows (V = 32) amortise the per-(row, seed) set-up best and are used once the
 // grid gives every SM at least ROW_LONG_MIN_WAVES waves of long-row tiles; smaller grids take SHORT rows (V = 16),
 // whose tiles are half as big, so that all SMs have work.
-using RowGeom3L = RowGeom<3, 32, 1, 16, 8, ROWMINB, 16>;    // tile 32 x 16 x 8 voxels, 128 threads
+#ifndef ROWGROUPL
+#define ROWGROUPL 16
+#endif
+using RowGeom3L = RowGeom<3, 32, 1, 16, 8, ROWMINB, ROWGROUPL>;    // tile 32 x 16 x 8 voxels, 128 threads
 using RowGeom3S = RowGeom<3, 16, 1, 16, 8, ROWMINB, 8>;    // tile 16 x 16 x 8 voxels
 using RowGeom2L = RowGeom<2, 32, 2, 64, 1, ROWMINB, 16>;    // tile 64 x 64 pixels
 using RowGeom2S = RowGeom<2, 16, 2, 64, 1, ROWMINB, 8>;    // tile 32 x 64 pixels
@@ -202,7 +234,7 @@ struct RowSmem {
 // One staged chunk of SEED_CHUNK seeds ibase .. ibase+SEED_CHUNK-1 (pair-interleaved records at `sp`) against the
 // thread's row: rows a3 + a4 of the brute-force kernel.
 template <int DIM, int V, int T, int ROW_GROUP>
-__device__ __forceinline__ void row_process_chunk(const float* __restrict__ sp, int ibase, f2 x0, f2 yy, f2 yz,
+__device__ __forceinline__ void row_process_chunk(const float* __restrict__ sp, int ibase, const RowRef<DIM>& rr,
                                                   const RowTau<V>& tt, float (&best)[V], float4* __restrict__ s_prev4,
                                                   int* __restrict__ s_lab, int tid) {
   constexpr int PREC = (DIM == 3) ? PREC3 : PREC2;
@@ -211,7 +243,7 @@ __device__ __forceinline__ void row_process_chunk(const float* __restrict__ sp, 
     const float* gp = sp + gidx * GROUP_PAIRS * PREC;
 #pragma unroll ROW_UNROLL
     for (int p = 0; p < GROUP_PAIRS; ++p) {
-      const RowCoef rc = row_setup<DIM>(gp + p * PREC, x0, yy, yz);
+      const RowCoef rc = row_setup<DIM>(gp + p * PREC, rr);
       row_sweep<V>(rc, tt, [&](int k, float lo, float hi) { best[k] = min3f(best[k], lo, hi); });
     }
     asm volatile("" ::: "memory");   // keep the prev[] loads below the group loop (they would cost V registers)
@@ -237,7 +269,7 @@ __device__ __forceinline__ void row_process_chunk(const float* __restrict__ sp, 
         s_prev4[k4 * T + tid] = pv;
       }
       for (int p = 0; p < GROUP_PAIRS && mask; ++p) {
-        const RowCoef rc = row_setup<DIM>(gp + p * PREC, x0, yy, yz);
+        const RowCoef rc = row_setup<DIM>(gp + p * PREC, rr);
         const int i0 = ibase + gidx * ROW_GROUP + 2 * p;
         // a new seed takes over an interval of the row, and neighbouring rows (the other lanes) similar ones: test
         // the row in blocks of 8 voxels so that the untouched blocks cost one branch
@@ -265,7 +297,8 @@ template <int DIM, class G>
 struct RowThread {
   int ix0, iy, iz;
   bool row_valid;
-  f2 x0, yy, yz;
+  RowRef<DIM> rr;
+  float xc, y0, z0;        // 3D: the tile's reference point (cook3)
   __device__ __forceinline__ void init(const AssignArgs& a, int b, int tid) {
     const int tx = tid % G::TXT, ty = (tid / G::TXT) % G::TYT, tz = tid / (G::TXT * G::TYT);
     const int bx = b % a.g.tiles_x, by = (b / a.g.tiles_x) % a.g.tiles_y, bz = b / (a.g.tiles_x * a.g.tiles_y);
@@ -274,11 +307,22 @@ struct RowThread {
   __device__ __forceinline__ void init_at(const AssignArgs& a, int bx, int by, int bz, int tx, int ty, int tz) {
     ix0 = (bx * G::TXT + tx) * G::V; iy = by * G::TYT + ty; iz = bz * G::TZT + tz;
     row_valid = (ix0 < a.g.nx) && (iy < a.g.ny) && (iz < a.g.nz);
-    // coordinates from the thread index (fp64 definition rounded once to fp32); x0 = the row's midpoint
-    const float x0f = (float)(a.g.lo[0] + ((double)ix0 + 0.5 * (double)G::V) * a.g.s[0]);
-    const float yyf = (float)(a.g.lo[1] + ((double)iy + 0.5) * a.g.s[1]);
-    const float yzf = (DIM == 3) ? (float)(a.g.lo[2] + ((double)iz + 0.5) * a.g.s[2]) : 0.0f;
-    x0 = f2_pack(x0f, x0f); yy = f2_pack(yyf, yyf); yz = f2_pack(yzf, yzf);
+    // coordinates from the indices (fp64 definitions rounded once to fp32); in x the row's midpoint
+    xc = (float)(a.g.lo[0] + ((double)ix0 + 0.5 * (double)G::V) * a.g.s[0]);
+    if constexpr (DIM == 3) {
+      static_assert(G::TXT == 1, "3D: one reference point per tile");
+      y0 = (float)(a.g.lo[1] + ((double)(by * G::TYT) + 0.5 * (double)G::TYT) * a.g.s[1]);
+      z0 = (float)(a.g.lo[2] + ((double)(bz * G::TZT) + 0.5 * (double)G::TZT) * a.g.s[2]);
+      const float Yf = (float)(((double)ty + 0.5 - 0.5 * (double)G::TYT) * a.g.s[1]);
+      const float Zf = (float)(((double)tz + 0.5 - 0.5 * (double)G::TZT) * a.g.s[2]);
+      const float YY = __fmul_rn(Yf, Yf), YZ = __fmul_rn(Yf, Zf), ZZ = __fmul_rn(Zf, Zf);
+      rr.Y = f2_pack(Yf, Yf); rr.Z = f2_pack(Zf, Zf);
+      rr.YY = f2_pack(YY, YY); rr.YZ = f2_pack(YZ, YZ); rr.ZZ = f2_pack(ZZ, ZZ);
+    } else {
+      y0 = 0.0f; z0 = 0.0f;
+      const float yyf = (float)(a.g.lo[1] + ((double)iy + 0.5) * a.g.s[1]);
+      rr.x0 = f2_pack(xc, xc); rr.yy = f2_pack(yyf, yyf);
+    }
   }
   // in-row offsets from the midpoint (kernel parameters: uniform)
   __device__ __forceinline__ void tau(const AssignArgs& a, RowTau<G::V>& t) const {
@@ -344,8 +388,18 @@ __global__ void __launch_bounds__(G::THREADS, G::MINB) assign_rowpoly_kernel(con
                    a.seeds + (size_t)(c + ROW_STAGES - 1) * CHUNK_PAIRS * PREC, CHUNK_BYTES, &s_full[s2]);
     }
     mbar_wait(&s_full[stage], (uint32_t)((c / ROW_STAGES) & 1));
-    row_process_chunk<DIM, V, T, G::GROUP>(s_seeds + (size_t)stage * CHUNK_PAIRS * PREC, c * SEED_CHUNK, rt.x0, rt.yy, rt.yz, tt,
-                                 best, s_prev4, s_lab, tid);
+    float* chunk = s_seeds + (size_t)stage * CHUNK_PAIRS * PREC;
+    if constexpr (DIM == 3) {
+      // re-expand the chunk's seeds about this tile's reference point, in place (cook3): one seed per thread
+      for (int sd = tid; sd < SEED_CHUNK; sd += T) {
+        float* p = chunk + (sd >> 1) * PREC + (sd & 1);
+        const Cooked3 ck = cook3(p[0], p[2], p[4], p[6], p[8], p[10], p[12], p[14], p[16], p[18], rt.xc, rt.y0, rt.z0);
+        p[0] = ck.b0; p[2] = ck.r1; p[4] = ck.r2; p[18] = ck.r0;
+      }
+      fence_proxy_async_smem();      // these generic-proxy writes precede the TMA refill of the stage
+      __syncthreads();
+    }
+    row_process_chunk<DIM, V, T, G::GROUP>(chunk, c * SEED_CHUNK, rt.rr, tt, best, s_prev4, s_lab, tid);
     __syncwarp();
     if ((tid & 31) == 0) mbar_arrive(&s_empty[stage]);
   }
@@ -429,6 +483,10 @@ __global__ void __launch_bounds__(128, 4) assign_rowpoly_culled_kernel(const Ass
       for (int q = 0; q < REC; ++q) r[q] = 0.0f;
       r[NP - 1] = CUDART_INF_F;      // padding candidate: cost +inf, never wins the strict '<'
     }
+    if constexpr (DIM == 3) {        // re-expand about the CTA tile's reference point, as the brute-force kernel does
+      const Cooked3 ck = cook3(r[0], r[1], r[2], r[3], r[4], r[5], r[6], r[7], r[8], r[9], rt.xc, rt.y0, rt.z0);
+      r[0] = ck.b0; r[1] = ck.r1; r[2] = ck.r2; r[9] = ck.r0;
+    }
     float* dst = &s_seeds[w][stage][(lane >> 1) * PREC + (lane & 1)];
 #pragma unroll
     for (int q = 0; q < NP; ++q) dst[2 * q] = r[q];
@@ -450,7 +508,7 @@ __global__ void __launch_bounds__(128, 4) assign_rowpoly_culled_kernel(const Ass
     const int* ip = s_idx[w][c & 1];
     const int npairs = min(WCHUNK / 2, (cnt - c * WCHUNK + 1) / 2);     // pairs that hold a real candidate
     for (int p = 0; p < npairs; ++p) {
-      const RowCoef rc = row_setup<DIM>(sp + p * PREC, rt.x0, rt.yy, rt.yz);
+      const RowCoef rc = row_setup<DIM>(sp + p * PREC, rt.rr);
       const int i0 = ip[2 * p], i1 = ip[2 * p + 1];
       row_sweep<V>(rc, tt, [&](int k, float lo, float hi) {
         const float m = min3f(best[k], lo, hi);
