@@ -182,8 +182,9 @@ def run_reference(args):
 # ------------------------------------------------------------------------------------------------
 # Algorithmic FP32 work per voxel-seed pair of each kernel form:
 #   DIRECT  : 3 FADD + 3 FMUL + 6 FFMA               = 18 flop   (12 FP32 instructions, 3D)
-#   ROWPOLY : 2 FMA (Horner) + 21 flop set-up per (row of 32 voxels, seed) = 4 + 21/32 = 4.65625 flop
-FLOP_PER_PAIR = {1: 18.0, 2: 4.0 + 21.0 / 32.0}
+#   ROWPOLY : 1.5 FMA (voxels at +-tau share the even part) + 7 FMA set-up per (row of 32 voxels, seed)
+#             = 3 + 14/32 = 3.4375 flop (the once-per-(tile, seed) re-expansion, ~25 flop / 4096 voxels, not counted)
+FLOP_PER_PAIR = {1: 18.0, 2: 3.0 + 14.0 / 32.0}
 FP32_LANES_PER_SM = 128
 # dram__bytes_read.sum + dram__bytes_write.sum of one assign_rowpoly_kernel launch on this workload, from the
 # `ncu --set full` capture summarised in profiles/ (None until a capture exists)

@@ -224,7 +224,7 @@ int apd_solve_host(apd_ctx* ctx, const apd_grid* grid, int32_t M,
  * apd_fp32_probe: runs a register-only FP32 microbenchmark on `device` and returns the
  *   achieved rate in *ops_per_s (HOST): variant 0 = scalar FFMA (2 flop each), 1 = packed
  *   fma.rn.f32x2 (4 flop each), 2 = 3-input min.f32, 3 = the ROWPOLY inner-loop mix
- *   (2 f32x2 FMA + 1 three-input min).  *ops_per_s counts FMA lanes (variants 0,1), min
+ *   (3 f32x2 FMA + 2 three-input min per 4 pairs).  *ops_per_s counts FMA lanes (variants 0,1), min
  *   instructions x32 lanes (2) or voxel-seed pairs (3).  Synchronous. */
 double apd_last_kernel_ms(apd_ctx* ctx);
 int    apd_fp32_probe(int32_t device, int32_t variant, double* ops_per_s, double* sm_clock_mhz);

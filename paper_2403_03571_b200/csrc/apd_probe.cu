@@ -54,23 +54,32 @@ __global__ void __launch_bounds__(256) probe_kernel(float* out, const float* in,
 #pragma unroll
     for (int k = 0; k < PROBE_ACC; ++k) res += acc[k];
   } else {
-    // the ROWPOLY inner loop: per voxel k and seed pair: u = fma2(a11, t_k, B); c = fma2(t_k, u, R);
-    // best_k = min3(best_k, c.lo, c.hi)
-    f2 tt[PROBE_ACC];
+    // the ROWPOLY inner loop: per pair of voxels at +-t_j and seed pair: e = fma2(a11, t_j^2, R); c+ = fma2(B, t_j, e);
+    // c- = fma2(-B, t_j, e); best_+ = min3(best_+, c+.lo, c+.hi); best_- likewise: 3 FFMA2 + 2 min3 per 4 pairs
+    f2 tt[PROBE_ACC / 2], tsq[PROBE_ACC / 2];
     float best[PROBE_ACC];
 #pragma unroll
-    for (int k = 0; k < PROBE_ACC; ++k) { tt[k] = f2_pack((float)k * c, (float)k * c); best[k] = 3.0e38f; }
+    for (int k = 0; k < PROBE_ACC; ++k) best[k] = 3.0e38f;
+#pragma unroll
+    for (int j = 0; j < PROBE_ACC / 2; ++j) {
+      const float t = ((float)j + 0.5f) * c;
+      tt[j] = f2_pack(t, t); tsq[j] = f2_pack(t * t, t * t);
+    }
     f2 a11 = f2_pack(b, c), B = f2_pack(c, b), R = f2_pack(b + c, b - c);
     const f2 inc = f2_pack(1e-3f, 2e-3f);
     for (int it = 0; it < PROBE_ITERS; ++it) {
+      const f2 nB = B ^ 0x8000000080000000ull;
 #pragma unroll
-      for (int k = 0; k < PROBE_ACC; ++k) {
-        f2 u, cst;
+      for (int j = 0; j < PROBE_ACC / 2; ++j) {
+        f2 e, cp, cm;
         float lo, hi;
-        asm volatile("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(u) : "l"(a11), "l"(tt[k]), "l"(B));
-        asm volatile("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(cst) : "l"(tt[k]), "l"(u), "l"(R));
-        f2_unpack(cst, lo, hi);
-        asm volatile("min.f32 %0, %0, %1, %2;" : "+f"(best[k]) : "f"(lo), "f"(hi));
+        asm volatile("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(e) : "l"(a11), "l"(tsq[j]), "l"(R));
+        asm volatile("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(cp) : "l"(B), "l"(tt[j]), "l"(e));
+        asm volatile("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(cm) : "l"(nB), "l"(tt[j]), "l"(e));
+        f2_unpack(cp, lo, hi);
+        asm volatile("min.f32 %0, %0, %1, %2;" : "+f"(best[PROBE_ACC / 2 + j]) : "f"(lo), "f"(hi));
+        f2_unpack(cm, lo, hi);
+        asm volatile("min.f32 %0, %0, %1, %2;" : "+f"(best[PROBE_ACC / 2 - 1 - j]) : "f"(lo), "f"(hi));
       }
       B = f2_add(B, inc);
       R = f2_add(R, inc);
