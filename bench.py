@@ -188,7 +188,7 @@ FLOP_PER_PAIR = {1: 18.0, 2: 3.0 + 14.0 / 32.0}
 FP32_LANES_PER_SM = 128
 # dram__bytes_read.sum + dram__bytes_write.sum of one assign_rowpoly_kernel launch on this workload, from the
 # `ncu --set full` capture summarised in profiles/ (None until a capture exists)
-NCU_TRAFFIC_BYTES = 529920 + 14650112      # profiles/r01_assign_rowpoly_full.md (labels mostly still in L2 at kernel end)
+NCU_TRAFFIC_BYTES = 489472 + 15261696      # profiles/r01_assign_rowpoly_full.md (labels mostly still in L2 at kernel end)
 
 
 def run_ours(args):
