@@ -51,8 +51,9 @@ enum {
   APD_KERNEL_AUTO   = 0,   /* the fastest one: APD_KERNEL_ROWPOLY, except on grids with n[0] < 8 (3D
                               also n[1] < 8 or n[2] < 4), which take APD_KERNEL_DIRECT (and ignore
                               opts.cull): the row kernels expand the cost about the midpoint of a
-                              row / tile, which there lies several domain widths outside the domain
-                              and costs up to (1 + 8/n)^2 in relative precision                    */
+                              row / tile, which there lies up to 8/n domain widths L outside the
+                              domain: a cost then carries a few fp32 ulp of a ((1 + 8/n) L)^2
+                              instead of a few ulp of itself                                        */
   APD_KERNEL_DIRECT = 1,   /* un-hoisted direct form: 12 (3D) / 7 (2D) FP32 instr. per pair;
                               the reference kernel the FP32-pipe fraction is quoted on             */
   APD_KERNEL_ROWPOLY = 2   /* quadratic in the offset from the row's midpoint (1.5 FMA per pair) with

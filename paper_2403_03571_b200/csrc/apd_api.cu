@@ -123,7 +123,8 @@ std::string make_grid(const apd_ctx* ctx, const apd_grid* grid, int kernel, bool
 // opts -> kernel (AUTO resolved) and whether culling runs.  AUTO on a grid with fewer voxels along an axis than
 // half a tile of the row kernels (x: 8, y: 8 in 3D, z: 4) takes DIRECT and drops opts.cull: those kernels expand the
 // cost about a row's midpoint in x and (3D) the tile's midpoint in y and z, which on such a grid lie several domain
-// widths outside it, and the cancellation costs up to (1 + 8/n)^2 in relative precision.
+// widths L outside it: a cost then carries a few fp32 ulp of a ((1 + 8/n) L)^2 instead of a few ulp of itself
+// (DESIGN.md 5).
 static bool narrow_grid(const apd_grid* grid) {
   if (!grid) return false;
   if (grid->n[0] < 8) return true;

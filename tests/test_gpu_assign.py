@@ -265,6 +265,26 @@ def test_culling_rejects_direct_kernel(apd):
     assert e.value.status == apd.APD_E_ARG
 
 
+@pytest.mark.parametrize("dim,n", [(2, (5, 200)), (3, (64, 6, 64)), (3, (64, 64, 3)), (3, (3, 40, 40))])
+def test_narrow_grids_take_the_direct_kernel(apd, dim, n):
+    """AUTO on a grid narrower than half a tile of the row kernels (include/apd.h) runs DIRECT and ignores opts.cull:
+    bit-identical outputs, N*M pairs.  An explicit ROWPOLY is honoured and stays inside the parity rule with the dual
+    bound of the expansion about a midpoint up to 8/n domain widths L outside the domain: a few fp32 ulp of
+    a ((1 + 8/n) L)^2 per cost, i.e. ((1 + 8/n) L / l)^2 ulp relative to costs of the size a l^2 (l = grain size)."""
+    wl = workloads.make_random(dim, n, 60, 4242, w_scale=0.1)
+    rd = run_assign(apd, wl, wl.w0, v=wl.v, kernel=KERNELS["direct"])
+    for cull in (0, 1):
+        ra = run_assign(apd, wl, wl.w0, v=wl.v, kernel=KERNELS["auto"], cull=cull)
+        assert np.array_equal(ra["labels"], rd["labels"]) and ra["dual"] == rd["dual"] and ra["pairs"] == wl.N * wl.M
+    parity.check_assign(wl, wl.w0, rd["labels"], rd["vol"], rd["dual"], v=wl.v, err_gpu=rd["err"])
+    rr = run_assign(apd, wl, wl.w0, v=wl.v, kernel=KERNELS["rowpoly"])
+    orc = parity.oracle_assign(parity.grid_of(wl), wl.X, wl.A, wl.w0, v=wl.v)
+    parity.check_labels(parity.grid_of(wl), wl.X, wl.A, wl.w0, rr["labels"], orc)
+    ell = (1.0 / wl.M) ** (1.0 / dim)                       # unit box
+    rel = 2.0 ** -23 * ((1.0 + 8.0 / min(n)) / ell) ** 2
+    assert abs(rr["dual"] - orc.dual) <= rel * max(abs(orc.dual), abs(orc.quad_part))
+
+
 def test_slab_decomposition_is_exact(apd):
     """The path shards by voxel slabs with the EXISTING call: a z-slab is an apd_grid with
     shifted lo/hi and fewer n_z.  On a power-of-two grid the slab's voxel centres are bit-identical, so labels
