@@ -304,24 +304,61 @@ struct SeedRec {
       return box_radius<2>(r, h.x, h.y, 0.0f);
     }
   }
-  // s and supp of seed_bounds() for the box y0 +- h -- the same expressions in the same order
-  __device__ __forceinline__ void at(float y0x, float y0y, float y0z, float3 h, float* s, float* supp) const {
+  // g = A (y0 - x) and q = |y0 - x|^2_A -- the same expressions in the same order as seed_bounds()
+  __device__ __forceinline__ void grad_at(float y0x, float y0y, float y0z, float* gx, float* gy, float* gz, float* q) const {
     if (DIM == 3) {
       const float dx = y0x - x, dy = y0y - y, dz = y0z - z;
-      const float gx = fmaf(0.5f * a13, dz, fmaf(0.5f * a12, dy, a11 * dx));
-      const float gy = fmaf(0.5f * a23, dz, fmaf(a22, dy, 0.5f * a12 * dx));
-      const float gz = fmaf(a33, dz, fmaf(0.5f * a23, dy, 0.5f * a13 * dx));
-      const float q = fmaf(dz, gz, fmaf(dy, gy, dx * gx));
-      *s = norm_of(q);
-      *supp = fmaf(fabsf(gz), h.z, fmaf(fabsf(gy), h.y, fabsf(gx) * h.x));
+      *gx = fmaf(0.5f * a13, dz, fmaf(0.5f * a12, dy, a11 * dx));
+      *gy = fmaf(0.5f * a23, dz, fmaf(a22, dy, 0.5f * a12 * dx));
+      *gz = fmaf(a33, dz, fmaf(0.5f * a23, dy, 0.5f * a13 * dx));
+      *q = fmaf(dz, *gz, fmaf(dy, *gy, dx * *gx));
     } else {
       const float dx = y0x - x, dy = y0y - y;
-      const float gx = fmaf(0.5f * a12, dy, a11 * dx);
-      const float gy = fmaf(a22, dy, 0.5f * a12 * dx);
-      const float q = fmaf(dy, gy, dx * gx);
-      *s = norm_of(q);
-      *supp = fmaf(fabsf(gy), h.y, fabsf(gx) * h.x);
+      *gx = fmaf(0.5f * a12, dy, a11 * dx);
+      *gy = fmaf(a22, dy, 0.5f * a12 * dx);
+      *gz = 0.0f;
+      *q = fmaf(dy, *gy, dx * *gx);
     }
+  }
+  // s and supp of seed_bounds() for the box y0 +- h
+  __device__ __forceinline__ void at(float y0x, float y0y, float y0z, float3 h, float* s, float* supp) const {
+    float gx, gy, gz, q;
+    grad_at(y0x, y0y, y0z, &gx, &gy, &gz, &q);
+    *s = norm_of(q);
+    *supp = (DIM == 3) ? fmaf(fabsf(gz), h.z, fmaf(fabsf(gy), h.y, fabsf(gx) * h.x)) : fmaf(fabsf(gy), h.y, fabsf(gx) * h.x);
+  }
+};
+
+// PAIRWISE test against one reference seed k of a box y0 +- h (the seed that attains the smallest upper bound):
+// D(y) = C_i(y) - C_k(y) is a quadratic whose large common part cancels; with t = y - y0, |t_m| <= h_m,
+//     D(y0 + t) = D(y0) + 2 (g_i - g_k).t + t^T (A_i - A_k) t
+//              >= D(y0) - 2 sum_m |g_i - g_k|_m h_m + sum_m min(0, dA_mm) h_m^2 - sum_{m<n} |dA'_mn| h_m h_n
+// (dA' = doubled off-diagonals, as stored).  If that is positive, seed k beats seed i at EVERY voxel of the box, so
+// i is never an argmin there.  For equal matrices this is the exact half-space test of the power diagram; it is much
+// sharper than comparing i's lower bound with k's upper bound, whose common variation over the box does not cancel.
+// Returns the bound minus a rounding slack of 8 * 2^-16 of the magnitudes involved.
+template <int DIM>
+struct RefSeed {
+  SeedRec<DIM> r;
+  float gx, gy, gz, q;
+  __device__ __forceinline__ void init(const float* __restrict__ rec, int k, float y0x, float y0y, float y0z) {
+    r.load(rec, k);
+    r.grad_at(y0x, y0y, y0z, &gx, &gy, &gz, &q);
+  }
+  __device__ __forceinline__ float pair_min(const SeedRec<DIM>& ri, float y0x, float y0y, float y0z, float3 h) const {
+    float ix, iy, iz, iq;
+    ri.grad_at(y0x, y0y, y0z, &ix, &iy, &iz, &iq);
+    const float d0 = (iq + ri.nw) - (q + r.nw);
+    float lin = 2.0f * (fabsf(ix - gx) * h.x + fabsf(iy - gy) * h.y);
+    float quad = fminf(ri.a11 - r.a11, 0.0f) * h.x * h.x + fminf(ri.a22 - r.a22, 0.0f) * h.y * h.y -
+                 fabsf(ri.a12 - r.a12) * h.x * h.y;
+    if (DIM == 3) {
+      lin += 2.0f * fabsf(iz - gz) * h.z;
+      quad += fminf(ri.a33 - r.a33, 0.0f) * h.z * h.z - fabsf(ri.a13 - r.a13) * h.x * h.z -
+              fabsf(ri.a23 - r.a23) * h.y * h.z;
+    }
+    const float mag = fabsf(iq) + fabsf(q) + fabsf(ri.nw) + fabsf(r.nw) + lin - quad;
+    return d0 - lin + quad - 8.0f * CULL_EPS * mag;
   }
 };
 
@@ -470,7 +507,10 @@ __global__ void __launch_bounds__(128) cull_bricks_kernel(const CullArgs c) {
     }
     warp_argmin(umin, imin);
     if (n > 0) umin = fminf(umin, exact_upper<DIM>(c.rec, imin, y0x, y0y, y0z, c.hb));
-    const float U = umin + 2.0f * delta * (1.0f + CULL_EPS);
+    const float slack2 = 2.0f * delta * (1.0f + CULL_EPS);
+    const float U = umin + slack2;
+    RefSeed<DIM> ref;                          // the seed that attains the smallest upper bound (warp-uniform)
+    if (n > 0) ref.init(c.rec, imin, y0x, y0y, y0z);
 
     const size_t tile = ((size_t)bz * c.g.tiles_y + by) * c.g.tiles_x + bx;
     const size_t brick = tile * 4 + w;
@@ -482,9 +522,12 @@ __global__ void __launch_bounds__(128) cull_bricks_kernel(const CullArgs c) {
       int i = 0;
       if (pos < n) {
         i = cand(pos);
-        float s, rho, supp, nw;
-        seed_bounds<DIM, 0>(c.rec, i, y0x, y0y, y0z, c.hb, &s, &rho, &supp, &nw);
-        keep = !(lower_bound(s, supp, nw) > U);
+        SeedRec<DIM> r;
+        r.load(c.rec, i);
+        float s, supp;
+        r.at(y0x, y0y, y0z, c.hb, &s, &supp);
+        keep = !(lower_bound(s, supp, r.nw) > U);
+        if (keep) keep = !(ref.pair_min(r, y0x, y0y, y0z, c.hb) > slack2);      // NaN keeps the seed
       }
       const unsigned int bal = __ballot_sync(0xffffffffu, keep);
       if (keep) {
