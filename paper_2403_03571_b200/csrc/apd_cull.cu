@@ -8,7 +8,8 @@
 // With U_T = min_k (s_k + rho_k)^2 - w_k, a seed whose lower bound exceeds U_T is beaten at EVERY voxel of the tile by
 // the seed attaining U_T, so it is never an argmin and can be skipped: the labels are those of brute force.
 // The kernels use two sharper forms of the same bounds (lower_bound(): support function of the box along the
-// A-gradient; exact_upper(): exact corner maximum of the best seed's cost) -- derivations at the functions.
+// A-gradient; exact_upper(): exact corner maximum of the best seed's cost) and, at brick level, a pairwise bound on
+// C_i - C_k* over the box (RefSeed::pair_min()) -- derivations at the functions.
 // All bounds are taken in fp32 with a relative slack of 2^-16 on every term, three orders above the rounding of the
 // fp32 cost evaluation, so rounding can never prune a winner (test: labels with culling == labels without, bit-exact).
 // A must be positive definite for the bound to hold (PAPER.md:51-54 assumes it; the library does not check).
