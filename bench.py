@@ -386,7 +386,7 @@ def run_ours(args):
                 "e2e": {"value": world * wl.pairs / e2e_s / 1e9, "unit": UNIT, "h2d_bytes_per_step": h2d,
                         "d2h_bytes_per_step": d2h, "ms_per_step": e2e_s * 1e3, "ms_per_step_max": max(e2e_each) * 1e3,
                         "steps": e2e_steps,
-                        "call": "apd_assign_host (pinned host buffers; device alloc + copies inside)"},
+                        "call": "apd_assign_host (pinned host buffers; H2D/D2H copies inside, device scratch kept by the context)"},
                 "gpu_launches": 3 * args.steps, "launches_per_step": ["pack_pairs_kernel", "assign_rowpoly_kernel",
                                                                       "finalize_kernel"]}
         line.update(extra)

@@ -205,9 +205,10 @@ int apd_solve_refine(apd_ctx* ctx, apd_grid* grid, int32_t M, const float* X, co
 double  apd_resolution_bound(int32_t dim, double domain_volume, double v_min, double eps, int32_t practical);
 int32_t apd_choose_resolution(int32_t dim, double domain_volume, double v_min, double eps, int32_t practical);
 
-/* Same two calls with HOST arrays: the library allocates device buffers, copies in, runs the
- * device call above, copies the results out and frees.  Every pointer is HOST memory; NULL is
- * allowed where the device call allows it.  Synchronous. */
+/* Same two calls with HOST arrays: the library copies in, runs the device call above and copies
+ * the results out.  The device buffers belong to the context (grow-only, reused by the next host
+ * call, freed by apd_destroy).  Every pointer is HOST memory (pinned memory makes the copies
+ * faster); NULL is allowed where the device call allows it.  Synchronous. */
 int apd_assign_host(apd_ctx* ctx, const apd_grid* grid, int32_t M,
                     const float* X, const float* A, const float* w, const float* target_vol,
                     int32_t* labels, double* vol, double* dual, double* max_rel_err,

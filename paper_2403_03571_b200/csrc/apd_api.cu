@@ -34,6 +34,7 @@ static void free_ws(Workspace& ws) {
   cudaFree(ws.super_count); cudaFree(ws.pairs_ctr);
   cudaFree(ws.seeds); cudaFree(ws.count); cudaFree(ws.idxsum); cudaFree(ws.dual_partial);
   cudaFree(ws.sstate); cudaFree(ws.svec); cudaFree(ws.gram); cudaFree(ws.w32); cudaFree(ws.wref); cudaFree(ws.e_vol); cudaFree(ws.e_scal); cudaFree(ws.hist);
+  for (int i = 0; i < Workspace::HOST_SLOTS; ++i) cudaFree(ws.host_buf[i]);
   if (ws.report) cudaFreeHost(ws.report);
   for (int i = 0; i < 2; ++i) if (ws.sev[i]) cudaEventDestroy(ws.sev[i]);
   if (ws.ev0) cudaEventDestroy(ws.ev0);

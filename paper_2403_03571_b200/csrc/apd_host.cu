@@ -1,22 +1,32 @@
 // apd_host.cu -- apd_assign_host / apd_solve_host: the same calls with HOST arrays.  The library
-// allocates device buffers, copies in (cudaMemcpyAsync, one per array), runs the device call,
-// copies out.  Used for the end-to-end ("e2e") measurement and by callers without a device
-// allocator of their own.
+// copies in (cudaMemcpyAsync, one per array), runs the device call, copies out.  The device
+// buffers belong to the context: grow-only, reused by the next host call, freed by apd_destroy
+// (a 64 MiB cudaMalloc + cudaFree per call cost more than the label copy).  Used for the
+// end-to-end ("e2e") measurement and by callers without a device allocator of their own.
 #include "apd_internal.cuh"
-#include <vector>
 
 namespace {
 
+// hands out the context's scratch slots in call order
 struct DevBufs {
-  std::vector<void*> ptrs;
-  ~DevBufs() { for (void* p : ptrs) cudaFree(p); }
+  apd::Workspace& ws;
+  int next = 0;
+  explicit DevBufs(apd::Workspace& w) : ws(w) {}
   template <typename T>
   cudaError_t alloc(T** out, size_t count) {
-    void* p = nullptr;
-    cudaError_t e = cudaMalloc(&p, count * sizeof(T));
-    if (e == cudaSuccess) ptrs.push_back(p);
-    *out = static_cast<T*>(p);
-    return e;
+    if (next >= apd::Workspace::HOST_SLOTS) return cudaErrorMemoryAllocation;
+    const int k = next++;                       // count == 0 (an optional array not asked for) still takes its slot
+    const size_t bytes = count * sizeof(T);
+    if (bytes == 0) { *out = nullptr; return cudaSuccess; }
+    if (ws.host_cap[k] < bytes) {
+      cudaFree(ws.host_buf[k]);
+      ws.host_buf[k] = nullptr; ws.host_cap[k] = 0;
+      cudaError_t e = cudaMalloc(&ws.host_buf[k], bytes);
+      if (e != cudaSuccess) return e;
+      ws.host_cap[k] = bytes;
+    }
+    *out = static_cast<T*>(ws.host_buf[k]);
+    return cudaSuccess;
   }
 };
 
@@ -51,7 +61,7 @@ extern "C" int apd_assign_host(apd_ctx* ctx, const apd_grid* grid, int32_t M, co
   const long long N = grid_voxels(grid);
   if (N < 1 || N >= (1ll << 31)) { ctx->err = "apd_assign_host: bad grid"; return APD_E_ARG; }
   HOST_TRY(cudaSetDevice(ctx->ws.device));
-  DevBufs b;
+  DevBufs b(ctx->ws);
   float *dX, *dA, *dw, *dv = nullptr;
   int32_t* dl = nullptr;
   double *dvol, *dscal, *dcen = nullptr;
@@ -59,11 +69,11 @@ extern "C" int apd_assign_host(apd_ctx* ctx, const apd_grid* grid, int32_t M, co
   HOST_TRY(b.alloc(&dX, (size_t)M * d));
   HOST_TRY(b.alloc(&dA, (size_t)M * d * d));
   HOST_TRY(b.alloc(&dw, (size_t)M));
-  if (target_vol) HOST_TRY(b.alloc(&dv, (size_t)M));
-  if (labels) HOST_TRY(b.alloc(&dl, (size_t)N));
+  HOST_TRY(b.alloc(&dv, target_vol ? (size_t)M : 0));
+  HOST_TRY(b.alloc(&dl, labels ? (size_t)N : 0));
   HOST_TRY(b.alloc(&dvol, (size_t)M));
   HOST_TRY(b.alloc(&dscal, 2));
-  if (centroids) HOST_TRY(b.alloc(&dcen, (size_t)M * d));
+  HOST_TRY(b.alloc(&dcen, centroids ? (size_t)M * d : 0));
   HOST_TRY(b.alloc(&dpairs, 1));
   cudaStream_t st = nullptr;
   HOST_TRY(cudaMemcpyAsync(dX, X, sizeof(float) * M * d, cudaMemcpyHostToDevice, st));
@@ -101,18 +111,18 @@ extern "C" int apd_solve_host(apd_ctx* ctx, const apd_grid* grid, int32_t M, con
   const long long N = grid_voxels(grid);
   if (N < 1 || N >= (1ll << 31)) { ctx->err = "apd_solve_host: bad grid"; return APD_E_ARG; }
   HOST_TRY(cudaSetDevice(ctx->ws.device));
-  DevBufs b;
+  DevBufs b(ctx->ws);
   float *dX, *dA, *dv, *dwi = nullptr, *dw;
   int32_t* dl = nullptr;
   double *dvol = nullptr, *dw64 = nullptr;
   HOST_TRY(b.alloc(&dX, (size_t)M * d));
   HOST_TRY(b.alloc(&dA, (size_t)M * d * d));
   HOST_TRY(b.alloc(&dv, (size_t)M));
-  if (w_init) HOST_TRY(b.alloc(&dwi, (size_t)M));
+  HOST_TRY(b.alloc(&dwi, w_init ? (size_t)M : 0));
   HOST_TRY(b.alloc(&dw, (size_t)M));
-  if (labels) HOST_TRY(b.alloc(&dl, (size_t)N));
-  if (vol) HOST_TRY(b.alloc(&dvol, (size_t)M));
-  if (w64) HOST_TRY(b.alloc(&dw64, (size_t)M));
+  HOST_TRY(b.alloc(&dl, labels ? (size_t)N : 0));
+  HOST_TRY(b.alloc(&dvol, vol ? (size_t)M : 0));
+  HOST_TRY(b.alloc(&dw64, w64 ? (size_t)M : 0));
   cudaStream_t st = nullptr;
   HOST_TRY(cudaMemcpyAsync(dX, X, sizeof(float) * M * d, cudaMemcpyHostToDevice, st));
   HOST_TRY(cudaMemcpyAsync(dA, A, sizeof(float) * M * d * d, cudaMemcpyHostToDevice, st));

@@ -94,6 +94,10 @@ struct Workspace {
   int hist_len = 0;
   int last_rebuilds = 0;                // candidate-list rebuilds of the last solve (0 without culling)
   struct SolveReport* report = nullptr; // pinned, mapped host memory the step kernel writes
+  // device scratch of the *_host calls (apd_host.cu): grow-only, kept between calls, freed with the context
+  static constexpr int HOST_SLOTS = 10;
+  void* host_buf[HOST_SLOTS] = {};
+  size_t host_cap[HOST_SLOTS] = {};
   cudaEvent_t sev[2] = {nullptr, nullptr};
 };
 
