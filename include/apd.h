@@ -56,9 +56,14 @@ enum {
                               instead of a few ulp of itself                                        */
   APD_KERNEL_DIRECT = 1,   /* un-hoisted direct form: 12 (3D) / 7 (2D) FP32 instr. per pair;
                               the reference kernel the FP32-pipe fraction is quoted on             */
-  APD_KERNEL_ROWPOLY = 2   /* quadratic in the offset from the row's midpoint (1.5 FMA per pair) with
+  APD_KERNEL_ROWPOLY = 2,  /* quadratic in the offset from the row's midpoint (1.5 FMA per pair) with
                               coefficients polynomial in the row's offset from the tile's midpoint,
                               packed f32x2, deferred argmin                                        */
+  APD_KERNEL_TENSOR = 3    /* 3D only, brute force only (no opts.cull): the cost lifted to a 10-monomial
+                              polynomial in the integer voxel offset from a tile's reference voxel,
+                              coefficients split three ways into bf16, contracted on the tensor
+                              cores (tcgen05.mma, fp32 accumulators in TMEM); argmin epilogue on
+                              the CUDA cores.  Costs carry fp32 rounding; never chosen by AUTO     */
 };
 
 /* opts.cull = 1: exact culling (not in the paper).  Per block of voxels the library keeps only

@@ -25,6 +25,7 @@ APD_E_ARCH = -3
 KERNEL_AUTO = 0
 KERNEL_DIRECT = 1
 KERNEL_ROWPOLY = 2
+KERNEL_TENSOR = 3
 
 
 class ApdError(RuntimeError):

@@ -14,7 +14,7 @@ _PKG = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_PKG, "csrc")
 LIB_PATH = os.path.join(_PKG, "libapd_b200.so")
 SOURCES = ["apd_api.cu", "apd_kernels.cu", "apd_rowpoly.cu", "apd_finalize.cu", "apd_lbfgs.cu",
-           "apd_host.cu", "apd_probe.cu", "apd_cull.cu", "apd_lloyd.cu", "apd_points.cu"]
+           "apd_host.cu", "apd_probe.cu", "apd_cull.cu", "apd_lloyd.cu", "apd_points.cu", "apd_tensor.cu"]
 HEADERS = ["apd_internal.cuh", "apd_device.cuh", "apd_epilogue.cuh", os.path.join("..", "..", "include", "apd.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v"]

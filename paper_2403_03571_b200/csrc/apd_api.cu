@@ -30,7 +30,7 @@ extern "C" void apd_default_opts(apd_opts* o) {
 }
 
 static void free_ws(Workspace& ws) {
-  cudaFree(ws.pt_acc); cudaFree(ws.rec); cudaFree(ws.brick_list); cudaFree(ws.brick_count); cudaFree(ws.super_list);
+  cudaFree(ws.pt_acc); cudaFree(ws.qfix); cudaFree(ws.rec); cudaFree(ws.brick_list); cudaFree(ws.brick_count); cudaFree(ws.super_list);
   cudaFree(ws.super_count); cudaFree(ws.pairs_ctr);
   cudaFree(ws.seeds); cudaFree(ws.count); cudaFree(ws.idxsum); cudaFree(ws.dual_partial);
   cudaFree(ws.sstate); cudaFree(ws.svec); cudaFree(ws.gram); cudaFree(ws.w32); cudaFree(ws.wref); cudaFree(ws.e_vol); cudaFree(ws.e_scal); cudaFree(ws.hist);
@@ -133,7 +133,8 @@ static bool narrow_grid(const apd_grid* grid) {
 }
 int resolve_kernel(const apd_opts* o, const apd_grid* grid, bool* cull, std::string* err) {
   int k = o ? o->kernel : APD_KERNEL_AUTO;
-  if (k != APD_KERNEL_AUTO && k != APD_KERNEL_DIRECT && k != APD_KERNEL_ROWPOLY) { *err = "unknown opts.kernel"; return -1; }
+  if (k != APD_KERNEL_AUTO && k != APD_KERNEL_DIRECT && k != APD_KERNEL_ROWPOLY && k != APD_KERNEL_TENSOR) { *err = "unknown opts.kernel"; return -1; }
+  if (k == APD_KERNEL_TENSOR && grid && grid->dim != 3) { *err = "APD_KERNEL_TENSOR is 3D only"; return -1; }
   if (o && (o->cull != 0 && o->cull != 1)) { *err = "opts.cull must be 0 or 1"; return -1; }
   if (o && (o->reserved[0] || o->reserved[1] || o->reserved[2])) { *err = "opts.reserved must be 0"; return -1; }
   *cull = o && o->cull;
@@ -170,6 +171,13 @@ int enqueue_evaluation(apd_ctx* ctx, const GridDev& g, int kernel, int M, const 
   else
     APD_CUDA_TRY(ctx, launch_pack_seeds(g.dim, M, M_pad, X, A, w, ws.seeds, ws.count,
                                         centroids ? ws.idxsum : nullptr, done_flag, st));
+  if (kernel == APD_KERNEL_TENSOR) {
+    if (!ws.qfix) {
+      const size_t m_pad_max = ((size_t)ws.max_seeds + SEED_CHUNK - 1) / SEED_CHUNK * SEED_CHUNK;
+      APD_CUDA_TRY(ctx, cudaMalloc(&ws.qfix, m_pad_max * 3 * sizeof(uint4)));
+    }
+    APD_CUDA_TRY(ctx, launch_pack_qfix(g, M_pad, ws.seeds, ws.qfix, done_flag, st));
+  }
   AssignArgs a;
   a.g = g; a.M = M; a.M_pad = M_pad; a.seeds = ws.seeds; a.labels = labels; a.count = ws.count;
   for (int j = 0; j < 16; ++j) {      // in-row offsets from a row's midpoint and their squares (apd_rowpoly.cu: RowTau)
@@ -181,6 +189,7 @@ int enqueue_evaluation(apd_ctx* ctx, const GridDev& g, int kernel, int M, const 
   a.rec = nullptr; a.brick_list = nullptr; a.brick_count = nullptr; a.super_list = nullptr; a.super_count = nullptr;
   a.super_x = a.super_y = 0; a.pairs_ctr = nullptr;
   a.done_flag = done_flag;
+  a.qfix = ws.qfix;
   if (cull) {
     // a7: two-level candidate lists, rebuilt every evaluation (the bounds depend on w)
     int nsx, nsy, nsz;

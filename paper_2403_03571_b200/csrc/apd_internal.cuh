@@ -60,6 +60,7 @@ struct AssignArgs {
   // centre, and exactly the centre on power-of-two grids.)
   float tt[32];
   const int* done_flag;  // solve loop only: kernels return at once when *done_flag != 0; else nullptr
+  const uint4* qfix;     // TENSOR kernel only: [M_pad, 3] tile-independent bf16 coefficient parts (apd_tensor.cu)
 };
 
 struct Workspace {
@@ -78,6 +79,7 @@ struct Workspace {
   int* super_count = nullptr;          // [super_cap_n]
   size_t super_cap_n = 0;
   unsigned long long* pairs_ctr = nullptr;
+  uint4* qfix = nullptr;               // TENSOR kernel: [M_pad, 3], allocated on first use
   double* pt_acc = nullptr;            // apd_assign_points: fp64 accumulators vol[max_seeds] | csum[max_seeds,3]
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
   bool timed = false;
@@ -111,6 +113,11 @@ cudaError_t launch_pack_pairs(int dim, int M, int M_pad, const float* X, const f
                               float* seeds, unsigned int* count, unsigned long long* idxsum,
                               const int* done_flag, cudaStream_t st);
 cudaError_t launch_assign_rowpoly(const AssignArgs& a, cudaStream_t st);
+// TENSOR kernel (apd_tensor.cu, row a8): reads the DIRECT record table plus its own bf16 table
+void tensor_tile_counts(int nx, int ny, int nz, int* tx, int* ty, int* tz);
+cudaError_t launch_pack_qfix(const GridDev& g, int M_pad, const float* rec, uint4* qfix, const int* done_flag,
+                             cudaStream_t st);
+cudaError_t launch_assign_tensor(const AssignArgs& a, cudaStream_t st);
 // ---- culling geometry (a7) --------------------------------------------------------------------------------
 // The culled kernel always runs the SHORT-row geometry: CTA tile 16 x 16 x 8 voxels (3D) / 32 x 64 pixels (2D),
 // 128 threads = 4 warps, each warp owning one BRICK of 32 rows of 16 voxels:

@@ -175,6 +175,7 @@ static inline int cdiv(int a, int b) { return (a + b - 1) / b; }
 // Returns the ROWPOLY row-length choice (0 for the DIRECT kernel).
 int assign_tile_counts(int kernel, int dim, int nx, int ny, int nz, int sm_count, bool cull, int* tx, int* ty, int* tz) {
   if (kernel == APD_KERNEL_ROWPOLY) return rowpoly_tile_counts(dim, nx, ny, nz, sm_count, cull, tx, ty, tz);
+  if (kernel == APD_KERNEL_TENSOR) { tensor_tile_counts(nx, ny, nz, tx, ty, tz); return 0; }
   if (dim == 3) {
     using G = DirectGeom<3>;
     *tx = cdiv(nx, G::TXT * G::V); *ty = cdiv(ny, G::TYT); *tz = cdiv(nz, G::TZT);
@@ -187,6 +188,7 @@ int assign_tile_counts(int kernel, int dim, int nx, int ny, int nz, int sm_count
 
 cudaError_t launch_assign(int kernel, const AssignArgs& a, cudaStream_t st) {
   if (kernel == APD_KERNEL_ROWPOLY) return launch_assign_rowpoly(a, st);
+  if (kernel == APD_KERNEL_TENSOR) return launch_assign_tensor(a, st);
   const int n_tiles = a.g.tiles_x * a.g.tiles_y * a.g.tiles_z;
   if (a.g.dim == 3) assign_direct_kernel<3><<<n_tiles, 256, 0, st>>>(a);
   else              assign_direct_kernel<2><<<n_tiles, 256, 0, st>>>(a);

@@ -1,0 +1,320 @@
+// apd_tensor.cu -- row a8 of the path: the cost matrix of Algorithm 1 step 1 (PAPER.md:131,
+// eq. 2.1 at PAPER.md:58-61) lifted to a bf16 tensor-core contraction, the argmin of step 2 as the
+// epilogue.  3D only.
+//
+// For a voxel at INTEGER offset t = (i, j, k) from the reference voxel y0 of its tile and a seed x with matrix A,
+//     C(t) = sum_{m<=n} a'_mn s_m s_n t_m t_n  +  sum_m (g_m s_m) t_m  +  r0,
+//     g = (A + A^T)(y0 - x),   r0 = (y0 - x)^T A (y0 - x) - w,   s = voxel sides,
+// a polynomial with 10 monomials.  Phi[voxel][.] holds the monomials -- integers of magnitude <= 64, exact in bf16 --
+// and Theta[seed][.] the 10 fp32 coefficients split three ways into bf16 (hi + mid + lo carries 24 bits), each
+// monomial repeated under its three parts: K = 30, padded to 32.  Every product is exact in fp32 and the tensor core
+// accumulates in fp32, so the cost carries fp32 rounding only.
+//
+// One CTA = one tile of 16 x 8 x 4 voxels = 4 UMMA M-tiles of 128 rows (one z-plane each; voxel <-> TMEM lane <->
+// thread) against chunks of 64 seeds: per chunk 4 x 2 tcgen05.mma (M 128, N 64, K 16, kind::f16, A and B K-major in
+// shared memory without swizzle), accumulators double-buffered in TMEM (2 x 4 x 64 = 512 columns).  Warps 0-15 drain
+// chunk k from TMEM (tcgen05.ld 32x32b, 3-input min, argmin found by a rescan of the registers only when some
+// voxel's minimum dropped) while the tensor core runs chunk k + 1 and warps 16-17 expand the coefficients of chunk
+// k + 2 about this tile's y0.
+#include "apd_internal.cuh"
+#include "apd_device.cuh"
+#include <cuda_bf16.h>
+#include <math_constants.h>
+
+namespace apd {
+
+constexpr int TC_TX = 16, TC_TY = 8, TC_TZ = 4;      // voxel tile
+constexpr int TC_N = 64;                              // seeds per chunk
+constexpr int TC_EPI_THREADS = TC_TX * TC_TY * TC_TZ; // 512: one per voxel
+constexpr int TC_BUILDERS = TC_N;                     // 64: one per seed of a chunk
+constexpr int TC_THREADS = TC_EPI_THREADS + TC_BUILDERS;
+constexpr int TC_QFIX = 24;                           // bf16 per seed in the tile-independent table (18 used)
+
+// ---- tcgen05 wrappers ----------------------------------------------------------------------------------------
+__device__ __forceinline__ void tc_alloc512(uint32_t* slot) {
+  asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(slot)) : "memory");
+  asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tc_free512(uint32_t addr) {
+  asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(addr) : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_mma_bf16(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc,
+                                            uint32_t accumulate) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "setp.ne.b32 p, %4, 0;\n"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n"
+      "}\n" ::"r"(d_tmem),
+      "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+__device__ __forceinline__ void tc_commit(uint64_t* bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar))
+               : "memory");
+}
+// K-major operand without swizzle: core matrix = 8 rows x 16 bytes, rows 16 bytes apart; the two core matrices of one
+// K = 16 step are LBO bytes apart, 8-row groups SBO bytes apart.
+__device__ __forceinline__ uint64_t tc_smem_desc(uint32_t saddr, uint32_t lbo, uint32_t sbo) {
+  uint64_t d = 0;
+  d |= (uint64_t)((saddr >> 4) & 0x3FFF);
+  d |= (uint64_t)((lbo >> 4) & 0x3FFF) << 16;
+  d |= (uint64_t)((sbo >> 4) & 0x3FFF) << 32;
+  d |= (uint64_t)1 << 46;                        // descriptor version of sm_100
+  return d;                                      // base offset 0, layout type 0 = no swizzle
+}
+#define TC_LD32(addr, v)                                                                                              \
+  asm volatile(                                                                                                       \
+      "tcgen05.ld.sync.aligned.32x32b.x32.b32 "                                                                       \
+      "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,"   \
+      "%29,%30,%31}, [%32];"                                                                                          \
+      : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]), "=f"(v[4]), "=f"(v[5]), "=f"(v[6]), "=f"(v[7]), "=f"(v[8]),   \
+        "=f"(v[9]), "=f"(v[10]), "=f"(v[11]), "=f"(v[12]), "=f"(v[13]), "=f"(v[14]), "=f"(v[15]), "=f"(v[16]),        \
+        "=f"(v[17]), "=f"(v[18]), "=f"(v[19]), "=f"(v[20]), "=f"(v[21]), "=f"(v[22]), "=f"(v[23]), "=f"(v[24]),       \
+        "=f"(v[25]), "=f"(v[26]), "=f"(v[27]), "=f"(v[28]), "=f"(v[29]), "=f"(v[30]), "=f"(v[31])                     \
+      : "r"(addr))
+__device__ __forceinline__ void tc_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+
+// fp32 -> three bf16 whose sum carries 24 bits of v (each remainder is exact in fp32)
+__device__ __forceinline__ void split3(float v, unsigned short& h, unsigned short& m, unsigned short& l) {
+  const __nv_bfloat16 bh = __float2bfloat16_rn(v);
+  const float r1 = v - __bfloat162float(bh);
+  const __nv_bfloat16 bm = __float2bfloat16_rn(r1);
+  const float r2 = r1 - __bfloat162float(bm);
+  const __nv_bfloat16 bl = __float2bfloat16_rn(r2);
+  h = __bfloat16_as_ushort(bh); m = __bfloat16_as_ushort(bm); l = __bfloat16_as_ushort(bl);
+}
+__device__ __forceinline__ uint32_t pk(unsigned short lo, unsigned short hi) { return (uint32_t)lo | ((uint32_t)hi << 16); }
+
+// ---- tile-independent part of Theta: the six quadratic coefficients in voxel units, split three ways ---------------
+__global__ void pack_qfix_kernel(int M_pad, const float* __restrict__ rec, double sx, double sy, double sz,
+                                 uint4* __restrict__ qfix, const int* __restrict__ done_flag) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= M_pad) return;
+  if (done_flag && *done_flag) return;
+  const float* r = rec + (size_t)i * REC3;
+  const float q[6] = {(float)((double)r[3] * sx * sx), (float)((double)r[6] * sy * sy), (float)((double)r[8] * sz * sz),
+                      (float)((double)r[4] * sx * sy), (float)((double)r[5] * sx * sz), (float)((double)r[7] * sy * sz)};
+  unsigned short b[TC_QFIX];
+#pragma unroll
+  for (int k = 0; k < TC_QFIX; ++k) b[k] = 0;
+#pragma unroll
+  for (int k = 0; k < 6; ++k) split3(q[k], b[3 * k], b[3 * k + 1], b[3 * k + 2]);
+  uint4* dst = qfix + (size_t)i * 3;
+#pragma unroll
+  for (int k = 0; k < 3; ++k)
+    dst[k] = make_uint4(pk(b[8 * k], b[8 * k + 1]), pk(b[8 * k + 2], b[8 * k + 3]), pk(b[8 * k + 4], b[8 * k + 5]),
+                        pk(b[8 * k + 6], b[8 * k + 7]));
+}
+
+struct TcSeedRegs { float4 p0, p1, p2; uint4 q0, q1, q2; };
+
+__device__ __forceinline__ void tc_load_seed(const AssignArgs& a, int i, TcSeedRegs& s) {
+  const float4* rp = reinterpret_cast<const float4*>(a.seeds) + (size_t)i * 3;
+  const uint4* qp = a.qfix + (size_t)i * 3;
+  s.p0 = __ldg(rp); s.p1 = __ldg(rp + 1); s.p2 = __ldg(rp + 2);
+  s.q0 = __ldg(qp); s.q1 = __ldg(qp + 1); s.q2 = __ldg(qp + 2);
+}
+
+// Theta row of one seed about the tile's reference point -> rows of the K-major B tile (4 pieces of 16 bytes)
+__device__ __forceinline__ void tc_build_seed(const TcSeedRegs& s, bool real, float y0x, float y0y, float y0z, float sx,
+                                              float sy, float sz, unsigned char* btile, int row) {
+  uint4 k0 = s.q0, k1 = s.q1, k2, k3;
+  if (real) {
+    const float dx = y0x - s.p0.x, dy = y0y - s.p0.y, dz = y0z - s.p0.z;
+    const float a11 = s.p0.w, a12 = s.p1.x, a13 = s.p1.y, a22 = s.p1.z, a23 = s.p1.w, a33 = s.p2.x, nw = s.p2.y;
+    const float u = fmaf(a13, dz, fmaf(a12, dy, a11 * dx));
+    const float v = fmaf(a23, dz, a22 * dy);
+    const float t = a33 * dz;
+    float r0 = fmaf(dx, u, nw);
+    r0 = fmaf(dy, v, r0);
+    r0 = fmaf(dz, t, r0);
+    const float gx = fmaf(a13, dz, fmaf(a12, dy, 2.0f * a11 * dx)) * sx;
+    const float gy = fmaf(a23, dz, fmaf(a12, dx, 2.0f * a22 * dy)) * sy;
+    const float gz = fmaf(a23, dy, fmaf(a13, dx, 2.0f * a33 * dz)) * sz;
+    unsigned short xh, xm, xl, yh, ym, yl, zh, zm, zl, rh, rm, rl;
+    split3(gx, xh, xm, xl); split3(gy, yh, ym, yl); split3(gz, zh, zm, zl); split3(r0, rh, rm, rl);
+    k2 = make_uint4(s.q2.x, pk(xh, xm), pk(xl, yh), pk(ym, yl));
+    k3 = make_uint4(pk(zh, zm), pk(zl, rh), pk(rm, rl), 0u);
+  } else {   // padding seed: constant cost 2^100, never the minimum of a chunk that holds a real seed
+    k0 = k1 = make_uint4(0u, 0u, 0u, 0u);
+    k2 = make_uint4(0u, 0u, 0u, 0u);
+    k3 = make_uint4(0u, 0x71800000u, 0u, 0u);   // K = 27: bf16 0x7180 = 2^100
+  }
+  unsigned char* p = btile + (row >> 3) * 512 + (row & 7) * 16;
+  *reinterpret_cast<uint4*>(p) = k0;
+  *reinterpret_cast<uint4*>(p + 128) = k1;
+  *reinterpret_cast<uint4*>(p + 256) = k2;
+  *reinterpret_cast<uint4*>(p + 384) = k3;
+}
+
+__global__ void __launch_bounds__(TC_THREADS, 1) assign_tensor_kernel(const AssignArgs a) {
+  __shared__ __align__(128) unsigned char s_A[4 * 128 * 64];       // Phi: 4 M-tiles x 128 rows x 32 bf16
+  __shared__ __align__(128) unsigned char s_B[2][TC_N * 64];       // Theta: 2 stages x 64 rows x 32 bf16
+  __shared__ __align__(8) uint64_t s_bar[2];
+  __shared__ uint32_t s_tmem;
+  __shared__ double s_red[TC_THREADS / 32];
+
+  if (a.done_flag && *a.done_flag) return;
+  const int tid = threadIdx.x, warp = tid >> 5;
+  const int b = blockIdx.x;
+  const int bx = b % a.g.tiles_x, by = (b / a.g.tiles_x) % a.g.tiles_y, bz = b / (a.g.tiles_x * a.g.tiles_y);
+  const bool builder = tid >= TC_EPI_THREADS;
+  const int nch = a.M_pad / TC_N;
+
+  // reference voxel of the tile and the voxel sides
+  const float y0x = (float)(a.g.lo[0] + ((double)(bx * TC_TX + TC_TX / 2) + 0.5) * a.g.s[0]);
+  const float y0y = (float)(a.g.lo[1] + ((double)(by * TC_TY + TC_TY / 2) + 0.5) * a.g.s[1]);
+  const float y0z = (float)(a.g.lo[2] + ((double)(bz * TC_TZ + TC_TZ / 2) + 0.5) * a.g.s[2]);
+  const float sx = (float)a.g.s[0], sy = (float)a.g.s[1], sz = (float)a.g.s[2];
+
+  if (tid == 0) {
+    mbar_init(&s_bar[0], 1);
+    mbar_init(&s_bar[1], 1);
+    mbar_fence_init();
+  }
+  if (warp == 0) tc_alloc512(&s_tmem);
+
+  TcSeedRegs sr;
+  const int sid = tid - TC_EPI_THREADS;
+  if (!builder) {
+    // Phi row of this thread's voxel: monomials of the integer offsets, each under its three coefficient parts
+    const int ti = (tid & 15) - TC_TX / 2, tj = ((tid >> 4) & 7) - TC_TY / 2, tk = (tid >> 7) - TC_TZ / 2;
+    const float mono[10] = {(float)(ti * ti), (float)(tj * tj), (float)(tk * tk), (float)(ti * tj), (float)(ti * tk),
+                            (float)(tj * tk), (float)ti, (float)tj, (float)tk, 1.0f};
+    unsigned short e[32];
+#pragma unroll
+    for (int m = 0; m < 10; ++m) {
+      const unsigned short h = __bfloat16_as_ushort(__float2bfloat16_rn(mono[m]));
+      e[3 * m] = h; e[3 * m + 1] = h; e[3 * m + 2] = h;
+    }
+    e[30] = 0; e[31] = 0;
+    const int mt = tid >> 7, row = tid & 127;
+    unsigned char* p = s_A + mt * 8192 + (row >> 3) * 512 + (row & 7) * 16;
+#pragma unroll
+    for (int kc = 0; kc < 4; ++kc)
+      *reinterpret_cast<uint4*>(p + kc * 128) = make_uint4(pk(e[8 * kc], e[8 * kc + 1]), pk(e[8 * kc + 2], e[8 * kc + 3]),
+                                                           pk(e[8 * kc + 4], e[8 * kc + 5]), pk(e[8 * kc + 6], e[8 * kc + 7]));
+  } else {
+    tc_load_seed(a, sid, sr);
+    tc_build_seed(sr, sid < a.M, y0x, y0y, y0z, sx, sy, sz, s_B[0], sid);
+    if (nch > 1) {
+      tc_load_seed(a, TC_N + sid, sr);
+      tc_build_seed(sr, TC_N + sid < a.M, y0x, y0y, y0z, sx, sy, sz, s_B[1], sid);
+    }
+    if (nch > 2) tc_load_seed(a, 2 * TC_N + sid, sr);
+  }
+  fence_proxy_async_smem();
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = s_tmem;
+
+  // instruction descriptor: D fp32, A and B bf16, both K-major, N = 64, M = 128
+  constexpr uint32_t IDESC = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(TC_N >> 3) << 17) | ((128u >> 4) << 24);
+  const uint32_t sA = smem_u32(s_A), sB = smem_u32(s_B[0]);
+  auto issue = [&](int c) {
+    const int st = c & 1;
+    tc_fence_after();
+#pragma unroll
+    for (int mt = 0; mt < 4; ++mt) {
+#pragma unroll
+      for (int ks = 0; ks < 2; ++ks) {
+        const uint64_t ad = tc_smem_desc(sA + mt * 8192 + ks * 256, 128, 512);
+        const uint64_t bd = tc_smem_desc(sB + st * (TC_N * 64) + ks * 256, 128, 512);
+        tc_mma_bf16(tmem + (uint32_t)((st * 4 + mt) * TC_N), ad, bd, IDESC, (uint32_t)ks);
+      }
+    }
+    tc_commit(&s_bar[st]);
+  };
+  if (tid == TC_EPI_THREADS) issue(0);
+
+  float best = CUDART_INF_F;
+  int lab = 0;
+  const uint32_t lane_addr = tmem + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)((warp >> 2) * TC_N);
+
+  for (int c = 0; c < nch; ++c) {
+    if (tid == TC_EPI_THREADS && c + 1 < nch) issue(c + 1);
+    mbar_wait(&s_bar[c & 1], (uint32_t)((c >> 1) & 1));
+    tc_fence_after();
+    if (builder) {
+      if (c + 2 < nch) {
+        tc_build_seed(sr, (c + 2) * TC_N + sid < a.M, y0x, y0y, y0z, sx, sy, sz, s_B[c & 1], sid);
+        if (c + 3 < nch) tc_load_seed(a, (c + 3) * TC_N + sid, sr);
+        fence_proxy_async_smem();
+      }
+    } else {
+      float va[32], vb[32];
+      const uint32_t ta = lane_addr + (uint32_t)((c & 1) * 4 * TC_N);
+      TC_LD32(ta, va);
+      TC_LD32(ta + 32, vb);
+      tc_wait_ld();
+      float m1 = best;
+#pragma unroll
+      for (int j = 0; j < 32; j += 2) m1 = min3f(m1, va[j], va[j + 1]);
+      float m2 = m1;
+#pragma unroll
+      for (int j = 0; j < 32; j += 2) m2 = min3f(m2, vb[j], vb[j + 1]);
+      if (__any_sync(0xffffffffu, m2 < best)) {
+        if (m2 < best) {
+          int idx = 0;
+          if (m2 < m1) {
+#pragma unroll
+            for (int j = 31; j >= 0; --j) idx = (vb[j] == m2) ? 32 + j : idx;
+          } else {
+#pragma unroll
+            for (int j = 31; j >= 0; --j) idx = (va[j] == m2) ? j : idx;
+          }
+          lab = c * TC_N + idx;
+          best = m2;
+        }
+      }
+    }
+    tc_fence_before();
+    __syncthreads();
+  }
+
+  // a5 + a6: label store, warp-aggregated counts, index sums, fp64 sum of the minima
+  double dsum = 0.0;
+  if (!builder) {
+    const int ix = bx * TC_TX + (tid & 15), iy = by * TC_TY + ((tid >> 4) & 7), iz = bz * TC_TZ + (tid >> 7);
+    const bool valid = ix < a.g.nx && iy < a.g.ny && iz < a.g.nz;
+    const unsigned vmask = __ballot_sync(0xffffffffu, valid);
+    if (valid) {
+      if (a.labels) a.labels[((long long)iz * a.g.ny + iy) * a.g.nx + ix] = lab;
+      dsum = (double)best;
+      const unsigned peers = __match_any_sync(vmask, lab);
+      if ((int)(threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(a.count + lab, (unsigned int)__popc(peers));
+      if (a.idxsum) {
+        atomicAdd(a.idxsum + (size_t)lab * 3 + 0, (unsigned long long)ix);
+        atomicAdd(a.idxsum + (size_t)lab * 3 + 1, (unsigned long long)iy);
+        atomicAdd(a.idxsum + (size_t)lab * 3 + 2, (unsigned long long)iz);
+      }
+    }
+  }
+  const double tot = block_sum_double<TC_THREADS>(dsum, s_red);
+  if (tid == 0) a.dual_partial[b] = tot;
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 0) tc_free512(tmem);
+}
+
+void tensor_tile_counts(int nx, int ny, int nz, int* tx, int* ty, int* tz) {
+  *tx = (nx + TC_TX - 1) / TC_TX; *ty = (ny + TC_TY - 1) / TC_TY; *tz = (nz + TC_TZ - 1) / TC_TZ;
+}
+
+cudaError_t launch_pack_qfix(const GridDev& g, int M_pad, const float* rec, uint4* qfix, const int* done_flag,
+                             cudaStream_t st) {
+  pack_qfix_kernel<<<(M_pad + 127) / 128, 128, 0, st>>>(M_pad, rec, g.s[0], g.s[1], g.s[2], qfix, done_flag);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_assign_tensor(const AssignArgs& a, cudaStream_t st) {
+  const int n_tiles = a.g.tiles_x * a.g.tiles_y * a.g.tiles_z;
+  assign_tensor_kernel<<<n_tiles, TC_THREADS, 0, st>>>(a);
+  return cudaGetLastError();
+}
+
+}  // namespace apd
