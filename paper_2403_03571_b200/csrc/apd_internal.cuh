@@ -60,7 +60,7 @@ struct AssignArgs {
   // centre, and exactly the centre on power-of-two grids.)
   float tt[32];
   const int* done_flag;  // solve loop only: kernels return at once when *done_flag != 0; else nullptr
-  const uint4* qfix;     // TENSOR kernel only: [M_pad, 3] tile-independent bf16 coefficient parts (apd_tensor.cu)
+  const uint4* qfix;     // TENSOR kernel only: [M_pad, 6] record + tile-independent bf16 coefficient parts (apd_tensor.cu)
 };
 
 struct Workspace {
@@ -79,7 +79,7 @@ struct Workspace {
   int* super_count = nullptr;          // [super_cap_n]
   size_t super_cap_n = 0;
   unsigned long long* pairs_ctr = nullptr;
-  uint4* qfix = nullptr;               // TENSOR kernel: [M_pad, 3], allocated on first use
+  uint4* qfix = nullptr;               // TENSOR kernel: [M_pad, 6] uint4, allocated on first use
   double* pt_acc = nullptr;            // apd_assign_points: fp64 accumulators vol[max_seeds] | csum[max_seeds,3]
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
   bool timed = false;

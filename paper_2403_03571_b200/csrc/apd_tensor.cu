@@ -12,10 +12,15 @@
 //
 // One CTA = one tile of 16 x 8 x 4 voxels = 4 UMMA M-tiles of 128 rows (one z-plane each; voxel <-> TMEM lane <->
 // thread) against chunks of 64 seeds: per chunk 4 x 2 tcgen05.mma (M 128, N 64, K 16, kind::f16, A and B K-major in
-// shared memory without swizzle), accumulators double-buffered in TMEM (2 x 4 x 64 = 512 columns).  Warps 0-15 drain
-// chunk k from TMEM (tcgen05.ld 32x32b, 3-input min, argmin found by a rescan of the registers only when some
-// voxel's minimum dropped) while the tensor core runs chunk k + 1 and warps 16-17 expand the coefficients of chunk
-// k + 2 about this tile's y0.
+// shared memory without swizzle), accumulators double-buffered in TMEM (2 x 4 x 64 = 512 columns).  Warp roles, coupled
+// by mbarriers only (no CTA barrier inside the seed loop):
+//   warp 21 (one lane): cp.async.bulk (TMA 1-D) of raw seed chunks into a 6-stage ring
+//   warp 20 (one lane): issues the MMAs of chunk c when Theta[c] is built and TMEM buffer c & 1 is drained;
+//                       tcgen05.commit signals both consumers
+//   warps 16-19:        two pairs; a pair expands the coefficients of every other chunk about this tile's y0 (one seed
+//                       per thread) into the Theta ring
+//   warps 0-15:         drain chunk c from TMEM (tcgen05.ld 32x32b), release the buffer, 3-input min; the argmin is
+//                       found by a rescan of the registers only when some voxel's minimum dropped.
 #include "apd_internal.cuh"
 #include "apd_device.cuh"
 #include <cuda_bf16.h>
@@ -26,9 +31,15 @@ namespace apd {
 constexpr int TC_TX = 16, TC_TY = 8, TC_TZ = 4;      // voxel tile
 constexpr int TC_N = 64;                              // seeds per chunk
 constexpr int TC_EPI_THREADS = TC_TX * TC_TY * TC_TZ; // 512: one per voxel
-constexpr int TC_BUILDERS = TC_N;                     // 64: one per seed of a chunk
-constexpr int TC_THREADS = TC_EPI_THREADS + TC_BUILDERS;
-constexpr int TC_QFIX = 24;                           // bf16 per seed in the tile-independent table (18 used)
+constexpr int TC_BUILD_WARPS = 4;                     // two pairs; pair p expands the chunks c = p (mod 2)
+constexpr int TC_THREADS = TC_EPI_THREADS + 32 * TC_BUILD_WARPS + 64;   // + the MMA-issuing warp + the TMA warp
+constexpr int TC_QFIX = 24;                           // bf16 per seed in the tile-independent part (18 used)
+constexpr int TC_REC = 24;                            // words per seed in the TENSOR seed table: 12 fp32 + 12 x 2 bf16
+constexpr int TC_RAW_STAGES = 6, TC_TH_STAGES = 4;
+constexpr uint32_t TC_RAW_BYTES = TC_N * TC_REC * 4;  // 6144 per chunk
+constexpr uint32_t TC_TH_BYTES = TC_N * 64;           // 4096 per chunk
+constexpr uint32_t TC_A_BYTES = 4 * 128 * 64;         // 32768
+constexpr uint32_t TC_SMEM = TC_A_BYTES + TC_TH_STAGES * TC_TH_BYTES + TC_RAW_STAGES * TC_RAW_BYTES;
 
 // ---- tcgen05 wrappers ----------------------------------------------------------------------------------------
 __device__ __forceinline__ void tc_alloc512(uint32_t* slot) {
@@ -50,6 +61,17 @@ __device__ __forceinline__ void tc_mma_bf16(uint32_t d_tmem, uint64_t adesc, uin
       "}\n" ::"r"(d_tmem),
       "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
       : "memory");
+}
+__device__ __forceinline__ uint32_t tc_elect_one() {
+  uint32_t pred;
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "elect.sync _|p, 0xffffffff;\n"
+      "selp.u32 %0, 1, 0, p;\n"
+      "}\n"
+      : "=r"(pred));
+  return pred;
 }
 __device__ __forceinline__ void tc_commit(uint64_t* bar) {
   asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar))
@@ -87,10 +109,18 @@ __device__ __forceinline__ void split3(float v, unsigned short& h, unsigned shor
   h = __bfloat16_as_ushort(bh); m = __bfloat16_as_ushort(bm); l = __bfloat16_as_ushort(bl);
 }
 __device__ __forceinline__ uint32_t pk(unsigned short lo, unsigned short hi) { return (uint32_t)lo | ((uint32_t)hi << 16); }
+// two fp32 -> packed bf16x2 {lo = a, hi = b} in one conversion, and the fp32 values of the two halves
+__device__ __forceinline__ uint32_t split_pair(float a, float b) {
+  const __nv_bfloat162 v = __floats2bfloat162_rn(a, b);
+  return *reinterpret_cast<const uint32_t*>(&v);
+}
+__device__ __forceinline__ float bf_lo(uint32_t v) { return __uint_as_float(v << 16); }
+__device__ __forceinline__ float bf_hi(uint32_t v) { return __uint_as_float(v & 0xffff0000u); }
 
-// ---- tile-independent part of Theta: the six quadratic coefficients in voxel units, split three ways ---------------
+// ---- TENSOR seed table: the DIRECT record (12 fp32) followed by the tile-independent part of Theta, the six
+//      quadratic coefficients in voxel units split three ways (18 bf16, padded to 24) --------------------------------
 __global__ void pack_qfix_kernel(int M_pad, const float* __restrict__ rec, double sx, double sy, double sz,
-                                 uint4* __restrict__ qfix, const int* __restrict__ done_flag) {
+                                 uint4* __restrict__ tcs, const int* __restrict__ done_flag) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= M_pad) return;
   if (done_flag && *done_flag) return;
@@ -102,21 +132,17 @@ __global__ void pack_qfix_kernel(int M_pad, const float* __restrict__ rec, doubl
   for (int k = 0; k < TC_QFIX; ++k) b[k] = 0;
 #pragma unroll
   for (int k = 0; k < 6; ++k) split3(q[k], b[3 * k], b[3 * k + 1], b[3 * k + 2]);
-  uint4* dst = qfix + (size_t)i * 3;
+  uint4* dst = tcs + (size_t)i * 6;
+  const uint4* src = reinterpret_cast<const uint4*>(r);
+#pragma unroll
+  for (int k = 0; k < 3; ++k) dst[k] = src[k];
 #pragma unroll
   for (int k = 0; k < 3; ++k)
-    dst[k] = make_uint4(pk(b[8 * k], b[8 * k + 1]), pk(b[8 * k + 2], b[8 * k + 3]), pk(b[8 * k + 4], b[8 * k + 5]),
-                        pk(b[8 * k + 6], b[8 * k + 7]));
+    dst[3 + k] = make_uint4(pk(b[8 * k], b[8 * k + 1]), pk(b[8 * k + 2], b[8 * k + 3]), pk(b[8 * k + 4], b[8 * k + 5]),
+                            pk(b[8 * k + 6], b[8 * k + 7]));
 }
 
 struct TcSeedRegs { float4 p0, p1, p2; uint4 q0, q1, q2; };
-
-__device__ __forceinline__ void tc_load_seed(const AssignArgs& a, int i, TcSeedRegs& s) {
-  const float4* rp = reinterpret_cast<const float4*>(a.seeds) + (size_t)i * 3;
-  const uint4* qp = a.qfix + (size_t)i * 3;
-  s.p0 = __ldg(rp); s.p1 = __ldg(rp + 1); s.p2 = __ldg(rp + 2);
-  s.q0 = __ldg(qp); s.q1 = __ldg(qp + 1); s.q2 = __ldg(qp + 2);
-}
 
 // Theta row of one seed about the tile's reference point -> rows of the K-major B tile (4 pieces of 16 bytes)
 __device__ __forceinline__ void tc_build_seed(const TcSeedRegs& s, bool real, float y0x, float y0y, float y0z, float sx,
@@ -134,14 +160,19 @@ __device__ __forceinline__ void tc_build_seed(const TcSeedRegs& s, bool real, fl
     const float gx = fmaf(a13, dz, fmaf(a12, dy, 2.0f * a11 * dx)) * sx;
     const float gy = fmaf(a23, dz, fmaf(a12, dx, 2.0f * a22 * dy)) * sy;
     const float gz = fmaf(a23, dy, fmaf(a13, dx, 2.0f * a33 * dz)) * sz;
-    unsigned short xh, xm, xl, yh, ym, yl, zh, zm, zl, rh, rm, rl;
-    split3(gx, xh, xm, xl); split3(gy, yh, ym, yl); split3(gz, zh, zm, zl); split3(r0, rh, rm, rl);
-    k2 = make_uint4(s.q2.x, pk(xh, xm), pk(xl, yh), pk(ym, yl));
-    k3 = make_uint4(pk(zh, zm), pk(zl, rh), pk(rm, rl), 0u);
+    // three-way bf16 split of (gx, gy) and (gz, r0), two values per packed conversion; K order of the 12 parts:
+    // [hx hy | hz hr | mx my | mz mr | lx ly | lz lr] (Phi carries [i j | k 1] under each)
+    const uint32_t h0 = split_pair(gx, gy), h1 = split_pair(gz, r0);
+    const float ex = gx - bf_lo(h0), ey = gy - bf_hi(h0), ez = gz - bf_lo(h1), er = r0 - bf_hi(h1);
+    const uint32_t m0 = split_pair(ex, ey), m1 = split_pair(ez, er);
+    const uint32_t l0 = split_pair(ex - bf_lo(m0), ey - bf_hi(m0)), l1 = split_pair(ez - bf_lo(m1), er - bf_hi(m1));
+    k2 = make_uint4(s.q2.x, h0, h1, m0);
+    k3 = make_uint4(m1, l0, l1, 0u);
   } else {   // padding seed: constant cost 2^100, never the minimum of a chunk that holds a real seed
     k0 = k1 = make_uint4(0u, 0u, 0u, 0u);
     k2 = make_uint4(0u, 0u, 0u, 0u);
-    k3 = make_uint4(0u, 0x71800000u, 0u, 0u);   // K = 27: bf16 0x7180 = 2^100
+    k3 = make_uint4(0u, 0u, 0u, 0u);
+    k2.z = 0x71800000u;                          // K = 21 (high part of r0): bf16 0x7180 = 2^100
   }
   unsigned char* p = btile + (row >> 3) * 512 + (row & 7) * 16;
   *reinterpret_cast<uint4*>(p) = k0;
@@ -151,45 +182,44 @@ __device__ __forceinline__ void tc_build_seed(const TcSeedRegs& s, bool real, fl
 }
 
 __global__ void __launch_bounds__(TC_THREADS, 1) assign_tensor_kernel(const AssignArgs a) {
-  __shared__ __align__(128) unsigned char s_A[4 * 128 * 64];       // Phi: 4 M-tiles x 128 rows x 32 bf16
-  __shared__ __align__(128) unsigned char s_B[2][TC_N * 64];       // Theta: 2 stages x 64 rows x 32 bf16
-  __shared__ __align__(8) uint64_t s_bar[2];
+  extern __shared__ __align__(128) unsigned char tc_smem[];
+  unsigned char* s_A = tc_smem;                                    // Phi: 4 M-tiles x 128 rows x 32 bf16
+  unsigned char* s_th = tc_smem + TC_A_BYTES;                      // Theta ring: stages x 64 rows x 32 bf16
+  unsigned char* s_raw = s_th + TC_TH_STAGES * TC_TH_BYTES;        // raw seed ring: stages x 64 seeds x 96 bytes
+  __shared__ __align__(8) uint64_t s_raw_full[TC_RAW_STAGES], s_raw_empty[TC_RAW_STAGES];
+  __shared__ __align__(8) uint64_t s_th_full[TC_TH_STAGES], s_th_empty[TC_TH_STAGES];
+  __shared__ __align__(8) uint64_t s_acc_full[2], s_acc_empty[2];
   __shared__ uint32_t s_tmem;
   __shared__ double s_red[TC_THREADS / 32];
 
   if (a.done_flag && *a.done_flag) return;
-  const int tid = threadIdx.x, warp = tid >> 5;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int b = blockIdx.x;
   const int bx = b % a.g.tiles_x, by = (b / a.g.tiles_x) % a.g.tiles_y, bz = b / (a.g.tiles_x * a.g.tiles_y);
-  const bool builder = tid >= TC_EPI_THREADS;
   const int nch = a.M_pad / TC_N;
 
-  // reference voxel of the tile and the voxel sides
-  const float y0x = (float)(a.g.lo[0] + ((double)(bx * TC_TX + TC_TX / 2) + 0.5) * a.g.s[0]);
-  const float y0y = (float)(a.g.lo[1] + ((double)(by * TC_TY + TC_TY / 2) + 0.5) * a.g.s[1]);
-  const float y0z = (float)(a.g.lo[2] + ((double)(bz * TC_TZ + TC_TZ / 2) + 0.5) * a.g.s[2]);
-  const float sx = (float)a.g.s[0], sy = (float)a.g.s[1], sz = (float)a.g.s[2];
-
   if (tid == 0) {
-    mbar_init(&s_bar[0], 1);
-    mbar_init(&s_bar[1], 1);
+    for (int s = 0; s < TC_RAW_STAGES; ++s) { mbar_init(&s_raw_full[s], 1); mbar_init(&s_raw_empty[s], 2); }
+    for (int s = 0; s < TC_TH_STAGES; ++s) { mbar_init(&s_th_full[s], 2); mbar_init(&s_th_empty[s], 1); }
+    for (int s = 0; s < 2; ++s) { mbar_init(&s_acc_full[s], 1); mbar_init(&s_acc_empty[s], 16); }
     mbar_fence_init();
   }
   if (warp == 0) tc_alloc512(&s_tmem);
-
-  TcSeedRegs sr;
-  const int sid = tid - TC_EPI_THREADS;
-  if (!builder) {
+  if (tid < TC_EPI_THREADS) {
     // Phi row of this thread's voxel: monomials of the integer offsets, each under its three coefficient parts
     const int ti = (tid & 15) - TC_TX / 2, tj = ((tid >> 4) & 7) - TC_TY / 2, tk = (tid >> 7) - TC_TZ / 2;
     const float mono[10] = {(float)(ti * ti), (float)(tj * tj), (float)(tk * tk), (float)(ti * tj), (float)(ti * tk),
                             (float)(tj * tk), (float)ti, (float)tj, (float)tk, 1.0f};
     unsigned short e[32];
 #pragma unroll
-    for (int m = 0; m < 10; ++m) {
+    for (int m = 0; m < 6; ++m) {            // quadratic monomials: [hi mid lo] per monomial
       const unsigned short h = __bfloat16_as_ushort(__float2bfloat16_rn(mono[m]));
       e[3 * m] = h; e[3 * m + 1] = h; e[3 * m + 2] = h;
     }
+#pragma unroll
+    for (int r = 0; r < 3; ++r)              // linear and constant: [i j k 1] under the hi, mid and lo parts
+#pragma unroll
+      for (int m = 0; m < 4; ++m) e[18 + 4 * r + m] = __bfloat16_as_ushort(__float2bfloat16_rn(mono[6 + m]));
     e[30] = 0; e[31] = 0;
     const int mt = tid >> 7, row = tid & 127;
     unsigned char* p = s_A + mt * 8192 + (row >> 3) * 512 + (row & 7) * 16;
@@ -197,60 +227,97 @@ __global__ void __launch_bounds__(TC_THREADS, 1) assign_tensor_kernel(const Assi
     for (int kc = 0; kc < 4; ++kc)
       *reinterpret_cast<uint4*>(p + kc * 128) = make_uint4(pk(e[8 * kc], e[8 * kc + 1]), pk(e[8 * kc + 2], e[8 * kc + 3]),
                                                            pk(e[8 * kc + 4], e[8 * kc + 5]), pk(e[8 * kc + 6], e[8 * kc + 7]));
-  } else {
-    tc_load_seed(a, sid, sr);
-    tc_build_seed(sr, sid < a.M, y0x, y0y, y0z, sx, sy, sz, s_B[0], sid);
-    if (nch > 1) {
-      tc_load_seed(a, TC_N + sid, sr);
-      tc_build_seed(sr, TC_N + sid < a.M, y0x, y0y, y0z, sx, sy, sz, s_B[1], sid);
-    }
-    if (nch > 2) tc_load_seed(a, 2 * TC_N + sid, sr);
+    fence_proxy_async_smem();
   }
-  fence_proxy_async_smem();
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = s_tmem;
 
-  // instruction descriptor: D fp32, A and B bf16, both K-major, N = 64, M = 128
-  constexpr uint32_t IDESC = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(TC_N >> 3) << 17) | ((128u >> 4) << 24);
-  const uint32_t sA = smem_u32(s_A), sB = smem_u32(s_B[0]);
-  auto issue = [&](int c) {
-    const int st = c & 1;
-    tc_fence_after();
-#pragma unroll
-    for (int mt = 0; mt < 4; ++mt) {
-#pragma unroll
-      for (int ks = 0; ks < 2; ++ks) {
-        const uint64_t ad = tc_smem_desc(sA + mt * 8192 + ks * 256, 128, 512);
-        const uint64_t bd = tc_smem_desc(sB + st * (TC_N * 64) + ks * 256, 128, 512);
-        tc_mma_bf16(tmem + (uint32_t)((st * 4 + mt) * TC_N), ad, bd, IDESC, (uint32_t)ks);
-      }
-    }
-    tc_commit(&s_bar[st]);
-  };
-  if (tid == TC_EPI_THREADS) issue(0);
-
   float best = CUDART_INF_F;
   int lab = 0;
-  const uint32_t lane_addr = tmem + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)((warp >> 2) * TC_N);
 
-  for (int c = 0; c < nch; ++c) {
-    if (tid == TC_EPI_THREADS && c + 1 < nch) issue(c + 1);
-    mbar_wait(&s_bar[c & 1], (uint32_t)((c >> 1) & 1));
-    tc_fence_after();
-    if (builder) {
-      if (c + 2 < nch) {
-        tc_build_seed(sr, (c + 2) * TC_N + sid < a.M, y0x, y0y, y0z, sx, sy, sz, s_B[c & 1], sid);
-        if (c + 3 < nch) tc_load_seed(a, (c + 3) * TC_N + sid, sr);
-        fence_proxy_async_smem();
+  if (warp == 21) {
+    // ===== TMA producer: one lane keeps the raw seed ring full =====
+    if (lane == 0) {
+      const unsigned char* src = reinterpret_cast<const unsigned char*>(a.qfix);
+      for (int p = 0; p < nch; ++p) {
+        const int rs = p % TC_RAW_STAGES;
+        if (p >= TC_RAW_STAGES) mbar_wait(&s_raw_empty[rs], (uint32_t)(((p / TC_RAW_STAGES) - 1) & 1));
+        mbar_arrive_expect_tx(&s_raw_full[rs], TC_RAW_BYTES);
+        tma_bulk_g2s(s_raw + rs * TC_RAW_BYTES, src + (size_t)p * TC_RAW_BYTES, TC_RAW_BYTES, &s_raw_full[rs]);
       }
-    } else {
+    }
+  } else if (warp == 20) {
+    // ===== MMA issuer: the whole warp walks the loop (uniform control flow, descriptors in uniform registers), one
+    //       elected lane issues.  Unrolled over the 4 Theta stages so that every descriptor is base + constant. =====
+    // instruction descriptor: D fp32, A and B bf16, both K-major, N = 64, M = 128
+    constexpr uint32_t IDESC = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(TC_N >> 3) << 17) | ((128u >> 4) << 24);
+    const uint64_t ad0 = tc_smem_desc(smem_u32(s_A), 128, 512), bd0 = tc_smem_desc(smem_u32(s_th), 128, 512);
+    static_assert(TC_TH_STAGES == 4, "the issue loop is unrolled over 4 Theta stages");
+    for (int c0 = 0; c0 < nch; c0 += 4) {
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int c = c0 + u;
+        if (c < nch) {
+          const int ab = u & 1;
+          mbar_wait(&s_th_full[u], (uint32_t)((c0 >> 2) & 1));
+          if (c >= 2) mbar_wait(&s_acc_empty[ab], (uint32_t)(((c >> 1) - 1) & 1));
+          tc_fence_after();
+          if (tc_elect_one()) {
+#pragma unroll
+            for (int mt = 0; mt < 4; ++mt) {
+#pragma unroll
+              for (int ks = 0; ks < 2; ++ks)
+                tc_mma_bf16(tmem + (uint32_t)((ab * 4 + mt) * TC_N), ad0 + (uint64_t)((mt * 8192 + ks * 256) >> 4),
+                            bd0 + (uint64_t)((u * (int)TC_TH_BYTES + ks * 256) >> 4), IDESC, (uint32_t)ks);
+            }
+            tc_commit(&s_th_empty[u]);
+            tc_commit(&s_acc_full[ab]);
+          }
+          __syncwarp();
+        }
+      }
+    }
+  } else if (warp >= 16) {
+    // ===== Theta builders: one seed of the chunk per thread =====
+    const int pair = (warp - 16) >> 1, sid = ((warp - 16) & 1) * 32 + lane;
+    // reference voxel of the tile and the voxel sides
+    const float y0x = (float)(a.g.lo[0] + ((double)(bx * TC_TX + TC_TX / 2) + 0.5) * a.g.s[0]);
+    const float y0y = (float)(a.g.lo[1] + ((double)(by * TC_TY + TC_TY / 2) + 0.5) * a.g.s[1]);
+    const float y0z = (float)(a.g.lo[2] + ((double)(bz * TC_TZ + TC_TZ / 2) + 0.5) * a.g.s[2]);
+    const float sx = (float)a.g.s[0], sy = (float)a.g.s[1], sz = (float)a.g.s[2];
+    for (int c = pair; c < nch; c += TC_BUILD_WARPS / 2) {
+      const int rs = c % TC_RAW_STAGES, ts = c % TC_TH_STAGES;
+      mbar_wait(&s_raw_full[rs], (uint32_t)((c / TC_RAW_STAGES) & 1));
+      const uint4* rp = reinterpret_cast<const uint4*>(s_raw + rs * TC_RAW_BYTES) + sid * 6;
+      TcSeedRegs sr;
+      const uint4 u0 = rp[0], u1 = rp[1], u2 = rp[2];
+      sr.p0 = make_float4(__uint_as_float(u0.x), __uint_as_float(u0.y), __uint_as_float(u0.z), __uint_as_float(u0.w));
+      sr.p1 = make_float4(__uint_as_float(u1.x), __uint_as_float(u1.y), __uint_as_float(u1.z), __uint_as_float(u1.w));
+      sr.p2 = make_float4(__uint_as_float(u2.x), __uint_as_float(u2.y), __uint_as_float(u2.z), __uint_as_float(u2.w));
+      sr.q0 = rp[3]; sr.q1 = rp[4]; sr.q2 = rp[5];
+      if (c >= TC_TH_STAGES) mbar_wait(&s_th_empty[ts], (uint32_t)(((c / TC_TH_STAGES) - 1) & 1));
+      tc_build_seed(sr, c * TC_N + sid < a.M, y0x, y0y, y0z, sx, sy, sz, s_th + ts * TC_TH_BYTES, sid);
+      fence_proxy_async_smem();
+      __syncwarp();
+      if (lane == 0) { mbar_arrive(&s_th_full[ts]); mbar_arrive(&s_raw_empty[rs]); }
+    }
+  } else {
+    // ===== epilogue: warps 0-15, thread <-> voxel <-> TMEM lane =====
+    const uint32_t lane_addr = tmem + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)((warp >> 2) * TC_N);
+    for (int c = 0; c < nch; ++c) {
+      const int ab = c & 1;
+      mbar_wait(&s_acc_full[ab], (uint32_t)((c >> 1) & 1));
+      tc_fence_after();
       float va[32], vb[32];
-      const uint32_t ta = lane_addr + (uint32_t)((c & 1) * 4 * TC_N);
+      const uint32_t ta = lane_addr + (uint32_t)(ab * 4 * TC_N);
       TC_LD32(ta, va);
       TC_LD32(ta + 32, vb);
       tc_wait_ld();
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&s_acc_empty[ab]);
       float m1 = best;
 #pragma unroll
       for (int j = 0; j < 32; j += 2) m1 = min3f(m1, va[j], va[j + 1]);
@@ -272,13 +339,11 @@ __global__ void __launch_bounds__(TC_THREADS, 1) assign_tensor_kernel(const Assi
         }
       }
     }
-    tc_fence_before();
-    __syncthreads();
   }
 
   // a5 + a6: label store, warp-aggregated counts, index sums, fp64 sum of the minima
   double dsum = 0.0;
-  if (!builder) {
+  if (tid < TC_EPI_THREADS) {
     const int ix = bx * TC_TX + (tid & 15), iy = by * TC_TY + ((tid >> 4) & 7), iz = bz * TC_TZ + (tid >> 7);
     const bool valid = ix < a.g.nx && iy < a.g.ny && iz < a.g.nz;
     const unsigned vmask = __ballot_sync(0xffffffffu, valid);
@@ -286,7 +351,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) assign_tensor_kernel(const Assi
       if (a.labels) a.labels[((long long)iz * a.g.ny + iy) * a.g.nx + ix] = lab;
       dsum = (double)best;
       const unsigned peers = __match_any_sync(vmask, lab);
-      if ((int)(threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(a.count + lab, (unsigned int)__popc(peers));
+      if (lane == __ffs(peers) - 1) atomicAdd(a.count + lab, (unsigned int)__popc(peers));
       if (a.idxsum) {
         atomicAdd(a.idxsum + (size_t)lab * 3 + 0, (unsigned long long)ix);
         atomicAdd(a.idxsum + (size_t)lab * 3 + 1, (unsigned long long)iy);
@@ -312,8 +377,14 @@ cudaError_t launch_pack_qfix(const GridDev& g, int M_pad, const float* rec, uint
 }
 
 cudaError_t launch_assign_tensor(const AssignArgs& a, cudaStream_t st) {
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(assign_tensor_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
   const int n_tiles = a.g.tiles_x * a.g.tiles_y * a.g.tiles_z;
-  assign_tensor_kernel<<<n_tiles, TC_THREADS, 0, st>>>(a);
+  assign_tensor_kernel<<<n_tiles, TC_THREADS, TC_SMEM, st>>>(a);
   return cudaGetLastError();
 }
 
