@@ -99,6 +99,46 @@ __device__ __forceinline__ uint64_t tc_smem_desc(uint32_t saddr, uint32_t lbo, u
       : "r"(addr))
 __device__ __forceinline__ void tc_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
+// min(m, v[0..31]) with four independent chains of 3-input minima (16 instructions, depth 6)
+__device__ __forceinline__ float tc_min32(float m, const float (&v)[32]) {
+  float t0 = min3f(v[0], v[1], v[2]), t1 = min3f(v[3], v[4], v[5]), t2 = min3f(v[6], v[7], v[8]), t3 = min3f(v[9], v[10], v[11]);
+  t0 = min3f(t0, v[12], v[13]); t1 = min3f(t1, v[14], v[15]); t2 = min3f(t2, v[16], v[17]); t3 = min3f(t3, v[18], v[19]);
+  t0 = min3f(t0, v[20], v[21]); t1 = min3f(t1, v[22], v[23]); t2 = min3f(t2, v[24], v[25]); t3 = min3f(t3, v[26], v[27]);
+  t0 = min3f(t0, v[28], v[29]); t1 = min3f(t1, v[30], v[31]);
+  return min3f(min3f(m, t0, t1), t2, t3);
+}
+
+// a4 for 32 consecutive seeds of one voxel: running minimum; the argmin is searched (first seed attaining the new
+// minimum: lowest index on ties) only when some voxel of the warp improved
+__device__ __forceinline__ void tc_take_half(const float (&v)[32], int base, float& best, int& lab) {
+  const float m = tc_min32(best, v);
+  if (__any_sync(0xffffffffu, m < best)) {
+    if (m < best) {
+      int idx = 0;
+#pragma unroll
+      for (int j = 31; j >= 0; --j) idx = (v[j] == m) ? j : idx;
+      lab = base + idx;
+      best = m;
+    }
+  }
+}
+__device__ __forceinline__ void mbar_wait_a(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONE_%=;\n"
+      "bra WAIT_%=;\n"
+      "DONE_%=:\n"
+      "}\n" ::"r"(bar),
+      "r"(parity)
+      : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_a(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+
 // fp32 -> three bf16 whose sum carries 24 bits of v (each remainder is exact in fp32)
 __device__ __forceinline__ void split3(float v, unsigned short& h, unsigned short& m, unsigned short& l) {
   const __nv_bfloat16 bh = __float2bfloat16_rn(v);
@@ -304,40 +344,37 @@ __global__ void __launch_bounds__(TC_THREADS, 1) assign_tensor_kernel(const Assi
       if (lane == 0) { mbar_arrive(&s_th_full[ts]); mbar_arrive(&s_raw_empty[rs]); }
     }
   } else {
-    // ===== epilogue: warps 0-15, thread <-> voxel <-> TMEM lane =====
+    // ===== epilogue: warps 0-15, thread <-> voxel <-> TMEM lane.  Software-pipelined by half chunks of 32 seeds:
+    //       the tcgen05.ld of the next half is in flight while the minima of the current half are taken. =====
     const uint32_t lane_addr = tmem + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)((warp >> 2) * TC_N);
-    for (int c = 0; c < nch; ++c) {
-      const int ab = c & 1;
-      mbar_wait(&s_acc_full[ab], (uint32_t)((c >> 1) & 1));
-      tc_fence_after();
-      float va[32], vb[32];
-      const uint32_t ta = lane_addr + (uint32_t)(ab * 4 * TC_N);
-      TC_LD32(ta, va);
-      TC_LD32(ta + 32, vb);
-      tc_wait_ld();
-      tc_fence_before();
-      __syncwarp();
-      if (lane == 0) mbar_arrive(&s_acc_empty[ab]);
-      float m1 = best;
+    const bool lane0 = lane == 0;
+    const uint32_t full0 = smem_u32(&s_acc_full[0]), full1 = smem_u32(&s_acc_full[1]);
+    const uint32_t empty0 = smem_u32(&s_acc_empty[0]), empty1 = smem_u32(&s_acc_empty[1]);
+    float ra[32], rb[32];
+    uint32_t phase = 0;
+    mbar_wait_a(full0, 0u);
+    tc_fence_after();
+    TC_LD32(lane_addr, ra);
+    tc_wait_ld();
+    for (int c0 = 0; c0 < nch; c0 += 2) {      // nch is even: M_pad is a multiple of 128
 #pragma unroll
-      for (int j = 0; j < 32; j += 2) m1 = min3f(m1, va[j], va[j + 1]);
-      float m2 = m1;
-#pragma unroll
-      for (int j = 0; j < 32; j += 2) m2 = min3f(m2, vb[j], vb[j + 1]);
-      if (__any_sync(0xffffffffu, m2 < best)) {
-        if (m2 < best) {
-          int idx = 0;
-          if (m2 < m1) {
-#pragma unroll
-            for (int j = 31; j >= 0; --j) idx = (vb[j] == m2) ? 32 + j : idx;
-          } else {
-#pragma unroll
-            for (int j = 31; j >= 0; --j) idx = (va[j] == m2) ? j : idx;
-          }
-          lab = c * TC_N + idx;
-          best = m2;
+      for (int ab = 0; ab < 2; ++ab) {
+        const int c = c0 + ab;
+        TC_LD32(lane_addr + (uint32_t)(ab * 4 * TC_N + 32), rb);      // second half of chunk c
+        tc_take_half(ra, c * TC_N, best, lab);
+        tc_wait_ld();
+        tc_fence_before();
+        __syncwarp();
+        if (lane0) mbar_arrive_a(ab ? empty1 : empty0);                 // chunk c is in registers: release its buffer
+        if (c + 1 < nch) {
+          mbar_wait_a(ab ? full0 : full1, ab ? (phase ^ 1u) : phase);
+          tc_fence_after();
+          TC_LD32(lane_addr + (uint32_t)((ab ^ 1) * 4 * TC_N), ra);     // first half of chunk c + 1
         }
+        tc_take_half(rb, c * TC_N + 32, best, lab);
+        tc_wait_ld();
       }
+      phase ^= 1u;
     }
   }
 
