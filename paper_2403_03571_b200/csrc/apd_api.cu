@@ -174,7 +174,7 @@ int enqueue_evaluation(apd_ctx* ctx, const GridDev& g, int kernel, int M, const 
   if (kernel == APD_KERNEL_TENSOR) {
     if (!ws.qfix) {
       const size_t m_pad_max = ((size_t)ws.max_seeds + SEED_CHUNK - 1) / SEED_CHUNK * SEED_CHUNK;
-      APD_CUDA_TRY(ctx, cudaMalloc(&ws.qfix, (size_t)tensor_padded_seeds((int)m_pad_max) * 6 * sizeof(uint4)));
+      APD_CUDA_TRY(ctx, cudaMalloc(&ws.qfix, m_pad_max * 6 * sizeof(uint4)));
     }
     APD_CUDA_TRY(ctx, launch_pack_qfix(g, M_pad, ws.seeds, ws.qfix, done_flag, st));
   }

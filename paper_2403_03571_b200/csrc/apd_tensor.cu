@@ -5,14 +5,14 @@
 // For a voxel at INTEGER offset t = (i, j, k) from the reference voxel y0 of its tile and a seed x with matrix A,
 //     C(t) = sum_{m<=n} a'_mn s_m s_n t_m t_n  +  sum_m (g_m s_m) t_m  +  r0,
 //     g = (A + A^T)(y0 - x),   r0 = (y0 - x)^T A (y0 - x) - w,   s = voxel sides,
-// a polynomial with 10 monomials.  Phi[voxel][.] holds the monomials -- integers of magnitude <= 64, exact in bf16 --
+// a polynomial with 10 monomials.  Phi[voxel][.] holds the monomials -- integers of magnitude <= 225, exact in bf16 --
 // and Theta[seed][.] the 10 fp32 coefficients split three ways into bf16 (hi + mid + lo carries 24 bits), each
 // monomial repeated under its three parts: K = 30, padded to 32.  Every product is exact in fp32 and the tensor core
 // accumulates in fp32, so the cost carries fp32 rounding only.
 //
 // One CTA = one tile of 16 x 8 x 4 voxels = 4 UMMA M-tiles of 128 rows (one z-plane each; voxel <-> TMEM lane <->
-// thread) against chunks of 64 seeds: per half chunk 4 x 2 tcgen05.mma (M 128, N 32, K 16, kind::f16, A and B K-major
-// in shared memory without swizzle) into one of four TMEM buffers (4 x 4 x 32 = 512 columns).  Warp roles, coupled
+// thread) against chunks of 64 seeds: per chunk 4 x 2 tcgen05.mma (M 128, N 64, K 16, kind::f16, A and B K-major in
+// shared memory without swizzle), accumulators double-buffered in TMEM (2 x 4 x 64 = 512 columns).  Warp roles, coupled
 // by mbarriers only (no CTA barrier inside the seed loop):
 //   warp 21 (one lane): cp.async.bulk (TMA 1-D) of raw seed chunks into a 6-stage ring
 //   warp 20 (one lane): issues the MMAs of chunk c when Theta[c] is built and TMEM buffer c & 1 is drained;
@@ -29,19 +29,17 @@
 namespace apd {
 
 constexpr int TC_TX = 16, TC_TY = 8, TC_TZ = 4;      // voxel tile
-constexpr int TC_N = 64;                              // seeds per chunk (one Theta stage)
-constexpr int TC_NH = 32;                             // seeds per MMA group = one TMEM buffer
+constexpr int TC_N = 64;                              // seeds per chunk
 constexpr int TC_EPI_THREADS = TC_TX * TC_TY * TC_TZ; // 512: one per voxel
 constexpr int TC_BUILD_WARPS = 4;                     // two pairs; pair p expands the chunks c = p (mod 2)
 constexpr int TC_THREADS = TC_EPI_THREADS + 32 * TC_BUILD_WARPS + 64;   // + the MMA-issuing warp + the TMA warp
 constexpr int TC_QFIX = 24;                           // bf16 per seed in the tile-independent part (18 used)
 constexpr int TC_REC = 24;                            // words per seed in the TENSOR seed table: 12 fp32 + 12 x 2 bf16
-constexpr int TC_RAW_STAGES = 6, TC_TH_STAGES = 3;
-constexpr int TC_BUFS = 3;                            // TMEM accumulator buffers of 4 M-tiles x 32 columns
-constexpr int TC_ACOL = TC_BUFS * 4 * 32;             // Phi lives in TMEM behind the accumulators: 4 M-tiles x 16 columns
+constexpr int TC_RAW_STAGES = 6, TC_TH_STAGES = 4;
 constexpr uint32_t TC_RAW_BYTES = TC_N * TC_REC * 4;  // 6144 per chunk
 constexpr uint32_t TC_TH_BYTES = TC_N * 64;           // 4096 per chunk
-constexpr uint32_t TC_SMEM = TC_TH_STAGES * TC_TH_BYTES + TC_RAW_STAGES * TC_RAW_BYTES;
+constexpr uint32_t TC_A_BYTES = 4 * 128 * 64;         // 32768
+constexpr uint32_t TC_SMEM = TC_A_BYTES + TC_TH_STAGES * TC_TH_BYTES + TC_RAW_STAGES * TC_RAW_BYTES;
 
 // ---- tcgen05 wrappers ----------------------------------------------------------------------------------------
 __device__ __forceinline__ void tc_alloc512(uint32_t* slot) {
@@ -63,27 +61,6 @@ __device__ __forceinline__ void tc_mma_bf16(uint32_t d_tmem, uint64_t adesc, uin
       "}\n" ::"r"(d_tmem),
       "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
       : "memory");
-}
-// D[tmem] (+)= A[tmem] * B[smem]
-__device__ __forceinline__ void tc_mma_bf16_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t bdesc, uint32_t idesc,
-                                               uint32_t accumulate) {
-  asm volatile(
-      "{\n"
-      ".reg .pred p;\n"
-      "setp.ne.b32 p, %4, 0;\n"
-      "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n"
-      "}\n" ::"r"(d_tmem),
-      "r"(a_tmem), "l"(bdesc), "r"(idesc), "r"(accumulate)
-      : "memory");
-}
-// 16 consecutive 32-bit columns of this thread's TMEM lane
-__device__ __forceinline__ void tc_st16(uint32_t addr, const uint32_t (&v)[16]) {
-  asm volatile(
-      "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};" ::"r"(addr),
-      "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]), "r"(v[8]), "r"(v[9]), "r"(v[10]),
-      "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15])
-      : "memory");
-  asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
 }
 __device__ __forceinline__ uint32_t tc_elect_one() {
   uint32_t pred;
@@ -182,12 +159,12 @@ __device__ __forceinline__ float bf_hi(uint32_t v) { return __uint_as_float(v & 
 
 // ---- TENSOR seed table: the DIRECT record (12 fp32) followed by the tile-independent part of Theta, the six
 //      quadratic coefficients in voxel units split three ways (18 bf16, padded to 24) --------------------------------
-__global__ void pack_qfix_kernel(int M_pad, int M_tc, const float* __restrict__ rec, double sx, double sy, double sz,
+__global__ void pack_qfix_kernel(int M_pad, const float* __restrict__ rec, double sx, double sy, double sz,
                                  uint4* __restrict__ tcs, const int* __restrict__ done_flag) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= M_tc) return;
+  if (i >= M_pad) return;
   if (done_flag && *done_flag) return;
-  const float* r = rec + (size_t)min(i, M_pad - 1) * REC3;     // rows past M are padding either way (the kernel tests i < M)
+  const float* r = rec + (size_t)i * REC3;
   const float q[6] = {(float)((double)r[3] * sx * sx), (float)((double)r[6] * sy * sy), (float)((double)r[8] * sz * sz),
                       (float)((double)r[4] * sx * sy), (float)((double)r[5] * sx * sz), (float)((double)r[7] * sy * sz)};
   unsigned short b[TC_QFIX];
@@ -246,11 +223,12 @@ __device__ __forceinline__ void tc_build_seed(const TcSeedRegs& s, bool real, fl
 
 __global__ void __launch_bounds__(TC_THREADS, 1) assign_tensor_kernel(const AssignArgs a) {
   extern __shared__ __align__(128) unsigned char tc_smem[];
-  unsigned char* s_th = tc_smem;                                   // Theta ring: stages x 64 rows x 32 bf16
+  unsigned char* s_A = tc_smem;                                    // Phi: 4 M-tiles x 128 rows x 32 bf16
+  unsigned char* s_th = tc_smem + TC_A_BYTES;                      // Theta ring: stages x 64 rows x 32 bf16
   unsigned char* s_raw = s_th + TC_TH_STAGES * TC_TH_BYTES;        // raw seed ring: stages x 64 seeds x 96 bytes
   __shared__ __align__(8) uint64_t s_raw_full[TC_RAW_STAGES], s_raw_empty[TC_RAW_STAGES];
   __shared__ __align__(8) uint64_t s_th_full[TC_TH_STAGES], s_th_empty[TC_TH_STAGES];
-  __shared__ __align__(8) uint64_t s_acc_full[TC_BUFS], s_acc_empty[TC_BUFS];
+  __shared__ __align__(8) uint64_t s_acc_full[2], s_acc_empty[2];
   __shared__ uint32_t s_tmem;
   __shared__ double s_red[TC_THREADS / 32];
 
@@ -258,23 +236,23 @@ __global__ void __launch_bounds__(TC_THREADS, 1) assign_tensor_kernel(const Assi
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int b = blockIdx.x;
   const int bx = b % a.g.tiles_x, by = (b / a.g.tiles_x) % a.g.tiles_y, bz = b / (a.g.tiles_x * a.g.tiles_y);
-  const int nch = ((a.M_pad + 3 * TC_N - 1) / (3 * TC_N)) * 3;     // chunks of 64 seeds, a multiple of 3
+  const int nch = a.M_pad / TC_N;
+  // reference voxel of the tile: the middle of its part inside the grid (a tile cut by the boundary must not expand
+  // the costs about a point outside the domain: that would cost precision on narrow grids).  Offsets stay within
+  // [-8, 15]: squares and products <= 225, exact in bf16.
+  const int rx = min(TC_TX, a.g.nx - bx * TC_TX) / 2, ry = min(TC_TY, a.g.ny - by * TC_TY) / 2,
+            rz = min(TC_TZ, a.g.nz - bz * TC_TZ) / 2;
 
   if (tid == 0) {
     for (int s = 0; s < TC_RAW_STAGES; ++s) { mbar_init(&s_raw_full[s], 1); mbar_init(&s_raw_empty[s], 2); }
     for (int s = 0; s < TC_TH_STAGES; ++s) { mbar_init(&s_th_full[s], 2); mbar_init(&s_th_empty[s], 1); }
-    for (int s = 0; s < TC_BUFS; ++s) { mbar_init(&s_acc_full[s], 1); mbar_init(&s_acc_empty[s], 16); }
+    for (int s = 0; s < 2; ++s) { mbar_init(&s_acc_full[s], 1); mbar_init(&s_acc_empty[s], 16); }
     mbar_fence_init();
   }
   if (warp == 0) tc_alloc512(&s_tmem);
-  tc_fence_before();
-  __syncthreads();
-  tc_fence_after();
-  const uint32_t tmem = s_tmem;
   if (tid < TC_EPI_THREADS) {
-    // Phi row of this thread's voxel, written once into TMEM (the A operand of every MMA): monomials of the integer
-    // offsets, each under its coefficient parts; 32 bf16 = 16 columns of this thread's lane
-    const int ti = (tid & 15) - TC_TX / 2, tj = ((tid >> 4) & 7) - TC_TY / 2, tk = (tid >> 7) - TC_TZ / 2;
+    // Phi row of this thread's voxel: monomials of the integer offsets, each under its three coefficient parts
+    const int ti = (tid & 15) - rx, tj = ((tid >> 4) & 7) - ry, tk = (tid >> 7) - rz;
     const float mono[10] = {(float)(ti * ti), (float)(tj * tj), (float)(tk * tk), (float)(ti * tj), (float)(ti * tk),
                             (float)(tj * tk), (float)ti, (float)tj, (float)tk, 1.0f};
     unsigned short e[32];
@@ -288,14 +266,18 @@ __global__ void __launch_bounds__(TC_THREADS, 1) assign_tensor_kernel(const Assi
 #pragma unroll
       for (int m = 0; m < 4; ++m) e[18 + 4 * r + m] = __bfloat16_as_ushort(__float2bfloat16_rn(mono[6 + m]));
     e[30] = 0; e[31] = 0;
-    uint32_t pw[16];
+    const int mt = tid >> 7, row = tid & 127;
+    unsigned char* p = s_A + mt * 8192 + (row >> 3) * 512 + (row & 7) * 16;
 #pragma unroll
-    for (int j = 0; j < 16; ++j) pw[j] = pk(e[2 * j], e[2 * j + 1]);
-    tc_st16(tmem + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)(TC_ACOL + (warp >> 2) * 16), pw);
+    for (int kc = 0; kc < 4; ++kc)
+      *reinterpret_cast<uint4*>(p + kc * 128) = make_uint4(pk(e[8 * kc], e[8 * kc + 1]), pk(e[8 * kc + 2], e[8 * kc + 3]),
+                                                           pk(e[8 * kc + 4], e[8 * kc + 5]), pk(e[8 * kc + 6], e[8 * kc + 7]));
+    fence_proxy_async_smem();
   }
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
+  const uint32_t tmem = s_tmem;
 
   float best = CUDART_INF_F;
   int lab = 0;
@@ -312,46 +294,43 @@ __global__ void __launch_bounds__(TC_THREADS, 1) assign_tensor_kernel(const Assi
       }
     }
   } else if (warp == 20) {
-    // ===== MMA issuer: the whole warp walks the loop (uniform control flow), one elected lane issues.  Unrolled
-    //       over the 3 Theta stages = 6 half chunks = 2 uses of each TMEM buffer, so every index is a constant. =====
-    // instruction descriptor: D fp32, A and B bf16, both K-major, N = 32, M = 128
-    constexpr uint32_t IDESC = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(TC_NH >> 3) << 17) | ((128u >> 4) << 24);
-    const uint64_t bd0 = tc_smem_desc(smem_u32(s_th), 128, 512);
-    static_assert(TC_TH_STAGES == 3 && TC_BUFS == 3, "the issue loop is unrolled over 3 Theta stages / 3 buffers");
-    uint32_t phase = 0;
-    for (int c0 = 0; c0 < nch; c0 += 3) {
+    // ===== MMA issuer: the whole warp walks the loop (uniform control flow, descriptors in uniform registers), one
+    //       elected lane issues.  Unrolled over the 4 Theta stages so that every descriptor is base + constant. =====
+    // instruction descriptor: D fp32, A and B bf16, both K-major, N = 64, M = 128
+    constexpr uint32_t IDESC = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(TC_N >> 3) << 17) | ((128u >> 4) << 24);
+    const uint64_t ad0 = tc_smem_desc(smem_u32(s_A), 128, 512), bd0 = tc_smem_desc(smem_u32(s_th), 128, 512);
+    static_assert(TC_TH_STAGES == 4, "the issue loop is unrolled over 4 Theta stages");
+    for (int c0 = 0; c0 < nch; c0 += 4) {
 #pragma unroll
-      for (int u = 0; u < 3; ++u) {
-        mbar_wait(&s_th_full[u], phase);
-#pragma unroll
-        for (int h = 0; h < 2; ++h) {                 // half chunk j of this group -> TMEM buffer j % 3
-          const int j = 2 * u + h, buf = j % 3;
-          if (c0 > 0 || j >= 3) mbar_wait(&s_acc_empty[buf], j >= 3 ? 0u : 1u);
+      for (int u = 0; u < 4; ++u) {
+        const int c = c0 + u;
+        if (c < nch) {
+          const int ab = u & 1;
+          mbar_wait(&s_th_full[u], (uint32_t)((c0 >> 2) & 1));
+          if (c >= 2) mbar_wait(&s_acc_empty[ab], (uint32_t)(((c >> 1) - 1) & 1));
           tc_fence_after();
           if (tc_elect_one()) {
 #pragma unroll
             for (int mt = 0; mt < 4; ++mt) {
 #pragma unroll
               for (int ks = 0; ks < 2; ++ks)
-                tc_mma_bf16_ts(tmem + (uint32_t)((buf * 4 + mt) * TC_NH), tmem + (uint32_t)(TC_ACOL + mt * 16 + ks * 8),
-                               bd0 + (uint64_t)((u * (int)TC_TH_BYTES + h * (TC_NH / 8) * 512 + ks * 256) >> 4), IDESC,
-                               (uint32_t)ks);
+                tc_mma_bf16(tmem + (uint32_t)((ab * 4 + mt) * TC_N), ad0 + (uint64_t)((mt * 8192 + ks * 256) >> 4),
+                            bd0 + (uint64_t)((u * (int)TC_TH_BYTES + ks * 256) >> 4), IDESC, (uint32_t)ks);
             }
-            if (h == 1) tc_commit(&s_th_empty[u]);
-            tc_commit(&s_acc_full[buf]);
+            tc_commit(&s_th_empty[u]);
+            tc_commit(&s_acc_full[ab]);
           }
           __syncwarp();
         }
       }
-      phase ^= 1u;
     }
   } else if (warp >= 16) {
     // ===== Theta builders: one seed of the chunk per thread =====
     const int pair = (warp - 16) >> 1, sid = ((warp - 16) & 1) * 32 + lane;
     // reference voxel of the tile and the voxel sides
-    const float y0x = (float)(a.g.lo[0] + ((double)(bx * TC_TX + TC_TX / 2) + 0.5) * a.g.s[0]);
-    const float y0y = (float)(a.g.lo[1] + ((double)(by * TC_TY + TC_TY / 2) + 0.5) * a.g.s[1]);
-    const float y0z = (float)(a.g.lo[2] + ((double)(bz * TC_TZ + TC_TZ / 2) + 0.5) * a.g.s[2]);
+    const float y0x = (float)(a.g.lo[0] + ((double)(bx * TC_TX + rx) + 0.5) * a.g.s[0]);
+    const float y0y = (float)(a.g.lo[1] + ((double)(by * TC_TY + ry) + 0.5) * a.g.s[1]);
+    const float y0z = (float)(a.g.lo[2] + ((double)(bz * TC_TZ + rz) + 0.5) * a.g.s[2]);
     const float sx = (float)a.g.s[0], sy = (float)a.g.s[1], sz = (float)a.g.s[2];
     for (int c = pair; c < nch; c += TC_BUILD_WARPS / 2) {
       const int rs = c % TC_RAW_STAGES, ts = c % TC_TH_STAGES;
@@ -370,43 +349,37 @@ __global__ void __launch_bounds__(TC_THREADS, 1) assign_tensor_kernel(const Assi
       if (lane == 0) { mbar_arrive(&s_th_full[ts]); mbar_arrive(&s_raw_empty[rs]); }
     }
   } else {
-    // ===== epilogue: warps 0-15, thread <-> voxel <-> TMEM lane.  One TMEM buffer = 32 seeds; software-pipelined:
-    //       the tcgen05.ld of the next buffer is in flight while the minima of the current one are taken.  Unrolled
-    //       over 6 half chunks = 2 uses of each of the 3 buffers. =====
-    uint32_t lane_addr = tmem + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)((warp >> 2) * TC_NH);
-    uint32_t full0 = smem_u32(&s_acc_full[0]), empty0 = smem_u32(&s_acc_empty[0]);
-    // opaque to the compiler: otherwise it re-derives these from %tid / %cluster_ctaid in every half chunk
-    asm volatile("" : "+r"(lane_addr), "+r"(full0), "+r"(empty0));
+    // ===== epilogue: warps 0-15, thread <-> voxel <-> TMEM lane.  Software-pipelined by half chunks of 32 seeds:
+    //       the tcgen05.ld of the next half is in flight while the minima of the current half are taken. =====
+    const uint32_t lane_addr = tmem + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)((warp >> 2) * TC_N);
     const bool lane0 = lane == 0;
+    const uint32_t full0 = smem_u32(&s_acc_full[0]), full1 = smem_u32(&s_acc_full[1]);
+    const uint32_t empty0 = smem_u32(&s_acc_empty[0]), empty1 = smem_u32(&s_acc_empty[1]);
     float ra[32], rb[32];
-    const int nq = 2 * nch;                    // a multiple of 6
+    uint32_t phase = 0;
     mbar_wait_a(full0, 0u);
     tc_fence_after();
     TC_LD32(lane_addr, ra);
     tc_wait_ld();
-    tc_fence_before();
-    __syncwarp();
-    if (lane0) mbar_arrive_a(empty0);
-    for (int q0 = 0; q0 < nq; q0 += 6) {
+    for (int c0 = 0; c0 < nch; c0 += 2) {      // nch is even: M_pad is a multiple of 128
 #pragma unroll
-      for (int j = 0; j < 6; ++j) {
-        const int jn = (j + 1) % 6, nb = jn % 3;          // the next half chunk and its buffer
-        const bool more = q0 + j + 1 < nq;
-        if (more) {
-          mbar_wait_a(full0 + 8u * nb, jn >= 3 ? 1u : 0u);
+      for (int ab = 0; ab < 2; ++ab) {
+        const int c = c0 + ab;
+        TC_LD32(lane_addr + (uint32_t)(ab * 4 * TC_N + 32), rb);      // second half of chunk c
+        tc_take_half(ra, c * TC_N, best, lab);
+        tc_wait_ld();
+        tc_fence_before();
+        __syncwarp();
+        if (lane0) mbar_arrive_a(ab ? empty1 : empty0);                 // chunk c is in registers: release its buffer
+        if (c + 1 < nch) {
+          mbar_wait_a(ab ? full0 : full1, ab ? (phase ^ 1u) : phase);
           tc_fence_after();
-          if (j & 1) TC_LD32(lane_addr + (uint32_t)(nb * 4 * TC_NH), ra);
-          else       TC_LD32(lane_addr + (uint32_t)(nb * 4 * TC_NH), rb);
+          TC_LD32(lane_addr + (uint32_t)((ab ^ 1) * 4 * TC_N), ra);     // first half of chunk c + 1
         }
-        if (j & 1) tc_take_half(rb, (q0 + j) * TC_NH, best, lab);
-        else       tc_take_half(ra, (q0 + j) * TC_NH, best, lab);
-        if (more) {
-          tc_wait_ld();
-          tc_fence_before();
-          __syncwarp();
-          if (tc_elect_one()) mbar_arrive_a(empty0 + 8u * nb);      // the buffer is in registers: release it
-        }
+        tc_take_half(rb, c * TC_N + 32, best, lab);
+        tc_wait_ld();
       }
+      phase ^= 1u;
     }
   }
 
@@ -439,12 +412,9 @@ void tensor_tile_counts(int nx, int ny, int nz, int* tx, int* ty, int* tz) {
   *tx = (nx + TC_TX - 1) / TC_TX; *ty = (ny + TC_TY - 1) / TC_TY; *tz = (nz + TC_TZ - 1) / TC_TZ;
 }
 
-int tensor_padded_seeds(int M) { return (M + 3 * TC_N - 1) / (3 * TC_N) * (3 * TC_N); }
-
 cudaError_t launch_pack_qfix(const GridDev& g, int M_pad, const float* rec, uint4* qfix, const int* done_flag,
                              cudaStream_t st) {
-  const int M_tc = (M_pad + 3 * TC_N - 1) / (3 * TC_N) * (3 * TC_N);
-  pack_qfix_kernel<<<(M_tc + 127) / 128, 128, 0, st>>>(M_pad, M_tc, rec, g.s[0], g.s[1], g.s[2], qfix, done_flag);
+  pack_qfix_kernel<<<(M_pad + 127) / 128, 128, 0, st>>>(M_pad, rec, g.s[0], g.s[1], g.s[2], qfix, done_flag);
   return cudaGetLastError();
 }
 
