@@ -184,7 +184,11 @@ def run_reference(args):
 #   DIRECT  : 3 FADD + 3 FMUL + 6 FFMA               = 18 flop   (12 FP32 instructions, 3D)
 #   ROWPOLY : 1.5 FMA (voxels at +-tau share the even part) + 7 FMA set-up per (row of 32 voxels, seed)
 #             = 3 + 14/32 = 3.4375 flop (the once-per-(tile, seed) re-expansion, ~25 flop / 4096 voxels, not counted)
-FLOP_PER_PAIR = {1: 18.0, 2: 3.0 + 14.0 / 32.0}
+#   TENSOR  : the K = 32 bf16 contraction of the lifted form = 64 tensor-core flop per pair (30 of the 32 K slots carry
+#             a product); reported against the MEASURED bf16 peak, bound "tensor" -- its real limit is the CUDA-core
+#             argmin epilogue
+FLOP_PER_PAIR = {1: 18.0, 2: 3.0 + 14.0 / 32.0, 3: 64.0}
+KERNEL_NAME = {1: "assign_direct_kernel<3>", 2: "assign_rowpoly_kernel<3>", 3: "assign_tensor_kernel"}
 FP32_LANES_PER_SM = 128
 # dram__bytes_read.sum + dram__bytes_write.sum of one assign_rowpoly_kernel launch on this workload, from the
 # `ncu --set full` capture summarised in profiles/ (None until a capture exists)
@@ -291,9 +295,11 @@ def run_ours(args):
         sm_max_mhz = float(peaks.get("sm_max_mhz", 1965.0))
         peak_tflops = sm_count * FP32_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
         ach = FLOP_PER_PAIR[kernel_id] * wl.pairs / (kernel_ms * 1e-3) / 1e12
-        roofline = {"bound": "alu", "kernel": "assign_rowpoly_kernel<3>" if kernel_id == 2 else "assign_direct_kernel<3>",
-                    "achieved": ach, "peak": peak_tflops, "unit": "TFLOP/s", "frac": ach / peak_tflops,
-                    "traffic": NCU_TRAFFIC_BYTES, "kernel_ms": kernel_ms,
+        bf16_peak = float(peaks.get("bf16_tflops", 1662.1))
+        roofline = {"bound": "tensor" if kernel_id == 3 else "alu", "kernel": KERNEL_NAME[kernel_id],
+                    "achieved": ach, "peak": bf16_peak if kernel_id == 3 else peak_tflops, "unit": "TFLOP/s",
+                    "frac": ach / (bf16_peak if kernel_id == 3 else peak_tflops),
+                    "traffic": NCU_TRAFFIC_BYTES if kernel_id == 2 else None, "kernel_ms": kernel_ms,
                     "flop_per_pair": FLOP_PER_PAIR[kernel_id],
                     "peak_is": f"{sm_count} SMs x {FP32_LANES_PER_SM} FP32 lanes x 2 flop x {sm_max_mhz:.0f} MHz "
                                "(guide unit counts and MEASURED_PEAKS.json sm_max_mhz; no FP32 figure is measured there)",
@@ -323,6 +329,24 @@ def run_ours(args):
             extra["roofline_direct"] = {"bound": "alu", "kernel": "assign_direct_kernel<3>", "achieved": dach,
                                         "peak": peak_tflops, "unit": "TFLOP/s", "frac": dach / peak_tflops,
                                         "kernel_ms": dm, "gpairs": wl.pairs / (dm * 1e-3) / 1e9, "flop_per_pair": 18.0}
+        if not args.no_direct and kernel_id != 3:
+            # row a8: the tensor-core lift of the cost matrix (opts.kernel = APD_KERNEL_TENSOR), same workload
+            o3 = apd.make_opts(kernel=apd.KERNEL_TENSOR)
+            t_ms = []
+            for _ in range(4):
+                flush.zero_()
+                ctx.apd_assign(grid, X, A, w, target_vol=v, labels=labels, vol=vol, dual=dual, max_rel_err=err, opts=o3)
+                torch.cuda.synchronize()
+                t_ms.append(ctx.last_kernel_ms())
+            tm = float(np.mean(t_ms[1:]))
+            tach = FLOP_PER_PAIR[3] * wl.pairs / (tm * 1e-3) / 1e12
+            extra["roofline_tensor"] = {"bound": "tensor", "kernel": "assign_tensor_kernel", "achieved": tach,
+                                        "peak": bf16_peak, "unit": "TFLOP/s", "frac": tach / bf16_peak, "kernel_ms": tm,
+                                        "gpairs": wl.pairs / (tm * 1e-3) / 1e9, "flop_per_pair": 64.0,
+                                        "peak_is": "MEASURED_PEAKS.json bf16_tflops (burst, cuBLAS 8192^3)",
+                                        "note": "K = 32 contraction per pair; the kernel is paced by its CUDA-core argmin "
+                                                "epilogue (one 3-input min per 2 pairs on the half-rate ALU pipe), not by "
+                                                "the tensor pipe (DESIGN.md 9)"}
         if not args.no_solve:
             pairs_t = torch.zeros(1, dtype=torch.int64, device=dev)
             oc = apd.make_opts(kernel=args.kernel, cull=1)
@@ -387,8 +411,11 @@ def run_ours(args):
                         "d2h_bytes_per_step": d2h, "ms_per_step": e2e_s * 1e3, "ms_per_step_max": max(e2e_each) * 1e3,
                         "steps": e2e_steps,
                         "call": "apd_assign_host (pinned host buffers; H2D/D2H copies inside, device scratch kept by the context)"},
-                "gpu_launches": 3 * args.steps, "launches_per_step": ["pack_pairs_kernel", "assign_rowpoly_kernel",
-                                                                      "finalize_kernel"]}
+                "gpu_launches": (4 if kernel_id == 3 else 3) * args.steps,
+                "launches_per_step": {1: ["pack_seeds_kernel", "assign_direct_kernel", "finalize_kernel"],
+                                      2: ["pack_pairs_kernel", "assign_rowpoly_kernel", "finalize_kernel"],
+                                      3: ["pack_seeds_kernel", "pack_qfix_kernel", "assign_tensor_kernel",
+                                          "finalize_kernel"]}[kernel_id]}
         line.update(extra)
     if world > 1:
         dist.barrier()
@@ -457,7 +484,7 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
-    ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 DIRECT, 2 ROWPOLY")
+    ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 DIRECT, 2 ROWPOLY, 3 TENSOR")
     ap.add_argument("--no-solve", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-probe", action="store_true")
