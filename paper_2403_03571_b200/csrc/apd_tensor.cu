@@ -11,14 +11,15 @@
 // accumulates in fp32, so the cost carries fp32 rounding only.
 //
 // One CTA = one tile of 16 x 8 x 4 voxels = 4 UMMA M-tiles of 128 rows (one z-plane each; voxel <-> TMEM lane <->
-// thread) against chunks of 64 seeds: per chunk 4 x 2 tcgen05.mma (M 128, N 64, K 16, kind::f16, A and B K-major in
-// shared memory without swizzle), accumulators double-buffered in TMEM (2 x 4 x 64 = 512 columns).  Warp roles, coupled
+// thread) against chunks of 128 seeds: per chunk 4 x 2 tcgen05.mma (M 128, N 128, K 16, kind::f16, A and B K-major in
+// shared memory without swizzle), one accumulator region of 128 TMEM columns per M-tile (4 x 128 = 512 columns): the
+// tensor core works on the other three M-tiles while one is drained.  Warp roles, coupled
 // by mbarriers only (no CTA barrier inside the seed loop):
-//   warp 21 (one lane): cp.async.bulk (TMA 1-D) of raw seed chunks into a 6-stage ring
-//   warp 20 (one lane): issues the MMAs of chunk c when Theta[c] is built and TMEM buffer c & 1 is drained;
-//                       tcgen05.commit signals both consumers
-//   warps 16-19:        two pairs; a pair expands the coefficients of every other chunk about this tile's y0 (one seed
-//                       per thread) into the Theta ring
+//   warp 21 (one lane): cp.async.bulk (TMA 1-D) of raw seed chunks into a 4-stage ring
+//   warp 20:            issues the MMAs of (chunk c, M-tile mt) when Theta[c] is built and the region of mt is drained
+//                       (one elected lane); tcgen05.commit signals both consumers
+//   warps 16-19:        expand the coefficients of a chunk about this tile's y0 (one seed per thread) into the Theta
+//                       ring
 //   warps 0-15:         drain chunk c from TMEM (tcgen05.ld 32x32b), release the buffer, 3-input min; the argmin is
 //                       found by a rescan of the registers only when some voxel's minimum dropped.
 #include "apd_internal.cuh"
@@ -29,13 +30,14 @@
 namespace apd {
 
 constexpr int TC_TX = 16, TC_TY = 8, TC_TZ = 4;      // voxel tile
-constexpr int TC_N = 64;                              // seeds per chunk
+constexpr int TC_N = 128;                             // seeds per chunk = N of one tcgen05.mma (N >= 128: below that an
+                                                      // MMA costs ~45 cycles whatever its N -- measured)
 constexpr int TC_EPI_THREADS = TC_TX * TC_TY * TC_TZ; // 512: one per voxel
-constexpr int TC_BUILD_WARPS = 4;                     // two pairs; pair p expands the chunks c = p (mod 2)
+constexpr int TC_BUILD_WARPS = 4;                     // 128 threads: one seed of every chunk each
 constexpr int TC_THREADS = TC_EPI_THREADS + 32 * TC_BUILD_WARPS + 64;   // + the MMA-issuing warp + the TMA warp
 constexpr int TC_QFIX = 24;                           // bf16 per seed in the tile-independent part (18 used)
 constexpr int TC_REC = 24;                            // words per seed in the TENSOR seed table: 12 fp32 + 12 x 2 bf16
-constexpr int TC_RAW_STAGES = 6, TC_TH_STAGES = 4;
+constexpr int TC_RAW_STAGES = 4, TC_TH_STAGES = 4;
 constexpr uint32_t TC_RAW_BYTES = TC_N * TC_REC * 4;  // 6144 per chunk
 constexpr uint32_t TC_TH_BYTES = TC_N * 64;           // 4096 per chunk
 constexpr uint32_t TC_A_BYTES = 4 * 128 * 64;         // 32768
@@ -228,7 +230,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) assign_tensor_kernel(const Assi
   unsigned char* s_raw = s_th + TC_TH_STAGES * TC_TH_BYTES;        // raw seed ring: stages x 64 seeds x 96 bytes
   __shared__ __align__(8) uint64_t s_raw_full[TC_RAW_STAGES], s_raw_empty[TC_RAW_STAGES];
   __shared__ __align__(8) uint64_t s_th_full[TC_TH_STAGES], s_th_empty[TC_TH_STAGES];
-  __shared__ __align__(8) uint64_t s_acc_full[2], s_acc_empty[2];
+  __shared__ __align__(8) uint64_t s_acc_full[4], s_acc_empty[4];      // one accumulator region per M-tile
   __shared__ uint32_t s_tmem;
   __shared__ double s_red[TC_THREADS / 32];
 
@@ -244,9 +246,9 @@ __global__ void __launch_bounds__(TC_THREADS, 1) assign_tensor_kernel(const Assi
             rz = min(TC_TZ, a.g.nz - bz * TC_TZ) / 2;
 
   if (tid == 0) {
-    for (int s = 0; s < TC_RAW_STAGES; ++s) { mbar_init(&s_raw_full[s], 1); mbar_init(&s_raw_empty[s], 2); }
-    for (int s = 0; s < TC_TH_STAGES; ++s) { mbar_init(&s_th_full[s], 2); mbar_init(&s_th_empty[s], 1); }
-    for (int s = 0; s < 2; ++s) { mbar_init(&s_acc_full[s], 1); mbar_init(&s_acc_empty[s], 16); }
+    for (int s = 0; s < TC_RAW_STAGES; ++s) { mbar_init(&s_raw_full[s], 1); mbar_init(&s_raw_empty[s], TC_BUILD_WARPS); }
+    for (int s = 0; s < TC_TH_STAGES; ++s) { mbar_init(&s_th_full[s], TC_BUILD_WARPS); mbar_init(&s_th_empty[s], 1); }
+    for (int s = 0; s < 4; ++s) { mbar_init(&s_acc_full[s], 1); mbar_init(&s_acc_empty[s], 4); }
     mbar_fence_init();
   }
   if (warp == 0) tc_alloc512(&s_tmem);
@@ -305,34 +307,33 @@ __global__ void __launch_bounds__(TC_THREADS, 1) assign_tensor_kernel(const Assi
       for (int u = 0; u < 4; ++u) {
         const int c = c0 + u;
         if (c < nch) {
-          const int ab = u & 1;
           mbar_wait(&s_th_full[u], (uint32_t)((c0 >> 2) & 1));
-          if (c >= 2) mbar_wait(&s_acc_empty[ab], (uint32_t)(((c >> 1) - 1) & 1));
-          tc_fence_after();
-          if (tc_elect_one()) {
 #pragma unroll
-            for (int mt = 0; mt < 4; ++mt) {
+          for (int mt = 0; mt < 4; ++mt) {      // M-tile mt accumulates into its own region of 128 columns
+            if (c > 0) mbar_wait(&s_acc_empty[mt], (uint32_t)((c - 1) & 1));
+            tc_fence_after();
+            if (tc_elect_one()) {
 #pragma unroll
               for (int ks = 0; ks < 2; ++ks)
-                tc_mma_bf16(tmem + (uint32_t)((ab * 4 + mt) * TC_N), ad0 + (uint64_t)((mt * 8192 + ks * 256) >> 4),
+                tc_mma_bf16(tmem + (uint32_t)(mt * TC_N), ad0 + (uint64_t)((mt * 8192 + ks * 256) >> 4),
                             bd0 + (uint64_t)((u * (int)TC_TH_BYTES + ks * 256) >> 4), IDESC, (uint32_t)ks);
+              if (mt == 3) tc_commit(&s_th_empty[u]);
+              tc_commit(&s_acc_full[mt]);
             }
-            tc_commit(&s_th_empty[u]);
-            tc_commit(&s_acc_full[ab]);
+            __syncwarp();
           }
-          __syncwarp();
         }
       }
     }
   } else if (warp >= 16) {
     // ===== Theta builders: one seed of the chunk per thread =====
-    const int pair = (warp - 16) >> 1, sid = ((warp - 16) & 1) * 32 + lane;
+    const int sid = tid - TC_EPI_THREADS;
     // reference voxel of the tile and the voxel sides
     const float y0x = (float)(a.g.lo[0] + ((double)(bx * TC_TX + rx) + 0.5) * a.g.s[0]);
     const float y0y = (float)(a.g.lo[1] + ((double)(by * TC_TY + ry) + 0.5) * a.g.s[1]);
     const float y0z = (float)(a.g.lo[2] + ((double)(bz * TC_TZ + rz) + 0.5) * a.g.s[2]);
     const float sx = (float)a.g.s[0], sy = (float)a.g.s[1], sz = (float)a.g.s[2];
-    for (int c = pair; c < nch; c += TC_BUILD_WARPS / 2) {
+    for (int c = 0; c < nch; ++c) {
       const int rs = c % TC_RAW_STAGES, ts = c % TC_TH_STAGES;
       mbar_wait(&s_raw_full[rs], (uint32_t)((c / TC_RAW_STAGES) & 1));
       const uint4* rp = reinterpret_cast<const uint4*>(s_raw + rs * TC_RAW_BYTES) + sid * 6;
@@ -349,37 +350,32 @@ __global__ void __launch_bounds__(TC_THREADS, 1) assign_tensor_kernel(const Assi
       if (lane == 0) { mbar_arrive(&s_th_full[ts]); mbar_arrive(&s_raw_empty[rs]); }
     }
   } else {
-    // ===== epilogue: warps 0-15, thread <-> voxel <-> TMEM lane.  Software-pipelined by half chunks of 32 seeds:
-    //       the tcgen05.ld of the next half is in flight while the minima of the current half are taken. =====
-    const uint32_t lane_addr = tmem + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)((warp >> 2) * TC_N);
-    const bool lane0 = lane == 0;
-    const uint32_t full0 = smem_u32(&s_acc_full[0]), full1 = smem_u32(&s_acc_full[1]);
-    const uint32_t empty0 = smem_u32(&s_acc_empty[0]), empty1 = smem_u32(&s_acc_empty[1]);
+    // ===== epilogue: warps 0-15, thread <-> voxel <-> TMEM lane; M-tile mt = warp / 4 drains its own region of 128
+    //       columns in 4 groups of 32 seeds, software-pipelined (the tcgen05.ld of the next group is in flight while
+    //       the minima of the current one are taken); the region is released as soon as it is in registers. =====
+    const int mt = warp >> 2;
+    uint32_t lane_addr = tmem + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)(mt * TC_N);
+    uint32_t full = smem_u32(&s_acc_full[mt]), empty = smem_u32(&s_acc_empty[mt]);
+    asm volatile("" : "+r"(lane_addr), "+r"(full), "+r"(empty));     // keep them in registers (no re-derivation per chunk)
     float ra[32], rb[32];
-    uint32_t phase = 0;
-    mbar_wait_a(full0, 0u);
-    tc_fence_after();
-    TC_LD32(lane_addr, ra);
-    tc_wait_ld();
-    for (int c0 = 0; c0 < nch; c0 += 2) {      // nch is even: M_pad is a multiple of 128
-#pragma unroll
-      for (int ab = 0; ab < 2; ++ab) {
-        const int c = c0 + ab;
-        TC_LD32(lane_addr + (uint32_t)(ab * 4 * TC_N + 32), rb);      // second half of chunk c
-        tc_take_half(ra, c * TC_N, best, lab);
-        tc_wait_ld();
-        tc_fence_before();
-        __syncwarp();
-        if (lane0) mbar_arrive_a(ab ? empty1 : empty0);                 // chunk c is in registers: release its buffer
-        if (c + 1 < nch) {
-          mbar_wait_a(ab ? full0 : full1, ab ? (phase ^ 1u) : phase);
-          tc_fence_after();
-          TC_LD32(lane_addr + (uint32_t)((ab ^ 1) * 4 * TC_N), ra);     // first half of chunk c + 1
-        }
-        tc_take_half(rb, c * TC_N + 32, best, lab);
-        tc_wait_ld();
-      }
-      phase ^= 1u;
+    for (int c = 0; c < nch; ++c) {
+      mbar_wait_a(full, (uint32_t)(c & 1));
+      tc_fence_after();
+      TC_LD32(lane_addr, ra);
+      tc_wait_ld();
+      TC_LD32(lane_addr + 32, rb);
+      tc_take_half(ra, c * TC_N, best, lab);
+      tc_wait_ld();
+      TC_LD32(lane_addr + 64, ra);
+      tc_take_half(rb, c * TC_N + 32, best, lab);
+      tc_wait_ld();
+      TC_LD32(lane_addr + 96, rb);
+      tc_take_half(ra, c * TC_N + 64, best, lab);
+      tc_wait_ld();
+      tc_fence_before();
+      __syncwarp();
+      if (tc_elect_one()) mbar_arrive_a(empty);                       // the region is in registers: release it
+      tc_take_half(rb, c * TC_N + 96, best, lab);
     }
   }
 
