@@ -301,8 +301,9 @@ def run_ours(args):
                     "frac": ach / (bf16_peak if kernel_id == 3 else peak_tflops),
                     "traffic": NCU_TRAFFIC_BYTES if kernel_id == 2 else None, "kernel_ms": kernel_ms,
                     "flop_per_pair": FLOP_PER_PAIR[kernel_id],
-                    "peak_is": f"{sm_count} SMs x {FP32_LANES_PER_SM} FP32 lanes x 2 flop x {sm_max_mhz:.0f} MHz "
-                               "(guide unit counts and MEASURED_PEAKS.json sm_max_mhz; no FP32 figure is measured there)",
+                    "peak_is": ("MEASURED_PEAKS.json bf16_tflops (burst, cuBLAS 8192^3)" if kernel_id == 3 else
+                                f"{sm_count} SMs x {FP32_LANES_PER_SM} FP32 lanes x 2 flop x {sm_max_mhz:.0f} MHz "
+                                "(guide unit counts and MEASURED_PEAKS.json sm_max_mhz; no FP32 figure is measured there)"),
                     "label_write_GBps": 4.0 * wl.N / (kernel_ms * 1e-3) / 1e9}
         extra = {}
         if not args.no_probe:
@@ -344,9 +345,9 @@ def run_ours(args):
                                         "peak": bf16_peak, "unit": "TFLOP/s", "frac": tach / bf16_peak, "kernel_ms": tm,
                                         "gpairs": wl.pairs / (tm * 1e-3) / 1e9, "flop_per_pair": 64.0,
                                         "peak_is": "MEASURED_PEAKS.json bf16_tflops (burst, cuBLAS 8192^3)",
-                                        "note": "K = 32 contraction per pair; the kernel is paced by its CUDA-core argmin "
-                                                "epilogue (one 3-input min per 2 pairs on the half-rate ALU pipe), not by "
-                                                "the tensor pipe (DESIGN.md 9)"}
+                                        "note": "K = 32 contraction per pair; paced by its CUDA-core argmin epilogue (one "
+                                                "3-input min per 2 pairs on the half-rate ALU pipe) and by the per-M-tile "
+                                                "accumulator ring, not by the tensor pipe (DESIGN.md 9)"}
         if not args.no_solve:
             pairs_t = torch.zeros(1, dtype=torch.int64, device=dev)
             oc = apd.make_opts(kernel=args.kernel, cull=1)
