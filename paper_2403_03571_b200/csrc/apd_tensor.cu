@@ -38,8 +38,8 @@ constexpr int TC_THREADS = TC_EPI_THREADS + 32 * TC_BUILD_WARPS + 64;   // + the
 constexpr int TC_QFIX = 24;                           // bf16 per seed in the tile-independent part (18 used)
 constexpr int TC_REC = 24;                            // words per seed in the TENSOR seed table: 12 fp32 + 12 x 2 bf16
 constexpr int TC_RAW_STAGES = 4, TC_TH_STAGES = 4;
-constexpr uint32_t TC_RAW_BYTES = TC_N * TC_REC * 4;  // 6144 per chunk
-constexpr uint32_t TC_TH_BYTES = TC_N * 64;           // 4096 per chunk
+constexpr uint32_t TC_RAW_BYTES = TC_N * TC_REC * 4;  // 12288 per chunk
+constexpr uint32_t TC_TH_BYTES = TC_N * 64;           // 8192 per chunk
 constexpr uint32_t TC_A_BYTES = 4 * 128 * 64;         // 32768
 constexpr uint32_t TC_SMEM = TC_A_BYTES + TC_TH_STAGES * TC_TH_BYTES + TC_RAW_STAGES * TC_RAW_BYTES;
 
@@ -226,8 +226,8 @@ __device__ __forceinline__ void tc_build_seed(const TcSeedRegs& s, bool real, fl
 __global__ void __launch_bounds__(TC_THREADS, 1) assign_tensor_kernel(const AssignArgs a) {
   extern __shared__ __align__(128) unsigned char tc_smem[];
   unsigned char* s_A = tc_smem;                                    // Phi: 4 M-tiles x 128 rows x 32 bf16
-  unsigned char* s_th = tc_smem + TC_A_BYTES;                      // Theta ring: stages x 64 rows x 32 bf16
-  unsigned char* s_raw = s_th + TC_TH_STAGES * TC_TH_BYTES;        // raw seed ring: stages x 64 seeds x 96 bytes
+  unsigned char* s_th = tc_smem + TC_A_BYTES;                      // Theta ring: stages x 128 rows x 32 bf16
+  unsigned char* s_raw = s_th + TC_TH_STAGES * TC_TH_BYTES;        // raw seed ring: stages x 128 seeds x 96 bytes
   __shared__ __align__(8) uint64_t s_raw_full[TC_RAW_STAGES], s_raw_empty[TC_RAW_STAGES];
   __shared__ __align__(8) uint64_t s_th_full[TC_TH_STAGES], s_th_empty[TC_TH_STAGES];
   __shared__ __align__(8) uint64_t s_acc_full[4], s_acc_empty[4];      // one accumulator region per M-tile
@@ -298,7 +298,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) assign_tensor_kernel(const Assi
   } else if (warp == 20) {
     // ===== MMA issuer: the whole warp walks the loop (uniform control flow, descriptors in uniform registers), one
     //       elected lane issues.  Unrolled over the 4 Theta stages so that every descriptor is base + constant. =====
-    // instruction descriptor: D fp32, A and B bf16, both K-major, N = 64, M = 128
+    // instruction descriptor: D fp32, A and B bf16, both K-major, N = 128, M = 128
     constexpr uint32_t IDESC = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(TC_N >> 3) << 17) | ((128u >> 4) << 24);
     const uint64_t ad0 = tc_smem_desc(smem_u32(s_A), 128, 512), bd0 = tc_smem_desc(smem_u32(s_th), 128, 512);
     static_assert(TC_TH_STAGES == 4, "the issue loop is unrolled over 4 Theta stages");
