@@ -415,12 +415,9 @@ cudaError_t launch_pack_qfix(const GridDev& g, int M_pad, const float* rec, uint
 }
 
 cudaError_t launch_assign_tensor(const AssignArgs& a, cudaStream_t st) {
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(assign_tensor_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM);
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
+  // per device and cheap: set on every launch (a process may drive several devices through several contexts)
+  cudaError_t e = cudaFuncSetAttribute(assign_tensor_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM);
+  if (e != cudaSuccess) return e;
   const int n_tiles = a.g.tiles_x * a.g.tiles_y * a.g.tiles_z;
   assign_tensor_kernel<<<n_tiles, TC_THREADS, TC_SMEM, st>>>(a);
   return cudaGetLastError();
