@@ -213,7 +213,10 @@ int32_t apd_choose_resolution(int32_t dim, double domain_volume, double v_min, d
 /* Same two calls with HOST arrays: the library copies in, runs the device call above and copies
  * the results out.  The device buffers belong to the context (grow-only, reused by the next host
  * call, freed by apd_destroy).  Every pointer is HOST memory (pinned memory makes the copies
- * faster); NULL is allowed where the device call allows it.  Synchronous. */
+ * faster); NULL is allowed where the device call allows it.  Synchronous.  apd_assign_host: when
+ * `labels` lies in pinned (page-locked) memory, 16-byte aligned, the kernel stores the labels
+ * straight into it during the evaluation (no device buffer, no copy afterwards); the array is
+ * complete when the call returns, as on the copy path. */
 int apd_assign_host(apd_ctx* ctx, const apd_grid* grid, int32_t M,
                     const float* X, const float* A, const float* w, const float* target_vol,
                     int32_t* labels, double* vol, double* dual, double* max_rel_err,

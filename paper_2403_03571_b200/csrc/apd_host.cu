@@ -1,9 +1,11 @@
 // apd_host.cu -- apd_assign_host / apd_solve_host: the same calls with HOST arrays.  The library
-// copies in (cudaMemcpyAsync, one per array), runs the device call, copies out.  The device
+// copies in (cudaMemcpyAsync, one per array), runs the device call, copies out (apd_assign_host writes the labels
+// in place when they live in pinned host memory).  The device
 // buffers belong to the context: grow-only, reused by the next host call, freed by apd_destroy
 // (a 64 MiB cudaMalloc + cudaFree per call cost more than the label copy).  Used for the
 // end-to-end ("e2e") measurement and by callers without a device allocator of their own.
 #include "apd_internal.cuh"
+#include <cstdint>
 
 namespace {
 
@@ -70,7 +72,19 @@ extern "C" int apd_assign_host(apd_ctx* ctx, const apd_grid* grid, int32_t M, co
   HOST_TRY(b.alloc(&dA, (size_t)M * d * d));
   HOST_TRY(b.alloc(&dw, (size_t)M));
   HOST_TRY(b.alloc(&dv, target_vol ? (size_t)M : 0));
-  HOST_TRY(b.alloc(&dl, labels ? (size_t)N : 0));
+  // labels in page-locked (pinned) host memory are device-accessible: the kernel then stores them straight there
+  // (posted writes over the host link, overlapped with the evaluation) instead of into a device buffer that is copied
+  // out afterwards -- the 4N bytes cross the link either way, but not after the kernel
+  int32_t* dl_direct = nullptr;
+  if (labels) {
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, labels) == cudaSuccess && at.type == cudaMemoryTypeHost && at.devicePointer &&
+        (reinterpret_cast<uintptr_t>(at.devicePointer) & 15) == 0)
+      dl_direct = static_cast<int32_t*>(at.devicePointer);
+    else
+      cudaGetLastError();          // pageable memory: not an error, take the copy path
+  }
+  HOST_TRY(b.alloc(&dl, labels && !dl_direct ? (size_t)N : 0));
   HOST_TRY(b.alloc(&dvol, (size_t)M));
   HOST_TRY(b.alloc(&dscal, 2));
   HOST_TRY(b.alloc(&dcen, centroids ? (size_t)M * d : 0));
@@ -81,9 +95,9 @@ extern "C" int apd_assign_host(apd_ctx* ctx, const apd_grid* grid, int32_t M, co
   HOST_TRY(cudaMemcpyAsync(dw, w, sizeof(float) * M, cudaMemcpyHostToDevice, st));
   if (target_vol) HOST_TRY(cudaMemcpyAsync(dv, target_vol, sizeof(float) * M, cudaMemcpyHostToDevice, st));
   HOST_TRY(cudaMemsetAsync(dscal, 0, 2 * sizeof(double), st));
-  const int rc = apd_assign(ctx, grid, M, dX, dA, dw, dv, dl, dvol, dscal, dscal + 1, dcen, dpairs, opts, st);
+  const int rc = apd_assign(ctx, grid, M, dX, dA, dw, dv, dl_direct ? dl_direct : dl, dvol, dscal, dscal + 1, dcen, dpairs, opts, st);
   if (rc != APD_OK) return rc;
-  if (labels) HOST_TRY(cudaMemcpyAsync(labels, dl, sizeof(int32_t) * N, cudaMemcpyDeviceToHost, st));
+  if (labels && !dl_direct) HOST_TRY(cudaMemcpyAsync(labels, dl, sizeof(int32_t) * N, cudaMemcpyDeviceToHost, st));
   HOST_TRY(cudaMemcpyAsync(vol, dvol, sizeof(double) * M, cudaMemcpyDeviceToHost, st));
   double scal[2] = {0, 0};
   HOST_TRY(cudaMemcpyAsync(scal, dscal, sizeof(scal), cudaMemcpyDeviceToHost, st));

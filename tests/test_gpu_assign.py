@@ -207,6 +207,26 @@ def test_host_call_matches_device_call(apd):
     assert np.array_equal(labels.numpy(), r["labels"]) and np.array_equal(vol.numpy(), r["vol"])
     assert dual == r["dual"] and err == r["err"] and pairs == wl.N * wl.M
     assert np.array_equal(cen.numpy(), r["centroids"])
+    ctx.close()
+
+
+@pytest.mark.parametrize("kernel,cull", [("direct", 0), ("auto", 0), ("auto", 1), ("tensor", 0)])
+def test_host_call_with_pinned_labels_writes_them_in_place(apd, kernel, cull):
+    """apd_assign_host stores the labels straight into PINNED host memory (no device buffer, no copy afterwards); the
+    result is the device call's, bit for bit, on a grid with ragged tiles (scalar and vector label stores)."""
+    kid = {"tensor": 3}.get(kernel, KERNELS.get(kernel, 0))
+    wl = workloads.make_random(3, (52, 40, 23), 77, 52, w_scale=0.1)
+    r = run_assign(apd, wl, wl.w0, v=wl.v, kernel=kid, cull=cull)
+    ctx = apd.ApdContext(3, 77)
+    grid = apd.make_grid(wl.dim, wl.n, wl.lo, wl.hi)
+    labels = torch.full((wl.N,), -7, dtype=torch.int32).pin_memory()
+    vol = torch.empty(wl.M, dtype=torch.float64).pin_memory()
+    dual, err, pairs = ctx.apd_assign_host(grid, torch.from_numpy(wl.X).pin_memory(), torch.from_numpy(wl.A).pin_memory(),
+                                           torch.from_numpy(wl.w0).pin_memory(), target_vol=torch.from_numpy(wl.v).pin_memory(),
+                                           labels=labels, vol=vol, opts=apd.make_opts(kernel=kid, cull=cull))
+    assert np.array_equal(labels.numpy(), r["labels"]) and np.array_equal(vol.numpy(), r["vol"])
+    assert dual == r["dual"] and err == r["err"]
+    ctx.close()
 
 
 # ------------------------------------------------------------------ a7: exact tile culling
