@@ -248,7 +248,10 @@ class SolveResult:
 
 
 def _two_loop(g, S_hist, Y_hist, rho, gamma):
-    """Liu-Nocedal two-loop recursion [70]: returns H*g with H0 = gamma*I."""
+    """Liu-Nocedal two-loop recursion [70]: returns H*g with H0 = gamma*I.
+    Pinned (tests/test_oracle_lbfgs_pins.py) against the dense BFGS inverse update
+    H <- (I - rho s y^T) H (I - rho y s^T) + rho s s^T applied from gamma*I, and by finite termination on a
+    strictly convex quadratic under exact line minimisation."""
     q = g.copy()
     alphas = []
     for s_i, y_i, r_i in zip(reversed(S_hist), reversed(Y_hist), reversed(rho)):
@@ -262,12 +265,108 @@ def _two_loop(g, S_hist, Y_hist, rho, gamma):
     return r
 
 
+LS_ACCEPTED, LS_STOP, LS_BUDGET, LS_FAILED = "accepted", "stop", "budget", "failed"
+
+
+def weak_wolfe_search(phi, f0: float, gp0: float, c1: float = 1e-4, c2: float = 0.9, max_trials: int = 30):
+    """The line search of specification S9 on phi(alpha) = f(w + alpha p), as a function of
+    its own so that it can be pinned without oracle_assign.
+      phi(alpha) -> (f1, gp1, stop, out_of_budget): value, directional derivative g(w + alpha p).p, "the outer
+                    stopping test holds at this point" and "no evaluation is left after this one"
+      f0, gp0     : phi(0) and phi'(0) < 0
+    alpha = 1, lo = 0, hi = inf; per trial: stop -> (LS_STOP, alpha); Armijo fails (f1 > f0 + c1 alpha gp0) ->
+    hi = alpha; else curvature fails (gp1 < c2 gp0) -> lo = alpha; else (LS_ACCEPTED, alpha); out of budget ->
+    (LS_BUDGET, alpha); next alpha = (lo + hi)/2 when hi is finite, else 2 alpha.  After max_trials: LS_FAILED.
+    An accepted alpha satisfies both weak-Wolfe inequalities by construction of the two tests."""
+    alpha, lo_a, hi_a = 1.0, 0.0, math.inf
+    for _trial in range(max_trials):
+        f1, gp1, stop, out_of_budget = phi(alpha)
+        if stop:
+            return LS_STOP, alpha
+        if f1 > f0 + c1 * alpha * gp0:
+            hi_a = alpha
+        elif gp1 < c2 * gp0:
+            lo_a = alpha
+        else:
+            return LS_ACCEPTED, alpha
+        if out_of_budget:
+            return LS_BUDGET, alpha
+        alpha = 0.5 * (lo_a + hi_a) if math.isfinite(hi_a) else 2.0 * alpha
+    return LS_FAILED, alpha
+
+
+def lbfgs_s9(evaluate, w0: np.ndarray, gamma0: float, eps: float, history: int = 10, max_iters: int = 1000,
+             max_evals: Optional[int] = None):
+    """Specification S9 as a generic minimiser of f, driven by a callable (oracle_solve passes the APD dual).
+      evaluate(w) -> (f, g, err): value, gradient and the quantity the stopping test `err <= eps` is applied to
+                     (after EVERY evaluation, S9c)
+    Returns (status, w, iters, evals) with status OK (stopping test met at w, the last point evaluated) or
+    NOT_CONVERGED (w is then None: the caller keeps track of the best point it saw).
+      * direction p = -H g by the two-loop recursion, H0 = gamma I, first gamma = gamma0, then s.y / y.y
+      * g.p >= 0: clear the history and take p = -gamma g
+      * weak_wolfe_search; on failure clear the history and retry once with p = -gamma g, else NOT_CONVERGED
+      * curvature pair kept iff s.y > 1e-12 |s| |y|; at most `history` pairs
+    """
+    if max_evals is None:
+        max_evals = 20 * max_iters
+    c1, c2 = 1e-4, 0.9
+    w = np.asarray(w0, dtype=np.float64).copy()
+    f, g, err = evaluate(w)
+    evals, iters = 1, 0
+    if err <= eps:
+        return OK, w, iters, evals
+    gamma = gamma0
+    S_hist: List[np.ndarray] = []
+    Y_hist: List[np.ndarray] = []
+    rho: List[float] = []
+    while True:
+        p = -_two_loop(g, S_hist, Y_hist, rho, gamma)
+        gp = float(np.dot(g, p))
+        if gp >= 0.0:
+            S_hist, Y_hist, rho = [], [], []
+            p = -gamma * g
+            gp = float(np.dot(g, p))
+        last = {}
+
+        def phi(alpha):
+            nonlocal evals
+            w_try = w + alpha * p
+            f1, g1, err1 = evaluate(w_try)
+            evals += 1
+            last.update(w=w_try, f=f1, g=g1)
+            return f1, float(np.dot(g1, p)), err1 <= eps, evals >= max_evals
+
+        outcome, alpha = weak_wolfe_search(phi, f, gp, c1, c2, 30)
+        if outcome == LS_STOP:
+            return OK, last["w"], iters + 1, evals
+        if outcome == LS_BUDGET:
+            return NOT_CONVERGED, None, iters, evals
+        if outcome == LS_FAILED:
+            if S_hist:
+                S_hist, Y_hist, rho = [], [], []
+                continue                                  # retry once with p = -gamma g
+            return NOT_CONVERGED, None, iters, evals
+        w_try, f1, g1 = last["w"], last["f"], last["g"]
+        s = alpha * p
+        yv = g1 - g
+        sy = float(np.dot(s, yv))
+        if sy > 1e-12 * math.sqrt(float(np.dot(s, s))) * math.sqrt(float(np.dot(yv, yv))):
+            S_hist.append(s); Y_hist.append(yv); rho.append(1.0 / sy)
+            if len(S_hist) > history:
+                S_hist.pop(0); Y_hist.pop(0); rho.pop(0)
+            gamma = sy / float(np.dot(yv, yv))
+        w, f, g = w_try, f1, g1
+        iters += 1
+        if iters >= max_iters or evals >= max_evals:
+            return NOT_CONVERGED, None, iters, evals
+
+
 def oracle_solve(grid: Grid, X, A, v, eps: float, w_init=None, history: int = 10,
                  max_iters: int = 1000, max_evals: Optional[int] = None,
                  record: bool = False) -> SolveResult:
     """Maximise g~ (eq. 2.7) <=> minimise f = -g~ from W0 = 0 (Alg. 2 step 2) with L-BFGS,
     stop when max_i |vol_i - v_i|/v_i <= eps (Alg. 2 step 3, eq. 2.5; '<=' is reading S7).
-    Specification S9 (shared with the CUDA path):
+    Specification S9 (shared with the CUDA path; the optimiser itself is lbfgs_s9 above):
       * fp64 optimiser state; every evaluation uses fl32(w) (round-to-nearest-even), S10
       * f = -g~(fl32 w), grad f = vol - v  (eq. 2.8 with the sign of f)
       * first-direction scale gamma = l^(2-d)/d, l = (|Omega|/M)^(1/d)  (S9a)
@@ -281,14 +380,11 @@ def oracle_solve(grid: Grid, X, A, v, eps: float, w_init=None, history: int = 10
     d = grid.dim
     M = np.asarray(X).reshape(-1, d).shape[0]
     v64 = np.asarray(v, dtype=np.float64).reshape(M)
-    if max_evals is None:
-        max_evals = 20 * max_iters
-    c1, c2 = 1e-4, 0.9
     traj: Optional[List[dict]] = [] if record else None
-
     best = {"err": math.inf}
+    last = {}
 
-    def evaluate(wd, tag):
+    def evaluate(wd):
         w32 = wd.astype(np.float32)                     # RNE rounding, S10
         if isinstance(grid, PointSet):                  # user-supplied discretisation
             r = oracle_assign_points(grid.Y, grid.pvol, X, A, w32, v=v64)
@@ -299,72 +395,21 @@ def oracle_solve(grid: Grid, X, A, v, eps: float, w_init=None, history: int = 10
         if r.err < best["err"]:
             best.update(err=r.err, w=wd.copy(), w32=w32.copy(), labels=r.labels, vol=r.vol, dual=r.dual)
         if traj is not None:
-            traj.append(dict(tag=tag, w=wd.copy(), f=f, err=r.err))
-        return f, g, r.err, w32, r
+            traj.append(dict(tag="init" if not traj else "ls", w=wd.copy(), f=f, err=r.err))
+        last.update(w32=w32, r=r)
+        return f, g, r.err
 
-    def finish(status, wd, w32, r, iters, evals):
-        return SolveResult(status=status, w=wd, w32=w32, labels=r.labels, vol=r.vol, iters=iters,
-                           evals=evals, err=r.err, dual=r.dual, trajectory=traj)
-
-    def finish_best(iters, evals):
-        return SolveResult(status=NOT_CONVERGED, w=best["w"], w32=best["w32"], labels=best["labels"],
-                           vol=best["vol"], iters=iters, evals=evals, err=best["err"], dual=best["dual"],
-                           trajectory=traj)
-
-    w = np.zeros(M, dtype=np.float64) if w_init is None else np.asarray(w_init, dtype=np.float64).copy()
-    f, g, err, w32, r = evaluate(w, "init")
-    evals, iters = 1, 0
-    if err <= eps:
-        return finish(OK, w, w32, r, iters, evals)
-
+    w0 = np.zeros(M, dtype=np.float64) if w_init is None else np.asarray(w_init, dtype=np.float64).copy()
     ell = (grid.domain_volume / M) ** (1.0 / d)
-    gamma = ell ** (2 - d) / d
-    S_hist: List[np.ndarray] = []
-    Y_hist: List[np.ndarray] = []
-    rho: List[float] = []
-
-    while True:
-        p = -_two_loop(g, S_hist, Y_hist, rho, gamma)
-        gp = float(np.dot(g, p))
-        if gp >= 0.0:
-            S_hist, Y_hist, rho = [], [], []
-            p = -gamma * g
-            gp = float(np.dot(g, p))
-        alpha, lo_a, hi_a = 1.0, 0.0, math.inf
-        accepted = False
-        for _trial in range(30):
-            w_try = w + alpha * p
-            f1, g1, err1, w32_1, r1 = evaluate(w_try, "ls")
-            evals += 1
-            if err1 <= eps:
-                return finish(OK, w_try, w32_1, r1, iters + 1, evals)
-            if f1 > f + c1 * alpha * gp:
-                hi_a = alpha
-            elif float(np.dot(g1, p)) < c2 * gp:
-                lo_a = alpha
-            else:
-                accepted = True
-                break
-            if evals >= max_evals:
-                return finish_best(iters, evals)
-            alpha = 0.5 * (lo_a + hi_a) if math.isfinite(hi_a) else 2.0 * alpha
-        if not accepted:
-            if S_hist:
-                S_hist, Y_hist, rho = [], [], []
-                continue                                  # retry once with p = -gamma g
-            return finish_best(iters, evals)
-        s = alpha * p
-        yv = g1 - g
-        sy = float(np.dot(s, yv))
-        if sy > 1e-12 * math.sqrt(float(np.dot(s, s))) * math.sqrt(float(np.dot(yv, yv))):
-            S_hist.append(s); Y_hist.append(yv); rho.append(1.0 / sy)
-            if len(S_hist) > history:
-                S_hist.pop(0); Y_hist.pop(0); rho.pop(0)
-            gamma = sy / float(np.dot(yv, yv))
-        w, f, g = w_try, f1, g1
-        iters += 1
-        if iters >= max_iters or evals >= max_evals:
-            return finish_best(iters, evals)
+    gamma0 = ell ** (2 - d) / d
+    status, w, iters, evals = lbfgs_s9(evaluate, w0, gamma0, eps, history=history, max_iters=max_iters,
+                                       max_evals=max_evals)
+    if status == OK:
+        r = last["r"]
+        return SolveResult(status=OK, w=w, w32=last["w32"], labels=r.labels, vol=r.vol, iters=iters, evals=evals,
+                           err=r.err, dual=r.dual, trajectory=traj)
+    return SolveResult(status=NOT_CONVERGED, w=best["w"], w32=best["w32"], labels=best["labels"], vol=best["vol"],
+                       iters=iters, evals=evals, err=best["err"], dual=best["dual"], trajectory=traj)
 
 
 # ----------------------------------------------------------------------------------------
