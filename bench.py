@@ -308,9 +308,10 @@ def run_ours(args):
         extra = {}
         if not args.no_probe:
             try:
-                p0, mhz0 = apd.apd_fp32_probe(0, local)
-                p1, _ = apd.apd_fp32_probe(1, local)
-                p3, _ = apd.apd_fp32_probe(3, local)
+                from paper_2403_03571_b200 import probe
+                p0, mhz0 = probe.apd_fp32_probe(0, local)
+                p1, _ = probe.apd_fp32_probe(1, local)
+                p3, _ = probe.apd_fp32_probe(3, local)
                 extra["fp32_probe"] = {"ffma_tflops": 2 * p0 / 1e12, "ffma2_tflops": 2 * p1 / 1e12,
                                        "rowpoly_mix_gpairs": p3 / 1e9, "sm_mhz": mhz0}
                 roofline["frac_of_rowpoly_mix_probe"] = (wl.pairs / (kernel_ms * 1e-3)) / p3
@@ -453,32 +454,6 @@ def run_solve_only(args):
     print(json.dumps(out), flush=True)
 
 
-def run_paper_like(args):
-    """--paper-like: the paper's own runtime test (b) recipe on this library, for CONTEXT beside the
-    paper's A100 prose numbers.  One JSON line per case; not part of the headline metric."""
-    import torch
-    from paper_2403_03571_b200 import binding as apd
-    dev = torch.device("cuda", 0)
-    cases = [(3, 10000, 0.0, False, 200), (3, 10000, 0.3, False, 200), (3, 10000, 0.7, False, 200),
-             (3, 10000, 0.3, True, None), (2, 5000, 0.3, False, None), (2, 5000, 0.3, True, None)]
-    for dim, M, alpha, multi, n_axis in cases:
-        wl = workloads.make_paper_test(dim, M, alpha, multi, n_axis)
-        ctx = apd.ApdContext(wl.dim, wl.M)
-        grid = apd.make_grid(wl.dim, wl.n, wl.lo, wl.hi)
-        X = torch.from_numpy(wl.X).to(dev); A = torch.from_numpy(wl.A).to(dev); v = torch.from_numpy(wl.v).to(dev)
-        vol = torch.zeros(wl.M, dtype=torch.float64, device=dev)
-        secs = []
-        for _ in range(2):
-            wS = torch.zeros(wl.M, dtype=torch.float32, device=dev)
-            torch.cuda.synchronize(); ts = time.perf_counter()
-            info = ctx.apd_solve(grid, X, A, v, 0.01, w=wS, vol=vol, opts=apd.make_opts(cull=1, max_iters=args.solve_max_iters))
-            torch.cuda.synchronize(); secs.append(time.perf_counter() - ts)
-        print(json.dumps({"case": wl.name, "grid": list(wl.n), "grains": wl.M, "alpha": alpha, "multiphase": multi,
-                          "seconds": secs[-1], "status": info.status, "iters": info.iters, "evals": info.evals,
-                          "max_rel_err": info.max_rel_err}), flush=True)
-        ctx.close()
-
-
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -491,7 +466,6 @@ def main():
     ap.add_argument("--no-probe", action="store_true")
     ap.add_argument("--no-direct", action="store_true")
     ap.add_argument("--no-cfg5", action="store_true")
-    ap.add_argument("--paper-like", action="store_true", help="context runs on the paper's own runtime-test recipe")
     ap.add_argument("--solve-only", action="store_true", help="only the culled apd_solve of the headline workload")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--solve-max-iters", type=int, default=1000)
@@ -501,8 +475,6 @@ def main():
         run_reference(args)
     elif args.solve_only:
         run_solve_only(args)
-    elif args.paper_like:
-        run_paper_like(args)
     else:
         run_ours(args)
 

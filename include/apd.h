@@ -117,7 +117,13 @@ const char* apd_last_error(const apd_ctx* ctx);
  *   pairs_evaluated [1]     DEVICE uint64 out or NULL: voxel-seed pairs whose cost was
  *                           evaluated (= N*M without culling)
  * Asynchronous on `cuda_stream` (a cudaStream_t; NULL = the legacy default stream): returns
- * after enqueueing; outputs are valid once the stream reaches this point.
+ * after enqueueing; outputs are valid once the stream reaches this point.  The one exception: the FIRST call on a
+ * grid with more tiles than any before it (or the first with opts.cull / APD_KERNEL_TENSOR) grows the context's
+ * workspace, which synchronises `cuda_stream` and calls cudaMalloc -- not allowed under stream capture.  apd_reserve
+ * does that growth ahead of time; after it, calls on that grid (or a smaller one) never allocate or synchronise.
+ * A context serialises on ONE stream at a time: every call uses the context's single workspace, so two calls in
+ * flight on different streams race; the caller orders them (events), or uses one context per stream.
+ * `labels` needs only int32 alignment; a 16-byte aligned pointer gets vectorised stores.
  * APD_E_ARG: NULL ctx/grid/required pointer, grid.dim != ctx dim, n_k < 1, hi <= lo,
  * N >= 2^31, M < 1 or M > max_seeds, unknown opts value.  opts == NULL means defaults. */
 int apd_assign(apd_ctx* ctx, const apd_grid* grid, int32_t M,
@@ -132,14 +138,18 @@ int apd_assign(apd_ctx* ctx, const apd_grid* grid, int32_t M,
  * every evaluation at fl32(w), weak-Wolfe bracketing line search, stopping test after every
  * evaluation.  The loop runs on the device; the host reads one mapped status word per
  * evaluation and nothing else.
- *   X, A, target_vol, w_init   DEVICE fp32 in (as apd_assign); sum target_vol must equal
- *                              |Omega| to 1e-5 relative else APD_E_ARG
+ *   X, A, target_vol, w_init   DEVICE fp32 in (as apd_assign); every target_vol_i > 0 and
+ *                              sum target_vol = |Omega| to 1e-6 relative, else APD_E_ARG.  This one
+ *                              check runs on the device with the first evaluation: APD_E_ARG from it is returned
+ *                              after that evaluation ran (outputs untouched)
  *   w          [M]  DEVICE fp32 out, required: exactly the weights the final evaluation used
  *   labels     [N]  DEVICE int32 out or NULL: Algorithm 1 at the returned w
  *   vol        [M]  DEVICE fp64 out or NULL: cell volumes at the returned w
  *   w64        [M]  DEVICE fp64 out or NULL: the optimiser's fp64 iterate (w = fl32(w64))
  *   iters, evals, max_rel_err, dual   HOST out, each may be NULL
- * Blocks until the solve has finished (synchronises `cuda_stream`).
+ * max_iters / max_evals are tested after each line-search evaluation (as the oracle's specification S9 does): unless
+ * the start already meets the tolerance at least two evaluations run.
+ * Blocks until the solve has finished (synchronises `cuda_stream`).  Workspace growth as for apd_assign (apd_reserve).
  * Returns APD_OK, APD_NOT_CONVERGED, or a negative error. */
 int apd_solve(apd_ctx* ctx, const apd_grid* grid, int32_t M,
               const float* X, const float* A, const float* target_vol, double tol,
@@ -166,7 +176,7 @@ int apd_assign_points(apd_ctx* ctx, int64_t N, const float* Y, const float* pvol
 
 /* Algorithm 2 on a user-supplied discretisation: the L-BFGS of apd_solve (same specification S9) with every evaluation
  * done by the point kernel of apd_assign_points.  total_volume = sum_j |P_j| (HOST; it replaces |Omega|: sum
- * target_vol must equal it to 1e-5 relative, else APD_E_ARG).  Y, pvol, X, A, target_vol, w_init, w, labels [N],
+ * target_vol must equal it to 1e-6 relative, else APD_E_ARG).  Y, pvol, X, A, target_vol, w_init, w, labels [N],
  * vol [M]: DEVICE as above; iters, evals, max_rel_err: HOST out.  No culling (opts.cull must be 0).  Because cell
  * volumes are fp64 sums accumulated in no fixed order, two runs can differ in the last bits and, rarely, in a
  * line-search decision.  Blocks until finished; returns APD_OK, APD_NOT_CONVERGED or a negative error. */
@@ -227,17 +237,19 @@ int apd_solve_host(apd_ctx* ctx, const apd_grid* grid, int32_t M,
                    int32_t* iters, int32_t* evals, double* max_rel_err, double* dual,
                    const apd_opts* opts);
 
-/* Measurement helpers: not part of the method.
- * apd_last_kernel_ms: device time in ms (CUDA events on the launching stream) of the voxel x
- *   seed kernel of the most recent apd_assign on this context; synchronises that event.
- *   Returns a negative value if no evaluation has run.
- * apd_fp32_probe: runs a register-only FP32 microbenchmark on `device` and returns the
- *   achieved rate in *ops_per_s (HOST): variant 0 = scalar FFMA (2 flop each), 1 = packed
- *   fma.rn.f32x2 (4 flop each), 2 = 3-input min.f32, 3 = the ROWPOLY inner-loop mix
- *   (3 f32x2 FMA + 2 three-input min per 4 pairs).  *ops_per_s counts FMA lanes (variants 0,1), min
- *   instructions x32 lanes (2) or voxel-seed pairs (3).  Synchronous. */
-double apd_last_kernel_ms(apd_ctx* ctx);
-int    apd_fp32_probe(int32_t device, int32_t variant, double* ops_per_s, double* sm_clock_mhz);
+/* Grows the context's workspace to what apd_assign / apd_solve / apd_lloyd need on `grid` with `opts` (dual partials:
+ * 8 bytes per tile; with opts.cull the candidate lists, 1 KiB per 512 voxels; L-BFGS state for opts.lbfgs_history),
+ * so that those calls, on this grid or any grid with no more tiles, neither allocate nor synchronise.  Synchronous
+ * (cudaMalloc).  APD_E_ARG as apd_assign; APD_E_CUDA on allocation failure. */
+int apd_reserve(apd_ctx* ctx, const apd_grid* grid, const apd_opts* opts);
+
+/* What the most recent evaluation on this context launched (HOST out, each may be NULL): the kernel after AUTO was
+ * resolved (APD_KERNEL_*), whether the ROWPOLY kernel ran its long-row geometry (rows of 32 voxels per thread; 0 =
+ * rows of 16), whether culling ran, the number of CTA tiles, and the device time in ms of the voxel x seed kernel
+ * alone (CUDA events on the launching stream around that one launch; the call waits for the second event; -1 inside
+ * apd_solve's loop, which is not timed).  APD_E_ARG if no evaluation has run. */
+int apd_assign_stats(apd_ctx* ctx, int32_t* kernel, int32_t* row_long, int32_t* cull, int32_t* n_tiles,
+                     double* kernel_ms);
 
 #ifdef __cplusplus
 }

@@ -102,18 +102,17 @@ def load_library() -> ctypes.CDLL:
     lib.apd_choose_resolution.argtypes = [ctypes.c_int32, ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_int32]
     lib.apd_solve_history.restype = ctypes.c_int
     lib.apd_solve_history.argtypes = [_P, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double), ctypes.c_int32]
-    lib.apd_last_kernel_ms.restype = ctypes.c_double
-    lib.apd_last_kernel_ms.argtypes = [_P]
-    lib.apd_fp32_probe.restype = ctypes.c_int
-    lib.apd_fp32_probe.argtypes = [ctypes.c_int32, ctypes.c_int32, ctypes.POINTER(ctypes.c_double),
-                                   ctypes.POINTER(ctypes.c_double)]
+    lib.apd_reserve.restype = ctypes.c_int
+    lib.apd_reserve.argtypes = [_P, ctypes.POINTER(apd_grid), ctypes.POINTER(apd_opts)]
+    lib.apd_assign_stats.restype = ctypes.c_int
+    lib.apd_assign_stats.argtypes = [_P] + [ctypes.POINTER(ctypes.c_int32)] * 4 + [ctypes.POINTER(ctypes.c_double)]
     _lib = lib
     return lib
 
 
 EXPORTED_SYMBOLS = ["apd_default_opts", "apd_create", "apd_destroy", "apd_last_error", "apd_assign", "apd_solve",
                     "apd_assign_host", "apd_solve_host", "apd_solve_history", "apd_assign_points", "apd_solve_points", "apd_solve_stats", "apd_lloyd", "apd_solve_refine", "apd_resolution_bound",
-                    "apd_choose_resolution", "apd_last_kernel_ms", "apd_fp32_probe"]
+                    "apd_choose_resolution", "apd_reserve", "apd_assign_stats"]
 
 
 def make_grid(dim: int, n: Sequence[int], lo: Sequence[float], hi: Sequence[float]) -> apd_grid:
@@ -337,8 +336,20 @@ class ApdContext:
             self._check(n)
         return np.array(d[:n], dtype=np.float64), np.array(e[:n], dtype=np.float64)
 
+    def reserve(self, grid: apd_grid, opts: Optional[apd_opts] = None):
+        """apd_reserve of include/apd.h: grow the workspace ahead of time."""
+        self._check(self._lib.apd_reserve(self._h, ctypes.byref(grid), ctypes.byref(opts) if opts is not None else None))
+
+    def assign_stats(self) -> dict:
+        """apd_assign_stats of include/apd.h: what the most recent evaluation launched."""
+        k, rl, cu, nt = (ctypes.c_int32(0) for _ in range(4))
+        ms = ctypes.c_double(0.0)
+        self._check(self._lib.apd_assign_stats(self._h, ctypes.byref(k), ctypes.byref(rl), ctypes.byref(cu),
+                                               ctypes.byref(nt), ctypes.byref(ms)))
+        return dict(kernel=k.value, row_long=rl.value, cull=cu.value, n_tiles=nt.value, kernel_ms=ms.value)
+
     def last_kernel_ms(self) -> float:
-        return float(self._lib.apd_last_kernel_ms(self._h))
+        return float(self.assign_stats()["kernel_ms"])
 
 
 def apd_resolution_bound(dim: int, domain_volume: float, v_min: float, eps: float, practical: bool) -> float:
@@ -347,13 +358,3 @@ def apd_resolution_bound(dim: int, domain_volume: float, v_min: float, eps: floa
 
 def apd_choose_resolution(dim: int, domain_volume: float, v_min: float, eps: float, practical: bool) -> int:
     return int(load_library().apd_choose_resolution(dim, domain_volume, v_min, eps, int(practical)))
-
-
-def apd_fp32_probe(variant: int, device: int = 0):
-    """(ops_per_s, sm_clock_mhz) of the library's FP32 microbenchmark `variant` (include/apd.h)."""
-    lib = load_library()
-    ops, mhz = ctypes.c_double(0.0), ctypes.c_double(0.0)
-    rc = lib.apd_fp32_probe(device, variant, ctypes.byref(ops), ctypes.byref(mhz))
-    if rc != APD_OK:
-        raise ApdError(rc, "apd_fp32_probe failed")
-    return ops.value, mhz.value

@@ -30,7 +30,7 @@ extern "C" void apd_default_opts(apd_opts* o) {
 }
 
 static void free_ws(Workspace& ws) {
-  cudaFree(ws.pt_acc); cudaFree(ws.qfix); cudaFree(ws.rec); cudaFree(ws.brick_list); cudaFree(ws.brick_count); cudaFree(ws.super_list);
+  cudaFree(ws.lloyd_buf); cudaFree(ws.pt_acc); cudaFree(ws.qfix); cudaFree(ws.rec); cudaFree(ws.brick_list); cudaFree(ws.brick_count); cudaFree(ws.super_list);
   cudaFree(ws.super_count); cudaFree(ws.pairs_ctr);
   cudaFree(ws.seeds); cudaFree(ws.count); cudaFree(ws.idxsum); cudaFree(ws.dual_partial);
   cudaFree(ws.sstate); cudaFree(ws.svec); cudaFree(ws.gram); cudaFree(ws.w32); cudaFree(ws.wref); cudaFree(ws.e_vol); cudaFree(ws.e_scal); cudaFree(ws.hist);
@@ -146,6 +146,46 @@ int resolve_kernel(const apd_opts* o, const apd_grid* grid, bool* cull, std::str
   return k;
 }
 
+int ensure_eval_buffers(apd_ctx* ctx, const GridDev& g, int kernel, bool cull, cudaStream_t st) {
+  Workspace& ws = ctx->ws;
+  const size_t n_tiles = (size_t)g.tiles_x * g.tiles_y * g.tiles_z;
+  const size_t n_partials = cull ? 4 * n_tiles : n_tiles;      // the culled kernel writes one partial per brick (warp)
+  const size_t m_pad_max = ((size_t)ws.max_seeds + SEED_CHUNK - 1) / SEED_CHUNK * SEED_CHUNK;
+  if (n_partials > ws.partial_cap) {
+    APD_CUDA_TRY(ctx, cudaStreamSynchronize(st));            // earlier work on st may still read the old buffer
+    APD_CUDA_TRY(ctx, cudaFree(ws.dual_partial));
+    ws.dual_partial = nullptr;
+    ws.partial_cap = 0;
+    APD_CUDA_TRY(ctx, cudaMalloc(&ws.dual_partial, n_partials * sizeof(double)));
+    ws.partial_cap = n_partials;
+  }
+  if (kernel == APD_KERNEL_TENSOR && !ws.qfix)
+    APD_CUDA_TRY(ctx, cudaMalloc(&ws.qfix, m_pad_max * 6 * sizeof(uint4)));
+  if (cull) {
+    int nsx, nsy, nsz;
+    cull_super_counts(g, &nsx, &nsy, &nsz);
+    const size_t n_super = (size_t)nsx * nsy * nsz, n_bricks = n_tiles * 4;
+    if (!ws.rec) {
+      APD_CUDA_TRY(ctx, cudaMalloc(&ws.rec, m_pad_max * rec_floats(ws.dim) * sizeof(float)));
+      APD_CUDA_TRY(ctx, cudaMalloc(&ws.pairs_ctr, sizeof(unsigned long long)));
+    }
+    if (n_bricks > ws.brick_cap_n || n_super > ws.super_cap_n) {
+      APD_CUDA_TRY(ctx, cudaStreamSynchronize(st));
+      cudaFree(ws.brick_list); cudaFree(ws.brick_count); cudaFree(ws.super_list); cudaFree(ws.super_count);
+      ws.brick_list = ws.brick_count = ws.super_list = ws.super_count = nullptr;
+      const size_t nb = n_bricks > ws.brick_cap_n ? n_bricks : ws.brick_cap_n;
+      const size_t ns = n_super > ws.super_cap_n ? n_super : ws.super_cap_n;
+      ws.brick_cap_n = ws.super_cap_n = 0;
+      APD_CUDA_TRY(ctx, cudaMalloc(&ws.brick_list, nb * BRICK_CAP * sizeof(int)));
+      APD_CUDA_TRY(ctx, cudaMalloc(&ws.brick_count, nb * sizeof(int)));
+      APD_CUDA_TRY(ctx, cudaMalloc(&ws.super_list, ns * SUPER_CAP * sizeof(int)));
+      APD_CUDA_TRY(ctx, cudaMalloc(&ws.super_count, ns * sizeof(int)));
+      ws.brick_cap_n = nb; ws.super_cap_n = ns;
+    }
+  }
+  return APD_OK;
+}
+
 // Enqueues one evaluation (pack -> assign -> finalize) on `st`.  All pointers device.
 int enqueue_evaluation(apd_ctx* ctx, const GridDev& g, int kernel, int M, const float* X, const float* A,
                        const float* w, const float* target_vol, int32_t* labels, double* vol, double* dual,
@@ -154,15 +194,9 @@ int enqueue_evaluation(apd_ctx* ctx, const GridDev& g, int kernel, int M, const 
   Workspace& ws = ctx->ws;
   const int M_pad = (M + SEED_CHUNK - 1) / SEED_CHUNK * SEED_CHUNK;
   const int n_tiles = g.tiles_x * g.tiles_y * g.tiles_z;
-  const int n_partials = cull ? 4 * n_tiles : n_tiles;      // the culled kernel writes one partial per brick (warp)
-  if ((size_t)n_partials > ws.partial_cap) {
-    // grow the per-tile partial buffer (stream-ordered free/alloc keeps earlier work valid)
-    APD_CUDA_TRY(ctx, cudaStreamSynchronize(st));
-    APD_CUDA_TRY(ctx, cudaFree(ws.dual_partial));
-    ws.dual_partial = nullptr;
-    ws.partial_cap = (size_t)n_partials;
-    APD_CUDA_TRY(ctx, cudaMalloc(&ws.dual_partial, ws.partial_cap * sizeof(double)));
-  }
+  const int n_partials = cull ? 4 * n_tiles : n_tiles;
+  const int rc_buf = ensure_eval_buffers(ctx, g, kernel, cull, st);   // no-op after apd_reserve / a call of this size
+  if (rc_buf != APD_OK) return rc_buf;
   if (cull) {
     // the culled kernel reads the per-seed record table that launch_cull packs (and which zeroes the accumulators)
   } else if (kernel == APD_KERNEL_ROWPOLY)
@@ -171,15 +205,11 @@ int enqueue_evaluation(apd_ctx* ctx, const GridDev& g, int kernel, int M, const 
   else
     APD_CUDA_TRY(ctx, launch_pack_seeds(g.dim, M, M_pad, X, A, w, ws.seeds, ws.count,
                                         centroids ? ws.idxsum : nullptr, done_flag, st));
-  if (kernel == APD_KERNEL_TENSOR) {
-    if (!ws.qfix) {
-      const size_t m_pad_max = ((size_t)ws.max_seeds + SEED_CHUNK - 1) / SEED_CHUNK * SEED_CHUNK;
-      APD_CUDA_TRY(ctx, cudaMalloc(&ws.qfix, m_pad_max * 6 * sizeof(uint4)));
-    }
+  if (kernel == APD_KERNEL_TENSOR)
     APD_CUDA_TRY(ctx, launch_pack_qfix(g, M_pad, ws.seeds, ws.qfix, done_flag, st));
-  }
   AssignArgs a;
   a.g = g; a.M = M; a.M_pad = M_pad; a.seeds = ws.seeds; a.labels = labels; a.count = ws.count;
+  a.labels_vec = (reinterpret_cast<uintptr_t>(labels) & 15) == 0;
   for (int j = 0; j < 16; ++j) {      // in-row offsets from a row's midpoint and their squares (apd_rowpoly.cu: RowTau)
     const double tau = ((double)j + 0.5) * g.s[0];
     a.tt[j] = (float)tau;
@@ -191,32 +221,16 @@ int enqueue_evaluation(apd_ctx* ctx, const GridDev& g, int kernel, int M, const 
   a.done_flag = done_flag;
   a.qfix = ws.qfix;
   if (cull) {
-    // a7: two-level candidate lists, rebuilt every evaluation (the bounds depend on w)
+    // a7: two-level candidate lists (rebuilt when the weights left the slack they were built with)
     int nsx, nsy, nsz;
     cull_super_counts(g, &nsx, &nsy, &nsz);
-    const size_t n_super = (size_t)nsx * nsy * nsz, n_bricks = (size_t)n_tiles * 4;
-    if (!ws.rec) {
-      const size_t m_pad_max = ((size_t)ws.max_seeds + SEED_CHUNK - 1) / SEED_CHUNK * SEED_CHUNK;
-      APD_CUDA_TRY(ctx, cudaMalloc(&ws.rec, m_pad_max * rec_floats(ws.dim) * sizeof(float)));
-      APD_CUDA_TRY(ctx, cudaMalloc(&ws.pairs_ctr, sizeof(unsigned long long)));
-    }
-    if (n_bricks > ws.brick_cap_n || n_super > ws.super_cap_n) {
-      APD_CUDA_TRY(ctx, cudaStreamSynchronize(st));
-      cudaFree(ws.brick_list); cudaFree(ws.brick_count); cudaFree(ws.super_list); cudaFree(ws.super_count);
-      ws.brick_list = ws.brick_count = ws.super_list = ws.super_count = nullptr;
-      ws.brick_cap_n = ws.super_cap_n = 0;
-      APD_CUDA_TRY(ctx, cudaMalloc(&ws.brick_list, n_bricks * BRICK_CAP * sizeof(int)));
-      APD_CUDA_TRY(ctx, cudaMalloc(&ws.brick_count, n_bricks * sizeof(int)));
-      APD_CUDA_TRY(ctx, cudaMalloc(&ws.super_list, n_super * SUPER_CAP * sizeof(int)));
-      APD_CUDA_TRY(ctx, cudaMalloc(&ws.super_count, n_super * sizeof(int)));
-      ws.brick_cap_n = n_bricks; ws.super_cap_n = n_super;
-    }
     CullBuffers cb{ws.rec, ws.brick_list, ws.brick_count, ws.super_list, ws.super_count, ws.pairs_ctr};
     APD_CUDA_TRY(ctx, launch_cull(g, M, M_pad, X, A, w, cb, nsx, nsy, nsz, ws.count, centroids ? ws.idxsum : nullptr, done_flag,
                                   cull_rebuild, cull_delta, st));
     a.rec = ws.rec; a.brick_list = ws.brick_list; a.brick_count = ws.brick_count; a.super_list = ws.super_list;
     a.super_count = ws.super_count; a.super_x = nsx; a.super_y = nsy; a.pairs_ctr = ws.pairs_ctr;
   }
+  ws.last_kernel = kernel; ws.last_row_long = g.row_long; ws.last_cull = cull ? 1 : 0; ws.last_tiles = n_tiles;
   if (timed) APD_CUDA_TRY(ctx, cudaEventRecord(ws.ev0, st));
   APD_CUDA_TRY(ctx, launch_assign(kernel, a, st));
   if (timed) { APD_CUDA_TRY(ctx, cudaEventRecord(ws.ev1, st)); ws.timed = true; }
@@ -248,10 +262,48 @@ extern "C" int apd_assign(apd_ctx* ctx, const apd_grid* grid, int32_t M, const f
                             pairs_evaluated, true, cull, nullptr, static_cast<cudaStream_t>(cuda_stream));
 }
 
-extern "C" double apd_last_kernel_ms(apd_ctx* ctx) {
-  if (!ctx || !ctx->ws.timed) return -1.0;
-  if (cudaEventSynchronize(ctx->ws.ev1) != cudaSuccess) return -1.0;
-  float ms = 0.f;
-  if (cudaEventElapsedTime(&ms, ctx->ws.ev0, ctx->ws.ev1) != cudaSuccess) return -1.0;
-  return (double)ms;
+extern "C" int apd_assign_stats(apd_ctx* ctx, int32_t* kernel, int32_t* row_long, int32_t* cull, int32_t* n_tiles,
+                                double* kernel_ms) {
+  if (!ctx) return APD_E_ARG;
+  const Workspace& ws = ctx->ws;
+  if (ws.last_kernel < 0) { ctx->err = "apd_assign_stats: no evaluation has run on this context"; return APD_E_ARG; }
+  if (kernel) *kernel = ws.last_kernel;
+  if (row_long) *row_long = ws.last_row_long;
+  if (cull) *cull = ws.last_cull;
+  if (n_tiles) *n_tiles = ws.last_tiles;
+  if (kernel_ms) {
+    *kernel_ms = -1.0;
+    if (ws.timed) {
+      float ms = 0.f;
+      if (cudaEventSynchronize(ws.ev1) != cudaSuccess || cudaEventElapsedTime(&ms, ws.ev0, ws.ev1) != cudaSuccess) {
+        ctx->err = "apd_assign_stats: the kernel's events could not be read";
+        return APD_E_CUDA;
+      }
+      *kernel_ms = (double)ms;
+    }
+  }
+  return APD_OK;
+}
+
+extern "C" int apd_reserve(apd_ctx* ctx, const apd_grid* grid, const apd_opts* opts) {
+  if (!ctx) return APD_E_ARG;
+  ctx->err.clear();
+  std::string e;
+  bool cull = false;
+  const int kernel = resolve_kernel(opts, grid, &cull, &e);
+  if (kernel < 0) { ctx->err = "apd_reserve: " + e; return APD_E_ARG; }
+  GridDev g;
+  e = make_grid(ctx, grid, kernel, cull, &g);
+  if (!e.empty()) { ctx->err = "apd_reserve: " + e; return APD_E_ARG; }
+  APD_CUDA_TRY(ctx, cudaSetDevice(ctx->ws.device));
+  int rc = ensure_eval_buffers(ctx, g, kernel, cull, nullptr);
+  if (rc != APD_OK) return rc;
+  const int hist = opts ? opts->lbfgs_history : 10;
+  if (hist < 1 || hist > 64) { ctx->err = "apd_reserve: lbfgs_history must be in [1,64]"; return APD_E_ARG; }
+  rc = ensure_solve_state(ctx, hist);
+  if (rc != APD_OK) return rc;
+  Workspace& ws = ctx->ws;
+  if (!ws.lloyd_buf)
+    APD_CUDA_TRY(ctx, cudaMalloc(&ws.lloyd_buf, ((size_t)ws.max_seeds * (ws.dim + 1) + 2) * sizeof(double)));
+  return APD_OK;
 }

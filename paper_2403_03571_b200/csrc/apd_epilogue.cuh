@@ -14,8 +14,9 @@ __device__ __forceinline__ double row_epilogue(const AssignArgs& a, bool row_val
   const int nvalid = min(V, a.g.nx - ix0);
   const long long j0 = ((long long)iz * a.g.ny + iy) * a.g.nx + ix0;
   if (a.labels) {
-    if (nvalid == V && (a.g.nx & 3) == 0) {
-      int4* p = reinterpret_cast<int4*>(a.labels + j0);      // j0 % 4 == 0 because nx % 4 == 0, ix0 % V == 0
+    if (nvalid == V && (a.g.nx & 3) == 0 && a.labels_vec) {
+      int4* p = reinterpret_cast<int4*>(a.labels + j0);      // 16-byte aligned: the base is (labels_vec), and j0 % 4 == 0
+                                                             // because nx % 4 == 0 and ix0 % V == 0
 #pragma unroll
       for (int k = 0; k < V / 4; ++k) p[k] = make_int4(lab[4 * k], lab[4 * k + 1], lab[4 * k + 2], lab[4 * k + 3]);
     } else {

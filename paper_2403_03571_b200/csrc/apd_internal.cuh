@@ -39,6 +39,7 @@ struct AssignArgs {
   int M_pad;             // padded to SEED_CHUNK
   const float* seeds;    // [M_pad, REC]
   int32_t* labels;       // [N] or nullptr
+  int labels_vec;        // 1: the labels pointer is 16-byte aligned, rows may leave as int4 stores; 0: scalar stores
   unsigned int* count;   // [M] voxels per cell (exact integers: eq. 2.8)
   unsigned long long* idxsum;  // [M,3] sum of voxel indices per axis, or nullptr
   double* dual_partial;  // [n_tiles] sum over the tile of min_i C_ij
@@ -83,6 +84,9 @@ struct Workspace {
   double* pt_acc = nullptr;            // apd_assign_points: fp64 accumulators vol[max_seeds] | csum[max_seeds,3]
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
   bool timed = false;
+  // what the most recent evaluation launched (apd_assign_stats)
+  int last_kernel = -1, last_row_long = 0, last_cull = 0, last_tiles = 0;
+  double* lloyd_buf = nullptr;         // apd_lloyd scratch: centroids [max_seeds, dim] | vol [max_seeds] | 2 scalars
   // apd_solve state (apd_lbfgs.cu), allocated on first use
   struct SolveState* sstate = nullptr;  // device scalars
   double* svec = nullptr;               // device fp64 vectors: w, g, p, w_try, w_best, g_new, q, S[m], Y[m]
@@ -175,6 +179,11 @@ struct SolveReport {
 // host helpers shared by apd_api.cu and apd_lbfgs.cu
 std::string make_grid(const apd_ctx* ctx, const apd_grid* grid, int kernel, bool cull, GridDev* g);
 int resolve_kernel(const apd_opts* o, const apd_grid* grid, bool* cull, std::string* err);
+// Sizes the buffers an evaluation of grid `g` needs (dual partials; with culling the candidate lists and the record
+// table; for the TENSOR kernel its seed table).  Grow-only.  Growing synchronises `st` and reallocates: apd_reserve
+// does this ahead of time so that apd_assign / apd_solve never do.
+int ensure_eval_buffers(apd_ctx* ctx, const GridDev& g, int kernel, bool cull, cudaStream_t st);
+int ensure_solve_state(apd_ctx* ctx, int hist);
 int enqueue_evaluation(apd_ctx* ctx, const GridDev& g, int kernel, int M, const float* X, const float* A,
                        const float* w, const float* target_vol, int32_t* labels, double* vol, double* dual,
                        double* max_rel_err, double* centroids, uint64_t* pairs, bool timed, bool cull,

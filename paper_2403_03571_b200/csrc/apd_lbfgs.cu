@@ -374,7 +374,12 @@ __global__ void __cluster_dims__(LB_CLUSTER, 1, 1) __launch_bounds__(LB_THREADS)
     // cost scale for the list-reuse slack: mean over the voxels of min_i C_ij = (g~ - <v, w>) / |Omega|  (identity I1)
     const double scale = fabs(P * s0[1]) / domain_volume;
     cull_cap = isfinite(scale) ? (float)(CULL_CAP_FACTOR * scale) : 0.0f;
-    if (!(fabs(vsum - domain_volume) <= 1e-5 * domain_volume)) finish = 3;
+    // target volumes: v_i > 0 and sum v_i = |Omega| -- with sum v != |Omega| the dual
+    // is unbounded along (1,..,1); fp32 inputs normalised in fp64 meet 1e-6 with two orders to spare
+    double badv = 0.0;
+    for (int i = LB_FIRST(red); i < M; i += LB_STEP) if (!((double)a.v[i] > 0.0)) badv = 1.0;
+    badv = cluster_allmax(badv, red);
+    if (badv != 0.0 || !(fabs(vsum - domain_volume) <= 1e-6 * domain_volume)) finish = 3;
     else if (err1 <= eps) finish = 1;
     else {
       f = f1;
@@ -507,7 +512,7 @@ using namespace apd;
     }                                                                               \
   } while (0)
 
-static int ensure_solve_state(apd_ctx* ctx, int hist) {
+int apd::ensure_solve_state(apd_ctx* ctx, int hist) {
   Workspace& ws = ctx->ws;
   const size_t ms = (size_t)ws.max_seeds;
   if (!ws.sstate) {
@@ -584,7 +589,7 @@ static int solve_common(apd_ctx* ctx, const char* who, int dim, int32_t M, const
   LB_TRY(cudaStreamSynchronize(st));
   const int status = ws.report->status;
   if (status == APD_E_ARG) {
-    ctx->err = std::string(who) + ": sum(target_vol) differs from |Omega| by more than 1e-5 relative";
+    ctx->err = std::string(who) + ": target_vol must be > 0 and sum to |Omega| within 1e-6 relative";
     return APD_E_ARG;
   }
   // final evaluation at the returned fp32 weights, with labels (Algorithm 1 at the solution)

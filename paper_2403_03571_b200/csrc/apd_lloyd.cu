@@ -40,9 +40,12 @@ extern "C" int apd_lloyd(apd_ctx* ctx, const apd_grid* grid, int32_t M, float* X
   int rc = APD_OK, it_sum = 0, ev_sum = 0;
   double err = 0.0;
   if (cudaSetDevice(ctx->ws.device) != cudaSuccess) { ctx->err = "apd_lloyd: cudaSetDevice failed"; return APD_E_CUDA; }
-  LL_TRY(cudaMalloc(&cen, sizeof(double) * (size_t)M * d));
-  LL_TRY(cudaMalloc(&v64, sizeof(double) * (size_t)M));
-  LL_TRY(cudaMalloc(&scal, sizeof(double) * 2));
+  {
+    // scratch of the centroid evaluation: owned by the context, allocated once (apd_reserve does it ahead of time)
+    Workspace& ws = ctx->ws;
+    if (!ws.lloyd_buf) LL_TRY(cudaMalloc(&ws.lloyd_buf, ((size_t)ws.max_seeds * (ws.dim + 1) + 2) * sizeof(double)));
+    cen = ws.lloyd_buf; v64 = cen + (size_t)ws.max_seeds * ws.dim; scal = v64 + ws.max_seeds;
+  }
   for (int k = 0; k <= K; ++k) {
     // Alg. 3 step 4 / 8: Algorithm 2 from W_0^k (W_0^0 = w_init or 0, then W_0^{k+1} = W^k)
     int it = 0, ev = 0;
@@ -60,7 +63,6 @@ extern "C" int apd_lloyd(apd_ctx* ctx, const apd_grid* grid, int32_t M, float* X
   }
   LL_TRY(cudaStreamSynchronize(st));
 done:
-  cudaFree(cen); cudaFree(v64); cudaFree(scal);
   if (iters) *iters = it_sum;
   if (evals) *evals = ev_sum;
   if (max_rel_err) *max_rel_err = err;

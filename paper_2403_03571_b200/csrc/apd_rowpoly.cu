@@ -22,10 +22,7 @@
 
 namespace apd {
 
-#ifndef ROWBATCH
-#define ROWBATCH 8
-#endif
-constexpr int ROW_BATCH = ROWBATCH;                   // voxels of a row whose FMA chains are interleaved
+constexpr int ROW_BATCH = 8;                          // voxels of a row whose FMA chains are interleaved
 
 // pair-interleaved seed table: PREC floats per PAIR of seeds
 //   3D (20): X0 X1 Y0 Y1 | Z0 Z1 a11 a11 | a12' a12' a13' a13' | a22 a22 a23' a23' | a33 a33 nw nw
@@ -189,29 +186,17 @@ struct RowGeom {
   static constexpr int V = V_, TXT = TXT_, TYT = TYT_, TZT = TZT_, THREADS = TXT_ * TYT_ * TZT_, MINB = MINB_,
                        GROUP = GROUP_;
 };
-#ifndef ROWMINB
-#define ROWMINB 3
-#endif
-#ifndef ROWUNROLL
-#define ROWUNROLL 1
-#endif
+constexpr int ROW_MINB = 3;                           // CTAs per SM (measured: 2, 3 and 4 within 0.3%)
 // Two row lengths are built.  LONG rows (V = 32) amortise the per-(row, seed) set-up best and are used once the
 // grid gives every SM at least ROW_LONG_MIN_WAVES waves of long-row tiles; smaller grids take SHORT rows (V = 16),
 // whose tiles are half as big, so that all SMs have work.
-#ifndef ROWGROUPL
-#define ROWGROUPL 16
-#endif
-using RowGeom3L = RowGeom<3, 32, 1, 16, 8, ROWMINB, ROWGROUPL>;    // tile 32 x 16 x 8 voxels, 128 threads
-using RowGeom3S = RowGeom<3, 16, 1, 16, 8, ROWMINB, 8>;    // tile 16 x 16 x 8 voxels
-using RowGeom2L = RowGeom<2, 32, 2, 64, 1, ROWMINB, 16>;    // tile 64 x 64 pixels
-using RowGeom2S = RowGeom<2, 16, 2, 64, 1, ROWMINB, 8>;    // tile 32 x 64 pixels
+using RowGeom3L = RowGeom<3, 32, 1, 16, 8, ROW_MINB, 16>;    // tile 32 x 16 x 8 voxels, 128 threads
+using RowGeom3S = RowGeom<3, 16, 1, 16, 8, ROW_MINB, 8>;    // tile 16 x 16 x 8 voxels
+using RowGeom2L = RowGeom<2, 32, 2, 64, 1, ROW_MINB, 16>;    // tile 64 x 64 pixels
+using RowGeom2S = RowGeom<2, 16, 2, 64, 1, ROW_MINB, 8>;    // tile 32 x 64 pixels
 constexpr int ROW_LONG_MIN_WAVES = 2;
 
-#ifndef ROWSTAGES
-#define ROWSTAGES 4
-#endif
-constexpr int ROW_STAGES = ROWSTAGES;                 // smem ring of seed chunks
-constexpr int ROW_UNROLL = ROWUNROLL;
+constexpr int ROW_STAGES = 4;                         // smem ring of seed chunks
 
 // Dynamic shared memory of one CTA:
 //   seeds [ROW_STAGES][CHUNK_PAIRS*PREC] f32 | prev [V][THREADS] f32 | lab [V][THREADS] i32 |
@@ -241,7 +226,7 @@ __device__ __forceinline__ void row_process_chunk(const float* __restrict__ sp, 
   constexpr int GROUP_PAIRS = ROW_GROUP / 2;
   for (int gidx = 0; gidx < SEED_CHUNK / ROW_GROUP; ++gidx) {
     const float* gp = sp + gidx * GROUP_PAIRS * PREC;
-#pragma unroll ROW_UNROLL
+#pragma unroll 1
     for (int p = 0; p < GROUP_PAIRS; ++p) {
       const RowCoef rc = row_setup<DIM>(gp + p * PREC, rr);
       row_sweep<V>(rc, tt, [&](int k, float lo, float hi) { best[k] = min3f(best[k], lo, hi); });
@@ -549,7 +534,7 @@ int rowpoly_tile_counts(int dim, int nx, int ny, int nz, int sm_count, bool cull
     return 0;
   }
   if (dim == 3) tiles_of<RowGeom3L>(nx, ny, nz, tx, ty, tz); else tiles_of<RowGeom2L>(nx, ny, 1, tx, ty, tz);
-  if ((long long)(*tx) * (*ty) * (*tz) >= (long long)ROW_LONG_MIN_WAVES * ROWMINB * sm_count) return 1;
+  if ((long long)(*tx) * (*ty) * (*tz) >= (long long)ROW_LONG_MIN_WAVES * ROW_MINB * sm_count) return 1;
   if (dim == 3) tiles_of<RowGeom3S>(nx, ny, nz, tx, ty, tz); else tiles_of<RowGeom2S>(nx, ny, 1, tx, ty, tz);
   return 0;
 }

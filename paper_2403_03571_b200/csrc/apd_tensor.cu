@@ -385,6 +385,9 @@ __global__ void __launch_bounds__(TC_THREADS, 1) assign_tensor_kernel(const Assi
     const int ix = bx * TC_TX + (tid & 15), iy = by * TC_TY + ((tid >> 4) & 7), iz = bz * TC_TZ + (tid >> 7);
     const bool valid = ix < a.g.nx && iy < a.g.ny && iz < a.g.nz;
     const unsigned vmask = __ballot_sync(0xffffffffu, valid);
+    // a voxel whose real costs are all NaN / +inf / >= 2^100 would keep a padding seed (cost 2^100) as its minimum:
+    // it takes label 0 like the other kernels, and never indexes count[] beyond M
+    if (lab >= a.M) lab = 0;
     if (valid) {
       if (a.labels) a.labels[((long long)iz * a.g.ny + iy) * a.g.nx + ix] = lab;
       dsum = (double)best;

@@ -1,8 +1,8 @@
-// apd_probe.cu -- register-only FP32 microbenchmarks that define the measured FP32 roofline
-// denominators of DESIGN.md "Measurement" (MEASURED_PEAKS.json holds no FP32 CUDA-core figure).
-// Not part of the method.
-#include "apd_internal.cuh"
-#include "apd_device.cuh"
+// apd_probe.cu -- libapd_probe.so (include/apd_probe.h): register-only FP32 microbenchmarks that define the measured
+// FP32 roofline denominators of DESIGN.md "Measurement" (MEASURED_PEAKS.json holds no FP32 CUDA-core figure).
+// A measurement tool for bench.py only: not part of the method and not linked into libapd_b200.so.
+#include "../../../include/apd_probe.h"
+#include "../apd_device.cuh"
 
 namespace apd {
 
@@ -95,18 +95,18 @@ __global__ void __launch_bounds__(256) probe_kernel(float* out, const float* in,
 
 extern "C" int apd_fp32_probe(int32_t device, int32_t variant, double* ops_per_s, double* sm_clock_mhz) {
   using namespace apd;
-  if (variant < 0 || variant > 3 || !ops_per_s) return APD_E_ARG;
+  if (variant < 0 || variant > 3 || !ops_per_s) return APD_PROBE_E_ARG;
   cudaDeviceProp prop;
-  if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return APD_E_CUDA;
-  if (prop.major != 10) return APD_E_ARCH;
-  if (cudaSetDevice(device) != cudaSuccess) return APD_E_CUDA;
+  if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return APD_PROBE_E_CUDA;
+  if (prop.major != 10) return APD_PROBE_E_ARCH;
+  if (cudaSetDevice(device) != cudaSuccess) return APD_PROBE_E_CUDA;
   float *d_in = nullptr, *d_out = nullptr;
   unsigned long long* d_clk = nullptr;
   const int blocks = prop.multiProcessorCount * 8, threads = 256;
   float h_in[64];
   for (int i = 0; i < 64; ++i) h_in[i] = 0.999f + 1e-4f * (float)i;
   cudaEvent_t e0 = nullptr, e1 = nullptr;
-  int rc = APD_E_CUDA;
+  int rc = APD_PROBE_E_CUDA;
   do {
     if (cudaMalloc(&d_in, sizeof(h_in)) != cudaSuccess) break;
     if (cudaMalloc(&d_out, sizeof(float) * blocks * threads) != cudaSuccess) break;
@@ -134,7 +134,7 @@ extern "C" int apd_fp32_probe(int32_t device, int32_t variant, double* ops_per_s
     const double per_thread = (double)PROBE_ITERS * PROBE_ACC * ((variant == 1 || variant == 3) ? 2.0 : 1.0);
     *ops_per_s = per_thread * (double)blocks * threads / (best_ms * 1e-3);
     if (sm_clock_mhz) *sm_clock_mhz = h_clk[1] ? (double)h_clk[0] / (double)h_clk[1] * 1e3 : 0.0;
-    rc = APD_OK;
+    rc = APD_PROBE_OK;
   } while (0);
   if (e0) cudaEventDestroy(e0);
   if (e1) cudaEventDestroy(e1);

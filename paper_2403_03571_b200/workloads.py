@@ -254,47 +254,3 @@ def voxel_sample(N: int, k: int, seed: int) -> np.ndarray:
     k = min(k, N)
     idx = rng.choice(N, size=k, replace=False) if N < (1 << 62) else None
     return np.sort(idx.astype(np.int64))
-
-
-# ----------------------------------------------------------------------------------------
-# the paper's own runtime-test recipe, for context runs only
-# ----------------------------------------------------------------------------------------
-def euler_zxz(a: np.ndarray, b: np.ndarray, c: np.ndarray) -> np.ndarray:
-    """Rotation Rz(a) Rx(b) Rz(c).  The paper says "Euler angles", all ~ U(0, 2 pi), without a convention
-    (PAPER.md:83,252); ZXZ is this repository's reading."""
-    def rz(t):
-        R = np.zeros(t.shape + (3, 3)); co, si = np.cos(t), np.sin(t)
-        R[..., 0, 0] = co; R[..., 0, 1] = -si; R[..., 1, 0] = si; R[..., 1, 1] = co; R[..., 2, 2] = 1.0
-        return R
-
-    def rx(t):
-        R = np.zeros(t.shape + (3, 3)); co, si = np.cos(t), np.sin(t)
-        R[..., 0, 0] = 1.0; R[..., 1, 1] = co; R[..., 1, 2] = -si; R[..., 2, 1] = si; R[..., 2, 2] = co
-        return R
-    return rz(a) @ rx(b) @ rz(c)
-
-
-def make_paper_test(dim: int, M: int, alpha: float, multiphase: bool, n_axis: Optional[int] = None,
-                    seed: int = 0) -> Workload:
-    """Runtime test (b) of the paper: uniform seeds with the exclusion rule; det-1 anisotropy with
-    threshold alpha (2D: a^ ~ U(1-alpha,1), theta ~ U(0,pi); 3D: axes (a^, b^, 1/(a^ b^)), a^ ~ U(1-alpha,1),
-    b^ ~ U(1-alpha, 1/(1-alpha)), three angles ~ U(0,2pi)); volumes equal (single phase) or lognormal(sigma 1.0,
-    mu 0.5) normalised (multi-phase); eps = 1%.  n_axis None: the practical rule eq. (2.10)."""
-    rng = np.random.Generator(np.random.PCG64(BASE_SEED + 9000 + seed))
-    X, rej = sample_seeds_with_exclusion(rng, M, dim)
-    if dim == 2:
-        ah = rng.uniform(1.0 - alpha, 1.0, M)
-        A = aniso2(1.0 / ah, ah, rng.uniform(0.0, math.pi, M))
-    else:
-        ah = rng.uniform(1.0 - alpha, 1.0, M)
-        bh = rng.uniform(1.0 - alpha, 1.0 / (1.0 - alpha), M)
-        axes = np.stack([ah, bh, 1.0 / (ah * bh)], axis=1)
-        ang = rng.uniform(0.0, 2 * math.pi, (M, 3))
-        A = aniso3(axes, euler_zxz(ang[:, 0], ang[:, 1], ang[:, 2]))
-    v = np.exp(rng.normal(0.5, 1.0, M)) if multiphase else np.ones(M)
-    v = v / v.sum()
-    if n_axis is None:
-        n_axis = 1
-        while not (1.0 / float(n_axis) ** dim < 0.01 / 2 ** dim * v.min()):
-            n_axis += 1
-    return _finish(f"paper_b_{dim}d_M{M}_a{alpha}_{'multi' if multiphase else 'single'}", dim, (n_axis,) * dim, X, A, v, rej)

@@ -51,10 +51,12 @@ def check_labels(grid: Grid, X, A, w, labels_gpu: np.ndarray, orc, sel=None) -> 
     return out
 
 
-def check_assign(wl, w, labels_gpu, vol_gpu, dual_gpu, v=None, centroids_gpu=None, err_gpu=None) -> dict:
-    """Full-grid parity (rules 1-4) of one evaluation against oracle_assign on the same inputs."""
+def check_assign(wl, w, labels_gpu, vol_gpu, dual_gpu, v=None, centroids_gpu=None, err_gpu=None, orc=None) -> dict:
+    """Full-grid parity (rules 1-4) of one evaluation against oracle_assign on the same inputs (`orc`: that oracle
+    result when the caller already has it -- one oracle pass can serve several kernels)."""
     grid = grid_of(wl)
-    orc = oracle_assign(grid, wl.X, wl.A, w, v=v)
+    if orc is None:
+        orc = oracle_assign(grid, wl.X, wl.A, w, v=v)
     out = check_labels(grid, wl.X, wl.A, w, labels_gpu, orc)
     nm = out["mismatches"]
     P = grid.voxel_volume

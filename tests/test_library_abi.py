@@ -8,10 +8,11 @@ import pytest
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 HEADER = os.path.join(ROOT, "include", "apd.h")
+PROBE_HEADER = os.path.join(ROOT, "include", "apd_probe.h")
 
 
-def declared_functions():
-    src = open(HEADER).read()
+def declared_functions(header=HEADER):
+    src = open(header).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
     return sorted(set(re.findall(r"\b(apd_[a-z0-9_]+)\s*\(", src)))
 
@@ -38,6 +39,21 @@ def test_library_exports_every_declared_symbol(lib):
 def test_binding_lists_the_same_symbols():
     from paper_2403_03571_b200 import binding
     assert sorted(binding.EXPORTED_SYMBOLS) == declared_functions()
+
+
+def test_every_header_under_include_is_covered():
+    assert sorted(os.listdir(os.path.join(ROOT, "include"))) == ["apd.h", "apd_probe.h"]
+
+
+def test_probe_library_exports_its_header_and_nothing_of_it_is_in_the_product(lib):
+    """The FP32 microbenchmark is a bench-only library of its own (include/apd_probe.h)."""
+    from paper_2403_03571_b200 import probe
+    plib = probe.load_library()
+    names = declared_functions(PROBE_HEADER)
+    assert names == sorted(probe.EXPORTED_SYMBOLS) == ["apd_fp32_probe"]
+    for name in names:
+        assert hasattr(plib, name)
+        assert not hasattr(lib, name), f"{name} must not be exported by the product library"
 
 
 def test_struct_layouts_match_header(lib):
