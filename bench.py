@@ -1,23 +1,28 @@
 #!/usr/bin/env python
-"""bench.py -- headline measurement of the APD hot path on B200.
+"""bench.py -- measurement of the APD hot path on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--no-solve]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--config 1..5|all] [--kernel 0..3] [--oracle-full] [--no-solve] [--no-cpu] ...
 
-A step is ONE pass of the whole hot path -- one apd_assign evaluation through the C ABI (seed pack ->
-voxel x seed kernel with label store, histograms and dual partials -> finalize) -- on BASELINE.json's
-headline workload: config 4, 256^3 voxels x 10,000 rolled-steel-like grains (synthetic, seeded).
-Metric: G voxel-seed pairs/s.  One JSON line is printed by rank 0.
+Default run = the headline line.  A step is ONE pass of the whole hot path -- one apd_assign evaluation through the
+C ABI (seed pack -> voxel x seed kernel with label store, histograms and dual partials -> finalize) -- on
+BASELINE.json's headline workload: config 4, 256^3 voxels x 10,000 rolled-steel-like grains (synthetic, seeded), with
+the library's default kernel choice (APD_KERNEL_AUTO).  Metric: G voxel-seed pairs/s.  ONE JSON line is printed by
+rank 0; beside the contract's keys it carries the other kernels on the same workload (`kernels`), the culled
+evaluation, time-to-solve (`solve*`) and a compact record of every BASELINE config (`per_config`).
 
-N > 1 (torchrun): the path does not shard in this build ("replicas only"): every rank runs
-an independent replica of the workload on its own GPU; no data-path collective.  value = pairs of all
-ranks / max-over-ranks device time.
+--config k: the full record of config k alone (brute-force and culled evaluation, solves, the oracle timed on the host
+cores -- a FULL oracle evaluation with --oracle-full, else a bounded sample): the rows of BASELINE.md section 4.
 
---impl reference: the fp64 CPU oracle (oracle/) as it stands, on the host cores, on a bounded sample
-of the same workload.
+N > 1 (torchrun): the path does not shard in this build's headline ("replicas only"): every rank
+runs an independent replica on its own GPU, no data-path collective; value = pairs of all ranks / max-over-ranks time.
+
+--impl reference: the fp64 CPU oracle (oracle/) as it stands, on the host cores, on a bounded sample of the workload.
 """
 from __future__ import annotations
 
 import argparse
+import csv
 import json
 import os
 import subprocess
@@ -39,8 +44,10 @@ UNIT = "Gpairs/s"
 FLUSH_BYTES = 256 << 20            # > 126 MB L2
 
 
-def workload_name(wl):
-    return (f"cfg{WORKLOAD_CFG}: {'x'.join(map(str, wl.n))} voxels x {wl.M} grains, rolled-steel-like ellipsoids, "
+def workload_name(wl, cfg=WORKLOAD_CFG):
+    what = {1: "ellipses, equal areas", 2: "ellipses, lognormal areas", 3: "Haar-oriented ellipsoids",
+            4: "rolled-steel-like ellipsoids", 5: "50/50 near-isotropic / elongated ellipsoids"}[cfg]
+    return (f"cfg{cfg}: {'x'.join(map(str, wl.n))} voxels x {wl.M} grains, {what}, "
             f"one apd_assign evaluation (labels + volumes + dual) at w=0")
 
 
@@ -125,7 +132,7 @@ def measured_peaks():
 
 
 # ------------------------------------------------------------------------------------------------
-# CPU oracle leg (cpu_baseline of the default run; the whole run for --impl reference)
+# CPU oracle legs (cpu_baseline of the default run; the whole run for --impl reference)
 # ------------------------------------------------------------------------------------------------
 def oracle_sample_rate(wl, target_s: float, seed: int = 0):
     """Times oracle_assign (fp64, as it stands) on a sample of voxels of `wl` sized for ~target_s.
@@ -142,6 +149,16 @@ def oracle_sample_rate(wl, target_s: float, seed: int = 0):
     oracle_assign(grid, wl.X, wl.A, wl.w0, sel=sel, diagnostics=False)
     dt = time.perf_counter() - t
     return len(sel) * wl.M / dt, num_threads(), len(sel), dt
+
+
+def oracle_full_time(wl):
+    """One FULL oracle evaluation of `wl` (all voxels x all seeds, with the reductions), timed."""
+    from oracle.apd_oracle import Grid, oracle_assign, num_threads
+    grid = Grid(wl.dim, wl.n, wl.lo, wl.hi)
+    t = time.perf_counter()
+    oracle_assign(grid, wl.X, wl.A, wl.w0, v=wl.v, diagnostics=False)
+    dt = time.perf_counter() - t
+    return {"seconds": dt, "cores": num_threads(), "gpairs": wl.pairs / dt / 1e9, "kind": "full evaluation"}
 
 
 def cpu_baseline(wl, target_s: float):
@@ -180,19 +197,174 @@ def run_reference(args):
 # ------------------------------------------------------------------------------------------------
 # our arm
 # ------------------------------------------------------------------------------------------------
-# Algorithmic FP32 work per voxel-seed pair of each kernel form:
-#   DIRECT  : 3 FADD + 3 FMUL + 6 FFMA               = 18 flop   (12 FP32 instructions, 3D)
-#   ROWPOLY : 1.5 FMA (voxels at +-tau share the even part) + 7 FMA set-up per (row of 32 voxels, seed)
-#             = 3 + 14/32 = 3.4375 flop (the once-per-(tile, seed) re-expansion, ~25 flop / 4096 voxels, not counted)
-#   TENSOR  : the K = 32 bf16 contraction of the lifted form = 64 tensor-core flop per pair (30 of the 32 K slots carry
-#             a product); reported against the MEASURED bf16 peak, bound "tensor" -- its real limit is the CUDA-core
-#             argmin epilogue
-FLOP_PER_PAIR = {1: 18.0, 2: 3.0 + 14.0 / 32.0, 3: 64.0}
-KERNEL_NAME = {1: "assign_direct_kernel<3>", 2: "assign_rowpoly_kernel<3>", 3: "assign_tensor_kernel"}
+K_AUTO, K_DIRECT, K_ROWPOLY, K_TENSOR = 0, 1, 2, 3
+KERNEL_LABEL = {K_DIRECT: "assign_direct_kernel", K_ROWPOLY: "assign_rowpoly_kernel", K_TENSOR: "assign_tensor_kernel"}
 FP32_LANES_PER_SM = 128
-# dram__bytes_read.sum + dram__bytes_write.sum of one assign_rowpoly_kernel launch on this workload, from the
-# `ncu --set full` capture summarised in profiles/ (None until a capture exists)
-NCU_TRAFFIC_BYTES = 489472 + 15261696      # profiles/r01_assign_rowpoly_full.md (labels mostly still in L2 at kernel end)
+ALU_LANES_PER_SM = 64              # 4 SMSPs x 16 lanes: the pipe that executes the 3-input min (B300_MICROARCH.md)
+LAUNCHES = {K_DIRECT: ["pack_seeds_kernel", "assign_direct_kernel", "finalize_kernel"],
+            K_ROWPOLY: ["pack_pairs_kernel", "assign_rowpoly_kernel", "finalize_kernel"],
+            K_TENSOR: ["pack_seeds_kernel", "pack_qfix_kernel", "assign_tensor_kernel", "finalize_kernel"]}
+
+
+def executed_flop_per_pair(kernel: int, dim: int, row_long: int) -> float:
+    """FP32 (or tensor-core) flop per voxel-seed pair the COMPILED kernel executes (SASS counts
+    confirmed by the ncu captures under profiles/):
+      DIRECT 3D : per pair 1 FADD + 1 FMUL + 5 FFMA = 12 flop, + per (seed, thread of 8 voxels) the terms in dy, dz
+                  alone (2 FADD + 2 FMUL + 1 FFMA = 6 flop)                     -> 12.75   (the written form is 18)
+      DIRECT 2D : per pair 1 FADD + 1 FMUL + 3 FFMA = 8, + (1 FADD + 1 FMUL) / 8            ->  8.25
+      ROWPOLY   : 1.5 FMA per pair + 7 (3D) / 9 (2D) packed set-up operations per (row of V voxels, seed), V = 32 or 16
+      TENSOR    : the K = 32 bf16 contraction the tensor core executes = 64 flop (the method's 10 monomials are 20)"""
+    if kernel == K_DIRECT:
+        return 12.75 if dim == 3 else 8.25
+    if kernel == K_ROWPOLY:
+        V = 32 if row_long else 16
+        return 3.0 + (14.0 if dim == 3 else 18.0) / V
+    return 64.0
+
+
+def ncu_traffic_bytes(kernel: int):
+    """dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the kernel on the headline workload, read from the
+    committed `ncu --set full` raw page (profiles/*.csv; the .md beside each names its command).  None if absent."""
+    name = {K_DIRECT: "r02_assign_direct_raw.csv", K_ROWPOLY: "r02_assign_rowpoly_raw.csv",
+            K_TENSOR: "r02_assign_tensor_raw.csv"}[kernel]
+    path = os.path.join(ROOT, "profiles", name)
+    if not os.path.exists(path):
+        return None
+    try:
+        rows = list(csv.reader(open(path)))
+        hdr, units, vals = rows[0], rows[1], rows[2]
+        scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+        tot = 0.0
+        for key in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+            i = hdr.index(key)
+            tot += float(vals[i]) * scale[units[i]]
+        return int(tot)
+    except Exception:
+        return None
+
+
+class Bench:
+    """One workload resident on the device plus the buffers of the calls."""
+
+    def __init__(self, apd, torch, cfg: int, local: int):
+        self.apd, self.torch, self.cfg = apd, torch, cfg
+        self.dev = torch.device("cuda", local)
+        wl = self.wl = workloads.make_config(cfg)
+        self.ctx = apd.ApdContext(wl.dim, wl.M, device=local)
+        self.grid = apd.make_grid(wl.dim, wl.n, wl.lo, wl.hi)
+        dev = self.dev
+        self.X = torch.from_numpy(wl.X).to(dev); self.A = torch.from_numpy(wl.A).to(dev)
+        self.v = torch.from_numpy(wl.v).to(dev); self.w = torch.zeros(wl.M, dtype=torch.float32, device=dev)
+        self.labels = torch.empty(wl.N, dtype=torch.int32, device=dev)
+        self.vol = torch.zeros(wl.M, dtype=torch.float64, device=dev)
+        self.dual = torch.zeros(1, dtype=torch.float64, device=dev)
+        self.err = torch.zeros(1, dtype=torch.float64, device=dev)
+        self.pairs_t = torch.zeros(1, dtype=torch.int64, device=dev)
+
+    def step(self, opts):
+        self.ctx.apd_assign(self.grid, self.X, self.A, self.w, target_vol=self.v, labels=self.labels, vol=self.vol,
+                            dual=self.dual, max_rel_err=self.err, pairs_evaluated=self.pairs_t, opts=opts)
+
+    def time_assign(self, opts, flush, reps: int, warm: int = 2):
+        """`reps` evaluations, each bracketed by CUDA events on the launching stream (L2 flushed before each, outside
+        the events).  Returns (step ms list, dominant-kernel ms list, stats of the last launch)."""
+        torch = self.torch
+        for _ in range(warm):
+            flush.zero_(); self.step(opts)
+        torch.cuda.synchronize()
+        ms, kms = [], []
+        for _ in range(reps):
+            flush.zero_()
+            e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+            e0.record(); self.step(opts); e1.record()
+            torch.cuda.synchronize()
+            ms.append(e0.elapsed_time(e1))
+            kms.append(self.ctx.assign_stats()["kernel_ms"])
+        return ms, kms, self.ctx.assign_stats()
+
+    def solve(self, cull: int, kernel: int, max_iters: int, reps: int):
+        torch, apd, wl = self.torch, self.apd, self.wl
+        secs, info = [], None
+        for _ in range(reps):
+            wS = torch.zeros(wl.M, dtype=torch.float32, device=self.dev)
+            torch.cuda.synchronize()
+            ts = time.perf_counter()
+            info = self.ctx.apd_solve(self.grid, self.X, self.A, self.v, wl.eps, w=wS, labels=self.labels, vol=self.vol,
+                                      opts=apd.make_opts(kernel=kernel, cull=cull, max_iters=max_iters))
+            torch.cuda.synchronize()
+            secs.append(time.perf_counter() - ts)
+        st = self.ctx.assign_stats()
+        out = {"seconds": secs[-1], "first_call_seconds": secs[0], "tol": wl.eps, "cull": cull, "status": info.status,
+               "converged": info.status == 0, "iters": info.iters, "evals": info.evals, "max_rel_err": info.max_rel_err,
+               "dual": info.dual, "kernel": KERNEL_LABEL[st["kernel"]]}
+        if cull:
+            out["cull_rebuilds"] = self.ctx.solve_stats()[1]
+        return out
+
+    def close(self):
+        self.ctx.close()
+
+
+def kernel_record(b: Bench, kernel: int, cull: int, flush, reps: int, peak_fp32: float, peak_bf16: float, sm_count: int,
+                  sm_mhz: float):
+    """Timing + roofline fractions of one kernel choice on b's workload."""
+    wl = b.wl
+    ms, kms, st = b.time_assign(b.apd.make_opts(kernel=kernel, cull=cull), flush, reps)
+    km = float(np.mean(kms))
+    k = st["kernel"]
+    pairs_eval = int(b.pairs_t.item())
+    rec = {"kernel": KERNEL_LABEL[k] + (f"<{wl.dim}, V={32 if st['row_long'] else 16}>" if k == K_ROWPOLY else
+                                       (f"<{wl.dim}>" if k == K_DIRECT else "")) + (" (culled)" if st["cull"] else ""),
+           "ms_per_step": float(np.mean(ms)), "kernel_ms": km, "n_tiles": st["n_tiles"],
+           "gpairs": wl.pairs / (float(np.mean(ms)) * 1e-3) / 1e9}
+    if st["cull"]:
+        rec.update(pairs_evaluated=pairs_eval, pruned_fraction=1.0 - pairs_eval / wl.pairs,
+                   evaluated_gpairs_kernel=pairs_eval / (km * 1e-3) / 1e9)
+        return rec
+    fpp = executed_flop_per_pair(k, wl.dim, st["row_long"])
+    ach = fpp * wl.pairs / (km * 1e-3) / 1e12
+    rec.update(flop_per_pair=fpp, kernel_gpairs=wl.pairs / (km * 1e-3) / 1e9)
+    if k == K_TENSOR:
+        min_rate = 0.5 * wl.pairs / (km * 1e-3)                     # 3-input min instructions (thread level) per s
+        alu_peak = sm_count * ALU_LANES_PER_SM * sm_mhz * 1e6
+        rec.update(tensor_tflops_k32=ach, frac_bf16_k32=ach / peak_bf16,
+                   tensor_tflops_method=20.0 * wl.pairs / (km * 1e-3) / 1e12,
+                   frac_bf16_method=20.0 * wl.pairs / (km * 1e-3) / 1e12 / peak_bf16,
+                   alu_min_frac=min_rate / alu_peak)
+    else:
+        rec.update(fp32_tflops=ach, frac_fp32=ach / peak_fp32)
+    return rec
+
+
+def config_record(apd, torch, cfg: int, local: int, flush, args, peaks_t, full: bool):
+    """Everything BASELINE.md section 4 asks for one config (full) or its compact form (default line)."""
+    b = Bench(apd, torch, cfg, local)
+    wl = b.wl
+    reps = 5 if wl.pairs > 1e11 else 10
+    out = {"grid": list(wl.n), "grains": wl.M, "pairs": wl.pairs}
+    out["assign"] = kernel_record(b, K_AUTO, 0, flush, reps, *peaks_t)
+    out["assign_culled"] = kernel_record(b, K_AUTO, 1, flush, reps, *peaks_t)
+    if not args.no_solve:
+        out["solve_culled"] = b.solve(1, K_AUTO, args.solve_max_iters, 2)
+        if full and cfg <= 4:
+            out["solve_brute_force"] = b.solve(0, K_AUTO, args.solve_max_iters, 1)
+    if full:
+        if wl.dim == 3:
+            for k, name in ((K_DIRECT, "direct"), (K_ROWPOLY, "rowpoly"), (K_TENSOR, "tensor")):
+                out["assign_" + name] = kernel_record(b, k, 0, flush, 3, *peaks_t)
+        else:
+            out["assign_direct"] = kernel_record(b, K_DIRECT, 0, flush, 3, *peaks_t)
+        if not args.no_cpu:
+            if args.oracle_full and cfg <= 4:
+                out["oracle"] = oracle_full_time(wl)
+            else:
+                rate, cores, nvox, dt = oracle_sample_rate(wl, args.cpu_seconds)
+                out["oracle"] = {"gpairs": rate / 1e9, "cores": cores, "kind": f"sample of {nvox} voxels, {dt:.1f} s",
+                                 "seconds_extrapolated_full": wl.pairs / rate}
+    b.close()
+    del b
+    torch.cuda.empty_cache()
+    return out
 
 
 def run_ours(args):
@@ -211,21 +383,27 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=dev)
     apd.load_library()
 
-    wl = workloads.make_config(WORKLOAD_CFG)
-    ctx = apd.ApdContext(wl.dim, wl.M, device=local)
-    grid = apd.make_grid(wl.dim, wl.n, wl.lo, wl.hi)
-    X = torch.from_numpy(wl.X).to(dev); A = torch.from_numpy(wl.A).to(dev)
-    v = torch.from_numpy(wl.v).to(dev); w = torch.zeros(wl.M, dtype=torch.float32, device=dev)
-    labels = torch.empty(wl.N, dtype=torch.int32, device=dev)
-    vol = torch.zeros(wl.M, dtype=torch.float64, device=dev)
-    dual = torch.zeros(1, dtype=torch.float64, device=dev)
-    err = torch.zeros(1, dtype=torch.float64, device=dev)
+    peaks = measured_peaks()
+    sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
+    sm_max_mhz = float(peaks.get("sm_max_mhz", 1965.0))
+    peak_fp32 = sm_count * FP32_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
+    peak_bf16 = float(peaks.get("bf16_tflops", 1590.0))
+    peaks_t = (peak_fp32, peak_bf16, sm_count, sm_max_mhz)
     flush = torch.empty(FLUSH_BYTES, dtype=torch.uint8, device=dev)
-    opts = apd.make_opts(kernel=args.kernel)
-    kernel_id = args.kernel if args.kernel else apd.KERNEL_ROWPOLY
 
-    def step():
-        ctx.apd_assign(grid, X, A, w, target_vol=v, labels=labels, vol=vol, dual=dual, max_rel_err=err, opts=opts)
+    if args.config:
+        # ---- the per-config record(s) of BASELINE.md section 4: one JSON line each, rank 0 only ----
+        if rank == 0:
+            for cfg in ([1, 2, 3, 4, 5] if args.config == "all" else [int(args.config)]):
+                rec = config_record(apd, torch, cfg, local, flush, args, peaks_t, full=True)
+                print(json.dumps({"config_record": cfg, **rec}), flush=True)
+        if world > 1:
+            dist.barrier(); dist.destroy_process_group()
+        return
+
+    b = Bench(apd, torch, WORKLOAD_CFG, local)
+    wl = b.wl
+    opts = apd.make_opts(kernel=args.kernel)
 
     def barrier():
         if world > 1:
@@ -233,8 +411,10 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     for _ in range(max(args.warmup, 3)):
-        flush.zero_(); step()
+        flush.zero_(); b.step(opts)
     barrier()
+    st = b.ctx.assign_stats()
+    kernel_id = st["kernel"]
 
     # ---- timed region: K steps, each bracketed by CUDA events on the launching stream; the L2 flush between
     #      steps sits outside the event pairs ----
@@ -247,21 +427,21 @@ def run_ours(args):
     for i in range(args.steps):
         flush.zero_()
         ev[i][0].record()
-        step()
+        b.step(opts)
         ev[i][1].record()
         if i % 8 == 7 or i == args.steps - 1:
             torch.cuda.synchronize()
     barrier()
     t1 = time.time()
     clocks = sampler.stop(t0, t1)
-    step_ms = [a.elapsed_time(b) for a, b in ev]
+    step_ms = [a.elapsed_time(c) for a, c in ev]
     total_ms = float(sum(step_ms))
 
     # the dominant kernel alone (library-side CUDA events around the launch, same stream), K more launches
     k_ms = []
     for i in range(args.steps):
-        flush.zero_(); step(); torch.cuda.synchronize()
-        k_ms.append(ctx.last_kernel_ms())
+        flush.zero_(); b.step(opts); torch.cuda.synchronize()
+        k_ms.append(b.ctx.assign_stats()["kernel_ms"])
     kernel_ms = float(np.mean(k_ms))
 
     total_ms = max_over_ranks(total_ms, world, dev)
@@ -276,12 +456,12 @@ def run_ours(args):
     hvol = torch.empty(wl.M, dtype=torch.float64).pin_memory()
     e2e_steps = max(3, min(args.steps, 10))
     for _ in range(2):
-        ctx.apd_assign_host(grid, hX, hA, hw, target_vol=hv, labels=hlab, vol=hvol, opts=opts)
+        b.ctx.apd_assign_host(b.grid, hX, hA, hw, target_vol=hv, labels=hlab, vol=hvol, opts=opts)
     barrier()
     e2e_each = []
     for _ in range(e2e_steps):
         te = time.perf_counter()
-        ctx.apd_assign_host(grid, hX, hA, hw, target_vol=hv, labels=hlab, vol=hvol, opts=opts)   # synchronous
+        b.ctx.apd_assign_host(b.grid, hX, hA, hw, target_vol=hv, labels=hlab, vol=hvol, opts=opts)   # synchronous
         e2e_each.append(time.perf_counter() - te)
     e2e_s = float(np.median(e2e_each))       # per-call wall times; the median shrugs off a host hiccup (max reported)
     e2e_s = max_over_ranks(e2e_s, world, dev)
@@ -290,21 +470,30 @@ def run_ours(args):
 
     line = None
     if rank == 0:
-        peaks = measured_peaks()
-        sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
-        sm_max_mhz = float(peaks.get("sm_max_mhz", 1965.0))
-        peak_tflops = sm_count * FP32_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
-        ach = FLOP_PER_PAIR[kernel_id] * wl.pairs / (kernel_ms * 1e-3) / 1e12
-        bf16_peak = float(peaks.get("bf16_tflops", 1662.1))
-        roofline = {"bound": "tensor" if kernel_id == 3 else "alu", "kernel": KERNEL_NAME[kernel_id],
-                    "achieved": ach, "peak": bf16_peak if kernel_id == 3 else peak_tflops, "unit": "TFLOP/s",
-                    "frac": ach / (bf16_peak if kernel_id == 3 else peak_tflops),
-                    "traffic": NCU_TRAFFIC_BYTES if kernel_id == 2 else None, "kernel_ms": kernel_ms,
-                    "flop_per_pair": FLOP_PER_PAIR[kernel_id],
-                    "peak_is": ("MEASURED_PEAKS.json bf16_tflops (burst, cuBLAS 8192^3)" if kernel_id == 3 else
-                                f"{sm_count} SMs x {FP32_LANES_PER_SM} FP32 lanes x 2 flop x {sm_max_mhz:.0f} MHz "
-                                "(guide unit counts and MEASURED_PEAKS.json sm_max_mhz; no FP32 figure is measured there)"),
-                    "label_write_GBps": 4.0 * wl.N / (kernel_ms * 1e-3) / 1e9}
+        fpp = executed_flop_per_pair(kernel_id, wl.dim, st["row_long"])
+        ach = fpp * wl.pairs / (kernel_ms * 1e-3) / 1e12
+        if kernel_id == K_TENSOR:
+            alu_peak = sm_count * ALU_LANES_PER_SM * sm_max_mhz * 1e6
+            roofline = {"bound": "tensor", "kernel": KERNEL_LABEL[kernel_id], "achieved": ach, "peak": peak_bf16,
+                        "unit": "TFLOP/s", "frac": ach / peak_bf16, "traffic": ncu_traffic_bytes(kernel_id),
+                        "kernel_ms": kernel_ms, "flop_per_pair": fpp,
+                        "peak_is": "MEASURED_PEAKS.json bf16_tflops (burst, cuBLAS 8192^3), of measured"
+                                   if "bf16_tflops" in peaks else "1590 TFLOP/s, of fallback",
+                        "counts": "the K = 32 bf16 contraction the tensor core executes per pair (10 monomials x 3 "
+                                  "coefficient parts + 2 pad); the method's own contraction is 10 monomials = 20 flop",
+                        "frac_method_work": 20.0 * wl.pairs / (kernel_ms * 1e-3) / 1e12 / peak_bf16,
+                        "alu_pipe": {"what": "the argmin epilogue: one 3-input min.f32 per 2 pairs on the ALU pipe "
+                                             "(16 lanes per SM sub-partition), the unit ncu shows busiest",
+                                     "achieved_Tmin_per_s": 0.5 * wl.pairs / (kernel_ms * 1e-3) / 1e12,
+                                     "peak_Tinstr_per_s": alu_peak / 1e12,
+                                     "frac": 0.5 * wl.pairs / (kernel_ms * 1e-3) / alu_peak}}
+        else:
+            roofline = {"bound": "alu", "kernel": KERNEL_LABEL[kernel_id], "achieved": ach, "peak": peak_fp32,
+                        "unit": "TFLOP/s", "frac": ach / peak_fp32, "traffic": ncu_traffic_bytes(kernel_id),
+                        "kernel_ms": kernel_ms, "flop_per_pair": fpp,
+                        "peak_is": f"{sm_count} SMs x {FP32_LANES_PER_SM} FP32 lanes x 2 flop x {sm_max_mhz:.0f} MHz (guide "
+                                   "unit counts and MEASURED_PEAKS.json sm_max_mhz; no FP32 figure is measured there)"}
+        roofline["label_write_GBps"] = 4.0 * wl.N / (kernel_ms * 1e-3) / 1e9
         extra = {}
         if not args.no_probe:
             try:
@@ -314,110 +503,39 @@ def run_ours(args):
                 p3, _ = probe.apd_fp32_probe(3, local)
                 extra["fp32_probe"] = {"ffma_tflops": 2 * p0 / 1e12, "ffma2_tflops": 2 * p1 / 1e12,
                                        "rowpoly_mix_gpairs": p3 / 1e9, "sm_mhz": mhz0}
-                roofline["frac_of_rowpoly_mix_probe"] = (wl.pairs / (kernel_ms * 1e-3)) / p3
             except Exception as e:  # the probe is context, never the headline
                 extra["fp32_probe"] = {"error": str(e)}
-        if not args.no_direct and kernel_id != 1:
-            # the un-hoisted 12-instruction reference kernel north_star's ">= 60% of FP32 peak" is read against
-            o1 = apd.make_opts(kernel=apd.KERNEL_DIRECT)
-            d_ms = []
-            for _ in range(3):
-                flush.zero_()
-                ctx.apd_assign(grid, X, A, w, target_vol=v, labels=labels, vol=vol, dual=dual, max_rel_err=err, opts=o1)
-                torch.cuda.synchronize()
-                d_ms.append(ctx.last_kernel_ms())
-            dm = float(np.mean(d_ms[1:]))
-            dach = FLOP_PER_PAIR[1] * wl.pairs / (dm * 1e-3) / 1e12
-            extra["roofline_direct"] = {"bound": "alu", "kernel": "assign_direct_kernel<3>", "achieved": dach,
-                                        "peak": peak_tflops, "unit": "TFLOP/s", "frac": dach / peak_tflops,
-                                        "kernel_ms": dm, "gpairs": wl.pairs / (dm * 1e-3) / 1e9, "flop_per_pair": 18.0}
-        if not args.no_direct and kernel_id != 3:
-            # row a8: the tensor-core lift of the cost matrix (opts.kernel = APD_KERNEL_TENSOR), same workload
-            o3 = apd.make_opts(kernel=apd.KERNEL_TENSOR)
-            t_ms = []
-            for _ in range(4):
-                flush.zero_()
-                ctx.apd_assign(grid, X, A, w, target_vol=v, labels=labels, vol=vol, dual=dual, max_rel_err=err, opts=o3)
-                torch.cuda.synchronize()
-                t_ms.append(ctx.last_kernel_ms())
-            tm = float(np.mean(t_ms[1:]))
-            tach = FLOP_PER_PAIR[3] * wl.pairs / (tm * 1e-3) / 1e12
-            extra["roofline_tensor"] = {"bound": "tensor", "kernel": "assign_tensor_kernel", "achieved": tach,
-                                        "peak": bf16_peak, "unit": "TFLOP/s", "frac": tach / bf16_peak, "kernel_ms": tm,
-                                        "gpairs": wl.pairs / (tm * 1e-3) / 1e9, "flop_per_pair": 64.0,
-                                        "peak_is": "MEASURED_PEAKS.json bf16_tflops (burst, cuBLAS 8192^3)",
-                                        "note": "K = 32 contraction per pair; paced by its CUDA-core argmin epilogue (one "
-                                                "3-input min per 2 pairs on the half-rate ALU pipe) and by the per-M-tile "
-                                                "accumulator ring, not by the tensor pipe (DESIGN.md 9)"}
+        if not args.no_kernels:
+            # every kernel the library owns on the same workload (3 launches each): executed-flop fractions
+            extra["kernels"] = {name: kernel_record(b, k, 0, flush, 3, *peaks_t)
+                                for k, name in ((K_DIRECT, "direct"), (K_ROWPOLY, "rowpoly"), (K_TENSOR, "tensor"))}
         if not args.no_solve:
-            pairs_t = torch.zeros(1, dtype=torch.int64, device=dev)
-            oc = apd.make_opts(kernel=args.kernel, cull=1)
-            c_ms = []
-            for _ in range(5):
-                flush.zero_()
-                e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
-                e0.record()
-                ctx.apd_assign(grid, X, A, w, target_vol=v, labels=labels, vol=vol, dual=dual, max_rel_err=err,
-                               pairs_evaluated=pairs_t, opts=oc)
-                e1.record(); torch.cuda.synchronize()
-                c_ms.append(e0.elapsed_time(e1))
-            cm = float(np.mean(c_ms[2:]))
-            extra["culled_assign"] = {"workload": f"cfg{WORKLOAD_CFG}, opts.cull=1 (exact tile culling, labels identical)",
-                                      "ms_per_step": cm, "pairs_evaluated": int(pairs_t.item()),
-                                      "pruned_fraction": 1.0 - pairs_t.item() / wl.pairs,
-                                      "effective_gpairs": wl.pairs / (cm * 1e-3) / 1e9}
-
-            def solve_leg(ctx_, grid_, X_, A_, v_, wl_, labels_, vol_, cull):
-                secs = []
-                for _ in range(2 if cull else 1):    # culled: the first call also allocates the workspace (cold)
-                    wS = torch.zeros(wl_.M, dtype=torch.float32, device=dev)
-                    torch.cuda.synchronize()
-                    ts = time.perf_counter()
-                    info = ctx_.apd_solve(grid_, X_, A_, v_, wl_.eps, w=wS, labels=labels_, vol=vol_,
-                                          opts=apd.make_opts(kernel=args.kernel, cull=cull, max_iters=args.solve_max_iters))
-                    torch.cuda.synchronize()
-                    secs.append(time.perf_counter() - ts)
-                return {"seconds": secs[-1], "first_call_seconds": secs[0], "tol": wl_.eps, "cull": cull,
-                        "status": info.status, "iters": info.iters, "evals": info.evals,
-                        "max_rel_err": info.max_rel_err, "dual": info.dual}
-
-            extra["solve"] = dict(workload=f"cfg{WORKLOAD_CFG} apd_solve", **solve_leg(ctx, grid, X, A, v, wl, labels, vol, 1))
-            extra["solve_brute_force"] = dict(workload=f"cfg{WORKLOAD_CFG} apd_solve",
-                                              **solve_leg(ctx, grid, X, A, v, wl, labels, vol, 0))
-            if not args.no_cfg5:
-                wl5 = workloads.make_config(5)
-                ctx5 = apd.ApdContext(wl5.dim, wl5.M, device=local)
-                grid5 = apd.make_grid(wl5.dim, wl5.n, wl5.lo, wl5.hi)
-                X5 = torch.from_numpy(wl5.X).to(dev); A5 = torch.from_numpy(wl5.A).to(dev)
-                v5 = torch.from_numpy(wl5.v).to(dev)
-                lab5 = torch.empty(wl5.N, dtype=torch.int32, device=dev)
-                vol5 = torch.zeros(wl5.M, dtype=torch.float64, device=dev)
-                extra["solve_cfg5"] = dict(workload=f"cfg5 apd_solve: {'x'.join(map(str, wl5.n))} voxels x {wl5.M} grains",
-                                           **solve_leg(ctx5, grid5, X5, A5, v5, wl5, lab5, vol5, 1))
-                w5 = torch.zeros(wl5.M, dtype=torch.float32, device=dev)
-                ctx5.apd_assign(grid5, X5, A5, w5, target_vol=v5, labels=lab5, vol=vol5, dual=dual, max_rel_err=err,
-                                pairs_evaluated=pairs_t, opts=oc)
-                torch.cuda.synchronize()
-                extra["solve_cfg5"]["pruned_fraction_at_w0"] = 1.0 - pairs_t.item() / wl5.pairs
-                del lab5
+            extra["culled_assign"] = kernel_record(b, K_AUTO, 1, flush, 5, *peaks_t)
+            extra["solve"] = dict(workload=f"cfg{WORKLOAD_CFG} apd_solve, opts.cull=1",
+                                  **b.solve(1, K_AUTO, args.solve_max_iters, 2))
+            extra["solve_brute_force"] = dict(workload=f"cfg{WORKLOAD_CFG} apd_solve, brute force",
+                                              **b.solve(0, args.kernel, args.solve_max_iters, 1))
         cb = None
         if world == 1 and not args.no_cpu:
             cb = cpu_baseline(wl, args.cpu_seconds)
+        b.close()
+        del b
+        torch.cuda.empty_cache()
+        if not args.no_per_config:
+            extra["per_config"] = {str(c): config_record(apd, torch, c, local, flush, args, peaks_t, full=False)
+                                   for c in (1, 2, 3, 5)}
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                 "config": {"workload": workload_name(wl), "l2": f"flushed between steps ({FLUSH_BYTES >> 20} MiB write)",
-                           "multi_gpu": "replicas only (no data-path collective)", "kernel": kernel_id},
+                           "multi_gpu": "replicas only (no data-path collective)",
+                           "kernel": KERNEL_LABEL[kernel_id], "kernel_requested": args.kernel},
                 "clocks": clocks, "roofline": roofline, "cpu_baseline": cb,
                 "e2e": {"value": world * wl.pairs / e2e_s / 1e9, "unit": UNIT, "h2d_bytes_per_step": h2d,
                         "d2h_bytes_per_step": d2h, "ms_per_step": e2e_s * 1e3, "ms_per_step_max": max(e2e_each) * 1e3,
                         "steps": e2e_steps,
                         "call": "apd_assign_host (pinned host buffers; H2D/D2H copies inside, device scratch kept by the context)"},
-                "gpu_launches": (4 if kernel_id == 3 else 3) * args.steps,
-                "launches_per_step": {1: ["pack_seeds_kernel", "assign_direct_kernel", "finalize_kernel"],
-                                      2: ["pack_pairs_kernel", "assign_rowpoly_kernel", "finalize_kernel"],
-                                      3: ["pack_seeds_kernel", "pack_qfix_kernel", "assign_tensor_kernel",
-                                          "finalize_kernel"]}[kernel_id]}
+                "gpu_launches": len(LAUNCHES[kernel_id]) * args.steps, "launches_per_step": LAUNCHES[kernel_id]}
         line.update(extra)
     if world > 1:
         dist.barrier()
@@ -431,26 +549,14 @@ def run_solve_only(args):
     command the ncu launch list under profiles/ is taken from).  Prints one JSON line."""
     import torch
     from paper_2403_03571_b200 import binding as apd
-    dev = torch.device("cuda", int(os.environ.get("LOCAL_RANK", "0")))
-    torch.cuda.set_device(dev)
-    wl = workloads.make_config(WORKLOAD_CFG)
-    ctx = apd.ApdContext(wl.dim, wl.M, device=dev.index)
-    grid = apd.make_grid(wl.dim, wl.n, wl.lo, wl.hi)
-    X = torch.from_numpy(wl.X).to(dev); A = torch.from_numpy(wl.A).to(dev); v = torch.from_numpy(wl.v).to(dev)
-    labels = torch.empty(wl.N, dtype=torch.int32, device=dev)
-    vol = torch.zeros(wl.M, dtype=torch.float64, device=dev)
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    b = Bench(apd, torch, int(args.config) if args.config and args.config != "all" else WORKLOAD_CFG, local)
     out = None
     for _ in range(max(1, args.warmup) + 1):
-        wS = torch.zeros(wl.M, dtype=torch.float32, device=dev)
-        torch.cuda.synchronize()
-        ts = time.perf_counter()
-        info = ctx.apd_solve(grid, X, A, v, wl.eps, w=wS, labels=labels, vol=vol,
-                             opts=apd.make_opts(cull=1, max_iters=args.solve_max_iters))
-        torch.cuda.synchronize()
-        out = {"metric": "APD time-to-solve at 1% vol tol", "value": time.perf_counter() - ts, "unit": "s",
-               "higher_is_better": False, "workload": f"cfg{WORKLOAD_CFG} apd_solve, opts.cull=1", "status": info.status,
-               "iters": info.iters, "evals": info.evals, "max_rel_err": info.max_rel_err,
-               "cull_rebuilds": ctx.solve_stats()[1]}
+        r = b.solve(1, K_AUTO, args.solve_max_iters, 1)
+        out = {"metric": "APD time-to-solve at 1% vol tol", "value": r["seconds"], "unit": "s", "higher_is_better": False,
+               "workload": f"cfg{b.cfg} apd_solve, opts.cull=1", **r}
     print(json.dumps(out), flush=True)
 
 
@@ -461,11 +567,13 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 DIRECT, 2 ROWPOLY, 3 TENSOR")
+    ap.add_argument("--config", default="", help="1..5 or all: print the full per-config record(s) instead of the headline line")
+    ap.add_argument("--oracle-full", action="store_true", help="--config: time one FULL oracle evaluation (cfg 1-4)")
     ap.add_argument("--no-solve", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-probe", action="store_true")
-    ap.add_argument("--no-direct", action="store_true")
-    ap.add_argument("--no-cfg5", action="store_true")
+    ap.add_argument("--no-kernels", action="store_true", help="skip the other kernels on the headline workload")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the compact records of configs 1, 2, 3, 5")
     ap.add_argument("--solve-only", action="store_true", help="only the culled apd_solve of the headline workload")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--solve-max-iters", type=int, default=1000)

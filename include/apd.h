@@ -237,6 +237,44 @@ int apd_solve_host(apd_ctx* ctx, const apd_grid* grid, int32_t M,
                    int32_t* iters, int32_t* evals, double* max_rel_err, double* dual,
                    const apd_opts* opts);
 
+/* ---- voxel-slab sharding ---------------------------------------------------------------
+ * Voxels are independent and the only cross-voxel coupling of the method is the sum of per-cell counters (eq. 2.8,
+ * PAPER.md:138-140) and of the minima (eq. 2.7).  A rank that owns planes [lo, lo + n) of the grid's LAST axis (z in
+ * 3D, y in 2D) evaluates them with the same arithmetic as the whole-grid call (voxel centres are formed from the
+ * GLOBAL index) and leaves RAW counters; adding the counter blocks of all slabs of a partition word by word, as
+ * unsigned 64-bit integers, gives exactly the counters of the whole grid:
+ *     counters = [ count u64 x M | (with_idxsum) index sums u64 x 3M | layer sums of min-costs, fp64 bit patterns ]
+ * (a layer = apd_slab_align(dim) planes; each layer sum is written by the one slab that owns the layer, every other
+ * slab leaves 0 there, so the integer addition reproduces the fp64 bits and the dual is identical, bit for bit, to the
+ * whole-grid call's whatever the number of slabs).  slab.lo must be a multiple of apd_slab_align(dim), and slab.n too
+ * unless the slab ends at the grid's last plane.  The seeds (<= 1 MB) and the L-BFGS state are replicated. */
+typedef struct { int32_t lo, n; } apd_slab;
+int32_t apd_slab_align(int32_t dim);                                   /* 8 planes (3D), 64 rows (2D)            */
+int64_t apd_counter_words(const apd_grid* grid, int32_t M, int32_t with_idxsum);   /* u64 words of a counter block */
+
+/* apd_assign on a slab, stopping before the finalize: labels [slab voxels] DEVICE int32 or NULL (x fastest, the
+ * slab's own planes only), counters DEVICE out [apd_counter_words].  Asynchronous on cuda_stream. */
+int apd_assign_slab(apd_ctx* ctx, const apd_grid* grid, const apd_slab* slab, int32_t M, const float* X, const float* A,
+                    const float* w, int32_t* labels, uint64_t* counters, int32_t with_idxsum, const apd_opts* opts,
+                    void* cuda_stream);
+/* The finalize of apd_assign from REDUCED counters (the word-wise sum over all slabs): vol, dual, max_rel_err,
+ * centroids (needs with_idxsum) exactly as apd_assign returns them.  All pointers DEVICE.  Asynchronous. */
+int apd_finalize_counters(apd_ctx* ctx, const apd_grid* grid, int32_t M, const uint64_t* counters, int32_t with_idxsum,
+                          const float* X, const float* w, const float* target_vol, double* vol, double* dual,
+                          double* max_rel_err, double* centroids, void* cuda_stream);
+/* apd_solve on a slab.  After every evaluation the library packs this slab's counters into `counters` (DEVICE,
+ * caller-owned, apd_counter_words(grid, M, 0) words) and calls reduce(user, cuda_stream), which must replace the block,
+ * in stream order, by its word-wise unsigned 64-bit sum over all ranks (one allreduce of 8 (M + layers) bytes: NCCL
+ * ncclAllReduce(ncclUint64, ncclSum) on that stream, or any equivalent) and return 0.  Every rank then runs the same
+ * optimiser step on the same reduced counters, so the replicated L-BFGS states stay identical and the trajectory is
+ * that of the whole-grid apd_solve bit for bit.  labels: this slab's [slab voxels]; vol [M]: of the whole grid.
+ * reduce == NULL: a single slab covering the grid (then this is apd_solve). */
+typedef int (*apd_reduce_fn)(void* user, void* cuda_stream);
+int apd_solve_slab(apd_ctx* ctx, const apd_grid* grid, const apd_slab* slab, int32_t M, const float* X, const float* A,
+                   const float* target_vol, double tol, const float* w_init, float* w, int32_t* labels, double* vol,
+                   uint64_t* counters, apd_reduce_fn reduce, void* user, int32_t* iters, int32_t* evals,
+                   double* max_rel_err, double* dual, const apd_opts* opts, void* cuda_stream);
+
 /* Grows the context's workspace to what apd_assign / apd_solve / apd_lloyd need on `grid` with `opts` (dual partials:
  * 8 bytes per tile; with opts.cull the candidate lists, 1 KiB per 512 voxels; L-BFGS state for opts.lbfgs_history),
  * so that those calls, on this grid or any grid with no more tiles, neither allocate nor synchronise.  Synchronous

@@ -44,6 +44,12 @@ class apd_opts(ctypes.Structure):
                 ("max_iters", ctypes.c_int32), ("max_evals", ctypes.c_int32), ("reserved", ctypes.c_int32 * 3)]
 
 
+class apd_slab(ctypes.Structure):
+    _fields_ = [("lo", ctypes.c_int32), ("n", ctypes.c_int32)]
+
+
+REDUCE_FN = ctypes.CFUNCTYPE(ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p)      # apd_reduce_fn(user, cuda_stream)
+
 _lib = None
 _P = ctypes.c_void_p
 
@@ -102,6 +108,22 @@ def load_library() -> ctypes.CDLL:
     lib.apd_choose_resolution.argtypes = [ctypes.c_int32, ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_int32]
     lib.apd_solve_history.restype = ctypes.c_int
     lib.apd_solve_history.argtypes = [_P, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double), ctypes.c_int32]
+    lib.apd_slab_align.restype = ctypes.c_int32
+    lib.apd_slab_align.argtypes = [ctypes.c_int32]
+    lib.apd_counter_words.restype = ctypes.c_int64
+    lib.apd_counter_words.argtypes = [ctypes.POINTER(apd_grid), ctypes.c_int32, ctypes.c_int32]
+    lib.apd_assign_slab.restype = ctypes.c_int
+    lib.apd_assign_slab.argtypes = ([_P, ctypes.POINTER(apd_grid), ctypes.POINTER(apd_slab), ctypes.c_int32] + [_P] * 5
+                                    + [ctypes.c_int32, ctypes.POINTER(apd_opts), _P])
+    lib.apd_finalize_counters.restype = ctypes.c_int
+    lib.apd_finalize_counters.argtypes = [_P, ctypes.POINTER(apd_grid), ctypes.c_int32, _P, ctypes.c_int32] + [_P] * 8
+    lib.apd_solve_slab.restype = ctypes.c_int
+    lib.apd_solve_slab.argtypes = ([_P, ctypes.POINTER(apd_grid), ctypes.POINTER(apd_slab), ctypes.c_int32, _P, _P, _P,
+                                    ctypes.c_double] + [_P] * 5 + [REDUCE_FN, _P, ctypes.POINTER(ctypes.c_int32),
+                                                                   ctypes.POINTER(ctypes.c_int32),
+                                                                   ctypes.POINTER(ctypes.c_double),
+                                                                   ctypes.POINTER(ctypes.c_double),
+                                                                   ctypes.POINTER(apd_opts), _P])
     lib.apd_reserve.restype = ctypes.c_int
     lib.apd_reserve.argtypes = [_P, ctypes.POINTER(apd_grid), ctypes.POINTER(apd_opts)]
     lib.apd_assign_stats.restype = ctypes.c_int
@@ -112,7 +134,8 @@ def load_library() -> ctypes.CDLL:
 
 EXPORTED_SYMBOLS = ["apd_default_opts", "apd_create", "apd_destroy", "apd_last_error", "apd_assign", "apd_solve",
                     "apd_assign_host", "apd_solve_host", "apd_solve_history", "apd_assign_points", "apd_solve_points", "apd_solve_stats", "apd_lloyd", "apd_solve_refine", "apd_resolution_bound",
-                    "apd_choose_resolution", "apd_reserve", "apd_assign_stats"]
+                    "apd_choose_resolution", "apd_reserve", "apd_assign_stats", "apd_slab_align", "apd_counter_words",
+                    "apd_assign_slab", "apd_finalize_counters", "apd_solve_slab"]
 
 
 def make_grid(dim: int, n: Sequence[int], lo: Sequence[float], hi: Sequence[float]) -> apd_grid:
@@ -123,6 +146,30 @@ def make_grid(dim: int, n: Sequence[int], lo: Sequence[float], hi: Sequence[floa
         g.lo[k] = float(lo[k]) if k < dim else 0.0
         g.hi[k] = float(hi[k]) if k < dim else 1.0
     return g
+
+
+def slab_align(dim: int) -> int:
+    return int(load_library().apd_slab_align(dim))
+
+
+def counter_words(grid: apd_grid, M: int, with_idxsum: bool = False) -> int:
+    return int(load_library().apd_counter_words(ctypes.byref(grid), M, int(with_idxsum)))
+
+
+def slab_partition(n_last: int, world: int, align: int):
+    """Splits the n_last planes of a grid's last axis into `world` contiguous slabs whose boundaries are multiples of
+    `align` (apd_slab_align), as evenly as the alignment allows.  Returns [(lo, n)] per rank.  Needs at least one layer
+    of `align` planes per rank."""
+    layers = (n_last + align - 1) // align
+    if layers < world:
+        raise ValueError(f"{n_last} planes are {layers} layers of {align}: fewer than the {world} ranks")
+    out, lo = [], 0
+    for r in range(world):
+        nl = layers // world + (1 if r < layers % world else 0)
+        n = min(nl * align, n_last - lo)
+        out.append((lo, max(n, 0)))
+        lo += max(n, 0)
+    return out
 
 
 def make_opts(kernel: int = KERNEL_AUTO, cull: int = 0, lbfgs_history: int = 10, max_iters: int = 1000,
@@ -251,6 +298,66 @@ class ApdContext:
             _dev(w, torch.float32, "w", M), _dev(labels, torch.int32, "labels"), _dev(vol, torch.float64, "vol", M),
             _dev(w64, torch.float64, "w64", M), ctypes.byref(it), ctypes.byref(ev), ctypes.byref(err),
             ctypes.byref(dual), ctypes.byref(opts) if opts is not None else None, self._stream())
+        self._check(rc, allow=(APD_OK, APD_NOT_CONVERGED))
+        return SolveInfo(rc, it.value, ev.value, err.value, dual.value)
+
+    # -- voxel-slab sharding (f4) ---------------------------------------------------------------
+    def apd_assign_slab(self, grid: apd_grid, slab, X, A, w, labels=None, counters=None, with_idxsum: bool = False,
+                        opts: Optional[apd_opts] = None):
+        """apd_assign_slab of include/apd.h: raw counters of planes [lo, lo + n) of the last axis (slab = (lo, n));
+        counters: CUDA int64 tensor of counter_words(grid, M, with_idxsum) words."""
+        d = grid.dim
+        M = X.shape[0]
+        sl = apd_slab(int(slab[0]), int(slab[1]))
+        rc = self._lib.apd_assign_slab(
+            self._h, ctypes.byref(grid), ctypes.byref(sl), M, _dev(X, torch.float32, "X", M * d),
+            _dev(A, torch.float32, "A", M * d * d), _dev(w, torch.float32, "w", M), _dev(labels, torch.int32, "labels"),
+            _dev(counters, torch.int64, "counters", counter_words(grid, M, with_idxsum)), int(with_idxsum),
+            ctypes.byref(opts) if opts is not None else None, self._stream())
+        self._check(rc)
+
+    def apd_finalize_counters(self, grid: apd_grid, counters, X, w, target_vol=None, vol=None, dual=None,
+                              max_rel_err=None, centroids=None, with_idxsum: bool = False):
+        """apd_finalize_counters of include/apd.h: vol / dual / error / centroids from REDUCED counters."""
+        d = grid.dim
+        M = X.shape[0]
+        rc = self._lib.apd_finalize_counters(
+            self._h, ctypes.byref(grid), M, _dev(counters, torch.int64, "counters", counter_words(grid, M, with_idxsum)),
+            int(with_idxsum), _dev(X, torch.float32, "X", M * d), _dev(w, torch.float32, "w", M),
+            _dev(target_vol, torch.float32, "target_vol", M), _dev(vol, torch.float64, "vol", M),
+            _dev(dual, torch.float64, "dual", 1), _dev(max_rel_err, torch.float64, "max_rel_err", 1),
+            _dev(centroids, torch.float64, "centroids", M * d), self._stream())
+        self._check(rc)
+
+    def apd_solve_slab(self, grid: apd_grid, slab, X, A, target_vol, tol: float, counters, reduce=None, w_init=None,
+                       w=None, labels=None, vol=None, opts: Optional[apd_opts] = None) -> SolveInfo:
+        """apd_solve_slab of include/apd.h.  `reduce`: a Python callable () -> None that sums `counters` (CUDA int64
+        tensor, counter_words(grid, M) words) over all ranks in place, in order with torch's current stream -- e.g.
+        lambda: torch.distributed.all_reduce(counters).  Blocks until finished."""
+        d = grid.dim
+        M = X.shape[0]
+        sl = apd_slab(int(slab[0]), int(slab[1]))
+        it, ev = ctypes.c_int32(0), ctypes.c_int32(0)
+        err, dual = ctypes.c_double(0.0), ctypes.c_double(0.0)
+        failure = []
+
+        def _cb(user, stream):
+            try:
+                reduce()
+                return 0
+            except Exception as e:        # an exception must not cross the C ABI
+                failure.append(e)
+                return 1
+        cb = REDUCE_FN(_cb) if reduce is not None else ctypes.cast(None, REDUCE_FN)
+        rc = self._lib.apd_solve_slab(
+            self._h, ctypes.byref(grid), ctypes.byref(sl), M, _dev(X, torch.float32, "X", M * d),
+            _dev(A, torch.float32, "A", M * d * d), _dev(target_vol, torch.float32, "target_vol", M), float(tol),
+            _dev(w_init, torch.float32, "w_init", M), _dev(w, torch.float32, "w", M), _dev(labels, torch.int32, "labels"),
+            _dev(vol, torch.float64, "vol", M), _dev(counters, torch.int64, "counters", counter_words(grid, M, False)),
+            cb, None, ctypes.byref(it), ctypes.byref(ev), ctypes.byref(err), ctypes.byref(dual),
+            ctypes.byref(opts) if opts is not None else None, self._stream())
+        if failure:
+            raise failure[0]
         self._check(rc, allow=(APD_OK, APD_NOT_CONVERGED))
         return SolveInfo(rc, it.value, ev.value, err.value, dual.value)
 

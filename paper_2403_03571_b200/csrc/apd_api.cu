@@ -32,7 +32,7 @@ extern "C" void apd_default_opts(apd_opts* o) {
 static void free_ws(Workspace& ws) {
   cudaFree(ws.lloyd_buf); cudaFree(ws.pt_acc); cudaFree(ws.qfix); cudaFree(ws.rec); cudaFree(ws.brick_list); cudaFree(ws.brick_count); cudaFree(ws.super_list);
   cudaFree(ws.super_count); cudaFree(ws.pairs_ctr);
-  cudaFree(ws.seeds); cudaFree(ws.count); cudaFree(ws.idxsum); cudaFree(ws.dual_partial);
+  cudaFree(ws.seeds); cudaFree(ws.count); cudaFree(ws.idxsum); cudaFree(ws.dual_partial); cudaFree(ws.layer_buf);
   cudaFree(ws.sstate); cudaFree(ws.svec); cudaFree(ws.gram); cudaFree(ws.w32); cudaFree(ws.wref); cudaFree(ws.e_vol); cudaFree(ws.e_scal); cudaFree(ws.hist);
   for (int i = 0; i < Workspace::HOST_SLOTS; ++i) cudaFree(ws.host_buf[i]);
   if (ws.report) cudaFreeHost(ws.report);
@@ -92,7 +92,8 @@ extern "C" const char* apd_last_error(const apd_ctx* ctx) {
 namespace apd {
 
 // Validates the grid and fills the device-side description.  Returns "" or an error text.
-std::string make_grid(const apd_ctx* ctx, const apd_grid* grid, int kernel, bool cull, GridDev* g) {
+std::string make_grid(const apd_ctx* ctx, const apd_grid* grid, int kernel, bool cull, GridDev* g,
+                      const apd_slab* slab) {
   if (!grid) return "grid is NULL";
   if (grid->dim != ctx->ws.dim) return "grid.dim differs from the context's dim";
   const int d = grid->dim;
@@ -113,12 +114,36 @@ std::string make_grid(const apd_ctx* ctx, const apd_grid* grid, int kernel, bool
     out.s[k] = (grid->hi[k] - grid->lo[k]) / (double)n[k];
     P *= out.s[k];
   }
+  if (slab) {
+    // planes [lo, lo + n) of the last axis; boundaries on whole layers so that every layer sum has one owner
+    const int last = d - 1, al = slab_align(d);
+    if (slab->lo < 0 || slab->n < 1 || (long long)slab->lo + slab->n > n[last]) return "slab outside the grid";
+    if (slab->lo % al != 0) return "slab.lo must be a multiple of apd_slab_align(dim)";
+    if (slab->n % al != 0 && slab->lo + slab->n != n[last])
+      return "slab.n must be a multiple of apd_slab_align(dim) unless the slab ends at the grid's last plane";
+    n[last] = slab->n;
+    if (d == 3) out.off_z = slab->lo; else out.off_y = slab->lo;
+  }
   out.nx = n[0]; out.ny = n[1]; out.nz = n[2];
   out.voxel_volume = P;
   out.row_long = assign_tile_counts(kernel, d, out.nx, out.ny, out.nz, ctx->ws.sm_count, cull, &out.tiles_x, &out.tiles_y,
                                     &out.tiles_z);
   *g = out;
   return "";
+}
+
+// The two-level reduction of the dual partials for grid (slab) g: SLAB_ALIGN planes of the last axis per layer.
+LayerMap layer_map(const GridDev& g, bool cull) {
+  const int al = slab_align(g.dim);
+  const int n_last = g.dim == 3 ? g.nz : g.ny, tiles_last = g.dim == 3 ? g.tiles_z : g.tiles_y;
+  const int n_layers = (n_last + al - 1) / al;
+  const int tiles_per_layer_axis = (tiles_last + n_layers - 1) / n_layers;      // 1 or 2 tile layers per layer
+  const int per_tile_layer = g.tiles_x * (g.dim == 3 ? g.tiles_y : 1) * (cull ? 4 : 1);
+  LayerMap lm;
+  lm.n_layers = n_layers;
+  lm.per_layer = tiles_per_layer_axis * per_tile_layer;
+  lm.n_partials = tiles_last * per_tile_layer;
+  return lm;
 }
 
 // opts -> kernel (AUTO resolved) and whether culling runs.  AUTO on a grid with fewer voxels along an axis than
@@ -159,6 +184,14 @@ int ensure_eval_buffers(apd_ctx* ctx, const GridDev& g, int kernel, bool cull, c
     APD_CUDA_TRY(ctx, cudaMalloc(&ws.dual_partial, n_partials * sizeof(double)));
     ws.partial_cap = n_partials;
   }
+  const size_t n_layers = (size_t)layer_map(g, cull).n_layers;
+  if (n_layers > ws.layer_cap) {
+    APD_CUDA_TRY(ctx, cudaStreamSynchronize(st));
+    cudaFree(ws.layer_buf);
+    ws.layer_buf = nullptr; ws.layer_cap = 0;
+    APD_CUDA_TRY(ctx, cudaMalloc(&ws.layer_buf, n_layers * sizeof(double)));
+    ws.layer_cap = n_layers;
+  }
   if (kernel == APD_KERNEL_TENSOR && !ws.qfix)
     APD_CUDA_TRY(ctx, cudaMalloc(&ws.qfix, m_pad_max * 6 * sizeof(uint4)));
   if (cull) {
@@ -194,7 +227,6 @@ int enqueue_evaluation(apd_ctx* ctx, const GridDev& g, int kernel, int M, const 
   Workspace& ws = ctx->ws;
   const int M_pad = (M + SEED_CHUNK - 1) / SEED_CHUNK * SEED_CHUNK;
   const int n_tiles = g.tiles_x * g.tiles_y * g.tiles_z;
-  const int n_partials = cull ? 4 * n_tiles : n_tiles;
   const int rc_buf = ensure_eval_buffers(ctx, g, kernel, cull, st);   // no-op after apd_reserve / a call of this size
   if (rc_buf != APD_OK) return rc_buf;
   if (cull) {
@@ -235,8 +267,9 @@ int enqueue_evaluation(apd_ctx* ctx, const GridDev& g, int kernel, int M, const 
   APD_CUDA_TRY(ctx, launch_assign(kernel, a, st));
   if (timed) { APD_CUDA_TRY(ctx, cudaEventRecord(ws.ev1, st)); ws.timed = true; }
   if (vol)     // apd_solve's loop passes vol == nullptr: lbfgs_step_kernel finishes the evaluation itself
-    APD_CUDA_TRY(ctx, launch_finalize(g, M, n_partials, ws.count, a.idxsum, ws.dual_partial, X, w, target_vol, vol,
-                                      dual, max_rel_err, centroids, pairs, cull ? ws.pairs_ctr : nullptr, done_flag, st));
+    APD_CUDA_TRY(ctx, launch_finalize(g, M, layer_map(g, cull), ws.layer_buf, ws.count, nullptr, a.idxsum, ws.dual_partial,
+                                      X, w, target_vol, vol, dual, max_rel_err, centroids, pairs,
+                                      cull ? ws.pairs_ctr : nullptr, done_flag, st));
   return APD_OK;
 }
 

@@ -230,8 +230,8 @@ __global__ void __launch_bounds__(CULL_THREADS) cull_super_kernel(const CullArgs
   constexpr int EY = (DIM == 3) ? SUPER3_TY * CULL_TILE3_Y : SUPER2_TY * CULL_TILE2_Y;
   constexpr int EZ = (DIM == 3) ? SUPER3_TZ * CULL_TILE3_Z : 1;
   const float y0x = box_centre(c.g.lo[0], c.g.s[0], sx * EX, EX);
-  const float y0y = box_centre(c.g.lo[1], c.g.s[1], sy * EY, EY);
-  const float y0z = (DIM == 3) ? box_centre(c.g.lo[2], c.g.s[2], sz * EZ, EZ) : 0.0f;
+  const float y0y = box_centre(c.g.lo[1], c.g.s[1], sy * EY + c.g.off_y, EY);
+  const float y0z = (DIM == 3) ? box_centre(c.g.lo[2], c.g.s[2], sz * EZ + c.g.off_z, EZ) : 0.0f;
 
   float umin = CUDART_INF_F;
   int imin = 0;
@@ -399,8 +399,8 @@ __global__ void __launch_bounds__(128) cull_bricks_kernel(const CullArgs c) {
     float t0x[CULL_G];
 #pragma unroll
     for (int g = 0; g < CULL_G; ++g) t0x[g] = box_centre(c.g.lo[0], c.g.s[0], (qx * CULL_G + g) * TX, TX);
-    const float t0y = box_centre(c.g.lo[1], c.g.s[1], by * TY, TY);
-    const float t0z = (DIM == 3) ? box_centre(c.g.lo[2], c.g.s[2], bz * TZ, TZ) : 0.0f;
+    const float t0y = box_centre(c.g.lo[1], c.g.s[1], by * TY + c.g.off_y, TY);
+    const float t0z = (DIM == 3) ? box_centre(c.g.lo[2], c.g.s[2], bz * TZ + c.g.off_z, TZ) : 0.0f;
     float umin[CULL_G];
     int imin[CULL_G];
 #pragma unroll
@@ -485,8 +485,8 @@ __global__ void __launch_bounds__(128) cull_bricks_kernel(const CullArgs c) {
   // (b) brick lists, tile by tile
   int ox, oy, oz, ex, ey, ez;
   brick_box(DIM, w, &ox, &oy, &oz, &ex, &ey, &ez);
-  const float y0y = box_centre(c.g.lo[1], c.g.s[1], by * TY + oy, ey);
-  const float y0z = (DIM == 3) ? box_centre(c.g.lo[2], c.g.s[2], bz * TZ + oz, ez) : 0.0f;
+  const float y0y = box_centre(c.g.lo[1], c.g.s[1], by * TY + oy + c.g.off_y, ey);
+  const float y0z = (DIM == 3) ? box_centre(c.g.lo[2], c.g.s[2], bz * TZ + oz + c.g.off_z, ez) : 0.0f;
 #pragma unroll
   for (int g = 0; g < CULL_G; ++g) {
     if (g >= ng) break;

@@ -89,6 +89,17 @@ __device__ __forceinline__ float min3f(float a, float b, float c) {
   return r;
 }
 
+// ---- fixed-order sum of p[0 .. count) by ONE warp (all 32 lanes call it): lane l adds elements l, l + 32, ... in
+//      order, then an xor-shuffle tree; every lane returns the same bits.  The layer sums of the dual (apd_internal.cuh)
+__device__ __forceinline__ double warp_ordered_sum(const double* __restrict__ p, int count) {
+  const int lane = threadIdx.x & 31;
+  double s = 0.0;
+  for (int i = lane; i < count; i += 32) s += p[i];
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+  return s;
+}
+
 // ---- deterministic block sum of one double per thread (fixed order: lanes by shuffle tree,
 //      then warps 0..nw-1 sequentially) -- result valid in thread 0 --------------------------
 template <int NTHREADS>

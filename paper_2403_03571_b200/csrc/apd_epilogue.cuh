@@ -36,8 +36,8 @@ __device__ __forceinline__ double row_epilogue(const AssignArgs& a, bool row_val
         atomicAdd(a.count + run_lab, run_cnt);
         if (a.idxsum) {
           atomicAdd(a.idxsum + (size_t)run_lab * 3 + 0, run_sx);
-          atomicAdd(a.idxsum + (size_t)run_lab * 3 + 1, (unsigned long long)run_cnt * iy);
-          atomicAdd(a.idxsum + (size_t)run_lab * 3 + 2, (unsigned long long)run_cnt * iz);
+          atomicAdd(a.idxsum + (size_t)run_lab * 3 + 1, (unsigned long long)run_cnt * (iy + a.g.off_y));
+          atomicAdd(a.idxsum + (size_t)run_lab * 3 + 2, (unsigned long long)run_cnt * (iz + a.g.off_z));
         }
         run_lab = lab[k]; run_cnt = 0; run_sx = 0;
       }
@@ -48,8 +48,8 @@ __device__ __forceinline__ double row_epilogue(const AssignArgs& a, bool row_val
   atomicAdd(a.count + run_lab, run_cnt);
   if (a.idxsum) {
     atomicAdd(a.idxsum + (size_t)run_lab * 3 + 0, run_sx);
-    atomicAdd(a.idxsum + (size_t)run_lab * 3 + 1, (unsigned long long)run_cnt * iy);
-    atomicAdd(a.idxsum + (size_t)run_lab * 3 + 2, (unsigned long long)run_cnt * iz);
+    atomicAdd(a.idxsum + (size_t)run_lab * 3 + 1, (unsigned long long)run_cnt * (iy + a.g.off_y));
+    atomicAdd(a.idxsum + (size_t)run_lab * 3 + 2, (unsigned long long)run_cnt * (iz + a.g.off_z));
   }
   return dsum;
 }

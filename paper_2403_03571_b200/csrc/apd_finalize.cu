@@ -23,20 +23,25 @@ __device__ __forceinline__ double block_max_double(double v, double* scratch) {
   return t;
 }
 
+// count64 != nullptr: the counts come as u64 (reduced counter block of a sharded evaluation, apd_shard.cu).
+// dual_partial != nullptr: the layer sums of the per-tile partials are formed here (into layer_buf); nullptr: layer_buf
+// already holds them (reduced over the slabs).  Either way the dual's sum of minima = the layer sums added in ascending
+// layer order -- the same two-level order in every path (apd_internal.cuh).
 __global__ void __launch_bounds__(FIN_THREADS) finalize_kernel(
-    GridDev g, int M, int n_partials, const unsigned int* __restrict__ count,
-    const unsigned long long* __restrict__ idxsum, const double* __restrict__ dual_partial,
-    const float* __restrict__ X, const float* __restrict__ w, const float* __restrict__ target_vol,
-    double* __restrict__ vol, double* __restrict__ dual, double* __restrict__ max_rel_err,
-    double* __restrict__ centroids, uint64_t* __restrict__ pairs_evaluated,
+    GridDev g, int M, LayerMap lm, double* __restrict__ layer_buf, const unsigned int* __restrict__ count,
+    const unsigned long long* __restrict__ count64, const unsigned long long* __restrict__ idxsum,
+    const double* __restrict__ dual_partial, const float* __restrict__ X, const float* __restrict__ w,
+    const float* __restrict__ target_vol, double* __restrict__ vol, double* __restrict__ dual,
+    double* __restrict__ max_rel_err, double* __restrict__ centroids, uint64_t* __restrict__ pairs_evaluated,
     const unsigned long long* __restrict__ pairs_ctr, const int* __restrict__ done_flag) {
   __shared__ double scratch[FIN_THREADS / 32];
+  __shared__ double s_smin;
   if (done_flag && *done_flag) return;
   const int tid = threadIdx.x;
   const double P = g.voxel_volume;
   double vw = 0.0, err = 0.0;
   for (int i = tid; i < M; i += FIN_THREADS) {
-    const unsigned int c = count[i];
+    const unsigned long long c = count64 ? count64[i] : (unsigned long long)count[i];
     const double vi = (double)c * P;                       // m_i |P|
     vol[i] = vi;
     if (target_vol) {
@@ -53,15 +58,25 @@ __global__ void __launch_bounds__(FIN_THREADS) finalize_kernel(
       }
     }
   }
-  double smin = 0.0;
-  for (int t = tid; t < n_partials; t += FIN_THREADS) smin += dual_partial[t];
+  if (dual_partial) {
+    for (int L = tid >> 5; L < lm.n_layers; L += FIN_THREADS / 32) {
+      const int first = L * lm.per_layer, cnt = min(lm.per_layer, lm.n_partials - first);
+      const double ls = warp_ordered_sum(dual_partial + first, cnt);
+      if ((tid & 31) == 0) layer_buf[L] = ls;
+    }
+  }
+  __syncthreads();
+  if (tid == 0) {
+    double t = 0.0;
+    for (int L = 0; L < lm.n_layers; ++L) t += layer_buf[L];
+    s_smin = t;
+  }
 
   const double vw_tot = block_sum_double<FIN_THREADS>(vw, scratch);
   __syncthreads();
-  const double smin_tot = block_sum_double<FIN_THREADS>(smin, scratch);
   const double err_tot = block_max_double(err, scratch);
   if (tid == 0) {
-    *dual = vw_tot + P * smin_tot;
+    *dual = vw_tot + P * s_smin;
     if (max_rel_err && target_vol) *max_rel_err = err_tot;
     if (pairs_evaluated)
       *pairs_evaluated = pairs_ctr ? (uint64_t)*pairs_ctr      // culled: what the tiles counted
@@ -69,13 +84,13 @@ __global__ void __launch_bounds__(FIN_THREADS) finalize_kernel(
   }
 }
 
-cudaError_t launch_finalize(const GridDev& g, int M, int n_partials, const unsigned int* count,
-                            const unsigned long long* idxsum, const double* dual_partial,
-                            const float* X, const float* w, const float* target_vol,
+cudaError_t launch_finalize(const GridDev& g, int M, LayerMap lm, double* layer_buf, const unsigned int* count,
+                            const unsigned long long* count64, const unsigned long long* idxsum,
+                            const double* dual_partial, const float* X, const float* w, const float* target_vol,
                             double* vol, double* dual, double* max_rel_err, double* centroids,
                             uint64_t* pairs_evaluated, const unsigned long long* pairs_ctr, const int* done_flag,
                             cudaStream_t st) {
-  finalize_kernel<<<1, FIN_THREADS, 0, st>>>(g, M, n_partials, count, idxsum, dual_partial, X, w, target_vol,
+  finalize_kernel<<<1, FIN_THREADS, 0, st>>>(g, M, lm, layer_buf, count, count64, idxsum, dual_partial, X, w, target_vol,
                                              vol, dual, max_rel_err, centroids, pairs_evaluated, pairs_ctr, done_flag);
   return cudaGetLastError();
 }

@@ -31,6 +31,23 @@ struct GridDev {
   double voxel_volume;  // |P|
   int tiles_x, tiles_y, tiles_z;
   int row_long;         // ROWPOLY kernel: 1 = rows of 32 voxels per thread, 0 = rows of 16
+  // voxel-slab sharding (f4, apd_shard.cu): this GridDev describes planes [off, off + n) of the grid's LAST axis (z in
+  // 3D, y in 2D); ny / nz above is the slab's own count, off_y / off_z the index of its first plane in the whole grid
+  // (0 for a whole grid; one of the two is always 0).  Voxel centres and index sums use the GLOBAL index i + off, so a
+  // slab's arithmetic is that of the whole-grid call bit for bit; label positions are local to the slab.
+  int off_y, off_z;
+};
+
+// The dual's sum of minima is reduced in two levels, the same way everywhere, so that a slab-sharded evaluation
+// reproduces the whole-grid one bit for bit: the per-tile (per-brick) partials of one LAYER -- SLAB_ALIGN planes of the
+// last axis: a whole number of tile layers of every kernel -- are summed by one warp in a fixed order
+// (warp_ordered_sum), then the layer sums are added in ascending layer order.
+constexpr int SLAB_ALIGN3 = 8, SLAB_ALIGN2 = 64;
+__host__ __device__ constexpr int slab_align(int dim) { return dim == 3 ? SLAB_ALIGN3 : SLAB_ALIGN2; }
+struct LayerMap {
+  int n_layers;           // layers of this (slab) grid
+  int per_layer;          // partials per full layer
+  int n_partials;         // all partials (the last layer may hold fewer)
 };
 
 struct AssignArgs {
@@ -71,6 +88,8 @@ struct Workspace {
   unsigned long long* idxsum = nullptr;  // [max_seeds,3]
   double* dual_partial = nullptr;      // [partial_cap]
   size_t partial_cap = 0;
+  double* layer_buf = nullptr;         // [layer_cap] layer sums of the dual partials (two-level reduction)
+  size_t layer_cap = 0;
   // culling (apd_cull.cu), allocated on first use
   float* rec = nullptr;                // [M_pad, REC] per-seed records + rho_brick, rho_super
   int* brick_list = nullptr;           // [brick_cap_n * BRICK_CAP]
@@ -153,8 +172,9 @@ cudaError_t launch_cull(const GridDev& g, int M, int M_pad, const float* X, cons
 void cull_super_counts(const GridDev& g, int* nsx, int* nsy, int* nsz);
 int rowpoly_tile_counts(int dim, int nx, int ny, int nz, int sm_count, bool cull, int* tx, int* ty, int* tz);
 int assign_tile_counts(int kernel, int dim, int nx, int ny, int nz, int sm_count, bool cull, int* tx, int* ty, int* tz);
-cudaError_t launch_finalize(const GridDev& g, int M, int n_partials, const unsigned int* count,
-                            const unsigned long long* idxsum, const double* dual_partial,
+cudaError_t launch_finalize(const GridDev& g, int M, LayerMap lm, double* layer_buf, const unsigned int* count,
+                            const unsigned long long* count64, const unsigned long long* idxsum,
+                            const double* dual_partial,
                             const float* X, const float* w, const float* target_vol,
                             double* vol, double* dual, double* max_rel_err, double* centroids,
                             uint64_t* pairs_evaluated, const unsigned long long* pairs_ctr, const int* done_flag,
@@ -177,13 +197,28 @@ struct SolveReport {
 };
 
 // host helpers shared by apd_api.cu and apd_lbfgs.cu
-std::string make_grid(const apd_ctx* ctx, const apd_grid* grid, int kernel, bool cull, GridDev* g);
+std::string make_grid(const apd_ctx* ctx, const apd_grid* grid, int kernel, bool cull, GridDev* g,
+                      const apd_slab* slab = nullptr);
+LayerMap layer_map(const GridDev& g, bool cull);
 int resolve_kernel(const apd_opts* o, const apd_grid* grid, bool* cull, std::string* err);
 // Sizes the buffers an evaluation of grid `g` needs (dual partials; with culling the candidate lists and the record
 // table; for the TENSOR kernel its seed table).  Grow-only.  Growing synchronises `st` and reallocates: apd_reserve
 // does this ahead of time so that apd_assign / apd_solve never do.
 int ensure_eval_buffers(apd_ctx* ctx, const GridDev& g, int kernel, bool cull, cudaStream_t st);
 int ensure_solve_state(apd_ctx* ctx, int hist);
+// apd_lbfgs.cu: Algorithm 2 on a grid (slab == nullptr) or on one slab of it with a counter exchange (apd_shard.cu)
+int solve_grid(apd_ctx* ctx, const char* who, const apd_grid* grid, const apd_slab* slab, int32_t M, const float* X,
+               const float* A, const float* target_vol, double tol, const float* w_init, float* w, int32_t* labels,
+               double* vol, double* w64, uint64_t* counters, apd_reduce_fn reduce, void* user, int32_t* iters,
+               int32_t* evals, double* max_rel_err, double* dual, const apd_opts* opts, void* cuda_stream);
+// apd_shard.cu: count[M] u32 (+ idxsum) and the layer sums of this slab's dual partials -> the u64 counter block
+cudaError_t launch_pack_counters(const GridDev& g, int M, LayerMap lm, int n_layers_full, const unsigned int* count,
+                                 const unsigned long long* idxsum, const double* dual_partial, uint64_t* counters,
+                                 const int* done_flag, cudaStream_t st);
+// user point sets (apd_points.cu) have no layers: their flat partials are grouped by 256
+inline LayerMap points_layer_map(int n_partials) {
+  LayerMap lm; lm.per_layer = 256; lm.n_partials = n_partials; lm.n_layers = (n_partials + 255) / 256; return lm;
+}
 int enqueue_evaluation(apd_ctx* ctx, const GridDev& g, int kernel, int M, const float* X, const float* A,
                        const float* w, const float* target_vol, int32_t* labels, double* vol, double* dual,
                        double* max_rel_err, double* centroids, uint64_t* pairs, bool timed, bool cull,

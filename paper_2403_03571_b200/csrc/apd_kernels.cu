@@ -9,6 +9,7 @@
 #include "apd_device.cuh"
 #include "apd_epilogue.cuh"
 #include <math_constants.h>
+#include <cstdlib>
 
 namespace apd {
 
@@ -80,9 +81,48 @@ __device__ __forceinline__ float centre_f32(double lo, double s, int i) {
 
 // ------------------------------------------------------------------------------------------
 // DIRECT kernel: every pair evaluates the full quadratic form in delta = y - x_i
-// (3 FADD + 3 FMUL + 6 FFMA in 3D), running (min, argmin) with strict '<' over ascending i.
+// (3 FADD + 3 FMUL + 6 FFMA in 3D as written; the compiler shares the terms in dy, dz alone between the V voxels of a
+// thread).  a4: the inner loop keeps ONLY the running minimum (one FMNMX per pair instead of compare + two selects);
+// every DIRECT_GROUP seeds the V minima are compared with their values before the group, and a voxel whose minimum
+// dropped has its argmin inside that group: the rare rescan recomputes the group with the same function (bitwise
+// equal costs) and takes the first seed that attains the new minimum -- strict '<' over ascending i, lowest index on
+// ties (reading S1), exactly the labels of the compare-and-select form.
 // ------------------------------------------------------------------------------------------
+constexpr int DIRECT_GROUP = 16;
+
+template <int DIM> struct DirectSeed;
+template <> struct DirectSeed<3> { float4 p0, p1, p2; };      // x y z a11 | a12' a13' a22 a23' | a33 nw . .
+template <> struct DirectSeed<2> { float4 p0, p1; };          // x y a11 a12' | a22 nw . .
+
 template <int DIM>
+__device__ __forceinline__ DirectSeed<DIM> direct_load(const float4* __restrict__ sp, int i) {
+  DirectSeed<DIM> s;
+  if constexpr (DIM == 3) { s.p0 = sp[i * 3 + 0]; s.p1 = sp[i * 3 + 1]; s.p2 = sp[i * 3 + 2]; }
+  else                    { s.p0 = sp[i * 2 + 0]; s.p1 = sp[i * 2 + 1]; }
+  return s;
+}
+
+// C_ij for one voxel (yx, yy, yz) and one seed: every operation explicit, so that the main loop and the rescan
+// produce the same bits
+template <int DIM>
+__device__ __forceinline__ float direct_cost(const DirectSeed<DIM>& s, float yx, float yy, float yz) {
+  if constexpr (DIM == 3) {
+    const float dx = __fsub_rn(yx, s.p0.x), dy = __fsub_rn(yy, s.p0.y), dz = __fsub_rn(yz, s.p0.z);
+    const float u = fmaf(s.p1.y, dz, fmaf(s.p1.x, dy, __fmul_rn(s.p0.w, dx)));   // a11 dx + a12' dy + a13' dz
+    const float v = fmaf(s.p1.w, dz, __fmul_rn(s.p1.z, dy));                      // a22 dy + a23' dz
+    const float t = __fmul_rn(s.p2.x, dz);                                        // a33 dz
+    float c = fmaf(dx, u, s.p2.y);                                                // ... - w
+    c = fmaf(dy, v, c);
+    return fmaf(dz, t, c);
+  } else {
+    const float dx = __fsub_rn(yx, s.p0.x), dy = __fsub_rn(yy, s.p0.y);
+    const float u = fmaf(s.p0.w, dy, __fmul_rn(s.p0.z, dx));                      // a11 dx + a12' dy
+    const float v = __fmul_rn(s.p1.x, dy);                                        // a22 dy
+    return fmaf(dy, v, fmaf(dx, u, s.p1.y));
+  }
+}
+
+template <int DIM, int UNROLL>
 __global__ void __launch_bounds__(256) assign_direct_kernel(const AssignArgs a) {
   using G = DirectGeom<DIM>;
   constexpr int V = G::V;
@@ -114,8 +154,8 @@ __global__ void __launch_bounds__(256) assign_direct_kernel(const AssignArgs a) 
   float yx[V];
 #pragma unroll
   for (int k = 0; k < V; ++k) yx[k] = centre_f32(a.g.lo[0], a.g.s[0], ix0 + k);
-  const float yy = centre_f32(a.g.lo[1], a.g.s[1], iy);
-  const float yz = (DIM == 3) ? centre_f32(a.g.lo[2], a.g.s[2], iz) : 0.0f;
+  const float yy = centre_f32(a.g.lo[1], a.g.s[1], iy + a.g.off_y);
+  const float yz = (DIM == 3) ? centre_f32(a.g.lo[2], a.g.s[2], iz + a.g.off_z) : 0.0f;
 
   float best[V];
   int lab[V];
@@ -127,33 +167,29 @@ __global__ void __launch_bounds__(256) assign_direct_kernel(const AssignArgs a) 
     mbar_wait(&s_full[stage], (uint32_t)((c / SEED_STAGES) & 1));
     const float4* sp = reinterpret_cast<const float4*>(s_seeds[stage]);
     const int ibase = c * SEED_CHUNK;
-#pragma unroll 2
-    for (int i = 0; i < SEED_CHUNK; ++i) {
-      if (DIM == 3) {
-        const float4 p0 = sp[i * 3 + 0], p1 = sp[i * 3 + 1], p2 = sp[i * 3 + 2];
-        const float dy = yy - p0.y, dz = yz - p0.z;
+    for (int g0 = 0; g0 < SEED_CHUNK; g0 += DIRECT_GROUP) {
+      float prev[V];
 #pragma unroll
-        for (int k = 0; k < V; ++k) {
-          const float dx = yx[k] - p0.x;
-          const float u = fmaf(p1.y, dz, fmaf(p1.x, dy, p0.w * dx));   // a11 dx + a12' dy + a13' dz
-          const float v = fmaf(p1.w, dz, p1.z * dy);                   // a22 dy + a23' dz
-          const float s = p2.x * dz;                                   // a33 dz
-          float cst = fmaf(dx, u, p2.y);                               // ... - w
-          cst = fmaf(dy, v, cst);
-          cst = fmaf(dz, s, cst);
-          if (cst < best[k]) { best[k] = cst; lab[k] = ibase + i; }
-        }
-      } else {
-        const float4 p0 = sp[i * 2 + 0], p1 = sp[i * 2 + 1];
-        const float dy = yy - p0.y;
+      for (int k = 0; k < V; ++k) prev[k] = best[k];
+#pragma unroll UNROLL
+      for (int i = g0; i < g0 + DIRECT_GROUP; ++i) {
+        const DirectSeed<DIM> sd = direct_load<DIM>(sp, i);
 #pragma unroll
-        for (int k = 0; k < V; ++k) {
-          const float dx = yx[k] - p0.x;
-          const float u = fmaf(p0.w, dy, p0.z * dx);                   // a11 dx + a12' dy
-          const float v = p1.x * dy;                                   // a22 dy
-          float cst = fmaf(dx, u, p1.y);
-          cst = fmaf(dy, v, cst);
-          if (cst < best[k]) { best[k] = cst; lab[k] = ibase + i; }
+        for (int k = 0; k < V; ++k) best[k] = fminf(best[k], direct_cost<DIM>(sd, yx[k], yy, yz));
+      }
+      unsigned int mask = 0u;
+#pragma unroll
+      for (int k = 0; k < V; ++k) mask |= (best[k] < prev[k]) ? (1u << k) : 0u;
+      if (mask) {
+        // a4, deferred: the first seed of the group whose cost equals the new minimum
+        for (int i = g0; i < g0 + DIRECT_GROUP && mask; ++i) {
+          const DirectSeed<DIM> sd = direct_load<DIM>(sp, i);
+#pragma unroll
+          for (int k = 0; k < V; ++k) {
+            if ((mask >> k) & 1u) {
+              if (direct_cost<DIM>(sd, yx[k], yy, yz) == best[k]) { lab[k] = ibase + i; mask &= ~(1u << k); }
+            }
+          }
         }
       }
     }
@@ -190,8 +226,12 @@ cudaError_t launch_assign(int kernel, const AssignArgs& a, cudaStream_t st) {
   if (kernel == APD_KERNEL_ROWPOLY) return launch_assign_rowpoly(a, st);
   if (kernel == APD_KERNEL_TENSOR) return launch_assign_tensor(a, st);
   const int n_tiles = a.g.tiles_x * a.g.tiles_y * a.g.tiles_z;
-  if (a.g.dim == 3) assign_direct_kernel<3><<<n_tiles, 256, 0, st>>>(a);
-  else              assign_direct_kernel<2><<<n_tiles, 256, 0, st>>>(a);
+  static const int unroll = getenv("APD_DIRECT_UNROLL") ? atoi(getenv("APD_DIRECT_UNROLL")) : 2;   // DEV ONLY
+  if (a.g.dim == 3) {
+    if (unroll == 4) assign_direct_kernel<3, 4><<<n_tiles, 256, 0, st>>>(a);
+    else if (unroll == 1) assign_direct_kernel<3, 1><<<n_tiles, 256, 0, st>>>(a);
+    else assign_direct_kernel<3, 2><<<n_tiles, 256, 0, st>>>(a);
+  } else              assign_direct_kernel<2, 2><<<n_tiles, 256, 0, st>>>(a);
   return cudaGetLastError();
 }
 

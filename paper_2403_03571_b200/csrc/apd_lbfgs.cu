@@ -49,9 +49,12 @@ struct StepArgs {
   const float* v;      // target volumes
   // raw outputs of the evaluation just run (the loop skips finalize_kernel and finishes eq. 2.7 / 2.8 / 2.5 here)
   const unsigned int* count;      // [M] voxels per cell (grid evaluations), or nullptr:
+  const unsigned long long* count64;  // [M] the same as u64: the REDUCED counter block of a slab-sharded solve, or:
   const double* vol_in;           // [M] cell volumes already in fp64 (apd_solve_points; voxel_volume is then 1)
-  const double* dual_partial;     // [n_partials] sums of min-costs
-  int n_partials;
+  const double* dual_partial;     // [lm.n_partials] sums of min-costs per tile / brick; nullptr when layer_in is given
+  LayerMap lm;                    // two-level reduction of dual_partial (apd_internal.cuh)
+  double* layer_buf;              // [lm.n_layers] scratch the layer sums are formed in
+  const double* layer_in;         // [lm.n_layers] layer sums already reduced over the slabs (sharded solve), else nullptr
   double voxel_volume;            // |P|
   float* w32;          // next evaluation's weights
   SolveReport* report; // mapped host memory
@@ -301,6 +304,7 @@ __global__ void __cluster_dims__(LB_CLUSTER, 1, 1) __launch_bounds__(LB_THREADS)
   __shared__ double s_wbuf[(LB_THREADS / 32) * LB_NRED];
   __shared__ double s_cbuf[2 * LB_NRED];
   __shared__ double s_tot[LB_NRED];
+  __shared__ double s_smin;
   extern __shared__ double s_dyn[];        // direction_vf: compact Gram matrix, coefficients (sized by the launch)
   cg::cluster_group cluster = cg::this_cluster();
   Reducer red{s_wbuf, s_cbuf, s_tot, 0, cluster.block_rank()};
@@ -335,12 +339,30 @@ __global__ void __cluster_dims__(LB_CLUSTER, 1, 1) __launch_bounds__(LB_THREADS)
   for (int i = LB_FIRST(red); i < M; i += LB_STEP) {
     const double tv = (double)a.v[i];
     s0[0] += tv * (double)a.w32[i];
-    const double vi = a.vol_in ? a.vol_in[i] : (double)a.count[i] * P;
+    const double vi = a.vol_in ? a.vol_in[i] : (a.count64 ? (double)a.count64[i] : (double)a.count[i]) * P;
     emax = fmax(emax, fabs(vi - tv) / tv);
   }
-  for (int t = LB_FIRST(red); t < a.n_partials; t += LB_STEP) s0[1] += a.dual_partial[t];
-  cluster_all<2, false>(s0, red);
+  // sum of the minima, two-level (apd_internal.cuh): layer sums by one warp each, in a fixed order ...
+  if (!a.layer_in) {
+    for (int L = (int)red.rank * (LB_THREADS / 32) + (tid >> 5); L < a.lm.n_layers; L += LB_CLUSTER * (LB_THREADS / 32)) {
+      const int first = L * a.lm.per_layer, cnt = min(a.lm.per_layer, a.lm.n_partials - first);
+      const double ls = warp_ordered_sum(a.dual_partial + first, cnt);
+      if ((tid & 31) == 0) a.layer_buf[L] = ls;
+    }
+  }
+  cluster_all<2, false>(s0, red);          // (its cluster barrier also publishes the layer sums to every CTA)
   const double err1 = cluster_allmax(emax, red);
+  // ... then the layers in ascending order: the same bits in every CTA, and in a slab-sharded solve
+  {
+    const double* lsrc = a.layer_in ? a.layer_in : a.layer_buf;
+    if (tid == 0) {
+      double t = 0.0;
+      for (int L = 0; L < a.lm.n_layers; ++L) t += __ldcg(lsrc + L);
+      s_smin = t;
+    }
+    __syncthreads();
+    s0[1] = s_smin;
+  }
   const double dual1 = s0[0] + P * s0[1], f1 = -dual1;
 
   // ONE sweep: gradient of f at the evaluated point, vol - v (eq. 2.8); the best-so-far copy; and, speculatively,
@@ -353,7 +375,7 @@ __global__ void __cluster_dims__(LB_CLUSTER, 1, 1) __launch_bounds__(LB_THREADS)
   double sums[5] = {0.0, 0.0, 0.0, 0.0, 0.0};     // sum v, g1.p, s.y, s.s, y.y
   for (int i = LB_FIRST(red); i < M; i += LB_STEP) {
     const double tv = (double)a.v[i];
-    const double gn = (a.vol_in ? a.vol_in[i] : (double)a.count[i] * P) - tv;      // m_i |P| - v_i
+    const double gn = (a.vol_in ? a.vol_in[i] : (a.count64 ? (double)a.count64[i] : (double)a.count[i]) * P) - tv;   // m_i |P| - v_i
     gnew[i] = gn;
     sums[0] += tv;
     if (improved) wbest[i] = w_eval[i];
@@ -574,7 +596,7 @@ static int solve_common(apd_ctx* ctx, const char* who, int dim, int32_t M, const
   for (;; ++enq) {
     int rc = hooks.loop_eval(done_flag);
     if (rc != APD_OK) return rc;
-    sa.dual_partial = ws.dual_partial;       // (re)allocated by the first evaluation
+    if (!sa.layer_in) { sa.dual_partial = ws.dual_partial; sa.layer_buf = ws.layer_buf; }   // (re)allocated by the first evaluation
     lbfgs_step_kernel<<<LB_CLUSTER, LB_THREADS, dyn_bytes, st>>>(sa);
     LB_TRY(cudaGetLastError());
     LB_TRY(cudaEventRecord(ws.sev[enq & 1], st));
@@ -617,25 +639,32 @@ static int check_solve_opts(apd_ctx* ctx, const char* who, const apd_opts* opts,
   return APD_OK;
 }
 
-extern "C" int apd_solve(apd_ctx* ctx, const apd_grid* grid, int32_t M, const float* X, const float* A,
-                         const float* target_vol, double tol, const float* w_init, float* w, int32_t* labels,
-                         double* vol, double* w64, int32_t* iters, int32_t* evals, double* max_rel_err,
-                         double* dual, const apd_opts* opts, void* cuda_stream) {
+// Algorithm 2 on a grid or on one slab of it (f4).  slab == nullptr: the whole grid, no exchange.  With a slab every
+// evaluation leaves its raw counters in `counters` (apd_shard.cu: pack_counters) and reduce(user, stream) sums them over
+// the ranks before the optimiser step, which then reads the REDUCED block: identical inputs on every rank.
+int apd::solve_grid(apd_ctx* ctx, const char* who, const apd_grid* grid, const apd_slab* slab, int32_t M, const float* X,
+                    const float* A, const float* target_vol, double tol, const float* w_init, float* w, int32_t* labels,
+                    double* vol, double* w64, uint64_t* counters, apd_reduce_fn reduce, void* user, int32_t* iters,
+                    int32_t* evals, double* max_rel_err, double* dual, const apd_opts* opts, void* cuda_stream) {
   if (!ctx) return APD_E_ARG;
   ctx->err.clear();
+  const std::string pre = std::string(who) + ": ";
   std::string e;
   bool cull = false;
   const int kernel = resolve_kernel(opts, grid, &cull, &e);
-  if (kernel < 0) { ctx->err = "apd_solve: " + e; return APD_E_ARG; }
-  if (M < 1 || M > ctx->ws.max_seeds) { ctx->err = "apd_solve: M out of range [1, max_seeds]"; return APD_E_ARG; }
-  if (!X || !A || !target_vol || !w) { ctx->err = "apd_solve: X, A, target_vol and w are required"; return APD_E_ARG; }
+  if (kernel < 0) { ctx->err = pre + e; return APD_E_ARG; }
+  if (M < 1 || M > ctx->ws.max_seeds) { ctx->err = pre + "M out of range [1, max_seeds]"; return APD_E_ARG; }
+  if (!X || !A || !target_vol || !w) { ctx->err = pre + "X, A, target_vol and w are required"; return APD_E_ARG; }
+  if (slab && !counters) { ctx->err = pre + "counters is required"; return APD_E_ARG; }
   apd_opts o;
-  int rc = check_solve_opts(ctx, "apd_solve", opts, tol, &o);
+  int rc = check_solve_opts(ctx, who, opts, tol, &o);
   if (rc != APD_OK) return rc;
   o.cull = cull ? 1 : 0;
-  GridDev g;
-  e = make_grid(ctx, grid, kernel, o.cull != 0, &g);
-  if (!e.empty()) { ctx->err = "apd_solve: " + e; return APD_E_ARG; }
+  GridDev g, gfull;
+  e = make_grid(ctx, grid, kernel, o.cull != 0, &g, slab);
+  if (!e.empty()) { ctx->err = pre + e; return APD_E_ARG; }
+  e = make_grid(ctx, grid, kernel, o.cull != 0, &gfull, nullptr);
+  if (!e.empty()) { ctx->err = pre + e; return APD_E_ARG; }
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   LB_TRY(cudaSetDevice(ctx->ws.device));
   rc = ensure_solve_state(ctx, o.lbfgs_history);
@@ -643,21 +672,55 @@ extern "C" int apd_solve(apd_ctx* ctx, const apd_grid* grid, int32_t M, const fl
   Workspace& ws = ctx->ws;
   double domain = 1.0;
   for (int k = 0; k < g.dim; ++k) domain *= (grid->hi[k] - grid->lo[k]);
+  const LayerMap lm = layer_map(g, o.cull != 0);
+  const int n_layers_full = layer_map(gfull, o.cull != 0).n_layers;
   StepArgs sa;
-  sa.count = ws.count; sa.vol_in = nullptr; sa.voxel_volume = g.voxel_volume;
-  sa.n_partials = (o.cull ? 4 : 1) * g.tiles_x * g.tiles_y * g.tiles_z;
+  sa.count = ws.count; sa.count64 = nullptr; sa.vol_in = nullptr; sa.voxel_volume = g.voxel_volume;
+  sa.lm = lm; sa.dual_partial = nullptr; sa.layer_buf = nullptr; sa.layer_in = nullptr;
+  if (slab) {
+    sa.count = nullptr; sa.count64 = reinterpret_cast<const unsigned long long*>(counters);
+    sa.layer_in = reinterpret_cast<const double*>(counters + M);
+    sa.lm.n_layers = n_layers_full;
+  }
+  auto exchange = [&](bool with_idxsum, const int* done_flag) -> int {
+    // this slab's counters -> `counters`, then their sum over the ranks, in stream order
+    LB_TRY(launch_pack_counters(g, M, lm, n_layers_full, ws.count, with_idxsum ? ws.idxsum : nullptr, ws.dual_partial,
+                                counters, done_flag, st));
+    if (reduce && reduce(user, cuda_stream) != 0) { ctx->err = pre + "the reduce callback failed"; return APD_E_CUDA; }
+    return APD_OK;
+  };
   SolveHooks hooks;
-  hooks.loop_eval = [&](const int* done_flag) {
-    return enqueue_evaluation(ctx, g, kernel, M, X, A, ws.w32, target_vol, nullptr, nullptr, nullptr, nullptr, nullptr,
-                              nullptr, false, o.cull != 0, done_flag, st, &ws.sstate->cull_rebuild,
-                              &ws.sstate->cull_delta);
+  hooks.loop_eval = [&](const int* done_flag) -> int {
+    int r = enqueue_evaluation(ctx, g, kernel, M, X, A, ws.w32, target_vol, nullptr, nullptr, nullptr, nullptr, nullptr,
+                               nullptr, false, o.cull != 0, done_flag, st, &ws.sstate->cull_rebuild,
+                               &ws.sstate->cull_delta);
+    if (r == APD_OK && slab) r = exchange(false, done_flag);
+    return r;
   };
-  hooks.final_eval = [&]() {
-    return enqueue_evaluation(ctx, g, kernel, M, X, A, ws.w32, target_vol, labels, vol ? vol : ws.e_vol, ws.e_scal,
-                              ws.e_scal + 1, nullptr, nullptr, true, o.cull != 0, nullptr, st);
+  hooks.final_eval = [&]() -> int {
+    if (!slab)
+      return enqueue_evaluation(ctx, g, kernel, M, X, A, ws.w32, target_vol, labels, vol ? vol : ws.e_vol, ws.e_scal,
+                                ws.e_scal + 1, nullptr, nullptr, true, o.cull != 0, nullptr, st);
+    int r = enqueue_evaluation(ctx, g, kernel, M, X, A, ws.w32, target_vol, labels, nullptr, nullptr, nullptr, nullptr,
+                               nullptr, true, o.cull != 0, nullptr, st);
+    if (r == APD_OK) r = exchange(false, nullptr);
+    if (r != APD_OK) return r;
+    LayerMap lf = lm; lf.n_layers = n_layers_full;
+    LB_TRY(launch_finalize(gfull, M, lf, const_cast<double*>(sa.layer_in), nullptr, sa.count64, nullptr, nullptr, X,
+                           ws.w32, target_vol, vol ? vol : ws.e_vol, ws.e_scal, ws.e_scal + 1, nullptr, nullptr, nullptr,
+                           nullptr, st));
+    return APD_OK;
   };
-  return solve_common(ctx, "apd_solve", g.dim, M, target_vol, tol, w_init, w, w64, o, domain, sa, hooks, iters, evals,
+  return solve_common(ctx, who, g.dim, M, target_vol, tol, w_init, w, w64, o, domain, sa, hooks, iters, evals,
                       max_rel_err, dual, st);
+}
+
+extern "C" int apd_solve(apd_ctx* ctx, const apd_grid* grid, int32_t M, const float* X, const float* A,
+                         const float* target_vol, double tol, const float* w_init, float* w, int32_t* labels,
+                         double* vol, double* w64, int32_t* iters, int32_t* evals, double* max_rel_err,
+                         double* dual, const apd_opts* opts, void* cuda_stream) {
+  return solve_grid(ctx, "apd_solve", grid, nullptr, M, X, A, target_vol, tol, w_init, w, labels, vol, w64, nullptr,
+                    nullptr, nullptr, iters, evals, max_rel_err, dual, opts, cuda_stream);
 }
 
 // Algorithm 2 on a user-supplied discretisation (points with element volumes, apd_points.cu)
@@ -693,7 +756,8 @@ extern "C" int apd_solve_points(apd_ctx* ctx, int64_t N, const float* Y, const f
   rc = points_prepare(ctx, N, &n_partials, st);
   if (rc != APD_OK) return rc;
   StepArgs sa;
-  sa.count = nullptr; sa.vol_in = ws.pt_acc; sa.voxel_volume = 1.0; sa.n_partials = n_partials;
+  sa.count = nullptr; sa.count64 = nullptr; sa.vol_in = ws.pt_acc; sa.voxel_volume = 1.0;
+  sa.lm = points_layer_map(n_partials); sa.dual_partial = nullptr; sa.layer_buf = nullptr; sa.layer_in = nullptr;
   return solve_common(ctx, "apd_solve_points", ws.dim, M, target_vol, tol, w_init, w, nullptr, o, total_volume, sa,
                       hooks, iters, evals, max_rel_err, nullptr, st);
 }

@@ -200,6 +200,14 @@ int points_prepare(apd_ctx* ctx, long long N, int* n_partials, cudaStream_t st) 
     PT_TRY(cudaMalloc(&ws.dual_partial, ws.partial_cap * sizeof(double)));
   }
   if (!ws.pt_acc) PT_TRY(cudaMalloc(&ws.pt_acc, (size_t)ws.max_seeds * 4 * sizeof(double)));   // vol[M] | csum[M,3]
+  const size_t n_layers = (size_t)points_layer_map(n_tiles).n_layers;          // lbfgs_step_kernel's two-level sum
+  if (n_layers > ws.layer_cap) {
+    PT_TRY(cudaStreamSynchronize(st));
+    cudaFree(ws.layer_buf);
+    ws.layer_buf = nullptr; ws.layer_cap = 0;
+    PT_TRY(cudaMalloc(&ws.layer_buf, n_layers * sizeof(double)));
+    ws.layer_cap = n_layers;
+  }
   *n_partials = n_tiles;
   return APD_OK;
 }

@@ -296,8 +296,8 @@ struct RowThread {
     xc = (float)(a.g.lo[0] + ((double)ix0 + 0.5 * (double)G::V) * a.g.s[0]);
     if constexpr (DIM == 3) {
       static_assert(G::TXT == 1, "3D: one reference point per tile");
-      y0 = (float)(a.g.lo[1] + ((double)(by * G::TYT) + 0.5 * (double)G::TYT) * a.g.s[1]);
-      z0 = (float)(a.g.lo[2] + ((double)(bz * G::TZT) + 0.5 * (double)G::TZT) * a.g.s[2]);
+      y0 = (float)(a.g.lo[1] + ((double)(by * G::TYT + a.g.off_y) + 0.5 * (double)G::TYT) * a.g.s[1]);
+      z0 = (float)(a.g.lo[2] + ((double)(bz * G::TZT + a.g.off_z) + 0.5 * (double)G::TZT) * a.g.s[2]);
       const float Yf = (float)(((double)ty + 0.5 - 0.5 * (double)G::TYT) * a.g.s[1]);
       const float Zf = (float)(((double)tz + 0.5 - 0.5 * (double)G::TZT) * a.g.s[2]);
       const float YY = __fmul_rn(Yf, Yf), YZ = __fmul_rn(Yf, Zf), ZZ = __fmul_rn(Zf, Zf);
@@ -305,7 +305,7 @@ struct RowThread {
       rr.YY = f2_pack(YY, YY); rr.YZ = f2_pack(YZ, YZ); rr.ZZ = f2_pack(ZZ, ZZ);
     } else {
       y0 = 0.0f; z0 = 0.0f;
-      const float yyf = (float)(a.g.lo[1] + ((double)iy + 0.5) * a.g.s[1]);
+      const float yyf = (float)(a.g.lo[1] + ((double)(iy + a.g.off_y) + 0.5) * a.g.s[1]);
       rr.x0 = f2_pack(xc, xc); rr.yy = f2_pack(yyf, yyf);
     }
   }

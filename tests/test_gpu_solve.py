@@ -69,37 +69,80 @@ def test_cfg1_full(apd):
     print(f"cfg1: iters {info.iters} evals {info.evals} err {info.max_rel_err:.4g}")
 
 
-def check_prefix(wl, hist_gpu, orc, min_prefix):
-    """Parity rule 5 fallback: when a branch of the optimiser flips on a near-tie voxel count the two
-    runs leave the common path; up to there every evaluation must agree -- dual to 1e-5 relative and the error
-    to a few voxels of the smallest cell."""
+def flips_along_path(apd, wl, orc, kernel, cull, which=None):
+    """Voxels whose GPU label differs from the oracle's, at the ORACLE's own iterates fl32(w_k) (k in `which`, default
+    all): the fp32 kernels against the fp64 definition on identical inputs.  Each such evaluation is also held to parity
+    rules 1-3 (labels near-ties only, counts within 2 x flips, dual 1e-6).  Returns {k: flips}."""
+    from test_gpu_assign import run_assign
+    grid = parity.grid_of(wl)
+    ctx = apd.ApdContext(wl.dim, wl.M)
+    out = {}
+    for k in (range(len(orc.trajectory)) if which is None else which):
+        w32 = orc.trajectory[k]["w"].astype(np.float32)
+        r = run_assign(apd, wl, w32, v=wl.v, kernel=kernel, cull=cull, ctx=ctx)
+        o = oracle_assign(grid, wl.X, wl.A, w32, v=wl.v)
+        info = parity.check_assign(wl, w32, r["labels"], r["vol"], r["dual"], v=wl.v, err_gpu=r["err"], orc=o)
+        out[k] = info["mismatches"]
+    ctx.close()
+    return out
+
+
+def check_prefix(wl, hist_gpu, orc, flips):
+    """Parity rule 5, part (ii).  The two optimisers receive identical inputs -- integer counts,
+    hence identical fp64 gradients -- until the first evaluation at which some voxel's fp32 label differs from the fp64
+    one.  Up to (excluding) that evaluation the recorded (dual, error) histories must agree to rounding: error
+    exactly (same integers), dual to rule 3's 1e-6 relative (measured: 1e-10 CUDA-core kernels, 4e-8 TENSOR).  From that evaluation on one flipped
+    voxel changes two gradient entries by |P| and L-BFGS amplifies it: nothing is asserted about the path there (the
+    evaluation AT the oracle's iterates is still checked, by flips_along_path).  Returns the length of that prefix."""
     dual_g, err_g = hist_gpu
     dual_o = np.array([-t["f"] for t in orc.trajectory]); err_o = np.array([t["err"] for t in orc.trajectory])
     n = min(len(dual_g), len(dual_o))
-    P = parity.grid_of(wl).voxel_volume
-    ok = (np.abs(dual_g[:n] - dual_o[:n]) <= 1e-5 * np.abs(dual_o[:n])) & \
-         (np.abs(err_g[:n] - err_o[:n]) <= 6 * P / float(wl.v.min()) + 1e-3 * err_o[:n])
-    first_bad = int(np.argmin(ok)) if not ok.all() else n
-    assert first_bad >= min(min_prefix, n), f"histories agree only on the first {first_bad} evaluations"
-    return first_bad
+    ks = sorted(flips)
+    first_flip = next((k for k in ks if flips[k] > 0), None)
+    # evaluations known to be flip-free: the checked ones before the first flip, contiguous from 0
+    clean = 0
+    for k in ks:
+        if k != clean or flips[k] > 0:
+            break
+        clean += 1
+    clean = min(clean, n)
+    if clean:
+        assert np.array_equal(err_g[:clean], err_o[:clean]) or np.abs(err_g[:clean] - err_o[:clean]).max() <= 1e-12, \
+            "error histories differ before any voxel flipped"
+        assert np.all(np.abs(dual_g[:clean] - dual_o[:clean]) <= 1e-6 * np.abs(dual_o[:clean]))      # parity rule 3
+    return clean, first_flip
 
 
-@pytest.mark.parametrize("kernel,cull", [(1, 0), (2, 0), (2, 1)])
-# wtol: 1e-4 (north_star) holds when no voxel label flips between fp32 and fp64 anywhere on the path; ONE flipped
-# near-tie voxel perturbs a gradient entry by |P| (~1/1700 of a cell here) and the weights by ~1e-3 relative, so
-# the 3D cases, whose paths cross ~1 such voxel (2e-7 N per evaluation), are held to 5e-3 (DESIGN.md, parity rule 5).
-@pytest.mark.parametrize("cfg,n,M,eps,wtol", [(2, (256, 256), 60, 0.01, 1e-4), (3, (64, 64, 64), 80, 0.01, 5e-3),
-                                              (4, (96, 96, 96), 150, 0.02, 5e-3), (5, (80, 80, 80), 120, 0.02, 5e-3)])
-def test_reduced_configs_trajectory(apd, cfg, n, M, eps, wtol, kernel, cull):
+@pytest.mark.parametrize("kernel,cull", [(1, 0), (2, 0), (2, 1), (3, 0)])
+@pytest.mark.parametrize("cfg,n,M,eps", [(2, (256, 256), 60, 0.01), (3, (64, 64, 64), 80, 0.01),
+                                         (4, (96, 96, 96), 150, 0.02), (5, (80, 80, 80), 120, 0.02)])
+def test_reduced_configs_trajectory(apd, cfg, n, M, eps, kernel, cull):
+    """Parity rule 5 with its tolerance backed by a measurement: the label flips between the fp32 kernel and the fp64
+    oracle are COUNTED at every iterate of the oracle's path.  No flip anywhere => both optimisers see identical
+    integer gradients => same iters/evals and north_star's 1e-4 on the centred weights.  Otherwise the histories must
+    agree exactly up to the first flip, the status must agree, and the oracle's own evaluation at the GPU's weights
+    must meet the tolerance (check_against_oracle)."""
     wl = workloads.make_config(cfg, n=n, M=M)
+    if kernel == 3 and wl.dim == 2:
+        pytest.skip("APD_KERNEL_TENSOR is 3D only")
     orc = oracle_solve(parity.grid_of(wl), wl.X, wl.A, wl.v, eps, record=True)
+    flips = flips_along_path(apd, wl, orc, kernel, cull)
     info, w32, w64, labels, vol, hist = run_solve(apd, wl, eps, kernel=kernel, cull=cull, want_hist=True)
     assert len(hist[0]) == info.evals
-    same = check_against_oracle(wl, eps, info, w32, w64, labels, vol, orc, require_same_path=False, wtol=wtol)
-    prefix = check_prefix(wl, hist, orc, min_prefix=8)
-    print(f"cfg{cfg} reduced kernel {kernel} cull {cull}: gpu {info.iters}/{info.evals}/{info.status} err "
-          f"{info.max_rel_err:.4g}; oracle {orc.iters}/{orc.evals}/{orc.status} err {orc.err:.4g}; same path: {same}; "
-          f"common prefix {prefix} evaluations")
+    total = sum(flips.values())
+    # weights: north_star's 1e-4 when no voxel flips on the path (measured: 6e-16); with flips and still the same
+    # iters/evals 2e-3 = 2 x the worst deviation measured (9.0e-4, DESIGN.md section 8); else nothing (fallback rule)
+    same = check_against_oracle(wl, eps, info, w32, w64, labels, vol, orc, require_same_path=(total == 0),
+                                wtol=1e-4 if total == 0 else 2e-3)
+    clean, first_flip = check_prefix(wl, hist, orc, flips)
+    a = w64 - w64.mean(); b = orc.w - orc.w.mean()
+    dev = float(np.abs(a - b).max() / np.abs(b).max())
+    print(f"RULE5 cfg{cfg} {n} M={M} kernel {kernel} cull {cull}: gpu {info.iters}/{info.evals}/{info.status} err "
+          f"{info.max_rel_err:.4g}; oracle {orc.iters}/{orc.evals}/{orc.status} err {orc.err:.4g}; flipped voxels along the "
+          f"oracle's path: total {total} in {sum(f > 0 for f in flips.values())} of {len(flips)} evaluations (max "
+          f"{max(flips.values())}), first at evaluation {first_flip}; flip-free prefix {clean}; same iters/evals: {same}; "
+          f"centred-weight deviation {dev:.3e}")
+    assert max(flips.values()) <= max(2, int(1e-5 * wl.N))
     assert info.status == orc.status
     if not same:      # both converged, by different last steps: the counts must still be close
         assert abs(info.evals - orc.evals) <= max(4, orc.evals // 4)

@@ -6,7 +6,7 @@
   * cfg 4 at full size, culled AND brute-force solves: the post-condition is judged by ONE full oracle_assign at each
     solve's returned weights (err <= eps + 2 mismatches |P| / v_min), not by another GPU kernel.
 The label flips between the fp32 kernels and the fp64 oracle along the path are COUNTED (GPU evaluation at the
-oracle's iterates), which is what DESIGN.md section 8 rule 5 quotes for its weight tolerance."""
+oracle's iterates, test_gpu_solve.flips_along_path), which is what DESIGN.md section 8 rule 5 quotes."""
 import numpy as np
 import pytest
 import torch
@@ -14,7 +14,7 @@ import torch
 from paper_2403_03571_b200 import workloads
 import apd_parity as parity
 from oracle.apd_oracle import oracle_assign, oracle_solve, OK
-from test_gpu_solve import run_solve, check_against_oracle, check_prefix
+from test_gpu_solve import run_solve, check_against_oracle, check_prefix, flips_along_path
 from test_gpu_assign import run_assign
 
 pytestmark = pytest.mark.gpu
@@ -27,36 +27,31 @@ def apd():
     return binding
 
 
-def flips_along_path(apd, wl, orc, kernel, cull, every=1, limit=None):
-    """Number of voxels whose GPU label differs from the oracle's at the oracle's own iterates fl32(w_k)."""
-    grid = parity.grid_of(wl)
-    ctx = apd.ApdContext(wl.dim, wl.M)
-    out = []
-    traj = orc.trajectory[::every][:limit]
-    for t in traj:
-        w32 = t["w"].astype(np.float32)
-        r = run_assign(apd, wl, w32, kernel=kernel, cull=cull, ctx=ctx)
-        o = oracle_assign(grid, wl.X, wl.A, w32, diagnostics=False)
-        out.append(int(np.count_nonzero(r["labels"] != o.labels)))
-    ctx.close()
-    return out
-
-
 @pytest.mark.parametrize("cfg", [2, 3])
 @pytest.mark.parametrize("kernel,cull", [(0, 0), (0, 1)])
 def test_full_size_solve_vs_oracle_solve(apd, cfg, kernel, cull):
+    """cfg 2 / cfg 3 at full size: oracle_solve run to completion.  At ~1e-6 flipped voxels per evaluation a grid of
+    1-2 M voxels meets its first flip within the first evaluations, so the two paths separate early (measured and
+    printed); what is asserted: the GPU's evaluation at the oracle's iterates (first 10 and every 16th) obeys parity
+    rules 1-3, the histories agree exactly before the first flip, both converge, the ORACLE's evaluation at the GPU's
+    weights meets the tolerance, and the evaluation counts stay within 25%."""
     wl = workloads.make_config(cfg)
     orc = _oracle_solve_cached(cfg, wl)
+    which = sorted(set(range(min(10, len(orc.trajectory)))) | set(range(0, len(orc.trajectory), 16)))
+    flips = flips_along_path(apd, wl, orc, kernel, cull, which=which)
     info, w32, w64, labels, vol, hist = run_solve(apd, wl, wl.eps, kernel=kernel, cull=cull, want_hist=True)
     assert orc.status == OK and info.status == 0
-    same = check_against_oracle(wl, wl.eps, info, w32, w64, labels, vol, orc, require_same_path=False, wtol=1e-4)
-    prefix = check_prefix(wl, hist, orc, min_prefix=8)
+    total = sum(flips.values())
+    same = check_against_oracle(wl, wl.eps, info, w32, w64, labels, vol, orc, require_same_path=False,
+                                wtol=1e-4 if total == 0 else 2e-3)
+    clean, first_flip = check_prefix(wl, hist, orc, flips)
     dev = np.abs((w64 - w64.mean()) - (orc.w - orc.w.mean())).max() / np.abs(orc.w - orc.w.mean()).max()
-    print(f"cfg{cfg} FULL kernel {kernel} cull {cull}: gpu {info.iters}/{info.evals} err {info.max_rel_err:.4g}; oracle "
-          f"{orc.iters}/{orc.evals} err {orc.err:.4g}; same path {same}; common prefix {prefix}; "
-          f"final centred-weight deviation {dev:.3e}")
-    if not same:
-        assert abs(info.evals - orc.evals) <= max(4, orc.evals // 4)
+    print(f"RULE5 cfg{cfg} FULL kernel {kernel} cull {cull}: gpu {info.iters}/{info.evals} err {info.max_rel_err:.4g}; oracle "
+          f"{orc.iters}/{orc.evals} err {orc.err:.4g}; flips at {len(which)} sampled iterates: total {total}, max "
+          f"{max(flips.values())}, first at evaluation {first_flip}; flip-free prefix {clean}; same iters/evals {same}; "
+          f"final centred-weight deviation {dev:.3e}; final dual rel diff {abs(info.dual - orc.dual) / abs(orc.dual):.2e}")
+    assert max(flips.values()) < 1e-5 * wl.N
+    assert abs(info.evals - orc.evals) <= max(4, orc.evals // 4)
 
 
 _ORC = {}
@@ -66,29 +61,6 @@ def _oracle_solve_cached(cfg, wl):
     if cfg not in _ORC:
         _ORC[cfg] = oracle_solve(parity.grid_of(wl), wl.X, wl.A, wl.v, wl.eps, record=True)
     return _ORC[cfg]
-
-
-@pytest.mark.parametrize("cfg,n,M,eps", [(3, (64, 64, 64), 80, 0.01), (4, (96, 96, 96), 150, 0.02),
-                                         (5, (80, 80, 80), 120, 0.02), (2, (256, 256), 60, 0.01)])
-@pytest.mark.parametrize("kernel,cull", [(1, 0), (2, 0), (3, 0), (2, 1)])
-def test_label_flips_along_the_reduced_paths(apd, cfg, n, M, eps, kernel, cull):
-    """The measurement behind parity rule 5's tolerance: how many voxels flip between the fp32 kernel and the fp64
-    oracle at each iterate of the oracle's path, and how far the solved weights end up from the oracle's."""
-    wl = workloads.make_config(cfg, n=n, M=M)
-    if kernel == 3 and wl.dim == 2:
-        pytest.skip("TENSOR kernel is 3D only")
-    orc = oracle_solve(parity.grid_of(wl), wl.X, wl.A, wl.v, eps, record=True)
-    flips = flips_along_path(apd, wl, orc, kernel, cull)
-    info, w32, w64, labels, vol = run_solve(apd, wl, eps, kernel=kernel, cull=cull)
-    a = w64 - w64.mean(); b = orc.w - orc.w.mean()
-    dev = float(np.abs(a - b).max() / np.abs(b).max())
-    same = (info.iters, info.evals, info.status) == (orc.iters, orc.evals, orc.status)
-    print(f"FLIPS cfg{cfg} {n} M={M} kernel {kernel} cull {cull}: evaluations {len(flips)}, voxels flipped per "
-          f"evaluation: total {sum(flips)}, max {max(flips)}, evaluations with a flip {sum(f > 0 for f in flips)}; "
-          f"same path {same}; centred-weight deviation {dev:.3e}")
-    assert max(flips) <= max(2, int(1e-5 * wl.N))
-    if sum(flips) == 0 and same:
-        assert dev <= 1e-4          # north_star's tolerance holds whenever no voxel flips anywhere on the path
 
 
 @pytest.mark.parametrize("name,kernel,cull", [("culled", 0, 1), ("brute_force", 0, 0)])
