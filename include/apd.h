@@ -48,11 +48,12 @@ typedef struct {
 /* Which implementation of the voxel x seed reduction runs (all give labels by the same rule:
  * fp32 cost, lowest seed index among equal fp32 costs). */
 enum {
-  APD_KERNEL_AUTO   = 0,   /* the fastest one: APD_KERNEL_ROWPOLY, except on grids with n[0] < 8 (3D
-                              also n[1] < 8 or n[2] < 4), which take APD_KERNEL_DIRECT (and ignore
-                              opts.cull): the row kernels expand the cost about the midpoint of a
-                              row / tile, which there lies up to 8/n domain widths L outside the
-                              domain: a cost then carries a few fp32 ulp of a ((1 + 8/n) L)^2
+  APD_KERNEL_AUTO   = 0,   /* the fastest one for the call.  Brute force in 3D: APD_KERNEL_TENSOR when M >= 1536, or
+                              when M >= 384 on a grid too small for ROWPOLY's long rows (below ~3.6 M voxels);
+                              otherwise, in 2D and with opts.cull: APD_KERNEL_ROWPOLY.  Grids with n[0] < 8 (3D also
+                              n[1] < 8 or n[2] < 4) take APD_KERNEL_DIRECT (and ignore opts.cull): the row kernels
+                              expand the cost about the midpoint of a row / tile, which there lies up to 8/n domain
+                              widths L outside the domain: a cost then carries a few fp32 ulp of a ((1 + 8/n) L)^2
                               instead of a few ulp of itself                                        */
   APD_KERNEL_DIRECT = 1,   /* un-hoisted direct form: 12 (3D) / 7 (2D) FP32 instr. per pair;
                               the reference kernel the FP32-pipe fraction is quoted on             */
@@ -63,14 +64,15 @@ enum {
                               polynomial in the integer voxel offset from a tile's reference voxel,
                               coefficients split three ways into bf16, contracted on the tensor
                               cores (tcgen05.mma, fp32 accumulators in TMEM); argmin epilogue on
-                              the CUDA cores.  Costs carry fp32 rounding; never chosen by AUTO     */
+                              the CUDA cores.  Costs carry fp32 rounding                           */
 };
 
 /* opts.cull = 1: exact culling (not in the paper).  Per block of voxels the library keeps only
  * the seeds that can be an argmin somewhere in the block (bounds from the triangle inequality in the A_i-norm, taken
  * conservatively in fp32), nested super-tile -> tile -> 16x4x8-voxel brick, and evaluates those.  The labels are those
- * of the brute-force reduction with the same fp32 arithmetic (identical bit for bit whenever brute force runs the same
- * short-row kernel, i.e. on grids below ~10^3 long-row tiles; on larger grids the two can differ on fp32 near-ties).
+ * of the brute-force reduction with the same fp32 arithmetic: identical bit for bit to APD_KERNEL_ROWPOLY without culling
+ * whenever that runs its short rows (grids below ~10^3 long-row tiles); against the long-row or the TENSOR brute-force
+ * kernels (what AUTO picks on large grids / many seeds) the labels can differ on fp32 near-ties only.
  * Requires kernel AUTO or ROWPOLY and positive definite A_i (not checked).  Workspace grows by
  * O(number of bricks): 1 KiB per 512 voxels.  pairs_evaluated reports the pairs actually evaluated. */
 typedef struct {

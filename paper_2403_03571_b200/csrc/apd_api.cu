@@ -156,7 +156,7 @@ static bool narrow_grid(const apd_grid* grid) {
   if (grid->n[0] < 8) return true;
   return grid->dim == 3 && (grid->n[1] < 8 || grid->n[2] < 4);
 }
-int resolve_kernel(const apd_opts* o, const apd_grid* grid, bool* cull, std::string* err) {
+int resolve_kernel(const apd_ctx* ctx, const apd_opts* o, const apd_grid* grid, int M, bool* cull, std::string* err) {
   int k = o ? o->kernel : APD_KERNEL_AUTO;
   if (k != APD_KERNEL_AUTO && k != APD_KERNEL_DIRECT && k != APD_KERNEL_ROWPOLY && k != APD_KERNEL_TENSOR) { *err = "unknown opts.kernel"; return -1; }
   if (k == APD_KERNEL_TENSOR && grid && grid->dim != 3) { *err = "APD_KERNEL_TENSOR is 3D only"; return -1; }
@@ -166,6 +166,14 @@ int resolve_kernel(const apd_opts* o, const apd_grid* grid, bool* cull, std::str
   if (k == APD_KERNEL_AUTO) {
     if (narrow_grid(grid)) { *cull = false; return APD_KERNEL_DIRECT; }
     k = APD_KERNEL_ROWPOLY;
+    // brute force in 3D: the tensor-core kernel once there are enough seeds to amortise its per-tile set-up (Phi, TMEM,
+    // pipeline fill: ~3 chunks of 128 seeds).  Measured on B200: TENSOR / ROWPOLY time 0.63-0.75 at
+    // M >= 2000, 0.92 (128^3) and 1.10 (256^3, where ROWPOLY runs its long rows) at M = 1000, 1.09-1.2 at M <= 256.
+    if (grid && grid->dim == 3 && !*cull && ctx) {
+      int tx, ty, tz;
+      const bool long_rows = rowpoly_tile_counts(3, grid->n[0], grid->n[1], grid->n[2], ctx->ws.sm_count, false, &tx, &ty, &tz) != 0;
+      if (M >= 1536 || (!long_rows && M >= 384)) k = APD_KERNEL_TENSOR;
+    }
   }
   if (*cull && k != APD_KERNEL_ROWPOLY) { *err = "opts.cull needs kernel AUTO or ROWPOLY"; return -1; }
   return k;
@@ -283,7 +291,7 @@ extern "C" int apd_assign(apd_ctx* ctx, const apd_grid* grid, int32_t M, const f
   ctx->err.clear();
   std::string e;
   bool cull = false;
-  const int kernel = resolve_kernel(opts, grid, &cull, &e);
+  const int kernel = resolve_kernel(ctx, opts, grid, M, &cull, &e);
   if (kernel < 0) { ctx->err = "apd_assign: " + e; return APD_E_ARG; }
   if (M < 1 || M > ctx->ws.max_seeds) { ctx->err = "apd_assign: M out of range [1, max_seeds]"; return APD_E_ARG; }
   if (!X || !A || !w || !vol || !dual) { ctx->err = "apd_assign: X, A, w, vol and dual are required"; return APD_E_ARG; }
@@ -323,7 +331,7 @@ extern "C" int apd_reserve(apd_ctx* ctx, const apd_grid* grid, const apd_opts* o
   ctx->err.clear();
   std::string e;
   bool cull = false;
-  const int kernel = resolve_kernel(opts, grid, &cull, &e);
+  const int kernel = resolve_kernel(ctx, opts, grid, ctx->ws.max_seeds, &cull, &e);
   if (kernel < 0) { ctx->err = "apd_reserve: " + e; return APD_E_ARG; }
   GridDev g;
   e = make_grid(ctx, grid, kernel, cull, &g);
@@ -331,6 +339,16 @@ extern "C" int apd_reserve(apd_ctx* ctx, const apd_grid* grid, const apd_opts* o
   APD_CUDA_TRY(ctx, cudaSetDevice(ctx->ws.device));
   int rc = ensure_eval_buffers(ctx, g, kernel, cull, nullptr);
   if (rc != APD_OK) return rc;
+  if ((!opts || opts->kernel == APD_KERNEL_AUTO) && grid->dim == 3 && !cull) {
+    // AUTO picks ROWPOLY or TENSOR by the number of seeds of the call: size the workspace for both
+    for (int k2 : {APD_KERNEL_ROWPOLY, APD_KERNEL_TENSOR}) {
+      GridDev g2;
+      e = make_grid(ctx, grid, k2, false, &g2);
+      if (!e.empty()) { ctx->err = "apd_reserve: " + e; return APD_E_ARG; }
+      rc = ensure_eval_buffers(ctx, g2, k2, false, nullptr);
+      if (rc != APD_OK) return rc;
+    }
+  }
   const int hist = opts ? opts->lbfgs_history : 10;
   if (hist < 1 || hist > 64) { ctx->err = "apd_reserve: lbfgs_history must be in [1,64]"; return APD_E_ARG; }
   rc = ensure_solve_state(ctx, hist);

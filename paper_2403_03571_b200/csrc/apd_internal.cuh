@@ -200,7 +200,7 @@ struct SolveReport {
 std::string make_grid(const apd_ctx* ctx, const apd_grid* grid, int kernel, bool cull, GridDev* g,
                       const apd_slab* slab = nullptr);
 LayerMap layer_map(const GridDev& g, bool cull);
-int resolve_kernel(const apd_opts* o, const apd_grid* grid, bool* cull, std::string* err);
+int resolve_kernel(const apd_ctx* ctx, const apd_opts* o, const apd_grid* grid, int M, bool* cull, std::string* err);
 // Sizes the buffers an evaluation of grid `g` needs (dual partials; with culling the candidate lists and the record
 // table; for the TENSOR kernel its seed table).  Grow-only.  Growing synchronises `st` and reallocates: apd_reserve
 // does this ahead of time so that apd_assign / apd_solve never do.

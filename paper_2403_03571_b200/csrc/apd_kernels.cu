@@ -9,7 +9,6 @@
 #include "apd_device.cuh"
 #include "apd_epilogue.cuh"
 #include <math_constants.h>
-#include <cstdlib>
 
 namespace apd {
 
@@ -122,7 +121,7 @@ __device__ __forceinline__ float direct_cost(const DirectSeed<DIM>& s, float yx,
   }
 }
 
-template <int DIM, int UNROLL>
+template <int DIM>
 __global__ void __launch_bounds__(256) assign_direct_kernel(const AssignArgs a) {
   using G = DirectGeom<DIM>;
   constexpr int V = G::V;
@@ -171,7 +170,7 @@ __global__ void __launch_bounds__(256) assign_direct_kernel(const AssignArgs a) 
       float prev[V];
 #pragma unroll
       for (int k = 0; k < V; ++k) prev[k] = best[k];
-#pragma unroll UNROLL
+#pragma unroll 4
       for (int i = g0; i < g0 + DIRECT_GROUP; ++i) {
         const DirectSeed<DIM> sd = direct_load<DIM>(sp, i);
 #pragma unroll
@@ -226,12 +225,8 @@ cudaError_t launch_assign(int kernel, const AssignArgs& a, cudaStream_t st) {
   if (kernel == APD_KERNEL_ROWPOLY) return launch_assign_rowpoly(a, st);
   if (kernel == APD_KERNEL_TENSOR) return launch_assign_tensor(a, st);
   const int n_tiles = a.g.tiles_x * a.g.tiles_y * a.g.tiles_z;
-  static const int unroll = getenv("APD_DIRECT_UNROLL") ? atoi(getenv("APD_DIRECT_UNROLL")) : 2;   // DEV ONLY
-  if (a.g.dim == 3) {
-    if (unroll == 4) assign_direct_kernel<3, 4><<<n_tiles, 256, 0, st>>>(a);
-    else if (unroll == 1) assign_direct_kernel<3, 1><<<n_tiles, 256, 0, st>>>(a);
-    else assign_direct_kernel<3, 2><<<n_tiles, 256, 0, st>>>(a);
-  } else              assign_direct_kernel<2, 2><<<n_tiles, 256, 0, st>>>(a);
+  if (a.g.dim == 3) assign_direct_kernel<3><<<n_tiles, 256, 0, st>>>(a);
+  else              assign_direct_kernel<2><<<n_tiles, 256, 0, st>>>(a);
   return cudaGetLastError();
 }
 

@@ -76,7 +76,9 @@ constexpr double CULL_CAP_FACTOR = 0.5;     // ... but at most this x the mean m
 // thread of every CTA (lanes by shuffle tree, warps in order, CTAs in rank order), which keeps the control flow
 // uniform over the whole cluster.  Cluster partials are exchanged through distributed shared memory; two buffers
 // are used alternately so that one cluster barrier per reduction suffices.
-constexpr int LB_NRED = 13;                          // most values reduced at once (gram_rows)
+constexpr int LB_GRAM_SLOTS = 10;                    // history slots whose inner products one Gram pass forms at once
+constexpr int LB_NRED = 3 * 2 * LB_GRAM_SLOTS + 1;   // most values reduced at once (gram_rows: 3 new vectors x (S, Y) of
+                                                     // LB_GRAM_SLOTS slots, + g.g)
 
 struct Reducer {
   double* wbuf;        // [LB_THREADS / 32][LB_NRED]   warp partials of this CTA
@@ -86,11 +88,13 @@ struct Reducer {
   unsigned int rank;
 };
 
-template <int N, bool MAX>
-__device__ __forceinline__ void cluster_all(double (&v)[N], Reducer& r) {
+// v[0 .. N-NMAX) are SUMMED, v[N-NMAX .. N) are MAXIMISED, all in one exchange (one cluster barrier)
+template <int N, int NMAX>
+__device__ __forceinline__ void cluster_all_mixed(double (&v)[N], Reducer& r) {
   cg::cluster_group cluster = cg::this_cluster();
 #pragma unroll
   for (int n = 0; n < N; ++n) {
+    const bool MAX = n >= N - NMAX;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
       const double u = __shfl_xor_sync(0xffffffffu, v[n], o);
@@ -107,6 +111,7 @@ __device__ __forceinline__ void cluster_all(double (&v)[N], Reducer& r) {
   r.flip ^= 1;
   double* mine = r.cbuf + r.flip * LB_NRED;
   if (threadIdx.x < N) {
+    const bool MAX = (int)threadIdx.x >= N - NMAX;
     double t = r.wbuf[threadIdx.x];
 #pragma unroll
     for (int k = 1; k < LB_THREADS / 32; ++k) {
@@ -119,6 +124,7 @@ __device__ __forceinline__ void cluster_all(double (&v)[N], Reducer& r) {
   // N threads fetch the other CTAs' totals (one distributed-shared-memory read each: every thread reading all of
   // them cost more than the sweeps), add them in rank order and hand the result to the CTA through shared memory
   if (threadIdx.x < N) {
+    const bool MAX = (int)threadIdx.x >= N - NMAX;
     double t = cluster.map_shared_rank(mine, 0)[threadIdx.x];
 #pragma unroll
     for (int c = 1; c < LB_CLUSTER; ++c) {
@@ -131,6 +137,8 @@ __device__ __forceinline__ void cluster_all(double (&v)[N], Reducer& r) {
 #pragma unroll
   for (int n = 0; n < N; ++n) v[n] = r.tot[n];
 }
+template <int N, bool MAX>
+__device__ __forceinline__ void cluster_all(double (&v)[N], Reducer& r) { cluster_all_mixed<N, MAX ? N : 0>(v, r); }
 
 __device__ __forceinline__ double cluster_allsum(double x, Reducer& r) {
   double v[1] = {x};
@@ -161,7 +169,10 @@ __device__ __forceinline__ double* gram_of(const StepArgs& a, int cap, unsigned 
 }
 
 // Inner products of the NNEW vectors nv[] (Gram indices nidx[]; nv[NNEW-1] is g) with S_j and Y_j of every active
-// slot, and g.g, written to both triangles of this CTA's Gram copy.
+// slot, and g.g, written to both triangles of this CTA's Gram copy.  LB_GRAM_SLOTS slots per pass over the vectors (one
+// pass and ONE cluster barrier for the default history of 10; it used to be one barrier per two slots): every inner
+// product is accumulated per thread in the same element order and reduced by the same tree as before, so its bits do
+// not depend on how many are formed at once.
 template <int NNEW>
 __device__ void gram_rows(const StepArgs& a, int cap, int hist_len, int hist_start, const double* (&nv)[NNEW],
                           const int (&nidx)[NNEW], Reducer& r) {
@@ -169,38 +180,39 @@ __device__ void gram_rows(const StepArgs& a, int cap, int hist_len, int hist_sta
   const double* S = a.vec + (size_t)V_HIST * stride;
   const double* Y = S + (size_t)cap * stride;
   double* gm = gram_of(a, cap, r.rank);
-  for (int t0 = 0; t0 < hist_len; t0 += 2) {
-    const bool has1 = t0 + 1 < hist_len;
-    const int j0 = (hist_start + t0) % cap, j1 = has1 ? (hist_start + t0 + 1) % cap : j0;
-    const double *s0 = S + (size_t)j0 * stride, *y0 = Y + (size_t)j0 * stride;
-    const double *s1 = S + (size_t)j1 * stride, *y1 = Y + (size_t)j1 * stride;
-    double acc[LB_NRED];
+  constexpr int NS = LB_GRAM_SLOTS, NACC = NNEW * 2 * NS + 1;
+  for (int t0 = 0; t0 < hist_len; t0 += NS) {
+    const int ns = min(NS, hist_len - t0);
+    int slot[NS];
 #pragma unroll
-    for (int n = 0; n < LB_NRED; ++n) acc[n] = 0.0;
+    for (int q = 0; q < NS; ++q) slot[q] = (hist_start + t0 + (q < ns ? q : 0)) % cap;   // inactive: a duplicate, ignored
+    double acc[NACC];
+#pragma unroll
+    for (int n = 0; n < NACC; ++n) acc[n] = 0.0;
     for (int i = LB_FIRST(r); i < M; i += LB_STEP) {
-      const double a0 = s0[i], b0 = y0[i], a1 = s1[i], b1 = y1[i];
       double x[NNEW];
 #pragma unroll
       for (int n = 0; n < NNEW; ++n) x[n] = nv[n][i];
 #pragma unroll
-      for (int n = 0; n < NNEW; ++n) {
-        acc[4 * n + 0] += x[n] * a0; acc[4 * n + 1] += x[n] * b0;
-        acc[4 * n + 2] += x[n] * a1; acc[4 * n + 3] += x[n] * b1;
+      for (int q = 0; q < NS; ++q) {
+        const double sv = S[(size_t)slot[q] * stride + i], yv = Y[(size_t)slot[q] * stride + i];
+#pragma unroll
+        for (int n = 0; n < NNEW; ++n) { acc[(n * NS + q) * 2] += x[n] * sv; acc[(n * NS + q) * 2 + 1] += x[n] * yv; }
       }
-      acc[12] += x[NNEW - 1] * x[NNEW - 1];
+      acc[NACC - 1] += x[NNEW - 1] * x[NNEW - 1];
     }
-    cluster_all<LB_NRED, false>(acc, r);
+    cluster_all<NACC, false>(acc, r);
     if (threadIdx.x == 0) {
       for (int n = 0; n < NNEW; ++n) {
         const int q = nidx[n];
-        gm[(size_t)q * ld + j0] = acc[4 * n + 0]; gm[(size_t)j0 * ld + q] = acc[4 * n + 0];
-        gm[(size_t)q * ld + cap + j0] = acc[4 * n + 1]; gm[(size_t)(cap + j0) * ld + q] = acc[4 * n + 1];
-        if (has1) {
-          gm[(size_t)q * ld + j1] = acc[4 * n + 2]; gm[(size_t)j1 * ld + q] = acc[4 * n + 2];
-          gm[(size_t)q * ld + cap + j1] = acc[4 * n + 3]; gm[(size_t)(cap + j1) * ld + q] = acc[4 * n + 3];
+        for (int k = 0; k < ns; ++k) {
+          const int j = slot[k];
+          const double vs = acc[(n * NS + k) * 2], vy = acc[(n * NS + k) * 2 + 1];
+          gm[(size_t)q * ld + j] = vs; gm[(size_t)j * ld + q] = vs;
+          gm[(size_t)q * ld + cap + j] = vy; gm[(size_t)(cap + j) * ld + q] = vy;
         }
       }
-      if (t0 == 0) gm[(size_t)(2 * cap) * ld + 2 * cap] = acc[12];
+      if (t0 == 0) gm[(size_t)(2 * cap) * ld + 2 * cap] = acc[NACC - 1];
     }
   }
   __syncthreads();          // thread 0's global writes are ordered before the CTA's reads in direction_vf
@@ -334,13 +346,25 @@ __global__ void __cluster_dims__(LB_CLUSTER, 1, 1) __launch_bounds__(LB_THREADS)
 
   // a9 for the loop: g~ = <v, fl32 w> + |P| sum_j min_i C_ij (identity I1), eq. (2.5) error
   const double P = a.voxel_volume;
-  double s0[2] = {0.0, 0.0};
-  double emax = 0.0;
+  // ONE sweep and ONE exchange for everything that depends only on the evaluation just run and on the state at
+  // entry: <v, fl32 w> and the eq. (2.5) error (a9), the gradient of f at the evaluated point, vol - v (eq. 2.8), and,
+  // speculatively, every inner product the line-search tests and the curvature pair need (s = alpha p, y = g1 - g).
+  // Each sum is accumulated per thread in element order and reduced by the same tree whatever shares the exchange.
+  double red8[8] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};   // <v,w32>, sum v, g1.p, s.y, s.s, y.y, (unused), max err
   for (int i = LB_FIRST(red); i < M; i += LB_STEP) {
     const double tv = (double)a.v[i];
-    s0[0] += tv * (double)a.w32[i];
+    red8[0] += tv * (double)a.w32[i];
     const double vi = a.vol_in ? a.vol_in[i] : (a.count64 ? (double)a.count64[i] : (double)a.count[i]) * P;
-    emax = fmax(emax, fabs(vi - tv) / tv);
+    red8[7] = fmax(red8[7], fabs(vi - tv) / tv);
+    const double gn = vi - tv;                                  // m_i |P| - v_i
+    gnew[i] = gn;
+    red8[1] += tv;
+    if (phase != 0) {
+      const double pi = p[i];
+      const double si = __dmul_rn(alpha, pi);
+      const double yi = __dsub_rn(gn, g[i]);
+      red8[2] += gn * pi; red8[3] += si * yi; red8[4] += si * si; red8[5] += yi * yi;
+    }
   }
   // sum of the minima, two-level (apd_internal.cuh): layer sums by one warp each, in a fixed order ...
   if (!a.layer_in) {
@@ -350,8 +374,7 @@ __global__ void __cluster_dims__(LB_CLUSTER, 1, 1) __launch_bounds__(LB_THREADS)
       if ((tid & 31) == 0) a.layer_buf[L] = ls;
     }
   }
-  cluster_all<2, false>(s0, red);          // (its cluster barrier also publishes the layer sums to every CTA)
-  const double err1 = cluster_allmax(emax, red);
+  cluster_all_mixed<8, 1>(red8, red);      // (its cluster barrier also publishes the layer sums to every CTA)
   // ... then the layers in ascending order: the same bits in every CTA, and in a slab-sharded solve
   {
     const double* lsrc = a.layer_in ? a.layer_in : a.layer_buf;
@@ -361,32 +384,17 @@ __global__ void __cluster_dims__(LB_CLUSTER, 1, 1) __launch_bounds__(LB_THREADS)
       s_smin = t;
     }
     __syncthreads();
-    s0[1] = s_smin;
   }
-  const double dual1 = s0[0] + P * s0[1], f1 = -dual1;
+  const double smin = s_smin;
+  const double err1 = red8[7];
+  const double dual1 = red8[0] + P * smin, f1 = -dual1;
 
-  // ONE sweep: gradient of f at the evaluated point, vol - v (eq. 2.8); the best-so-far copy; and, speculatively,
-  // every inner product the line-search tests and the curvature pair need (s = alpha p, y = g1 - g)
   evals += 1;
   if (lead && tid == 0 && evals <= a.hist_cap) { a.hist[2 * (evals - 1)] = -f1; a.hist[2 * (evals - 1) + 1] = err1; }
   const double* w_eval = (phase == 0) ? w : wtry;
-  const bool improved = err1 < best_err;
+  const bool improved = err1 < best_err;      // the best-so-far copy is made in the last sweep of this call
   if (improved) { best_err = err1; best_dual = -f1; }
-  double sums[5] = {0.0, 0.0, 0.0, 0.0, 0.0};     // sum v, g1.p, s.y, s.s, y.y
-  for (int i = LB_FIRST(red); i < M; i += LB_STEP) {
-    const double tv = (double)a.v[i];
-    const double gn = (a.vol_in ? a.vol_in[i] : (a.count64 ? (double)a.count64[i] : (double)a.count[i]) * P) - tv;   // m_i |P| - v_i
-    gnew[i] = gn;
-    sums[0] += tv;
-    if (improved) wbest[i] = w_eval[i];
-    if (phase != 0) {
-      const double pi = p[i];
-      const double si = __dmul_rn(alpha, pi);
-      const double yi = __dsub_rn(gn, g[i]);
-      sums[1] += gn * pi; sums[2] += si * yi; sums[3] += si * si; sums[4] += yi * yi;
-    }
-  }
-  cluster_all<5, false>(sums, red);
+  const double sums[5] = {red8[1], red8[2], red8[3], red8[4], red8[5]};
   const double vsum = sums[0], g1p = sums[1], sy = sums[2], ss = sums[3], yy = sums[4];
 
   int finish = 0;          // 1: OK at w_eval, 2: NOT_CONVERGED at best, 3: bad target volumes
@@ -394,7 +402,7 @@ __global__ void __cluster_dims__(LB_CLUSTER, 1, 1) __launch_bounds__(LB_THREADS)
   int new_slot = -1;       // ring slot a curvature pair was pushed into by this call, else -1
   if (phase == 0) {
     // cost scale for the list-reuse slack: mean over the voxels of min_i C_ij = (g~ - <v, w>) / |Omega|  (identity I1)
-    const double scale = fabs(P * s0[1]) / domain_volume;
+    const double scale = fabs(P * smin) / domain_volume;
     cull_cap = isfinite(scale) ? (float)(CULL_CAP_FACTOR * scale) : 0.0f;
     // target volumes: v_i > 0 and sum v_i = |Omega| -- with sum v != |Omega| the dual
     // is unbounded along (1,..,1); fp32 inputs normalised in fp64 meet 1e-6 with two orders to spare
@@ -479,6 +487,7 @@ __global__ void __cluster_dims__(LB_CLUSTER, 1, 1) __launch_bounds__(LB_THREADS)
     // next trial point w + alpha p, rounded to fp32 for the evaluation (S10)
     double mx[2] = {0.0, 0.0};   // max |change since the last evaluation|, max |distance from wref|
     for (int i = LB_FIRST(red); i < M; i += LB_STEP) {
+      if (improved) wbest[i] = w_eval[i];      // best-so-far copy of the point just evaluated (before wtry is rewritten)
       const double wt = __dadd_rn(w[i], __dmul_rn(alpha, p[i]));
       wtry[i] = wt;
       const float wn = (float)wt;
@@ -497,7 +506,10 @@ __global__ void __cluster_dims__(LB_CLUSTER, 1, 1) __launch_bounds__(LB_THREADS)
   } else if (finish == 1) {
     if (phase != 0) for (int i = LB_FIRST(red); i < M; i += LB_STEP) w[i] = wtry[i];
   } else if (finish == 2) {
-    for (int i = LB_FIRST(red); i < M; i += LB_STEP) { w[i] = wbest[i]; a.w32[i] = (float)wbest[i]; }
+    for (int i = LB_FIRST(red); i < M; i += LB_STEP) {
+      const double wb = improved ? w_eval[i] : wbest[i];
+      wbest[i] = wb; w[i] = wb; a.w32[i] = (float)wb;
+    }
   }
   cluster.sync();        // no CTA leaves while its shared memory may still be read; all vector writes are done
   if (lead && tid == 0) {
@@ -651,7 +663,7 @@ int apd::solve_grid(apd_ctx* ctx, const char* who, const apd_grid* grid, const a
   const std::string pre = std::string(who) + ": ";
   std::string e;
   bool cull = false;
-  const int kernel = resolve_kernel(opts, grid, &cull, &e);
+  const int kernel = resolve_kernel(ctx, opts, grid, M, &cull, &e);
   if (kernel < 0) { ctx->err = pre + e; return APD_E_ARG; }
   if (M < 1 || M > ctx->ws.max_seeds) { ctx->err = pre + "M out of range [1, max_seeds]"; return APD_E_ARG; }
   if (!X || !A || !target_vol || !w) { ctx->err = pre + "X, A, target_vol and w are required"; return APD_E_ARG; }

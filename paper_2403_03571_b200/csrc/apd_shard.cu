@@ -85,7 +85,7 @@ extern "C" int apd_assign_slab(apd_ctx* ctx, const apd_grid* grid, const apd_sla
   ctx->err.clear();
   std::string e;
   bool cull = false;
-  const int kernel = resolve_kernel(opts, grid, &cull, &e);
+  const int kernel = resolve_kernel(ctx, opts, grid, M, &cull, &e);
   if (kernel < 0) { ctx->err = "apd_assign_slab: " + e; return APD_E_ARG; }
   if (M < 1 || M > ctx->ws.max_seeds) { ctx->err = "apd_assign_slab: M out of range [1, max_seeds]"; return APD_E_ARG; }
   if (!X || !A || !w || !counters || !slab) { ctx->err = "apd_assign_slab: slab, X, A, w and counters are required"; return APD_E_ARG; }

@@ -234,12 +234,12 @@ def test_host_call_with_pinned_labels_writes_them_in_place(apd, kernel, cull):
                                      (5, (128, 128, 128), 2500)])
 @pytest.mark.parametrize("wscale", [0.0, 0.2])
 def test_culling_is_exact(apd, cfg, n, M, wscale):
-    """Labels, volumes and centroids with culling == without, bit for bit (grids small enough that brute force runs
-    the same short-row arithmetic as the culled kernel); the dual up to the order of the fp64 partial sums."""
+    """Labels, volumes and centroids with culling == ROWPOLY without, bit for bit (grids small enough that brute force
+    runs the same short-row arithmetic as the culled kernel); the dual up to the order of the fp64 partial sums."""
     wl = workloads.make_config(cfg, n=n, M=M)
     w = wl.w0 if wscale == 0.0 else rand_w(wl, wscale, 300 + cfg)
-    r0 = run_assign(apd, wl, w, v=wl.v, want_centroids=True, cull=0)
-    r1 = run_assign(apd, wl, w, v=wl.v, want_centroids=True, cull=1)
+    r0 = run_assign(apd, wl, w, v=wl.v, want_centroids=True, cull=0, kernel=KERNELS["rowpoly"])   # (AUTO would take
+    r1 = run_assign(apd, wl, w, v=wl.v, want_centroids=True, cull=1, kernel=KERNELS["rowpoly"])   #  TENSOR at M >= 384)
     assert np.array_equal(r0["labels"], r1["labels"])
     assert np.array_equal(r0["vol"], r1["vol"]) and np.array_equal(r0["centroids"], r1["centroids"])
     assert abs(r1["dual"] - r0["dual"]) <= 1e-13 * abs(r0["dual"]) and r1["err"] == r0["err"]   # same fp32 minima
@@ -254,7 +254,7 @@ def test_culling_edge_cases_parity(apd, case):
     r = run_assign(apd, wl, wl.w0, v=wl.v, want_centroids=True, cull=1)
     parity.check_assign(wl, wl.w0, r["labels"], r["vol"], r["dual"], v=wl.v, centroids_gpu=r["centroids"],
                         err_gpu=r["err"])
-    r0 = run_assign(apd, wl, wl.w0, v=wl.v, cull=0)
+    r0 = run_assign(apd, wl, wl.w0, v=wl.v, cull=0, kernel=KERNELS["rowpoly"])
     assert np.array_equal(r0["labels"], r["labels"])
 
 

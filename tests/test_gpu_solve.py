@@ -152,8 +152,8 @@ def test_culled_solve_is_the_same_solve(apd):
     """Culling is exact (same labels, same integer gradients), so apd_solve with and without it walks the identical
     trajectory: identical weights bit for bit; the recorded duals agree up to the order of the fp64 partial sums."""
     wl = workloads.make_config(4, n=(128, 96, 96), M=400)
-    a = run_solve(apd, wl, 0.02, cull=0, want_hist=True)
-    b = run_solve(apd, wl, 0.02, cull=1, want_hist=True)
+    a = run_solve(apd, wl, 0.02, cull=0, kernel=2, want_hist=True)      # ROWPOLY (AUTO brute force would take TENSOR)
+    b = run_solve(apd, wl, 0.02, cull=1, kernel=2, want_hist=True)
     assert (a[0].status, a[0].iters, a[0].evals) == (b[0].status, b[0].iters, b[0].evals)
     assert np.array_equal(a[2], b[2]) and np.array_equal(a[3], b[3]) and np.array_equal(a[4], b[4])
     np.testing.assert_allclose(a[5][0], b[5][0], rtol=1e-13, atol=0)
