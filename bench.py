@@ -246,10 +246,10 @@ def ncu_traffic_bytes(kernel: int):
 class Bench:
     """One workload resident on the device plus the buffers of the calls."""
 
-    def __init__(self, apd, torch, cfg: int, local: int):
+    def __init__(self, apd, torch, cfg: int, local: int, n=None, M=None):
         self.apd, self.torch, self.cfg = apd, torch, cfg
         self.dev = torch.device("cuda", local)
-        wl = self.wl = workloads.make_config(cfg)
+        wl = self.wl = workloads.make_config(cfg, n=n, M=M)
         self.ctx = apd.ApdContext(wl.dim, wl.M, device=local)
         self.grid = apd.make_grid(wl.dim, wl.n, wl.lo, wl.hi)
         dev = self.dev
@@ -391,6 +391,15 @@ def run_ours(args):
     peaks_t = (peak_fp32, peak_bf16, sm_count, sm_max_mhz)
     flush = torch.empty(FLUSH_BYTES, dtype=torch.uint8, device=dev)
 
+    if args.two_d:
+        if rank == 0:
+            b2 = Bench(apd, torch, 2, local, n=(2048, 2048), M=5000)
+            print(json.dumps(dict(workload="cfg2 recipe on 2048x2048 pixels x 5000 grains",
+                                  **kernel_record(b2, args.kernel, 0, flush, max(args.steps, 3), *peaks_t))), flush=True)
+            b2.close()
+        if world > 1:
+            dist.barrier(); dist.destroy_process_group()
+        return
     if args.config:
         # ---- the per-config record(s) of BASELINE.md section 4: one JSON line each, rank 0 only ----
         if rank == 0:
@@ -522,6 +531,12 @@ def run_ours(args):
         del b
         torch.cuda.empty_cache()
         if not args.no_per_config:
+            # a 2D workload large enough for ROWPOLY's long rows (cfg 2's recipe on 2048^2 pixels x 5000 grains)
+            b2 = Bench(apd, torch, 2, local, n=(2048, 2048), M=5000)
+            extra["assign_2d"] = dict(workload="cfg2 recipe on 2048x2048 pixels x 5000 grains",
+                                      **kernel_record(b2, K_AUTO, 0, flush, 5, *peaks_t))
+            b2.close()
+            del b2
             extra["per_config"] = {str(c): config_record(apd, torch, c, local, flush, args, peaks_t, full=False)
                                    for c in (1, 2, 3, 5)}
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -568,6 +583,7 @@ def main():
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 DIRECT, 2 ROWPOLY, 3 TENSOR")
     ap.add_argument("--config", default="", help="1..5 or all: print the full per-config record(s) instead of the headline line")
+    ap.add_argument("--two-d", action="store_true", help="only the 2D long-row leg (2048^2 x 5000); the ncu capture of the 2D kernel uses it")
     ap.add_argument("--oracle-full", action="store_true", help="--config: time one FULL oracle evaluation (cfg 1-4)")
     ap.add_argument("--no-solve", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")

@@ -66,10 +66,14 @@ __global__ void __launch_bounds__(FIN_THREADS) finalize_kernel(
     }
   }
   __syncthreads();
-  if (tid == 0) {
+  if (tid < 32) {        // ascending-order sum, 32 loads in flight per round (as in lbfgs_step_kernel: the same bits)
     double t = 0.0;
-    for (int L = 0; L < lm.n_layers; ++L) t += layer_buf[L];
-    s_smin = t;
+    for (int L0 = 0; L0 < lm.n_layers; L0 += 32) {
+      const double mine = (L0 + tid < lm.n_layers) ? layer_buf[L0 + tid] : 0.0;
+      const int cnt = min(32, lm.n_layers - L0);
+      for (int l = 0; l < cnt; ++l) t += __shfl_sync(0xffffffffu, mine, l);
+    }
+    if (tid == 0) s_smin = t;
   }
 
   const double vw_tot = block_sum_double<FIN_THREADS>(vw, scratch);

@@ -183,9 +183,9 @@ __device__ void gram_rows(const StepArgs& a, int cap, int hist_len, int hist_sta
   constexpr int NS = LB_GRAM_SLOTS, NACC = NNEW * 2 * NS + 1;
   for (int t0 = 0; t0 < hist_len; t0 += NS) {
     const int ns = min(NS, hist_len - t0);
-    int slot[NS];
+    size_t soff[NS];
 #pragma unroll
-    for (int q = 0; q < NS; ++q) slot[q] = (hist_start + t0 + (q < ns ? q : 0)) % cap;   // inactive: a duplicate, ignored
+    for (int q = 0; q < NS; ++q) soff[q] = (size_t)((hist_start + t0 + (q < ns ? q : 0)) % cap) * stride;   // inactive: a duplicate, ignored
     double acc[NACC];
 #pragma unroll
     for (int n = 0; n < NACC; ++n) acc[n] = 0.0;
@@ -195,25 +195,23 @@ __device__ void gram_rows(const StepArgs& a, int cap, int hist_len, int hist_sta
       for (int n = 0; n < NNEW; ++n) x[n] = nv[n][i];
 #pragma unroll
       for (int q = 0; q < NS; ++q) {
-        const double sv = S[(size_t)slot[q] * stride + i], yv = Y[(size_t)slot[q] * stride + i];
+        const double sv = S[soff[q] + i], yv = Y[soff[q] + i];
 #pragma unroll
         for (int n = 0; n < NNEW; ++n) { acc[(n * NS + q) * 2] += x[n] * sv; acc[(n * NS + q) * 2 + 1] += x[n] * yv; }
       }
       acc[NACC - 1] += x[NNEW - 1] * x[NNEW - 1];
     }
     cluster_all<NACC, false>(acc, r);
-    if (threadIdx.x == 0) {
-      for (int n = 0; n < NNEW; ++n) {
-        const int q = nidx[n];
-        for (int k = 0; k < ns; ++k) {
-          const int j = slot[k];
-          const double vs = acc[(n * NS + k) * 2], vy = acc[(n * NS + k) * 2 + 1];
-          gm[(size_t)q * ld + j] = vs; gm[(size_t)j * ld + q] = vs;
-          gm[(size_t)q * ld + cap + j] = vy; gm[(size_t)(cap + j) * ld + q] = vy;
-        }
-      }
-      if (t0 == 0) gm[(size_t)(2 * cap) * ld + 2 * cap] = acc[NACC - 1];
+    // the totals also sit in r.tot (shared memory): the write-back indexes THAT with its run-time slot count, so that
+    // acc[] is only ever indexed by constants and stays in registers
+    if ((int)threadIdx.x < NNEW * ns) {
+      const int n = (int)threadIdx.x / ns, k = (int)threadIdx.x % ns;
+      const int q = nidx[n], j = (hist_start + t0 + k) % cap;
+      const double vs = r.tot[(n * NS + k) * 2], vy = r.tot[(n * NS + k) * 2 + 1];
+      gm[(size_t)q * ld + j] = vs; gm[(size_t)j * ld + q] = vs;
+      gm[(size_t)q * ld + cap + j] = vy; gm[(size_t)(cap + j) * ld + q] = vy;
     }
+    if (threadIdx.x == 0 && t0 == 0) gm[(size_t)(2 * cap) * ld + 2 * cap] = r.tot[NACC - 1];
   }
   __syncthreads();          // thread 0's global writes are ordered before the CTA's reads in direction_vf
 }
@@ -378,10 +376,16 @@ __global__ void __cluster_dims__(LB_CLUSTER, 1, 1) __launch_bounds__(LB_THREADS)
   // ... then the layers in ascending order: the same bits in every CTA, and in a slab-sharded solve
   {
     const double* lsrc = a.layer_in ? a.layer_in : a.layer_buf;
-    if (tid == 0) {
+    if (tid < 32) {
+      // ascending-order sum with the loads in flight together: 32 layers per round, one per lane, then the lanes' values
+      // are added in lane order (a serial loop of dependent loads cost ~0.3 us per layer)
       double t = 0.0;
-      for (int L = 0; L < a.lm.n_layers; ++L) t += __ldcg(lsrc + L);
-      s_smin = t;
+      for (int L0 = 0; L0 < a.lm.n_layers; L0 += 32) {
+        const double mine = (L0 + tid < a.lm.n_layers) ? __ldcg(lsrc + L0 + tid) : 0.0;
+        const int cnt = min(32, a.lm.n_layers - L0);
+        for (int l = 0; l < cnt; ++l) t += __shfl_sync(0xffffffffu, mine, l);
+      }
+      if (tid == 0) s_smin = t;
     }
     __syncthreads();
   }
