@@ -414,7 +414,7 @@ template <> struct CullGeom<2> { static constexpr int V = 16, TXT = 2, TYT = CUL
 static_assert(CullGeom<3>::TXT * CullGeom<3>::V == CULL_TILE3_X && CullGeom<2>::TXT * CullGeom<2>::V == CULL_TILE2_X, "tile");
 
 template <int DIM>
-__global__ void __launch_bounds__(128, 4) assign_rowpoly_culled_kernel(const AssignArgs a) {
+__global__ void __launch_bounds__(128, 6) assign_rowpoly_culled_kernel(const AssignArgs a) {
   using G = CullGeom<DIM>;
   constexpr int V = G::V;
   constexpr int PREC = (DIM == 3) ? PREC3 : PREC2;
