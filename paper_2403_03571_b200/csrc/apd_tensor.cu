@@ -223,6 +223,62 @@ __device__ __forceinline__ void tc_build_seed(const TcSeedRegs& s, bool real, fl
   *reinterpret_cast<uint4*>(p + 384) = k3;
 }
 
+// Writes the Phi rows (A operand) of the CTA's 512 voxels for a tile whose reference voxel is (rx, ry, rz).
+__device__ __forceinline__ void tc_write_phi(unsigned char* s_A, int tid, int rx, int ry, int rz) {
+  // Phi row of this thread's voxel: monomials of the integer offsets, each under its three coefficient parts
+  const int ti = (tid & 15) - rx, tj = ((tid >> 4) & 7) - ry, tk = (tid >> 7) - rz;
+  const float mono[10] = {(float)(ti * ti), (float)(tj * tj), (float)(tk * tk), (float)(ti * tj), (float)(ti * tk),
+                          (float)(tj * tk), (float)ti, (float)tj, (float)tk, 1.0f};
+  unsigned short e[32];
+#pragma unroll
+  for (int m = 0; m < 6; ++m) {            // quadratic monomials: [hi mid lo] per monomial
+    const unsigned short h = __bfloat16_as_ushort(__float2bfloat16_rn(mono[m]));
+    e[3 * m] = h; e[3 * m + 1] = h; e[3 * m + 2] = h;
+  }
+#pragma unroll
+  for (int r = 0; r < 3; ++r)              // linear and constant: [i j k 1] under the hi, mid and lo parts
+#pragma unroll
+    for (int m = 0; m < 4; ++m) e[18 + 4 * r + m] = __bfloat16_as_ushort(__float2bfloat16_rn(mono[6 + m]));
+  e[30] = 0; e[31] = 0;
+  const int mt = tid >> 7, row = tid & 127;
+  unsigned char* p = s_A + mt * 8192 + (row >> 3) * 512 + (row & 7) * 16;
+#pragma unroll
+  for (int kc = 0; kc < 4; ++kc)
+    *reinterpret_cast<uint4*>(p + kc * 128) = make_uint4(pk(e[8 * kc], e[8 * kc + 1]), pk(e[8 * kc + 2], e[8 * kc + 3]),
+                                                         pk(e[8 * kc + 4], e[8 * kc + 5]), pk(e[8 * kc + 6], e[8 * kc + 7]));
+  fence_proxy_async_smem();
+}
+
+// The MMAs of chunk G (Theta stage U = G & 3) for the four M-tiles: the whole issuing warp walks this (uniform control
+// flow), one elected lane issues.  D fp32, A and B bf16, both K-major, N = 128, M = 128.
+template <int U>
+__device__ __forceinline__ void tc_issue_chunk(int G, uint32_t tmem, uint64_t ad0, uint64_t bd0, uint64_t* s_th_full,
+                                               uint64_t* s_th_empty, uint64_t* s_acc_full, uint64_t* s_acc_empty) {
+  constexpr uint32_t IDESC = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(TC_N >> 3) << 17) | ((128u >> 4) << 24);
+  mbar_wait(&s_th_full[U], (uint32_t)((G >> 2) & 1));
+#pragma unroll
+  for (int mt = 0; mt < 4; ++mt) {        // M-tile mt accumulates into its own region of 128 columns
+    if (G > 0) mbar_wait(&s_acc_empty[mt], (uint32_t)((G - 1) & 1));
+    tc_fence_after();
+    if (tc_elect_one()) {
+#pragma unroll
+      for (int ks = 0; ks < 2; ++ks)
+        tc_mma_bf16(tmem + (uint32_t)(mt * TC_N), ad0 + (uint64_t)((mt * 8192 + ks * 256) >> 4),
+                    bd0 + (uint64_t)((U * (int)TC_TH_BYTES + ks * 256) >> 4), IDESC, (uint32_t)ks);
+      if (mt == 3) tc_commit(&s_th_empty[U]);
+      tc_commit(&s_acc_full[mt]);
+    }
+    __syncwarp();
+  }
+}
+
+// PERSISTENT: one CTA per SM walks the tiles b = blockIdx.x, blockIdx.x + gridDim.x, ...  TMEM, the barriers and -- as
+// long as the tile's reference voxel keeps its place in the tile, i.e. for every tile not cut by the grid's boundary --
+// Phi are set up once; the TMA, builder and MMA warps simply keep streaming chunks across the tile boundary (the
+// mbarrier phases run on the CTA's global chunk count G), so the next tile's first accumulators are ready while the
+// epilogue warps still store the labels of the current one: no pipeline fill / drain per tile (it was ~3 of a tile's
+// 79 chunks at cfg 4, ~3 of 8 at cfg 3).  A tile whose reference voxel differs (ragged edge) drains the pipeline with
+// two CTA barriers and rewrites Phi.
 __global__ void __launch_bounds__(TC_THREADS, 1) assign_tensor_kernel(const AssignArgs a) {
   extern __shared__ __align__(128) unsigned char tc_smem[];
   unsigned char* s_A = tc_smem;                                    // Phi: 4 M-tiles x 128 rows x 32 bf16
@@ -232,21 +288,15 @@ __global__ void __launch_bounds__(TC_THREADS, 1) assign_tensor_kernel(const Assi
   __shared__ __align__(8) uint64_t s_th_full[TC_TH_STAGES], s_th_empty[TC_TH_STAGES];
   __shared__ __align__(8) uint64_t s_acc_full[4], s_acc_empty[4];      // one accumulator region per M-tile
   __shared__ uint32_t s_tmem;
-  __shared__ double s_red[TC_THREADS / 32];
+  __shared__ double s_red[2][TC_EPI_THREADS / 32];
 
   if (a.done_flag && *a.done_flag) return;
   const int tid = threadIdx.x, lane = tid & 31;
   // the warp index read through a shuffle is PROVABLY warp-uniform: the role branches below become uniform branches
   // and the barrier / TMEM addresses of each role live in uniform registers (measured: 11.58 -> 10.33 ms on cfg 4)
   const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
-  const int b = blockIdx.x;
-  const int bx = b % a.g.tiles_x, by = (b / a.g.tiles_x) % a.g.tiles_y, bz = b / (a.g.tiles_x * a.g.tiles_y);
+  const int n_tiles = a.g.tiles_x * a.g.tiles_y * a.g.tiles_z;
   const int nch = a.M_pad / TC_N;
-  // reference voxel of the tile: the middle of its part inside the grid (a tile cut by the boundary must not expand
-  // the costs about a point outside the domain: that would cost precision on narrow grids).  Offsets stay within
-  // [-8, 15]: squares and products <= 225, exact in bf16.
-  const int rx = min(TC_TX, a.g.nx - bx * TC_TX) / 2, ry = min(TC_TY, a.g.ny - by * TC_TY) / 2,
-            rz = min(TC_TZ, a.g.nz - bz * TC_TZ) / 2;
 
   if (tid == 0) {
     for (int s = 0; s < TC_RAW_STAGES; ++s) { mbar_init(&s_raw_full[s], 1); mbar_init(&s_raw_empty[s], TC_BUILD_WARPS); }
@@ -255,156 +305,157 @@ __global__ void __launch_bounds__(TC_THREADS, 1) assign_tensor_kernel(const Assi
     mbar_fence_init();
   }
   if (warp == 0) tc_alloc512(&s_tmem);
-  if (tid < TC_EPI_THREADS) {
-    // Phi row of this thread's voxel: monomials of the integer offsets, each under its three coefficient parts
-    const int ti = (tid & 15) - rx, tj = ((tid >> 4) & 7) - ry, tk = (tid >> 7) - rz;
-    const float mono[10] = {(float)(ti * ti), (float)(tj * tj), (float)(tk * tk), (float)(ti * tj), (float)(ti * tk),
-                            (float)(tj * tk), (float)ti, (float)tj, (float)tk, 1.0f};
-    unsigned short e[32];
-#pragma unroll
-    for (int m = 0; m < 6; ++m) {            // quadratic monomials: [hi mid lo] per monomial
-      const unsigned short h = __bfloat16_as_ushort(__float2bfloat16_rn(mono[m]));
-      e[3 * m] = h; e[3 * m + 1] = h; e[3 * m + 2] = h;
-    }
-#pragma unroll
-    for (int r = 0; r < 3; ++r)              // linear and constant: [i j k 1] under the hi, mid and lo parts
-#pragma unroll
-      for (int m = 0; m < 4; ++m) e[18 + 4 * r + m] = __bfloat16_as_ushort(__float2bfloat16_rn(mono[6 + m]));
-    e[30] = 0; e[31] = 0;
-    const int mt = tid >> 7, row = tid & 127;
-    unsigned char* p = s_A + mt * 8192 + (row >> 3) * 512 + (row & 7) * 16;
-#pragma unroll
-    for (int kc = 0; kc < 4; ++kc)
-      *reinterpret_cast<uint4*>(p + kc * 128) = make_uint4(pk(e[8 * kc], e[8 * kc + 1]), pk(e[8 * kc + 2], e[8 * kc + 3]),
-                                                           pk(e[8 * kc + 4], e[8 * kc + 5]), pk(e[8 * kc + 6], e[8 * kc + 7]));
-    fence_proxy_async_smem();
-  }
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = s_tmem;
 
-  float best = CUDART_INF_F;
-  int lab = 0;
+  // role constants
+  const uint64_t ad0 = tc_smem_desc(smem_u32(s_A), 128, 512), bd0 = tc_smem_desc(smem_u32(s_th), 128, 512);
+  const float sx = (float)a.g.s[0], sy = (float)a.g.s[1], sz = (float)a.g.s[2];
+  const int mt_e = (warp >> 2) & 3;
+  uint32_t lane_addr = tmem + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)(mt_e * TC_N);
+  uint32_t full = smem_u32(&s_acc_full[mt_e]), empty = smem_u32(&s_acc_empty[mt_e]);
+  asm volatile("" : "+r"(lane_addr), "+r"(full), "+r"(empty));     // keep them in registers (measured: without this 10.30 instead of 10.13 ms)
+
+  // every role walks the same tile sequence; TILE_BEGIN gives the tile's indices and, when its reference voxel differs
+  // from the previous tile's (uniform over the CTA), drains the pipeline with two CTA barriers and rewrites Phi
+#define TC_TILE_LOOP                                                                                                   \
+  int sig_cur = -1, G0 = 0;                                                                                            \
+  for (int b = blockIdx.x, it = 0; b < n_tiles; b += gridDim.x, ++it, G0 += nch)
+#define TC_TILE_BEGIN                                                                                                  \
+  const int bx = b % a.g.tiles_x, by = (b / a.g.tiles_x) % a.g.tiles_y, bz = b / (a.g.tiles_x * a.g.tiles_y);         \
+  const int rx = min(TC_TX, a.g.nx - bx * TC_TX) / 2, ry = min(TC_TY, a.g.ny - by * TC_TY) / 2,                       \
+            rz = min(TC_TZ, a.g.nz - bz * TC_TZ) / 2;                                                                  \
+  const int sig = rx | (ry << 8) | (rz << 16);                                                                         \
+  if (sig != sig_cur) {                                                                                                \
+    __syncthreads();                                                                                                   \
+    if (tid < TC_EPI_THREADS) tc_write_phi(s_A, tid, rx, ry, rz);                                                      \
+    tc_fence_before();                                                                                                 \
+    __syncthreads();                                                                                                   \
+    tc_fence_after();                                                                                                  \
+    sig_cur = sig;                                                                                                     \
+  }                                                                                                                    \
+  (void)bx; (void)by; (void)bz; (void)it;
 
   if (warp == 21) {
     // ===== TMA producer: one lane keeps the raw seed ring full =====
-    if (lane == 0) {
-      const unsigned char* src = reinterpret_cast<const unsigned char*>(a.qfix);
-      for (int p = 0; p < nch; ++p) {
-        const int rs = p % TC_RAW_STAGES;
-        if (p >= TC_RAW_STAGES) mbar_wait(&s_raw_empty[rs], (uint32_t)(((p / TC_RAW_STAGES) - 1) & 1));
-        mbar_arrive_expect_tx(&s_raw_full[rs], TC_RAW_BYTES);
-        tma_bulk_g2s(s_raw + rs * TC_RAW_BYTES, src + (size_t)p * TC_RAW_BYTES, TC_RAW_BYTES, &s_raw_full[rs]);
+    const unsigned char* src = reinterpret_cast<const unsigned char*>(a.qfix);
+    TC_TILE_LOOP {
+      TC_TILE_BEGIN
+      if (lane == 0) {
+        for (int c = 0; c < nch; ++c) {
+          const int G = G0 + c, rs = G % TC_RAW_STAGES;
+          if (G >= TC_RAW_STAGES) mbar_wait(&s_raw_empty[rs], (uint32_t)(((G / TC_RAW_STAGES) - 1) & 1));
+          mbar_arrive_expect_tx(&s_raw_full[rs], TC_RAW_BYTES);
+          tma_bulk_g2s(s_raw + rs * TC_RAW_BYTES, src + (size_t)c * TC_RAW_BYTES, TC_RAW_BYTES, &s_raw_full[rs]);
+        }
       }
+      __syncwarp();
     }
   } else if (warp == 20) {
-    // ===== MMA issuer: the whole warp walks the loop (uniform control flow, descriptors in uniform registers), one
-    //       elected lane issues.  Unrolled over the 4 Theta stages so that every descriptor is base + constant. =====
-    // instruction descriptor: D fp32, A and B bf16, both K-major, N = 128, M = 128
-    constexpr uint32_t IDESC = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(TC_N >> 3) << 17) | ((128u >> 4) << 24);
-    const uint64_t ad0 = tc_smem_desc(smem_u32(s_A), 128, 512), bd0 = tc_smem_desc(smem_u32(s_th), 128, 512);
-    static_assert(TC_TH_STAGES == 4, "the issue loop is unrolled over 4 Theta stages");
-    for (int c0 = 0; c0 < nch; c0 += 4) {
-#pragma unroll
-      for (int u = 0; u < 4; ++u) {
-        const int c = c0 + u;
-        if (c < nch) {
-          mbar_wait(&s_th_full[u], (uint32_t)((c0 >> 2) & 1));
-#pragma unroll
-          for (int mt = 0; mt < 4; ++mt) {      // M-tile mt accumulates into its own region of 128 columns
-            if (c > 0) mbar_wait(&s_acc_empty[mt], (uint32_t)((c - 1) & 1));
-            tc_fence_after();
-            if (tc_elect_one()) {
-#pragma unroll
-              for (int ks = 0; ks < 2; ++ks)
-                tc_mma_bf16(tmem + (uint32_t)(mt * TC_N), ad0 + (uint64_t)((mt * 8192 + ks * 256) >> 4),
-                            bd0 + (uint64_t)((u * (int)TC_TH_BYTES + ks * 256) >> 4), IDESC, (uint32_t)ks);
-              if (mt == 3) tc_commit(&s_th_empty[u]);
-              tc_commit(&s_acc_full[mt]);
-            }
-            __syncwarp();
-          }
+    // ===== MMA issuer =====
+    static_assert(TC_TH_STAGES == 4, "Theta stage = chunk count & 3");
+    TC_TILE_LOOP {
+      TC_TILE_BEGIN
+      for (int c = 0; c < nch; ++c) {
+        const int G = G0 + c;
+        switch (G & 3) {        // the Theta stage as a compile-time constant: every descriptor is base + constant
+          case 0: tc_issue_chunk<0>(G, tmem, ad0, bd0, s_th_full, s_th_empty, s_acc_full, s_acc_empty); break;
+          case 1: tc_issue_chunk<1>(G, tmem, ad0, bd0, s_th_full, s_th_empty, s_acc_full, s_acc_empty); break;
+          case 2: tc_issue_chunk<2>(G, tmem, ad0, bd0, s_th_full, s_th_empty, s_acc_full, s_acc_empty); break;
+          default: tc_issue_chunk<3>(G, tmem, ad0, bd0, s_th_full, s_th_empty, s_acc_full, s_acc_empty); break;
         }
       }
     }
   } else if (warp >= 16) {
     // ===== Theta builders: one seed of the chunk per thread =====
     const int sid = tid - TC_EPI_THREADS;
-    // reference voxel of the tile and the voxel sides
-    const float y0x = (float)(a.g.lo[0] + ((double)(bx * TC_TX + rx) + 0.5) * a.g.s[0]);
-    const float y0y = (float)(a.g.lo[1] + ((double)(by * TC_TY + ry + a.g.off_y) + 0.5) * a.g.s[1]);
-    const float y0z = (float)(a.g.lo[2] + ((double)(bz * TC_TZ + rz + a.g.off_z) + 0.5) * a.g.s[2]);
-    const float sx = (float)a.g.s[0], sy = (float)a.g.s[1], sz = (float)a.g.s[2];
-    for (int c = 0; c < nch; ++c) {
-      const int rs = c % TC_RAW_STAGES, ts = c % TC_TH_STAGES;
-      mbar_wait(&s_raw_full[rs], (uint32_t)((c / TC_RAW_STAGES) & 1));
-      const uint4* rp = reinterpret_cast<const uint4*>(s_raw + rs * TC_RAW_BYTES) + sid * 6;
-      TcSeedRegs sr;
-      const uint4 u0 = rp[0], u1 = rp[1], u2 = rp[2];
-      sr.p0 = make_float4(__uint_as_float(u0.x), __uint_as_float(u0.y), __uint_as_float(u0.z), __uint_as_float(u0.w));
-      sr.p1 = make_float4(__uint_as_float(u1.x), __uint_as_float(u1.y), __uint_as_float(u1.z), __uint_as_float(u1.w));
-      sr.p2 = make_float4(__uint_as_float(u2.x), __uint_as_float(u2.y), __uint_as_float(u2.z), __uint_as_float(u2.w));
-      sr.q0 = rp[3]; sr.q1 = rp[4]; sr.q2 = rp[5];
-      if (c >= TC_TH_STAGES) mbar_wait(&s_th_empty[ts], (uint32_t)(((c / TC_TH_STAGES) - 1) & 1));
-      tc_build_seed(sr, c * TC_N + sid < a.M, y0x, y0y, y0z, sx, sy, sz, s_th + ts * TC_TH_BYTES, sid);
-      fence_proxy_async_smem();
-      __syncwarp();
-      if (lane == 0) { mbar_arrive(&s_th_full[ts]); mbar_arrive(&s_raw_empty[rs]); }
+    TC_TILE_LOOP {
+      TC_TILE_BEGIN
+      // reference voxel of the tile
+      const float y0x = (float)(a.g.lo[0] + ((double)(bx * TC_TX + rx) + 0.5) * a.g.s[0]);
+      const float y0y = (float)(a.g.lo[1] + ((double)(by * TC_TY + ry + a.g.off_y) + 0.5) * a.g.s[1]);
+      const float y0z = (float)(a.g.lo[2] + ((double)(bz * TC_TZ + rz + a.g.off_z) + 0.5) * a.g.s[2]);
+      for (int c = 0; c < nch; ++c) {
+        const int G = G0 + c, rs = G % TC_RAW_STAGES, ts = G % TC_TH_STAGES;
+        mbar_wait(&s_raw_full[rs], (uint32_t)((G / TC_RAW_STAGES) & 1));
+        const uint4* rp = reinterpret_cast<const uint4*>(s_raw + rs * TC_RAW_BYTES) + sid * 6;
+        TcSeedRegs sr;
+        const uint4 u0 = rp[0], u1 = rp[1], u2 = rp[2];
+        sr.p0 = make_float4(__uint_as_float(u0.x), __uint_as_float(u0.y), __uint_as_float(u0.z), __uint_as_float(u0.w));
+        sr.p1 = make_float4(__uint_as_float(u1.x), __uint_as_float(u1.y), __uint_as_float(u1.z), __uint_as_float(u1.w));
+        sr.p2 = make_float4(__uint_as_float(u2.x), __uint_as_float(u2.y), __uint_as_float(u2.z), __uint_as_float(u2.w));
+        sr.q0 = rp[3]; sr.q1 = rp[4]; sr.q2 = rp[5];
+        if (G >= TC_TH_STAGES) mbar_wait(&s_th_empty[ts], (uint32_t)(((G / TC_TH_STAGES) - 1) & 1));
+        tc_build_seed(sr, c * TC_N + sid < a.M, y0x, y0y, y0z, sx, sy, sz, s_th + ts * TC_TH_BYTES, sid);
+        fence_proxy_async_smem();
+        __syncwarp();
+        if (lane == 0) { mbar_arrive(&s_th_full[ts]); mbar_arrive(&s_raw_empty[rs]); }
+      }
     }
   } else {
-    // ===== epilogue: warps 0-15, thread <-> voxel <-> TMEM lane; M-tile mt = warp / 4 drains its own region of 128
-    //       columns in 4 groups of 32 seeds, software-pipelined (the tcgen05.ld of the next group is in flight while
-    //       the minima of the current one are taken); the region is released as soon as it is in registers. =====
-    const int mt = warp >> 2;
-    uint32_t lane_addr = tmem + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)(mt * TC_N);
-    uint32_t full = smem_u32(&s_acc_full[mt]), empty = smem_u32(&s_acc_empty[mt]);
-    asm volatile("" : "+r"(lane_addr), "+r"(full), "+r"(empty));     // keep them in registers (no re-derivation per chunk)
-    float ra[32], rb[32];
-    for (int c = 0; c < nch; ++c) {
-      mbar_wait_a(full, (uint32_t)(c & 1));
-      tc_fence_after();
-      TC_LD32(lane_addr, ra);
-      tc_wait_ld();
-      TC_LD32(lane_addr + 32, rb);
-      tc_take_half(ra, c * TC_N, best, lab);
-      tc_wait_ld();
-      TC_LD32(lane_addr + 64, ra);
-      tc_take_half(rb, c * TC_N + 32, best, lab);
-      tc_wait_ld();
-      TC_LD32(lane_addr + 96, rb);
-      tc_take_half(ra, c * TC_N + 64, best, lab);
-      tc_wait_ld();
-      tc_fence_before();
-      __syncwarp();
-      if (tc_elect_one()) mbar_arrive_a(empty);                       // the region is in registers: release it
-      tc_take_half(rb, c * TC_N + 96, best, lab);
-    }
-  }
+    // ===== epilogue: warps 0-15 =====
+    TC_TILE_LOOP {
+      TC_TILE_BEGIN
+      float best = CUDART_INF_F;
+      int lab = 0;
+      float ra[32], rb[32];
+      for (int c = 0; c < nch; ++c) {
+        mbar_wait_a(full, (uint32_t)((G0 + c) & 1));
+        tc_fence_after();
+        TC_LD32(lane_addr, ra);
+        tc_wait_ld();
+        TC_LD32(lane_addr + 32, rb);
+        tc_take_half(ra, c * TC_N, best, lab);
+        tc_wait_ld();
+        TC_LD32(lane_addr + 64, ra);
+        tc_take_half(rb, c * TC_N + 32, best, lab);
+        tc_wait_ld();
+        TC_LD32(lane_addr + 96, rb);
+        tc_take_half(ra, c * TC_N + 64, best, lab);
+        tc_wait_ld();
+        tc_fence_before();
+        __syncwarp();
+        if (tc_elect_one()) mbar_arrive_a(empty);                       // the region is in registers: release it
+        tc_take_half(rb, c * TC_N + 96, best, lab);
+      }
 
-  // a5 + a6: label store, warp-aggregated counts, index sums, fp64 sum of the minima
-  double dsum = 0.0;
-  if (tid < TC_EPI_THREADS) {
-    const int ix = bx * TC_TX + (tid & 15), iy = by * TC_TY + ((tid >> 4) & 7), iz = bz * TC_TZ + (tid >> 7);
-    const bool valid = ix < a.g.nx && iy < a.g.ny && iz < a.g.nz;
-    const unsigned vmask = __ballot_sync(0xffffffffu, valid);
-    // a voxel whose real costs are all NaN / +inf / >= 2^100 would keep a padding seed (cost 2^100) as its minimum:
-    // it takes label 0 like the other kernels, and never indexes count[] beyond M
-    if (lab >= a.M) lab = 0;
-    if (valid) {
-      if (a.labels) a.labels[((long long)iz * a.g.ny + iy) * a.g.nx + ix] = lab;
-      dsum = (double)best;
-      const unsigned peers = __match_any_sync(vmask, lab);
-      if (lane == __ffs(peers) - 1) atomicAdd(a.count + lab, (unsigned int)__popc(peers));
-      if (a.idxsum) {
-        atomicAdd(a.idxsum + (size_t)lab * 3 + 0, (unsigned long long)ix);
-        atomicAdd(a.idxsum + (size_t)lab * 3 + 1, (unsigned long long)(iy + a.g.off_y));
-        atomicAdd(a.idxsum + (size_t)lab * 3 + 2, (unsigned long long)(iz + a.g.off_z));
+      // a5 + a6: label store, warp-aggregated counts, index sums, fp64 sum of the minima
+      double dsum = 0.0;
+      const int ix = bx * TC_TX + (tid & 15), iy = by * TC_TY + ((tid >> 4) & 7), iz = bz * TC_TZ + (tid >> 7);
+      const bool valid = ix < a.g.nx && iy < a.g.ny && iz < a.g.nz;
+      const unsigned vmask = __ballot_sync(0xffffffffu, valid);
+      // a voxel whose real costs are all NaN / +inf / >= 2^100 would keep a padding seed (cost 2^100) as its minimum:
+      // it takes label 0 like the other kernels, and never indexes count[] beyond M
+      if (lab >= a.M) lab = 0;
+      if (valid) {
+        if (a.labels) a.labels[((long long)iz * a.g.ny + iy) * a.g.nx + ix] = lab;
+        dsum = (double)best;
+        const unsigned peers = __match_any_sync(vmask, lab);
+        if (lane == __ffs(peers) - 1) atomicAdd(a.count + lab, (unsigned int)__popc(peers));
+        if (a.idxsum) {
+          atomicAdd(a.idxsum + (size_t)lab * 3 + 0, (unsigned long long)ix);
+          atomicAdd(a.idxsum + (size_t)lab * 3 + 1, (unsigned long long)(iy + a.g.off_y));
+          atomicAdd(a.idxsum + (size_t)lab * 3 + 2, (unsigned long long)(iz + a.g.off_z));
+        }
+      }
+      // the tile's sum of minima: lanes by shuffle tree, the 16 epilogue warps in order (a named barrier of the 512
+      // epilogue threads only: the producer warps are already streaming the next tile); s_red is double-buffered
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) dsum += __shfl_down_sync(0xffffffffu, dsum, o);
+      if (lane == 0) s_red[it & 1][warp] = dsum;
+      asm volatile("bar.sync 1, %0;" ::"n"(TC_EPI_THREADS) : "memory");
+      if (tid == 0) {
+        double tot = 0.0;
+#pragma unroll
+        for (int i = 0; i < TC_EPI_THREADS / 32; ++i) tot += s_red[it & 1][i];
+        a.dual_partial[b] = tot;
       }
     }
   }
-  const double tot = block_sum_double<TC_THREADS>(dsum, s_red);
-  if (tid == 0) a.dual_partial[b] = tot;
+#undef TC_TILE_LOOP
+#undef TC_TILE_BEGIN
   tc_fence_before();
   __syncthreads();
   if (warp == 0) tc_free512(tmem);
@@ -423,11 +474,14 @@ cudaError_t launch_pack_qfix(const GridDev& g, int M_pad, const float* rec, uint
 
 cudaError_t launch_assign_tensor(const AssignArgs& a, cudaStream_t st) {
   // per device and cheap: set on every launch (a process may drive several devices through several contexts)
-  cudaError_t e = cudaSuccess;
-  const int n_tiles = a.g.tiles_x * a.g.tiles_y * a.g.tiles_z;
-  e = cudaFuncSetAttribute(assign_tensor_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM);
+  cudaError_t e = cudaFuncSetAttribute(assign_tensor_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM);
   if (e != cudaSuccess) return e;
-  assign_tensor_kernel<<<n_tiles, TC_THREADS, TC_SMEM, st>>>(a);
+  int dev = 0, sms = 0;
+  if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
+  if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
+  const int n_tiles = a.g.tiles_x * a.g.tiles_y * a.g.tiles_z;
+  const int n_ctas = n_tiles < sms ? n_tiles : sms;                 // persistent: one CTA per SM (112 KB smem, all of TMEM)
+  assign_tensor_kernel<<<n_ctas, TC_THREADS, TC_SMEM, st>>>(a);
   return cudaGetLastError();
 }
 
