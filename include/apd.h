@@ -48,13 +48,12 @@ typedef struct {
 /* Which implementation of the voxel x seed reduction runs (all give labels by the same rule:
  * fp32 cost, lowest seed index among equal fp32 costs). */
 enum {
-  APD_KERNEL_AUTO   = 0,   /* the fastest one for the call.  Brute force in 3D: APD_KERNEL_TENSOR when M >= 1536, or
-                              when M >= 384 on a grid too small for ROWPOLY's long rows (below ~3.6 M voxels);
-                              otherwise, in 2D and with opts.cull: APD_KERNEL_ROWPOLY.  Grids with n[0] < 8 (3D also
-                              n[1] < 8 or n[2] < 4) take APD_KERNEL_DIRECT (and ignore opts.cull): the row kernels
-                              expand the cost about the midpoint of a row / tile, which there lies up to 8/n domain
-                              widths L outside the domain: a cost then carries a few fp32 ulp of a ((1 + 8/n) L)^2
-                              instead of a few ulp of itself                                        */
+  APD_KERNEL_AUTO   = 0,   /* the fastest one for the call: brute force in 3D APD_KERNEL_TENSOR; in 2D and with
+                              opts.cull APD_KERNEL_ROWPOLY.  Grids with n[0] < 8 (3D also n[1] < 8 or n[2] < 4) take
+                              APD_KERNEL_DIRECT (and ignore opts.cull): the row kernels expand the cost about the
+                              midpoint of a row / tile, which there lies up to 8/n domain widths L outside the
+                              domain: a cost then carries a few fp32 ulp of a ((1 + 8/n) L)^2 instead of a few ulp
+                              of itself                                                             */
   APD_KERNEL_DIRECT = 1,   /* un-hoisted direct form: 12 (3D) / 7 (2D) FP32 instr. per pair;
                               the reference kernel the FP32-pipe fraction is quoted on             */
   APD_KERNEL_ROWPOLY = 2,  /* quadratic in the offset from the row's midpoint (1.5 FMA per pair) with

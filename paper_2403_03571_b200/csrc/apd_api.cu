@@ -156,7 +156,7 @@ static bool narrow_grid(const apd_grid* grid) {
   if (grid->n[0] < 8) return true;
   return grid->dim == 3 && (grid->n[1] < 8 || grid->n[2] < 4);
 }
-int resolve_kernel(const apd_ctx* ctx, const apd_opts* o, const apd_grid* grid, int M, bool* cull, std::string* err) {
+int resolve_kernel(const apd_ctx* /*ctx*/, const apd_opts* o, const apd_grid* grid, int /*M*/, bool* cull, std::string* err) {
   int k = o ? o->kernel : APD_KERNEL_AUTO;
   if (k != APD_KERNEL_AUTO && k != APD_KERNEL_DIRECT && k != APD_KERNEL_ROWPOLY && k != APD_KERNEL_TENSOR) { *err = "unknown opts.kernel"; return -1; }
   if (k == APD_KERNEL_TENSOR && grid && grid->dim != 3) { *err = "APD_KERNEL_TENSOR is 3D only"; return -1; }
@@ -166,14 +166,9 @@ int resolve_kernel(const apd_ctx* ctx, const apd_opts* o, const apd_grid* grid, 
   if (k == APD_KERNEL_AUTO) {
     if (narrow_grid(grid)) { *cull = false; return APD_KERNEL_DIRECT; }
     k = APD_KERNEL_ROWPOLY;
-    // brute force in 3D: the tensor-core kernel once there are enough seeds to amortise its per-tile set-up (Phi, TMEM,
-    // pipeline fill: ~3 chunks of 128 seeds).  Measured on B200: TENSOR / ROWPOLY time 0.63-0.75 at
-    // M >= 2000, 0.92 (128^3) and 1.10 (256^3, where ROWPOLY runs its long rows) at M = 1000, 1.09-1.2 at M <= 256.
-    if (grid && grid->dim == 3 && !*cull && ctx) {
-      int tx, ty, tz;
-      const bool long_rows = rowpoly_tile_counts(3, grid->n[0], grid->n[1], grid->n[2], ctx->ws.sm_count, false, &tx, &ty, &tz) != 0;
-      if (M >= 1536 || (!long_rows && M >= 384)) k = APD_KERNEL_TENSOR;
-    }
+    // brute force in 3D: the tensor-core kernel.  Measured on B200 with the persistent kernel: TENSOR /
+    // ROWPOLY time 0.22-0.88 on every grid and seed count tried (32^3 .. 256^3 voxels, M = 64 .. 10^4).
+    if (grid && grid->dim == 3 && !*cull) k = APD_KERNEL_TENSOR;
   }
   if (*cull && k != APD_KERNEL_ROWPOLY) { *err = "opts.cull needs kernel AUTO or ROWPOLY"; return -1; }
   return k;

@@ -219,12 +219,12 @@ def test_P14_closed_form_weights(apd):
 def test_warm_start_and_not_converged(apd):
     wl = workloads.make_config(3, n=(48, 48, 48), M=60)
     orc = oracle_solve(parity.grid_of(wl), wl.X, wl.A, wl.v, 0.01, max_iters=3)
-    info, w32, w64, labels, vol = run_solve(apd, wl, 0.01, max_iters=3)
+    info, w32, w64, labels, vol = run_solve(apd, wl, 0.01, max_iters=3, kernel=2)
     assert orc.status == NOT_CONVERGED and info.status == 1
     check_against_oracle(wl, 0.01, info, w32, w64, labels, vol, orc)
     # warm start from the returned fp32 weights (Alg. 3 warm start W0^{k+1} = W^k)
     orc2 = oracle_solve(parity.grid_of(wl), wl.X, wl.A, wl.v, 0.01, w_init=w32)
-    info2, w32b, w64b, labels2, vol2 = run_solve(apd, wl, 0.01, w_init=w32)
+    info2, w32b, w64b, labels2, vol2 = run_solve(apd, wl, 0.01, w_init=w32, kernel=2)
     assert info2.status == 0 and orc2.status == OK
     check_against_oracle(wl, 0.01, info2, w32b, w64b, labels2, vol2, orc2)
 
