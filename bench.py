@@ -301,6 +301,23 @@ class Bench:
             out["cull_rebuilds"] = self.ctx.solve_stats()[1]
         return out
 
+    def solve_continuation(self, levels: int, max_iters: int, reps: int):
+        """apd_solve_continuation (coarse-to-fine; an extension, NOT the headline Algorithm 2 number), culling on."""
+        torch, apd, wl = self.torch, self.apd, self.wl
+        secs, out = [], None
+        for _ in range(reps):
+            wS = torch.zeros(wl.M, dtype=torch.float32, device=self.dev)
+            torch.cuda.synchronize()
+            ts = time.perf_counter()
+            rc, its, evs, err = self.ctx.apd_solve_continuation(self.grid, levels, self.X, self.A, self.v, wl.eps, w=wS,
+                                                                labels=self.labels, vol=self.vol,
+                                                                opts=apd.make_opts(cull=1, max_iters=max_iters))
+            torch.cuda.synchronize()
+            secs.append(time.perf_counter() - ts)
+            out = {"seconds": secs[-1], "first_call_seconds": secs[0], "levels": levels, "status": rc,
+                   "evals_per_level_coarsest_first": evs, "iters_per_level": its, "max_rel_err": err, "tol": wl.eps}
+        return out
+
     def close(self):
         self.ctx.close()
 
@@ -346,6 +363,8 @@ def config_record(apd, torch, cfg: int, local: int, flush, args, peaks_t, full: 
     out["assign_culled"] = kernel_record(b, K_AUTO, 1, flush, reps, *peaks_t)
     if not args.no_solve:
         out["solve_culled"] = b.solve(1, K_AUTO, args.solve_max_iters, 2)
+        if cfg >= 2:
+            out["solve_continuation"] = b.solve_continuation(2, args.solve_max_iters, 2)
         if full and cfg <= 4:
             out["solve_brute_force"] = b.solve(0, K_AUTO, args.solve_max_iters, 1)
     if full:
@@ -522,6 +541,9 @@ def run_ours(args):
             extra["culled_assign"] = kernel_record(b, K_AUTO, 1, flush, 5, *peaks_t)
             extra["solve"] = dict(workload=f"cfg{WORKLOAD_CFG} apd_solve, opts.cull=1",
                                   **b.solve(1, K_AUTO, args.solve_max_iters, 2))
+            extra["solve_continuation"] = dict(workload=f"cfg{WORKLOAD_CFG} apd_solve_continuation, 2 coarser levels, "
+                                                        "opts.cull=1 (extension: not Algorithm 2's number)",
+                                               **b.solve_continuation(2, args.solve_max_iters, 2))
             extra["solve_brute_force"] = dict(workload=f"cfg{WORKLOAD_CFG} apd_solve, brute force",
                                               **b.solve(0, args.kernel, args.solve_max_iters, 1))
         cb = None

@@ -213,6 +213,18 @@ int apd_solve_refine(apd_ctx* ctx, apd_grid* grid, int32_t M, const float* X, co
                      double* vol, int32_t* refinements, int32_t* iters, int32_t* evals, double* max_rel_err,
                      const apd_opts* opts, void* cuda_stream);
 
+/* Coarse-to-fine continuation (an extension of Alg. 2 step 4, PAPER.md:157 -- not in the paper): the
+ * weights do not depend on the resolution, so Algorithm 2 is run on `grid` coarsened by 2^levels, ..., 2, 1 per axis
+ * (n_k -> ceil(n_k / 2^l); a level with some n_k < 16 is skipped), each level started from the weights of the one
+ * before (a level that ends APD_NOT_CONVERGED hands on its best iterate).  The last level is apd_solve on `grid` itself:
+ * same post-condition, w, labels, vol; the return value is its status.  levels = 0 is apd_solve.
+ *   iters, evals   HOST out [levels + 1], coarsest level first (0 for a skipped level); each may be NULL
+ *   max_rel_err    HOST out, of the last level.   Everything else as apd_solve.  Blocks until finished. */
+int apd_solve_continuation(apd_ctx* ctx, const apd_grid* grid, int32_t levels, int32_t M, const float* X, const float* A,
+                           const float* target_vol, double tol, const float* w_init, float* w, int32_t* labels,
+                           double* vol, int32_t* iters, int32_t* evals, double* max_rel_err, const apd_opts* opts,
+                           void* cuda_stream);
+
 /* Resolution rules of PAPER.md:182-197 for a cubic grid of M voxels per axis on a domain of volume |Omega|:
  * |Omega| / M^D < factor * v_min with factor = eps (necessary: one misassigned voxel is already the tolerance; eq. 2.9
  * when v_min = |Omega|/N) or eps / 2^D (practical, eq. 2.10).  apd_resolution_bound returns the real number M must

@@ -102,6 +102,11 @@ def load_library() -> ctypes.CDLL:
     lib.apd_solve_refine.argtypes = ([_P, ctypes.POINTER(apd_grid), ctypes.c_int32, _P, _P, _P, ctypes.c_double, ctypes.c_int32]
                                      + [_P] * 3 + [ctypes.POINTER(ctypes.c_int32)] * 3
                                      + [ctypes.POINTER(ctypes.c_double), ctypes.POINTER(apd_opts), _P])
+    lib.apd_solve_continuation.restype = ctypes.c_int
+    lib.apd_solve_continuation.argtypes = ([_P, ctypes.POINTER(apd_grid), ctypes.c_int32, ctypes.c_int32, _P, _P, _P,
+                                            ctypes.c_double] + [_P] * 4
+                                           + [ctypes.POINTER(ctypes.c_int32), ctypes.POINTER(ctypes.c_int32),
+                                              ctypes.POINTER(ctypes.c_double), ctypes.POINTER(apd_opts), _P])
     lib.apd_resolution_bound.restype = ctypes.c_double
     lib.apd_resolution_bound.argtypes = [ctypes.c_int32, ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_int32]
     lib.apd_choose_resolution.restype = ctypes.c_int32
@@ -135,7 +140,7 @@ def load_library() -> ctypes.CDLL:
 EXPORTED_SYMBOLS = ["apd_default_opts", "apd_create", "apd_destroy", "apd_last_error", "apd_assign", "apd_solve",
                     "apd_assign_host", "apd_solve_host", "apd_solve_history", "apd_assign_points", "apd_solve_points", "apd_solve_stats", "apd_lloyd", "apd_solve_refine", "apd_resolution_bound",
                     "apd_choose_resolution", "apd_reserve", "apd_assign_stats", "apd_slab_align", "apd_counter_words",
-                    "apd_assign_slab", "apd_finalize_counters", "apd_solve_slab"]
+                    "apd_assign_slab", "apd_finalize_counters", "apd_solve_slab", "apd_solve_continuation"]
 
 
 def make_grid(dim: int, n: Sequence[int], lo: Sequence[float], hi: Sequence[float]) -> apd_grid:
@@ -426,6 +431,24 @@ class ApdContext:
             ctypes.byref(opts) if opts is not None else None, self._stream())
         self._check(rc, allow=(APD_OK, APD_NOT_CONVERGED))
         return SolveInfo(rc, it.value, ev.value, err.value, float("nan")), rf.value
+
+    def apd_solve_continuation(self, grid: apd_grid, levels: int, X, A, target_vol, tol: float, w_init=None, w=None,
+                               labels=None, vol=None, opts: Optional[apd_opts] = None):
+        """apd_solve_continuation of include/apd.h.  Returns (status, iters per level, evals per level, max_rel_err),
+        coarsest level first."""
+        d = grid.dim
+        M = X.shape[0]
+        it = (ctypes.c_int32 * (levels + 1))()
+        ev = (ctypes.c_int32 * (levels + 1))()
+        err = ctypes.c_double(0.0)
+        rc = self._lib.apd_solve_continuation(
+            self._h, ctypes.byref(grid), int(levels), M, _dev(X, torch.float32, "X", M * d),
+            _dev(A, torch.float32, "A", M * d * d), _dev(target_vol, torch.float32, "target_vol", M), float(tol),
+            _dev(w_init, torch.float32, "w_init", M), _dev(w, torch.float32, "w", M), _dev(labels, torch.int32, "labels"),
+            _dev(vol, torch.float64, "vol", M), it, ev, ctypes.byref(err),
+            ctypes.byref(opts) if opts is not None else None, self._stream())
+        self._check(rc, allow=(APD_OK, APD_NOT_CONVERGED))
+        return rc, list(it), list(ev), err.value
 
     def solve_stats(self):
         """(evaluations recorded, candidate-list rebuilds) of the most recent apd_solve."""

@@ -117,3 +117,39 @@ extern "C" int apd_solve_refine(apd_ctx* ctx, apd_grid* grid, int32_t M, const f
   if (max_rel_err) *max_rel_err = err;
   return rc;
 }
+
+// Coarse-to-fine continuation ("natural extension" of Alg. 2 step 4): the weights do
+// not depend on the resolution, so Algorithm 2 is run on the grid coarsened by 2^levels, ..., 2, 1 per axis, each level
+// started from the weights of the one before; only the last level runs on `grid` itself, and it starts almost converged.
+extern "C" int apd_solve_continuation(apd_ctx* ctx, const apd_grid* grid, int32_t levels, int32_t M, const float* X,
+                                      const float* A, const float* target_vol, double tol, const float* w_init, float* w,
+                                      int32_t* labels, double* vol, int32_t* iters, int32_t* evals, double* max_rel_err,
+                                      const apd_opts* opts, void* cuda_stream) {
+  if (!ctx) return APD_E_ARG;
+  ctx->err.clear();
+  if (!grid || !w || levels < 0 || levels > 8) { ctx->err = "apd_solve_continuation: grid, w required, 0 <= levels <= 8"; return APD_E_ARG; }
+  if (grid->dim != 2 && grid->dim != 3) { ctx->err = "apd_solve_continuation: grid.dim must be 2 or 3"; return APD_E_ARG; }
+  int rc = APD_OK;
+  double err = 0.0;
+  bool started = false;
+  for (int l = levels; l >= 0; --l) {
+    apd_grid g = *grid;
+    bool too_coarse = false;
+    for (int k = 0; k < grid->dim; ++k) {
+      g.n[k] = (grid->n[k] + (1 << l) - 1) >> l;
+      if (l > 0 && g.n[k] < 16) too_coarse = true;          // a level this coarse says nothing about the cells
+    }
+    int it = 0, ev = 0;
+    if (!too_coarse) {
+      const bool last = (l == 0);
+      rc = apd_solve(ctx, &g, M, X, A, target_vol, tol, started ? w : w_init, w, last ? labels : nullptr,
+                     last ? vol : nullptr, nullptr, &it, &ev, &err, nullptr, opts, cuda_stream);
+      if (rc < 0) return rc;
+      started = true;
+    }
+    if (iters) iters[levels - l] = it;
+    if (evals) evals[levels - l] = ev;
+  }
+  if (max_rel_err) *max_rel_err = err;
+  return rc;
+}

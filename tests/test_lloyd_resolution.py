@@ -174,3 +174,56 @@ def test_gpu_refine_and_restart(apd):
     # the work is comparable
     assert abs(info.evals - ev_or) <= max(10, ev_or // 2)
     print(f"refinements {r}, final grid {grid.n[0]}x{grid.n[1]}, gpu evals {info.evals} vs oracle {ev_or}")
+
+
+# ---------------------------------------------------------------- coarse-to-fine continuation (f2 extension)
+def test_oracle_continuation_levels0_is_solve_and_postcondition():
+    from oracle.apd_oracle import oracle_solve_continuation
+    wl = workloads.make_config(2, n=(128, 128), M=30)
+    g = Grid(wl.dim, wl.n, wl.lo, wl.hi)
+    plain = oracle_solve(g, wl.X, wl.A, wl.v, 0.01)
+    r0, it0, ev0 = oracle_solve_continuation(g, wl.X, wl.A, wl.v, 0.01, 0)
+    assert (r0.status, r0.iters, r0.evals) == (plain.status, plain.iters, plain.evals) and np.array_equal(r0.w, plain.w)
+    assert it0 == [plain.iters] and ev0 == [plain.evals]
+    r2, it2, ev2 = oracle_solve_continuation(g, wl.X, wl.A, wl.v, 0.01, 2)
+    assert r2.status == OK and len(ev2) == 3
+    chk = oracle_assign(g, wl.X, wl.A, r2.w32, v=wl.v)
+    assert chk.err <= 0.01                                    # the last level is Algorithm 2 on the grid itself (P15)
+    assert ev2[-1] < plain.evals                              # it starts almost converged
+    # a level coarser than 16 voxels per axis is skipped
+    r5, it5, ev5 = oracle_solve_continuation(g, wl.X, wl.A, wl.v, 0.01, 5)
+    assert ev5[0] == 0 and ev5[1] == 0 and ev5[-1] > 0
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("cfg,n,M,eps,cull,levels", [(2, (256, 256), 60, 0.01, 1, 2), (3, (96, 96, 96), 120, 0.02, 1, 2),
+                                                     (4, (128, 128, 128), 300, 0.02, 0, 1)])
+def test_gpu_continuation_parity(apd, cfg, n, M, eps, cull, levels):
+    """apd_solve_continuation against oracle_solve_continuation: same level structure, the oracle's evaluation at the
+    GPU's weights meets the tolerance, labels agree up to near-ties, per-level evaluation counts close (identical when
+    no voxel flips: parity rule 5), and the fine level needs fewer evaluations than plain apd_solve."""
+    from oracle.apd_oracle import oracle_solve_continuation
+    import torch
+    import apd_parity as parity
+    wl = workloads.make_config(cfg, n=n, M=M)
+    grid_o = Grid(wl.dim, wl.n, wl.lo, wl.hi)
+    ro, it_o, ev_o = oracle_solve_continuation(grid_o, wl.X, wl.A, wl.v, eps, levels)
+    dev = torch.device("cuda:0")
+    ctx = apd.ApdContext(wl.dim, wl.M)
+    grid = apd.make_grid(wl.dim, wl.n, wl.lo, wl.hi)
+    X = torch.from_numpy(wl.X).to(dev); A = torch.from_numpy(wl.A).to(dev); v = torch.from_numpy(wl.v).to(dev)
+    w = torch.zeros(wl.M, dtype=torch.float32, device=dev); labels = torch.empty(wl.N, dtype=torch.int32, device=dev)
+    vol = torch.zeros(wl.M, dtype=torch.float64, device=dev)
+    rc, it_g, ev_g, err = ctx.apd_solve_continuation(grid, levels, X, A, v, eps, w=w, labels=labels, vol=vol,
+                                                     opts=apd.make_opts(cull=cull))
+    plain = ctx.apd_solve(grid, X, A, v, eps, w=torch.zeros_like(w), opts=apd.make_opts(cull=cull))
+    assert rc == 0 and ro.status == OK and err <= eps
+    chk = oracle_assign(grid_o, wl.X, wl.A, w.cpu().numpy(), v=wl.v)
+    nm = parity.check_labels(grid_o, wl.X, wl.A, w.cpu().numpy(), labels.cpu().numpy(), chk)["mismatches"]
+    assert chk.err <= eps + 2 * nm * grid_o.voxel_volume / float(wl.v.min())
+    assert len(ev_g) == levels + 1 and [e > 0 for e in ev_g] == [e > 0 for e in ev_o]
+    for a, b in zip(ev_g, ev_o):
+        assert abs(a - b) <= max(6, b // 3)
+    assert ev_g[-1] < plain.evals
+    print(f"continuation cfg{cfg} {n}: evals per level gpu {ev_g} oracle {ev_o}; plain apd_solve {plain.evals} evaluations")
+    ctx.close()
