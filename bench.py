@@ -364,7 +364,7 @@ def config_record(apd, torch, cfg: int, local: int, flush, args, peaks_t, full: 
     if not args.no_solve:
         out["solve_culled"] = b.solve(1, K_AUTO, args.solve_max_iters, 2)
         if cfg >= 2:
-            out["solve_continuation"] = b.solve_continuation(2, args.solve_max_iters, 2)
+            out["solve_continuation"] = b.solve_continuation(1, args.solve_max_iters, 2)
         if full and cfg <= 4:
             out["solve_brute_force"] = b.solve(0, K_AUTO, args.solve_max_iters, 1)
     if full:
@@ -541,9 +541,9 @@ def run_ours(args):
             extra["culled_assign"] = kernel_record(b, K_AUTO, 1, flush, 5, *peaks_t)
             extra["solve"] = dict(workload=f"cfg{WORKLOAD_CFG} apd_solve, opts.cull=1",
                                   **b.solve(1, K_AUTO, args.solve_max_iters, 2))
-            extra["solve_continuation"] = dict(workload=f"cfg{WORKLOAD_CFG} apd_solve_continuation, 2 coarser levels, "
+            extra["solve_continuation"] = dict(workload=f"cfg{WORKLOAD_CFG} apd_solve_continuation, 1 coarser level, "
                                                         "opts.cull=1 (extension: not Algorithm 2's number)",
-                                               **b.solve_continuation(2, args.solve_max_iters, 2))
+                                               **b.solve_continuation(1, args.solve_max_iters, 2))
             extra["solve_brute_force"] = dict(workload=f"cfg{WORKLOAD_CFG} apd_solve, brute force",
                                               **b.solve(0, args.kernel, args.solve_max_iters, 1))
         cb = None

@@ -216,7 +216,9 @@ int apd_solve_refine(apd_ctx* ctx, apd_grid* grid, int32_t M, const float* X, co
 /* Coarse-to-fine continuation (an extension of Alg. 2 step 4, PAPER.md:157 -- not in the paper): the
  * weights do not depend on the resolution, so Algorithm 2 is run on `grid` coarsened by 2^levels, ..., 2, 1 per axis
  * (n_k -> ceil(n_k / 2^l); a level with some n_k < 16 is skipped), each level started from the weights of the one
- * before (a level that ends APD_NOT_CONVERGED hands on its best iterate).  The last level is apd_solve on `grid` itself:
+ * before (a level that ends APD_NOT_CONVERGED hands on its best iterate).  A coarse level is asked only for what its
+ * voxels can resolve, eq. (2.10) read backwards: tol_l = max(tol, 2^D |P_l| / min_i target_vol_i) (the call reads
+ * target_vol back to the host once for this).  The last level is apd_solve on `grid` itself with tol:
  * same post-condition, w, labels, vol; the return value is its status.  levels = 0 is apd_solve.
  *   iters, evals   HOST out [levels + 1], coarsest level first (0 for a skipped level); each may be NULL
  *   max_rel_err    HOST out, of the last level.   Everything else as apd_solve.  Blocks until finished. */

@@ -474,16 +474,21 @@ def oracle_solve_refine(grid: Grid, X, A, v, eps: float, max_refinements: int, w
 def oracle_solve_continuation(grid: Grid, X, A, v, eps: float, levels: int, w_init=None, **solve_kw):
     """Coarse-to-fine continuation (an extension of Alg. 2 step 4; reading S18b): Algorithm 2 on
     the grid coarsened by 2^levels, ..., 2, 1 per axis (n_k -> ceil(n_k / 2^l); a level with some n_k < 16 is skipped),
-    each level from the fp32 weights of the one before (a NOT_CONVERGED level hands on its best iterate).
+    each level from the fp32 weights of the one before (a NOT_CONVERGED level hands on its best iterate); a coarse
+    level's tolerance is eps_l = max(eps, 2^D |P_l| / v_min), the last level's is eps.
     Returns (SolveResult of the last level = on `grid`, [iters per level], [evals per level]), coarsest first."""
     w0 = w_init
     iters, evals, res = [], [], None
+    v_min = float(np.min(np.asarray(v, dtype=np.float32).astype(np.float64)))
     for l in range(levels, -1, -1):
         n = tuple((int(k) + (1 << l) - 1) >> l for k in grid.n[: grid.dim])
         if l > 0 and min(n) < 16:
             iters.append(0); evals.append(0)
             continue
-        res = oracle_solve(Grid(grid.dim, n, grid.lo, grid.hi), X, A, v, eps, w_init=w0, **solve_kw)
+        g_l = Grid(grid.dim, n, grid.lo, grid.hi)
+        # a coarse level is asked only for what its voxels can resolve: eq. (2.10) read backwards (PAPER.md:195-197)
+        eps_l = eps if l == 0 else max(eps, 2.0 ** grid.dim * g_l.voxel_volume / v_min)
+        res = oracle_solve(g_l, X, A, v, eps_l, w_init=w0, **solve_kw)
         iters.append(res.iters); evals.append(res.evals)
         w0 = res.w32
     return res, iters, evals

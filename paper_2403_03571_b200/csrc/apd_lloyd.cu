@@ -2,6 +2,7 @@
 // over apd_solve + the discrete centroids of the same pass, and the resolution rules of PAPER.md:182-197.
 #include "apd_internal.cuh"
 #include <cmath>
+#include <vector>
 
 namespace apd {
 
@@ -129,20 +130,39 @@ extern "C" int apd_solve_continuation(apd_ctx* ctx, const apd_grid* grid, int32_
   ctx->err.clear();
   if (!grid || !w || levels < 0 || levels > 8) { ctx->err = "apd_solve_continuation: grid, w required, 0 <= levels <= 8"; return APD_E_ARG; }
   if (grid->dim != 2 && grid->dim != 3) { ctx->err = "apd_solve_continuation: grid.dim must be 2 or 3"; return APD_E_ARG; }
+  if (!target_vol || M < 1 || M > ctx->ws.max_seeds) { ctx->err = "apd_solve_continuation: target_vol required, 1 <= M <= max_seeds"; return APD_E_ARG; }
   int rc = APD_OK;
   double err = 0.0;
   bool started = false;
+  // smallest target volume (host copy of the M floats): a coarse level is only asked for the tolerance its voxels can
+  // resolve, the paper's practical rule eq. (2.10) read backwards: eps_l = max(tol, 2^D |P_l| / v_min)
+  double v_min = 0.0;
+  if (levels > 0) {
+    std::vector<float> hv((size_t)M);
+    if (cudaSetDevice(ctx->ws.device) != cudaSuccess ||
+        cudaStreamSynchronize(static_cast<cudaStream_t>(cuda_stream)) != cudaSuccess ||
+        cudaMemcpy(hv.data(), target_vol, sizeof(float) * (size_t)M, cudaMemcpyDeviceToHost) != cudaSuccess) {
+      ctx->err = "apd_solve_continuation: could not read target_vol";
+      return APD_E_CUDA;
+    }
+    v_min = (double)hv[0];
+    for (int i = 1; i < M; ++i) v_min = std::fmin(v_min, (double)hv[i]);
+    if (!(v_min > 0.0)) { ctx->err = "apd_solve_continuation: target_vol must be > 0"; return APD_E_ARG; }
+  }
   for (int l = levels; l >= 0; --l) {
     apd_grid g = *grid;
     bool too_coarse = false;
+    double P = 1.0;
     for (int k = 0; k < grid->dim; ++k) {
       g.n[k] = (grid->n[k] + (1 << l) - 1) >> l;
       if (l > 0 && g.n[k] < 16) too_coarse = true;          // a level this coarse says nothing about the cells
+      P *= (grid->hi[k] - grid->lo[k]) / (double)g.n[k];
     }
     int it = 0, ev = 0;
     if (!too_coarse) {
       const bool last = (l == 0);
-      rc = apd_solve(ctx, &g, M, X, A, target_vol, tol, started ? w : w_init, w, last ? labels : nullptr,
+      const double tol_l = last ? tol : std::fmax(tol, std::pow(2.0, (double)grid->dim) * P / v_min);
+      rc = apd_solve(ctx, &g, M, X, A, target_vol, tol_l, started ? w : w_init, w, last ? labels : nullptr,
                      last ? vol : nullptr, nullptr, &it, &ev, &err, nullptr, opts, cuda_stream);
       if (rc < 0) return rc;
       started = true;
