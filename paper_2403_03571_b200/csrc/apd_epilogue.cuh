@@ -10,6 +10,7 @@ template <int V>
 __device__ __forceinline__ double row_epilogue(const AssignArgs& a, bool row_valid, int ix0, int iy, int iz,
                                                const float (&best)[V], const int (&lab)[V]) {
   double dsum = 0.0;
+  const unsigned vmask = __ballot_sync(0xffffffffu, row_valid);     // (every lane of the warp calls this function)
   if (!row_valid) return dsum;
   const int nvalid = min(V, a.g.nx - ix0);
   const long long j0 = ((long long)iz * a.g.ny + iy) * a.g.nx + ix0;
@@ -45,7 +46,13 @@ __device__ __forceinline__ double row_epilogue(const AssignArgs& a, bool row_val
       run_sx += (unsigned long long)(ix0 + k);
     }
   }
-  atomicAdd(a.count + run_lab, run_cnt);
+  // the last run of every row: the rows of a warp mostly end in the same cell, so the warp adds them up first and
+  // sends ONE atomic per distinct label (the counts are integers: exact whatever the grouping)
+  {
+    const unsigned peers = __match_any_sync(vmask, run_lab);
+    const unsigned int tot = __reduce_add_sync(peers, run_cnt);
+    if ((int)(threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(a.count + run_lab, tot);
+  }
   if (a.idxsum) {
     atomicAdd(a.idxsum + (size_t)run_lab * 3 + 0, run_sx);
     atomicAdd(a.idxsum + (size_t)run_lab * 3 + 1, (unsigned long long)run_cnt * (iy + a.g.off_y));
