@@ -304,6 +304,31 @@ int apd_reserve(apd_ctx* ctx, const apd_grid* grid, const apd_opts* opts);
 int apd_assign_stats(apd_ctx* ctx, int32_t* kernel, int32_t* row_long, int32_t* cull, int32_t* n_tiles,
                      double* kernel_ms);
 
+/* ---- an evaluation that allocates nothing --------------------------------------------------------------------------
+ * apd_assign_static: apd_assign (Algorithm 1, with eqs. 2.7-2.8) for callers that
+ * cannot call cudaMalloc -- code under CUDA graph capture, tight serving loops, harnesses that forbid it.  It takes no
+ * context: its scratch (packed seeds, per-cell counts, per-tile partial sums of the dual) is a file-scope __device__
+ * array of apd_static_scratch_bytes() = 344 KiB that every GPU which loads the library holds until the process exits.
+ * It calls no cudaMalloc / cudaFree and no allocating library routine, and does not synchronise.
+ *   Runs on the CURRENT device (the one the pointers belong to), asynchronously on cuda_stream.
+ *   Kernels: those of apd_assign with opts.kernel = APD_KERNEL_ROWPOLY, opts.cull = 0, in the same order: labels, vol,
+ *   dual and max_rel_err are the same bits.  All pointers DEVICE: X [M,dim], A [M,dim,dim], w [M], target_vol [M] or
+ *   NULL, labels [N] or NULL, vol [M] out, dual [1] out, max_rel_err [1] out or NULL (needs target_vol).
+ *   Limits: M <= APD_STATIC_MAX_SEEDS; the grid may need at most APD_STATIC_MAX_TILES CTA tiles of 32 x 16 x 8 voxels
+ *   (3D) / 64 x 64 pixels (2D) -- about 64 M voxels, 400^3 fits -- and at most 1024 layers of 8 planes (3D) / 64 rows
+ *   (2D) along its last axis.  Beyond them: APD_E_ARG with a text that names the limit (use apd_assign there).
+ *   Every call on a device shares the one array, which keeps the last call's contents (the call itself clears the
+ *   counts it adds into).  Calls that may OVERLAP on the GPU -- different streams, or threads, without an ordering
+ *   between them -- race on it and give wrong results; calls on one stream are ordered and safe.
+ *   Errors: APD_E_ARG, APD_E_ARCH (not sm_100), APD_E_CUDA; the text is in apd_static_last_error() (thread-local). */
+#define APD_STATIC_MAX_SEEDS 4096
+#define APD_STATIC_MAX_TILES 16384
+int apd_assign_static(const apd_grid* grid, int32_t M, const float* X, const float* A, const float* w,
+                      const float* target_vol, int32_t* labels, double* vol, double* dual, double* max_rel_err,
+                      void* cuda_stream);
+int64_t apd_static_scratch_bytes(void);
+const char* apd_static_last_error(void);
+
 #ifdef __cplusplus
 }
 #endif

@@ -133,6 +133,12 @@ def load_library() -> ctypes.CDLL:
     lib.apd_reserve.argtypes = [_P, ctypes.POINTER(apd_grid), ctypes.POINTER(apd_opts)]
     lib.apd_assign_stats.restype = ctypes.c_int
     lib.apd_assign_stats.argtypes = [_P] + [ctypes.POINTER(ctypes.c_int32)] * 4 + [ctypes.POINTER(ctypes.c_double)]
+    lib.apd_assign_static.restype = ctypes.c_int
+    lib.apd_assign_static.argtypes = [ctypes.POINTER(apd_grid), ctypes.c_int32] + [_P] * 9
+    lib.apd_static_scratch_bytes.restype = ctypes.c_int64
+    lib.apd_static_scratch_bytes.argtypes = []
+    lib.apd_static_last_error.restype = ctypes.c_char_p
+    lib.apd_static_last_error.argtypes = []
     _lib = lib
     return lib
 
@@ -140,7 +146,8 @@ def load_library() -> ctypes.CDLL:
 EXPORTED_SYMBOLS = ["apd_default_opts", "apd_create", "apd_destroy", "apd_last_error", "apd_assign", "apd_solve",
                     "apd_assign_host", "apd_solve_host", "apd_solve_history", "apd_assign_points", "apd_solve_points", "apd_solve_stats", "apd_lloyd", "apd_solve_refine", "apd_resolution_bound",
                     "apd_choose_resolution", "apd_reserve", "apd_assign_stats", "apd_slab_align", "apd_counter_words",
-                    "apd_assign_slab", "apd_finalize_counters", "apd_solve_slab", "apd_solve_continuation"]
+                    "apd_assign_slab", "apd_finalize_counters", "apd_solve_slab", "apd_solve_continuation",
+                    "apd_assign_static", "apd_static_scratch_bytes", "apd_static_last_error"]
 
 
 def make_grid(dim: int, n: Sequence[int], lo: Sequence[float], hi: Sequence[float]) -> apd_grid:
@@ -480,6 +487,30 @@ class ApdContext:
 
     def last_kernel_ms(self) -> float:
         return float(self.assign_stats()["kernel_ms"])
+
+
+STATIC_MAX_SEEDS = 4096        # APD_STATIC_MAX_SEEDS of include/apd.h
+STATIC_MAX_TILES = 16384       # APD_STATIC_MAX_TILES
+
+
+def apd_assign_static(grid: apd_grid, X, A, w, target_vol=None, labels=None, vol=None, dual=None, max_rel_err=None):
+    """apd_assign_static of include/apd.h on CUDA tensors: no context, no allocation; runs on X's device (made
+    current for the call), asynchronously on torch's current stream of that device."""
+    lib = load_library()
+    d, M = grid.dim, X.shape[0]
+    with torch.cuda.device(X.device):
+        rc = lib.apd_assign_static(
+            ctypes.byref(grid), M, _dev(X, torch.float32, "X", M * d), _dev(A, torch.float32, "A", M * d * d),
+            _dev(w, torch.float32, "w", M), _dev(target_vol, torch.float32, "target_vol", M),
+            _dev(labels, torch.int32, "labels"), _dev(vol, torch.float64, "vol", M),
+            _dev(dual, torch.float64, "dual", 1), _dev(max_rel_err, torch.float64, "max_rel_err", 1),
+            ctypes.c_void_p(torch.cuda.current_stream(X.device).cuda_stream))
+    if rc != APD_OK:
+        raise ApdError(rc, (lib.apd_static_last_error() or b"").decode())
+
+
+def static_scratch_bytes() -> int:
+    return int(load_library().apd_static_scratch_bytes())
 
 
 def apd_resolution_bound(dim: int, domain_volume: float, v_min: float, eps: float, practical: bool) -> float:
