@@ -168,14 +168,27 @@ __device__ __forceinline__ double* gram_of(const StepArgs& a, int cap, unsigned 
   return a.gram + (size_t)rank * ((size_t)(2 * cap + 1) * (2 * cap + 1) + cap);
 }
 
+// What an ACCEPTED step writes per element -- the curvature pair s = alpha p, y = g1 - g into ring slot `slot`,
+// w <- w_try, g <- g1 -- fused into the Gram pass (gram_rows<3, true>): the pass needs s, y and g1 anyway, so the
+// step saves a sweep over the vectors.
+struct PushArgs {
+  double alpha;
+  const double* p; const double* gnew; const double* wtry;
+  double* g; double* w; double* s_new; double* y_new;
+  int slot;
+};
+
 // Inner products of the NNEW vectors nv[] (Gram indices nidx[]; nv[NNEW-1] is g) with S_j and Y_j of every active
 // slot, and g.g, written to both triangles of this CTA's Gram copy.  LB_GRAM_SLOTS slots per pass over the vectors (one
-// pass and ONE cluster barrier for the default history of 10; it used to be one barrier per two slots): every inner
-// product is accumulated per thread in the same element order and reduced by the same tree as before, so its bits do
-// not depend on how many are formed at once.
-template <int NNEW>
+// pass and ONE cluster barrier for the default history of 10): every inner product is accumulated per thread in
+// element order and reduced by the same tree, so its bits do not depend on how many are formed at once.
+// PUSH (NNEW == 3): nv[0], nv[1] are the pair being pushed, formed HERE from (alpha, p, g1, g) and written to their
+// slot together with w <- w_try and g <- g1 (PushArgs); all loads of an element are issued before its stores, and the
+// products with the slot being overwritten use the new values from registers.
+template <int NNEW, bool PUSH>
 __device__ void gram_rows(const StepArgs& a, int cap, int hist_len, int hist_start, const double* (&nv)[NNEW],
-                          const int (&nidx)[NNEW], Reducer& r) {
+                          const int (&nidx)[NNEW], const PushArgs& pu, Reducer& r) {
+  static_assert(!PUSH || NNEW == 3, "a pushed pair comes with the new gradient");
   const int M = a.M, stride = a.stride, ld = 2 * cap + 1;
   const double* S = a.vec + (size_t)V_HIST * stride;
   const double* Y = S + (size_t)cap * stride;
@@ -183,21 +196,39 @@ __device__ void gram_rows(const StepArgs& a, int cap, int hist_len, int hist_sta
   constexpr int NS = LB_GRAM_SLOTS, NACC = NNEW * 2 * NS + 1;
   for (int t0 = 0; t0 < hist_len; t0 += NS) {
     const int ns = min(NS, hist_len - t0);
+    const bool push_now = PUSH && t0 == 0;          // the first pass writes the pair; later passes read it back
     size_t soff[NS];
+    int qnew = -1;                                  // position in this pass of the slot being pushed, if it is here
 #pragma unroll
-    for (int q = 0; q < NS; ++q) soff[q] = (size_t)((hist_start + t0 + (q < ns ? q : 0)) % cap) * stride;   // inactive: a duplicate, ignored
+    for (int q = 0; q < NS; ++q) {
+      const int sl = (hist_start + t0 + (q < ns ? q : 0)) % cap;      // inactive: a duplicate, ignored
+      soff[q] = (size_t)sl * stride;
+      if (push_now && q < ns && sl == pu.slot) qnew = q;
+    }
     double acc[NACC];
 #pragma unroll
     for (int n = 0; n < NACC; ++n) acc[n] = 0.0;
     for (int i = LB_FIRST(r); i < M; i += LB_STEP) {
-      double x[NNEW];
+      double x[NNEW], sv[NS], yv[NS], wt = 0.0;
+      if (push_now) {
+        const double pi = pu.p[i], gn = pu.gnew[i], go = pu.g[i];
+        wt = pu.wtry[i];
+        x[0] = __dmul_rn(pu.alpha, pi); x[1] = __dsub_rn(gn, go); x[NNEW - 1] = gn;
+      } else {
 #pragma unroll
-      for (int n = 0; n < NNEW; ++n) x[n] = nv[n][i];
+        for (int n = 0; n < NNEW; ++n) x[n] = nv[n][i];
+      }
+#pragma unroll
+      for (int q = 0; q < NS; ++q) { sv[q] = S[soff[q] + i]; yv[q] = Y[soff[q] + i]; }
+      if (push_now) {
+        pu.s_new[i] = x[0]; pu.y_new[i] = x[1]; pu.w[i] = wt; pu.g[i] = x[NNEW - 1];
+#pragma unroll
+        for (int q = 0; q < NS; ++q) if (q == qnew) { sv[q] = x[0]; yv[q] = x[1]; }
+      }
 #pragma unroll
       for (int q = 0; q < NS; ++q) {
-        const double sv = S[soff[q] + i], yv = Y[soff[q] + i];
 #pragma unroll
-        for (int n = 0; n < NNEW; ++n) { acc[(n * NS + q) * 2] += x[n] * sv; acc[(n * NS + q) * 2 + 1] += x[n] * yv; }
+        for (int n = 0; n < NNEW; ++n) { acc[(n * NS + q) * 2] += x[n] * sv[q]; acc[(n * NS + q) * 2 + 1] += x[n] * yv[q]; }
       }
       acc[NACC - 1] += x[NNEW - 1] * x[NNEW - 1];
     }
@@ -213,19 +244,20 @@ __device__ void gram_rows(const StepArgs& a, int cap, int hist_len, int hist_sta
     }
     if (threadIdx.x == 0 && t0 == 0) gm[(size_t)(2 * cap) * ld + 2 * cap] = r.tot[NACC - 1];
   }
-  __syncthreads();          // thread 0's global writes are ordered before the CTA's reads in direction_vf
+  __syncthreads();          // thread 0's global writes are ordered before the CTA's reads in direction_coeffs
 }
 
-// p = -H g with H0 = gamma I; returns g.p to all threads of the cluster.  dyn: dynamic shared memory of the CTA,
-// (2m+1)^2 + (2m+1) + 2m doubles and m ints (m = hist_len <= cap).  Every CTA runs the (tiny) coefficient recursion
-// redundantly on its own Gram copy; the combination pass is shared out over the cluster's threads.
-__device__ double direction_vf(const StepArgs& a, int cap, int hist_len, int hist_start, double gamma, Reducer& r,
-                               double* dyn) {
-  const int M = a.M, stride = a.stride, ld = 2 * cap + 1, hl = hist_len, n = 2 * hl + 1, tid = threadIdx.x;
-  double* g = a.vec + (size_t)V_G * stride;
-  double* p = a.vec + (size_t)V_P * stride;
-  const double* S = a.vec + (size_t)V_HIST * stride;
-  const double* Y = S + (size_t)cap * stride;
+// The coefficients of p = -H g (H0 = gamma I) in the basis (S.., Y.., g), left in the CTA's dynamic shared memory
+// `dyn`: (2m+1)^2 + (2m+1) + 2m doubles and m ints (m = hist_len <= cap).  Every CTA runs the (tiny) coefficient
+// recursion redundantly on its own Gram copy.
+struct DirCoef {
+  const double* delta;     // [2 hl + 1]: S coefficients, Y coefficients, g coefficient
+  const int* slot_of;      // [hl] ring slot of pair t (0 = oldest)
+  int hl;
+};
+__device__ DirCoef direction_coeffs(const StepArgs& a, int cap, int hist_len, int hist_start, double gamma,
+                                    const Reducer& r, double* dyn) {
+  const int ld = 2 * cap + 1, hl = hist_len, n = 2 * hl + 1, tid = threadIdx.x;
   const double* gm = gram_of(a, cap, r.rank);
   const double* rho_g = gm + (size_t)ld * ld;
   double* Cm = dyn;                    // [n][n] compact Gram matrix in RING order (0 = oldest pair)
@@ -241,7 +273,41 @@ __device__ double direction_vf(const StepArgs& a, int cap, int hist_len, int his
   }
   if (tid < hl) { const int sl = (hist_start + tid) % cap; slot_of[tid] = sl; rho[tid] = rho_g[sl]; }
   __syncthreads();
-  if (tid < 32) {
+  if (tid < 32 && hl <= 32) {
+    // The two-loop recursion [70] on coefficients, as two TRIANGULAR substitutions with lane t owning pair t (ring
+    // order, 0 = oldest).  Written out, the first loop's alpha_t = rho_t s_t.q_t with q_t = g - sum_{u>t} alpha_u y_u is
+    //     alpha_t / rho_t = s_t.g - sum_{u>t} (s_t.y_u) alpha_u,
+    // and the second loop's beta_t = rho_t y_t.r_t with r_t = gamma q_0 + sum_{u<t} c_u s_u, c_u = alpha_u - beta_u, is
+    //     beta_t / rho_t = gamma (y_t.g - sum_u (y_t.y_u) alpha_u) + sum_{u<t} (y_t.s_u) c_u:
+    // once alpha_u (c_u) is known every lane folds it into its own right-hand side, so a step of the dependent chain
+    // is one multiply, one shuffle and one FMA instead of a 5-round shuffle reduction through shared memory (9 us of
+    // the step at m = 10).  The same terms as the textbook loops, summed pair by pair.
+    const int lane = tid;
+    const bool mine = lane < hl;
+    const double* rowS = Cm + (size_t)(mine ? lane : 0) * n;            // s_t . (S.., Y.., g)
+    const double* rowY = Cm + (size_t)(mine ? hl + lane : 0) * n;       // y_t . (S.., Y.., g)
+    const double rho_me = mine ? rho[lane] : 0.0;
+    double rhs = mine ? rowS[2 * hl] : 0.0, alpha_me = 0.0;
+    for (int u = hl - 1; u >= 0; --u) {                 // newest -> oldest
+      const double au = __shfl_sync(0xffffffffu, __dmul_rn(rho_me, rhs), u);
+      if (lane == u) alpha_me = au;
+      if (lane < u) rhs = __fma_rn(-rowS[hl + u], au, rhs);
+    }
+    double b = mine ? rowY[2 * hl] : 0.0;
+    for (int u = 0; u < hl; ++u) {
+      const double au = __shfl_sync(0xffffffffu, alpha_me, u);
+      if (mine) b = __fma_rn(-rowY[hl + u], au, b);
+    }
+    double acc = __dmul_rn(gamma, b), c_me = 0.0;
+    for (int u = 0; u < hl; ++u) {                      // oldest -> newest
+      const double cu = __shfl_sync(0xffffffffu, __dsub_rn(alpha_me, __dmul_rn(rho_me, acc)), u);
+      if (lane == u) c_me = cu;
+      if (mine && lane > u) acc = __fma_rn(rowY[u], cu, acc);
+    }
+    if (mine) { delta[lane] = c_me; delta[hl + lane] = -__dmul_rn(gamma, alpha_me); }
+    if (lane == 0) delta[2 * hl] = gamma;
+  } else if (tid < 32) {
+    // histories longer than a warp: the textbook loops on the coefficient vector
     const int lane = tid;
     for (int j = lane; j < n; j += 32) delta[j] = (j == n - 1) ? 1.0 : 0.0;
     __syncwarp();
@@ -266,22 +332,63 @@ __device__ double direction_vf(const StepArgs& a, int cap, int hist_len, int his
     }
   }
   __syncthreads();
-  // combination pass: p = -sum_j delta_j b_j, and g.p in the same sweep
-  const double dg = delta[2 * hl];
-  double gp = 0.0;
+  return DirCoef{delta, slot_of, hl};
+}
+
+// The combination pass fused with the trial point: for every element
+//     p = -(delta_g g + sum_t delta_t s_t + delta_{m+t} y_t),   w_try = w + alpha p  (alpha = 1: a new direction),
+// w32 = fl32(w_try) (S10), the best-so-far copy of the point just evaluated, and ONE exchange for g.p (sum) and the two
+// maxima the candidate-list reuse needs (|change since the last evaluation|, |distance from wref|).  The history
+// loads of an element are issued LB_COMB_SLOTS pairs at a time before any of them is used (a loop of dependent
+// load-FMA pairs ran at one L2 round trip per four pairs: 9 of the step's 36 us at M = 10^4).
+constexpr int LB_COMB_SLOTS = 10;
+struct TrialArgs {
+  bool improved;             // copy w_eval -> w_best first
+  const double* w_eval;      // the point the evaluation just run was taken at
+  double alpha;
+};
+__device__ void combine_and_trial(const StepArgs& a, int cap, const DirCoef& dc, const TrialArgs& ta, Reducer& r,
+                                  double* gp_out, double (&mx_out)[2]) {
+  const int M = a.M, stride = a.stride, hl = dc.hl;
+  const double* g = a.vec + (size_t)V_G * stride;
+  double* p = a.vec + (size_t)V_P * stride;
+  const double* w = a.vec + (size_t)V_W * stride;
+  double* wtry = a.vec + (size_t)V_WTRY * stride;
+  double* wbest = a.vec + (size_t)V_WBEST * stride;
+  const double* S = a.vec + (size_t)V_HIST * stride;
+  const double* Y = S + (size_t)cap * stride;
+  const double dg = dc.delta[2 * hl];
+  double red3[3] = {0.0, 0.0, 0.0};      // g.p | max |change since the last evaluation|, max |distance from wref|
+  constexpr int NC = LB_COMB_SLOTS;
   for (int i = LB_FIRST(r); i < M; i += LB_STEP) {
-    const double gi = g[i];
+    const double gi = g[i], wi = w[i];
+    const double we = ta.improved ? ta.w_eval[i] : 0.0;
+    const float w32_old = a.w32[i], wref = a.wref[i];
     double acc = dg * gi;
-#pragma unroll 4
-    for (int t = 0; t < hl; ++t) {
-      const size_t off = (size_t)slot_of[t] * stride + i;
-      acc += delta[t] * S[off] + delta[hl + t] * Y[off];
+    for (int t0 = 0; t0 < hl; t0 += NC) {
+      double sv[NC], yv[NC];
+#pragma unroll
+      for (int q = 0; q < NC; ++q) {
+        const size_t off = (size_t)dc.slot_of[t0 + q < hl ? t0 + q : t0] * stride + i;     // past the end: a duplicate
+        sv[q] = S[off]; yv[q] = Y[off];
+      }
+#pragma unroll
+      for (int q = 0; q < NC; ++q)
+        if (t0 + q < hl) acc = __dadd_rn(acc, __fma_rn(dc.delta[hl + t0 + q], yv[q], __dmul_rn(dc.delta[t0 + q], sv[q])));
     }
     const double pi = -acc;
     p[i] = pi;
-    gp += gi * pi;
+    red3[0] += gi * pi;
+    if (ta.improved) wbest[i] = we;        // (w_eval may be w_try: read above, before w_try is rewritten)
+    const double wt = __dadd_rn(wi, __dmul_rn(ta.alpha, pi));
+    wtry[i] = wt;
+    const float wn = (float)wt;
+    red3[1] = fmax(red3[1], fabs((double)wn - (double)w32_old));      // differences of floats: exact in fp64
+    red3[2] = fmax(red3[2], fabs((double)wn - (double)wref));
+    a.w32[i] = wn;
   }
-  return cluster_allsum(gp, r);
+  cluster_all_mixed<3, 2>(red3, r);
+  *gp_out = red3[0]; mx_out[0] = red3[1]; mx_out[1] = red3[2];
 }
 
 __global__ void solve_init_kernel(StepArgs a, const float* w_init, int hist_cap, int max_iters, int max_evals,
@@ -403,7 +510,9 @@ __global__ void __cluster_dims__(LB_CLUSTER, 1, 1) __launch_bounds__(LB_THREADS)
 
   int finish = 0;          // 1: OK at w_eval, 2: NOT_CONVERGED at best, 3: bad target volumes
   bool need_direction = false;
+  double mx[2] = {0.0, 0.0};   // max |change of fl32 w since the last evaluation|, max |distance from wref|
   int new_slot = -1;       // ring slot a curvature pair was pushed into by this call, else -1
+  PushArgs push{};
   if (phase == 0) {
     // cost scale for the list-reuse slack: mean over the voxels of min_i C_ij = (g~ - <v, w>) / |Omega|  (identity I1)
     const double scale = fabs(P * smin) / domain_volume;
@@ -451,15 +560,19 @@ __global__ void __cluster_dims__(LB_CLUSTER, 1, 1) __launch_bounds__(LB_THREADS)
           if (hist_len < cap) hist_len += 1; else hist_start = (hist_start + 1) % cap;
           gamma = sy / yy;
         }
-        for (int i = LB_FIRST(red); i < M; i += LB_STEP) {
-          const double gn = gnew[i];
-          if (keep) { s_new[i] = __dmul_rn(alpha, p[i]); y_new[i] = __dsub_rn(gn, g[i]); }
-          w[i] = wtry[i]; g[i] = gn;
-        }
         f = f1;
         iters += 1;
         if (iters >= max_iters || evals >= max_evals) finish = 2;
         else need_direction = true;
+        push.alpha = alpha; push.p = p; push.gnew = gnew; push.wtry = wtry; push.g = g; push.w = w;
+        push.s_new = s_new; push.y_new = y_new; push.slot = slot;
+        if (!(keep && need_direction)) {      // (else these writes ride on the Gram pass below)
+          for (int i = LB_FIRST(red); i < M; i += LB_STEP) {
+            const double gn = gnew[i];
+            if (keep) { s_new[i] = __dmul_rn(alpha, p[i]); y_new[i] = __dsub_rn(gn, g[i]); }
+            w[i] = wtry[i]; g[i] = gn;
+          }
+        }
       }
     }
   }
@@ -467,39 +580,46 @@ __global__ void __cluster_dims__(LB_CLUSTER, 1, 1) __launch_bounds__(LB_THREADS)
   if (need_direction) {
     if (hist_len > 0) {
       // refresh the Gram rows that changed: those of the pushed pair (if any) and the row of the new gradient
-      if (new_slot >= 0) {
+      if (new_slot >= 0) {      // (an accepted step whose pair is kept: its vector writes happen in this pass)
         const double* nv[3] = {S + (size_t)new_slot * stride, Y + (size_t)new_slot * stride, g};
         const int nidx[3] = {new_slot, cap + new_slot, 2 * cap};
-        gram_rows<3>(a, cap, hist_len, hist_start, nv, nidx, red);
+        gram_rows<3, true>(a, cap, hist_len, hist_start, nv, nidx, push, red);
       } else {
         const double* nv[1] = {g};
         const int nidx[1] = {2 * cap};
-        gram_rows<1>(a, cap, hist_len, hist_start, nv, nidx, red);
+        gram_rows<1, false>(a, cap, hist_len, hist_start, nv, nidx, push, red);
       }
     }
-    gp = direction_vf(a, cap, hist_len, hist_start, gamma, red, s_dyn);
+    // the new direction and, in the same pass, the first trial point along it (alpha = 1)
+    alpha = 1.0; lo = 0.0; hi = INFINITY; trial = 0;
+    DirCoef dc = direction_coeffs(a, cap, hist_len, hist_start, gamma, red, s_dyn);
+    combine_and_trial(a, cap, dc, TrialArgs{improved, w_eval, alpha}, red, &gp, mx);
     if (gp >= 0.0) {    // safeguard: not a descent direction -> steepest descent scaled by gamma
       hist_len = 0; hist_start = 0;
-      gp = direction_vf(a, cap, 0, 0, gamma, red, s_dyn);
+      const double mx0 = mx[0];
+      dc = direction_coeffs(a, cap, 0, 0, gamma, red, s_dyn);
+      combine_and_trial(a, cap, dc, TrialArgs{false, w_eval, alpha}, red, &gp, mx);     // (the best-so-far copy is made)
+      mx[0] += mx0;     // w32 was rewritten by the first pass: |change since the last evaluation| <= the sum (it only
+                        // sizes the slack of a rebuilt candidate list; any value is exact)
     }
-    alpha = 1.0; lo = 0.0; hi = INFINITY; trial = 0;
   }
 
   int cull_rebuild = 1;
   float cull_delta = 0.0f;
   if (finish == 0) {
-    // next trial point w + alpha p, rounded to fp32 for the evaluation (S10)
-    double mx[2] = {0.0, 0.0};   // max |change since the last evaluation|, max |distance from wref|
-    for (int i = LB_FIRST(red); i < M; i += LB_STEP) {
-      if (improved) wbest[i] = w_eval[i];      // best-so-far copy of the point just evaluated (before wtry is rewritten)
-      const double wt = __dadd_rn(w[i], __dmul_rn(alpha, p[i]));
-      wtry[i] = wt;
-      const float wn = (float)wt;
-      mx[0] = fmax(mx[0], fabs((double)wn - (double)a.w32[i]));     // differences of floats: exact in fp64
-      mx[1] = fmax(mx[1], fabs((double)wn - (double)a.wref[i]));
-      a.w32[i] = wn;
+    if (!need_direction) {
+      // next trial point w + alpha p of the line search, rounded to fp32 for the evaluation (S10)
+      for (int i = LB_FIRST(red); i < M; i += LB_STEP) {
+        if (improved) wbest[i] = w_eval[i];      // best-so-far copy of the point just evaluated (before wtry is rewritten)
+        const double wt = __dadd_rn(w[i], __dmul_rn(alpha, p[i]));
+        wtry[i] = wt;
+        const float wn = (float)wt;
+        mx[0] = fmax(mx[0], fabs((double)wn - (double)a.w32[i]));     // differences of floats: exact in fp64
+        mx[1] = fmax(mx[1], fabs((double)wn - (double)a.wref[i]));
+        a.w32[i] = wn;
+      }
+      cluster_all<2, true>(mx, red);
     }
-    cluster_all<2, true>(mx, red);
     cull_delta = cull_delta_old;
     cull_rebuild = !(mx[1] <= (double)cull_delta);
     if (cull_rebuild) {
