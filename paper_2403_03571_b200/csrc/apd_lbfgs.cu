@@ -76,9 +76,12 @@ constexpr double CULL_CAP_FACTOR = 0.5;     // ... but at most this x the mean m
 // thread of every CTA (lanes by shuffle tree, warps in order, CTAs in rank order), which keeps the control flow
 // uniform over the whole cluster.  Cluster partials are exchanged through distributed shared memory; two buffers
 // are used alternately so that one cluster barrier per reduction suffices.
-constexpr int LB_GRAM_SLOTS = 10;                    // history slots whose inner products one Gram pass forms at once
-constexpr int LB_NRED = 3 * 2 * LB_GRAM_SLOTS + 1;   // most values reduced at once (gram_rows: 3 new vectors x (S, Y) of
-                                                     // LB_GRAM_SLOTS slots, + g.g)
+constexpr int LB_GRAM_SLOTS = 10;                    // history slots whose inner products one pass forms at once
+constexpr int LB_NPROD = 3 * 2 * LB_GRAM_SLOTS;      // (s, y, g1) x (S_j, Y_j) of LB_GRAM_SLOTS slots
+constexpr int LB_NPROD_PAD = (LB_NPROD + 31) / 32 * 32;   // padded to whole warps: the products are reduced TRANSPOSED
+// scalars of the evaluation sweep (the last one is a maximum, the others sums)
+enum { SC_VW = 0, SC_V, SC_G1P, SC_SY, SC_SS, SC_YY, SC_G1S, SC_G1Y, SC_G1G1, SC_ERR, LB_NSCAL };
+constexpr int LB_NRED = LB_NPROD_PAD + LB_NSCAL;     // most values reduced at once (eval_sweep)
 
 struct Reducer {
   double* wbuf;        // [LB_THREADS / 32][LB_NRED]   warp partials of this CTA
@@ -88,12 +91,39 @@ struct Reducer {
   unsigned int rank;
 };
 
-// v[0 .. N-NMAX) are SUMMED, v[N-NMAX .. N) are MAXIMISED, all in one exchange (one cluster barrier)
-template <int N, int NMAX>
+// One halving step of the TRANSPOSED warp reduction: lanes whose BIT is set keep the upper HALF of the values, the
+// others the lower, and each adds what its partner sends of the half it keeps (one shuffle per PAIR of values).
+template <int HALF, int BIT, int N>
+__device__ __forceinline__ void warp_transpose_step(double (&v)[N], int lane) {
+  const bool up = (lane & BIT) != 0;
+#pragma unroll
+  for (int k = 0; k < HALF; ++k) {
+    const double keep = up ? v[k + HALF] : v[k];
+    const double send = up ? v[k] : v[k + HALF];
+    v[k] = keep + __shfl_xor_sync(0xffffffffu, send, BIT);
+  }
+}
+
+// v[0 .. N-NMAX) are SUMMED, v[N-NMAX .. N) are MAXIMISED, all in one exchange (one cluster barrier).  Every value
+// goes through one fixed tree: lanes, then warps in order, then CTAs in rank order.  The lane stage of the first
+// NT = 32 floor((N - NMAX) / 32) sums is the transposed reduction (5 halving steps, after which each lane holds the
+// totals of NT / 32 values: NT - NT/32 shuffles instead of 5 NT -- the warp shuffle unit, one instruction per clock
+// per SM, was what a 70-value exchange waited for); the rest go through the xor butterfly.  A value's tree depends
+// only on whether its index is below NT.  READBACK = false: the totals are left in r.tot[] only.
+template <int N, int NMAX, bool READBACK = true>
 __device__ __forceinline__ void cluster_all_mixed(double (&v)[N], Reducer& r) {
   cg::cluster_group cluster = cg::this_cluster();
+  constexpr int NT = (N - NMAX) / 32 * 32, PER = NT / 32;
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  if constexpr (NT > 0) {
+    warp_transpose_step<NT / 2, 16>(v, lane);
+    warp_transpose_step<NT / 4, 8>(v, lane);
+    warp_transpose_step<NT / 8, 4>(v, lane);
+    warp_transpose_step<NT / 16, 2>(v, lane);
+    warp_transpose_step<NT / 32, 1>(v, lane);
+  }
 #pragma unroll
-  for (int n = 0; n < N; ++n) {
+  for (int n = NT; n < N; ++n) {
     const bool MAX = n >= N - NMAX;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
@@ -101,11 +131,17 @@ __device__ __forceinline__ void cluster_all_mixed(double (&v)[N], Reducer& r) {
       v[n] = MAX ? fmax(v[n], u) : v[n] + u;
     }
   }
-  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   __syncthreads();                                   // wbuf free (its last readers are past this point)
+  if constexpr (NT > 0) {
+    // lane L holds the totals of values base(L) + j, j < PER
+    const int base = ((lane >> 4) & 1) * (NT / 2) + ((lane >> 3) & 1) * (NT / 4) + ((lane >> 2) & 1) * (NT / 8) +
+                     ((lane >> 1) & 1) * (NT / 16) + (lane & 1) * (NT / 32);
+#pragma unroll
+    for (int j = 0; j < PER; ++j) r.wbuf[wid * LB_NRED + base + j] = v[j];
+  }
   if (lane == 0) {
 #pragma unroll
-    for (int n = 0; n < N; ++n) r.wbuf[wid * LB_NRED + n] = v[n];
+    for (int n = NT; n < N; ++n) r.wbuf[wid * LB_NRED + n] = v[n];
   }
   __syncthreads();
   r.flip ^= 1;
@@ -134,8 +170,10 @@ __device__ __forceinline__ void cluster_all_mixed(double (&v)[N], Reducer& r) {
     r.tot[threadIdx.x] = t;
   }
   __syncthreads();
+  if constexpr (READBACK) {
 #pragma unroll
-  for (int n = 0; n < N; ++n) v[n] = r.tot[n];
+    for (int n = 0; n < N; ++n) v[n] = r.tot[n];
+  }
 }
 template <int N, bool MAX>
 __device__ __forceinline__ void cluster_all(double (&v)[N], Reducer& r) { cluster_all_mixed<N, MAX ? N : 0>(v, r); }
@@ -168,224 +206,323 @@ __device__ __forceinline__ double* gram_of(const StepArgs& a, int cap, unsigned 
   return a.gram + (size_t)rank * ((size_t)(2 * cap + 1) * (2 * cap + 1) + cap);
 }
 
-// What an ACCEPTED step writes per element -- the curvature pair s = alpha p, y = g1 - g into ring slot `slot`,
-// w <- w_try, g <- g1 -- fused into the Gram pass (gram_rows<3, true>): the pass needs s, y and g1 anyway, so the
-// step saves a sweep over the vectors.
-struct PushArgs {
-  double alpha;
-  const double* p; const double* gnew; const double* wtry;
-  double* g; double* w; double* s_new; double* y_new;
-  int slot;
-};
-
-// Inner products of the NNEW vectors nv[] (Gram indices nidx[]; nv[NNEW-1] is g) with S_j and Y_j of every active
-// slot, and g.g, written to both triangles of this CTA's Gram copy.  LB_GRAM_SLOTS slots per pass over the vectors (one
-// pass and ONE cluster barrier for the default history of 10): every inner product is accumulated per thread in
-// element order and reduced by the same tree, so its bits do not depend on how many are formed at once.
-// PUSH (NNEW == 3): nv[0], nv[1] are the pair being pushed, formed HERE from (alpha, p, g1, g) and written to their
-// slot together with w <- w_try and g <- g1 (PushArgs); all loads of an element are issued before its stores, and the
-// products with the slot being overwritten use the new values from registers.
-template <int NNEW, bool PUSH>
-__device__ void gram_rows(const StepArgs& a, int cap, int hist_len, int hist_start, const double* (&nv)[NNEW],
-                          const int (&nidx)[NNEW], const PushArgs& pu, Reducer& r) {
-  static_assert(!PUSH || NNEW == 3, "a pushed pair comes with the new gradient");
-  const int M = a.M, stride = a.stride, ld = 2 * cap + 1;
+// ---- the sweep over the evaluation just run ---------------------------------------------------------------------
+// ONE pass and ONE exchange for everything that depends only on that evaluation and on the state at entry:
+// <v, fl32 w> and the eq. (2.5) error (a9), the gradient g1 = vol - v of f at the evaluated point (eq. 2.8), the inner
+// products of the line-search tests and of the curvature pair s = alpha p, y = g1 - g, and -- GRAM, i.e. when there
+// is a history -- speculatively the Gram rows an ACCEPTED step needs: (s, y, g1) . (S_j, Y_j) for the first
+// LB_GRAM_SLOTS active slots (nearly every evaluation is accepted: 161 of 163 on cfg 4; a rejected trial wastes
+// the products, not a pass).  Sums are accumulated per thread in element order and reduced by one tree each, so a
+// value's bits do not depend on what shares the exchange.  Leaves g1 in gnew; writes nothing else.
+// The cluster totals are left in r.tot[]:
+//   GRAM:  [0 .. LB_NPROD) products, [(n * LB_GRAM_SLOTS + q) * 2 + (0: S, 1: Y)], n = 0: s, 1: y, 2: g1, q = position
+//          of the slot in ring order (0 = oldest); [LB_NPROD_PAD + SC_*] the scalars;     !GRAM: [SC_*] the scalars.
+template <bool GRAM>
+__device__ void eval_sweep(const StepArgs& a, int phase, double alpha, int cap, int hist_len, int hist_start,
+                           Reducer& r) {
+  double out[LB_NRED];
+  const int M = a.M, stride = a.stride;
+  const double P = a.voxel_volume;
+  const double* g = a.vec + (size_t)V_G * stride;
+  const double* p = a.vec + (size_t)V_P * stride;
+  double* gnew = a.vec + (size_t)V_GNEW * stride;
   const double* S = a.vec + (size_t)V_HIST * stride;
   const double* Y = S + (size_t)cap * stride;
-  double* gm = gram_of(a, cap, r.rank);
-  constexpr int NS = LB_GRAM_SLOTS, NACC = NNEW * 2 * NS + 1;
-  for (int t0 = 0; t0 < hist_len; t0 += NS) {
-    const int ns = min(NS, hist_len - t0);
-    const bool push_now = PUSH && t0 == 0;          // the first pass writes the pair; later passes read it back
-    size_t soff[NS];
-    int qnew = -1;                                  // position in this pass of the slot being pushed, if it is here
+  constexpr int NS = LB_GRAM_SLOTS;
+  size_t soff[NS];
 #pragma unroll
-    for (int q = 0; q < NS; ++q) {
-      const int sl = (hist_start + t0 + (q < ns ? q : 0)) % cap;      // inactive: a duplicate, ignored
-      soff[q] = (size_t)sl * stride;
-      if (push_now && q < ns && sl == pu.slot) qnew = q;
-    }
-    double acc[NACC];
+  for (int q = 0; q < NS; ++q) soff[q] = (size_t)((hist_start + (q < hist_len ? q : 0)) % cap) * stride;   // inactive: a duplicate
 #pragma unroll
-    for (int n = 0; n < NACC; ++n) acc[n] = 0.0;
-    for (int i = LB_FIRST(r); i < M; i += LB_STEP) {
-      double x[NNEW], sv[NS], yv[NS], wt = 0.0;
-      if (push_now) {
-        const double pi = pu.p[i], gn = pu.gnew[i], go = pu.g[i];
-        wt = pu.wtry[i];
-        x[0] = __dmul_rn(pu.alpha, pi); x[1] = __dsub_rn(gn, go); x[NNEW - 1] = gn;
-      } else {
-#pragma unroll
-        for (int n = 0; n < NNEW; ++n) x[n] = nv[n][i];
-      }
+  for (int n = 0; n < LB_NRED; ++n) out[n] = 0.0;
+  double* sc = out + LB_NPROD_PAD;
+  for (int i = LB_FIRST(r); i < M; i += LB_STEP) {
+    const double tv = (double)a.v[i];
+    const double w32 = (double)a.w32[i];
+    const double vi = a.vol_in ? a.vol_in[i] : (a.count64 ? (double)a.count64[i] : (double)a.count[i]) * P;
+    double pi = 0.0, go = 0.0, sv[NS], yv[NS];
+    if (phase != 0) { pi = p[i]; go = g[i]; }
+    if (GRAM) {
 #pragma unroll
       for (int q = 0; q < NS; ++q) { sv[q] = S[soff[q] + i]; yv[q] = Y[soff[q] + i]; }
-      if (push_now) {
-        pu.s_new[i] = x[0]; pu.y_new[i] = x[1]; pu.w[i] = wt; pu.g[i] = x[NNEW - 1];
-#pragma unroll
-        for (int q = 0; q < NS; ++q) if (q == qnew) { sv[q] = x[0]; yv[q] = x[1]; }
-      }
-#pragma unroll
-      for (int q = 0; q < NS; ++q) {
-#pragma unroll
-        for (int n = 0; n < NNEW; ++n) { acc[(n * NS + q) * 2] += x[n] * sv[q]; acc[(n * NS + q) * 2 + 1] += x[n] * yv[q]; }
-      }
-      acc[NACC - 1] += x[NNEW - 1] * x[NNEW - 1];
     }
-    cluster_all<NACC, false>(acc, r);
-    // the totals also sit in r.tot (shared memory): the write-back indexes THAT with its run-time slot count, so that
-    // acc[] is only ever indexed by constants and stays in registers
-    if ((int)threadIdx.x < NNEW * ns) {
-      const int n = (int)threadIdx.x / ns, k = (int)threadIdx.x % ns;
-      const int q = nidx[n], j = (hist_start + t0 + k) % cap;
-      const double vs = r.tot[(n * NS + k) * 2], vy = r.tot[(n * NS + k) * 2 + 1];
-      gm[(size_t)q * ld + j] = vs; gm[(size_t)j * ld + q] = vs;
-      gm[(size_t)q * ld + cap + j] = vy; gm[(size_t)(cap + j) * ld + q] = vy;
+    sc[SC_VW] += tv * w32;
+    sc[SC_ERR] = fmax(sc[SC_ERR], fabs(vi - tv) / tv);
+    const double gn = vi - tv;                                  // m_i |P| - v_i
+    gnew[i] = gn;
+    sc[SC_V] += tv;
+    sc[SC_G1G1] += gn * gn;
+    if (phase != 0) {
+      const double si = __dmul_rn(alpha, pi);
+      const double yi = __dsub_rn(gn, go);
+      sc[SC_G1P] += gn * pi; sc[SC_SY] += si * yi; sc[SC_SS] += si * si; sc[SC_YY] += yi * yi;
+      sc[SC_G1S] += gn * si; sc[SC_G1Y] += gn * yi;
+      if (GRAM) {
+        const double x[3] = {si, yi, gn};
+#pragma unroll
+        for (int q = 0; q < NS; ++q) {
+#pragma unroll
+          for (int n = 0; n < 3; ++n) { out[(n * NS + q) * 2] += x[n] * sv[q]; out[(n * NS + q) * 2 + 1] += x[n] * yv[q]; }
+        }
+      }
     }
-    if (threadIdx.x == 0 && t0 == 0) gm[(size_t)(2 * cap) * ld + 2 * cap] = r.tot[NACC - 1];
   }
-  __syncthreads();          // thread 0's global writes are ordered before the CTA's reads in direction_coeffs
+  if (GRAM) cluster_all_mixed<LB_NRED, 1, false>(out, r);
+  else {
+    double t[LB_NSCAL];
+#pragma unroll
+    for (int n = 0; n < LB_NSCAL; ++n) t[n] = sc[n];
+    cluster_all_mixed<LB_NSCAL, 1, false>(t, r);
+  }
 }
 
-// The coefficients of p = -H g (H0 = gamma I) in the basis (S.., Y.., g), left in the CTA's dynamic shared memory
-// `dyn`: (2m+1)^2 + (2m+1) + 2m doubles and m ints (m = hist_len <= cap).  Every CTA runs the (tiny) coefficient
-// recursion redundantly on its own Gram copy.
+// The same products for the active slots [t0, t0 + ns) of a history longer than LB_GRAM_SLOTS (t0 > 0): run after an
+// accepted step's decision and BEFORE its vector writes (s, y, g1 are formed from alpha, p, gnew and the old g).
+// The cluster totals are left in r.tot[0 .. LB_NPROD).
+__device__ void gram_products(const StepArgs& a, double alpha, int cap, int hist_start, int t0, int ns, Reducer& r) {
+  const int M = a.M, stride = a.stride;
+  const double* g = a.vec + (size_t)V_G * stride;
+  const double* p = a.vec + (size_t)V_P * stride;
+  const double* gnew = a.vec + (size_t)V_GNEW * stride;
+  const double* S = a.vec + (size_t)V_HIST * stride;
+  const double* Y = S + (size_t)cap * stride;
+  constexpr int NS = LB_GRAM_SLOTS;
+  size_t soff[NS];
+#pragma unroll
+  for (int q = 0; q < NS; ++q) soff[q] = (size_t)((hist_start + t0 + (q < ns ? q : 0)) % cap) * stride;
+  double acc[LB_NPROD_PAD];
+#pragma unroll
+  for (int n = 0; n < LB_NPROD_PAD; ++n) acc[n] = 0.0;
+  for (int i = LB_FIRST(r); i < M; i += LB_STEP) {
+    const double gn = gnew[i];
+    const double x[3] = {__dmul_rn(alpha, p[i]), __dsub_rn(gn, g[i]), gn};
+    double sv[NS], yv[NS];
+#pragma unroll
+    for (int q = 0; q < NS; ++q) { sv[q] = S[soff[q] + i]; yv[q] = Y[soff[q] + i]; }
+#pragma unroll
+    for (int q = 0; q < NS; ++q) {
+#pragma unroll
+      for (int n = 0; n < 3; ++n) { acc[(n * NS + q) * 2] += x[n] * sv[q]; acc[(n * NS + q) * 2 + 1] += x[n] * yv[q]; }
+    }
+  }
+  cluster_all_mixed<LB_NPROD_PAD, 0, false>(acc, r);
+}
+
+// The CTA's working copy of the Gram matrix lives in its dynamic shared memory for the length of a step (GramSmem):
+// prefetched from the CTA's global copy at entry, patched after the decision, read by direction_coeffs; every patch
+// is also written through to the global copy, which carries it to the next launch.  Layout (doubles): the matrix in
+// SLOT space [ld x ld], ld = 2 cap + 1 (S slot j -> j, Y slot j -> cap + j, g -> 2 cap), rho [cap], then the
+// coefficient vectors of direction_coeffs.
+struct GramSmem {
+  double* m;         // [ld * ld]
+  double* rho;       // [cap]
+  double* delta;     // [ld]
+  double* al;        // [cap]
+  int* slot_of;      // [cap]
+  double* glob;      // this CTA's global copy: matrix, then rho
+  int ld;
+  __device__ void set(int r, int c, double v) const { m[(size_t)r * ld + c] = v; glob[(size_t)r * ld + c] = v; }
+  __device__ void set_sym(int r, int c, double v) const { set(r, c, v); set(c, r, v); }
+};
+__device__ __forceinline__ GramSmem gram_smem(const StepArgs& a, int cap, unsigned int rank, double* dyn) {
+  GramSmem G;
+  G.ld = 2 * cap + 1;
+  G.m = dyn; G.rho = G.m + (size_t)G.ld * G.ld; G.delta = G.rho + cap; G.al = G.delta + G.ld;
+  G.slot_of = reinterpret_cast<int*>(G.al + cap);
+  G.glob = gram_of(a, cap, rank);
+  return G;
+}
+
+// Writes the products prod[] (layout of eval_sweep) of the active slots [t0, t0 + ns) -- ring positions BEFORE the
+// push -- into both triangles of the Gram matrix: the row of g always; the rows of the pushed pair when
+// new_slot >= 0, except against the pair it evicts (`evicts`: the ring was full, position 0 is overwritten).
+__device__ void gram_writeback(const GramSmem& G, int cap, const double* prod, int hist_start, int t0, int ns,
+                               int new_slot, bool evicts) {
+  constexpr int NS = LB_GRAM_SLOTS;
+  if ((int)threadIdx.x < 3 * ns) {
+    const int n = (int)threadIdx.x / ns, k = (int)threadIdx.x % ns;
+    const bool skip = (n < 2 && new_slot < 0) || (evicts && t0 + k == 0);     // (that slot now holds the new pair)
+    if (!skip) {
+      const int q = (n == 0) ? new_slot : (n == 1 ? cap + new_slot : 2 * cap);
+      const int j = (hist_start + t0 + k) % cap;
+      G.set_sym(q, j, prod[(n * NS + k) * 2]);
+      G.set_sym(q, cap + j, prod[(n * NS + k) * 2 + 1]);
+    }
+  }
+}
+
+// The coefficients of p = -H g (H0 = gamma I) in the basis (S.., Y.., g), from the Gram matrix in shared memory
+// (complete and visible to the CTA: the caller has synchronised after its last patch).
 struct DirCoef {
   const double* delta;     // [2 hl + 1]: S coefficients, Y coefficients, g coefficient
   const int* slot_of;      // [hl] ring slot of pair t (0 = oldest)
   int hl;
 };
-__device__ DirCoef direction_coeffs(const StepArgs& a, int cap, int hist_len, int hist_start, double gamma,
-                                    const Reducer& r, double* dyn) {
-  const int ld = 2 * cap + 1, hl = hist_len, n = 2 * hl + 1, tid = threadIdx.x;
-  const double* gm = gram_of(a, cap, r.rank);
-  const double* rho_g = gm + (size_t)ld * ld;
-  double* Cm = dyn;                    // [n][n] compact Gram matrix in RING order (0 = oldest pair)
-  double* delta = Cm + n * n;          // [n] coefficients of q, then of r, in the basis (S.., Y.., g)
-  double* al = delta + n;              // [hl]
-  double* rho = al + hl;               // [hl]
-  int* slot_of = reinterpret_cast<int*>(rho + hl);   // [hl]
-  __syncthreads();                     // dyn free
-  for (int e = tid; e < n * n; e += LB_THREADS) {
-    const int rr = e / n, cc = e % n;
-    auto gi = [&](int c) { return c < hl ? (hist_start + c) % cap : (c < 2 * hl ? cap + (hist_start + c - hl) % cap : 2 * cap); };
-    Cm[e] = (hl > 0) ? gm[(size_t)gi(rr) * ld + gi(cc)] : 0.0;
-  }
-  if (tid < hl) { const int sl = (hist_start + tid) % cap; slot_of[tid] = sl; rho[tid] = rho_g[sl]; }
-  __syncthreads();
+__device__ DirCoef direction_coeffs(const GramSmem& G, int cap, int hist_len, int hist_start, double gamma) {
+  const int ld = G.ld, hl = hist_len, n = 2 * hl + 1, tid = threadIdx.x;
+  double* delta = G.delta;
   if (tid < 32 && hl <= 32) {
     // The two-loop recursion [70] on coefficients, as two TRIANGULAR substitutions with lane t owning pair t (ring
     // order, 0 = oldest).  Written out, the first loop's alpha_t = rho_t s_t.q_t with q_t = g - sum_{u>t} alpha_u y_u is
     //     alpha_t / rho_t = s_t.g - sum_{u>t} (s_t.y_u) alpha_u,
     // and the second loop's beta_t = rho_t y_t.r_t with r_t = gamma q_0 + sum_{u<t} c_u s_u, c_u = alpha_u - beta_u, is
     //     beta_t / rho_t = gamma (y_t.g - sum_u (y_t.y_u) alpha_u) + sum_{u<t} (y_t.s_u) c_u:
-    // once alpha_u (c_u) is known every lane folds it into its own right-hand side, so a step of the dependent chain
+    // once alpha_u (c_u) is known every lane folds it into its own right-hand sides, so a step of the dependent chain
     // is one multiply, one shuffle and one FMA instead of a 5-round shuffle reduction through shared memory (9 us of
     // the step at m = 10).  The same terms as the textbook loops, summed pair by pair.
     const int lane = tid;
     const bool mine = lane < hl;
-    const double* rowS = Cm + (size_t)(mine ? lane : 0) * n;            // s_t . (S.., Y.., g)
-    const double* rowY = Cm + (size_t)(mine ? hl + lane : 0) * n;       // y_t . (S.., Y.., g)
-    const double rho_me = mine ? rho[lane] : 0.0;
-    double rhs = mine ? rowS[2 * hl] : 0.0, alpha_me = 0.0;
+    const int my_slot = (hist_start + (mine ? lane : 0)) % cap;
+    const double* rowS = G.m + (size_t)my_slot * ld;                // s_t . (S.., Y.., g), slot space
+    const double* rowY = G.m + (size_t)(cap + my_slot) * ld;        // y_t . (S.., Y.., g)
+    const double rho_me = mine ? G.rho[my_slot] : 0.0;
+    double rhs = mine ? rowS[2 * cap] : 0.0, b = mine ? rowY[2 * cap] : 0.0, alpha_me = 0.0;
+    int su = (hist_start + (hl > 0 ? hl - 1 : 0)) % cap;              // slot of pair u
     for (int u = hl - 1; u >= 0; --u) {                 // newest -> oldest
       const double au = __shfl_sync(0xffffffffu, __dmul_rn(rho_me, rhs), u);
       if (lane == u) alpha_me = au;
-      if (lane < u) rhs = __fma_rn(-rowS[hl + u], au, rhs);
-    }
-    double b = mine ? rowY[2 * hl] : 0.0;
-    for (int u = 0; u < hl; ++u) {
-      const double au = __shfl_sync(0xffffffffu, alpha_me, u);
-      if (mine) b = __fma_rn(-rowY[hl + u], au, b);
+      if (lane < u) rhs = __fma_rn(-rowS[cap + su], au, rhs);
+      if (mine) b = __fma_rn(-rowY[cap + su], au, b);    // (the second loop's alpha sum, folded in as alpha_u appears)
+      su = (su == 0) ? cap - 1 : su - 1;
     }
     double acc = __dmul_rn(gamma, b), c_me = 0.0;
+    su = hist_start % cap;
     for (int u = 0; u < hl; ++u) {                      // oldest -> newest
       const double cu = __shfl_sync(0xffffffffu, __dsub_rn(alpha_me, __dmul_rn(rho_me, acc)), u);
       if (lane == u) c_me = cu;
-      if (mine && lane > u) acc = __fma_rn(rowY[u], cu, acc);
+      if (mine && lane > u) acc = __fma_rn(rowY[su], cu, acc);
+      su = (su + 1 == cap) ? 0 : su + 1;
     }
-    if (mine) { delta[lane] = c_me; delta[hl + lane] = -__dmul_rn(gamma, alpha_me); }
+    if (mine) { delta[lane] = c_me; delta[hl + lane] = -__dmul_rn(gamma, alpha_me); G.slot_of[lane] = my_slot; }
     if (lane == 0) delta[2 * hl] = gamma;
   } else if (tid < 32) {
     // histories longer than a warp: the textbook loops on the coefficient vector
     const int lane = tid;
+    auto gi = [&](int c) { return c < hl ? (hist_start + c) % cap : (c < 2 * hl ? cap + (hist_start + c - hl) % cap : 2 * cap); };
+    for (int j = lane; j < hl; j += 32) G.slot_of[j] = (hist_start + j) % cap;
     for (int j = lane; j < n; j += 32) delta[j] = (j == n - 1) ? 1.0 : 0.0;
     __syncwarp();
     for (int t = hl - 1; t >= 0; --t) {                 // newest -> oldest: alpha_t = rho_t s_t.q ; q -= alpha_t y_t
       double part = 0.0;
-      for (int j = lane; j < n; j += 32) part += delta[j] * Cm[t * n + j];
+      for (int j = lane; j < n; j += 32) part += delta[j] * G.m[(size_t)gi(t) * ld + gi(j)];
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
-      const double alv = rho[t] * part;
-      if (lane == 0) { al[t] = alv; delta[hl + t] = __dsub_rn(delta[hl + t], alv); }
+      const double alv = G.rho[gi(t)] * part;
+      if (lane == 0) { G.al[t] = alv; delta[hl + t] = __dsub_rn(delta[hl + t], alv); }
       __syncwarp();
     }
     for (int j = lane; j < n; j += 32) delta[j] = __dmul_rn(gamma, delta[j]);    // r = gamma q
     __syncwarp();
     for (int t = 0; t < hl; ++t) {                       // oldest -> newest: r += s_t (alpha_t - rho_t y_t.r)
       double part = 0.0;
-      for (int j = lane; j < n; j += 32) part += delta[j] * Cm[(hl + t) * n + j];
+      for (int j = lane; j < n; j += 32) part += delta[j] * G.m[(size_t)gi(hl + t) * ld + gi(j)];
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
-      if (lane == 0) delta[t] = __dadd_rn(delta[t], al[t] - rho[t] * part);
+      if (lane == 0) delta[t] = __dadd_rn(delta[t], G.al[t] - G.rho[gi(t)] * part);
       __syncwarp();
     }
   }
   __syncthreads();
-  return DirCoef{delta, slot_of, hl};
+  return DirCoef{delta, G.slot_of, hl};
 }
 
-// The combination pass fused with the trial point: for every element
+// The combination pass fused with the trial point and, after an accepted step whose pair is kept, with that step's
+// vector writes: for every element
+//     [push]  s = alpha_old p, y = g1 - g  -> ring slot push.slot;   w <- w_try;   g <- g1
 //     p = -(delta_g g + sum_t delta_t s_t + delta_{m+t} y_t),   w_try = w + alpha p  (alpha = 1: a new direction),
 // w32 = fl32(w_try) (S10), the best-so-far copy of the point just evaluated, and ONE exchange for g.p (sum) and the two
-// maxima the candidate-list reuse needs (|change since the last evaluation|, |distance from wref|).  The history
-// loads of an element are issued LB_COMB_SLOTS pairs at a time before any of them is used (a loop of dependent
-// load-FMA pairs ran at one L2 round trip per four pairs: 9 of the step's 36 us at M = 10^4).
+// maxima the candidate-list reuse needs (|change since the last evaluation|, |distance from wref|).  Two elements
+// per thread are in flight, and the history loads of an element are issued LB_COMB_SLOTS pairs at a time before any
+// of them is used (a loop of dependent load-FMA pairs ran at one L2 round trip per four pairs: 9 of the step's 36 us
+// at M = 10^4).  All loads of an element precede its stores; the pushed pair is used from registers.
 constexpr int LB_COMB_SLOTS = 10;
+constexpr int LB_COMB_U = 2;
+struct PushArgs {
+  bool on;                   // this step pushes the pair (alpha_old p, g1 - g) into ring slot `slot`
+  double alpha_old;
+  int slot;
+};
 struct TrialArgs {
   bool improved;             // copy w_eval -> w_best first
   const double* w_eval;      // the point the evaluation just run was taken at
   double alpha;
 };
-__device__ void combine_and_trial(const StepArgs& a, int cap, const DirCoef& dc, const TrialArgs& ta, Reducer& r,
-                                  double* gp_out, double (&mx_out)[2]) {
+__device__ void combine_and_trial(const StepArgs& a, int cap, const DirCoef& dc, const TrialArgs& ta,
+                                  const PushArgs& pu, Reducer& r, double* gp_out, double (&mx_out)[2]) {
   const int M = a.M, stride = a.stride, hl = dc.hl;
-  const double* g = a.vec + (size_t)V_G * stride;
+  double* g = a.vec + (size_t)V_G * stride;
   double* p = a.vec + (size_t)V_P * stride;
-  const double* w = a.vec + (size_t)V_W * stride;
+  double* w = a.vec + (size_t)V_W * stride;
   double* wtry = a.vec + (size_t)V_WTRY * stride;
   double* wbest = a.vec + (size_t)V_WBEST * stride;
-  const double* S = a.vec + (size_t)V_HIST * stride;
-  const double* Y = S + (size_t)cap * stride;
+  const double* gnew = a.vec + (size_t)V_GNEW * stride;
+  double* S = a.vec + (size_t)V_HIST * stride;
+  double* Y = S + (size_t)cap * stride;
   const double dg = dc.delta[2 * hl];
   double red3[3] = {0.0, 0.0, 0.0};      // g.p | max |change since the last evaluation|, max |distance from wref|
-  constexpr int NC = LB_COMB_SLOTS;
-  for (int i = LB_FIRST(r); i < M; i += LB_STEP) {
-    const double gi = g[i], wi = w[i];
-    const double we = ta.improved ? ta.w_eval[i] : 0.0;
-    const float w32_old = a.w32[i], wref = a.wref[i];
-    double acc = dg * gi;
+  constexpr int NC = LB_COMB_SLOTS, U = LB_COMB_U;
+  for (int i0 = LB_FIRST(r); i0 < M; i0 += U * LB_STEP) {
+    double gi[U], wi[U], we[U], sn[U], yn[U], acc[U];
+    float w32_old[U], wref[U];
+    int idx[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const int i = i0 + u * LB_STEP;
+      idx[u] = i < M ? i : i0;                    // past the end: a duplicate of the first element, never stored
+      const int ii = idx[u];
+      we[u] = ta.improved ? ta.w_eval[ii] : 0.0;
+      w32_old[u] = a.w32[ii]; wref[u] = a.wref[ii];
+      if (pu.on) {
+        const double gn = gnew[ii];
+        sn[u] = __dmul_rn(pu.alpha_old, p[ii]); yn[u] = __dsub_rn(gn, g[ii]);
+        gi[u] = gn; wi[u] = wtry[ii];
+      } else {
+        sn[u] = 0.0; yn[u] = 0.0;
+        gi[u] = g[ii]; wi[u] = w[ii];
+      }
+      acc[u] = dg * gi[u];
+    }
     for (int t0 = 0; t0 < hl; t0 += NC) {
-      double sv[NC], yv[NC];
+      double sv[U][NC], yv[U][NC];
 #pragma unroll
       for (int q = 0; q < NC; ++q) {
-        const size_t off = (size_t)dc.slot_of[t0 + q < hl ? t0 + q : t0] * stride + i;     // past the end: a duplicate
-        sv[q] = S[off]; yv[q] = Y[off];
+        const int sl = dc.slot_of[t0 + q < hl ? t0 + q : t0];     // past the end: a duplicate
+        const size_t off = (size_t)sl * stride;
+        const bool is_new = pu.on && sl == pu.slot;
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+          sv[u][q] = S[off + idx[u]]; yv[u][q] = Y[off + idx[u]];
+          if (is_new) { sv[u][q] = sn[u]; yv[u][q] = yn[u]; }     // (what the slot holds in memory is the evicted pair)
+        }
       }
 #pragma unroll
-      for (int q = 0; q < NC; ++q)
-        if (t0 + q < hl) acc = __dadd_rn(acc, __fma_rn(dc.delta[hl + t0 + q], yv[q], __dmul_rn(dc.delta[t0 + q], sv[q])));
+      for (int q = 0; q < NC; ++q) {
+        if (t0 + q < hl) {
+          const double ds = dc.delta[t0 + q], dy = dc.delta[hl + t0 + q];
+#pragma unroll
+          for (int u = 0; u < U; ++u) acc[u] = __dadd_rn(acc[u], __fma_rn(dy, yv[u][q], __dmul_rn(ds, sv[u][q])));
+        }
+      }
     }
-    const double pi = -acc;
-    p[i] = pi;
-    red3[0] += gi * pi;
-    if (ta.improved) wbest[i] = we;        // (w_eval may be w_try: read above, before w_try is rewritten)
-    const double wt = __dadd_rn(wi, __dmul_rn(ta.alpha, pi));
-    wtry[i] = wt;
-    const float wn = (float)wt;
-    red3[1] = fmax(red3[1], fabs((double)wn - (double)w32_old));      // differences of floats: exact in fp64
-    red3[2] = fmax(red3[2], fabs((double)wn - (double)wref));
-    a.w32[i] = wn;
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const int i = i0 + u * LB_STEP;
+      if (i < M) {
+        if (pu.on) {
+          S[(size_t)pu.slot * stride + i] = sn[u]; Y[(size_t)pu.slot * stride + i] = yn[u];
+          w[i] = wi[u]; g[i] = gi[u];
+        }
+        const double pi = -acc[u];
+        p[i] = pi;
+        red3[0] += gi[u] * pi;
+        if (ta.improved) wbest[i] = we[u];
+        const double wt = __dadd_rn(wi[u], __dmul_rn(ta.alpha, pi));
+        wtry[i] = wt;
+        const float wn = (float)wt;
+        red3[1] = fmax(red3[1], fabs((double)wn - (double)w32_old[u]));      // differences of floats: exact in fp64
+        red3[2] = fmax(red3[2], fabs((double)wn - (double)wref[u]));
+        a.w32[i] = wn;
+      }
+    }
   }
   cluster_all_mixed<3, 2>(red3, r);
   *gp_out = red3[0]; mx_out[0] = red3[1]; mx_out[1] = red3[2];
@@ -422,6 +559,8 @@ __global__ void __cluster_dims__(LB_CLUSTER, 1, 1) __launch_bounds__(LB_THREADS)
   __shared__ double s_cbuf[2 * LB_NRED];
   __shared__ double s_tot[LB_NRED];
   __shared__ double s_smin;
+  __shared__ double s_prod[LB_NPROD];      // the sweep's Gram products and scalars (cluster totals)
+  __shared__ double s_scal[LB_NSCAL];
   extern __shared__ double s_dyn[];        // direction_vf: compact Gram matrix, coefficients (sized by the launch)
   cg::cluster_group cluster = cg::this_cluster();
   Reducer red{s_wbuf, s_cbuf, s_tot, 0, cluster.block_rank()};
@@ -435,8 +574,6 @@ __global__ void __cluster_dims__(LB_CLUSTER, 1, 1) __launch_bounds__(LB_THREADS)
   double* wtry = a.vec + (size_t)V_WTRY * stride;
   double* wbest = a.vec + (size_t)V_WBEST * stride;
   double* gnew = a.vec + (size_t)V_GNEW * stride;
-  double* S = a.vec + (size_t)V_HIST * stride;
-  double* Y = S + (size_t)st->hist_cap * stride;
 
   // copy the scalars (the state is rewritten only at the very end, after several cluster barriers)
   const int phase = st->phase;
@@ -449,29 +586,23 @@ __global__ void __cluster_dims__(LB_CLUSTER, 1, 1) __launch_bounds__(LB_THREADS)
   const float cull_delta_old = st->cull_delta;
   const int cull_rebuilds_old = st->cull_rebuilds;
 
+  // the Gram matrix of the history: fetched now, stored to shared memory after the layer sums (whose loads hide the
+  // latency), patched and used after the decision
+  const GramSmem G = gram_smem(a, cap, red.rank, s_dyn);
+  const int hl_old = hist_len, hs_old = hist_start;        // the ring as the sweep sees it (before a push)
+  const bool gram = phase != 0 && hl_old > 0;
+  constexpr int GPRE = 2;
+  const int gram_words = G.ld * G.ld + cap;
+  double gpre[GPRE] = {0.0, 0.0};
+  if (gram && gram_words <= GPRE * LB_THREADS) {
+#pragma unroll
+    for (int k = 0; k < GPRE; ++k) if (tid + k * LB_THREADS < gram_words) gpre[k] = G.glob[tid + k * LB_THREADS];
+  }
+
   // a9 for the loop: g~ = <v, fl32 w> + |P| sum_j min_i C_ij (identity I1), eq. (2.5) error
   const double P = a.voxel_volume;
-  // ONE sweep and ONE exchange for everything that depends only on the evaluation just run and on the state at
-  // entry: <v, fl32 w> and the eq. (2.5) error (a9), the gradient of f at the evaluated point, vol - v (eq. 2.8), and,
-  // speculatively, every inner product the line-search tests and the curvature pair need (s = alpha p, y = g1 - g).
-  // Each sum is accumulated per thread in element order and reduced by the same tree whatever shares the exchange.
-  double red8[8] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};   // <v,w32>, sum v, g1.p, s.y, s.s, y.y, (unused), max err
-  for (int i = LB_FIRST(red); i < M; i += LB_STEP) {
-    const double tv = (double)a.v[i];
-    red8[0] += tv * (double)a.w32[i];
-    const double vi = a.vol_in ? a.vol_in[i] : (a.count64 ? (double)a.count64[i] : (double)a.count[i]) * P;
-    red8[7] = fmax(red8[7], fabs(vi - tv) / tv);
-    const double gn = vi - tv;                                  // m_i |P| - v_i
-    gnew[i] = gn;
-    red8[1] += tv;
-    if (phase != 0) {
-      const double pi = p[i];
-      const double si = __dmul_rn(alpha, pi);
-      const double yi = __dsub_rn(gn, g[i]);
-      red8[2] += gn * pi; red8[3] += si * yi; red8[4] += si * si; red8[5] += yi * yi;
-    }
-  }
-  // sum of the minima, two-level (apd_internal.cuh): layer sums by one warp each, in a fixed order ...
+  // sum of the minima, two-level (apd_internal.cuh): layer sums by one warp each, in a fixed order (the sweep's
+  // cluster barrier publishes them to every CTA) ...
   if (!a.layer_in) {
     for (int L = (int)red.rank * (LB_THREADS / 32) + (tid >> 5); L < a.lm.n_layers; L += LB_CLUSTER * (LB_THREADS / 32)) {
       const int first = L * a.lm.per_layer, cnt = min(a.lm.per_layer, a.lm.n_partials - first);
@@ -479,7 +610,20 @@ __global__ void __cluster_dims__(LB_CLUSTER, 1, 1) __launch_bounds__(LB_THREADS)
       if ((tid & 31) == 0) a.layer_buf[L] = ls;
     }
   }
-  cluster_all_mixed<8, 1>(red8, red);      // (its cluster barrier also publishes the layer sums to every CTA)
+  if (gram) {
+    if (gram_words <= GPRE * LB_THREADS) {
+#pragma unroll
+      for (int k = 0; k < GPRE; ++k) if (tid + k * LB_THREADS < gram_words) G.m[tid + k * LB_THREADS] = gpre[k];
+    } else {
+      for (int e = tid; e < gram_words; e += LB_THREADS) G.m[e] = G.glob[e];
+    }
+  }
+  if (gram) eval_sweep<true>(a, phase, alpha, cap, hl_old, hs_old, red);
+  else      eval_sweep<false>(a, phase, alpha, cap, hl_old, hs_old, red);
+  // the totals sit in red.tot until the next exchange: keep the products and the scalars in shared memory of their
+  // own, where the write-back can index them with run-time slot numbers
+  if (gram && tid < LB_NPROD) s_prod[tid] = red.tot[tid];
+  if (tid < LB_NSCAL) s_scal[tid] = gram ? red.tot[LB_NPROD_PAD + tid] : red.tot[tid];
   // ... then the layers in ascending order: the same bits in every CTA, and in a slab-sharded solve
   {
     const double* lsrc = a.layer_in ? a.layer_in : a.layer_buf;
@@ -497,22 +641,23 @@ __global__ void __cluster_dims__(LB_CLUSTER, 1, 1) __launch_bounds__(LB_THREADS)
     __syncthreads();
   }
   const double smin = s_smin;
-  const double err1 = red8[7];
-  const double dual1 = red8[0] + P * smin, f1 = -dual1;
+  const double err1 = s_scal[SC_ERR];
+  const double dual1 = s_scal[SC_VW] + P * smin, f1 = -dual1;
 
   evals += 1;
   if (lead && tid == 0 && evals <= a.hist_cap) { a.hist[2 * (evals - 1)] = -f1; a.hist[2 * (evals - 1) + 1] = err1; }
   const double* w_eval = (phase == 0) ? w : wtry;
   const bool improved = err1 < best_err;      // the best-so-far copy is made in the last sweep of this call
   if (improved) { best_err = err1; best_dual = -f1; }
-  const double sums[5] = {red8[1], red8[2], red8[3], red8[4], red8[5]};
-  const double vsum = sums[0], g1p = sums[1], sy = sums[2], ss = sums[3], yy = sums[4];
+  const double vsum = s_scal[SC_V], g1p = s_scal[SC_G1P], sy = s_scal[SC_SY], ss = s_scal[SC_SS], yy = s_scal[SC_YY];
 
   int finish = 0;          // 1: OK at w_eval, 2: NOT_CONVERGED at best, 3: bad target volumes
   bool need_direction = false;
   double mx[2] = {0.0, 0.0};   // max |change of fl32 w since the last evaluation|, max |distance from wref|
-  int new_slot = -1;       // ring slot a curvature pair was pushed into by this call, else -1
-  PushArgs push{};
+  int new_slot = -1;       // ring slot a curvature pair is pushed into by this call, else -1
+  bool evicts = false;     // ... and that slot held the oldest pair (the ring was full)
+  bool accepted = false;
+  const double alpha_eval = alpha;     // the step length the evaluation just run was taken with
   if (phase == 0) {
     // cost scale for the list-reuse slack: mean over the voxels of min_i C_ij = (g~ - <v, w>) / |Omega|  (identity I1)
     const double scale = fabs(P * smin) / domain_volume;
@@ -532,7 +677,6 @@ __global__ void __cluster_dims__(LB_CLUSTER, 1, 1) __launch_bounds__(LB_THREADS)
   } else {
     if (err1 <= eps) { finish = 1; iters += 1; }
     else {
-      bool accepted = false;
       const double armijo_rhs = __dadd_rn(f, __dmul_rn(__dmul_rn(1e-4, alpha), gp));
       if (f1 > armijo_rhs) hi = alpha;
       else if (g1p < __dmul_rn(0.9, gp)) lo = alpha;
@@ -551,27 +695,21 @@ __global__ void __cluster_dims__(LB_CLUSTER, 1, 1) __launch_bounds__(LB_THREADS)
         // s = alpha p, yv = g1 - g  -> curvature pair in the next ring slot; when the ring is full that slot is
         // the oldest pair, which is dropped only if the new one is kept
         const int slot = (hist_len < cap) ? (hist_start + hist_len) % cap : hist_start;
-        double* s_new = S + (size_t)slot * stride;
-        double* y_new = Y + (size_t)slot * stride;
         const bool keep = sy > 1e-12 * sqrt(ss) * sqrt(yy);
-        if (keep) {
-          if (tid == 0) gram_of(a, cap, red.rank)[(size_t)(2 * cap + 1) * (2 * cap + 1) + slot] = 1.0 / sy;   // rho
-          new_slot = slot;
-          if (hist_len < cap) hist_len += 1; else hist_start = (hist_start + 1) % cap;
-          gamma = sy / yy;
-        }
         f = f1;
         iters += 1;
         if (iters >= max_iters || evals >= max_evals) finish = 2;
         else need_direction = true;
-        push.alpha = alpha; push.p = p; push.gnew = gnew; push.wtry = wtry; push.g = g; push.w = w;
-        push.s_new = s_new; push.y_new = y_new; push.slot = slot;
-        if (!(keep && need_direction)) {      // (else these writes ride on the Gram pass below)
-          for (int i = LB_FIRST(red); i < M; i += LB_STEP) {
-            const double gn = gnew[i];
-            if (keep) { s_new[i] = __dmul_rn(alpha, p[i]); y_new[i] = __dsub_rn(gn, g[i]); }
-            w[i] = wtry[i]; g[i] = gn;
-          }
+        if (keep && need_direction) {
+          // the pair's vectors, w <- w_try and g <- g1 are written by the combination pass below
+          if (tid == 0) { const double rh = 1.0 / sy; G.rho[slot] = rh; G.glob[(size_t)G.ld * G.ld + slot] = rh; }
+          new_slot = slot;
+          evicts = !(hist_len < cap);
+          if (hist_len < cap) hist_len += 1; else hist_start = (hist_start + 1) % cap;
+          gamma = sy / yy;
+        } else {
+          // (pair not kept, or the limits end the solve here: no history update is needed any more)
+          for (int i = LB_FIRST(red); i < M; i += LB_STEP) { w[i] = wtry[i]; g[i] = gnew[i]; }
         }
       }
     }
@@ -579,26 +717,35 @@ __global__ void __cluster_dims__(LB_CLUSTER, 1, 1) __launch_bounds__(LB_THREADS)
 
   if (need_direction) {
     if (hist_len > 0) {
-      // refresh the Gram rows that changed: those of the pushed pair (if any) and the row of the new gradient
-      if (new_slot >= 0) {      // (an accepted step whose pair is kept: its vector writes happen in this pass)
-        const double* nv[3] = {S + (size_t)new_slot * stride, Y + (size_t)new_slot * stride, g};
-        const int nidx[3] = {new_slot, cap + new_slot, 2 * cap};
-        gram_rows<3, true>(a, cap, hist_len, hist_start, nv, nidx, push, red);
-      } else {
-        const double* nv[1] = {g};
-        const int nidx[1] = {2 * cap};
-        gram_rows<1, false>(a, cap, hist_len, hist_start, nv, nidx, push, red);
+      // refresh the Gram rows that changed -- those of the pushed pair (if any) and the row of the new gradient --
+      // from the products the sweep formed against the ring as it was
+      gram_writeback(G, cap, s_prod, hs_old, 0, min(LB_GRAM_SLOTS, hl_old), new_slot, evicts);
+      for (int t0 = LB_GRAM_SLOTS; t0 < hl_old; t0 += LB_GRAM_SLOTS) {      // histories longer than one pass
+        const int ns = min(LB_GRAM_SLOTS, hl_old - t0);
+        gram_products(a, alpha_eval, cap, hs_old, t0, ns, red);
+        gram_writeback(G, cap, red.tot, hs_old, t0, ns, new_slot, evicts);
       }
+      if (tid == 0) {
+        const int gq = 2 * cap;
+        G.set(gq, gq, s_scal[SC_G1G1]);
+        if (new_slot >= 0) {
+          const int sq = new_slot, yq = cap + new_slot;
+          G.set(sq, sq, ss); G.set(yq, yq, yy); G.set_sym(sq, yq, sy);
+          G.set_sym(gq, sq, s_scal[SC_G1S]); G.set_sym(gq, yq, s_scal[SC_G1Y]);
+        }
+      }
+      __syncthreads();      // the patches are visible to the warp that runs the recursion
     }
     // the new direction and, in the same pass, the first trial point along it (alpha = 1)
     alpha = 1.0; lo = 0.0; hi = INFINITY; trial = 0;
-    DirCoef dc = direction_coeffs(a, cap, hist_len, hist_start, gamma, red, s_dyn);
-    combine_and_trial(a, cap, dc, TrialArgs{improved, w_eval, alpha}, red, &gp, mx);
+    DirCoef dc = direction_coeffs(G, cap, hist_len, hist_start, gamma);
+    combine_and_trial(a, cap, dc, TrialArgs{improved, w_eval, alpha}, PushArgs{new_slot >= 0, alpha_eval, new_slot}, red,
+                      &gp, mx);
     if (gp >= 0.0) {    // safeguard: not a descent direction -> steepest descent scaled by gamma
       hist_len = 0; hist_start = 0;
       const double mx0 = mx[0];
-      dc = direction_coeffs(a, cap, 0, 0, gamma, red, s_dyn);
-      combine_and_trial(a, cap, dc, TrialArgs{false, w_eval, alpha}, red, &gp, mx);     // (the best-so-far copy is made)
+      dc = direction_coeffs(G, cap, 0, 0, gamma);
+      combine_and_trial(a, cap, dc, TrialArgs{false, w_eval, alpha}, PushArgs{false, 0.0, -1}, red, &gp, mx);
       mx[0] += mx0;     // w32 was rewritten by the first pass: |change since the last evaluation| <= the sum (it only
                         // sizes the slack of a rebuilt candidate list; any value is exact)
     }
