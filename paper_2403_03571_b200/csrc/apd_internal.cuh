@@ -110,6 +110,7 @@ struct Workspace {
   struct SolveState* sstate = nullptr;  // device scalars
   double* svec = nullptr;               // device fp64 vectors: w, g, p, w_try, w_best, g_new, q, S[m], Y[m]
   int svec_hist = 0;                    // history capacity svec was sized for
+  int lb_cluster = 0;                   // CTAs of lbfgs_step_kernel's cluster on this device (0: not chosen yet)
   double* gram = nullptr;               // [(2 svec_hist + 1)^2] Gram matrix of the L-BFGS basis
   float* w32 = nullptr;                 // [max_seeds] fl32(w) the next evaluation uses
   float* wref = nullptr;                // [max_seeds] weights the current candidate lists were built at

@@ -11,7 +11,7 @@
 //   * curvature pair kept iff s.y > 1e-12 |s||y|; then gamma = s.y / y.y
 //   * line-search failure: clear the history and retry with p = -gamma g; with an empty history
 //     NOT_CONVERGED; NOT_CONVERGED returns the evaluated point with the smallest error.
-// The whole state machine is ONE kernel (lbfgs_step_kernel, a cluster of LB_CLUSTER CTAs) that runs after each
+// The whole state machine is ONE kernel (lbfgs_step_kernel, one cluster of 8 or 16 CTAs) that runs after each
 // evaluation on the same stream; the host only reads the mapped SolveReport.done word.  The same loop serves voxel
 // grids (apd_solve) and user-supplied point sets (apd_solve_points).
 #include "apd_internal.cuh"
@@ -25,7 +25,13 @@ namespace cg = cooperative_groups;
 namespace apd {
 
 constexpr int LB_THREADS = 256;
-constexpr int LB_CLUSTER = 8;      // CTAs (SMs) of the step kernel's thread-block cluster
+// CTAs (SMs) of the step kernel's thread-block cluster: 8 (the portable maximum), or 16 for M >= LB_CLUSTER_MAX_MIN_M
+// where the device can co-schedule such a cluster (a non-portable size: B200 can; lb_cluster_size asks once per
+// context).  The sweeps over the L-BFGS vectors (3.6 MB per step at M = 10^4, m = 10) go with 1 / CTAs, a cluster
+// barrier costs more on 16 CTAs.  Measured step time, 8 vs 16 CTAs: M = 10^4 21.4 vs 18.7 us, M = 2 10^4 37.0 vs 27.0,
+// M = 5000 13.3 vs 14.3, M = 1000 12.7 vs 13.7.
+constexpr int LB_CLUSTER_MAX = 16, LB_CLUSTER_PORTABLE = 8;
+constexpr int LB_CLUSTER_MAX_MIN_M = 8192;
 constexpr int LB_MAX_HIST = 64;
 constexpr int LB_MAX_TRIALS = 30;
 
@@ -61,7 +67,7 @@ struct StepArgs {
   double* hist;        // [2 * hist_cap] (dual, max_rel_err) of every evaluation, in order
   int hist_cap;
   float* wref;         // weights the candidate lists were built at (culling only)
-  double* gram;        // [LB_CLUSTER] copies of { (2 hist_cap + 1)^2 Gram matrix, hist_cap rho }, see direction_vf
+  double* gram;        // [LB_CLUSTER_MAX] copies of { (2 hist_cap + 1)^2 Gram matrix, hist_cap rho }, see GramSmem
 };
 
 constexpr double CULL_DELTA_FACTOR = 4.0;   // slack of a rebuilt list = this x the last change of the weights ...
@@ -69,9 +75,9 @@ constexpr double CULL_CAP_FACTOR = 0.5;     // ... but at most this x the mean m
                                             // slack would lengthen every list by more than it saves in rebuilds)
 
 // ---- reductions over the CLUSTER ------------------------------------------------------------------------------
-// The step kernel is ONE thread-block cluster of LB_CLUSTER CTAs (one per SM): a single CTA cannot keep enough loads
+// The step kernel is ONE thread-block cluster of nranks = 8 or 16 CTAs (one per SM): a single CTA cannot keep enough loads
 // in flight to stream the L-BFGS vectors (measured: its sweeps ran at pure L2 latency), eight can.  Element i of
-// every length-M vector is owned by one thread of one CTA in every sweep (i = tid + LB_THREADS (rank + LB_CLUSTER k)),
+// every length-M vector is owned by one thread of one CTA in every sweep (i = tid + LB_THREADS (rank + nranks k)),
 // so vectors need no synchronisation; scalars come from reductions that return the SAME value, bit for bit, to every
 // thread of every CTA (lanes by shuffle tree, warps in order, CTAs in rank order), which keeps the control flow
 // uniform over the whole cluster.  Cluster partials are exchanged through distributed shared memory; two buffers
@@ -88,7 +94,7 @@ struct Reducer {
   double* cbuf;        // [2][LB_NRED]                 CTA totals, read by the other CTAs of the cluster
   double* tot;         // [LB_NRED]                    cluster totals, for this CTA's threads
   int flip;
-  unsigned int rank;
+  unsigned int rank, nranks;     // this CTA's rank in the cluster, CTAs in the cluster
 };
 
 // One halving step of the TRANSPOSED warp reduction: lanes whose BIT is set keep the upper HALF of the values, the
@@ -162,10 +168,18 @@ __device__ __forceinline__ void cluster_all_mixed(double (&v)[N], Reducer& r) {
   if (threadIdx.x < N) {
     const bool MAX = (int)threadIdx.x >= N - NMAX;
     double t = cluster.map_shared_rank(mine, 0)[threadIdx.x];
+    if (r.nranks == LB_CLUSTER_MAX) {         // (both sizes unrolled: the remote reads are issued together)
 #pragma unroll
-    for (int c = 1; c < LB_CLUSTER; ++c) {
-      const double u = cluster.map_shared_rank(mine, c)[threadIdx.x];
-      t = MAX ? fmax(t, u) : t + u;
+      for (int c = 1; c < LB_CLUSTER_MAX; ++c) {
+        const double u = cluster.map_shared_rank(mine, c)[threadIdx.x];
+        t = MAX ? fmax(t, u) : t + u;
+      }
+    } else {
+#pragma unroll
+      for (int c = 1; c < LB_CLUSTER_PORTABLE; ++c) {
+        const double u = cluster.map_shared_rank(mine, c)[threadIdx.x];
+        t = MAX ? fmax(t, u) : t + u;
+      }
     }
     r.tot[threadIdx.x] = t;
   }
@@ -189,16 +203,17 @@ __device__ __forceinline__ double cluster_allmax(double x, Reducer& r) {
   return v[0];
 }
 
-// element loop of this thread: for (int i = LB_FIRST(r); i < M; i += LB_STEP)
+// element loop of this thread: for (int i = LB_FIRST(r); i < M; i += LB_STEP_R)
 #define LB_FIRST(r) ((int)threadIdx.x + LB_THREADS * (int)(r).rank)
-constexpr int LB_STEP = LB_THREADS * LB_CLUSTER;
+#define LB_STEP_OF(r) (LB_THREADS * (int)(r).nranks)
 
 // ---- the L-BFGS direction in "vector-free" form ---------------------------------------------------------------
 // The two-loop recursion of Liu & Nocedal [70] only ever forms linear combinations of the 2m+1 basis vectors
 // b = (s_0..s_{m-1}, y_0..y_{m-1}, g) and inner products with them, so it can be run on the COEFFICIENTS of q in
 // that basis given the Gram matrix B = b^T b: the same algorithm, the same result up to fp64 rounding, but the 2m
-// dependent passes over the length-M vectors (each a latency-bound reduction) become m/2 Gram passes when a pair is
-// pushed plus ONE combination pass.  Every CTA keeps its own copy of the Gram matrix and of rho in global memory
+// dependent passes over the length-M vectors (each a latency-bound reduction) become the Gram products, which ride on
+// the evaluation sweep (eval_sweep), plus ONE combination pass (combine_and_trial): an accepted step is two passes
+// over the vectors and two exchanges.  Every CTA keeps its own copy of the Gram matrix and of rho in global memory
 // (all copies are identical, no cross-CTA visibility to arrange), in SLOT space (ring slots of S and Y):
 //   index of S slot j = j,  of Y slot j = cap + j,  of g = 2 cap;  leading dimension ld = 2 cap + 1;
 //   a copy is ld*ld doubles of Gram matrix followed by cap doubles of rho.
@@ -229,13 +244,14 @@ __device__ void eval_sweep(const StepArgs& a, int phase, double alpha, int cap, 
   const double* S = a.vec + (size_t)V_HIST * stride;
   const double* Y = S + (size_t)cap * stride;
   constexpr int NS = LB_GRAM_SLOTS;
+  const int LB_STEP_R = LB_STEP_OF(r);
   size_t soff[NS];
 #pragma unroll
   for (int q = 0; q < NS; ++q) soff[q] = (size_t)((hist_start + (q < hist_len ? q : 0)) % cap) * stride;   // inactive: a duplicate
 #pragma unroll
   for (int n = 0; n < LB_NRED; ++n) out[n] = 0.0;
   double* sc = out + LB_NPROD_PAD;
-  for (int i = LB_FIRST(r); i < M; i += LB_STEP) {
+  for (int i = LB_FIRST(r); i < M; i += LB_STEP_R) {
     const double tv = (double)a.v[i];
     const double w32 = (double)a.w32[i];
     const double vi = a.vol_in ? a.vol_in[i] : (a.count64 ? (double)a.count64[i] : (double)a.count[i]) * P;
@@ -286,13 +302,14 @@ __device__ void gram_products(const StepArgs& a, double alpha, int cap, int hist
   const double* S = a.vec + (size_t)V_HIST * stride;
   const double* Y = S + (size_t)cap * stride;
   constexpr int NS = LB_GRAM_SLOTS;
+  const int LB_STEP_R = LB_STEP_OF(r);
   size_t soff[NS];
 #pragma unroll
   for (int q = 0; q < NS; ++q) soff[q] = (size_t)((hist_start + t0 + (q < ns ? q : 0)) % cap) * stride;
   double acc[LB_NPROD_PAD];
 #pragma unroll
   for (int n = 0; n < LB_NPROD_PAD; ++n) acc[n] = 0.0;
-  for (int i = LB_FIRST(r); i < M; i += LB_STEP) {
+  for (int i = LB_FIRST(r); i < M; i += LB_STEP_R) {
     const double gn = gnew[i];
     const double x[3] = {__dmul_rn(alpha, p[i]), __dsub_rn(gn, g[i]), gn};
     double sv[NS], yv[NS];
@@ -460,13 +477,14 @@ __device__ void combine_and_trial(const StepArgs& a, int cap, const DirCoef& dc,
   const double dg = dc.delta[2 * hl];
   double red3[3] = {0.0, 0.0, 0.0};      // g.p | max |change since the last evaluation|, max |distance from wref|
   constexpr int NC = LB_COMB_SLOTS, U = LB_COMB_U;
-  for (int i0 = LB_FIRST(r); i0 < M; i0 += U * LB_STEP) {
+  const int LB_STEP_R = LB_STEP_OF(r);
+  for (int i0 = LB_FIRST(r); i0 < M; i0 += U * LB_STEP_R) {
     double gi[U], wi[U], we[U], sn[U], yn[U], acc[U];
     float w32_old[U], wref[U];
     int idx[U];
 #pragma unroll
     for (int u = 0; u < U; ++u) {
-      const int i = i0 + u * LB_STEP;
+      const int i = i0 + u * LB_STEP_R;
       idx[u] = i < M ? i : i0;                    // past the end: a duplicate of the first element, never stored
       const int ii = idx[u];
       we[u] = ta.improved ? ta.w_eval[ii] : 0.0;
@@ -505,7 +523,7 @@ __device__ void combine_and_trial(const StepArgs& a, int cap, const DirCoef& dc,
     }
 #pragma unroll
     for (int u = 0; u < U; ++u) {
-      const int i = i0 + u * LB_STEP;
+      const int i = i0 + u * LB_STEP_R;
       if (i < M) {
         if (pu.on) {
           S[(size_t)pu.slot * stride + i] = sn[u]; Y[(size_t)pu.slot * stride + i] = yn[u];
@@ -551,19 +569,20 @@ __global__ void solve_init_kernel(StepArgs a, const float* w_init, int hist_cap,
   }
 }
 
-// Runs after every evaluation, as one cluster of LB_CLUSTER CTAs.  Control flow is uniform over the cluster: every
+// Runs after every evaluation, as one cluster of 8 or 16 CTAs.  Control flow is uniform over the cluster: every
 // decision is taken on values all threads hold identically (cluster reductions, state scalars read at entry).
 // Only CTA 0 writes the state scalars, the history trace and the host report.
-__global__ void __cluster_dims__(LB_CLUSTER, 1, 1) __launch_bounds__(LB_THREADS) lbfgs_step_kernel(StepArgs a) {
+__global__ void __launch_bounds__(LB_THREADS) lbfgs_step_kernel(StepArgs a) {
   __shared__ double s_wbuf[(LB_THREADS / 32) * LB_NRED];
   __shared__ double s_cbuf[2 * LB_NRED];
   __shared__ double s_tot[LB_NRED];
   __shared__ double s_smin;
   __shared__ double s_prod[LB_NPROD];      // the sweep's Gram products and scalars (cluster totals)
   __shared__ double s_scal[LB_NSCAL];
-  extern __shared__ double s_dyn[];        // direction_vf: compact Gram matrix, coefficients (sized by the launch)
+  extern __shared__ double s_dyn[];        // GramSmem: Gram matrix, rho, coefficient vectors (sized by the launch)
   cg::cluster_group cluster = cg::this_cluster();
-  Reducer red{s_wbuf, s_cbuf, s_tot, 0, cluster.block_rank()};
+  Reducer red{s_wbuf, s_cbuf, s_tot, 0, cluster.block_rank(), cluster.num_blocks()};
+  const int LB_STEP_R = LB_STEP_OF(red);
   SolveState* st = a.st;
   if (st->done) return;                    // uniform: written by the previous launch
   const bool lead = red.rank == 0;
@@ -604,7 +623,7 @@ __global__ void __cluster_dims__(LB_CLUSTER, 1, 1) __launch_bounds__(LB_THREADS)
   // sum of the minima, two-level (apd_internal.cuh): layer sums by one warp each, in a fixed order (the sweep's
   // cluster barrier publishes them to every CTA) ...
   if (!a.layer_in) {
-    for (int L = (int)red.rank * (LB_THREADS / 32) + (tid >> 5); L < a.lm.n_layers; L += LB_CLUSTER * (LB_THREADS / 32)) {
+    for (int L = (int)red.rank * (LB_THREADS / 32) + (tid >> 5); L < a.lm.n_layers; L += (int)red.nranks * (LB_THREADS / 32)) {
       const int first = L * a.lm.per_layer, cnt = min(a.lm.per_layer, a.lm.n_partials - first);
       const double ls = warp_ordered_sum(a.dual_partial + first, cnt);
       if ((tid & 31) == 0) a.layer_buf[L] = ls;
@@ -665,13 +684,13 @@ __global__ void __cluster_dims__(LB_CLUSTER, 1, 1) __launch_bounds__(LB_THREADS)
     // target volumes: v_i > 0 and sum v_i = |Omega| -- with sum v != |Omega| the dual
     // is unbounded along (1,..,1); fp32 inputs normalised in fp64 meet 1e-6 with two orders to spare
     double badv = 0.0;
-    for (int i = LB_FIRST(red); i < M; i += LB_STEP) if (!((double)a.v[i] > 0.0)) badv = 1.0;
+    for (int i = LB_FIRST(red); i < M; i += LB_STEP_R) if (!((double)a.v[i] > 0.0)) badv = 1.0;
     badv = cluster_allmax(badv, red);
     if (badv != 0.0 || !(fabs(vsum - domain_volume) <= 1e-6 * domain_volume)) finish = 3;
     else if (err1 <= eps) finish = 1;
     else {
       f = f1;
-      for (int i = LB_FIRST(red); i < M; i += LB_STEP) g[i] = gnew[i];
+      for (int i = LB_FIRST(red); i < M; i += LB_STEP_R) g[i] = gnew[i];
       need_direction = true;
     }
   } else {
@@ -709,7 +728,7 @@ __global__ void __cluster_dims__(LB_CLUSTER, 1, 1) __launch_bounds__(LB_THREADS)
           gamma = sy / yy;
         } else {
           // (pair not kept, or the limits end the solve here: no history update is needed any more)
-          for (int i = LB_FIRST(red); i < M; i += LB_STEP) { w[i] = wtry[i]; g[i] = gnew[i]; }
+          for (int i = LB_FIRST(red); i < M; i += LB_STEP_R) { w[i] = wtry[i]; g[i] = gnew[i]; }
         }
       }
     }
@@ -756,7 +775,7 @@ __global__ void __cluster_dims__(LB_CLUSTER, 1, 1) __launch_bounds__(LB_THREADS)
   if (finish == 0) {
     if (!need_direction) {
       // next trial point w + alpha p of the line search, rounded to fp32 for the evaluation (S10)
-      for (int i = LB_FIRST(red); i < M; i += LB_STEP) {
+      for (int i = LB_FIRST(red); i < M; i += LB_STEP_R) {
         if (improved) wbest[i] = w_eval[i];      // best-so-far copy of the point just evaluated (before wtry is rewritten)
         const double wt = __dadd_rn(w[i], __dmul_rn(alpha, p[i]));
         wtry[i] = wt;
@@ -772,12 +791,12 @@ __global__ void __cluster_dims__(LB_CLUSTER, 1, 1) __launch_bounds__(LB_THREADS)
     if (cull_rebuild) {
       // the next evaluation rebuilds its candidate lists at the new weights, valid within delta of them
       cull_delta = fminf((float)(CULL_DELTA_FACTOR * mx[0]), cull_cap);
-      for (int i = LB_FIRST(red); i < M; i += LB_STEP) a.wref[i] = a.w32[i];
+      for (int i = LB_FIRST(red); i < M; i += LB_STEP_R) a.wref[i] = a.w32[i];
     }
   } else if (finish == 1) {
-    if (phase != 0) for (int i = LB_FIRST(red); i < M; i += LB_STEP) w[i] = wtry[i];
+    if (phase != 0) for (int i = LB_FIRST(red); i < M; i += LB_STEP_R) w[i] = wtry[i];
   } else if (finish == 2) {
-    for (int i = LB_FIRST(red); i < M; i += LB_STEP) {
+    for (int i = LB_FIRST(red); i < M; i += LB_STEP_R) {
       const double wb = improved ? w_eval[i] : wbest[i];
       wbest[i] = wb; w[i] = wb; a.w32[i] = (float)wb;
     }
@@ -835,9 +854,30 @@ int apd::ensure_solve_state(apd_ctx* ctx, int hist) {
     if (ws.svec) { LB_TRY(cudaDeviceSynchronize()); LB_TRY(cudaFree(ws.svec)); ws.svec = nullptr; }
     LB_TRY(cudaMalloc(&ws.svec, (size_t)(V_HIST + 2 * hist) * ms * sizeof(double)));
     cudaFree(ws.gram); ws.gram = nullptr;
-    LB_TRY(cudaMalloc(&ws.gram, (size_t)LB_CLUSTER * ((size_t)(2 * hist + 1) * (2 * hist + 1) + hist) * sizeof(double)));
+    LB_TRY(cudaMalloc(&ws.gram, (size_t)LB_CLUSTER_MAX * ((size_t)(2 * hist + 1) * (2 * hist + 1) + hist) * sizeof(double)));
     ws.svec_hist = hist;
   }
+  return APD_OK;
+}
+
+// The step kernel's cluster size on this context's device: LB_CLUSTER_MAX if the device can hold one such cluster of
+// lbfgs_step_kernel (a non-portable size, opted into here), else LB_CLUSTER_PORTABLE.
+static int lb_cluster_size(apd_ctx* ctx, size_t dyn_bytes, int* out) {
+  *out = LB_CLUSTER_PORTABLE;
+  if (cudaFuncSetAttribute(lbfgs_step_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) != cudaSuccess) {
+    cudaGetLastError();
+    return APD_OK;
+  }
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = LB_CLUSTER_MAX; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(LB_CLUSTER_MAX); cfg.blockDim = dim3(LB_THREADS); cfg.dynamicSmemBytes = dyn_bytes;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  int n = 0;
+  if (cudaOccupancyMaxActiveClusters(&n, lbfgs_step_kernel, &cfg) == cudaSuccess && n >= 1) *out = LB_CLUSTER_MAX;
+  else cudaGetLastError();
+  (void)ctx;
   return APD_OK;
 }
 
@@ -868,11 +908,22 @@ static int solve_common(apd_ctx* ctx, const char* who, int dim, int32_t M, const
                                                     gamma0, domain);
   LB_TRY(cudaGetLastError());
 
-  // dynamic shared memory of the step kernel: compact Gram matrix + coefficient vectors of direction_vf
+  // dynamic shared memory of the step kernel: Gram matrix, rho and the coefficient vectors (GramSmem)
   const size_t nb = 2 * (size_t)o.lbfgs_history + 1;
   const size_t dyn_bytes = (nb * nb + nb + 2 * (size_t)o.lbfgs_history) * sizeof(double) + (size_t)o.lbfgs_history * sizeof(int);
   if (dyn_bytes > 32 * 1024)
     LB_TRY(cudaFuncSetAttribute(lbfgs_step_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn_bytes));
+  if (ws.lb_cluster == 0) {
+    const int rc = lb_cluster_size(ctx, dyn_bytes, &ws.lb_cluster);
+    if (rc != APD_OK) return rc;
+  }
+  cudaLaunchAttribute step_attr[1];
+  step_attr[0].id = cudaLaunchAttributeClusterDimension;
+  const unsigned n_cta = (ws.lb_cluster == LB_CLUSTER_MAX && M >= LB_CLUSTER_MAX_MIN_M) ? LB_CLUSTER_MAX : LB_CLUSTER_PORTABLE;
+  step_attr[0].val.clusterDim.x = n_cta; step_attr[0].val.clusterDim.y = 1; step_attr[0].val.clusterDim.z = 1;
+  cudaLaunchConfig_t step_cfg = {};
+  step_cfg.gridDim = dim3(n_cta); step_cfg.blockDim = dim3(LB_THREADS);
+  step_cfg.dynamicSmemBytes = dyn_bytes; step_cfg.stream = st; step_cfg.attrs = step_attr; step_cfg.numAttrs = 1;
   const int* done_flag = &ws.sstate->done;
   long long enq = 0;
   const long long hard_cap = (long long)max_evals + 64;
@@ -880,8 +931,7 @@ static int solve_common(apd_ctx* ctx, const char* who, int dim, int32_t M, const
     int rc = hooks.loop_eval(done_flag);
     if (rc != APD_OK) return rc;
     if (!sa.layer_in) { sa.dual_partial = ws.dual_partial; sa.layer_buf = ws.layer_buf; }   // (re)allocated by the first evaluation
-    lbfgs_step_kernel<<<LB_CLUSTER, LB_THREADS, dyn_bytes, st>>>(sa);
-    LB_TRY(cudaGetLastError());
+    LB_TRY(cudaLaunchKernelEx(&step_cfg, lbfgs_step_kernel, sa));
     LB_TRY(cudaEventRecord(ws.sev[enq & 1], st));
     if (enq >= 1) {
       // the convergence check: wait for the PREVIOUS evaluation's step while this one runs;
