@@ -33,7 +33,7 @@ static void free_ws(Workspace& ws) {
   cudaFree(ws.lloyd_buf); cudaFree(ws.pt_acc); cudaFree(ws.qfix); cudaFree(ws.rec); cudaFree(ws.brick_list); cudaFree(ws.brick_count); cudaFree(ws.super_list);
   cudaFree(ws.super_count); cudaFree(ws.pairs_ctr);
   cudaFree(ws.seeds); cudaFree(ws.count); cudaFree(ws.idxsum); cudaFree(ws.dual_partial); cudaFree(ws.layer_buf);
-  cudaFree(ws.sstate); cudaFree(ws.svec); cudaFree(ws.gram); cudaFree(ws.w32); cudaFree(ws.wref); cudaFree(ws.e_vol); cudaFree(ws.e_scal); cudaFree(ws.hist);
+  cudaFree(ws.sstate); cudaFree(ws.svec); cudaFree(ws.gram); cudaFree(ws.w32); cudaFree(ws.wref); cudaFree(ws.wref_s); cudaFree(ws.e_vol); cudaFree(ws.e_scal); cudaFree(ws.hist);
   for (int i = 0; i < Workspace::HOST_SLOTS; ++i) cudaFree(ws.host_buf[i]);
   if (ws.report) cudaFreeHost(ws.report);
   for (int i = 0; i < 2; ++i) if (ws.sev[i]) cudaEventDestroy(ws.sev[i]);
@@ -226,7 +226,8 @@ int ensure_eval_buffers(apd_ctx* ctx, const GridDev& g, int kernel, bool cull, c
 int enqueue_evaluation(apd_ctx* ctx, const GridDev& g, int kernel, int M, const float* X, const float* A,
                        const float* w, const float* target_vol, int32_t* labels, double* vol, double* dual,
                        double* max_rel_err, double* centroids, uint64_t* pairs, bool timed, bool cull,
-                       const int* done_flag, cudaStream_t st, const int* cull_rebuild, const float* cull_delta) {
+                       const int* done_flag, cudaStream_t st, const int* cull_rebuild, const float* cull_delta,
+                       const int* cull_rebuild_s, const float* cull_delta_s) {
   Workspace& ws = ctx->ws;
   const int M_pad = (M + SEED_CHUNK - 1) / SEED_CHUNK * SEED_CHUNK;
   const int n_tiles = g.tiles_x * g.tiles_y * g.tiles_z;
@@ -261,7 +262,7 @@ int enqueue_evaluation(apd_ctx* ctx, const GridDev& g, int kernel, int M, const 
     cull_super_counts(g, &nsx, &nsy, &nsz);
     CullBuffers cb{ws.rec, ws.brick_list, ws.brick_count, ws.super_list, ws.super_count, ws.pairs_ctr};
     APD_CUDA_TRY(ctx, launch_cull(g, M, M_pad, X, A, w, cb, nsx, nsy, nsz, ws.count, centroids ? ws.idxsum : nullptr, done_flag,
-                                  cull_rebuild, cull_delta, st));
+                                  cull_rebuild, cull_delta, cull_rebuild_s, cull_delta_s, st));
     a.rec = ws.rec; a.brick_list = ws.brick_list; a.brick_count = ws.brick_count; a.super_list = ws.super_list;
     a.super_count = ws.super_count; a.super_x = nsx; a.super_y = nsy; a.pairs_ctr = ws.pairs_ctr;
   }

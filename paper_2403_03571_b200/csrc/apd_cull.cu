@@ -52,6 +52,7 @@ __global__ void cull_pack_kernel(int M, int M_pad, const float* __restrict__ X, 
                                  const float* __restrict__ w, float3 hb, float3 hs, float* __restrict__ rec,
                                  unsigned long long* __restrict__ pairs_ctr, unsigned int* __restrict__ count,
                                  unsigned long long* __restrict__ idxsum, const int* __restrict__ done_flag) {
+  pdl_enter();
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (done_flag && *done_flag) return;
   if (i == 0) *pairs_ctr = 0ull;
@@ -98,10 +99,14 @@ struct CullArgs {
   int* brick_count;        // [n_tiles * 4]
   float3 hb, ht, hs;       // half-extents of the boxes of voxel centres of a brick, a CTA tile, a super-tile
   const int* done_flag;
-  // list reuse inside apd_solve: the lists are rebuilt only when *rebuild != 0, with the slack *delta on both
+  // list reuse inside apd_solve: the brick lists are rebuilt only when *rebuild != 0, with the slack *delta on both
   // bounds, which keeps them valid for every w' with max_i |w'_i - w_i| <= delta.  nullptr: always rebuild, delta 0.
+  // The super-tile lists have their own flag and (larger) slack: the step kernel rebuilds them only when the ball
+  // the brick lists must cover is no longer inside theirs (apd_lbfgs.cu).
   const int* rebuild;
   const float* delta;
+  const int* rebuild_s;
+  const float* delta_s;
 };
 
 // For one seed and a box y0 +- h:  s_i = |y0 - x_i|_{A_i};  rho_i = max_corners |(+-h)|_{A_i} (SLOT 0 = brick,
@@ -216,13 +221,14 @@ __device__ __forceinline__ float box_centre(double lo, double s, int i0, int e) 
 // {i : lower bound_i <= U} into the super-tile's parent list.
 template <int DIM>
 __global__ void __launch_bounds__(CULL_THREADS) cull_super_kernel(const CullArgs c) {
+  pdl_enter();
   __shared__ float s_min[CULL_THREADS / 32];
   __shared__ int s_imin[CULL_THREADS / 32];
   __shared__ int s_wsum[CULL_THREADS / 32];
   __shared__ float s_U;
   if (c.done_flag && *c.done_flag) return;
-  if (c.rebuild && !*c.rebuild) return;
-  const float delta = c.delta ? *c.delta : 0.0f;
+  if (c.rebuild_s && !*c.rebuild_s) return;
+  const float delta = c.delta_s ? *c.delta_s : 0.0f;
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   const int b = blockIdx.x;
   const int sx = b % c.nsx, sy = (b / c.nsx) % c.nsy, sz = b / (c.nsx * c.nsy);
@@ -374,6 +380,7 @@ constexpr int CULL_G = 4;
 static_assert(CULL_G == SUPER3_TX && CULL_G == SUPER2_TX, "a CTA of cull_bricks_kernel covers one super-tile row");
 template <int DIM>
 __global__ void __launch_bounds__(128) cull_bricks_kernel(const CullArgs c) {
+  pdl_enter();
   __shared__ int s_tile[CULL_G][TILE_CAP];
   __shared__ float s_min[CULL_G][4];
   __shared__ int s_imin[CULL_G][4];
@@ -553,7 +560,7 @@ void cull_super_counts(const GridDev& g, int* nsx, int* nsy, int* nsz) {
 cudaError_t launch_cull(const GridDev& g, int M, int M_pad, const float* X, const float* A, const float* w,
                         const CullBuffers& cb, int nsx, int nsy, int nsz, unsigned int* count,
                         unsigned long long* idxsum, const int* done_flag, const int* rebuild, const float* delta,
-                        cudaStream_t st) {
+                        const int* rebuild_s, const float* delta_s, cudaStream_t st) {
   // half-extents of the boxes of voxel CENTRES of a brick and of a super-tile
   int ox, oy, oz, ex, ey, ez;
   brick_box(g.dim, 0, &ox, &oy, &oz, &ex, &ey, &ez);
@@ -564,26 +571,24 @@ cudaError_t launch_cull(const GridDev& g, int M, int M_pad, const float* X, cons
   const float3 hb = make_float3(half(ex, 0), half(ey, 1), g.dim == 3 ? half(ez, 2) : 0.0f);
   const float3 hs = make_float3(half(sex, 0), half(sey, 1), g.dim == 3 ? half(sez, 2) : 0.0f);
   const int nb = (M_pad + 127) / 128;
-  if (g.dim == 3) cull_pack_kernel<3><<<nb, 128, 0, st>>>(M, M_pad, X, A, w, hb, hs, cb.rec, cb.pairs_ctr, count, idxsum, done_flag);
-  else            cull_pack_kernel<2><<<nb, 128, 0, st>>>(M, M_pad, X, A, w, hb, hs, cb.rec, cb.pairs_ctr, count, idxsum, done_flag);
-  cudaError_t e = cudaGetLastError();
+  cudaError_t e;
+  if (g.dim == 3) e = launch_pdl(cull_pack_kernel<3>, nb, 128, 0, st, M, M_pad, X, A, w, hb, hs, cb.rec, cb.pairs_ctr, count, idxsum, done_flag);
+  else            e = launch_pdl(cull_pack_kernel<2>, nb, 128, 0, st, M, M_pad, X, A, w, hb, hs, cb.rec, cb.pairs_ctr, count, idxsum, done_flag);
   if (e != cudaSuccess) return e;
   CullArgs c;
   c.g = g; c.M = M; c.rec = cb.rec; c.super_list = cb.super_list; c.super_count = cb.super_count;
   c.nsx = nsx; c.nsy = nsy; c.nsz = nsz; c.brick_list = cb.brick_list; c.brick_count = cb.brick_count;
-  c.done_flag = done_flag; c.rebuild = rebuild; c.delta = delta;
+  c.done_flag = done_flag; c.rebuild = rebuild; c.delta = delta; c.rebuild_s = rebuild_s; c.delta_s = delta_s;
   c.hb = hb; c.hs = hs;
   c.ht = make_float3(half(g.dim == 3 ? CULL_TILE3_X : CULL_TILE2_X, 0), half(g.dim == 3 ? CULL_TILE3_Y : CULL_TILE2_Y, 1),
                      g.dim == 3 ? half(CULL_TILE3_Z, 2) : 0.0f);
   const int n_super = nsx * nsy * nsz;
   const int n_runs = nsx * g.tiles_y * g.tiles_z;      // runs of CULL_G tiles along x
-  if (g.dim == 3) cull_super_kernel<3><<<n_super, CULL_THREADS, 0, st>>>(c);
-  else            cull_super_kernel<2><<<n_super, CULL_THREADS, 0, st>>>(c);
-  e = cudaGetLastError();
+  if (g.dim == 3) e = launch_pdl(cull_super_kernel<3>, n_super, CULL_THREADS, 0, st, c);
+  else            e = launch_pdl(cull_super_kernel<2>, n_super, CULL_THREADS, 0, st, c);
   if (e != cudaSuccess) return e;
-  if (g.dim == 3) cull_bricks_kernel<3><<<n_runs, 128, 0, st>>>(c);
-  else            cull_bricks_kernel<2><<<n_runs, 128, 0, st>>>(c);
-  return cudaGetLastError();
+  if (g.dim == 3) return launch_pdl(cull_bricks_kernel<3>, n_runs, 128, 0, st, c);
+  return launch_pdl(cull_bricks_kernel<2>, n_runs, 128, 0, st, c);
 }
 
 }  // namespace apd

@@ -52,6 +52,16 @@ __device__ __forceinline__ void tma_bulk_g2s(void* dst, const void* src, uint32_
       : "memory");
 }
 
+// ---- programmatic dependent launch: the kernels of an evaluation chain are launched with
+// cudaLaunchAttributeProgrammaticStreamSerialization (launch_pdl, apd_internal.cuh), so a kernel's CTAs may become
+// resident while the kernel before it in the stream is still draining.  pdl_enter() is the FIRST thing such a kernel
+// does: it lets ITS successor be scheduled early in turn, then blocks until the predecessor grid has completed and its
+// writes are visible.  Nothing is read from global memory before it.  On an ordinary launch both are no-ops.
+__device__ __forceinline__ void pdl_enter() {
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+
 // ---- packed fp32 pairs (FFMA2 / FADD2 / FMUL2 on sm_100a) -------------------------------------
 typedef unsigned long long f2;   // two fp32 in one 64-bit register pair: {lo, hi}
 

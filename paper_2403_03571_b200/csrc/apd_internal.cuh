@@ -113,7 +113,8 @@ struct Workspace {
   int lb_cluster = 0;                   // CTAs of lbfgs_step_kernel's cluster on this device (0: not chosen yet)
   double* gram = nullptr;               // [(2 svec_hist + 1)^2] Gram matrix of the L-BFGS basis
   float* w32 = nullptr;                 // [max_seeds] fl32(w) the next evaluation uses
-  float* wref = nullptr;                // [max_seeds] weights the current candidate lists were built at
+  float* wref = nullptr;                // [max_seeds] weights the current brick candidate lists were built at
+  float* wref_s = nullptr;              // [max_seeds] weights the current super-tile lists were built at
   double* e_vol = nullptr;              // [max_seeds] evaluation outputs inside the solve loop
   double* e_scal = nullptr;             // [2] dual, max_rel_err
   double* hist = nullptr;               // [2 * SOLVE_HIST_CAP] (dual, err) per evaluation of the last solve
@@ -162,6 +163,20 @@ __host__ __device__ inline void brick_box(int dim, int w, int* ox, int* oy, int*
   else          { *ox = 16 * (w & 1); *oy = 32 * (w >> 1); *oz = 0; *ex = 16; *ey = 32; *ez = 1; }
 }
 
+// Launch with programmatic stream serialization: the kernel's CTAs may be scheduled while the kernel before it in the
+// stream drains; the kernel starts with pdl_enter() (apd_device.cuh), which waits for that kernel's completion.
+template <class... KArgs, class... Args>
+static inline cudaError_t launch_pdl(void (*kernel)(KArgs...), int grid, int block, size_t smem, cudaStream_t st,
+                                     Args&&... args) {
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3((unsigned)block); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
 struct CullBuffers {
   float* rec; int* brick_list; int* brick_count; int* super_list; int* super_count;
   unsigned long long* pairs_ctr;
@@ -169,7 +184,7 @@ struct CullBuffers {
 cudaError_t launch_cull(const GridDev& g, int M, int M_pad, const float* X, const float* A, const float* w,
                         const CullBuffers& cb, int n_super_x, int n_super_y, int n_super_z, unsigned int* count,
                         unsigned long long* idxsum, const int* done_flag, const int* rebuild, const float* delta,
-                        cudaStream_t st);
+                        const int* rebuild_s, const float* delta_s, cudaStream_t st);
 void cull_super_counts(const GridDev& g, int* nsx, int* nsy, int* nsz);
 int rowpoly_tile_counts(int dim, int nx, int ny, int nz, int sm_count, bool cull, int* tx, int* ty, int* tz);
 int assign_tile_counts(int kernel, int dim, int nx, int ny, int nz, int sm_count, bool cull, int* tx, int* ty, int* tz);
@@ -194,7 +209,8 @@ struct SolveReport {
   volatile int status;    // apd_status
   volatile int iters, evals;
   volatile double err, dual;
-  volatile int cull_rebuilds;   // evaluations of the solve loop that rebuilt the candidate lists
+  volatile int cull_rebuilds;   // evaluations of the solve loop that rebuilt the brick candidate lists
+  volatile int cull_rebuilds_s; // ... and the super-tile lists
 };
 
 // host helpers shared by apd_api.cu and apd_lbfgs.cu
@@ -224,7 +240,8 @@ int enqueue_evaluation(apd_ctx* ctx, const GridDev& g, int kernel, int M, const 
                        const float* w, const float* target_vol, int32_t* labels, double* vol, double* dual,
                        double* max_rel_err, double* centroids, uint64_t* pairs, bool timed, bool cull,
                        const int* done_flag, cudaStream_t st, const int* cull_rebuild = nullptr,
-                       const float* cull_delta = nullptr);
+                       const float* cull_delta = nullptr, const int* cull_rebuild_s = nullptr,
+                       const float* cull_delta_s = nullptr);
 
 }  // namespace apd
 

@@ -39,10 +39,11 @@ struct SolveState {
   int done, phase, iters, evals, trial, hist_len, hist_start, hist_cap, max_iters, max_evals;
   double f, gp, alpha, lo, hi, gamma, eps, best_err, best_dual, domain_volume;
   double rho[LB_MAX_HIST];
-  // candidate-list reuse (apd_cull.cu): the lists were built at wref with slack cull_delta and stay valid while
-  // max_i |w32_i - wref_i| <= cull_delta
-  int cull_rebuild, cull_rebuilds;
-  float cull_delta, cull_cap;
+  // candidate-list reuse (apd_cull.cu): the brick lists were built at wref with slack cull_delta and stay valid while
+  // max_i |w32_i - wref_i| <= cull_delta; the super-tile lists they are cut from were built at wref_s with the larger
+  // slack cull_delta_s and are rebuilt only when the ball the brick lists must cover leaves theirs
+  int cull_rebuild, cull_rebuilds, cull_rebuild_s, cull_rebuilds_s;
+  float cull_delta, cull_cap, cull_delta_s;
 };
 
 enum { V_W = 0, V_G, V_P, V_WTRY, V_WBEST, V_GNEW, V_Q, V_HIST };   // rows of svec
@@ -66,13 +67,19 @@ struct StepArgs {
   SolveReport* report; // mapped host memory
   double* hist;        // [2 * hist_cap] (dual, max_rel_err) of every evaluation, in order
   int hist_cap;
-  float* wref;         // weights the candidate lists were built at (culling only)
+  float* wref;         // weights the brick candidate lists were built at (culling only)
+  float* wref_s;       // weights the super-tile lists were built at
   double* gram;        // [LB_CLUSTER_MAX] copies of { (2 hist_cap + 1)^2 Gram matrix, hist_cap rho }, see GramSmem
 };
 
 constexpr double CULL_DELTA_FACTOR = 4.0;   // slack of a rebuilt list = this x the last change of the weights ...
 constexpr double CULL_CAP_FACTOR = 0.5;     // ... but at most this x the mean min-cost of the first evaluation (a larger
                                             // slack would lengthen every list by more than it saves in rebuilds)
+constexpr double CULL_SUPER_FACTOR = 8.0;   // slack of a rebuilt super-tile list = this x the brick lists': a super-tile's
+                                            // bounds are loose anyway, so its list barely grows and it is rebuilt far less
+                                            // often.  Measured (cfg 4 / cfg 5 solve; super-tile rebuilds of 59 / 61 brick
+                                            // rebuilds): x1 (one slack for both) 59 / 61, 25.0 / 107 ms; x4 27 / 28, 23.7 /
+                                            // 99.9; x8 12 / 11, 23.3 / 96.7; x16 6 / 6, 23.3 / 97.1; x64 2 / 2, 24.5 / 106.6
 
 // ---- reductions over the CLUSTER ------------------------------------------------------------------------------
 // The step kernel is ONE thread-block cluster of nranks = 8 or 16 CTAs (one per SM): a single CTA cannot keep enough loads
@@ -447,7 +454,7 @@ __device__ DirCoef direction_coeffs(const GramSmem& G, int cap, int hist_len, in
 //     [push]  s = alpha_old p, y = g1 - g  -> ring slot push.slot;   w <- w_try;   g <- g1
 //     p = -(delta_g g + sum_t delta_t s_t + delta_{m+t} y_t),   w_try = w + alpha p  (alpha = 1: a new direction),
 // w32 = fl32(w_try) (S10), the best-so-far copy of the point just evaluated, and ONE exchange for g.p (sum) and the two
-// maxima the candidate-list reuse needs (|change since the last evaluation|, |distance from wref|).  Two elements
+// maxima the candidate-list reuse needs (|change since the last evaluation|, |distance from wref|, from wref_s).  Two elements
 // per thread are in flight, and the history loads of an element are issued LB_COMB_SLOTS pairs at a time before any
 // of them is used (a loop of dependent load-FMA pairs ran at one L2 round trip per four pairs: 9 of the step's 36 us
 // at M = 10^4).  All loads of an element precede its stores; the pushed pair is used from registers.
@@ -464,7 +471,7 @@ struct TrialArgs {
   double alpha;
 };
 __device__ void combine_and_trial(const StepArgs& a, int cap, const DirCoef& dc, const TrialArgs& ta,
-                                  const PushArgs& pu, Reducer& r, double* gp_out, double (&mx_out)[2]) {
+                                  const PushArgs& pu, Reducer& r, double* gp_out, double (&mx_out)[3]) {
   const int M = a.M, stride = a.stride, hl = dc.hl;
   double* g = a.vec + (size_t)V_G * stride;
   double* p = a.vec + (size_t)V_P * stride;
@@ -475,12 +482,12 @@ __device__ void combine_and_trial(const StepArgs& a, int cap, const DirCoef& dc,
   double* S = a.vec + (size_t)V_HIST * stride;
   double* Y = S + (size_t)cap * stride;
   const double dg = dc.delta[2 * hl];
-  double red3[3] = {0.0, 0.0, 0.0};      // g.p | max |change since the last evaluation|, max |distance from wref|
+  double red3[4] = {0.0, 0.0, 0.0, 0.0}; // g.p | max |change since the last evaluation|, |distance from wref|, from wref_s
   constexpr int NC = LB_COMB_SLOTS, U = LB_COMB_U;
   const int LB_STEP_R = LB_STEP_OF(r);
   for (int i0 = LB_FIRST(r); i0 < M; i0 += U * LB_STEP_R) {
     double gi[U], wi[U], we[U], sn[U], yn[U], acc[U];
-    float w32_old[U], wref[U];
+    float w32_old[U], wref[U], wref_s[U];
     int idx[U];
 #pragma unroll
     for (int u = 0; u < U; ++u) {
@@ -488,7 +495,7 @@ __device__ void combine_and_trial(const StepArgs& a, int cap, const DirCoef& dc,
       idx[u] = i < M ? i : i0;                    // past the end: a duplicate of the first element, never stored
       const int ii = idx[u];
       we[u] = ta.improved ? ta.w_eval[ii] : 0.0;
-      w32_old[u] = a.w32[ii]; wref[u] = a.wref[ii];
+      w32_old[u] = a.w32[ii]; wref[u] = a.wref[ii]; wref_s[u] = a.wref_s[ii];
       if (pu.on) {
         const double gn = gnew[ii];
         sn[u] = __dmul_rn(pu.alpha_old, p[ii]); yn[u] = __dsub_rn(gn, g[ii]);
@@ -538,12 +545,13 @@ __device__ void combine_and_trial(const StepArgs& a, int cap, const DirCoef& dc,
         const float wn = (float)wt;
         red3[1] = fmax(red3[1], fabs((double)wn - (double)w32_old[u]));      // differences of floats: exact in fp64
         red3[2] = fmax(red3[2], fabs((double)wn - (double)wref[u]));
+        red3[3] = fmax(red3[3], fabs((double)wn - (double)wref_s[u]));
         a.w32[i] = wn;
       }
     }
   }
-  cluster_all_mixed<3, 2>(red3, r);
-  *gp_out = red3[0]; mx_out[0] = red3[1]; mx_out[1] = red3[2];
+  cluster_all_mixed<4, 3>(red3, r);
+  *gp_out = red3[0]; mx_out[0] = red3[1]; mx_out[1] = red3[2]; mx_out[2] = red3[3];
 }
 
 __global__ void solve_init_kernel(StepArgs a, const float* w_init, int hist_cap, int max_iters, int max_evals,
@@ -554,10 +562,12 @@ __global__ void solve_init_kernel(StepArgs a, const float* w_init, int hist_cap,
     a.vec[(size_t)V_W * a.stride + i] = w;
     a.w32[i] = (float)w;
     a.wref[i] = (float)w;
+    a.wref_s[i] = (float)w;
   }
   if (i == 0) {
     SolveState* st = a.st;
     st->cull_rebuild = 1; st->cull_rebuilds = 1; st->cull_delta = 0.0f; st->cull_cap = 0.0f;
+    st->cull_rebuild_s = 1; st->cull_rebuilds_s = 1; st->cull_delta_s = 0.0f;
     st->done = 0; st->phase = 0; st->iters = 0; st->evals = 0; st->trial = 0;
     st->hist_len = 0; st->hist_start = 0; st->hist_cap = hist_cap;
     st->max_iters = max_iters; st->max_evals = max_evals;
@@ -565,7 +575,7 @@ __global__ void solve_init_kernel(StepArgs a, const float* w_init, int hist_cap,
     st->gamma = gamma0; st->eps = eps; st->best_err = INFINITY; st->best_dual = 0.0;
     st->domain_volume = domain_volume;
     a.report->done = 0; a.report->status = APD_OK; a.report->iters = 0; a.report->evals = 0;
-    a.report->err = 0.0; a.report->dual = 0.0; a.report->cull_rebuilds = 0;
+    a.report->err = 0.0; a.report->dual = 0.0; a.report->cull_rebuilds = 0; a.report->cull_rebuilds_s = 0;
   }
 }
 
@@ -584,6 +594,7 @@ __global__ void __launch_bounds__(LB_THREADS) lbfgs_step_kernel(StepArgs a) {
   Reducer red{s_wbuf, s_cbuf, s_tot, 0, cluster.block_rank(), cluster.num_blocks()};
   const int LB_STEP_R = LB_STEP_OF(red);
   SolveState* st = a.st;
+  pdl_enter();
   if (st->done) return;                    // uniform: written by the previous launch
   const bool lead = red.rank == 0;
   const int M = a.M, stride = a.stride, tid = threadIdx.x;
@@ -602,8 +613,8 @@ __global__ void __launch_bounds__(LB_THREADS) lbfgs_step_kernel(StepArgs a) {
   const double eps = st->eps, domain_volume = st->domain_volume;
   double best_err = st->best_err, best_dual = st->best_dual;
   float cull_cap = st->cull_cap;
-  const float cull_delta_old = st->cull_delta;
-  const int cull_rebuilds_old = st->cull_rebuilds;
+  const float cull_delta_old = st->cull_delta, cull_delta_s_old = st->cull_delta_s;
+  const int cull_rebuilds_old = st->cull_rebuilds, cull_rebuilds_s_old = st->cull_rebuilds_s;
 
   // the Gram matrix of the history: fetched now, stored to shared memory after the layer sums (whose loads hide the
   // latency), patched and used after the decision
@@ -672,7 +683,7 @@ __global__ void __launch_bounds__(LB_THREADS) lbfgs_step_kernel(StepArgs a) {
 
   int finish = 0;          // 1: OK at w_eval, 2: NOT_CONVERGED at best, 3: bad target volumes
   bool need_direction = false;
-  double mx[2] = {0.0, 0.0};   // max |change of fl32 w since the last evaluation|, max |distance from wref|
+  double mx[3] = {0.0, 0.0, 0.0};   // max |change of fl32 w since the last evaluation|, |distance from wref|, from wref_s
   int new_slot = -1;       // ring slot a curvature pair is pushed into by this call, else -1
   bool evicts = false;     // ... and that slot held the oldest pair (the ring was full)
   bool accepted = false;
@@ -770,8 +781,8 @@ __global__ void __launch_bounds__(LB_THREADS) lbfgs_step_kernel(StepArgs a) {
     }
   }
 
-  int cull_rebuild = 1;
-  float cull_delta = 0.0f;
+  int cull_rebuild = 1, cull_rebuild_s = 1;
+  float cull_delta = 0.0f, cull_delta_s = 0.0f;
   if (finish == 0) {
     if (!need_direction) {
       // next trial point w + alpha p of the line search, rounded to fp32 for the evaluation (S10)
@@ -782,16 +793,26 @@ __global__ void __launch_bounds__(LB_THREADS) lbfgs_step_kernel(StepArgs a) {
         const float wn = (float)wt;
         mx[0] = fmax(mx[0], fabs((double)wn - (double)a.w32[i]));     // differences of floats: exact in fp64
         mx[1] = fmax(mx[1], fabs((double)wn - (double)a.wref[i]));
+        mx[2] = fmax(mx[2], fabs((double)wn - (double)a.wref_s[i]));
         a.w32[i] = wn;
       }
-      cluster_all<2, true>(mx, red);
+      cluster_all<3, true>(mx, red);
     }
-    cull_delta = cull_delta_old;
+    cull_delta = cull_delta_old; cull_delta_s = cull_delta_s_old;
     cull_rebuild = !(mx[1] <= (double)cull_delta);
+    cull_rebuild_s = 0;
     if (cull_rebuild) {
-      // the next evaluation rebuilds its candidate lists at the new weights, valid within delta of them
+      // the next evaluation rebuilds its brick lists at the new weights, valid within delta of them; they are cut from
+      // the super-tile lists, which must hold on that whole ball: (distance from wref_s) + delta <= delta_s, else
+      // those are rebuilt too, with a slack CULL_SUPER_FACTOR times as large (sums of floats: exact in fp64)
       cull_delta = fminf((float)(CULL_DELTA_FACTOR * mx[0]), cull_cap);
-      for (int i = LB_FIRST(red); i < M; i += LB_STEP_R) a.wref[i] = a.w32[i];
+      cull_rebuild_s = !(mx[2] + (double)cull_delta <= (double)cull_delta_s);
+      if (cull_rebuild_s) cull_delta_s = (float)(CULL_SUPER_FACTOR * (double)cull_delta);
+      for (int i = LB_FIRST(red); i < M; i += LB_STEP_R) {
+        const float wn = a.w32[i];
+        a.wref[i] = wn;
+        if (cull_rebuild_s) a.wref_s[i] = wn;
+      }
     }
   } else if (finish == 1) {
     if (phase != 0) for (int i = LB_FIRST(red); i < M; i += LB_STEP_R) w[i] = wtry[i];
@@ -808,14 +829,16 @@ __global__ void __launch_bounds__(LB_THREADS) lbfgs_step_kernel(StepArgs a) {
     st->f = f; st->gp = gp; st->alpha = alpha; st->lo = lo; st->hi = hi; st->gamma = gamma;
     st->best_err = best_err; st->best_dual = best_dual;
     st->cull_cap = cull_cap; st->cull_rebuild = cull_rebuild; st->cull_delta = cull_delta;
+    st->cull_rebuild_s = cull_rebuild_s; st->cull_delta_s = cull_delta_s;
     st->cull_rebuilds = cull_rebuilds_old + (finish == 0 && cull_rebuild);
+    st->cull_rebuilds_s = cull_rebuilds_s_old + (finish == 0 && cull_rebuild_s);
     if (finish) {
       st->done = 1;
       a.report->status = (finish == 1) ? APD_OK : (finish == 2 ? APD_NOT_CONVERGED : APD_E_ARG);
       a.report->iters = iters; a.report->evals = evals;
       a.report->err = (finish == 2) ? best_err : err1;
       a.report->dual = (finish == 2) ? best_dual : -f1;
-      a.report->cull_rebuilds = st->cull_rebuilds;
+      a.report->cull_rebuilds = st->cull_rebuilds; a.report->cull_rebuilds_s = st->cull_rebuilds_s;
       __threadfence_system();
       a.report->done = 1;
       __threadfence_system();
@@ -843,6 +866,7 @@ int apd::ensure_solve_state(apd_ctx* ctx, int hist) {
     LB_TRY(cudaMalloc(&ws.sstate, sizeof(SolveState)));
     LB_TRY(cudaMalloc(&ws.w32, ms * sizeof(float)));
     LB_TRY(cudaMalloc(&ws.wref, ms * sizeof(float)));
+    LB_TRY(cudaMalloc(&ws.wref_s, ms * sizeof(float)));
     LB_TRY(cudaMalloc(&ws.e_vol, ms * sizeof(double)));
     LB_TRY(cudaMalloc(&ws.e_scal, 2 * sizeof(double)));
     LB_TRY(cudaMalloc(&ws.hist, 2 * (size_t)SOLVE_HIST_CAP * sizeof(double)));
@@ -898,7 +922,7 @@ static int solve_common(apd_ctx* ctx, const char* who, int dim, int32_t M, const
   const double ell = std::pow(domain / (double)M, 1.0 / (double)dim);
   const double gamma0 = std::pow(ell, (double)(2 - dim)) / (double)dim;
   sa.st = ws.sstate; sa.vec = ws.svec; sa.stride = ws.max_seeds; sa.M = M; sa.v = target_vol; sa.w32 = ws.w32;
-  sa.hist = ws.hist; sa.hist_cap = SOLVE_HIST_CAP; sa.wref = ws.wref; sa.gram = ws.gram;
+  sa.hist = ws.hist; sa.hist_cap = SOLVE_HIST_CAP; sa.wref = ws.wref; sa.wref_s = ws.wref_s; sa.gram = ws.gram;
   ws.hist_len = 0;
   SolveReport* dev_report = nullptr;
   LB_TRY(cudaHostGetDevicePointer((void**)&dev_report, ws.report, 0));
@@ -917,13 +941,15 @@ static int solve_common(apd_ctx* ctx, const char* who, int dim, int32_t M, const
     const int rc = lb_cluster_size(ctx, dyn_bytes, &ws.lb_cluster);
     if (rc != APD_OK) return rc;
   }
-  cudaLaunchAttribute step_attr[1];
+  cudaLaunchAttribute step_attr[2];
+  step_attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;     // apd_device.cuh: pdl_enter
+  step_attr[1].val.programmaticStreamSerializationAllowed = 1;
   step_attr[0].id = cudaLaunchAttributeClusterDimension;
   const unsigned n_cta = (ws.lb_cluster == LB_CLUSTER_MAX && M >= LB_CLUSTER_MAX_MIN_M) ? LB_CLUSTER_MAX : LB_CLUSTER_PORTABLE;
   step_attr[0].val.clusterDim.x = n_cta; step_attr[0].val.clusterDim.y = 1; step_attr[0].val.clusterDim.z = 1;
   cudaLaunchConfig_t step_cfg = {};
   step_cfg.gridDim = dim3(n_cta); step_cfg.blockDim = dim3(LB_THREADS);
-  step_cfg.dynamicSmemBytes = dyn_bytes; step_cfg.stream = st; step_cfg.attrs = step_attr; step_cfg.numAttrs = 1;
+  step_cfg.dynamicSmemBytes = dyn_bytes; step_cfg.stream = st; step_cfg.attrs = step_attr; step_cfg.numAttrs = 2;
   const int* done_flag = &ws.sstate->done;
   long long enq = 0;
   const long long hard_cap = (long long)max_evals + 64;
@@ -1026,7 +1052,7 @@ int apd::solve_grid(apd_ctx* ctx, const char* who, const apd_grid* grid, const a
   hooks.loop_eval = [&](const int* done_flag) -> int {
     int r = enqueue_evaluation(ctx, g, kernel, M, X, A, ws.w32, target_vol, nullptr, nullptr, nullptr, nullptr, nullptr,
                                nullptr, false, o.cull != 0, done_flag, st, &ws.sstate->cull_rebuild,
-                               &ws.sstate->cull_delta);
+                               &ws.sstate->cull_delta, &ws.sstate->cull_rebuild_s, &ws.sstate->cull_delta_s);
     if (r == APD_OK && slab) r = exchange(false, done_flag);
     return r;
   };

@@ -424,6 +424,7 @@ __global__ void __launch_bounds__(128, 6) assign_rowpoly_culled_kernel(const Ass
   __shared__ __align__(16) float s_seeds[4][2][STAGE_FLOATS];
   __shared__ int s_idx[4][2][WCHUNK];
 
+  pdl_enter();
   if (a.done_flag && *a.done_flag) return;
   const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
   const int b = blockIdx.x;
@@ -552,8 +553,7 @@ static cudaError_t launch_rowpoly_t(const AssignArgs& a, int n_tiles, cudaStream
 
 template <int DIM>
 static cudaError_t launch_culled_t(const AssignArgs& a, int n_tiles, cudaStream_t st) {
-  assign_rowpoly_culled_kernel<DIM><<<n_tiles, 128, 0, st>>>(a);
-  return cudaGetLastError();
+  return launch_pdl(assign_rowpoly_culled_kernel<DIM>, n_tiles, 128, 0, st, a);
 }
 
 cudaError_t launch_assign_rowpoly(const AssignArgs& a, cudaStream_t st) {
