@@ -30,10 +30,10 @@ extern "C" void apd_default_opts(apd_opts* o) {
 }
 
 static void free_ws(Workspace& ws) {
-  cudaFree(ws.lloyd_buf); cudaFree(ws.pt_acc); cudaFree(ws.qfix); cudaFree(ws.rec); cudaFree(ws.brick_list); cudaFree(ws.brick_count); cudaFree(ws.super_list);
+  cudaFree(ws.lloyd_buf); cudaFree(ws.pt_acc); cudaFree(ws.qfix); cudaFree(ws.rec); cudaFree(ws.brick_list); cudaFree(ws.brick_count); cudaFree(ws.tile_list); cudaFree(ws.tile_count); cudaFree(ws.super_list);
   cudaFree(ws.super_count); cudaFree(ws.pairs_ctr);
   cudaFree(ws.seeds); cudaFree(ws.count); cudaFree(ws.idxsum); cudaFree(ws.dual_partial); cudaFree(ws.layer_buf);
-  cudaFree(ws.sstate); cudaFree(ws.svec); cudaFree(ws.gram); cudaFree(ws.w32); cudaFree(ws.wref); cudaFree(ws.wref_s); cudaFree(ws.e_vol); cudaFree(ws.e_scal); cudaFree(ws.hist);
+  cudaFree(ws.sstate); cudaFree(ws.svec); cudaFree(ws.gram); cudaFree(ws.w32); cudaFree(ws.wref); cudaFree(ws.wref_s); cudaFree(ws.wref_t); cudaFree(ws.e_vol); cudaFree(ws.e_scal); cudaFree(ws.hist);
   for (int i = 0; i < Workspace::HOST_SLOTS; ++i) cudaFree(ws.host_buf[i]);
   if (ws.report) cudaFreeHost(ws.report);
   for (int i = 0; i < 2; ++i) if (ws.sev[i]) cudaEventDestroy(ws.sev[i]);
@@ -208,12 +208,15 @@ int ensure_eval_buffers(apd_ctx* ctx, const GridDev& g, int kernel, bool cull, c
     if (n_bricks > ws.brick_cap_n || n_super > ws.super_cap_n) {
       APD_CUDA_TRY(ctx, cudaStreamSynchronize(st));
       cudaFree(ws.brick_list); cudaFree(ws.brick_count); cudaFree(ws.super_list); cudaFree(ws.super_count);
-      ws.brick_list = ws.brick_count = ws.super_list = ws.super_count = nullptr;
+      cudaFree(ws.tile_list); cudaFree(ws.tile_count);
+      ws.brick_list = ws.brick_count = ws.super_list = ws.super_count = ws.tile_list = ws.tile_count = nullptr;
       const size_t nb = n_bricks > ws.brick_cap_n ? n_bricks : ws.brick_cap_n;
       const size_t ns = n_super > ws.super_cap_n ? n_super : ws.super_cap_n;
       ws.brick_cap_n = ws.super_cap_n = 0;
       APD_CUDA_TRY(ctx, cudaMalloc(&ws.brick_list, nb * BRICK_CAP * sizeof(int)));
       APD_CUDA_TRY(ctx, cudaMalloc(&ws.brick_count, nb * sizeof(int)));
+      APD_CUDA_TRY(ctx, cudaMalloc(&ws.tile_list, (nb / 4) * TILE_CAP * sizeof(int)));
+      APD_CUDA_TRY(ctx, cudaMalloc(&ws.tile_count, (nb / 4) * sizeof(int)));
       APD_CUDA_TRY(ctx, cudaMalloc(&ws.super_list, ns * SUPER_CAP * sizeof(int)));
       APD_CUDA_TRY(ctx, cudaMalloc(&ws.super_count, ns * sizeof(int)));
       ws.brick_cap_n = nb; ws.super_cap_n = ns;
@@ -227,7 +230,8 @@ int enqueue_evaluation(apd_ctx* ctx, const GridDev& g, int kernel, int M, const 
                        const float* w, const float* target_vol, int32_t* labels, double* vol, double* dual,
                        double* max_rel_err, double* centroids, uint64_t* pairs, bool timed, bool cull,
                        const int* done_flag, cudaStream_t st, const int* cull_rebuild, const float* cull_delta,
-                       const int* cull_rebuild_s, const float* cull_delta_s) {
+                       const int* cull_rebuild_s, const float* cull_delta_s, const int* cull_rebuild_t,
+                       const float* cull_delta_t) {
   Workspace& ws = ctx->ws;
   const int M_pad = (M + SEED_CHUNK - 1) / SEED_CHUNK * SEED_CHUNK;
   const int n_tiles = g.tiles_x * g.tiles_y * g.tiles_z;
@@ -260,9 +264,9 @@ int enqueue_evaluation(apd_ctx* ctx, const GridDev& g, int kernel, int M, const 
     // a7: two-level candidate lists (rebuilt when the weights left the slack they were built with)
     int nsx, nsy, nsz;
     cull_super_counts(g, &nsx, &nsy, &nsz);
-    CullBuffers cb{ws.rec, ws.brick_list, ws.brick_count, ws.super_list, ws.super_count, ws.pairs_ctr};
+    CullBuffers cb{ws.rec, ws.brick_list, ws.brick_count, ws.super_list, ws.super_count, ws.tile_list, ws.tile_count, ws.pairs_ctr};
     APD_CUDA_TRY(ctx, launch_cull(g, M, M_pad, X, A, w, cb, nsx, nsy, nsz, ws.count, centroids ? ws.idxsum : nullptr, done_flag,
-                                  cull_rebuild, cull_delta, cull_rebuild_s, cull_delta_s, st));
+                                  cull_rebuild, cull_delta, cull_rebuild_s, cull_delta_s, cull_rebuild_t, cull_delta_t, st));
     a.rec = ws.rec; a.brick_list = ws.brick_list; a.brick_count = ws.brick_count; a.super_list = ws.super_list;
     a.super_count = ws.super_count; a.super_x = nsx; a.super_y = nsy; a.pairs_ctr = ws.pairs_ctr;
   }

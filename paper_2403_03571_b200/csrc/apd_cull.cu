@@ -107,6 +107,12 @@ struct CullArgs {
   const float* delta;
   const int* rebuild_s;
   const float* delta_s;
+  // the CTA-tile lists (the middle level) are kept in global memory between the evaluations of a solve, with a
+  // slack of their own between the two: a brick rebuild then starts from its tile's stored list
+  int* tile_list;          // [n_tiles, TILE_CAP] or nullptr (single evaluations: the tile lists live in shared memory only)
+  int* tile_count;         // [n_tiles]
+  const int* rebuild_t;
+  const float* delta_t;
 };
 
 // For one seed and a box y0 +- h:  s_i = |y0 - x_i|_{A_i};  rho_i = max_corners |(+-h)|_{A_i} (SLOT 0 = brick,
@@ -375,7 +381,6 @@ struct RefSeed {
 // record is gathered ONCE per pass and tested against the CULL_G boxes, which is what this kernel is bound by;
 // (b) for each tile in turn, each warp cuts the tile's list down to its own brick.  Same two passes (U = min upper
 // bound, ordered compaction of lower bound <= U) at both steps.
-constexpr int TILE_CAP = 768;
 constexpr int CULL_G = 4;
 static_assert(CULL_G == SUPER3_TX && CULL_G == SUPER2_TX, "a CTA of cull_bricks_kernel covers one super-tile row");
 template <int DIM>
@@ -388,6 +393,8 @@ __global__ void __launch_bounds__(128) cull_bricks_kernel(const CullArgs c) {
   if (c.done_flag && *c.done_flag) return;
   if (c.rebuild && !*c.rebuild) return;
   const float delta = c.delta ? *c.delta : 0.0f;
+  const bool rebuild_t = !c.tile_list || !c.rebuild_t || *c.rebuild_t;
+  const float delta_t = (c.tile_list && c.delta_t) ? *c.delta_t : delta;
   const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
   const int b = blockIdx.x;
   const int qx = b % c.nsx, by = (b / c.nsx) % c.g.tiles_y, bz = b / (c.nsx * c.g.tiles_y);
@@ -400,9 +407,19 @@ __global__ void __launch_bounds__(128) cull_bricks_kernel(const CullArgs c) {
   const int* par = c.super_list + (size_t)sup * SUPER_CAP;
   if (n_par < 0) { n_par = c.M; par = nullptr; }
 
-  // (a) CTA-tile lists
+  // (a) CTA-tile lists: built from the parent list, or (inside a solve, while the weights stayed within the slack
+  // they were built with) read back from global memory
   int n_tile[CULL_G];
-  {
+  const size_t tile0 = ((size_t)bz * c.g.tiles_y + by) * c.g.tiles_x + (size_t)qx * CULL_G;
+  if (!rebuild_t) {
+#pragma unroll
+    for (int g = 0; g < CULL_G; ++g) {
+      n_tile[g] = (g < ng) ? c.tile_count[tile0 + g] : 0;
+      const int* src = c.tile_list + (tile0 + g) * TILE_CAP;
+      for (int q = tid; q < n_tile[g]; q += 128) s_tile[g][q] = src[q];
+    }
+    __syncthreads();
+  } else {
     float t0x[CULL_G];
 #pragma unroll
     for (int g = 0; g < CULL_G; ++g) t0x[g] = box_centre(c.g.lo[0], c.g.s[0], (qx * CULL_G + g) * TX, TX);
@@ -439,7 +456,7 @@ __global__ void __launch_bounds__(128) cull_bricks_kernel(const CullArgs c) {
 #pragma unroll
       for (int j = 1; j < 4; ++j) if (s_min[g][j] < u) { u = s_min[g][j]; kbest = s_imin[g][j]; }
       if (n_par > 0) u = fminf(u, exact_upper<DIM>(c.rec, kbest, t0x[g], t0y, t0z, c.ht));
-      U[g] = u + 2.0f * delta * (1.0f + CULL_EPS);
+      U[g] = u + 2.0f * delta_t * (1.0f + CULL_EPS);
     }
     int base[CULL_G];
 #pragma unroll
@@ -487,6 +504,15 @@ __global__ void __launch_bounds__(128) cull_bricks_kernel(const CullArgs c) {
     __syncthreads();
 #pragma unroll
     for (int g = 0; g < CULL_G; ++g) n_tile[g] = (base[g] <= TILE_CAP) ? base[g] : -1;   // -1: bricks cut the parent list
+    if (c.tile_list) {
+#pragma unroll
+      for (int g = 0; g < CULL_G; ++g) {
+        if (g >= ng) break;
+        int* dst = c.tile_list + (tile0 + g) * TILE_CAP;
+        for (int q = tid; q < n_tile[g]; q += 128) dst[q] = s_tile[g][q];
+        if (tid == 0) c.tile_count[tile0 + g] = n_tile[g];
+      }
+    }
   }
 
   // (b) brick lists, tile by tile
@@ -560,7 +586,8 @@ void cull_super_counts(const GridDev& g, int* nsx, int* nsy, int* nsz) {
 cudaError_t launch_cull(const GridDev& g, int M, int M_pad, const float* X, const float* A, const float* w,
                         const CullBuffers& cb, int nsx, int nsy, int nsz, unsigned int* count,
                         unsigned long long* idxsum, const int* done_flag, const int* rebuild, const float* delta,
-                        const int* rebuild_s, const float* delta_s, cudaStream_t st) {
+                        const int* rebuild_s, const float* delta_s, const int* rebuild_t, const float* delta_t,
+                        cudaStream_t st) {
   // half-extents of the boxes of voxel CENTRES of a brick and of a super-tile
   int ox, oy, oz, ex, ey, ez;
   brick_box(g.dim, 0, &ox, &oy, &oz, &ex, &ey, &ez);
@@ -579,6 +606,8 @@ cudaError_t launch_cull(const GridDev& g, int M, int M_pad, const float* X, cons
   c.g = g; c.M = M; c.rec = cb.rec; c.super_list = cb.super_list; c.super_count = cb.super_count;
   c.nsx = nsx; c.nsy = nsy; c.nsz = nsz; c.brick_list = cb.brick_list; c.brick_count = cb.brick_count;
   c.done_flag = done_flag; c.rebuild = rebuild; c.delta = delta; c.rebuild_s = rebuild_s; c.delta_s = delta_s;
+  // the tile lists are kept only inside a solve (rebuild flags given): a single evaluation builds them in shared memory
+  c.tile_list = rebuild ? cb.tile_list : nullptr; c.tile_count = cb.tile_count; c.rebuild_t = rebuild_t; c.delta_t = delta_t;
   c.hb = hb; c.hs = hs;
   c.ht = make_float3(half(g.dim == 3 ? CULL_TILE3_X : CULL_TILE2_X, 0), half(g.dim == 3 ? CULL_TILE3_Y : CULL_TILE2_Y, 1),
                      g.dim == 3 ? half(CULL_TILE3_Z, 2) : 0.0f);

@@ -94,6 +94,8 @@ struct Workspace {
   float* rec = nullptr;                // [M_pad, REC] per-seed records + rho_brick, rho_super
   int* brick_list = nullptr;           // [brick_cap_n * BRICK_CAP]
   int* brick_count = nullptr;          // [brick_cap_n]
+  int* tile_list = nullptr;            // [brick_cap_n / 4 * TILE_CAP] CTA-tile lists kept between the evaluations of a solve
+  int* tile_count = nullptr;           // [brick_cap_n / 4]
   size_t brick_cap_n = 0;
   int* super_list = nullptr;           // [super_cap_n * SUPER_CAP]
   int* super_count = nullptr;          // [super_cap_n]
@@ -115,6 +117,7 @@ struct Workspace {
   float* w32 = nullptr;                 // [max_seeds] fl32(w) the next evaluation uses
   float* wref = nullptr;                // [max_seeds] weights the current brick candidate lists were built at
   float* wref_s = nullptr;              // [max_seeds] weights the current super-tile lists were built at
+  float* wref_t = nullptr;              // [max_seeds] weights the current CTA-tile lists were built at
   double* e_vol = nullptr;              // [max_seeds] evaluation outputs inside the solve loop
   double* e_scal = nullptr;             // [2] dual, max_rel_err
   double* hist = nullptr;               // [2 * SOLVE_HIST_CAP] (dual, err) per evaluation of the last solve
@@ -155,6 +158,7 @@ constexpr int SUPER3_TX = 4, SUPER3_TY = 2, SUPER3_TZ = 4;
 constexpr int SUPER2_TX = 4, SUPER2_TY = 2;
 constexpr int BRICK_CAP = 256;         // candidate-list capacity of a brick
 constexpr int SUPER_CAP = 4096;        // candidate-list capacity of a super-tile
+constexpr int TILE_CAP = 768;          // candidate-list capacity of a CTA tile (shared memory; global inside a solve)
 constexpr int SOLVE_HIST_CAP = 8192;   // evaluations of a solve whose (dual, err) are kept for apd_solve_history
 
 // origin (relative to the CTA tile) and extent, in voxels, of brick w
@@ -178,13 +182,14 @@ static inline cudaError_t launch_pdl(void (*kernel)(KArgs...), int grid, int blo
 }
 
 struct CullBuffers {
-  float* rec; int* brick_list; int* brick_count; int* super_list; int* super_count;
+  float* rec; int* brick_list; int* brick_count; int* super_list; int* super_count; int* tile_list; int* tile_count;
   unsigned long long* pairs_ctr;
 };
 cudaError_t launch_cull(const GridDev& g, int M, int M_pad, const float* X, const float* A, const float* w,
                         const CullBuffers& cb, int n_super_x, int n_super_y, int n_super_z, unsigned int* count,
                         unsigned long long* idxsum, const int* done_flag, const int* rebuild, const float* delta,
-                        const int* rebuild_s, const float* delta_s, cudaStream_t st);
+                        const int* rebuild_s, const float* delta_s, const int* rebuild_t, const float* delta_t,
+                        cudaStream_t st);
 void cull_super_counts(const GridDev& g, int* nsx, int* nsy, int* nsz);
 int rowpoly_tile_counts(int dim, int nx, int ny, int nz, int sm_count, bool cull, int* tx, int* ty, int* tz);
 int assign_tile_counts(int kernel, int dim, int nx, int ny, int nz, int sm_count, bool cull, int* tx, int* ty, int* tz);
@@ -211,6 +216,7 @@ struct SolveReport {
   volatile double err, dual;
   volatile int cull_rebuilds;   // evaluations of the solve loop that rebuilt the brick candidate lists
   volatile int cull_rebuilds_s; // ... and the super-tile lists
+  volatile int cull_rebuilds_t; // ... and the CTA-tile lists
 };
 
 // host helpers shared by apd_api.cu and apd_lbfgs.cu
@@ -241,7 +247,8 @@ int enqueue_evaluation(apd_ctx* ctx, const GridDev& g, int kernel, int M, const 
                        double* max_rel_err, double* centroids, uint64_t* pairs, bool timed, bool cull,
                        const int* done_flag, cudaStream_t st, const int* cull_rebuild = nullptr,
                        const float* cull_delta = nullptr, const int* cull_rebuild_s = nullptr,
-                       const float* cull_delta_s = nullptr);
+                       const float* cull_delta_s = nullptr, const int* cull_rebuild_t = nullptr,
+                       const float* cull_delta_t = nullptr);
 
 }  // namespace apd
 

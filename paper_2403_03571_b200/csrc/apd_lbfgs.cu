@@ -42,8 +42,8 @@ struct SolveState {
   // candidate-list reuse (apd_cull.cu): the brick lists were built at wref with slack cull_delta and stay valid while
   // max_i |w32_i - wref_i| <= cull_delta; the super-tile lists they are cut from were built at wref_s with the larger
   // slack cull_delta_s and are rebuilt only when the ball the brick lists must cover leaves theirs
-  int cull_rebuild, cull_rebuilds, cull_rebuild_s, cull_rebuilds_s;
-  float cull_delta, cull_cap, cull_delta_s;
+  int cull_rebuild, cull_rebuilds, cull_rebuild_s, cull_rebuilds_s, cull_rebuild_t, cull_rebuilds_t;
+  float cull_delta, cull_cap, cull_delta_s, cull_delta_t;
 };
 
 enum { V_W = 0, V_G, V_P, V_WTRY, V_WBEST, V_GNEW, V_Q, V_HIST };   // rows of svec
@@ -69,17 +69,22 @@ struct StepArgs {
   int hist_cap;
   float* wref;         // weights the brick candidate lists were built at (culling only)
   float* wref_s;       // weights the super-tile lists were built at
+  float* wref_t;       // weights the CTA-tile lists were built at
   double* gram;        // [LB_CLUSTER_MAX] copies of { (2 hist_cap + 1)^2 Gram matrix, hist_cap rho }, see GramSmem
 };
 
 constexpr double CULL_DELTA_FACTOR = 4.0;   // slack of a rebuilt list = this x the last change of the weights ...
 constexpr double CULL_CAP_FACTOR = 0.5;     // ... but at most this x the mean min-cost of the first evaluation (a larger
                                             // slack would lengthen every list by more than it saves in rebuilds)
-constexpr double CULL_SUPER_FACTOR = 8.0;   // slack of a rebuilt super-tile list = this x the brick lists': a super-tile's
-                                            // bounds are loose anyway, so its list barely grows and it is rebuilt far less
-                                            // often.  Measured (cfg 4 / cfg 5 solve; super-tile rebuilds of 59 / 61 brick
-                                            // rebuilds): x1 (one slack for both) 59 / 61, 25.0 / 107 ms; x4 27 / 28, 23.7 /
-                                            // 99.9; x8 12 / 11, 23.3 / 96.7; x16 6 / 6, 23.3 / 97.1; x64 2 / 2, 24.5 / 106.6
+// The three list levels keep slacks of their own: a brick list is cut from its CTA tile's list, that from its
+// super-tile's, and the coarser a box the looser its bounds, so a coarser list barely grows with a larger slack while
+// it is rebuilt far less often.  Measured (cfg 4 / cfg 5 solve, 59 / 61 brick rebuilds in 163 / 147 evaluations), before
+// programmatic dependent launch: one slack for all levels 25.0 / 107 ms; super x4 23.7 / 99.9 (27 / 28 super-tile
+// rebuilds); x8 23.3 / 96.7 (12 / 11); x16 23.3 / 97.1; x64 24.5 / 106.6.  With it, super x16 and the CTA-tile lists kept
+// in global memory: tile x2 22.1 / 99.3 (56 tile rebuilds), x3 21.5 / 96.1 (38), x4 21.1 / 94.7 (27), x6 21.0 / 93.0
+// (17 / 14), x8 (super x24) 21.0 / 93.7, x12 (x32) 21.6 / 96.7, x24 (x64) 23.8 / 111.
+constexpr double CULL_TILE_FACTOR = 6.0;    // slack of a rebuilt CTA-tile list = this x the brick lists'
+constexpr double CULL_SUPER_FACTOR = 16.0;  // slack of a rebuilt super-tile list = this x the brick lists' (>= the tile factor)
 
 // ---- reductions over the CLUSTER ------------------------------------------------------------------------------
 // The step kernel is ONE thread-block cluster of nranks = 8 or 16 CTAs (one per SM): a single CTA cannot keep enough loads
@@ -471,7 +476,7 @@ struct TrialArgs {
   double alpha;
 };
 __device__ void combine_and_trial(const StepArgs& a, int cap, const DirCoef& dc, const TrialArgs& ta,
-                                  const PushArgs& pu, Reducer& r, double* gp_out, double (&mx_out)[3]) {
+                                  const PushArgs& pu, Reducer& r, double* gp_out, double (&mx_out)[4]) {
   const int M = a.M, stride = a.stride, hl = dc.hl;
   double* g = a.vec + (size_t)V_G * stride;
   double* p = a.vec + (size_t)V_P * stride;
@@ -482,12 +487,12 @@ __device__ void combine_and_trial(const StepArgs& a, int cap, const DirCoef& dc,
   double* S = a.vec + (size_t)V_HIST * stride;
   double* Y = S + (size_t)cap * stride;
   const double dg = dc.delta[2 * hl];
-  double red3[4] = {0.0, 0.0, 0.0, 0.0}; // g.p | max |change since the last evaluation|, |distance from wref|, from wref_s
+  double red3[5] = {0.0, 0.0, 0.0, 0.0, 0.0}; // g.p | max |change since the last evaluation|, |distance from wref|, wref_s, wref_t
   constexpr int NC = LB_COMB_SLOTS, U = LB_COMB_U;
   const int LB_STEP_R = LB_STEP_OF(r);
   for (int i0 = LB_FIRST(r); i0 < M; i0 += U * LB_STEP_R) {
     double gi[U], wi[U], we[U], sn[U], yn[U], acc[U];
-    float w32_old[U], wref[U], wref_s[U];
+    float w32_old[U], wref[U], wref_s[U], wref_t[U];
     int idx[U];
 #pragma unroll
     for (int u = 0; u < U; ++u) {
@@ -495,7 +500,7 @@ __device__ void combine_and_trial(const StepArgs& a, int cap, const DirCoef& dc,
       idx[u] = i < M ? i : i0;                    // past the end: a duplicate of the first element, never stored
       const int ii = idx[u];
       we[u] = ta.improved ? ta.w_eval[ii] : 0.0;
-      w32_old[u] = a.w32[ii]; wref[u] = a.wref[ii]; wref_s[u] = a.wref_s[ii];
+      w32_old[u] = a.w32[ii]; wref[u] = a.wref[ii]; wref_s[u] = a.wref_s[ii]; wref_t[u] = a.wref_t[ii];
       if (pu.on) {
         const double gn = gnew[ii];
         sn[u] = __dmul_rn(pu.alpha_old, p[ii]); yn[u] = __dsub_rn(gn, g[ii]);
@@ -546,12 +551,13 @@ __device__ void combine_and_trial(const StepArgs& a, int cap, const DirCoef& dc,
         red3[1] = fmax(red3[1], fabs((double)wn - (double)w32_old[u]));      // differences of floats: exact in fp64
         red3[2] = fmax(red3[2], fabs((double)wn - (double)wref[u]));
         red3[3] = fmax(red3[3], fabs((double)wn - (double)wref_s[u]));
+        red3[4] = fmax(red3[4], fabs((double)wn - (double)wref_t[u]));
         a.w32[i] = wn;
       }
     }
   }
-  cluster_all_mixed<4, 3>(red3, r);
-  *gp_out = red3[0]; mx_out[0] = red3[1]; mx_out[1] = red3[2]; mx_out[2] = red3[3];
+  cluster_all_mixed<5, 4>(red3, r);
+  *gp_out = red3[0]; mx_out[0] = red3[1]; mx_out[1] = red3[2]; mx_out[2] = red3[3]; mx_out[3] = red3[4];
 }
 
 __global__ void solve_init_kernel(StepArgs a, const float* w_init, int hist_cap, int max_iters, int max_evals,
@@ -563,11 +569,13 @@ __global__ void solve_init_kernel(StepArgs a, const float* w_init, int hist_cap,
     a.w32[i] = (float)w;
     a.wref[i] = (float)w;
     a.wref_s[i] = (float)w;
+    a.wref_t[i] = (float)w;
   }
   if (i == 0) {
     SolveState* st = a.st;
     st->cull_rebuild = 1; st->cull_rebuilds = 1; st->cull_delta = 0.0f; st->cull_cap = 0.0f;
     st->cull_rebuild_s = 1; st->cull_rebuilds_s = 1; st->cull_delta_s = 0.0f;
+    st->cull_rebuild_t = 1; st->cull_rebuilds_t = 1; st->cull_delta_t = 0.0f;
     st->done = 0; st->phase = 0; st->iters = 0; st->evals = 0; st->trial = 0;
     st->hist_len = 0; st->hist_start = 0; st->hist_cap = hist_cap;
     st->max_iters = max_iters; st->max_evals = max_evals;
@@ -613,8 +621,8 @@ __global__ void __launch_bounds__(LB_THREADS) lbfgs_step_kernel(StepArgs a) {
   const double eps = st->eps, domain_volume = st->domain_volume;
   double best_err = st->best_err, best_dual = st->best_dual;
   float cull_cap = st->cull_cap;
-  const float cull_delta_old = st->cull_delta, cull_delta_s_old = st->cull_delta_s;
-  const int cull_rebuilds_old = st->cull_rebuilds, cull_rebuilds_s_old = st->cull_rebuilds_s;
+  const float cull_delta_old = st->cull_delta, cull_delta_s_old = st->cull_delta_s, cull_delta_t_old = st->cull_delta_t;
+  const int cull_rebuilds_old = st->cull_rebuilds, cull_rebuilds_s_old = st->cull_rebuilds_s, cull_rebuilds_t_old = st->cull_rebuilds_t;
 
   // the Gram matrix of the history: fetched now, stored to shared memory after the layer sums (whose loads hide the
   // latency), patched and used after the decision
@@ -683,7 +691,7 @@ __global__ void __launch_bounds__(LB_THREADS) lbfgs_step_kernel(StepArgs a) {
 
   int finish = 0;          // 1: OK at w_eval, 2: NOT_CONVERGED at best, 3: bad target volumes
   bool need_direction = false;
-  double mx[3] = {0.0, 0.0, 0.0};   // max |change of fl32 w since the last evaluation|, |distance from wref|, from wref_s
+  double mx[4] = {0.0, 0.0, 0.0, 0.0};   // max |change of fl32 w since the last evaluation|, |distance from wref|, wref_s, wref_t
   int new_slot = -1;       // ring slot a curvature pair is pushed into by this call, else -1
   bool evicts = false;     // ... and that slot held the oldest pair (the ring was full)
   bool accepted = false;
@@ -781,8 +789,8 @@ __global__ void __launch_bounds__(LB_THREADS) lbfgs_step_kernel(StepArgs a) {
     }
   }
 
-  int cull_rebuild = 1, cull_rebuild_s = 1;
-  float cull_delta = 0.0f, cull_delta_s = 0.0f;
+  int cull_rebuild = 1, cull_rebuild_s = 1, cull_rebuild_t = 1;
+  float cull_delta = 0.0f, cull_delta_s = 0.0f, cull_delta_t = 0.0f;
   if (finish == 0) {
     if (!need_direction) {
       // next trial point w + alpha p of the line search, rounded to fp32 for the evaluation (S10)
@@ -794,23 +802,30 @@ __global__ void __launch_bounds__(LB_THREADS) lbfgs_step_kernel(StepArgs a) {
         mx[0] = fmax(mx[0], fabs((double)wn - (double)a.w32[i]));     // differences of floats: exact in fp64
         mx[1] = fmax(mx[1], fabs((double)wn - (double)a.wref[i]));
         mx[2] = fmax(mx[2], fabs((double)wn - (double)a.wref_s[i]));
+        mx[3] = fmax(mx[3], fabs((double)wn - (double)a.wref_t[i]));
         a.w32[i] = wn;
       }
-      cluster_all<3, true>(mx, red);
+      cluster_all<4, true>(mx, red);
     }
-    cull_delta = cull_delta_old; cull_delta_s = cull_delta_s_old;
+    cull_delta = cull_delta_old; cull_delta_s = cull_delta_s_old; cull_delta_t = cull_delta_t_old;
     cull_rebuild = !(mx[1] <= (double)cull_delta);
-    cull_rebuild_s = 0;
+    cull_rebuild_s = 0; cull_rebuild_t = 0;
     if (cull_rebuild) {
       // the next evaluation rebuilds its brick lists at the new weights, valid within delta of them; they are cut from
-      // the super-tile lists, which must hold on that whole ball: (distance from wref_s) + delta <= delta_s, else
-      // those are rebuilt too, with a slack CULL_SUPER_FACTOR times as large (sums of floats: exact in fp64)
+      // the CTA-tile lists, which must hold on that whole ball: (distance from wref_t) + delta <= delta_t, else those
+      // are rebuilt too, with a slack CULL_TILE_FACTOR times as large, from the super-tile lists, which must hold on
+      // THAT ball, else ... (sums of floats: exact in fp64)
       cull_delta = fminf((float)(CULL_DELTA_FACTOR * mx[0]), cull_cap);
-      cull_rebuild_s = !(mx[2] + (double)cull_delta <= (double)cull_delta_s);
-      if (cull_rebuild_s) cull_delta_s = (float)(CULL_SUPER_FACTOR * (double)cull_delta);
+      cull_rebuild_t = !(mx[3] + (double)cull_delta <= (double)cull_delta_t);
+      if (cull_rebuild_t) {
+        cull_delta_t = (float)(CULL_TILE_FACTOR * (double)cull_delta);
+        cull_rebuild_s = !(mx[2] + (double)cull_delta_t <= (double)cull_delta_s);
+        if (cull_rebuild_s) cull_delta_s = (float)(CULL_SUPER_FACTOR * (double)cull_delta);
+      }
       for (int i = LB_FIRST(red); i < M; i += LB_STEP_R) {
         const float wn = a.w32[i];
         a.wref[i] = wn;
+        if (cull_rebuild_t) a.wref_t[i] = wn;
         if (cull_rebuild_s) a.wref_s[i] = wn;
       }
     }
@@ -830,6 +845,8 @@ __global__ void __launch_bounds__(LB_THREADS) lbfgs_step_kernel(StepArgs a) {
     st->best_err = best_err; st->best_dual = best_dual;
     st->cull_cap = cull_cap; st->cull_rebuild = cull_rebuild; st->cull_delta = cull_delta;
     st->cull_rebuild_s = cull_rebuild_s; st->cull_delta_s = cull_delta_s;
+    st->cull_rebuild_t = cull_rebuild_t; st->cull_delta_t = cull_delta_t;
+    st->cull_rebuilds_t = cull_rebuilds_t_old + (finish == 0 && cull_rebuild_t);
     st->cull_rebuilds = cull_rebuilds_old + (finish == 0 && cull_rebuild);
     st->cull_rebuilds_s = cull_rebuilds_s_old + (finish == 0 && cull_rebuild_s);
     if (finish) {
@@ -838,7 +855,7 @@ __global__ void __launch_bounds__(LB_THREADS) lbfgs_step_kernel(StepArgs a) {
       a.report->iters = iters; a.report->evals = evals;
       a.report->err = (finish == 2) ? best_err : err1;
       a.report->dual = (finish == 2) ? best_dual : -f1;
-      a.report->cull_rebuilds = st->cull_rebuilds; a.report->cull_rebuilds_s = st->cull_rebuilds_s;
+      a.report->cull_rebuilds = st->cull_rebuilds; a.report->cull_rebuilds_s = st->cull_rebuilds_s; a.report->cull_rebuilds_t = st->cull_rebuilds_t;
       __threadfence_system();
       a.report->done = 1;
       __threadfence_system();
@@ -867,6 +884,7 @@ int apd::ensure_solve_state(apd_ctx* ctx, int hist) {
     LB_TRY(cudaMalloc(&ws.w32, ms * sizeof(float)));
     LB_TRY(cudaMalloc(&ws.wref, ms * sizeof(float)));
     LB_TRY(cudaMalloc(&ws.wref_s, ms * sizeof(float)));
+    LB_TRY(cudaMalloc(&ws.wref_t, ms * sizeof(float)));
     LB_TRY(cudaMalloc(&ws.e_vol, ms * sizeof(double)));
     LB_TRY(cudaMalloc(&ws.e_scal, 2 * sizeof(double)));
     LB_TRY(cudaMalloc(&ws.hist, 2 * (size_t)SOLVE_HIST_CAP * sizeof(double)));
@@ -922,7 +940,7 @@ static int solve_common(apd_ctx* ctx, const char* who, int dim, int32_t M, const
   const double ell = std::pow(domain / (double)M, 1.0 / (double)dim);
   const double gamma0 = std::pow(ell, (double)(2 - dim)) / (double)dim;
   sa.st = ws.sstate; sa.vec = ws.svec; sa.stride = ws.max_seeds; sa.M = M; sa.v = target_vol; sa.w32 = ws.w32;
-  sa.hist = ws.hist; sa.hist_cap = SOLVE_HIST_CAP; sa.wref = ws.wref; sa.wref_s = ws.wref_s; sa.gram = ws.gram;
+  sa.hist = ws.hist; sa.hist_cap = SOLVE_HIST_CAP; sa.wref = ws.wref; sa.wref_s = ws.wref_s; sa.wref_t = ws.wref_t; sa.gram = ws.gram;
   ws.hist_len = 0;
   SolveReport* dev_report = nullptr;
   LB_TRY(cudaHostGetDevicePointer((void**)&dev_report, ws.report, 0));
@@ -1052,7 +1070,8 @@ int apd::solve_grid(apd_ctx* ctx, const char* who, const apd_grid* grid, const a
   hooks.loop_eval = [&](const int* done_flag) -> int {
     int r = enqueue_evaluation(ctx, g, kernel, M, X, A, ws.w32, target_vol, nullptr, nullptr, nullptr, nullptr, nullptr,
                                nullptr, false, o.cull != 0, done_flag, st, &ws.sstate->cull_rebuild,
-                               &ws.sstate->cull_delta, &ws.sstate->cull_rebuild_s, &ws.sstate->cull_delta_s);
+                               &ws.sstate->cull_delta, &ws.sstate->cull_rebuild_s, &ws.sstate->cull_delta_s,
+                               &ws.sstate->cull_rebuild_t, &ws.sstate->cull_delta_t);
     if (r == APD_OK && slab) r = exchange(false, done_flag);
     return r;
   };
