@@ -213,7 +213,8 @@ def executed_flop_per_pair(kernel: int, dim: int, row_long: int) -> float:
                   alone (2 FADD + 2 FMUL + 1 FFMA = 6 flop)                     -> 12.75   (the written form is 18)
       DIRECT 2D : per pair 1 FADD + 1 FMUL + 3 FFMA = 8, + (1 FADD + 1 FMUL) / 8            ->  8.25
       ROWPOLY   : 1.5 FMA per pair + 7 (3D) / 9 (2D) packed set-up operations per (row of V voxels, seed), V = 32 or 16
-      TENSOR    : the K = 32 bf16 contraction the tensor core executes = 64 flop (the method's 10 monomials are 20)"""
+      TENSOR    : the K = 32 bf16 contraction the tensor core executes = 64 flop (the method's 10 monomials are 20;
+                  in 2D 6 monomials = 12)"""
     if kernel == K_DIRECT:
         return 12.75 if dim == 3 else 8.25
     if kernel == K_ROWPOLY:
@@ -344,9 +345,10 @@ def kernel_record(b: Bench, kernel: int, cull: int, flush, reps: int, peak_fp32:
     if k == K_TENSOR:
         min_rate = 0.5 * wl.pairs / (km * 1e-3)                     # 3-input min instructions (thread level) per s
         alu_peak = sm_count * ALU_LANES_PER_SM * sm_mhz * 1e6
+        method_flop = 20.0 if wl.dim == 3 else 12.0                 # 10 (3D) / 6 (2D) monomials
         rec.update(tensor_tflops_k32=ach, frac_bf16_k32=ach / peak_bf16,
-                   tensor_tflops_method=20.0 * wl.pairs / (km * 1e-3) / 1e12,
-                   frac_bf16_method=20.0 * wl.pairs / (km * 1e-3) / 1e12 / peak_bf16,
+                   tensor_tflops_method=method_flop * wl.pairs / (km * 1e-3) / 1e12,
+                   frac_bf16_method=method_flop * wl.pairs / (km * 1e-3) / 1e12 / peak_bf16,
                    alu_min_frac=min_rate / alu_peak)
     else:
         rec.update(fp32_tflops=ach, frac_fp32=ach / peak_fp32)
@@ -372,7 +374,8 @@ def config_record(apd, torch, cfg: int, local: int, flush, args, peaks_t, full: 
             for k, name in ((K_DIRECT, "direct"), (K_ROWPOLY, "rowpoly"), (K_TENSOR, "tensor")):
                 out["assign_" + name] = kernel_record(b, k, 0, flush, 3, *peaks_t)
         else:
-            out["assign_direct"] = kernel_record(b, K_DIRECT, 0, flush, 3, *peaks_t)
+            for k, name in ((K_DIRECT, "direct"), (K_ROWPOLY, "rowpoly"), (K_TENSOR, "tensor")):
+                out["assign_" + name] = kernel_record(b, k, 0, flush, 3, *peaks_t)
         if not args.no_cpu:
             if args.oracle_full and cfg <= 4:
                 out["oracle"] = oracle_full_time(wl)
@@ -553,10 +556,13 @@ def run_ours(args):
         del b
         torch.cuda.empty_cache()
         if not args.no_per_config:
-            # a 2D workload large enough for ROWPOLY's long rows (cfg 2's recipe on 2048^2 pixels x 5000 grains)
+            # a 2D workload large enough for ROWPOLY's long rows (cfg 2's recipe on 2048^2 pixels x 5000 grains):
+            # what AUTO runs (the tensor-core kernel on 32 x 16-pixel tiles) and the CUDA-core ROWPOLY kernel beside it
             b2 = Bench(apd, torch, 2, local, n=(2048, 2048), M=5000)
             extra["assign_2d"] = dict(workload="cfg2 recipe on 2048x2048 pixels x 5000 grains",
                                       **kernel_record(b2, K_AUTO, 0, flush, 5, *peaks_t))
+            extra["assign_2d_rowpoly"] = dict(workload="cfg2 recipe on 2048x2048 pixels x 5000 grains",
+                                              **kernel_record(b2, K_ROWPOLY, 0, flush, 5, *peaks_t))
             b2.close()
             del b2
             extra["per_config"] = {str(c): config_record(apd, torch, c, local, flush, args, peaks_t, full=False)

@@ -48,7 +48,7 @@ typedef struct {
 /* Which implementation of the voxel x seed reduction runs (all give labels by the same rule:
  * fp32 cost, lowest seed index among equal fp32 costs). */
 enum {
-  APD_KERNEL_AUTO   = 0,   /* the fastest one for the call: brute force in 3D APD_KERNEL_TENSOR; in 2D and with
+  APD_KERNEL_AUTO   = 0,   /* the fastest one for the call: brute force APD_KERNEL_TENSOR (2D and 3D); with
                               opts.cull APD_KERNEL_ROWPOLY.  Grids with n[0] < 8 (3D also n[1] < 8 or n[2] < 4) take
                               APD_KERNEL_DIRECT (and ignore opts.cull): the row kernels expand the cost about the
                               midpoint of a row / tile, which there lies up to 8/n domain widths L outside the
@@ -59,7 +59,7 @@ enum {
   APD_KERNEL_ROWPOLY = 2,  /* quadratic in the offset from the row's midpoint (1.5 FMA per pair) with
                               coefficients polynomial in the row's offset from the tile's midpoint,
                               packed f32x2, deferred argmin                                        */
-  APD_KERNEL_TENSOR = 3    /* 3D only, brute force only (no opts.cull): the cost lifted to a 10-monomial
+  APD_KERNEL_TENSOR = 3    /* brute force only (no opts.cull): the cost lifted to a 10-monomial (2D: 6)
                               polynomial in the integer voxel offset from a tile's reference voxel,
                               coefficients split three ways into bf16, contracted on the tensor
                               cores (tcgen05.mma, fp32 accumulators in TMEM); argmin epilogue on

@@ -159,16 +159,16 @@ static bool narrow_grid(const apd_grid* grid) {
 int resolve_kernel(const apd_ctx* /*ctx*/, const apd_opts* o, const apd_grid* grid, int /*M*/, bool* cull, std::string* err) {
   int k = o ? o->kernel : APD_KERNEL_AUTO;
   if (k != APD_KERNEL_AUTO && k != APD_KERNEL_DIRECT && k != APD_KERNEL_ROWPOLY && k != APD_KERNEL_TENSOR) { *err = "unknown opts.kernel"; return -1; }
-  if (k == APD_KERNEL_TENSOR && grid && grid->dim != 3) { *err = "APD_KERNEL_TENSOR is 3D only"; return -1; }
   if (o && (o->cull != 0 && o->cull != 1)) { *err = "opts.cull must be 0 or 1"; return -1; }
   if (o && (o->reserved[0] || o->reserved[1] || o->reserved[2])) { *err = "opts.reserved must be 0"; return -1; }
   *cull = o && o->cull;
   if (k == APD_KERNEL_AUTO) {
     if (narrow_grid(grid)) { *cull = false; return APD_KERNEL_DIRECT; }
     k = APD_KERNEL_ROWPOLY;
-    // brute force in 3D: the tensor-core kernel.  Measured on B200 with the persistent kernel: TENSOR /
-    // ROWPOLY time 0.22-0.88 on every grid and seed count tried (32^3 .. 256^3 voxels, M = 64 .. 10^4).
-    if (grid && grid->dim == 3 && !*cull) k = APD_KERNEL_TENSOR;
+    // brute force: the tensor-core kernel.  Measured on B200 with the persistent kernel: TENSOR /
+    // ROWPOLY time 0.22-0.88 on every 3D grid and seed count tried (32^3 .. 256^3 voxels, M = 64 .. 10^4), and
+    // 0.42-0.83 in 2D (64^2 x 10 .. 4096^2 x 1000; 1024^2 x 1000: 0.65, 2048^2 x 5000: 0.70).
+    if (grid && !*cull) k = APD_KERNEL_TENSOR;
   }
   if (*cull && k != APD_KERNEL_ROWPOLY) { *err = "opts.cull needs kernel AUTO or ROWPOLY"; return -1; }
   return k;
@@ -339,7 +339,7 @@ extern "C" int apd_reserve(apd_ctx* ctx, const apd_grid* grid, const apd_opts* o
   APD_CUDA_TRY(ctx, cudaSetDevice(ctx->ws.device));
   int rc = ensure_eval_buffers(ctx, g, kernel, cull, nullptr);
   if (rc != APD_OK) return rc;
-  if ((!opts || opts->kernel == APD_KERNEL_AUTO) && grid->dim == 3 && !cull) {
+  if ((!opts || opts->kernel == APD_KERNEL_AUTO) && !cull) {
     // AUTO picks ROWPOLY or TENSOR by the number of seeds of the call: size the workspace for both
     for (int k2 : {APD_KERNEL_ROWPOLY, APD_KERNEL_TENSOR}) {
       GridDev g2;

@@ -142,7 +142,7 @@ cudaError_t launch_pack_pairs(int dim, int M, int M_pad, const float* X, const f
                               const int* done_flag, cudaStream_t st);
 cudaError_t launch_assign_rowpoly(const AssignArgs& a, cudaStream_t st);
 // TENSOR kernel (apd_tensor.cu, row a8): reads the DIRECT record table plus its own bf16 table
-void tensor_tile_counts(int nx, int ny, int nz, int* tx, int* ty, int* tz);
+void tensor_tile_counts(int dim, int nx, int ny, int nz, int* tx, int* ty, int* tz);
 cudaError_t launch_pack_qfix(const GridDev& g, int M_pad, const float* rec, uint4* qfix, const int* done_flag,
                              cudaStream_t st);
 cudaError_t launch_assign_tensor(const AssignArgs& a, cudaStream_t st);

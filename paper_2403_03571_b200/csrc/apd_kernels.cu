@@ -210,7 +210,7 @@ static inline int cdiv(int a, int b) { return (a + b - 1) / b; }
 // Returns the ROWPOLY row-length choice (0 for the DIRECT kernel).
 int assign_tile_counts(int kernel, int dim, int nx, int ny, int nz, int sm_count, bool cull, int* tx, int* ty, int* tz) {
   if (kernel == APD_KERNEL_ROWPOLY) return rowpoly_tile_counts(dim, nx, ny, nz, sm_count, cull, tx, ty, tz);
-  if (kernel == APD_KERNEL_TENSOR) { tensor_tile_counts(nx, ny, nz, tx, ty, tz); return 0; }
+  if (kernel == APD_KERNEL_TENSOR) { tensor_tile_counts(dim, nx, ny, nz, tx, ty, tz); return 0; }
   if (dim == 3) {
     using G = DirectGeom<3>;
     *tx = cdiv(nx, G::TXT * G::V); *ty = cdiv(ny, G::TYT); *tz = cdiv(nz, G::TZT);

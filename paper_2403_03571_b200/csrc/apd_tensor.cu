@@ -1,6 +1,6 @@
 // apd_tensor.cu -- row a8 of the path: the cost matrix of Algorithm 1 step 1 (PAPER.md:131,
 // eq. 2.1 at PAPER.md:58-61) lifted to a bf16 tensor-core contraction, the argmin of step 2 as the
-// epilogue.  3D only.
+// epilogue.  3D, and 2D as the special case without z (tile 32 x 16 pixels; 6 of the 10 monomials are non-zero).
 //
 // For a voxel at INTEGER offset t = (i, j, k) from the reference voxel y0 of its tile and a seed x with matrix A,
 //     C(t) = sum_{m<=n} a'_mn s_m s_n t_m t_n  +  sum_m (g_m s_m) t_m  +  r0,
@@ -29,10 +29,15 @@
 
 namespace apd {
 
-constexpr int TC_TX = 16, TC_TY = 8, TC_TZ = 4;      // voxel tile
+// voxel tile: 512 voxels = 4 M-tiles of 128 (thread tid <-> voxel: x fastest, then y, then z).  |offset from the
+// reference voxel| <= 16, 8, 4: every monomial <= 256 in magnitude, exact in bf16
+template <int DIM> struct TcGeom;
+template <> struct TcGeom<3> { static constexpr int TX = 16, TY = 8, TZ = 4; };
+template <> struct TcGeom<2> { static constexpr int TX = 32, TY = 16, TZ = 1; };
 constexpr int TC_N = 128;                             // seeds per chunk = N of one tcgen05.mma (N >= 128: below that an
                                                       // MMA costs ~45 cycles whatever its N -- measured)
-constexpr int TC_EPI_THREADS = TC_TX * TC_TY * TC_TZ; // 512: one per voxel
+constexpr int TC_EPI_THREADS = 512;                   // one per voxel of the tile
+static_assert(TcGeom<3>::TX * TcGeom<3>::TY * TcGeom<3>::TZ == TC_EPI_THREADS && TcGeom<2>::TX * TcGeom<2>::TY == TC_EPI_THREADS, "tile");
 constexpr int TC_BUILD_WARPS = 4;                     // 128 threads: one seed of every chunk each
 constexpr int TC_THREADS = TC_EPI_THREADS + 32 * TC_BUILD_WARPS + 64;   // + the MMA-issuing warp + the TMA warp
 constexpr int TC_QFIX = 24;                           // bf16 per seed in the tile-independent part (18 used)
@@ -161,12 +166,22 @@ __device__ __forceinline__ float bf_hi(uint32_t v) { return __uint_as_float(v & 
 
 // ---- TENSOR seed table: the DIRECT record (12 fp32) followed by the tile-independent part of Theta, the six
 //      quadratic coefficients in voxel units split three ways (18 bf16, padded to 24) --------------------------------
-__global__ void pack_qfix_kernel(int M_pad, const float* __restrict__ rec, double sx, double sy, double sz,
+__global__ void pack_qfix_kernel(int dim, int M_pad, const float* __restrict__ rec, double sx, double sy, double sz,
                                  uint4* __restrict__ tcs, const int* __restrict__ done_flag) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= M_pad) return;
   if (done_flag && *done_flag) return;
-  const float* r = rec + (size_t)i * REC3;
+  // 2D: the record (x, y, a11, a12', a22, -w) becomes the 3D one with z = 0 and no z-terms
+  __align__(16) float r[REC3];
+  if (dim == 3) {
+#pragma unroll
+    for (int k = 0; k < REC3; ++k) r[k] = rec[(size_t)i * REC3 + k];
+  } else {
+    const float* p = rec + (size_t)i * REC2;
+#pragma unroll
+    for (int k = 0; k < REC3; ++k) r[k] = 0.0f;
+    r[0] = p[0]; r[1] = p[1]; r[3] = p[2]; r[4] = p[3]; r[6] = p[4]; r[9] = p[5];
+  }
   const float q[6] = {(float)((double)r[3] * sx * sx), (float)((double)r[6] * sy * sy), (float)((double)r[8] * sz * sz),
                       (float)((double)r[4] * sx * sy), (float)((double)r[5] * sx * sz), (float)((double)r[7] * sy * sz)};
   unsigned short b[TC_QFIX];
@@ -224,9 +239,11 @@ __device__ __forceinline__ void tc_build_seed(const TcSeedRegs& s, bool real, fl
 }
 
 // Writes the Phi rows (A operand) of the CTA's 512 voxels for a tile whose reference voxel is (rx, ry, rz).
+template <int DIM>
 __device__ __forceinline__ void tc_write_phi(unsigned char* s_A, int tid, int rx, int ry, int rz) {
+  using TG = TcGeom<DIM>;
   // Phi row of this thread's voxel: monomials of the integer offsets, each under its three coefficient parts
-  const int ti = (tid & 15) - rx, tj = ((tid >> 4) & 7) - ry, tk = (tid >> 7) - rz;
+  const int ti = (tid % TG::TX) - rx, tj = ((tid / TG::TX) % TG::TY) - ry, tk = (tid / (TG::TX * TG::TY)) - rz;
   const float mono[10] = {(float)(ti * ti), (float)(tj * tj), (float)(tk * tk), (float)(ti * tj), (float)(ti * tk),
                           (float)(tj * tk), (float)ti, (float)tj, (float)tk, 1.0f};
   unsigned short e[32];
@@ -279,7 +296,9 @@ __device__ __forceinline__ void tc_issue_chunk(int G, uint32_t tmem, uint64_t ad
 // epilogue warps still store the labels of the current one: no pipeline fill / drain per tile (it was ~3 of a tile's
 // 79 chunks at cfg 4, ~3 of 8 at cfg 3).  A tile whose reference voxel differs (ragged edge) drains the pipeline with
 // two CTA barriers and rewrites Phi.
+template <int DIM>
 __global__ void __launch_bounds__(TC_THREADS, 1) assign_tensor_kernel(const AssignArgs a) {
+  constexpr int TC_TX = TcGeom<DIM>::TX, TC_TY = TcGeom<DIM>::TY, TC_TZ = TcGeom<DIM>::TZ;
   extern __shared__ __align__(128) unsigned char tc_smem[];
   unsigned char* s_A = tc_smem;                                    // Phi: 4 M-tiles x 128 rows x 32 bf16
   unsigned char* s_th = tc_smem + TC_A_BYTES;                      // Theta ring: stages x 128 rows x 32 bf16
@@ -330,7 +349,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) assign_tensor_kernel(const Assi
   const int sig = rx | (ry << 8) | (rz << 16);                                                                         \
   if (sig != sig_cur) {                                                                                                \
     __syncthreads();                                                                                                   \
-    if (tid < TC_EPI_THREADS) tc_write_phi(s_A, tid, rx, ry, rz);                                                      \
+    if (tid < TC_EPI_THREADS) tc_write_phi<DIM>(s_A, tid, rx, ry, rz);                                                 \
     tc_fence_before();                                                                                                 \
     __syncthreads();                                                                                                   \
     tc_fence_after();                                                                                                  \
@@ -376,7 +395,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) assign_tensor_kernel(const Assi
       // reference voxel of the tile
       const float y0x = (float)(a.g.lo[0] + ((double)(bx * TC_TX + rx) + 0.5) * a.g.s[0]);
       const float y0y = (float)(a.g.lo[1] + ((double)(by * TC_TY + ry + a.g.off_y) + 0.5) * a.g.s[1]);
-      const float y0z = (float)(a.g.lo[2] + ((double)(bz * TC_TZ + rz + a.g.off_z) + 0.5) * a.g.s[2]);
+      const float y0z = (DIM == 3) ? (float)(a.g.lo[2] + ((double)(bz * TC_TZ + rz + a.g.off_z) + 0.5) * a.g.s[2]) : 0.0f;
       for (int c = 0; c < nch; ++c) {
         const int G = G0 + c, rs = G % TC_RAW_STAGES, ts = G % TC_TH_STAGES;
         mbar_wait(&s_raw_full[rs], (uint32_t)((G / TC_RAW_STAGES) & 1));
@@ -423,7 +442,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) assign_tensor_kernel(const Assi
 
       // a5 + a6: label store, warp-aggregated counts, index sums, fp64 sum of the minima
       double dsum = 0.0;
-      const int ix = bx * TC_TX + (tid & 15), iy = by * TC_TY + ((tid >> 4) & 7), iz = bz * TC_TZ + (tid >> 7);
+      const int ix = bx * TC_TX + (tid % TC_TX), iy = by * TC_TY + ((tid / TC_TX) % TC_TY), iz = bz * TC_TZ + tid / (TC_TX * TC_TY);
       const bool valid = ix < a.g.nx && iy < a.g.ny && iz < a.g.nz;
       const unsigned vmask = __ballot_sync(0xffffffffu, valid);
       // a voxel whose real costs are all NaN / +inf / >= 2^100 would keep a padding seed (cost 2^100) as its minimum:
@@ -462,27 +481,35 @@ __global__ void __launch_bounds__(TC_THREADS, 1) assign_tensor_kernel(const Assi
 }
 
 
-void tensor_tile_counts(int nx, int ny, int nz, int* tx, int* ty, int* tz) {
-  *tx = (nx + TC_TX - 1) / TC_TX; *ty = (ny + TC_TY - 1) / TC_TY; *tz = (nz + TC_TZ - 1) / TC_TZ;
+void tensor_tile_counts(int dim, int nx, int ny, int nz, int* tx, int* ty, int* tz) {
+  if (dim == 3) {
+    *tx = (nx + TcGeom<3>::TX - 1) / TcGeom<3>::TX; *ty = (ny + TcGeom<3>::TY - 1) / TcGeom<3>::TY; *tz = (nz + TcGeom<3>::TZ - 1) / TcGeom<3>::TZ;
+  } else {
+    *tx = (nx + TcGeom<2>::TX - 1) / TcGeom<2>::TX; *ty = (ny + TcGeom<2>::TY - 1) / TcGeom<2>::TY; *tz = 1;
+  }
 }
 
 cudaError_t launch_pack_qfix(const GridDev& g, int M_pad, const float* rec, uint4* qfix, const int* done_flag,
                              cudaStream_t st) {
-  pack_qfix_kernel<<<(M_pad + 127) / 128, 128, 0, st>>>(M_pad, rec, g.s[0], g.s[1], g.s[2], qfix, done_flag);
+  pack_qfix_kernel<<<(M_pad + 127) / 128, 128, 0, st>>>(g.dim, M_pad, rec, g.s[0], g.s[1], g.dim == 3 ? g.s[2] : 0.0, qfix, done_flag);
   return cudaGetLastError();
 }
 
-cudaError_t launch_assign_tensor(const AssignArgs& a, cudaStream_t st) {
+template <int DIM>
+static cudaError_t launch_assign_tensor_t(const AssignArgs& a, cudaStream_t st) {
   // per device and cheap: set on every launch (a process may drive several devices through several contexts)
-  cudaError_t e = cudaFuncSetAttribute(assign_tensor_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM);
+  cudaError_t e = cudaFuncSetAttribute(assign_tensor_kernel<DIM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM);
   if (e != cudaSuccess) return e;
   int dev = 0, sms = 0;
   if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
   if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
   const int n_tiles = a.g.tiles_x * a.g.tiles_y * a.g.tiles_z;
   const int n_ctas = n_tiles < sms ? n_tiles : sms;                 // persistent: one CTA per SM (112 KB smem, all of TMEM)
-  assign_tensor_kernel<<<n_ctas, TC_THREADS, TC_SMEM, st>>>(a);
+  assign_tensor_kernel<DIM><<<n_ctas, TC_THREADS, TC_SMEM, st>>>(a);
   return cudaGetLastError();
+}
+cudaError_t launch_assign_tensor(const AssignArgs& a, cudaStream_t st) {
+  return a.g.dim == 3 ? launch_assign_tensor_t<3>(a, st) : launch_assign_tensor_t<2>(a, st);
 }
 
 }  // namespace apd

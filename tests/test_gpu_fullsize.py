@@ -90,8 +90,10 @@ def test_long_rows_2d_full_grid(apd, case, kernel, cull):
                                aspect=4.0)
     r = run_with_stats(apd, wl, wl.w0, kernel, cull=cull, v=wl.v, want_centroids=True)
     st = r["stats"]
-    if kernel in (K_ROWPOLY, K_AUTO) and not cull:
+    if kernel == K_ROWPOLY and not cull:
         assert (st["kernel"], st["row_long"]) == (K_ROWPOLY, 1), st      # RowGeom2L: 64 x 64-pixel tiles
+    if kernel == K_AUTO:
+        assert st["kernel"] == K_TENSOR, st                              # 2D brute force: tiles of 32 x 16 pixels
     info = parity.check_assign(wl, wl.w0, r["labels"], r["vol"], r["dual"], v=wl.v, centroids_gpu=r["centroids"],
                                err_gpu=r["err"])
     print(f"2D {wl.n} kernel={kernel} cull={cull}: ran {st}; {info}")

@@ -32,8 +32,6 @@ CASES = [dict(dim=3, n=(52, 40, 44), lo=(0.0, -1.0, 0.5), hi=(1.3, 0.4, 1.6), M=
 @pytest.mark.parametrize("kernel,cull", [(1, 0), (2, 0), (2, 1), (3, 0), (0, 0)])
 @pytest.mark.parametrize("case", CASES, ids=lambda c: "x".join(map(str, c["n"])))
 def test_slab_counters_add_up_to_the_whole_grid_bit_for_bit(apd, case, kernel, cull):
-    if kernel == 3 and case["dim"] == 2:
-        pytest.skip("APD_KERNEL_TENSOR is 3D only")
     wl = workloads.make_random(case["dim"], case["n"], case["M"], 91, lo=case["lo"], hi=case["hi"], w_scale=0.1, aspect=4.0)
     ref = run_assign(apd, wl, wl.w0, v=wl.v, kernel=kernel, cull=cull, want_centroids=True)
     dev = torch.device("cuda:0")

@@ -123,8 +123,6 @@ def test_reduced_configs_trajectory(apd, cfg, n, M, eps, kernel, cull):
     agree exactly up to the first flip, the status must agree, and the oracle's own evaluation at the GPU's weights
     must meet the tolerance (check_against_oracle)."""
     wl = workloads.make_config(cfg, n=n, M=M)
-    if kernel == 3 and wl.dim == 2:
-        pytest.skip("APD_KERNEL_TENSOR is 3D only")
     orc = oracle_solve(parity.grid_of(wl), wl.X, wl.A, wl.v, eps, record=True)
     flips = flips_along_path(apd, wl, orc, kernel, cull)
     info, w32, w64, labels, vol, hist = run_solve(apd, wl, eps, kernel=kernel, cull=cull, want_hist=True)

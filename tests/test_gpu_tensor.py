@@ -51,6 +51,50 @@ def test_edge_cases(apd, case, nonsym):
                         err_gpu=r["err"])
 
 
+# ---- 2D: the same kernel on tiles of 32 x 16 pixels (6 of the 10 monomials are non-zero) ----------------------------
+
+@pytest.mark.parametrize("cfg,wscale", [(1, 0.0), (1, 0.1), (2, 0.0), (2, 0.002)])
+def test_2d_configs_full_parity(apd, cfg, wscale):
+    wl = workloads.make_config(cfg)
+    w = wl.w0 if wscale == 0.0 else rand_w(wl, wscale, 200 + cfg)
+    r = run_assign(apd, wl, w, v=wl.v, kernel=TENSOR, want_centroids=True)
+    info = parity.check_assign(wl, w, r["labels"], r["vol"], r["dual"], v=wl.v, centroids_gpu=r["centroids"],
+                               err_gpu=r["err"])
+    assert r["pairs"] == wl.N * wl.M
+    print(f"cfg{cfg} tensor 2D wscale={wscale}: {info}")
+
+
+EDGE2 = [
+    dict(n=(100, 70), M=130, lo=(0, 0), hi=(1, 1), seed=42),
+    dict(n=(33, 17), M=5, lo=(-1, 2), hi=(1, 5), seed=43),
+    dict(n=(5, 1), M=1, lo=(0, 0), hi=(1, 1), seed=45),
+    dict(n=(32, 16), M=2, lo=(0, 0), hi=(1, 1), seed=46),
+    dict(n=(33, 17), M=3, lo=(0, 0), hi=(2, 1), seed=47),
+    dict(n=(1, 40), M=7, lo=(0, 0), hi=(1, 3), seed=48),
+    dict(n=(257, 129), M=129, lo=(0, 0), hi=(1, 1), seed=49),
+    dict(n=(300, 200), M=1000, lo=(0, 0), hi=(1, 1), seed=50),
+]
+
+
+@pytest.mark.parametrize("case", EDGE2, ids=lambda c: f"{'x'.join(map(str, c['n']))}_M{c['M']}")
+@pytest.mark.parametrize("nonsym", [False, True])
+def test_2d_edge_cases(apd, case, nonsym):
+    wl = workloads.make_random(2, case["n"], case["M"], case["seed"], lo=case["lo"], hi=case["hi"], w_scale=0.1,
+                               nonsymmetric=nonsym)
+    r = run_assign(apd, wl, wl.w0, v=wl.v, kernel=TENSOR, want_centroids=True)
+    parity.check_assign(wl, wl.w0, r["labels"], r["vol"], r["dual"], v=wl.v, centroids_gpu=r["centroids"],
+                        err_gpu=r["err"])
+
+
+def test_2d_agrees_with_the_direct_kernel(apd):
+    wl = workloads.make_config(2)
+    w = rand_w(wl, 0.002, 77)
+    rt = run_assign(apd, wl, w, v=wl.v, kernel=TENSOR)
+    rd = run_assign(apd, wl, w, v=wl.v, kernel=DIRECT)
+    assert (rt["labels"] != rd["labels"]).sum() < 2e-5 * wl.N
+    assert abs(rt["dual"] - rd["dual"]) <= 1e-6 * abs(rd["dual"])
+
+
 def test_no_target_volume_no_labels_and_reproducible(apd):
     wl = workloads.make_random(3, (40, 24, 16), 50, 21, w_scale=0.1)
     r = run_assign(apd, wl, wl.w0, v=None, kernel=TENSOR)
@@ -113,13 +157,13 @@ def test_cfg4_full_size_sampled_parity(apd):
     print(f"cfg4 tensor sampled: {info}")
 
 
-def test_rejects_2d_and_culling(apd):
-    wl = workloads.make_config(1)
-    with pytest.raises(Exception):
-        run_assign(apd, wl, wl.w0, v=wl.v, kernel=TENSOR)
+def test_rejects_culling(apd):
     wl3 = workloads.make_random(3, (32, 32, 32), 20, 5)
     with pytest.raises(Exception):
         run_assign(apd, wl3, wl3.w0, v=wl3.v, kernel=TENSOR, cull=1)
+    wl2 = workloads.make_random(2, (64, 64), 20, 5)
+    with pytest.raises(Exception):
+        run_assign(apd, wl2, wl2.w0, v=wl2.v, kernel=TENSOR, cull=1)
 
 
 def test_solve_with_the_tensor_kernel_meets_the_tolerance(apd):
