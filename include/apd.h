@@ -290,6 +290,28 @@ int apd_solve_slab(apd_ctx* ctx, const apd_grid* grid, const apd_slab* slab, int
                    uint64_t* counters, apd_reduce_fn reduce, void* user, int32_t* iters, int32_t* evals,
                    double* max_rel_err, double* dual, const apd_opts* opts, void* cuda_stream);
 
+/* The input checks the hot path does NOT make (a debug call).  PAPER.md:51-54 assumes every A_i
+ * symmetric positive definite -- apd_assign evaluates the quadratic form of whatever matrix it is given (reading S13),
+ * but the culling bounds of opts.cull hold only for positive definite A_i -- and PAPER.md:65-69 target volumes
+ * v_i > 0 that sum to |Omega|.
+ *   X [M,dim], A [M,dim,dim]   DEVICE fp32 in, required
+ *   w [M], target_vol [M]      DEVICE fp32 in or NULL (not checked when NULL); target_vol needs `grid` (for |Omega|)
+ *   problems                   HOST out, required: 0 if every check passed, else the OR of APD_BAD_*
+ * One small kernel on `cuda_stream`; allocates 16 bytes and synchronises the stream (not for stream capture).
+ * Returns APD_OK whenever the checks ran (whatever they found); APD_E_ARG / APD_E_CUDA otherwise. */
+enum {
+  APD_BAD_X_NONFINITE             = 1,    /* a seed coordinate is NaN or +-inf                                   */
+  APD_BAD_A_NONFINITE             = 2,    /* an entry of some A_i is NaN or +-inf                                */
+  APD_BAD_A_NOT_SYMMETRIC         = 4,    /* |A_kl - A_lk| > 1e-6 max|A_i| for some i                            */
+  APD_BAD_A_NOT_POSITIVE_DEFINITE = 8,    /* a leading principal minor of (A_i + A_i^T)/2 is <= 0                */
+  APD_BAD_W_NONFINITE             = 16,   /* a weight is NaN or +-inf                                            */
+  APD_BAD_TARGET_VOL_NOT_POSITIVE = 32,   /* some v_i <= 0 or not finite                        */
+  APD_BAD_TARGET_VOL_SUM          = 64    /* |sum_i v_i - |Omega|| > 1e-6 |Omega|: apd_solve would
+                                             return APD_E_ARG                                                    */
+};
+int apd_validate(apd_ctx* ctx, const apd_grid* grid, int32_t M, const float* X, const float* A, const float* w,
+                 const float* target_vol, uint32_t* problems, void* cuda_stream);
+
 /* Grows the context's workspace to what apd_assign / apd_solve / apd_lloyd need on `grid` with `opts` (dual partials:
  * 8 bytes per tile; with opts.cull the candidate lists, 1 KiB per 512 voxels; L-BFGS state for opts.lbfgs_history),
  * so that those calls, on this grid or any grid with no more tiles, neither allocate nor synchronise.  Synchronous

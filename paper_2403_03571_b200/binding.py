@@ -26,6 +26,8 @@ KERNEL_AUTO = 0
 KERNEL_DIRECT = 1
 KERNEL_ROWPOLY = 2
 KERNEL_TENSOR = 3
+BAD_X_NONFINITE, BAD_A_NONFINITE, BAD_A_NOT_SYMMETRIC, BAD_A_NOT_POSITIVE_DEFINITE = 1, 2, 4, 8
+BAD_W_NONFINITE, BAD_TARGET_VOL_NOT_POSITIVE, BAD_TARGET_VOL_SUM = 16, 32, 64
 
 
 class ApdError(RuntimeError):
@@ -139,6 +141,9 @@ def load_library() -> ctypes.CDLL:
     lib.apd_static_scratch_bytes.argtypes = []
     lib.apd_static_last_error.restype = ctypes.c_char_p
     lib.apd_static_last_error.argtypes = []
+    lib.apd_validate.restype = ctypes.c_int
+    lib.apd_validate.argtypes = [_P, ctypes.POINTER(apd_grid), ctypes.c_int32, _P, _P, _P, _P,
+                                 ctypes.POINTER(ctypes.c_uint32), _P]
     _lib = lib
     return lib
 
@@ -147,7 +152,7 @@ EXPORTED_SYMBOLS = ["apd_default_opts", "apd_create", "apd_destroy", "apd_last_e
                     "apd_assign_host", "apd_solve_host", "apd_solve_history", "apd_assign_points", "apd_solve_points", "apd_solve_stats", "apd_lloyd", "apd_solve_refine", "apd_resolution_bound",
                     "apd_choose_resolution", "apd_reserve", "apd_assign_stats", "apd_slab_align", "apd_counter_words",
                     "apd_assign_slab", "apd_finalize_counters", "apd_solve_slab", "apd_solve_continuation",
-                    "apd_assign_static", "apd_static_scratch_bytes", "apd_static_last_error"]
+                    "apd_assign_static", "apd_static_scratch_bytes", "apd_static_last_error", "apd_validate"]
 
 
 def make_grid(dim: int, n: Sequence[int], lo: Sequence[float], hi: Sequence[float]) -> apd_grid:
@@ -472,6 +477,16 @@ class ApdContext:
         if n < 0:
             self._check(n)
         return np.array(d[:n], dtype=np.float64), np.array(e[:n], dtype=np.float64)
+
+    def validate(self, grid: Optional[apd_grid], X, A, w=None, target_vol=None) -> int:
+        """apd_validate of include/apd.h: 0, or the OR of the BAD_* flags."""
+        M, d = int(X.shape[0]), self.dim
+        out = ctypes.c_uint32(0)
+        self._check(self._lib.apd_validate(self._h, ctypes.byref(grid) if grid is not None else None, M,
+                                           _dev(X, torch.float32, "X", M * d), _dev(A, torch.float32, "A", M * d * d),
+                                           _dev(w, torch.float32, "w", M), _dev(target_vol, torch.float32, "target_vol", M),
+                                           ctypes.byref(out), self._stream()))
+        return int(out.value)
 
     def reserve(self, grid: apd_grid, opts: Optional[apd_opts] = None):
         """apd_reserve of include/apd.h: grow the workspace ahead of time."""

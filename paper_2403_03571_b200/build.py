@@ -16,7 +16,7 @@ _CSRC = os.path.join(_PKG, "csrc")
 LIB_PATH = os.path.join(_PKG, "libapd_b200.so")
 PROBE_LIB_PATH = os.path.join(_PKG, "libapd_probe.so")
 SOURCES = ["apd_api.cu", "apd_kernels.cu", "apd_rowpoly.cu", "apd_finalize.cu", "apd_lbfgs.cu",
-           "apd_host.cu", "apd_cull.cu", "apd_lloyd.cu", "apd_points.cu", "apd_tensor.cu", "apd_shard.cu", "apd_static.cu"]
+           "apd_host.cu", "apd_cull.cu", "apd_lloyd.cu", "apd_points.cu", "apd_tensor.cu", "apd_shard.cu", "apd_static.cu", "apd_validate.cu"]
 PROBE_SOURCES = [os.path.join("probe", "apd_probe.cu")]
 HEADERS = ["apd_internal.cuh", "apd_device.cuh", "apd_epilogue.cuh", os.path.join("..", "..", "include", "apd.h"),
            os.path.join("..", "..", "include", "apd_probe.h")]
