@@ -186,6 +186,16 @@ int apd_solve_points(apd_ctx* ctx, int64_t N, const float* Y, const float* pvol,
                      float* w, int32_t* labels, double* vol, int32_t* iters, int32_t* evals, double* max_rel_err,
                      const apd_opts* opts, void* cuda_stream);
 
+/* Algorithm 3 (generalised Lloyd) on a user-supplied discretisation: apd_lloyd (below) with every
+ * Algorithm 2 done by apd_solve_points and the centroid of a cell taken over its points, sum |P_j| y_j / sum |P_j|
+ * (an empty cell keeps its seed).  X [M,dim] DEVICE fp32 IN/OUT (X^0 on entry, X^K on return); the other arguments as
+ * apd_solve_points; iters / evals: totals over the K + 1 solves.  Blocks until finished.  Returns the status of the
+ * final Algorithm 2 (APD_OK / APD_NOT_CONVERGED) or a negative error. */
+int apd_lloyd_points(apd_ctx* ctx, int64_t N, const float* Y, const float* pvol, double total_volume, int32_t M,
+                     float* X, const float* A, const float* target_vol, double tol, int32_t K, const float* w_init,
+                     float* w, int32_t* labels, double* vol, int32_t* iters, int32_t* evals, double* max_rel_err,
+                     const apd_opts* opts, void* cuda_stream);
+
 /* Counters of the most recent apd_solve on this context (HOST out, each may be NULL): evaluations recorded by
  * apd_solve_history, and how many evaluations of the loop rebuilt the culling candidate lists (with opts.cull the
  * lists are built with a slack on the bounds and reused while the weights stay within it; 0 without culling). */

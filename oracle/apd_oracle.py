@@ -430,7 +430,10 @@ def oracle_lloyd(grid: Grid, X0, A, v, eps: float, K: int, w_init=None, **solve_
         evals += r.evals
         if k == K:
             return X, r, iters, evals
-        c = oracle_assign(grid, X, A, r.w32, v=v, diagnostics=False).centroids
+        if isinstance(grid, PointSet):      # user-supplied discretisation: centroid over the cell's points
+            c = oracle_assign_points(grid.Y, grid.pvol, X, A, r.w32, v=v).centroids
+        else:
+            c = oracle_assign(grid, X, A, r.w32, v=v, diagnostics=False).centroids
         X = np.ascontiguousarray(c.astype(np.float32))
         w0 = r.w32
 

@@ -141,6 +141,11 @@ def load_library() -> ctypes.CDLL:
     lib.apd_static_scratch_bytes.argtypes = []
     lib.apd_static_last_error.restype = ctypes.c_char_p
     lib.apd_static_last_error.argtypes = []
+    lib.apd_lloyd_points.restype = ctypes.c_int
+    lib.apd_lloyd_points.argtypes = ([_P, ctypes.c_int64, _P, _P, ctypes.c_double, ctypes.c_int32, _P, _P, _P,
+                                      ctypes.c_double, ctypes.c_int32] + [_P] * 4 +
+                                     [ctypes.POINTER(ctypes.c_int32), ctypes.POINTER(ctypes.c_int32),
+                                      ctypes.POINTER(ctypes.c_double), ctypes.POINTER(apd_opts), _P])
     lib.apd_validate.restype = ctypes.c_int
     lib.apd_validate.argtypes = [_P, ctypes.POINTER(apd_grid), ctypes.c_int32, _P, _P, _P, _P,
                                  ctypes.POINTER(ctypes.c_uint32), _P]
@@ -152,7 +157,7 @@ EXPORTED_SYMBOLS = ["apd_default_opts", "apd_create", "apd_destroy", "apd_last_e
                     "apd_assign_host", "apd_solve_host", "apd_solve_history", "apd_assign_points", "apd_solve_points", "apd_solve_stats", "apd_lloyd", "apd_solve_refine", "apd_resolution_bound",
                     "apd_choose_resolution", "apd_reserve", "apd_assign_stats", "apd_slab_align", "apd_counter_words",
                     "apd_assign_slab", "apd_finalize_counters", "apd_solve_slab", "apd_solve_continuation",
-                    "apd_assign_static", "apd_static_scratch_bytes", "apd_static_last_error", "apd_validate"]
+                    "apd_assign_static", "apd_static_scratch_bytes", "apd_static_last_error", "apd_validate", "apd_lloyd_points"]
 
 
 def make_grid(dim: int, n: Sequence[int], lo: Sequence[float], hi: Sequence[float]) -> apd_grid:
@@ -424,6 +429,23 @@ class ApdContext:
             _dev(w_init, torch.float32, "w_init", M), _dev(w, torch.float32, "w", M), _dev(labels, torch.int32, "labels"),
             _dev(vol, torch.float64, "vol", M), ctypes.byref(it), ctypes.byref(ev), ctypes.byref(err),
             ctypes.byref(opts) if opts is not None else None, self._stream())
+        self._check(rc, allow=(APD_OK, APD_NOT_CONVERGED))
+        return SolveInfo(rc, it.value, ev.value, err.value, float("nan"))
+
+    def apd_lloyd_points(self, Y, pvol, total_volume: float, X, A, target_vol, tol: float, K: int, w_init=None, w=None,
+                         labels=None, vol=None, opts: Optional[apd_opts] = None) -> SolveInfo:
+        """apd_lloyd_points of include/apd.h (Algorithm 3 on points with element volumes); X is updated in place."""
+        d = self.dim
+        N, M = int(Y.shape[0]), int(X.shape[0])
+        it, ev = ctypes.c_int32(0), ctypes.c_int32(0)
+        err = ctypes.c_double(0.0)
+        rc = self._lib.apd_lloyd_points(
+            self._h, N, _dev(Y, torch.float32, "Y", N * d), _dev(pvol, torch.float32, "pvol", N), float(total_volume), M,
+            _dev(X, torch.float32, "X", M * d), _dev(A, torch.float32, "A", M * d * d),
+            _dev(target_vol, torch.float32, "target_vol", M), float(tol), int(K),
+            _dev(w_init, torch.float32, "w_init", M), _dev(w, torch.float32, "w", M),
+            _dev(labels, torch.int32, "labels", N), _dev(vol, torch.float64, "vol", M), ctypes.byref(it), ctypes.byref(ev),
+            ctypes.byref(err), ctypes.byref(opts) if opts is not None else None, self._stream())
         self._check(rc, allow=(APD_OK, APD_NOT_CONVERGED))
         return SolveInfo(rc, it.value, ev.value, err.value, float("nan"))
 

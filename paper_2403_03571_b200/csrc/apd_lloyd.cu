@@ -70,6 +70,48 @@ done:
   return rc;
 }
 
+// Algorithm 3 on a user-supplied discretisation (points y_j with volumes |P_j|): the same loop with
+// apd_solve_points / apd_assign_points; the centroid of a cell is sum |P_j| y_j / sum |P_j| over its points.
+extern "C" int apd_lloyd_points(apd_ctx* ctx, int64_t N, const float* Y, const float* pvol, double total_volume, int32_t M,
+                                float* X, const float* A, const float* target_vol, double tol, int32_t K,
+                                const float* w_init, float* w, int32_t* labels, double* vol, int32_t* iters,
+                                int32_t* evals, double* max_rel_err, const apd_opts* opts, void* cuda_stream) {
+  if (!ctx) return APD_E_ARG;
+  ctx->err.clear();
+  if (K < 0) { ctx->err = "apd_lloyd_points: K must be >= 0"; return APD_E_ARG; }
+  if (!Y || !pvol || !X || !A || !target_vol || !w || M < 1 || N < 1) { ctx->err = "apd_lloyd_points: Y, pvol, X, A, target_vol and w are required"; return APD_E_ARG; }
+  const int d = ctx->ws.dim;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  double *cen = nullptr, *v64 = nullptr, *scal = nullptr;
+  int rc = APD_OK, it_sum = 0, ev_sum = 0;
+  double err = 0.0;
+  if (cudaSetDevice(ctx->ws.device) != cudaSuccess) { ctx->err = "apd_lloyd_points: cudaSetDevice failed"; return APD_E_CUDA; }
+  {
+    Workspace& ws = ctx->ws;
+    if (!ws.lloyd_buf) LL_TRY(cudaMalloc(&ws.lloyd_buf, ((size_t)ws.max_seeds * (ws.dim + 1) + 2) * sizeof(double)));
+    cen = ws.lloyd_buf; v64 = cen + (size_t)ws.max_seeds * ws.dim; scal = v64 + ws.max_seeds;
+  }
+  for (int k = 0; k <= K; ++k) {
+    int it = 0, ev = 0;
+    const bool last = (k == K);
+    rc = apd_solve_points(ctx, N, Y, pvol, total_volume, M, X, A, target_vol, tol, k == 0 ? w_init : w, w,
+                          last ? labels : nullptr, last ? vol : nullptr, &it, &ev, &err, opts, cuda_stream);
+    it_sum += it; ev_sum += ev;
+    if (rc < 0) goto done;
+    if (last) break;
+    rc = apd_assign_points(ctx, N, Y, pvol, M, X, A, w, target_vol, nullptr, v64, scal, scal + 1, cen, cuda_stream);
+    if (rc < 0) goto done;
+    centroids_to_seeds_kernel<<<(M * d + 255) / 256, 256, 0, st>>>(M * d, cen, X);
+    LL_TRY(cudaGetLastError());
+  }
+  LL_TRY(cudaStreamSynchronize(st));
+done:
+  if (iters) *iters = it_sum;
+  if (evals) *evals = ev_sum;
+  if (max_rel_err) *max_rel_err = err;
+  return rc;
+}
+
 // PAPER.md:182-197.  Smallest integer M (voxels per axis of a cubic grid on a domain of volume |Omega|) with
 //   |Omega| / M^D < factor * v_min,   factor = eps (necessary, eq. 2.9 for general v) or eps / 2^D (practical, eq. 2.10).
 extern "C" double apd_resolution_bound(int32_t dim, double domain_volume, double v_min, double eps, int32_t practical) {

@@ -176,3 +176,52 @@ def test_gpu_solve_points(apd):
     np.testing.assert_allclose(vol.cpu().numpy(), chk.vol, rtol=0, atol=2 * nm / N + 1e-12)
     assert abs(info.evals - orc.evals) <= max(4, orc.evals // 4)
     print(f"solve on points: gpu {info.iters}/{info.evals} err {info.max_rel_err:.4g}; oracle {orc.iters}/{orc.evals}")
+
+
+# ------------------------------------------------------------------------------------------------ Algorithm 3 on points
+def test_oracle_lloyd_on_points_equals_lloyd_on_grid():
+    """oracle_lloyd fed the voxel centres of a grid as a PointSet is Algorithm 3 on the grid itself (whose pins are in
+    tests/test_lloyd_resolution.py): same seeds after every round, same evaluation counts."""
+    from oracle.apd_oracle import PointSet, oracle_lloyd
+    wl = workloads.make_config(1)
+    Y, p = grid_points(wl)
+    Xa, ra, ia, ea = oracle_lloyd(Grid(2, wl.n, wl.lo, wl.hi), wl.X, wl.A, wl.v, 0.01, K=2)
+    Xb, rb, ib, eb = oracle_lloyd(PointSet(Y, p), wl.X, wl.A, wl.v, 0.01, K=2)
+    assert (ra.status, ia, ea) == (rb.status, ib, eb)
+    np.testing.assert_allclose(Xb, Xa, rtol=0, atol=1e-6)
+    np.testing.assert_allclose(rb.w, ra.w, rtol=0, atol=1e-7 * np.abs(ra.w).max() + 1e-12)
+    assert not np.allclose(Xa, wl.X, atol=1e-4)                         # the seeds did move
+
+
+@pytest.mark.gpu
+def test_gpu_lloyd_points(apd):
+    """K = 2 rounds of Algorithm 3 on a Monte-Carlo discretisation against oracle_lloyd(PointSet): the seeds agree to a
+    small fraction of the mean point spacing, and the post-condition is judged by the oracle at the GPU's (X, w)."""
+    import torch
+    from oracle.apd_oracle import PointSet, oracle_lloyd
+    rng = np.random.default_rng(11)
+    wl = workloads.make_config(2, n=(8, 8), M=24)
+    N = 50000
+    Y = rng.random((N, 2)).astype(np.float32)
+    p = np.full(N, 1.0 / N, np.float32)
+    tot = float(p.astype(np.float64).sum())
+    v = (wl.v.astype(np.float64) / wl.v.astype(np.float64).sum() * tot).astype(np.float32)
+    Xo, ro, it_o, ev_o = oracle_lloyd(PointSet(Y, p), wl.X, wl.A, v, 0.02, K=2)
+    dev = torch.device("cuda:0")
+    ctx = apd.ApdContext(2, wl.M)
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    X = t(wl.X.copy()); w = torch.zeros(wl.M, dtype=torch.float32, device=dev)
+    labels = torch.full((N,), -1, dtype=torch.int32, device=dev); vol = torch.zeros(wl.M, dtype=torch.float64, device=dev)
+    info = ctx.apd_lloyd_points(t(Y), t(p), tot, X, t(wl.A), t(v), 0.02, 2, w=w, labels=labels, vol=vol)
+    ctx.close()
+    assert info.status == ro.status == 0 and info.max_rel_err <= 0.02
+    Xg = X.cpu().numpy()
+    h = (1.0 / N) ** 0.5                                                 # mean point spacing
+    assert np.abs(Xg - Xo).max() <= 0.25 * h, f"seeds differ by {np.abs(Xg - Xo).max() / h:.3f} point spacings"
+    assert not np.allclose(Xg, wl.X, atol=1e-4)
+    chk = oracle_assign_points(Y, p, Xg, wl.A, w.cpu().numpy(), v=v)
+    nm = int((labels.cpu().numpy() != chk.labels).sum())
+    assert nm < max(1e-5 * N, 1) or nm == 0
+    assert chk.err <= 0.02 + 2 * nm / N / float(v.min())
+    assert abs(info.evals - ev_o) <= max(6, ev_o // 3)
+    print(f"lloyd on points: gpu evals {info.evals} vs oracle {ev_o}; max seed diff {np.abs(Xg - Xo).max() / h:.4f} spacings")
