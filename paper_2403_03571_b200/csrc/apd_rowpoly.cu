@@ -427,8 +427,10 @@ __global__ void __launch_bounds__(128, 6) assign_rowpoly_culled_kernel(const Ass
   pdl_enter();
   if (a.done_flag && *a.done_flag) return;
   const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
-  const int b = blockIdx.x;
-  const int bx = b % a.g.tiles_x, by = (b / a.g.tiles_x) % a.g.tiles_y, bz = b / (a.g.tiles_x * a.g.tiles_y);
+  // one CTA per tile, launched as a 3D grid: the tile's indices cost no integer divisions (three of them were ~65 of
+  // the ~1500 instructions a warp spends on a brick)
+  const int bx = blockIdx.x, by = blockIdx.y, bz = blockIdx.z;
+  const int b = (bz * a.g.tiles_y + by) * a.g.tiles_x + bx;
 
   // a1: this thread's row inside its warp's brick (apd_internal.cuh: brick_box)
   int tx, ty, tz;
@@ -449,7 +451,11 @@ __global__ void __launch_bounds__(128, 6) assign_rowpoly_culled_kernel(const Ass
     list = a.super_list + (size_t)sup * SUPER_CAP;
     if (cnt < 0) { cnt = a.M; list = nullptr; }
   }
-  const int nchunks = (cnt + WCHUNK - 1) / WCHUNK;
+  // at least one chunk and, below, at least one pair: an empty list (it cannot occur: the seed that attains the
+  // smallest upper bound always survives) would evaluate one padding pair of cost +inf and keep label 0.  Without the
+  // guarantee the compiler builds a second, specialised exit for the zero-trip case (~45 instructions of constant
+  // set-up in front of the loop, executed by every warp).
+  const int nchunks = max(1, (cnt + WCHUNK - 1) / WCHUNK);
 
   auto gather = [&](int c) {
     const int stage = c & 1;
@@ -478,7 +484,7 @@ __global__ void __launch_bounds__(128, 6) assign_rowpoly_culled_kernel(const Ass
     for (int q = 0; q < NP; ++q) dst[2 * q] = r[q];
     s_idx[w][stage][lane] = idx;
   };
-  if (nchunks > 0) gather(0);        // issued first: its latency overlaps the row set-up below
+  gather(0);        // issued first: its latency overlaps the row set-up below
 
   RowTau<V> tt;
   rt.tau(a, tt);
@@ -488,12 +494,14 @@ __global__ void __launch_bounds__(128, 6) assign_rowpoly_culled_kernel(const Ass
   for (int k = 0; k < V; ++k) { best[k] = CUDART_INF_F; lab[k] = 0; }
   __syncwarp();
 
-  for (int c = 0; c < nchunks; ++c) {
+  int c = 0;
+  do {
     if (c + 1 < nchunks) gather(c + 1);     // the other stage: the warp left it before the last __syncwarp
     const float* sp = s_seeds[w][c & 1];
     const int* ip = s_idx[w][c & 1];
-    const int npairs = min(WCHUNK / 2, (cnt - c * WCHUNK + 1) / 2);     // pairs that hold a real candidate
-    for (int p = 0; p < npairs; ++p) {
+    const int npairs = max(1, min(WCHUNK / 2, (cnt - c * WCHUNK + 1) / 2));     // pairs that hold a real candidate
+    int p = 0;
+    do {
       const RowCoef rc = row_setup<DIM>(sp + p * PREC, rt.rr);
       const int i0 = ip[2 * p], i1 = ip[2 * p + 1];
       row_sweep<V>(rc, tt, [&](int k, float lo, float hi) {
@@ -501,9 +509,9 @@ __global__ void __launch_bounds__(128, 6) assign_rowpoly_culled_kernel(const Ass
         if (m < best[k]) lab[k] = (lo == m) ? i0 : i1;    // lo == hi == m: the lower index
         best[k] = m;
       });
-    }
+    } while (++p < npairs);
     __syncwarp();
-  }
+  } while (++c < nchunks);
 
   double dsum = row_epilogue<V>(a, rt.row_valid, rt.ix0, rt.iy, rt.iz, best, lab);
 #pragma unroll
@@ -553,7 +561,9 @@ static cudaError_t launch_rowpoly_t(const AssignArgs& a, int n_tiles, cudaStream
 
 template <int DIM>
 static cudaError_t launch_culled_t(const AssignArgs& a, int n_tiles, cudaStream_t st) {
-  return launch_pdl(assign_rowpoly_culled_kernel<DIM>, n_tiles, 128, 0, st, a);
+  (void)n_tiles;
+  return launch_pdl(assign_rowpoly_culled_kernel<DIM>, dim3((unsigned)a.g.tiles_x, (unsigned)a.g.tiles_y, (unsigned)a.g.tiles_z),
+                    128, 0, st, a);
 }
 
 cudaError_t launch_assign_rowpoly(const AssignArgs& a, cudaStream_t st) {
