@@ -268,7 +268,8 @@ int enqueue_evaluation(apd_ctx* ctx, const GridDev& g, int kernel, int M, const 
     APD_CUDA_TRY(ctx, launch_cull(g, M, M_pad, X, A, w, cb, nsx, nsy, nsz, ws.count, centroids ? ws.idxsum : nullptr, done_flag,
                                   cull_rebuild, cull_delta, cull_rebuild_s, cull_delta_s, cull_rebuild_t, cull_delta_t, st));
     a.rec = ws.rec; a.brick_list = ws.brick_list; a.brick_count = ws.brick_count; a.super_list = ws.super_list;
-    a.super_count = ws.super_count; a.super_x = nsx; a.super_y = nsy; a.pairs_ctr = ws.pairs_ctr;
+    a.super_count = ws.super_count; a.super_x = nsx; a.super_y = nsy;
+    a.pairs_ctr = vol ? ws.pairs_ctr : nullptr;      // apd_solve's loop (vol == nullptr) has no use for the pair count
   }
   ws.last_kernel = kernel; ws.last_row_long = g.row_long; ws.last_cull = cull ? 1 : 0; ws.last_tiles = n_tiles;
   if (timed) APD_CUDA_TRY(ctx, cudaEventRecord(ws.ev0, st));

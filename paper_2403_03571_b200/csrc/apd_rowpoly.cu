@@ -441,8 +441,21 @@ __global__ void __launch_bounds__(128, 6) assign_rowpoly_culled_kernel(const Ass
 
   // the brick's candidate list; an overflowed list falls back to the super-tile's, then to all seeds
   const size_t brick = (size_t)b * 4 + w;
+  const int* const blist = a.brick_list + brick * BRICK_CAP;
+  // The first chunk's index and record are loaded SPECULATIVELY, before the count is known: count -> index -> record
+  // is a chain of three dependent global loads in front of every brick, and this takes one link out of it.  Slot
+  // `lane` of the list always exists (capacity 256); past the list's end it holds anything, so the index is clamped
+  // into the record table and the loaded record is simply not used.
+  const int idx_spec = __ldg(blist + lane);
   int cnt = a.brick_count[brick];
-  const int* list = a.brick_list + brick * BRICK_CAP;
+  float4 rec_spec[REC / 4];
+  {
+    const int ic = min(max(idx_spec, 0), a.M_pad - 1);
+    const float4* src = reinterpret_cast<const float4*>(a.rec + (size_t)ic * REC);
+#pragma unroll
+    for (int q = 0; q < REC / 4; ++q) rec_spec[q] = __ldg(src + q);
+  }
+  const int* list = blist;
   if (cnt < 0) {
     constexpr int STX = (DIM == 3) ? SUPER3_TX : SUPER2_TX, STY = (DIM == 3) ? SUPER3_TY : SUPER2_TY,
                   STZ = (DIM == 3) ? SUPER3_TZ : 1;
@@ -463,12 +476,20 @@ __global__ void __launch_bounds__(128, 6) assign_rowpoly_culled_kernel(const Ass
     float r[REC];
     int idx = 0;
     if (pos < cnt) {
-      idx = list ? __ldg(list + pos) : pos;
-      const float4* src = reinterpret_cast<const float4*>(a.rec + (size_t)idx * REC);
+      if (c == 0 && list == blist) {       // the speculative loads above
+        idx = idx_spec;
 #pragma unroll
-      for (int q = 0; q < REC / 4; ++q) {
-        const float4 v4 = __ldg(src + q);
-        r[4 * q] = v4.x; r[4 * q + 1] = v4.y; r[4 * q + 2] = v4.z; r[4 * q + 3] = v4.w;
+        for (int q = 0; q < REC / 4; ++q) {
+          r[4 * q] = rec_spec[q].x; r[4 * q + 1] = rec_spec[q].y; r[4 * q + 2] = rec_spec[q].z; r[4 * q + 3] = rec_spec[q].w;
+        }
+      } else {
+        idx = list ? __ldg(list + pos) : pos;
+        const float4* src = reinterpret_cast<const float4*>(a.rec + (size_t)idx * REC);
+#pragma unroll
+        for (int q = 0; q < REC / 4; ++q) {
+          const float4 v4 = __ldg(src + q);
+          r[4 * q] = v4.x; r[4 * q + 1] = v4.y; r[4 * q + 2] = v4.z; r[4 * q + 3] = v4.w;
+        }
       }
     } else {
 #pragma unroll
@@ -518,6 +539,7 @@ __global__ void __launch_bounds__(128, 6) assign_rowpoly_culled_kernel(const Ass
   for (int o = 16; o > 0; o >>= 1) dsum += __shfl_down_sync(0xffffffffu, dsum, o);     // fixed order
   if (lane == 0) {
     a.dual_partial[brick] = dsum;
+    if (!a.pairs_ctr) return;          // the evaluations inside a solve do not count pairs
     // voxel-seed pairs whose cost this brick evaluated (valid voxels only)
     int ox, oy, oz, ex, ey, ez;
     brick_box(DIM, w, &ox, &oy, &oz, &ex, &ey, &ez);
