@@ -522,6 +522,7 @@ __global__ void __launch_bounds__(128, 6) assign_rowpoly_culled_kernel(const Ass
     const int* ip = s_idx[w][c & 1];
     const int npairs = max(1, min(WCHUNK / 2, (cnt - c * WCHUNK + 1) / 2));     // pairs that hold a real candidate
     int p = 0;
+#pragma unroll 2
     do {
       const RowCoef rc = row_setup<DIM>(sp + p * PREC, rt.rr);
       const int i0 = ip[2 * p], i1 = ip[2 * p + 1];
