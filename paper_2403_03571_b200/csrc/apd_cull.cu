@@ -390,6 +390,7 @@ __global__ void __launch_bounds__(128) cull_bricks_kernel(const CullArgs c) {
   __shared__ float s_min[CULL_G][4];
   __shared__ int s_imin[CULL_G][4];
   __shared__ int s_wsum[4][CULL_G];
+  __shared__ RefSeed<DIM> s_ref[4][4];     // (b): per warp (tile), the reference seed of each of its four bricks
   if (c.done_flag && *c.done_flag) return;
   if (c.rebuild && !*c.rebuild) return;
   const float delta = c.delta ? *c.delta : 0.0f;
@@ -515,62 +516,100 @@ __global__ void __launch_bounds__(128) cull_bricks_kernel(const CullArgs c) {
     }
   }
 
-  // (b) brick lists, tile by tile
-  int ox, oy, oz, ex, ey, ez;
-  brick_box(DIM, w, &ox, &oy, &oz, &ex, &ey, &ez);
-  const float y0y = box_centre(c.g.lo[1], c.g.s[1], by * TY + oy + c.g.off_y, ey);
-  const float y0z = (DIM == 3) ? box_centre(c.g.lo[2], c.g.s[2], bz * TZ + oz + c.g.off_z, ez) : 0.0f;
-#pragma unroll
-  for (int g = 0; g < CULL_G; ++g) {
-    if (g >= ng) break;
+  // (b) brick lists: warp g of the CTA cuts tile g's list down to each of the tile's FOUR bricks.  Every candidate's
+  // record is gathered once per pass and tested against the four brick boxes (before: each warp walked all four tiles
+  // for its own brick, i.e. every record was gathered by four warps -- and this step waits for its 48-byte gathers at
+  // random indices: ncu long-scoreboard 5.7 per issue).  Same bounds, same order, same lists.
+  if (w < ng) {
+    const int g = w;
     const int bx = qx * CULL_G + g;
     const bool from_smem = n_tile[g] >= 0;
     const int n = from_smem ? n_tile[g] : n_par;
     const int* tl = s_tile[g];
     auto cand = [&](int pos) { return from_smem ? tl[pos] : (par ? __ldg(par + pos) : pos); };
-    const float y0x = box_centre(c.g.lo[0], c.g.s[0], bx * TX + ox, ex);
-
-    float umin = CUDART_INF_F;
-    int imin = 0;
-    for (int pos = lane; pos < n; pos += 32) {
-      const int i = cand(pos);
-      float s, rho, supp, nw;
-      seed_bounds<DIM, 0>(c.rec, i, y0x, y0y, y0z, c.hb, &s, &rho, &supp, &nw);
-      const float u = upper_bound(s, rho, nw);
-      if (u < umin) { umin = u; imin = i; }
+    constexpr int REC = (DIM == 3) ? REC3 : REC2;
+    constexpr int NB = 4;                      // bricks per tile
+    float b0x[NB], b0y[NB], b0z[NB];           // centres of the bricks' boxes of voxel centres
+#pragma unroll
+    for (int j = 0; j < NB; ++j) {
+      int ox, oy, oz, ex, ey, ez;
+      brick_box(DIM, j, &ox, &oy, &oz, &ex, &ey, &ez);
+      b0x[j] = box_centre(c.g.lo[0], c.g.s[0], bx * TX + ox, ex);
+      b0y[j] = box_centre(c.g.lo[1], c.g.s[1], by * TY + oy + c.g.off_y, ey);
+      b0z[j] = (DIM == 3) ? box_centre(c.g.lo[2], c.g.s[2], bz * TZ + oz + c.g.off_z, ez) : 0.0f;
     }
-    warp_argmin(umin, imin);
-    if (n > 0) umin = fminf(umin, exact_upper<DIM>(c.rec, imin, y0x, y0y, y0z, c.hb));
+    // a candidate's record and its brick radius (slot NP of the record)
+    auto load = [&](int i, SeedRec<DIM>& r, float& rho) {
+      r.load(c.rec, i);
+      rho = __ldg(c.rec + (size_t)i * REC + ((DIM == 3) ? 10 : 6));
+    };
+    // pass 1: per brick, the seed with the smallest upper bound (by position: the lists ascend in index)
+    float umin[NB];
+    int pmin[NB];
+#pragma unroll
+    for (int j = 0; j < NB; ++j) { umin[j] = CUDART_INF_F; pmin[j] = 0; }
+    for (int pos = lane; pos < n; pos += 32) {
+      SeedRec<DIM> r;
+      float rho;
+      load(cand(pos), r, rho);
+#pragma unroll
+      for (int j = 0; j < NB; ++j) {
+        float sj, supp;
+        r.at(b0x[j], b0y[j], b0z[j], c.hb, &sj, &supp);
+        const float u = upper_bound(sj, rho, r.nw);
+        if (u < umin[j]) { umin[j] = u; pmin[j] = pos; }
+      }
+    }
     const float slack2 = 2.0f * delta * (1.0f + CULL_EPS);
-    const float U = umin + slack2;
-    RefSeed<DIM> ref;                          // the seed that attains the smallest upper bound (warp-uniform)
-    if (n > 0) ref.init(c.rec, imin, y0x, y0y, y0z);
-
+    float U[NB];
+#pragma unroll
+    for (int j = 0; j < NB; ++j) {
+      warp_argmin(umin[j], pmin[j]);
+      const int kmin = n > 0 ? cand(pmin[j]) : 0;
+      if (n > 0) umin[j] = fminf(umin[j], exact_upper<DIM>(c.rec, kmin, b0x[j], b0y[j], b0z[j], c.hb));
+      U[j] = umin[j] + slack2;
+      if (lane == j && n > 0) s_ref[w][j].init(c.rec, kmin, b0x[j], b0y[j], b0z[j]);     // the reference seed of brick j
+    }
+    __syncwarp();
+    // pass 2: ordered compaction of the survivors into the four brick lists
     const size_t tile = ((size_t)bz * c.g.tiles_y + by) * c.g.tiles_x + bx;
-    const size_t brick = tile * 4 + w;
-    int* list = c.brick_list + brick * BRICK_CAP;
-    int base = 0;
+    int base[NB];
+#pragma unroll
+    for (int j = 0; j < NB; ++j) base[j] = 0;
     for (int p0 = 0; p0 < n; p0 += 32) {
       const int pos = p0 + lane;
-      bool keep = false;
+      bool keep[NB];
+#pragma unroll
+      for (int j = 0; j < NB; ++j) keep[j] = false;
       int i = 0;
       if (pos < n) {
         i = cand(pos);
         SeedRec<DIM> r;
         r.load(c.rec, i);
-        float s, supp;
-        r.at(y0x, y0y, y0z, c.hb, &s, &supp);
-        keep = !(lower_bound(s, supp, r.nw) > U);
-        if (keep) keep = !(ref.pair_min(r, y0x, y0y, y0z, c.hb) > slack2);      // NaN keeps the seed
+#pragma unroll
+        for (int j = 0; j < NB; ++j) {
+          float sj, supp;
+          r.at(b0x[j], b0y[j], b0z[j], c.hb, &sj, &supp);
+          keep[j] = !(lower_bound(sj, supp, r.nw) > U[j]);
+          if (keep[j]) keep[j] = !(s_ref[w][j].pair_min(r, b0x[j], b0y[j], b0z[j], c.hb) > slack2);   // NaN keeps the seed
+        }
       }
-      const unsigned int bal = __ballot_sync(0xffffffffu, keep);
-      if (keep) {
-        const int q = base + __popc(bal & ((1u << lane) - 1u));
-        if (q < BRICK_CAP) list[q] = i;
+#pragma unroll
+      for (int j = 0; j < NB; ++j) {
+        const unsigned int bal = __ballot_sync(0xffffffffu, keep[j]);
+        if (keep[j]) {
+          const int q = base[j] + __popc(bal & ((1u << lane) - 1u));
+          if (q < BRICK_CAP) c.brick_list[(tile * 4 + j) * BRICK_CAP + q] = i;
+        }
+        base[j] += __popc(bal);
       }
-      base += __popc(bal);
     }
-    if (lane == 0) c.brick_count[brick] = (base <= BRICK_CAP) ? base : -1;
+    if (lane < NB) {
+      int bj = base[0];
+#pragma unroll
+      for (int j = 1; j < NB; ++j) if (lane == j) bj = base[j];
+      c.brick_count[tile * 4 + lane] = (bj <= BRICK_CAP) ? bj : -1;
+    }
   }
 }
 
