@@ -231,7 +231,7 @@ int enqueue_evaluation(apd_ctx* ctx, const GridDev& g, int kernel, int M, const 
                        double* max_rel_err, double* centroids, uint64_t* pairs, bool timed, bool cull,
                        const int* done_flag, cudaStream_t st, const int* cull_rebuild, const float* cull_delta,
                        const int* cull_rebuild_s, const float* cull_delta_s, const int* cull_rebuild_t,
-                       const float* cull_delta_t) {
+                       const float* cull_delta_t, bool cull_skip_pack) {
   Workspace& ws = ctx->ws;
   const int M_pad = (M + SEED_CHUNK - 1) / SEED_CHUNK * SEED_CHUNK;
   const int n_tiles = g.tiles_x * g.tiles_y * g.tiles_z;
@@ -266,7 +266,7 @@ int enqueue_evaluation(apd_ctx* ctx, const GridDev& g, int kernel, int M, const 
     cull_super_counts(g, &nsx, &nsy, &nsz);
     CullBuffers cb{ws.rec, ws.brick_list, ws.brick_count, ws.super_list, ws.super_count, ws.tile_list, ws.tile_count, ws.pairs_ctr};
     APD_CUDA_TRY(ctx, launch_cull(g, M, M_pad, X, A, w, cb, nsx, nsy, nsz, ws.count, centroids ? ws.idxsum : nullptr, done_flag,
-                                  cull_rebuild, cull_delta, cull_rebuild_s, cull_delta_s, cull_rebuild_t, cull_delta_t, st));
+                                  cull_rebuild, cull_delta, cull_rebuild_s, cull_delta_s, cull_rebuild_t, cull_delta_t, cull_skip_pack, st));
     a.rec = ws.rec; a.brick_list = ws.brick_list; a.brick_count = ws.brick_count; a.super_list = ws.super_list;
     a.super_count = ws.super_count; a.super_x = nsx; a.super_y = nsy;
     a.pairs_ctr = vol ? ws.pairs_ctr : nullptr;      // apd_solve's loop (vol == nullptr) has no use for the pair count

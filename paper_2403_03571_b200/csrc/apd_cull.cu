@@ -626,7 +626,7 @@ cudaError_t launch_cull(const GridDev& g, int M, int M_pad, const float* X, cons
                         const CullBuffers& cb, int nsx, int nsy, int nsz, unsigned int* count,
                         unsigned long long* idxsum, const int* done_flag, const int* rebuild, const float* delta,
                         const int* rebuild_s, const float* delta_s, const int* rebuild_t, const float* delta_t,
-                        cudaStream_t st) {
+                        bool skip_pack, cudaStream_t st) {
   // half-extents of the boxes of voxel CENTRES of a brick and of a super-tile
   int ox, oy, oz, ex, ey, ez;
   brick_box(g.dim, 0, &ox, &oy, &oz, &ex, &ey, &ez);
@@ -637,10 +637,14 @@ cudaError_t launch_cull(const GridDev& g, int M, int M_pad, const float* X, cons
   const float3 hb = make_float3(half(ex, 0), half(ey, 1), g.dim == 3 ? half(ez, 2) : 0.0f);
   const float3 hs = make_float3(half(sex, 0), half(sey, 1), g.dim == 3 ? half(sez, 2) : 0.0f);
   const int nb = (M_pad + 127) / 128;
-  cudaError_t e;
-  if (g.dim == 3) e = launch_pdl(cull_pack_kernel<3>, nb, 128, 0, st, M, M_pad, X, A, w, hb, hs, cb.rec, cb.pairs_ctr, count, idxsum, done_flag);
-  else            e = launch_pdl(cull_pack_kernel<2>, nb, 128, 0, st, M, M_pad, X, A, w, hb, hs, cb.rec, cb.pairs_ctr, count, idxsum, done_flag);
-  if (e != cudaSuccess) return e;
+  cudaError_t e = cudaSuccess;
+  // skip_pack: inside a solve, after its first evaluation, the step kernel has already written -w into the records and
+  // zeroed the counts (apd_lbfgs.cu: StepArgs::rec_nw); everything else in a record is constant over the solve
+  if (!skip_pack) {
+    if (g.dim == 3) e = launch_pdl(cull_pack_kernel<3>, nb, 128, 0, st, M, M_pad, X, A, w, hb, hs, cb.rec, cb.pairs_ctr, count, idxsum, done_flag);
+    else            e = launch_pdl(cull_pack_kernel<2>, nb, 128, 0, st, M, M_pad, X, A, w, hb, hs, cb.rec, cb.pairs_ctr, count, idxsum, done_flag);
+    if (e != cudaSuccess) return e;
+  }
   CullArgs c;
   c.g = g; c.M = M; c.rec = cb.rec; c.super_list = cb.super_list; c.super_count = cb.super_count;
   c.nsx = nsx; c.nsy = nsy; c.nsz = nsz; c.brick_list = cb.brick_list; c.brick_count = cb.brick_count;

@@ -189,7 +189,7 @@ cudaError_t launch_cull(const GridDev& g, int M, int M_pad, const float* X, cons
                         const CullBuffers& cb, int n_super_x, int n_super_y, int n_super_z, unsigned int* count,
                         unsigned long long* idxsum, const int* done_flag, const int* rebuild, const float* delta,
                         const int* rebuild_s, const float* delta_s, const int* rebuild_t, const float* delta_t,
-                        cudaStream_t st);
+                        bool skip_pack, cudaStream_t st);
 void cull_super_counts(const GridDev& g, int* nsx, int* nsy, int* nsz);
 int rowpoly_tile_counts(int dim, int nx, int ny, int nz, int sm_count, bool cull, int* tx, int* ty, int* tz);
 int assign_tile_counts(int kernel, int dim, int nx, int ny, int nz, int sm_count, bool cull, int* tx, int* ty, int* tz);
@@ -248,7 +248,7 @@ int enqueue_evaluation(apd_ctx* ctx, const GridDev& g, int kernel, int M, const 
                        const int* done_flag, cudaStream_t st, const int* cull_rebuild = nullptr,
                        const float* cull_delta = nullptr, const int* cull_rebuild_s = nullptr,
                        const float* cull_delta_s = nullptr, const int* cull_rebuild_t = nullptr,
-                       const float* cull_delta_t = nullptr);
+                       const float* cull_delta_t = nullptr, bool cull_skip_pack = false);
 
 }  // namespace apd
 

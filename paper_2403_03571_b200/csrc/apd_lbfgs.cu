@@ -70,6 +70,12 @@ struct StepArgs {
   float* wref;         // weights the brick candidate lists were built at (culling only)
   float* wref_s;       // weights the super-tile lists were built at
   float* wref_t;       // weights the CTA-tile lists were built at
+  // culled solves: the step kernel itself refreshes what cull_pack_kernel would rewrite before the next evaluation --
+  // the -w slot of every seed's record and the zeroed voxel counts -- so the loop launches no pack kernel after the
+  // first evaluation (X, A and the box radii of a record do not change inside a solve)
+  float* rec_nw = nullptr;     // &rec[0][slot of -w], or nullptr (no culling / points)
+  int rec_stride = 0;          // floats per record
+  unsigned int* count_zero = nullptr;   // [M] the evaluation's voxel counts, to be zeroed for the next one
   double* gram;        // [LB_CLUSTER_MAX] copies of { (2 hist_cap + 1)^2 Gram matrix, hist_cap rho }, see GramSmem
 };
 
@@ -553,6 +559,7 @@ __device__ void combine_and_trial(const StepArgs& a, int cap, const DirCoef& dc,
         red3[3] = fmax(red3[3], fabs((double)wn - (double)wref_s[u]));
         red3[4] = fmax(red3[4], fabs((double)wn - (double)wref_t[u]));
         a.w32[i] = wn;
+        if (a.rec_nw) { a.rec_nw[(size_t)i * a.rec_stride] = -wn; a.count_zero[i] = 0u; }
       }
     }
   }
@@ -804,6 +811,7 @@ __global__ void __launch_bounds__(LB_THREADS) lbfgs_step_kernel(StepArgs a) {
         mx[2] = fmax(mx[2], fabs((double)wn - (double)a.wref_s[i]));
         mx[3] = fmax(mx[3], fabs((double)wn - (double)a.wref_t[i]));
         a.w32[i] = wn;
+        if (a.rec_nw) { a.rec_nw[(size_t)i * a.rec_stride] = -wn; a.count_zero[i] = 0u; }
       }
       cluster_all<4, true>(mx, red);
     }
@@ -1066,12 +1074,24 @@ int apd::solve_grid(apd_ctx* ctx, const char* who, const apd_grid* grid, const a
     if (reduce && reduce(user, cuda_stream) != 0) { ctx->err = pre + "the reduce callback failed"; return APD_E_CUDA; }
     return APD_OK;
   };
+  if (o.cull) {
+    // the record table exists before the loop starts: the step kernel writes into it (StepArgs::rec_nw)
+    rc = ensure_eval_buffers(ctx, g, kernel, true, st);
+    if (rc != APD_OK) return rc;
+    sa.rec_nw = ws.rec + (g.dim == 3 ? 9 : 5);
+    sa.rec_stride = rec_floats(g.dim);
+    sa.count_zero = ws.count;
+  }
+  int n_loop_evals = 0;
   SolveHooks hooks;
   hooks.loop_eval = [&](const int* done_flag) -> int {
+    // after the first evaluation the records' -w and the zeroed counts come from the step kernel: no pack launch
+    const bool skip_pack = o.cull != 0 && n_loop_evals > 0;
+    ++n_loop_evals;
     int r = enqueue_evaluation(ctx, g, kernel, M, X, A, ws.w32, target_vol, nullptr, nullptr, nullptr, nullptr, nullptr,
                                nullptr, false, o.cull != 0, done_flag, st, &ws.sstate->cull_rebuild,
                                &ws.sstate->cull_delta, &ws.sstate->cull_rebuild_s, &ws.sstate->cull_delta_s,
-                               &ws.sstate->cull_rebuild_t, &ws.sstate->cull_delta_t);
+                               &ws.sstate->cull_rebuild_t, &ws.sstate->cull_delta_t, skip_pack);
     if (r == APD_OK && slab) r = exchange(false, done_flag);
     return r;
   };
