@@ -73,7 +73,8 @@ enum {
  * whenever that runs its short rows (grids below ~10^3 long-row tiles); against the long-row or the TENSOR brute-force
  * kernels (what AUTO picks on large grids / many seeds) the labels can differ on fp32 near-ties only.
  * Requires kernel AUTO or ROWPOLY and positive definite A_i (not checked).  Workspace grows by
- * O(number of bricks): 1 KiB per 512 voxels.  pairs_evaluated reports the pairs actually evaluated. */
+ * O(number of bricks): 1 KiB per 512 voxels for the brick lists plus 3 KiB per 2048 voxels for the tile lists apd_solve
+ * keeps between its evaluations (3.5 bytes per voxel in all).  pairs_evaluated reports the pairs actually evaluated. */
 typedef struct {
   int32_t kernel;          /* APD_KERNEL_*                                   default AUTO         */
   int32_t cull;            /* 0 brute force, 1 exact conservative culling      default 0          */
@@ -323,7 +324,7 @@ int apd_validate(apd_ctx* ctx, const apd_grid* grid, int32_t M, const float* X, 
                  const float* target_vol, uint32_t* problems, void* cuda_stream);
 
 /* Grows the context's workspace to what apd_assign / apd_solve / apd_lloyd need on `grid` with `opts` (dual partials:
- * 8 bytes per tile; with opts.cull the candidate lists, 1 KiB per 512 voxels; L-BFGS state for opts.lbfgs_history),
+ * 8 bytes per tile; with opts.cull the candidate lists, 3.5 bytes per voxel; L-BFGS state for opts.lbfgs_history),
  * so that those calls, on this grid or any grid with no more tiles, neither allocate nor synchronise.  Synchronous
  * (cudaMalloc).  APD_E_ARG as apd_assign; APD_E_CUDA on allocation failure. */
 int apd_reserve(apd_ctx* ctx, const apd_grid* grid, const apd_opts* opts);
