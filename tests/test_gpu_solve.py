@@ -245,3 +245,33 @@ def test_solve_host_matches_device(apd):
                                w=w, labels=lab)
     assert (info2.status, info2.iters, info2.evals) == (info.status, info.iters, info.evals)
     assert np.array_equal(w.numpy(), w32) and np.array_equal(lab.numpy(), labels)
+
+
+def test_one_context_serves_solves_in_a_row(apd):
+    """The culled solve keeps state between its evaluations in the context (candidate lists of three levels with their
+    reference weights, the per-seed records whose -w the step kernel refreshes in place, counts zeroed by the step
+    kernel).  Solves that follow one another on ONE context -- other grids, fewer seeds, a cap of one evaluation, brute
+    force in between -- must each give, bit for bit, what a fresh context gives."""
+    dev = torch.device("cuda:0")
+    cases = [(workloads.make_config(3, n=(64, 64, 64), M=120), 0.02, 1, 0),
+             (workloads.make_config(2, n=(256, 256), M=60), 0.01, 1, 0),       # other dimension: its own context below
+             (workloads.make_config(3, n=(48, 40, 36), M=37), 0.02, 1, 0),     # fewer seeds, smaller ragged grid
+             (workloads.make_config(3, n=(48, 40, 36), M=37), 0.02, 1, 1),     # one evaluation only (NOT_CONVERGED)
+             (workloads.make_config(3, n=(64, 64, 64), M=120), 0.02, 0, 0),    # brute force on the same context
+             (workloads.make_config(3, n=(64, 64, 64), M=120), 0.02, 1, 0)]    # and the first case again
+    shared = {2: apd.ApdContext(2, 120), 3: apd.ApdContext(3, 120)}
+    for wl, eps, cull, max_evals in cases:
+        fresh = run_solve(apd, wl, eps, cull=cull, max_evals=max_evals)
+        ctx = shared[wl.dim]
+        grid = apd.make_grid(wl.dim, wl.n, wl.lo, wl.hi)
+        X = torch.from_numpy(wl.X).to(dev); A = torch.from_numpy(wl.A).to(dev); v = torch.from_numpy(wl.v).to(dev)
+        w = torch.zeros(wl.M, dtype=torch.float32, device=dev)
+        labels = torch.full((wl.N,), -1, dtype=torch.int32, device=dev)
+        vol = torch.zeros(wl.M, dtype=torch.float64, device=dev)
+        info = ctx.apd_solve(grid, X, A, v, eps, w=w, labels=labels, vol=vol,
+                             opts=apd.make_opts(cull=cull, max_evals=max_evals))
+        assert (info.status, info.iters, info.evals) == (fresh[0].status, fresh[0].iters, fresh[0].evals)
+        assert np.array_equal(w.cpu().numpy(), fresh[1]) and np.array_equal(labels.cpu().numpy(), fresh[3])
+        assert np.array_equal(vol.cpu().numpy(), fresh[4]) and info.dual == fresh[0].dual
+    for c in shared.values():
+        c.close()
